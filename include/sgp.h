@@ -1,0 +1,218 @@
+/*
+ * sgp.h -- C ABI of libsgp_b200: scaled gradient projection (SGP) and Richardson-Lucy (RL)
+ * deconvolution of Poisson images on one NVIDIA B200 (sm_100a).
+ *
+ * Method: Prato, Cavicchioli, Zanni, Boccacci, Bertero, "Efficient deconvolution methods for
+ * astronomical imaging: algorithms and IDL-GPU codes" (arXiv:1210.2258).  Citations below are
+ * PAPER.md:<line> + equation / algorithm; "A<n>" are the readings listed in DESIGN.md section 3.
+ *
+ *   minimise   J0(f) = sum_j sum_{m in S} { g_j ln( g_j / (A_j f + b_j) ) + A_j f + b_j - g_j }    (Eq.2 / Eq.12)
+ *   subject to f >= 0,
+ *   A_j f   = M_S o (K_j * (M_R o f))                                   (Eq.16)
+ *   A_j^T y = M_R o (K_j corr (M_S o y))                                (Eq.17)
+ *
+ * by Algorithm 1 with the scaling D_k = (M_R/alpha) o clip(f, L1, L2) (Eq.10 / Eq.23),
+ * the alternating Barzilai-Borwein step lengths (Eq.7-9) and Armijo backtracking on
+ * A f + lambda A d (Alg.1 steps 4-5), or by the RL iteration f <- (M_R/alpha) o f o sum_j A_j^T(g_j/(A_j f + b_j))
+ * (Eq.1 / Eq.13 / Eq.21).  Every step of the iteration runs in CUDA kernels of this library; there
+ * is no CPU fallback.
+ *
+ * Conventions
+ *   - Arrays are row-major and contiguous: element (y, x) of an ny x nx array is a[y*nx + x].
+ *   - Entry points WITHOUT the _host suffix take DEVICE pointers (cudaMalloc'ed or a torch CUDA
+ *     tensor's data_ptr); the *_host variants take HOST pointers and copy to / from the device inside
+ *     the call.  Arrays of pointers (g[], psf[], b_arr[]) are always HOST arrays holding p pointers.
+ *   - `dtype` selects the element type of every array argument: SGP_F32 = float, SGP_F64 = double.
+ *     All reductions (J0, dot products) are accumulated in double in both modes.
+ *   - `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).  The calls are
+ *     synchronous with respect to the host: they return after the work has completed on `stream`.
+ *   - Ownership: the caller owns every input and output; inputs are never modified; f_out may alias
+ *     f0.  The library owns only the plan's workspace, freed by sgp_plan_destroy.
+ *   - Errors: every entry point returns 0 (SGP_OK) or a negative sgp_status.  Nothing is printed, no
+ *     exception crosses the ABI.  After an error inside the iteration f_out holds the last accepted
+ *     iterate.  sgp_last_cuda_error() gives the text of the last CUDA error seen by this thread.
+ *   - Grid sizes: the native FFT supports ny, nx in {64,128,256,320,512,640,1024,1280,2048,4096};
+ *     any other size returns SGP_ERR_ARG.
+ *   - A plan is not thread-safe; different plans may be used from different threads.
+ */
+#ifndef SGP_B200_H
+#define SGP_B200_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define SGP_MAX_IMAGES 16
+#define SGP_MAX_MALPHA 16
+#define SGP_MAX_ARMIJO_MEMORY 64
+
+typedef enum { SGP_F32 = 0, SGP_F64 = 1 } sgp_dtype;
+/* stopping rules, PAPER.md:279-298 (Sect.3.3); max_iter is always an additional cap */
+typedef enum { SGP_STOP_MAXIT = 0, SGP_STOP_RELJ = 1, SGP_STOP_DISCREPANCY = 2 } sgp_stop;
+/* initial guess, PAPER.md:260-267 (Sect.3.1) */
+typedef enum { SGP_INIT_USER = 0, SGP_INIT_CONST = 1, SGP_INIT_ZERO = 2, SGP_INIT_G = 3 } sgp_init;
+/* where the PSF centre sits in the input array (A18) */
+typedef enum { SGP_PSF_CENTER = 0, SGP_PSF_CORNER = 1 } sgp_psf_origin;
+/* FFT backend: the library's own kernels, or cuFFT as the in-run comparison baseline */
+typedef enum { SGP_FFT_NATIVE = 0, SGP_FFT_CUFFT = 1 } sgp_backend;
+/* problem kind of a plan */
+typedef enum { SGP_KIND_SINGLE = 0, SGP_KIND_MULTI = 1, SGP_KIND_BOUNDARY = 2 } sgp_kind;
+/* algorithm run by sgp_plan_run */
+typedef enum { SGP_ALG_SGP = 0, SGP_ALG_RL = 1 } sgp_algorithm;
+
+typedef enum {
+    SGP_OK = 0,
+    SGP_ERR_ARG = -1,        /* null pointer, p out of range, unsupported size, bad option value */
+    SGP_ERR_PSF = -2,        /* PSF sum <= 0 or non-finite */
+    SGP_ERR_DATA = -3,       /* non-finite g, negative g in strict mode, negative user f0, no positive value for the adaptive bounds */
+    SGP_ERR_ALLOC = -4,      /* device or host allocation failed */
+    SGP_ERR_CUDA = -5,       /* a CUDA call failed; see sgp_last_cuda_error() */
+    SGP_ERR_LINESEARCH = -6, /* max_backtracks reductions of lambda without Armijo acceptance (A16) */
+    SGP_ERR_NONFINITE = -7,  /* J0 of the start point is not finite */
+    SGP_ERR_UNSUPPORTED = -8 /* option combination not available in this build */
+} sgp_status;
+
+/* stop_reason values in sgp_result */
+typedef enum { SGP_REASON_NONE = 0, SGP_REASON_MAXIT = 1, SGP_REASON_RELJ = 2, SGP_REASON_DISCREPANCY = 3 } sgp_reason;
+
+/* Options; sgp_options_default() fills the paper's values. */
+typedef struct sgp_options {
+    double beta, theta;                          /* Armijo: 1e-4, 0.4 */
+    double alpha0, alpha_min, alpha_max, tau1;   /* 1.3, 1e-5, 1e5, 0.5 */
+    int m_alpha;                                 /* memory of the BB2 minimum, Eq.9: 3 */
+    int alt_start;                               /* alternation only after this many iterations: 20 (A9) */
+    int armijo_memory;                           /* M >= 1; 1 = monotone line search, the paper     (A15) */
+    double L1, L2;                               /* scaling bounds of Eq.10 when adaptive_L = 0 */
+    int adaptive_L;                              /* 1: bounds from one RL step */
+    int max_iter;                                /* iteration cap (always active) */
+    int stop_rule;                               /* sgp_stop */
+    double tol;                                  /* Eq.24 */
+    double disc_threshold;                       /* Eq.26: stop at the first k with 2 J0/(p #S) <= this (A6, A7) */
+    double sigma_R;                              /* Eq.20 threshold defining R (A13) */
+    int max_backtracks;                          /* A16 */
+    int psf_origin;                              /* sgp_psf_origin */
+    int init;                                    /* sgp_init */
+    int refresh_every;                           /* A21: recompute A f from f every n iterations; 0 = never */
+    int strict;                                  /* A17: 1 = negative g is SGP_ERR_DATA instead of being clamped to 0 */
+    int check_every;                             /* iterations enqueued between two host reads of the device status; 0 = auto */
+    int backend;                                 /* sgp_backend */
+    int tile_cols;                               /* tuning: spectrum tile width in columns (power of 2); 0 = auto */
+    int rows_per_block;                          /* tuning: rows per CTA in the row-FFT kernels (power of 2); 0 = auto */
+    int use_graph;                               /* 1 = replay one iteration as a CUDA graph; 0 = plain stream launches */
+} sgp_options;
+
+/* Result of a run.  The trace pointers are optional caller-allocated HOST arrays of max_iter+1 entries
+ * (NULL = not wanted): trace_J[k] = J0(f(k)) for k = 0..iterations; trace_alpha[k], trace_lambda[k],
+ * trace_rule[k] (0 = alpha0, 1 = BB1, 2 = Eq.9 minimum of BB2), trace_backtracks[k] describe the step
+ * f(k) -> f(k+1).  RL fills trace_J only.
+ * force_alpha / force_lambda (HOST arrays of max_iter doubles, NaN = not forced, NULL = off) are a
+ * TEST-ONLY replay mode: alpha_k / lambda_k are taken from them instead of the BB rules / Armijo loop. */
+typedef struct sgp_result {
+    int iterations;
+    int stop_reason;            /* sgp_reason */
+    double J0_final;
+    double discrepancy_final;   /* 2 J0 / (p #S), Eq.26 */
+    int total_backtracks;
+    double L1_used, L2_used;
+    long n_fft2;                /* 2-D transforms executed inside the iteration loop (2p+2 per iteration) */
+    double setup_ms, loop_ms;   /* device time of the start-point phase and of the iteration loop (CUDA events) */
+    long kernel_launches;       /* kernels of this library launched by the call */
+    double *trace_J, *trace_alpha, *trace_lambda;
+    int *trace_rule, *trace_backtracks;
+    const double *force_alpha, *force_lambda;
+} sgp_result;
+
+typedef struct sgp_plan sgp_plan;
+
+void sgp_options_default(sgp_options *opt);
+void sgp_result_init(sgp_result *res);           /* zero everything, NULL traces */
+const char *sgp_strerror(int status);
+const char *sgp_version(void);
+const char *sgp_last_cuda_error(void);
+/* bytes of device workspace a plan of this shape allocates (0 for unsupported arguments) */
+size_t sgp_workspace_bytes(int kind, int p, int ny, int nx, int dtype);
+
+/* ---- one-shot entry points: DEVICE pointers ------------------------------------------------------
+ * g: detected image(s), psf: PSF(s) on the object grid (any positive scale; normalised to unit sum
+ * inside), b_arr: background array(s) or NULL to use the constant(s) b_const,
+ * f0: initial image (required for SGP_INIT_USER, else may be NULL), f_out: ny x nx result. */
+int sgp_single(const void *g, const void *psf, const void *b_arr, double b_const, const void *f0,
+               void *f_out, int ny, int nx, int dtype, const sgp_options *opt, sgp_result *res,
+               void *stream);
+int sgp_multi(int p, const void *const *g, const void *const *psf, const void *const *b_arr,
+              const double *b_const, const void *f0, void *f_out, int ny, int nx, int dtype,
+              const sgp_options *opt, sgp_result *res, void *stream);
+/* Boundary-effect correction (Sect.2.4): g[j], b_arr[j] are sy x sx detected images occupying
+ * S = [oy,oy+sy) x [ox,ox+sx) of the ny x nx object grid S-bar; psf[j], f0, f_out are ny x nx;
+ * maskR_out (optional, ny*nx bytes, device) receives M_R of Eq.20; f_out is zero outside R. */
+int sgp_boundary(int p, const void *const *g, const void *const *psf, const void *const *b_arr,
+                 const double *b_const, int oy, int ox, int sy, int sx, int ny, int nx,
+                 const void *f0, void *f_out, unsigned char *maskR_out, int dtype,
+                 const sgp_options *opt, sgp_result *res, void *stream);
+/* Richardson-Lucy on the same kernels (Eq.1 / Eq.13 / Eq.21); uses only the stopping fields,
+ * init, psf_origin, sigma_R, strict and the tuning fields of opt. */
+int rl_single(const void *g, const void *psf, const void *b_arr, double b_const, const void *f0,
+              void *f_out, int ny, int nx, int dtype, const sgp_options *opt, sgp_result *res,
+              void *stream);
+int rl_multi(int p, const void *const *g, const void *const *psf, const void *const *b_arr,
+             const double *b_const, const void *f0, void *f_out, int ny, int nx, int dtype,
+             const sgp_options *opt, sgp_result *res, void *stream);
+int rl_boundary(int p, const void *const *g, const void *const *psf, const void *const *b_arr,
+                const double *b_const, int oy, int ox, int sy, int sx, int ny, int nx,
+                const void *f0, void *f_out, unsigned char *maskR_out, int dtype,
+                const sgp_options *opt, sgp_result *res, void *stream);
+
+/* ---- the same six calls with HOST pointers (copies inside the call; what bench.py times as e2e) -- */
+int sgp_single_host(const void *g, const void *psf, const void *b_arr, double b_const, const void *f0,
+                    void *f_out, int ny, int nx, int dtype, const sgp_options *opt, sgp_result *res,
+                    void *stream);
+int sgp_multi_host(int p, const void *const *g, const void *const *psf, const void *const *b_arr,
+                   const double *b_const, const void *f0, void *f_out, int ny, int nx, int dtype,
+                   const sgp_options *opt, sgp_result *res, void *stream);
+int sgp_boundary_host(int p, const void *const *g, const void *const *psf, const void *const *b_arr,
+                      const double *b_const, int oy, int ox, int sy, int sx, int ny, int nx,
+                      const void *f0, void *f_out, unsigned char *maskR_out, int dtype,
+                      const sgp_options *opt, sgp_result *res, void *stream);
+int rl_single_host(const void *g, const void *psf, const void *b_arr, double b_const, const void *f0,
+                   void *f_out, int ny, int nx, int dtype, const sgp_options *opt, sgp_result *res,
+                   void *stream);
+int rl_multi_host(int p, const void *const *g, const void *const *psf, const void *const *b_arr,
+                  const double *b_const, const void *f0, void *f_out, int ny, int nx, int dtype,
+                  const sgp_options *opt, sgp_result *res, void *stream);
+int rl_boundary_host(int p, const void *const *g, const void *const *psf, const void *const *b_arr,
+                     const double *b_const, int oy, int ox, int sy, int sx, int ny, int nx,
+                     const void *f0, void *f_out, unsigned char *maskR_out, int dtype,
+                     const sgp_options *opt, sgp_result *res, void *stream);
+
+/* ---- plan form: set-up once (workspace, twiddles, transfer functions, boundary weights), run many -- */
+/* kind SINGLE requires p = 1; for SINGLE / MULTI the (oy,ox,sy,sx) arguments are ignored (S = S-bar). */
+int sgp_plan_create(sgp_plan **plan, int kind, int p, int ny, int nx, int oy, int ox, int sy, int sx,
+                    int dtype, const sgp_options *opt);
+/* K^_j = FFT2 of the normalised, origin-shifted PSFs; for BOUNDARY plans also alpha_j, alpha, R and
+ * M_R/alpha (Eq.19-20).  psf: HOST array of p DEVICE pointers (ny x nx each). */
+int sgp_plan_set_psf(sgp_plan *plan, const void *const *psf, void *stream);
+/* One reconstruction.  g, b_arr: HOST arrays of p DEVICE pointers (sy x sx each; b_arr or its entries may
+ * be NULL -> b_const[j]).  algorithm: sgp_algorithm.  opt (may be NULL = the plan's options) replaces the
+ * run-time options (everything except backend, tile_cols, rows_per_block, sigma_R, psf_origin). */
+int sgp_plan_run(sgp_plan *plan, int algorithm, const void *const *g, const void *const *b_arr,
+                 const double *b_const, const void *f0, void *f_out, const sgp_options *opt,
+                 sgp_result *res, void *stream);
+/* Operators of the plan, for callers and tests: out = A_j x (Eq.16) / out = A_j^T y (Eq.17),
+ * all ny x nx DEVICE arrays on the S-bar grid. */
+int sgp_plan_apply_A(sgp_plan *plan, int j, const void *x, void *out, void *stream);
+int sgp_plan_apply_AT(sgp_plan *plan, int j, const void *y, void *out, void *stream);
+/* M_R (bytes), alpha = sum_j alpha_j and #R of a plan whose PSFs are set; pointers may be NULL (DEVICE). */
+int sgp_plan_get_mask(sgp_plan *plan, unsigned char *maskR_out, void *alpha_out, long *nR, void *stream);
+/* Unnormalised 2-D real-to-complex DFT of an ny x nx DEVICE array with the plan's own FFT kernels, written
+ * as ny x (nx/2+1) interleaved complex numbers (the layout of numpy.fft.rfft2); for tests and for the
+ * in-run comparison with cuFFT.  sgp_plan_irfft2 is the inverse including the 1/(ny nx) factor. */
+int sgp_plan_rfft2(sgp_plan *plan, const void *x, void *spec_out, void *stream);
+int sgp_plan_irfft2(sgp_plan *plan, const void *spec_in, void *x_out, void *stream);
+void sgp_plan_destroy(sgp_plan *plan);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SGP_B200_H */

@@ -1,0 +1,354 @@
+// api.cu -- the C ABI of include/sgp.h: argument checks, plan life cycle, one-shot and host-pointer wrappers.
+#include <new>
+#include "plan.cuh"
+
+namespace sgpk {
+
+thread_local std::string g_last_cuda_error;
+
+int validate_options(const sgp_options *o)
+{
+    if (!o) return SGP_ERR_ARG;
+    if (!(o->beta > 0 && o->beta < 1 && o->theta > 0 && o->theta < 1)) return SGP_ERR_ARG;
+    if (!(o->alpha_min > 0 && o->alpha_min < o->alpha_max)) return SGP_ERR_ARG;
+    if (!(o->alpha0 > 0) || !(o->tau1 > 0)) return SGP_ERR_ARG;
+    if (o->m_alpha < 1 || o->m_alpha > SGP_MAX_MALPHA) return SGP_ERR_ARG;
+    if (o->armijo_memory < 1 || o->armijo_memory > SGP_MAX_ARMIJO_MEMORY) return SGP_ERR_ARG;
+    if (o->max_iter < 0 || o->max_backtracks < 0 || o->alt_start < 0) return SGP_ERR_ARG;
+    if (!o->adaptive_L && !(o->L1 > 0 && o->L1 < o->L2)) return SGP_ERR_ARG;
+    if (o->stop_rule < SGP_STOP_MAXIT || o->stop_rule > SGP_STOP_DISCREPANCY) return SGP_ERR_ARG;
+    if (o->init < SGP_INIT_USER || o->init > SGP_INIT_G) return SGP_ERR_ARG;
+    if (o->psf_origin != SGP_PSF_CENTER && o->psf_origin != SGP_PSF_CORNER) return SGP_ERR_ARG;
+    if (o->check_every < 0 || o->refresh_every < 0) return SGP_ERR_ARG;
+    if (o->backend != SGP_FFT_NATIVE && o->backend != SGP_FFT_CUFFT) return SGP_ERR_ARG;
+    return SGP_OK;
+}
+
+static int floor_pow2(int v) { int r = 1; while (r * 2 <= v) r *= 2; return r; }
+static bool is_pow2(int v) { return v > 0 && (v & (v - 1)) == 0; }
+
+// Spectrum tile width C (columns per CTA of the column kernel) and rows per CTA of the row kernels.
+int choose_tiles(int ny, int nx, int dtype, const sgp_options *opt, int *C_out, int *RB_out)
+{
+    const int esz = dtype == SGP_F64 ? 16 : 8;                     // bytes per complex number
+    const int Lr = nx / 2, Lc = ny;
+    const int Ec = (Lc % 5 == 0) ? 20 : (dtype == SGP_F64 ? 8 : 16);
+    const int Er = (Lr % 5 == 0) ? 20 : (dtype == SGP_F64 ? 8 : 16);
+    // column kernel: at most 512 threads and ~96 KB of shared memory per CTA
+    int C = floor_pow2(512 * Ec / Lc);
+    if (C > 32) C = 32;
+    while (C > 1 && (size_t)C * (Lc + Lc / 16) * esz > 96 * 1024) C /= 2;
+    while (C > 1 && Lr % C != 0) C /= 2;
+    if (opt && opt->tile_cols > 0) {
+        if (!is_pow2(opt->tile_cols) || Lr % opt->tile_cols != 0) return SGP_ERR_ARG;
+        C = opt->tile_cols;
+    }
+    const int TFc = Lc / Ec;
+    if (C * TFc > 512 || (size_t)C * (Lc + Lc / 16) * esz > 227 * 1024) return SGP_ERR_ARG;
+    // row kernels: about 256 threads per CTA
+    const int TFr = Lr / Er;
+    int RB = floor_pow2(256 / TFr > 1 ? 256 / TFr : 1);
+    if (RB > 32) RB = 32;
+    while (RB > 1 && (size_t)RB * (Lr + Lr / 16 + 2) * esz > 96 * 1024) RB /= 2;
+    if (opt && opt->rows_per_block > 0) {
+        if (!is_pow2(opt->rows_per_block)) return SGP_ERR_ARG;
+        RB = opt->rows_per_block;
+    }
+    while (RB > 1 && ny % RB != 0) RB /= 2;
+    if (RB * TFr > 512 || (size_t)RB * (Lr + Lr / 16 + 2) * esz > 227 * 1024) return SGP_ERR_ARG;
+    // the store mapping of the row kernels needs RB*C to divide the RB*Lr outputs of a CTA: true since C | Lr
+    *C_out = C; *RB_out = RB;
+    return SGP_OK;
+}
+
+size_t workspace_bytes(int kind, int p, int ny, int nx, int dtype)
+{
+    if (p < 1 || p > SGP_MAX_IMAGES || !size_supported(ny) || !size_supported(nx)) return 0;
+    const size_t r = dtype == SGP_F64 ? 8 : 4;
+    const size_t n = (size_t)ny * nx;
+    size_t planes = 6 * (size_t)p + 4;                 // khat, spec, g, b, q, u per image; f, grad, d, scratch
+    size_t b = planes * n * r;
+    if (kind == SGP_KIND_BOUNDARY) b += 2 * n * r + n;
+    b += ((size_t)nx + 1 + 2 * (size_t)ny + (size_t)ny * p) * 2 * r;   // twiddles, pack line, khatB
+    b += (size_t)(ny * (6 + 2 * p) + 1024 * p + 2048) * sizeof(double) + sizeof(Ctrl);
+    return b;
+}
+
+}  // namespace sgpk
+
+using namespace sgpk;
+
+struct sgp_plan { PlanBase *impl; };
+
+extern "C" {
+
+void sgp_options_default(sgp_options *o)
+{
+    if (!o) return;
+    memset(o, 0, sizeof(*o));
+    o->beta = 1e-4; o->theta = 0.4;
+    o->alpha0 = 1.3; o->alpha_min = 1e-5; o->alpha_max = 1e5;
+    o->tau1 = 0.5; o->m_alpha = 3;
+    o->alt_start = 20;
+    o->armijo_memory = 1;
+    o->L1 = 1e-10; o->L2 = 1e10; o->adaptive_L = 1;
+    o->max_iter = 100; o->stop_rule = SGP_STOP_MAXIT; o->tol = 1e-5;
+    o->disc_threshold = 1.0; o->sigma_R = 1e-2; o->max_backtracks = 30;
+    o->psf_origin = SGP_PSF_CENTER; o->init = SGP_INIT_CONST;
+    o->refresh_every = 0; o->strict = 0; o->check_every = 0;
+    o->backend = SGP_FFT_NATIVE; o->tile_cols = 0; o->rows_per_block = 0; o->use_graph = 0;
+}
+
+void sgp_result_init(sgp_result *r) { if (r) memset(r, 0, sizeof(*r)); }
+
+const char *sgp_strerror(int s)
+{
+    switch (s) {
+    case SGP_OK: return "ok";
+    case SGP_ERR_ARG: return "invalid argument (null pointer, p out of range, unsupported grid size or option value)";
+    case SGP_ERR_PSF: return "PSF sum is not positive or not finite";
+    case SGP_ERR_DATA: return "invalid data (non-finite or negative image values, negative start image, no positive value for the scaling bounds)";
+    case SGP_ERR_ALLOC: return "allocation failed";
+    case SGP_ERR_CUDA: return "CUDA error (see sgp_last_cuda_error)";
+    case SGP_ERR_LINESEARCH: return "line search failed: max_backtracks reductions without Armijo acceptance";
+    case SGP_ERR_NONFINITE: return "objective J0 is not finite";
+    case SGP_ERR_UNSUPPORTED: return "option combination not supported by this build";
+    default: return "unknown status";
+    }
+}
+
+const char *sgp_version(void) { return "sgp-b200 0.1.0 (sm_100a)"; }
+const char *sgp_last_cuda_error(void) { return g_last_cuda_error.c_str(); }
+
+size_t sgp_workspace_bytes(int kind, int p, int ny, int nx, int dtype) { return workspace_bytes(kind, p, ny, nx, dtype); }
+
+int sgp_plan_create(sgp_plan **plan, int kind, int p, int ny, int nx, int oy, int ox, int sy, int sx, int dtype,
+                    const sgp_options *opt)
+{
+    if (!plan) return SGP_ERR_ARG;
+    *plan = nullptr;
+    sgp_options o;
+    if (opt) o = *opt; else sgp_options_default(&o);
+    int rc = validate_options(&o);
+    if (rc) return rc;
+    if (o.backend != SGP_FFT_NATIVE) return SGP_ERR_UNSUPPORTED;
+    if (dtype != SGP_F32 && dtype != SGP_F64) return SGP_ERR_ARG;
+    if (kind < SGP_KIND_SINGLE || kind > SGP_KIND_BOUNDARY) return SGP_ERR_ARG;
+    if (p < 1 || p > SGP_MAX_IMAGES || (kind == SGP_KIND_SINGLE && p != 1)) return SGP_ERR_ARG;
+    if (!size_supported(ny) || !size_supported(nx)) return SGP_ERR_ARG;
+    if (kind == SGP_KIND_BOUNDARY) {
+        if (oy < 0 || ox < 0 || sy < 1 || sx < 1 || oy + sy > ny || ox + sx > nx) return SGP_ERR_ARG;
+        if (!(o.sigma_R > 0)) return SGP_ERR_ARG;
+    } else { oy = 0; ox = 0; sy = ny; sx = nx; }
+    PlanBase *b = dtype == SGP_F32 ? make_plan_f32() : make_plan_f64();
+    if (!b) return SGP_ERR_ALLOC;
+    b->kind = kind; b->p = p; b->ny = ny; b->nx = nx; b->dtype = dtype; b->opt = o;
+    b->G.ny = ny; b->G.nx = nx; b->G.oy = oy; b->G.ox = ox; b->G.sy = sy; b->G.sx = sx;
+    b->G.masked = kind == SGP_KIND_BOUNDARY ? 1 : 0; b->G.p = p;
+    rc = b->init();
+    if (rc) { delete b; return rc; }
+    sgp_plan *pl = new (std::nothrow) sgp_plan;
+    if (!pl) { delete b; return SGP_ERR_ALLOC; }
+    pl->impl = b;
+    *plan = pl;
+    return SGP_OK;
+}
+
+void sgp_plan_destroy(sgp_plan *plan)
+{
+    if (!plan) return;
+    delete plan->impl;
+    delete plan;
+}
+
+int sgp_plan_set_psf(sgp_plan *plan, const void *const *psf, void *stream)
+{
+    if (!plan || !psf) return SGP_ERR_ARG;
+    return plan->impl->set_psf(psf, (cudaStream_t)stream);
+}
+
+int sgp_plan_run(sgp_plan *plan, int algorithm, const void *const *g, const void *const *b_arr, const double *b_const,
+                 const void *f0, void *f_out, const sgp_options *opt, sgp_result *res, void *stream)
+{
+    if (!plan) return SGP_ERR_ARG;
+    return plan->impl->run(algorithm, g, b_arr, b_const, f0, f_out, opt, res, (cudaStream_t)stream);
+}
+
+int sgp_plan_apply_A(sgp_plan *plan, int j, const void *x, void *out, void *stream)
+{
+    if (!plan) return SGP_ERR_ARG;
+    return plan->impl->apply(false, j, x, out, (cudaStream_t)stream);
+}
+int sgp_plan_apply_AT(sgp_plan *plan, int j, const void *y, void *out, void *stream)
+{
+    if (!plan) return SGP_ERR_ARG;
+    return plan->impl->apply(true, j, y, out, (cudaStream_t)stream);
+}
+int sgp_plan_get_mask(sgp_plan *plan, unsigned char *maskR_out, void *alpha_out, long *nR, void *stream)
+{
+    if (!plan) return SGP_ERR_ARG;
+    return plan->impl->get_mask(maskR_out, alpha_out, nR, (cudaStream_t)stream);
+}
+int sgp_plan_rfft2(sgp_plan *plan, const void *x, void *spec_out, void *stream)
+{
+    if (!plan) return SGP_ERR_ARG;
+    return plan->impl->rfft2(x, spec_out, (cudaStream_t)stream);
+}
+int sgp_plan_irfft2(sgp_plan *plan, const void *spec_in, void *x_out, void *stream)
+{
+    if (!plan) return SGP_ERR_ARG;
+    return plan->impl->irfft2(spec_in, x_out, (cudaStream_t)stream);
+}
+
+// ---- one-shot calls: create a plan, set the PSFs, run, destroy
+static int one_shot(int algorithm, int kind, int p, const void *const *g, const void *const *psf, const void *const *b_arr,
+                    const double *b_const, int oy, int ox, int sy, int sx, int ny, int nx, const void *f0, void *f_out,
+                    unsigned char *maskR_out, int dtype, const sgp_options *opt, sgp_result *res, void *stream)
+{
+    if (!g || !psf || !f_out || !res || !opt) return SGP_ERR_ARG;
+    sgp_plan *pl = nullptr;
+    int rc = sgp_plan_create(&pl, kind, p, ny, nx, oy, ox, sy, sx, dtype, opt);
+    if (rc) return rc;
+    rc = sgp_plan_set_psf(pl, psf, stream);
+    if (!rc) rc = sgp_plan_run(pl, algorithm, g, b_arr, b_const, f0, f_out, opt, res, stream);
+    if (maskR_out && (rc == SGP_OK || rc == SGP_ERR_LINESEARCH)) {
+        int r2 = sgp_plan_get_mask(pl, maskR_out, nullptr, nullptr, stream);
+        if (!rc) rc = r2;
+    }
+    if (res) res->kernel_launches = pl->impl->launches;
+    sgp_plan_destroy(pl);
+    return rc;
+}
+
+int sgp_single(const void *g, const void *psf, const void *b_arr, double b_const, const void *f0, void *f_out, int ny, int nx,
+               int dtype, const sgp_options *opt, sgp_result *res, void *stream)
+{
+    const void *gg[1] = {g}, *pp[1] = {psf}, *bb[1] = {b_arr};
+    return one_shot(SGP_ALG_SGP, SGP_KIND_SINGLE, 1, gg, pp, b_arr ? bb : nullptr, &b_const, 0, 0, ny, nx, ny, nx, f0, f_out, nullptr,
+                    dtype, opt, res, stream);
+}
+int rl_single(const void *g, const void *psf, const void *b_arr, double b_const, const void *f0, void *f_out, int ny, int nx,
+              int dtype, const sgp_options *opt, sgp_result *res, void *stream)
+{
+    const void *gg[1] = {g}, *pp[1] = {psf}, *bb[1] = {b_arr};
+    return one_shot(SGP_ALG_RL, SGP_KIND_SINGLE, 1, gg, pp, b_arr ? bb : nullptr, &b_const, 0, 0, ny, nx, ny, nx, f0, f_out, nullptr,
+                    dtype, opt, res, stream);
+}
+int sgp_multi(int p, const void *const *g, const void *const *psf, const void *const *b_arr, const double *b_const,
+              const void *f0, void *f_out, int ny, int nx, int dtype, const sgp_options *opt, sgp_result *res, void *stream)
+{
+    return one_shot(SGP_ALG_SGP, SGP_KIND_MULTI, p, g, psf, b_arr, b_const, 0, 0, ny, nx, ny, nx, f0, f_out, nullptr, dtype, opt, res, stream);
+}
+int rl_multi(int p, const void *const *g, const void *const *psf, const void *const *b_arr, const double *b_const,
+             const void *f0, void *f_out, int ny, int nx, int dtype, const sgp_options *opt, sgp_result *res, void *stream)
+{
+    return one_shot(SGP_ALG_RL, SGP_KIND_MULTI, p, g, psf, b_arr, b_const, 0, 0, ny, nx, ny, nx, f0, f_out, nullptr, dtype, opt, res, stream);
+}
+int sgp_boundary(int p, const void *const *g, const void *const *psf, const void *const *b_arr, const double *b_const,
+                 int oy, int ox, int sy, int sx, int ny, int nx, const void *f0, void *f_out, unsigned char *maskR_out,
+                 int dtype, const sgp_options *opt, sgp_result *res, void *stream)
+{
+    return one_shot(SGP_ALG_SGP, SGP_KIND_BOUNDARY, p, g, psf, b_arr, b_const, oy, ox, sy, sx, ny, nx, f0, f_out, maskR_out, dtype, opt, res, stream);
+}
+int rl_boundary(int p, const void *const *g, const void *const *psf, const void *const *b_arr, const double *b_const,
+                int oy, int ox, int sy, int sx, int ny, int nx, const void *f0, void *f_out, unsigned char *maskR_out,
+                int dtype, const sgp_options *opt, sgp_result *res, void *stream)
+{
+    return one_shot(SGP_ALG_RL, SGP_KIND_BOUNDARY, p, g, psf, b_arr, b_const, oy, ox, sy, sx, ny, nx, f0, f_out, maskR_out, dtype, opt, res, stream);
+}
+
+// ---- host-pointer variants: stage through device buffers (pinned staging is the caller's choice)
+struct DevBufs {
+    std::vector<void *> bufs;
+    ~DevBufs() { for (void *b : bufs) cudaFree(b); }
+    int up(const void *host, size_t bytes, cudaStream_t st, void **dev)
+    {
+        *dev = nullptr;
+        if (!host) return SGP_OK;
+        SGP_CUDA_TRY(cudaMalloc(dev, bytes));
+        bufs.push_back(*dev);
+        SGP_CUDA_TRY(cudaMemcpyAsync(*dev, host, bytes, cudaMemcpyHostToDevice, st));
+        return SGP_OK;
+    }
+    int blank(size_t bytes, void **dev)
+    {
+        SGP_CUDA_TRY(cudaMalloc(dev, bytes));
+        bufs.push_back(*dev);
+        return SGP_OK;
+    }
+};
+
+static int host_shot(int algorithm, int kind, int p, const void *const *g, const void *const *psf, const void *const *b_arr,
+                     const double *b_const, int oy, int ox, int sy, int sx, int ny, int nx, const void *f0, void *f_out,
+                     unsigned char *maskR_out, int dtype, const sgp_options *opt, sgp_result *res, void *stream)
+{
+    if (!g || !psf || !f_out || !res || !opt || p < 1 || p > SGP_MAX_IMAGES) return SGP_ERR_ARG;
+    if (dtype != SGP_F32 && dtype != SGP_F64) return SGP_ERR_ARG;
+    if (ny < 1 || nx < 1 || sy < 1 || sx < 1) return SGP_ERR_ARG;
+    cudaStream_t st = (cudaStream_t)stream;
+    const size_t r = dtype == SGP_F64 ? 8 : 4;
+    const size_t nb = (size_t)ny * nx * r, sb = (size_t)sy * sx * r;
+    DevBufs D;
+    const void *dg[SGP_MAX_IMAGES], *dk[SGP_MAX_IMAGES], *db[SGP_MAX_IMAGES];
+    int rc;
+    bool have_b = false;
+    for (int j = 0; j < p; ++j) {
+        if (!g[j] || !psf[j]) return SGP_ERR_ARG;
+        void *t;
+        if ((rc = D.up(g[j], sb, st, &t))) return rc; dg[j] = t;
+        if ((rc = D.up(psf[j], nb, st, &t))) return rc; dk[j] = t;
+        if ((rc = D.up(b_arr ? b_arr[j] : nullptr, sb, st, &t))) return rc; db[j] = t;
+        if (t) have_b = true;
+    }
+    void *df0 = nullptr, *dout = nullptr, *dmask = nullptr;
+    if ((rc = D.up(f0, nb, st, &df0))) return rc;
+    if ((rc = D.blank(nb, &dout))) return rc;
+    if (maskR_out && (rc = D.blank((size_t)ny * nx, &dmask))) return rc;
+    rc = one_shot(algorithm, kind, p, dg, dk, have_b ? db : nullptr, b_const, oy, ox, sy, sx, ny, nx, df0, dout,
+                  (unsigned char *)dmask, dtype, opt, res, stream);
+    if (rc == SGP_OK || rc == SGP_ERR_LINESEARCH) {
+        SGP_CUDA_TRY(cudaMemcpyAsync(f_out, dout, nb, cudaMemcpyDeviceToHost, st));
+        if (maskR_out) SGP_CUDA_TRY(cudaMemcpyAsync(maskR_out, dmask, (size_t)ny * nx, cudaMemcpyDeviceToHost, st));
+        SGP_CUDA_TRY(cudaStreamSynchronize(st));
+    }
+    return rc;
+}
+
+int sgp_single_host(const void *g, const void *psf, const void *b_arr, double b_const, const void *f0, void *f_out, int ny,
+                    int nx, int dtype, const sgp_options *opt, sgp_result *res, void *stream)
+{
+    const void *gg[1] = {g}, *pp[1] = {psf}, *bb[1] = {b_arr};
+    return host_shot(SGP_ALG_SGP, SGP_KIND_SINGLE, 1, gg, pp, b_arr ? bb : nullptr, &b_const, 0, 0, ny, nx, ny, nx, f0, f_out, nullptr,
+                     dtype, opt, res, stream);
+}
+int rl_single_host(const void *g, const void *psf, const void *b_arr, double b_const, const void *f0, void *f_out, int ny,
+                   int nx, int dtype, const sgp_options *opt, sgp_result *res, void *stream)
+{
+    const void *gg[1] = {g}, *pp[1] = {psf}, *bb[1] = {b_arr};
+    return host_shot(SGP_ALG_RL, SGP_KIND_SINGLE, 1, gg, pp, b_arr ? bb : nullptr, &b_const, 0, 0, ny, nx, ny, nx, f0, f_out, nullptr,
+                     dtype, opt, res, stream);
+}
+int sgp_multi_host(int p, const void *const *g, const void *const *psf, const void *const *b_arr, const double *b_const,
+                   const void *f0, void *f_out, int ny, int nx, int dtype, const sgp_options *opt, sgp_result *res, void *stream)
+{
+    return host_shot(SGP_ALG_SGP, SGP_KIND_MULTI, p, g, psf, b_arr, b_const, 0, 0, ny, nx, ny, nx, f0, f_out, nullptr, dtype, opt, res, stream);
+}
+int rl_multi_host(int p, const void *const *g, const void *const *psf, const void *const *b_arr, const double *b_const,
+                  const void *f0, void *f_out, int ny, int nx, int dtype, const sgp_options *opt, sgp_result *res, void *stream)
+{
+    return host_shot(SGP_ALG_RL, SGP_KIND_MULTI, p, g, psf, b_arr, b_const, 0, 0, ny, nx, ny, nx, f0, f_out, nullptr, dtype, opt, res, stream);
+}
+int sgp_boundary_host(int p, const void *const *g, const void *const *psf, const void *const *b_arr, const double *b_const,
+                      int oy, int ox, int sy, int sx, int ny, int nx, const void *f0, void *f_out, unsigned char *maskR_out,
+                      int dtype, const sgp_options *opt, sgp_result *res, void *stream)
+{
+    return host_shot(SGP_ALG_SGP, SGP_KIND_BOUNDARY, p, g, psf, b_arr, b_const, oy, ox, sy, sx, ny, nx, f0, f_out, maskR_out, dtype, opt, res, stream);
+}
+int rl_boundary_host(int p, const void *const *g, const void *const *psf, const void *const *b_arr, const double *b_const,
+                     int oy, int ox, int sy, int sx, int ny, int nx, const void *f0, void *f_out, unsigned char *maskR_out,
+                     int dtype, const sgp_options *opt, sgp_result *res, void *stream)
+{
+    return host_shot(SGP_ALG_RL, SGP_KIND_BOUNDARY, p, g, psf, b_arr, b_const, oy, ox, sy, sx, ny, nx, f0, f_out, maskR_out, dtype, opt, res, stream);
+}
+
+}  // extern "C"

@@ -1,0 +1,25 @@
+// dispatch.h -- look-up of the kernel instantiations by FFT length (defined in inst_*.cu, one translation
+// unit per element type and kernel family so that they compile in parallel).
+#pragma once
+#include "kernels.cuh"
+
+namespace sgpk {
+
+template <typename T> using row_kernel_t = void (*)(const RowParams<T>);
+template <typename T> using col_kernel_t = void (*)(const ColParams<T>);
+
+// L = nx/2 (row kernels) or ny (column kernel); nullptr if the length is not supported
+template <typename T> row_kernel_t<T> get_row_fwd(int L);
+template <typename T> row_kernel_t<T> get_row_inv(int L);
+template <typename T> col_kernel_t<T> get_col(int L, int mode, bool multi);
+
+// supported grid sizes (ny and nx independently)
+inline bool size_supported(int n)
+{
+    switch (n) {
+    case 64: case 128: case 256: case 320: case 512: case 640: case 1024: case 1280: case 2048: case 4096: return true;
+    default: return false;
+    }
+}
+
+}  // namespace sgpk

@@ -1,0 +1,260 @@
+// fft_core.cuh -- register-resident Stockham FFT building blocks for sm_100a.
+//
+// One complex FFT of length L is computed by TF = L/E threads; every thread keeps E complex values in
+// registers.  Contract of fft_passes<>: on entry v[e] = x[t + TF*e], on exit v[e] = X[t + TF*e]
+// (t = the thread's index inside its FFT), i.e. both sides are in natural order with the SAME
+// thread/register mapping, so forward transform -> pointwise multiply -> inverse transform needs no
+// data movement in between.  Between two passes the values are exchanged through shared memory
+// (autosort Stockham indexing: out[(j/Ns)*Ns*R + j%Ns + s*Ns], in[j + r*L/R]).
+//
+// This is the FFT that evaluates the convolutions A f and A^T y "by means of FFT".
+#pragma once
+#include <cuda_runtime.h>
+
+namespace sgpk {
+
+template <typename T> struct cx_of;
+template <> struct cx_of<float>  { using type = float2; };
+template <> struct cx_of<double> { using type = double2; };
+template <typename T> using cx = typename cx_of<T>::type;
+
+template <typename T> __device__ __forceinline__ cx<T> mk(T a, T b) { cx<T> r; r.x = a; r.y = b; return r; }
+template <typename C> __device__ __forceinline__ C cadd(C a, C b) { C r; r.x = a.x + b.x; r.y = a.y + b.y; return r; }
+template <typename C> __device__ __forceinline__ C csub(C a, C b) { C r; r.x = a.x - b.x; r.y = a.y - b.y; return r; }
+template <typename C> __device__ __forceinline__ C cmul(C a, C b) { C r; r.x = a.x * b.x - a.y * b.y; r.y = a.x * b.y + a.y * b.x; return r; }
+// a * conj(b)
+template <typename C> __device__ __forceinline__ C cmulc(C a, C b) { C r; r.x = a.x * b.x + a.y * b.y; r.y = a.y * b.x - a.x * b.y; return r; }
+template <typename C> __device__ __forceinline__ C cconj(C a) { C r; r.x = a.x; r.y = -a.y; return r; }
+// multiply by -i (forward, DIR = -1) or +i (inverse, DIR = +1)
+template <int DIR, typename C> __device__ __forceinline__ C mul_dir_i(C a)
+{
+    C r;
+    if (DIR < 0) { r.x = a.y; r.y = -a.x; } else { r.x = -a.y; r.y = a.x; }
+    return r;
+}
+// multiply by cos - i sin (forward) or cos + i sin (inverse): the constant twiddle W_R^k with (c,s) = (cos, sin)(2 pi k / R)
+template <int DIR, typename C, typename T> __device__ __forceinline__ C tw_const(C a, T c, T s)
+{
+    C r;
+    if (DIR < 0) { r.x = a.x * c + a.y * s; r.y = a.y * c - a.x * s; }
+    else         { r.x = a.x * c - a.y * s; r.y = a.y * c + a.x * s; }
+    return r;
+}
+
+// ---------------------------------------------------------------- small DFTs, natural order in and out
+template <int DIR, typename C> __device__ __forceinline__ void dft2(C &a0, C &a1)
+{
+    C t = a0; a0 = cadd(t, a1); a1 = csub(t, a1);
+}
+template <int DIR, typename C> __device__ __forceinline__ void dft4(C &a0, C &a1, C &a2, C &a3)
+{
+    C t0 = cadd(a0, a2), t1 = csub(a0, a2), t2 = cadd(a1, a3), t3 = mul_dir_i<DIR>(csub(a1, a3));
+    a0 = cadd(t0, t2); a1 = cadd(t1, t3); a2 = csub(t0, t2); a3 = csub(t1, t3);
+}
+template <int DIR, typename T, typename C> __device__ __forceinline__ void dft5(C &a0, C &a1, C &a2, C &a3, C &a4)
+{
+    const T c1 = (T)0.30901699437494742410, c2 = (T)-0.80901699437494742410;   // cos(2pi/5), cos(4pi/5)
+    const T s1 = (T)0.95105651629515357212, s2 = (T)0.58778525229247312917;    // sin(2pi/5), sin(4pi/5)
+    C p1 = cadd(a1, a4), p2 = cadd(a2, a3), m1 = csub(a1, a4), m2 = csub(a2, a3);
+    C r1, r2, q1, q2;
+    r1.x = a0.x + c1 * p1.x + c2 * p2.x; r1.y = a0.y + c1 * p1.y + c2 * p2.y;
+    r2.x = a0.x + c2 * p1.x + c1 * p2.x; r2.y = a0.y + c2 * p1.y + c1 * p2.y;
+    q1.x = s1 * m1.x + s2 * m2.x; q1.y = s1 * m1.y + s2 * m2.y;
+    q2.x = s2 * m1.x - s1 * m2.x; q2.y = s2 * m1.y - s1 * m2.y;
+    a0.x = a0.x + p1.x + p2.x; a0.y = a0.y + p1.y + p2.y;
+    C iq1 = mul_dir_i<DIR>(q1), iq2 = mul_dir_i<DIR>(q2);   // forward: -i q
+    a1 = cadd(r1, iq1); a4 = csub(r1, iq1);
+    a2 = cadd(r2, iq2); a3 = csub(r2, iq2);
+}
+
+// In-register DFT of R points, a[r] -> a[s] (natural order).  Composite radices are Cooley-Tukey
+// products R = R1*R2 with input index r = R2*a + b and output index s = s1 + R1*s2.
+template <int R, int DIR, typename T, typename C> __device__ __forceinline__ void dft(C (&a)[R])
+{
+    const T h = (T)0.70710678118654752440;   // sqrt(1/2)
+    if constexpr (R == 2) {
+        dft2<DIR>(a[0], a[1]);
+    } else if constexpr (R == 4) {
+        dft4<DIR>(a[0], a[1], a[2], a[3]);
+    } else if constexpr (R == 5) {
+        dft5<DIR, T>(a[0], a[1], a[2], a[3], a[4]);
+    } else if constexpr (R == 8) {
+        // R1 = 4 (over a), R2 = 2 (b): r = 2a + b
+        dft4<DIR>(a[0], a[2], a[4], a[6]);
+        dft4<DIR>(a[1], a[3], a[5], a[7]);
+        a[3] = tw_const<DIR>(a[3], h, h);            // W8^1  (s1 = 1, b = 1)
+        a[5] = mul_dir_i<DIR>(a[5]);                 // W8^2
+        a[7] = tw_const<DIR>(a[7], -h, h);           // W8^3
+        dft2<DIR>(a[0], a[1]); dft2<DIR>(a[2], a[3]); dft2<DIR>(a[4], a[5]); dft2<DIR>(a[6], a[7]);
+        // position 2*s1 + s2 holds X[s1 + 4*s2]
+        C o1 = a[2], o2 = a[4], o3 = a[6], o4 = a[1], o5 = a[3], o6 = a[5], o7 = a[7];
+        a[1] = o1; a[2] = o2; a[3] = o3; a[4] = o4; a[5] = o5; a[6] = o6; a[7] = o7;
+    } else if constexpr (R == 16) {
+        // R1 = 4, R2 = 4: r = 4a + b
+        const T c1 = (T)0.92387953251128675613, s1 = (T)0.38268343236508977173;   // cos, sin (pi/8)
+#pragma unroll
+        for (int b = 0; b < 4; ++b) dft4<DIR>(a[b], a[4 + b], a[8 + b], a[12 + b]);
+        // u[4*s1 + b] *= W16^(b*s1)
+        a[5]  = tw_const<DIR>(a[5], c1, s1);         // k = 1
+        a[6]  = tw_const<DIR>(a[6], h, h);           // k = 2
+        a[7]  = tw_const<DIR>(a[7], s1, c1);         // k = 3
+        a[9]  = tw_const<DIR>(a[9], h, h);           // k = 2
+        a[10] = mul_dir_i<DIR>(a[10]);               // k = 4
+        a[11] = tw_const<DIR>(a[11], -h, h);         // k = 6
+        a[13] = tw_const<DIR>(a[13], s1, c1);        // k = 3
+        a[14] = tw_const<DIR>(a[14], -h, h);         // k = 6
+        a[15] = tw_const<DIR>(a[15], -c1, -s1);      // k = 9
+#pragma unroll
+        for (int q = 0; q < 4; ++q) dft4<DIR>(a[4 * q], a[4 * q + 1], a[4 * q + 2], a[4 * q + 3]);
+        // position 4*s1 + s2 holds X[s1 + 4*s2]: transpose the 4x4 register tile
+#pragma unroll
+        for (int i = 0; i < 4; ++i)
+#pragma unroll
+            for (int j = i + 1; j < 4; ++j) { C t = a[4 * i + j]; a[4 * i + j] = a[4 * j + i]; a[4 * j + i] = t; }
+    } else if constexpr (R == 20) {
+        // R1 = 4 (over a), R2 = 5 (b): r = 5a + b
+#pragma unroll
+        for (int b = 0; b < 5; ++b) dft4<DIR>(a[b], a[5 + b], a[10 + b], a[15 + b]);
+        // u[5*s1 + b] *= W20^(b*s1); (cos, sin)(2 pi k / 20)
+        const T C1 = (T)0.95105651629515357212, S1 = (T)0.30901699437494742410;   // k = 1
+        const T C2 = (T)0.80901699437494742410, S2 = (T)0.58778525229247312917;   // k = 2
+        const T C3 = (T)0.58778525229247312917, S3 = (T)0.80901699437494742410;   // k = 3
+        const T C4 = (T)0.30901699437494742410, S4 = (T)0.95105651629515357212;   // k = 4
+        a[6]  = tw_const<DIR>(a[6], C1, S1);         // s1=1,b=1: k=1
+        a[7]  = tw_const<DIR>(a[7], C2, S2);         // k=2
+        a[8]  = tw_const<DIR>(a[8], C3, S3);         // k=3
+        a[9]  = tw_const<DIR>(a[9], C4, S4);         // k=4
+        a[11] = tw_const<DIR>(a[11], C2, S2);        // s1=2,b=1: k=2
+        a[12] = tw_const<DIR>(a[12], C4, S4);        // k=4
+        a[13] = tw_const<DIR>(a[13], -S1, C1);       // k=6: cos(108deg) = -sin(18deg), sin(108deg) = cos(18deg)
+        a[14] = tw_const<DIR>(a[14], -C2, S2);       // k=8: cos(144deg), sin(144deg)
+        a[16] = tw_const<DIR>(a[16], C3, S3);        // s1=3,b=1: k=3
+        a[17] = tw_const<DIR>(a[17], -S1, C1);       // k=6
+        a[18] = tw_const<DIR>(a[18], -C1, S1);       // k=9: cos(162deg), sin(162deg)
+        a[19] = tw_const<DIR>(a[19], -C2, -S2);      // k=12: cos(216deg), sin(216deg)
+#pragma unroll
+        for (int q = 0; q < 4; ++q) dft5<DIR, T>(a[5 * q], a[5 * q + 1], a[5 * q + 2], a[5 * q + 3], a[5 * q + 4]);
+        // position 5*s1 + s2 holds X[s1 + 4*s2]
+        C o[20];
+#pragma unroll
+        for (int q = 0; q < 4; ++q)
+#pragma unroll
+            for (int s2 = 0; s2 < 5; ++s2) o[q + 4 * s2] = a[5 * q + s2];
+#pragma unroll
+        for (int i = 0; i < 20; ++i) a[i] = o[i];
+    } else {
+        static_assert(R == 2, "unsupported radix");
+    }
+}
+
+// ---------------------------------------------------------------- plans
+// Elements per thread: 16 (float, 2^k), 8 (double, 2^k), 20 (5*2^k).
+template <typename T> __host__ __device__ constexpr int fft_E(int L)
+{
+    return (L % 5 == 0) ? 20 : (sizeof(T) == 8 ? 8 : 16);
+}
+// radix of pass ip (0 = not a pass of this plan)
+__host__ __device__ constexpr int plan_radix(int L, int E, int ip)
+{
+    if (E == 16) {
+        switch (L) {
+        case 16:   return ip == 0 ? 16 : 0;
+        case 32:   return ip == 0 ? 16 : ip == 1 ? 2 : 0;
+        case 64:   return ip == 0 ? 16 : ip == 1 ? 4 : 0;
+        case 128:  return ip == 0 ? 16 : ip == 1 ? 8 : 0;
+        case 256:  return ip <= 1 ? 16 : 0;
+        case 512:  return ip == 0 ? 16 : ip == 1 ? 8 : ip == 2 ? 4 : 0;
+        case 1024: return ip <= 1 ? 16 : ip == 2 ? 4 : 0;
+        case 2048: return ip <= 1 ? 16 : ip == 2 ? 8 : 0;
+        case 4096: return ip <= 2 ? 16 : 0;
+        }
+    } else if (E == 8) {
+        switch (L) {
+        case 8:    return ip == 0 ? 8 : 0;
+        case 16:   return ip == 0 ? 8 : ip == 1 ? 2 : 0;
+        case 32:   return ip == 0 ? 8 : ip == 1 ? 4 : 0;
+        case 64:   return ip <= 1 ? 8 : 0;
+        case 128:  return ip == 0 ? 8 : ip <= 2 ? 4 : 0;
+        case 256:  return ip <= 1 ? 8 : ip == 2 ? 4 : 0;
+        case 512:  return ip <= 2 ? 8 : 0;
+        case 1024: return ip <= 1 ? 8 : ip <= 3 ? 4 : 0;
+        case 2048: return ip <= 2 ? 8 : ip == 3 ? 4 : 0;
+        case 4096: return ip <= 3 ? 8 : 0;
+        }
+    } else if (E == 20) {
+        switch (L) {
+        case 20:   return ip == 0 ? 20 : 0;
+        case 40:   return ip == 0 ? 20 : ip == 1 ? 2 : 0;
+        case 80:   return ip == 0 ? 20 : ip == 1 ? 4 : 0;
+        case 160:  return ip == 0 ? 20 : ip == 1 ? 4 : ip == 2 ? 2 : 0;
+        case 320:  return ip == 0 ? 20 : ip <= 2 ? 4 : 0;
+        case 640:  return ip == 0 ? 20 : ip <= 2 ? 4 : ip == 3 ? 2 : 0;
+        case 1280: return ip == 0 ? 20 : ip <= 3 ? 4 : 0;
+        }
+    }
+    return 0;
+}
+__host__ __device__ constexpr bool plan_ok(int L, int E) { return plan_radix(L, E, 0) != 0; }
+
+// shared-memory index padding: one extra slot every 16 keeps the stride-R stores of the first pass
+// and the reversed reads of the real<->complex untangling spread over the banks
+__host__ __device__ constexpr int fft_pad(int i) { return i + (i >> 4); }
+__host__ __device__ constexpr int fft_padded_len(int L) { return L + (L >> 4); }
+
+// All passes of one FFT.  sm points at element 0 of this FFT's shared-memory line; consecutive
+// elements are `cs` apart (1 for a row FFT; C for a column FFT stored as [element][column]).
+// tw[k] = exp(-2 pi i k / L).  Every exchange is bracketed sync / store / sync / load, so shared memory
+// the caller used before the call is safe to reuse, and on return nobody is writing it.
+template <typename T, int L, int E, int DIR, int IP, int NS>
+__device__ __forceinline__ void fft_passes(cx<T> (&v)[E], cx<T> *__restrict__ sm, const int cs, const int t,
+                                           const cx<T> *__restrict__ tw)
+{
+    using C = cx<T>;
+    constexpr int R = plan_radix(L, E, IP);
+    static_assert(R > 0 && E % R == 0, "bad plan");
+    constexpr int B = E / R;
+    constexpr int TF = L / E;
+    constexpr bool LAST = (NS * R == L);
+    int j0s[B];
+#pragma unroll
+    for (int b = 0; b < B; ++b) {
+        C a[R];
+#pragma unroll
+        for (int r = 0; r < R; ++r) a[r] = v[b + r * B];
+        const int j = t + b * TF;
+        if constexpr (NS > 1) {
+            const int jm = j % NS;                       // NS is a compile-time constant
+            const int m = jm * (L / (NS * R));
+#pragma unroll
+            for (int r = 1; r < R; ++r) {
+                C w = __ldg(&tw[r * m]);
+                a[r] = (DIR < 0) ? cmul(a[r], w) : cmulc(a[r], w);
+            }
+            j0s[b] = (j / NS) * (NS * R) + jm;
+        } else {
+            j0s[b] = j * R;
+        }
+        dft<R, DIR, T>(a);
+#pragma unroll
+        for (int s = 0; s < R; ++s) v[b + s * B] = a[s];
+    }
+    if constexpr (!LAST) {
+        __syncthreads();
+#pragma unroll
+        for (int b = 0; b < B; ++b)
+#pragma unroll
+            for (int s = 0; s < R; ++s) sm[fft_pad(j0s[b] + s * NS) * cs] = v[b + s * B];
+        __syncthreads();
+#pragma unroll
+        for (int e = 0; e < E; ++e) v[e] = sm[fft_pad(t + TF * e) * cs];
+        fft_passes<T, L, E, DIR, IP + 1, NS * R>(v, sm, cs, t, tw);
+    }
+}
+
+template <typename T, int L, int DIR>
+__device__ __forceinline__ void fft_block(cx<T> (&v)[fft_E<T>(L)], cx<T> *sm, int cs, int t, const cx<T> *tw)
+{
+    fft_passes<T, L, fft_E<T>(L), DIR, 0, 1>(v, sm, cs, t, tw);
+}
+
+}  // namespace sgpk

@@ -1,0 +1,305 @@
+// plan_impl.inl -- included by plan_f32.cu / plan_f64.cu with SGP_T and SGP_MAKE defined.
+#include "plan.cuh"
+
+namespace sgpk {
+
+template <typename T> struct PlanImpl : PlanBase {
+    using C = cx<T>;
+    size_t n = 0, nspec = 0;       // reals per plane, complex numbers per half spectrum (= n/2)
+    int Lr = 0, Lc = 0;            // FFT lengths: nx/2 (rows), ny (columns)
+    int row_threads = 0, col_threads = 0, nrb = 0, ntiles = 0, upd_grid = 0;
+    size_t row_smem = 0, col_smem = 0;
+    row_kernel_t<T> k_rowf = nullptr, k_rowi = nullptr;
+    col_kernel_t<T> k_colf = nullptr, k_conj = nullptr, k_mult = nullptr;
+    // device memory
+    std::vector<void *> allocs;
+    C *tw_r = nullptr, *tw_h = nullptr, *tw_c = nullptr, *pack = nullptr;
+    C *khat = nullptr, *khatB = nullptr, *spec = nullptr;
+    T *Gp = nullptr, *Bp = nullptr, *q = nullptr, *u = nullptr, *f = nullptr, *grad = nullptr, *d = nullptr;
+    T *alphaR = nullptr, *alpha = nullptr, *scratch = nullptr;
+    unsigned char *MR = nullptr;
+    double *part_bb = nullptr, *part_gd = nullptr, *part_J = nullptr, *part_upd = nullptr, *part_misc = nullptr;
+    Ctrl *ct = nullptr;
+    // per-run trace buffers
+    double *trJ = nullptr, *trA = nullptr, *trL = nullptr, *fA = nullptr, *fL = nullptr;
+    int *trR = nullptr, *trB = nullptr;
+    int trace_cap = 0;
+    cudaEvent_t ev0 = nullptr, ev1 = nullptr, ev2 = nullptr;
+
+    ~PlanImpl() override
+    {
+        for (void *a : allocs) cudaFree(a);
+        free_trace();
+        if (ev0) cudaEventDestroy(ev0);
+        if (ev1) cudaEventDestroy(ev1);
+        if (ev2) cudaEventDestroy(ev2);
+    }
+    void free_trace()
+    {
+        cudaFree(trJ); cudaFree(trA); cudaFree(trL); cudaFree(fA); cudaFree(fL); cudaFree(trR); cudaFree(trB);
+        trJ = trA = trL = fA = fL = nullptr; trR = trB = nullptr; trace_cap = 0;
+    }
+    template <typename U> int dalloc(U **ptr, size_t count)
+    {
+        void *raw = nullptr;
+        SGP_CUDA_TRY(cudaMalloc(&raw, count * sizeof(U)));
+        allocs.push_back(raw);
+        bytes_allocated += count * sizeof(U);
+        *ptr = static_cast<U *>(raw);
+        return SGP_OK;
+    }
+
+    int init() override
+    {
+        n = (size_t)ny * nx; nspec = n / 2;
+        Lr = nx / 2; Lc = ny;
+        constexpr int dummy = 0; (void)dummy;
+        const int Er = fft_E<T>(Lr), Ec = fft_E<T>(Lc);
+        k_rowf = get_row_fwd<T>(Lr); k_rowi = get_row_inv<T>(Lr);
+        const bool multi = p > 1;
+        k_colf = get_col<T>(Lc, CM_FWD, false); k_conj = get_col<T>(Lc, CM_CONJSUM, multi); k_mult = get_col<T>(Lc, CM_MULT, multi);
+        if (!k_rowf || !k_rowi || !k_colf || !k_conj || !k_mult) return SGP_ERR_ARG;
+        int Cc = 0, RB = 0;
+        int rc = choose_tiles(ny, nx, dtype, &opt, &Cc, &RB);
+        if (rc) return rc;
+        G.C = Cc; G.RB = RB;
+        row_threads = RB * (Lr / Er);
+        col_threads = Cc * (Lc / Ec);
+        nrb = ny / RB; ntiles = Lr / Cc;
+        row_smem = (size_t)RB * row_stride(Lr) * sizeof(C);
+        col_smem = (size_t)Cc * fft_padded_len(Lc) * sizeof(C);
+        if (row_threads > 512 || col_threads > 512 || row_smem > 227 * 1024 || col_smem > 227 * 1024) return SGP_ERR_ARG;
+        SGP_CUDA_TRY(cudaFuncSetAttribute((const void *)k_rowf, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)row_smem));
+        SGP_CUDA_TRY(cudaFuncSetAttribute((const void *)k_rowi, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)row_smem));
+        SGP_CUDA_TRY(cudaFuncSetAttribute((const void *)k_colf, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)col_smem));
+        SGP_CUDA_TRY(cudaFuncSetAttribute((const void *)k_conj, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)col_smem));
+        SGP_CUDA_TRY(cudaFuncSetAttribute((const void *)k_mult, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)col_smem));
+        // cooperative grid of the update kernel
+        int dev = 0, nsm = 0, per_sm = 0;
+        SGP_CUDA_TRY(cudaGetDevice(&dev));
+        SGP_CUDA_TRY(cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev));
+        SGP_CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, update_kernel<T>, 256, 0));
+        if (per_sm < 1) return SGP_ERR_CUDA;
+        if (per_sm > 8) per_sm = 8;
+        upd_grid = nsm * per_sm;
+        size_t want = (n / vec4_of<T>::N + 255) / 256;
+        if ((size_t)upd_grid > want) upd_grid = (int)(want < 1 ? 1 : want);
+
+        // twiddles, computed in double on the host
+        std::vector<C> h;
+        auto upload = [&](C **dst, int len, int count, bool half) -> int {
+            h.resize(count);
+            for (int k = 0; k < count; ++k) {
+                double a = -2.0 * M_PI * (double)k / (double)len;
+                h[k].x = (T)cos(a); h[k].y = (T)sin(a);
+            }
+            (void)half;
+            int r = dalloc(dst, (size_t)count);
+            if (r) return r;
+            SGP_CUDA_TRY(cudaMemcpy(*dst, h.data(), sizeof(C) * count, cudaMemcpyHostToDevice));
+            return SGP_OK;
+        };
+        if ((rc = upload(&tw_r, Lr, Lr, false))) return rc;
+        if ((rc = upload(&tw_h, nx, Lr + 1, true))) return rc;
+        if ((rc = upload(&tw_c, Lc, Lc, false))) return rc;
+        if ((rc = dalloc(&pack, (size_t)ny))) return rc;
+        if ((rc = dalloc(&khat, nspec * p))) return rc;
+        if ((rc = dalloc(&khatB, (size_t)ny * p))) return rc;
+        if ((rc = dalloc(&spec, nspec * p))) return rc;
+        if ((rc = dalloc(&Gp, n * p))) return rc;
+        if ((rc = dalloc(&Bp, n * p))) return rc;
+        if ((rc = dalloc(&q, n * p))) return rc;
+        if ((rc = dalloc(&u, n * p))) return rc;
+        if ((rc = dalloc(&f, n))) return rc;
+        if ((rc = dalloc(&grad, n))) return rc;
+        if ((rc = dalloc(&d, n))) return rc;
+        if ((rc = dalloc(&scratch, n))) return rc;
+        if (G.masked) {
+            if ((rc = dalloc(&alphaR, n))) return rc;
+            if ((rc = dalloc(&alpha, n))) return rc;
+            if ((rc = dalloc(&MR, n))) return rc;
+        }
+        if ((rc = dalloc(&part_bb, (size_t)nrb * 4))) return rc;
+        if ((rc = dalloc(&part_gd, (size_t)nrb))) return rc;
+        if ((rc = dalloc(&part_J, (size_t)nrb * p * 2))) return rc;
+        if ((rc = dalloc(&part_upd, (size_t)upd_grid))) return rc;
+        if ((rc = dalloc(&part_misc, (size_t)1024 * p))) return rc;
+        if ((rc = dalloc(&ct, (size_t)1))) return rc;
+        SGP_CUDA_TRY(cudaMemset(ct, 0, sizeof(Ctrl)));
+        SGP_CUDA_TRY(cudaEventCreate(&ev0));
+        SGP_CUDA_TRY(cudaEventCreate(&ev1));
+        SGP_CUDA_TRY(cudaEventCreate(&ev2));
+        return SGP_OK;
+    }
+
+    // ------------------------------------------------------------------ launch helpers
+    RowParams<T> row_params(int mode) const
+    {
+        RowParams<T> P;
+        memset(&P, 0, sizeof(P));
+        P.G = G; P.ct = ct; P.mode = mode;
+        P.plane = n; P.specplane = nspec; P.spec = spec;
+        P.tw = tw_r; P.twh = tw_h; P.alphaR = alphaR;
+        return P;
+    }
+    int launch_row(row_kernel_t<T> k, const RowParams<T> &P, int images, cudaStream_t st)
+    {
+        k<<<dim3(nrb, images), row_threads, row_smem, st>>>(P);
+        launches++;
+        SGP_CUDA_TRY(cudaGetLastError());
+        return SGP_OK;
+    }
+    ColParams<T> col_params() const
+    {
+        ColParams<T> P;
+        memset(&P, 0, sizeof(P));
+        P.G = G; P.ct = ct; P.in = spec; P.out = spec; P.khat = khat; P.khatB = khatB;
+        P.specplane = nspec; P.tw = tw_c; P.pack = pack; P.p = p;
+        return P;
+    }
+    int launch_col(col_kernel_t<T> k, const ColParams<T> &P, cudaStream_t st)
+    {
+        k<<<ntiles, col_threads, col_smem, st>>>(P);
+        launches++;
+        SGP_CUDA_TRY(cudaGetLastError());
+        return SGP_OK;
+    }
+    static int ew_grid(size_t count) { size_t b = (count + 255) / 256; return (int)(b > 1184 ? 1184 : (b < 1 ? 1 : b)); }
+
+    // ------------------------------------------------------------------ transfer functions and boundary weights
+    int set_psf(const void *const *psf, cudaStream_t st) override
+    {
+        if (!psf) return SGP_ERR_ARG;
+        for (int j = 0; j < p; ++j) if (!psf[j]) return SGP_ERR_ARG;
+        const int cy = opt.psf_origin == SGP_PSF_CENTER ? ny / 2 : 0, cxs = opt.psf_origin == SGP_PSF_CENTER ? nx / 2 : 0;
+        int rc;
+        for (int j = 0; j < p; ++j) {
+            plane_sum_kernel<T><<<1, 1024, 0, st>>>((const T *)psf[j], n, ct);
+            launches++;
+            Ctrl h;
+            SGP_CUDA_TRY(cudaMemcpyAsync(&h, ct, sizeof(Ctrl), cudaMemcpyDeviceToHost, st));
+            SGP_CUDA_TRY(cudaStreamSynchronize(st));
+            if (!(h.psf_sum > 0.0) || !std::isfinite(h.psf_sum)) return SGP_ERR_PSF;       // PAPER.md:27 needs a positive volume
+            RowParams<T> P = row_params(RF_PSF);
+            P.in0 = (const T *)psf[j]; P.cy = cy; P.cxs = cxs;
+            P.spec = (C *)scratch;          // raw spectrum of this PSF
+            if ((rc = launch_row(k_rowf, P, 1, st))) return rc;
+            ColParams<T> Q = col_params();
+            Q.in = (const C *)scratch; Q.out = (C *)scratch;
+            if ((rc = launch_col(k_colf, Q, st))) return rc;
+            khat_fixup_kernel<T><<<ew_grid(nspec), 256, 0, st>>>((const C *)scratch, khat + (size_t)j * nspec, khatB + (size_t)j * ny, ny, nx, G.C);
+            launches++;
+            SGP_CUDA_TRY(cudaGetLastError());
+        }
+        if (G.masked) {
+            // alpha_j = A_j^T 1_S = IFFT2(conj K^_j FFT2(M_S)) (Eq.19 in reading A5), alpha = sum_j alpha_j, R by Eq.20
+            for (int j = 0; j < p; ++j) {
+                RowParams<T> P = row_params(RF_MASK_S);
+                if ((rc = launch_row(k_rowf, P, 1, st))) return rc;
+                ColParams<T> Q = col_params();
+                Q.khat = khat + (size_t)j * nspec; Q.khatB = khatB + (size_t)j * ny; Q.p = 1;
+                col_kernel_t<T> k1 = get_col<T>(Lc, CM_CONJSUM, false);
+                SGP_CUDA_TRY(cudaFuncSetAttribute((const void *)k1, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)col_smem));
+                if ((rc = launch_col(k1, Q, st))) return rc;
+                RowParams<T> R = row_params(RI_PLAIN);
+                R.out0 = scratch; R.maskmode = MM_NONE;
+                if ((rc = launch_row(k_rowi, R, 1, st))) return rc;
+                alpha_accum_kernel<T><<<ew_grid(n), 256, 0, st>>>(scratch, alpha, MR, n, opt.sigma_R, j == 0);
+                launches++;
+            }
+            alpha_finish_kernel<T><<<ew_grid(n), 256, 0, st>>>(alpha, MR, alphaR, n);
+            launches++;
+            SGP_CUDA_TRY(cudaGetLastError());
+            std::vector<unsigned char> hm(n);
+            SGP_CUDA_TRY(cudaMemcpyAsync(hm.data(), MR, n, cudaMemcpyDeviceToHost, st));
+            SGP_CUDA_TRY(cudaStreamSynchronize(st));
+            nR = 0;
+            for (size_t i = 0; i < n; ++i) nR += hm[i];
+        } else {
+            nR = (long)n;
+        }
+        SGP_CUDA_TRY(cudaStreamSynchronize(st));
+        psf_set = true;
+        return SGP_OK;
+    }
+
+    int get_mask(unsigned char *maskR_out, void *alpha_out, long *nR_out, cudaStream_t st) override
+    {
+        if (!psf_set) return SGP_ERR_ARG;
+        if (G.masked) {
+            if (maskR_out) SGP_CUDA_TRY(cudaMemcpyAsync(maskR_out, MR, n, cudaMemcpyDeviceToDevice, st));
+            if (alpha_out) SGP_CUDA_TRY(cudaMemcpyAsync(alpha_out, alpha, n * sizeof(T), cudaMemcpyDeviceToDevice, st));
+        } else {
+            if (maskR_out) SGP_CUDA_TRY(cudaMemsetAsync(maskR_out, 1, n, st));
+            if (alpha_out) {
+                std::vector<T> h(n, (T)p);
+                SGP_CUDA_TRY(cudaMemcpyAsync(alpha_out, h.data(), n * sizeof(T), cudaMemcpyHostToDevice, st));
+            }
+        }
+        SGP_CUDA_TRY(cudaStreamSynchronize(st));
+        if (nR_out) *nR_out = nR;
+        return SGP_OK;
+    }
+
+    // out = A_j x (Eq.16) or A_j^T x (Eq.17)
+    int apply(bool transpose, int j, const void *x, void *out, cudaStream_t st) override
+    {
+        if (!psf_set || j < 0 || j >= p || !x || !out) return SGP_ERR_ARG;
+        int rc;
+        RowParams<T> P = row_params(RF_PLAIN);
+        P.in0 = (const T *)x; P.maskmode = transpose ? MM_S : MM_R;
+        if ((rc = launch_row(k_rowf, P, 1, st))) return rc;
+        ColParams<T> Q = col_params();
+        Q.khat = khat + (size_t)j * nspec; Q.khatB = khatB + (size_t)j * ny; Q.p = 1;
+        col_kernel_t<T> k1 = get_col<T>(Lc, transpose ? CM_CONJSUM : CM_MULT, false);
+        SGP_CUDA_TRY(cudaFuncSetAttribute((const void *)k1, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)col_smem));
+        if ((rc = launch_col(k1, Q, st))) return rc;
+        RowParams<T> R = row_params(RI_PLAIN);
+        R.out0 = scratch; R.maskmode = transpose ? MM_R : MM_S;
+        if ((rc = launch_row(k_rowi, R, 1, st))) return rc;
+        SGP_CUDA_TRY(cudaMemcpyAsync(out, scratch, n * sizeof(T), cudaMemcpyDeviceToDevice, st));
+        SGP_CUDA_TRY(cudaStreamSynchronize(st));
+        return SGP_OK;
+    }
+
+    int rfft2(const void *x, void *spec_out, cudaStream_t st) override
+    {
+        if (!x || !spec_out) return SGP_ERR_ARG;
+        int rc;
+        RowParams<T> P = row_params(RF_PLAIN);
+        P.in0 = (const T *)x;
+        if ((rc = launch_row(k_rowf, P, 1, st))) return rc;
+        ColParams<T> Q = col_params();
+        if ((rc = launch_col(k_colf, Q, st))) return rc;
+        spec_to_rfft2_kernel<T><<<ew_grid(n), 256, 0, st>>>(spec, (C *)spec_out, ny, nx, G.C);
+        launches++;
+        SGP_CUDA_TRY(cudaGetLastError());
+        SGP_CUDA_TRY(cudaStreamSynchronize(st));
+        return SGP_OK;
+    }
+    int irfft2(const void *spec_in, void *x_out, cudaStream_t st) override
+    {
+        if (!spec_in || !x_out) return SGP_ERR_ARG;
+        int rc;
+        rfft2_to_spec_kernel<T><<<ew_grid(nspec), 256, 0, st>>>((const C *)spec_in, spec, ny, nx, G.C, (T)(1.0 / ((double)ny * (double)nx)));
+        launches++;
+        SGP_CUDA_TRY(cudaGetLastError());
+        col_kernel_t<T> ki = get_col<T>(Lc, CM_INV, false);
+        SGP_CUDA_TRY(cudaFuncSetAttribute((const void *)ki, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)col_smem));
+        ColParams<T> Q = col_params();
+        if ((rc = launch_col(ki, Q, st))) return rc;
+        RowParams<T> R = row_params(RI_PLAIN);
+        R.out0 = (T *)x_out; R.maskmode = MM_NONE;
+        if ((rc = launch_row(k_rowi, R, 1, st))) return rc;
+        SGP_CUDA_TRY(cudaStreamSynchronize(st));
+        return SGP_OK;
+    }
+
+    int run(int algorithm, const void *const *g, const void *const *b_arr, const double *b_const,
+            const void *f0, void *f_out, const sgp_options *ropt, sgp_result *res, cudaStream_t st) override;
+    int ensure_trace(int max_iter, const sgp_result *res, Trace *tr, cudaStream_t st);
+    int enqueue_sgp_iteration(const RowParams<T> &Pbase, const DevOpts &o, const Trace &tr, const double *bconst, int b_is_array, cudaStream_t st);
+    int enqueue_rl_round(const DevOpts &o, const Trace &tr, const double *bconst, int b_is_array, cudaStream_t st);
+};
+
+}  // namespace sgpk

@@ -1,0 +1,244 @@
+// plan_run.inl -- the iteration drivers of PlanImpl<T> (included after plan_impl.inl).
+//
+// Nothing in the loops below waits for the device: the step length, the Armijo decision, the
+// stopping rules and the traces are computed by device code (sgp_dev.cuh); kernels return at once when
+// the device status is no longer "running".  The host reads the control block only every
+// `check_every` iterations (once, at the end, for a fixed iteration count).
+namespace sgpk {
+
+template <typename T>
+int PlanImpl<T>::ensure_trace(int max_iter, const sgp_result *res, Trace *tr, cudaStream_t st)
+{
+    const int need = max_iter + 1;
+    if (need > trace_cap) {
+        free_trace();
+        SGP_CUDA_TRY(cudaMalloc((void **)&trJ, sizeof(double) * need));
+        SGP_CUDA_TRY(cudaMalloc((void **)&trA, sizeof(double) * need));
+        SGP_CUDA_TRY(cudaMalloc((void **)&trL, sizeof(double) * need));
+        SGP_CUDA_TRY(cudaMalloc((void **)&fA, sizeof(double) * need));
+        SGP_CUDA_TRY(cudaMalloc((void **)&fL, sizeof(double) * need));
+        SGP_CUDA_TRY(cudaMalloc((void **)&trR, sizeof(int) * need));
+        SGP_CUDA_TRY(cudaMalloc((void **)&trB, sizeof(int) * need));
+        trace_cap = need;
+    }
+    SGP_CUDA_TRY(cudaMemsetAsync(trJ, 0, sizeof(double) * need, st));
+    SGP_CUDA_TRY(cudaMemsetAsync(trA, 0, sizeof(double) * need, st));
+    SGP_CUDA_TRY(cudaMemsetAsync(trL, 0, sizeof(double) * need, st));
+    SGP_CUDA_TRY(cudaMemsetAsync(trR, 0, sizeof(int) * need, st));
+    SGP_CUDA_TRY(cudaMemsetAsync(trB, 0, sizeof(int) * need, st));
+    tr->J = trJ; tr->alpha = trA; tr->lambda = trL; tr->rule = trR; tr->backtracks = trB;
+    tr->force_alpha = nullptr; tr->force_lambda = nullptr;
+    if (res->force_alpha && max_iter > 0) {
+        SGP_CUDA_TRY(cudaMemcpyAsync(fA, res->force_alpha, sizeof(double) * max_iter, cudaMemcpyHostToDevice, st));
+        tr->force_alpha = fA;
+    }
+    if (res->force_lambda && max_iter > 0) {
+        SGP_CUDA_TRY(cudaMemcpyAsync(fL, res->force_lambda, sizeof(double) * max_iter, cudaMemcpyHostToDevice, st));
+        tr->force_lambda = fL;
+    }
+    return SGP_OK;
+}
+
+// One SGP iteration = 7 launches (SURVEY.md 8(d) schedule A): K1 ratio + row FFT, K2 column pass with conj(K^) summed
+// over the images, K3 inverse rows + gradient + BB sums + step length, K4 projection + row FFT of d, K5 column pass
+// with K^_j, K6 inverse rows + u_j + J(lambda = 1) + Armijo test, K7 backtracks (elementwise) + update + book-keeping.
+template <typename T>
+int PlanImpl<T>::enqueue_sgp_iteration(const RowParams<T> &Pb, const DevOpts &o, const Trace &tr, const double *bconst,
+                                       int b_is_array, cudaStream_t st)
+{
+    int rc;
+    {   // K1 (a1)
+        RowParams<T> P = Pb; P.mode = RF_RATIO; P.in0 = Gp; P.in1 = q; P.in2 = Bp;
+        if ((rc = launch_row(k_rowf, P, p, st))) return rc;
+    }
+    {   // K2 (a2)
+        ColParams<T> Q = col_params(); Q.check_status = 1;
+        if ((rc = launch_col(k_conj, Q, st))) return rc;
+    }
+    {   // K3 (a3, a5, a6)
+        RowParams<T> P = Pb; P.mode = RI_GRAD; P.in0 = f; P.in1 = d; P.out0 = grad; P.part = part_bb;
+        if ((rc = launch_row(k_rowi, P, 1, st))) return rc;
+    }
+    {   // K4 (a4, a7)
+        RowParams<T> P = Pb; P.mode = RF_PROJECT; P.in0 = f; P.in1 = grad; P.out0 = d; P.part = part_gd;
+        if ((rc = launch_row(k_rowf, P, 1, st))) return rc;
+    }
+    {   // K5 (a8)
+        ColParams<T> Q = col_params(); Q.check_status = 1;
+        if ((rc = launch_col(k_mult, Q, st))) return rc;
+    }
+    {   // K6 (a8 tail, a9 at lambda = 1)
+        RowParams<T> P = Pb; P.mode = RI_LS; P.in0 = Gp; P.in1 = q; P.in2 = Bp; P.out0 = u; P.part = part_J; P.part2 = part_gd;
+        if ((rc = launch_row(k_rowi, P, p, st))) return rc;
+    }
+    {   // K7 (a9 backtracks, a10, a11)
+        UpdParams<T> U;
+        memset(&U, 0, sizeof(U));
+        U.G = G; U.o = o; U.tr = tr; U.ct = ct; U.f = f; U.d = d; U.q = q; U.u = u; U.g = Gp; U.b = Bp;
+        U.plane = n; U.b_is_array = b_is_array; U.part = part_upd;
+        for (int j = 0; j < p; ++j) U.bconst[j] = bconst[j];
+        void *args[] = {(void *)&U};
+        SGP_CUDA_TRY(cudaLaunchCooperativeKernel((const void *)update_kernel<T>, dim3(upd_grid), dim3(256), args, 0, st));
+        launches++;
+    }
+    return SGP_OK;
+}
+
+// One RL round (Eq.1/13/21): q_j = A_j f and J0(f(k)) with the stopping rules, then the multiplicative update.
+template <typename T>
+int PlanImpl<T>::enqueue_rl_round(const DevOpts &o, const Trace &tr, const double *bconst, int b_is_array, cudaStream_t st)
+{
+    int rc;
+    RowParams<T> Pb = row_params(RF_PLAIN);
+    Pb.o = o; Pb.tr = tr; Pb.check_status = 1; Pb.b_is_array = b_is_array;
+    for (int j = 0; j < p; ++j) Pb.bconst[j] = bconst[j];
+    { RowParams<T> P = Pb; P.mode = RF_PLAIN; P.in0 = f; P.maskmode = MM_NONE; if ((rc = launch_row(k_rowf, P, 1, st))) return rc; }
+    { ColParams<T> Q = col_params(); Q.check_status = 1; if ((rc = launch_col(k_mult, Q, st))) return rc; }
+    { RowParams<T> P = Pb; P.mode = RI_QJ; P.submode = QJ_RL; P.in0 = Gp; P.in2 = Bp; P.out0 = q; P.part = part_J; if ((rc = launch_row(k_rowi, P, p, st))) return rc; }
+    { RowParams<T> P = Pb; P.mode = RF_RATIO; P.in0 = Gp; P.in1 = q; P.in2 = Bp; if ((rc = launch_row(k_rowf, P, p, st))) return rc; }
+    { ColParams<T> Q = col_params(); Q.check_status = 1; if ((rc = launch_col(k_conj, Q, st))) return rc; }
+    { RowParams<T> P = Pb; P.mode = RI_RLUPDATE; P.in0 = f; P.out0 = f; if ((rc = launch_row(k_rowi, P, 1, st))) return rc; }
+    return SGP_OK;
+}
+
+template <typename T>
+int PlanImpl<T>::run(int algorithm, const void *const *g, const void *const *b_arr, const double *b_const,
+                     const void *f0, void *f_out, const sgp_options *ropt, sgp_result *res, cudaStream_t st)
+{
+    if (!psf_set || !g || !f_out || !res) return SGP_ERR_ARG;
+    if (!b_arr && !b_const) return SGP_ERR_ARG;
+    if (algorithm != SGP_ALG_SGP && algorithm != SGP_ALG_RL) return SGP_ERR_ARG;
+    sgp_options ro = ropt ? *ropt : opt;
+    int rc = validate_options(&ro);
+    if (rc) return rc;
+    if (ro.refresh_every != 0) return SGP_ERR_UNSUPPORTED;
+    if (ro.init == SGP_INIT_USER && !f0) return SGP_ERR_ARG;
+    for (int j = 0; j < p; ++j) if (!g[j]) return SGP_ERR_ARG;
+    int b_is_array = 0;
+    double bconst[kMaxP] = {0};
+    for (int j = 0; j < p; ++j) {
+        const bool arr = b_arr && b_arr[j];
+        if (j == 0) b_is_array = arr ? 1 : 0;
+        else if ((arr ? 1 : 0) != b_is_array) return SGP_ERR_ARG;     // all arrays or all constants
+        if (!arr) { if (!b_const) return SGP_ERR_ARG; bconst[j] = b_const[j]; }
+    }
+    const long launches0 = launches;
+
+    DevOpts o;
+    memset(&o, 0, sizeof(o));
+    o.beta = ro.beta; o.theta = ro.theta; o.alpha0 = ro.alpha0; o.alpha_min = ro.alpha_min; o.alpha_max = ro.alpha_max;
+    o.tol = ro.tol; o.disc_threshold = ro.disc_threshold; o.m_alpha = ro.m_alpha; o.alt_start = ro.alt_start;
+    o.armijo_memory = ro.armijo_memory; o.max_iter = ro.max_iter; o.stop_rule = ro.stop_rule;
+    o.max_backtracks = ro.max_backtracks; o.adaptive_L = ro.adaptive_L; o.p = p;
+    o.nS_total = (double)p * (double)G.sy * (double)G.sx;
+
+    Trace tr;
+    if ((rc = ensure_trace(ro.max_iter, res, &tr, st))) return rc;
+
+    // ---- start-point phase (a0''): clean inputs, f(0), q_j = A_j f(0), J0(f(0)), adaptive bounds
+    SGP_CUDA_TRY(cudaEventRecord(ev0, st));
+    Ctrl h;
+    memset(&h, 0, sizeof(h));
+    h.alpha_prev = ro.alpha0; h.tau = ro.tau1; h.L1 = ro.L1; h.L2 = ro.L2; h.lambda = 1.0;
+    SGP_CUDA_TRY(cudaMemcpyAsync(ct, &h, sizeof(Ctrl), cudaMemcpyHostToDevice, st));
+    const int eg = ew_grid(n) > 1024 ? 1024 : ew_grid(n);
+    for (int j = 0; j < p; ++j) {
+        embed_inputs_kernel<T><<<eg, 256, 0, st>>>((const T *)g[j], b_is_array ? (const T *)b_arr[j] : nullptr, Gp + (size_t)j * n,
+                                                   b_is_array ? Bp + (size_t)j * n : nullptr, G, bconst[j], ro.strict, ct,
+                                                   part_misc + (size_t)j * 1024);
+        launches++;
+        if (eg < 1024) SGP_CUDA_TRY(cudaMemsetAsync(part_misc + (size_t)j * 1024 + eg, 0, sizeof(double) * (1024 - eg), st));
+    }
+    const_start_kernel<T><<<1, 32, 0, st>>>(part_misc, 1024 * p, o.nS_total, ct);
+    launches++;
+    start_point_kernel<T><<<ew_grid(n), 256, 0, st>>>(f, (const T *)f0, Gp, alphaR, G, ro.init, ct);
+    launches++;
+    SGP_CUDA_TRY(cudaGetLastError());
+
+    RowParams<T> Pb = row_params(RF_PLAIN);
+    Pb.o = o; Pb.tr = tr; Pb.check_status = 1; Pb.b_is_array = b_is_array;
+    for (int j = 0; j < p; ++j) Pb.bconst[j] = bconst[j];
+
+    if (algorithm == SGP_ALG_SGP) {
+        { RowParams<T> P = Pb; P.mode = RF_PLAIN; P.in0 = f; if ((rc = launch_row(k_rowf, P, 1, st))) return rc; }
+        { ColParams<T> Q = col_params(); Q.check_status = 1; if ((rc = launch_col(k_mult, Q, st))) return rc; }
+        { RowParams<T> P = Pb; P.mode = RI_QJ; P.submode = QJ_INIT; P.in0 = Gp; P.in2 = Bp; P.out0 = q; P.part = part_J;
+          if ((rc = launch_row(k_rowi, P, p, st))) return rc; }
+        if (ro.adaptive_L) {     // bounds from one RL step
+            { RowParams<T> P = Pb; P.mode = RF_RATIO; P.in0 = Gp; P.in1 = q; P.in2 = Bp; if ((rc = launch_row(k_rowf, P, p, st))) return rc; }
+            { ColParams<T> Q = col_params(); Q.check_status = 1; if ((rc = launch_col(k_conj, Q, st))) return rc; }
+            { RowParams<T> P = Pb; P.mode = RI_RLMINMAX; P.in0 = f; P.part = part_J; if ((rc = launch_row(k_rowi, P, 1, st))) return rc; }
+        }
+    }
+    SGP_CUDA_TRY(cudaEventRecord(ev1, st));
+    SGP_CUDA_TRY(cudaMemcpyAsync(&h, ct, sizeof(Ctrl), cudaMemcpyDeviceToHost, st));
+    SGP_CUDA_TRY(cudaStreamSynchronize(st));
+    int status = h.status;
+    if (h.flag_data & 1) status = SGP_ERR_DATA;
+    else if (h.flag_data & 2) status = SGP_ERR_DATA;
+    else if (h.flag_data & 4) status = SGP_ERR_DATA;
+
+    // ---- iteration loop
+    long fft2 = 0;
+    if (status == 0) {
+        int chunk = ro.check_every > 0 ? ro.check_every : (ro.stop_rule == SGP_STOP_MAXIT ? 200 : 20);
+        if (algorithm == SGP_ALG_SGP) {
+            if (ro.max_iter == 0) status = SGP_REASON_MAXIT;
+            int done = 0;
+            while (status == 0) {
+                int todo = ro.max_iter - done; if (todo > chunk) todo = chunk;
+                if (todo < 1) { status = SGP_REASON_MAXIT; break; }
+                for (int i = 0; i < todo; ++i)
+                    if ((rc = enqueue_sgp_iteration(Pb, o, tr, bconst, b_is_array, st))) return rc;
+                SGP_CUDA_TRY(cudaMemcpyAsync(&h, ct, sizeof(Ctrl), cudaMemcpyDeviceToHost, st));
+                SGP_CUDA_TRY(cudaStreamSynchronize(st));
+                status = h.status; done = h.k;
+                if (status == 0 && done >= ro.max_iter) status = SGP_REASON_MAXIT;   // not reachable: the device sets it
+            }
+            fft2 = (long)h.k * (2 * p + 2);
+        } else {
+            int rounds = 0;     // round k evaluates J0(f(k)) and, unless a rule fires, makes update k+1
+            while (status == 0) {
+                int todo = ro.max_iter + 1 - rounds; if (todo > chunk) todo = chunk; if (todo < 1) todo = 1;
+                for (int i = 0; i < todo; ++i)
+                    if ((rc = enqueue_rl_round(o, tr, bconst, b_is_array, st))) return rc;
+                rounds += todo;
+                SGP_CUDA_TRY(cudaMemcpyAsync(&h, ct, sizeof(Ctrl), cudaMemcpyDeviceToHost, st));
+                SGP_CUDA_TRY(cudaStreamSynchronize(st));
+                status = h.status;
+            }
+            fft2 = (long)h.k * (2 * p + 2) + (p + 1);
+        }
+    }
+    SGP_CUDA_TRY(cudaEventRecord(ev2, st));
+    copy_plane_kernel<T><<<ew_grid(n), 256, 0, st>>>(f, (T *)f_out, n);
+    launches++;
+    SGP_CUDA_TRY(cudaGetLastError());
+    const int kdone = h.k;
+    if (res->trace_J) SGP_CUDA_TRY(cudaMemcpyAsync(res->trace_J, trJ, sizeof(double) * (kdone + 1), cudaMemcpyDeviceToHost, st));
+    if (kdone > 0) {
+        if (res->trace_alpha) SGP_CUDA_TRY(cudaMemcpyAsync(res->trace_alpha, trA, sizeof(double) * kdone, cudaMemcpyDeviceToHost, st));
+        if (res->trace_lambda) SGP_CUDA_TRY(cudaMemcpyAsync(res->trace_lambda, trL, sizeof(double) * kdone, cudaMemcpyDeviceToHost, st));
+        if (res->trace_rule) SGP_CUDA_TRY(cudaMemcpyAsync(res->trace_rule, trR, sizeof(int) * kdone, cudaMemcpyDeviceToHost, st));
+        if (res->trace_backtracks) SGP_CUDA_TRY(cudaMemcpyAsync(res->trace_backtracks, trB, sizeof(int) * kdone, cudaMemcpyDeviceToHost, st));
+    }
+    SGP_CUDA_TRY(cudaStreamSynchronize(st));
+    float ms01 = 0.f, ms12 = 0.f;
+    cudaEventElapsedTime(&ms01, ev0, ev1);
+    cudaEventElapsedTime(&ms12, ev1, ev2);
+    res->iterations = kdone;
+    res->stop_reason = status > 0 ? status : 0;
+    res->J0_final = h.J;
+    res->discrepancy_final = 2.0 * h.J / o.nS_total;
+    res->total_backtracks = h.total_backtracks;
+    res->L1_used = algorithm == SGP_ALG_SGP ? h.L1 : 0.0;
+    res->L2_used = algorithm == SGP_ALG_SGP ? h.L2 : 0.0;
+    res->n_fft2 = fft2;
+    res->setup_ms = ms01; res->loop_ms = ms12;
+    res->kernel_launches = launches - launches0;
+    return status < 0 ? status : SGP_OK;
+}
+
+PlanBase *SGP_MAKE() { return new PlanImpl<SGP_T>(); }
+
+}  // namespace sgpk

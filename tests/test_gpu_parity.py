@@ -1,0 +1,327 @@
+"""GPU parity tests: the CUDA path (through the C ABI, via paper_1210_2258_b200.binding) against the CPU
+oracle (oracle/, plain C, fp64) on the same seeded synthetic inputs.
+
+Tolerances are the ones BASELINE.json's north_star states: fp32 relative L2 of f <= 1e-5 after one
+iteration and <= 1e-3 after 100, J0 within 1e-4 relative, same stopping iteration +-1; fp64 mode <= 1e-10.
+"""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+
+import oracle  # noqa: E402  (test infrastructure)
+from paper_1210_2258_b200 import binding as B  # noqa: E402
+from paper_1210_2258_b200 import synth  # noqa: E402
+
+
+def _need_gpu():
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+
+
+def dev(a, dt):
+    return torch.as_tensor(np.ascontiguousarray(a, dtype=dt), device="cuda")
+
+
+def rel_l2(a, b):
+    cplx = np.iscomplexobj(a) or np.iscomplexobj(b)
+    a = np.asarray(a, np.complex128 if cplx else np.float64); b = np.asarray(b, np.complex128 if cplx else np.float64)
+    return float(np.linalg.norm(a - b) / max(np.linalg.norm(b), 1e-300))
+
+
+TDT = {np.float32: torch.float32, np.float64: torch.float64}
+_ORACLE_CACHE = {}
+
+
+def gpu_plan(w, dt, **optkw):
+    o = B.default_options(**{**w["opts"], **optkw})
+    psfs = [dev(k, dt) for k in w["psf"]]
+    return B.Plan(psfs, S=w["S"], opts=o), o
+
+
+def oracle_opts(w, **optkw):
+    kw = {**w["opts"], **optkw}
+    kw = {k: v for k, v in kw.items() if k not in ("check_every", "tile_cols", "rows_per_block", "use_graph", "backend")}
+    return oracle.default_options(**kw)
+
+
+def oracle_problem(w, o):
+    return oracle.Problem(w["psf"], masked=w["S"] is not None, S=w["S"], sigma_R=o.sigma_R)
+
+
+def run_both(w, dt, alg="sgp", **optkw):
+    """returns (f_gpu, res_gpu, f_oracle, res_oracle)"""
+    _need_gpu()
+    plan, o = gpu_plan(w, dt, **optkw)
+    g = [dev(a, dt) for a in w["g"]]
+    fg, rg = (plan.sgp if alg == "sgp" else plan.rl)(g, w["b"], opts=o)
+    torch.cuda.synchronize()
+    plan.close()
+    key = (w["name"], alg, tuple(sorted({**w["opts"], **optkw}.items())))
+    if key not in _ORACLE_CACHE:          # the fp64 oracle result serves both the fp32 and the fp64 GPU run
+        oo = oracle_opts(w, **optkw)
+        P = oracle_problem(w, oo)
+        ge = P.embed(w["g"]); be = [np.full((P.ny, P.nx), float(v)) for v in w["b"]]
+        _ORACLE_CACHE[key] = (P.sgp if alg == "sgp" else P.rl)(ge, be, opts=oo)
+    fo, ro = _ORACLE_CACHE[key]
+    return fg.cpu().numpy(), rg, fo, ro
+
+
+# ------------------------------------------------------------------------------------------------ FFT
+@pytest.mark.parametrize("ny,nx", [(64, 64), (128, 64), (64, 320), (256, 256), (320, 128), (512, 1024), (1280, 640), (2048, 2048)])
+@pytest.mark.parametrize("dt", [np.float32, np.float64])
+def test_rfft2_matches_numpy(ny, nx, dt):
+    """the library's own FFT kernels (row R2C + column pass, tile-major spectrum) against numpy.fft.rfft2,
+    and the round trip through irfft2"""
+    _need_gpu()
+    rng = np.random.default_rng(ny * 7 + nx)
+    x = rng.standard_normal((ny, nx))
+    delta = np.zeros((ny, nx)); delta[0, 0] = 1.0; delta /= delta.sum()
+    plan = B.Plan([dev(delta + 1.0 / (ny * nx), dt)])
+    X = plan.rfft2(dev(x, dt)).cpu().numpy()
+    ref = np.fft.rfft2(x)
+    tol = 2e-6 if dt == np.float32 else 1e-13
+    assert rel_l2(X, ref) < tol
+    xb = plan.irfft2(dev(ref, np.complex64 if dt == np.float32 else np.complex128)).cpu().numpy()
+    assert rel_l2(xb, x) < tol
+    plan.close()
+
+
+# ------------------------------------------------------------------------------------------------ operators
+@pytest.mark.parametrize("dt", [np.float32, np.float64])
+def test_operators_periodic(dt):
+    """A x and A^T y (Eq.16-17, M_S = M_R = 1) against the oracle, 3 PSFs on a non-square grid"""
+    _need_gpu()
+    ny, nx = 128, 256
+    rng = np.random.default_rng(5)
+    psfs = [synth.psf_gaussian(ny, nx, 1.5 + j) * (1 + 0.3 * rng.random((ny, nx))) for j in range(3)]
+    P = oracle.Problem(psfs)
+    plan = B.Plan([dev(k, dt) for k in psfs])
+    x = rng.random((ny, nx)) * 100
+    tol = 3e-6 if dt == np.float32 else 1e-12
+    for j in range(3):
+        assert rel_l2(plan.apply_A(j, dev(x, dt)).cpu().numpy(), P.A(j, x)) < tol
+        assert rel_l2(plan.apply_AT(j, dev(x, dt)).cpu().numpy(), P.AT(j, x)) < tol
+    plan.close()
+
+
+@pytest.mark.parametrize("dt", [np.float32, np.float64])
+def test_operators_boundary(dt):
+    """masked operators, alpha and M_R (Eq.16-20) against the oracle: S = 200 x 232 inside 320 x 256"""
+    _need_gpu()
+    ny, nx = 320, 256
+    S = (50, 10, 200, 232)
+    rng = np.random.default_rng(6)
+    psfs = [synth.psf_gauss_moffat(ny, nx, 2.0, 16.0 + 8 * j) for j in range(2)]
+    P = oracle.Problem(psfs, masked=True, S=S, sigma_R=1e-2)
+    info = P.info()
+    plan = B.Plan([dev(k, dt) for k in psfs], S=S, opts=B.default_options(sigma_R=1e-2))
+    m, a, nR = plan.mask()
+    m = m.cpu().numpy(); a = a.cpu().numpy()
+    tol = 3e-6 if dt == np.float32 else 1e-12
+    assert rel_l2(a, info["alpha"]) < tol
+    # the threshold test alpha_j >= sigma may flip where alpha_j is within rounding of sigma
+    diff = (m != info["MR"])
+    assert diff.sum() <= (0 if dt == np.float64 else 8)
+    x = rng.random((ny, nx)) * 100
+    for j in range(2):
+        if diff.sum() == 0:
+            assert rel_l2(plan.apply_A(j, dev(x, dt)).cpu().numpy(), P.A(j, x)) < tol
+            assert rel_l2(plan.apply_AT(j, dev(x, dt)).cpu().numpy(), P.AT(j, x)) < tol
+    plan.close()
+
+
+# ------------------------------------------------------------------------------------------------ SGP
+@pytest.mark.parametrize("dt,tol", [(np.float32, 1e-5), (np.float64, 1e-10)])
+def test_sgp_one_iteration_C0(dt, tol):
+    """north_star: relative L2 <= 1e-5 (fp32) / 1e-10 (fp64) after one iteration; J0 within 1e-4"""
+    w = synth.make("C0")
+    fg, rg, fo, ro = run_both(w, dt, max_iter=1)
+    assert rg.iterations == ro.iterations == 1
+    assert rel_l2(fg, fo) < tol
+    assert abs(rg.J[0] - ro.J[0]) <= 1e-4 * abs(ro.J[0]) and abs(rg.J[1] - ro.J[1]) <= 1e-4 * abs(ro.J[1])
+    assert rg.alpha[0] == ro.alpha[0] == 1.3 and rg.lam[0] == ro.lam[0]
+
+
+@pytest.mark.parametrize("dt,tol,jtol", [(np.float32, 1e-3, 1e-4), (np.float64, 1e-10, 1e-12)])
+def test_sgp_C0_100_iterations(dt, tol, jtol):
+    """config C0 in full: 256^2, 20 stars, Gaussian PSF, M = 10, fixed L, 100 iterations"""
+    w = synth.make("C0")
+    fg, rg, fo, ro = run_both(w, dt)
+    assert rg.iterations == ro.iterations == 100
+    assert rg.stop_reason == ro.stop_reason == 1
+    assert abs(rg.J0_final - ro.J0_final) <= jtol * abs(ro.J0_final)
+    assert rel_l2(fg, fo) < tol
+    assert (fg >= 0).all()
+    if dt == np.float64:
+        np.testing.assert_array_equal(rg.backtracks, ro.backtracks)
+        np.testing.assert_array_equal(rg.rule, ro.rule)
+        np.testing.assert_allclose(rg.alpha, ro.alpha, rtol=1e-9)
+        np.testing.assert_allclose(rg.J, ro.J, rtol=1e-12)
+        assert rg.total_backtracks == ro.total_backtracks > 0      # the backtracking path was exercised
+    assert rg.n_fft2 == ro.n_fft2 == 100 * 4
+
+
+@pytest.mark.parametrize("dt,tol", [(np.float32, 1e-3), (np.float64, 1e-10)])
+def test_sgp_adaptive_bounds_and_discrepancy_stop_C1(dt, tol):
+    """config C1 at 256^2: paper defaults (adaptive L1/L2, monotone Armijo), stop by the discrepancy
+    principle (Eq.26): same stopping iteration +-1"""
+    w = synth.make("C1", n=256, max_iter=300)
+    fg, rg, fo, ro = run_both(w, dt)
+    assert ro.stop_reason == 3, "the oracle run must stop by discrepancy for this test to mean anything"
+    assert rg.stop_reason == 3
+    assert abs(rg.iterations - ro.iterations) <= 1
+    assert abs(rg.L1_used - ro.L1_used) <= 1e-5 * ro.L1_used and abs(rg.L2_used - ro.L2_used) <= 1e-5 * ro.L2_used
+    if rg.iterations == ro.iterations:
+        assert rel_l2(fg, fo) < tol
+        assert abs(rg.J0_final - ro.J0_final) <= 1e-4 * abs(ro.J0_final)
+    assert rg.discrepancy_final <= 1.0
+
+
+@pytest.mark.parametrize("dt,tol", [(np.float32, 1e-3), (np.float64, 1e-10)])
+def test_sgp_multi_C2_small(dt, tol):
+    """config C2 at 128^2 x 3 images, 100 iterations (Eq.12-14, scaling f/p)"""
+    w = synth.make("C2", n=128, max_iter=100)
+    fg, rg, fo, ro = run_both(w, dt)
+    assert rg.iterations == ro.iterations == 100
+    assert abs(rg.J0_final - ro.J0_final) <= 1e-4 * abs(ro.J0_final)
+    assert rel_l2(fg, fo) < tol
+    assert rg.n_fft2 == ro.n_fft2 == 100 * 8
+
+
+@pytest.mark.parametrize("dt,tol", [(np.float32, 1e-3), (np.float64, 1e-10)])
+def test_sgp_boundary_C3_small(dt, tol):
+    """config C3 scaled down: S = 256^2 inside 320^2 (radix-5 grid), 60 iterations (Eq.16-23)"""
+    w = synth.make("C3", s=256, sbar=320, n_stars=150, max_iter=60, fwhm=64.0)
+    fg, rg, fo, ro = run_both(w, dt)
+    assert rg.iterations == ro.iterations == 60
+    assert abs(rg.J0_final - ro.J0_final) <= 1e-4 * abs(ro.J0_final)
+    assert rel_l2(fg, fo) < tol
+
+
+def test_sgp_replay_mode_fp32():
+    """kernel parity separated from trajectory branching: the GPU takes alpha_k, lambda_k
+    from the oracle's trace; 100 iterations of C1 at 256^2 in fp32"""
+    _need_gpu()
+    w = synth.make("C1", n=256, max_iter=100, stop_rule=0)
+    oo = oracle_opts(w)
+    P = oracle_problem(w, oo)
+    ge = P.embed(w["g"]); be = [np.full((P.ny, P.nx), float(v)) for v in w["b"]]
+    fo, ro = P.sgp(ge, be, opts=oo)
+    plan, o = gpu_plan(w, np.float32)
+    fg, rg = plan.sgp([dev(a, np.float32) for a in w["g"]], w["b"], opts=o, force_alpha=ro.alpha, force_lambda=ro.lam)
+    assert rg.iterations == 100
+    assert rel_l2(fg.cpu().numpy(), fo) < 1e-4
+    np.testing.assert_allclose(rg.J, ro.J, rtol=1e-5)
+    plan.close()
+
+
+# ------------------------------------------------------------------------------------------------ RL
+@pytest.mark.parametrize("dt,tol", [(np.float32, 1e-4), (np.float64, 1e-11)])
+@pytest.mark.parametrize("cfg", ["C0", "C2", "C3"])
+def test_rl_parity(cfg, dt, tol):
+    """Richardson-Lucy (Eq.1 / 13 / 21) on the same kernels, 30 iterations"""
+    kw = {"C0": {}, "C2": dict(n=128), "C3": dict(s=256, sbar=320, n_stars=150)}[cfg]
+    w = synth.make(cfg, **kw)
+    fg, rg, fo, ro = run_both(w, dt, alg="rl", max_iter=30, stop_rule=0)
+    assert rg.iterations == ro.iterations == 30
+    np.testing.assert_allclose(rg.J, ro.J, rtol=1e-5 if dt == np.float32 else 1e-12)
+    assert rel_l2(fg, fo) < tol
+
+
+def test_rl_relative_change_stop():
+    """Eq.24 stopping rule on RL: same stopping iteration as the oracle (+-1) in fp64"""
+    w = synth.make("C0")
+    fg, rg, fo, ro = run_both(w, np.float64, alg="rl", max_iter=400, stop_rule=1, tol=1e-3)
+    assert ro.stop_reason == 2 and rg.stop_reason == 2
+    assert abs(rg.iterations - ro.iterations) <= 1
+
+
+# ------------------------------------------------------------------------------------------------ C ABI behaviour
+def test_one_shot_entry_points_device_and_host():
+    """sgp_single (device pointers) and sgp_single_host (host pointers) give the result of the plan form"""
+    _need_gpu()
+    w = synth.make("C0", n=128)
+    o = B.default_options(**{**w["opts"], "max_iter": 10})
+    g, k, b = w["g"][0].astype(np.float32), w["psf"][0].astype(np.float32), w["b"][0]
+    f_dev, r_dev = B.sgp_single(dev(g, np.float32), dev(k, np.float32), b, opts=o)
+    f_host, r_host = B.sgp_single(g, k, b, opts=o, host=True)
+    plan = B.Plan([dev(k, np.float32)], opts=o)
+    f_plan, r_plan = plan.sgp([dev(g, np.float32)], [b], opts=o)
+    np.testing.assert_array_equal(f_dev.cpu().numpy(), f_plan.cpu().numpy())
+    np.testing.assert_array_equal(f_host, f_plan.cpu().numpy())
+    assert r_dev.iterations == r_host.iterations == r_plan.iterations == 10
+    f_rl, r_rl = B.rl_single(g, k, b, opts=o, host=True)
+    assert r_rl.iterations == 10 and np.isfinite(f_rl).all()
+    plan.close()
+
+
+def test_multi_and_boundary_one_shot_host():
+    _need_gpu()
+    w = synth.make("C2", n=64, max_iter=5)
+    o = B.default_options(**w["opts"])
+    g = [a.astype(np.float32) for a in w["g"]]; k = [a.astype(np.float32) for a in w["psf"]]
+    f, r = B.sgp_multi(g, k, w["b"], opts=o, host=True)
+    assert r.iterations == 5 and (f >= 0).all()
+    f, r = B.rl_multi(g, k, w["b"], opts=o, host=True)
+    assert r.iterations == 5
+    w = synth.make("C3", s=64, sbar=128, n_stars=30, max_iter=5, fwhm=8.0)
+    o = B.default_options(**w["opts"])
+    g = [a.astype(np.float32) for a in w["g"]]; k = [a.astype(np.float32) for a in w["psf"]]
+    oy, ox, sy, sx = w["S"]
+    f, r = B.sgp_boundary(g, k, w["b"], oy, ox, opts=o, host=True)
+    assert r.iterations == 5 and r.maskR is not None and (f[r.maskR == 0] == 0).all()
+    fo, ro = oracle.sgp_boundary(w["g"], w["psf"], w["b"], oy, ox, opts=oracle.default_options(**w["opts"]))
+    assert rel_l2(f, fo) < 1e-4
+    assert (ro.maskR != r.maskR).sum() <= 8
+    f, r = B.rl_boundary(g, k, w["b"], oy, ox, opts=o, host=True)
+    assert r.iterations == 5
+
+
+def test_background_arrays_and_user_start():
+    """b given as arrays and f0 given by the caller (SGP_INIT_USER)"""
+    _need_gpu()
+    w = synth.make("C0", n=128)
+    rng = np.random.default_rng(3)
+    barr = 10.0 + rng.random((128, 128))
+    f0 = 50.0 + rng.random((128, 128))
+    kw = {**w["opts"], "max_iter": 20, "init": B.INIT_USER}
+    plan = B.Plan([dev(w["psf"][0], np.float64)], opts=B.default_options(**kw))
+    fg, rg = plan.sgp([dev(w["g"][0], np.float64)], [dev(barr, np.float64)], f0=dev(f0, np.float64))
+    P = oracle.Problem(w["psf"])
+    fo, ro = P.sgp(w["g"], [barr], f0=f0, opts=oracle.default_options(**kw))
+    assert rel_l2(fg.cpu().numpy(), fo) < 1e-10
+    plan.close()
+
+
+def test_error_codes_and_edge_cases():
+    _need_gpu()
+    w = synth.make("C0", n=64)
+    g, k = dev(w["g"][0], np.float32), dev(w["psf"][0], np.float32)
+    o = B.default_options(**w["opts"])
+    # max_iter = 0: the start point comes back, J0 evaluated
+    o0 = B.default_options(**{**w["opts"], "max_iter": 0})
+    f, r = B.sgp_single(g, k, 10.0, opts=o0)
+    assert r.iterations == 0 and r.stop_reason == 1 and np.isfinite(r.J0_final)
+    assert np.allclose(f.cpu().numpy(), max(0.0, float((w["g"][0] - 10.0).mean())), rtol=1e-6)
+    # zero PSF
+    _, r = B.sgp_single(g, torch.zeros_like(k), 10.0, opts=o, check=False)
+    assert r.rc == B.ERR_PSF
+    # negative data in strict mode / clamped otherwise
+    gneg = g.clone(); gneg[3, 3] = -1.0
+    _, r = B.sgp_single(gneg, k, 10.0, opts=B.default_options(**{**w["opts"], "strict": 1}), check=False)
+    assert r.rc == B.ERR_DATA
+    _, r = B.sgp_single(gneg, k, 10.0, opts=o, check=False)
+    assert r.rc == B.OK
+    # non-finite data
+    gnan = g.clone(); gnan[0, 0] = float("nan")
+    _, r = B.sgp_single(gnan, k, 10.0, opts=o, check=False)
+    assert r.rc == B.ERR_DATA
+    # unsupported size
+    with pytest.raises(B.SgpError):
+        B.Plan([torch.ones((100, 100), device="cuda")])
+    # all-zero image, zero background: J0 = sum(Af) decreases to 0, f -> 0, no NaN
+    f, r = B.sgp_single(torch.zeros_like(g), k, 0.0, f0=torch.ones_like(g), opts=B.default_options(max_iter=3, init=B.INIT_USER, adaptive_L=0), check=False)
+    assert r.rc in (B.OK, B.ERR_LINESEARCH) and torch.isfinite(f).all()
