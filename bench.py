@@ -1,0 +1,387 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the SGP hot path (arXiv:1210.2258, Algorithm 1) on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload C4c|C4a|C4b|C1|C0] [--alg sgp|rl] [--dtype f32|f64]
+    python bench.py --impl reference ...     # the CPU oracle on the host cores (the tier's reference arm)
+
+One STEP is one whole reconstruction of the workload through the plan form of the C ABI (sgp_plan_run):
+the start-point phase (SURVEY.md 8(a) row a0'') followed by a FIXED number of SGP iterations (rows a1-a11;
+200 for C4c, BASELINE.json configs[4]) with the inputs already resident in HBM.  The metric is SGP
+iterations per second (BASELINE.json `metric`), whole job over all ranks; `gpixel_iter_per_s` = value x
+object-grid pixels / 1e9.  The default workload is C4c: single image 2048 x 2048 fp32, galaxies + stars,
+Airy PSF, b = 20, paper-default SGP options, 200 iterations -- the configuration the metric is quoted on.
+
+The printed JSON line also carries
+  e2e          the same metric through sgp_single_host / sgp_multi_host: HOST (pinned) buffers, plan creation, PSF
+               transfer functions, host->device and device->host copies all inside the timed region;
+  roofline     for the kernel with the largest share of the iteration: algorithmic bytes per launch
+                / its mean duration, measured with CUDA event pairs around every launch
+               in an instrumented pass of the same step right after the timed region (sgp_plan_set_profiling);
+               `iteration` gives the same for the whole iteration from the un-instrumented timed region;
+  cpu_baseline the oracle (oracle/, plain C, fp64, as it stands) on the host cores, on a bounded sample.
+N > 1: independent replicas, one problem per GPU ("replicas only"), no collective on
+the data path; time = max over ranks.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+from pathlib import Path
+
+ROOT = Path(__file__).resolve().parent
+if str(ROOT) not in sys.path:
+    sys.path.insert(0, str(ROOT))
+
+import numpy as np  # noqa: E402
+
+WORKLOADS = {
+    # name: (synth config, kwargs, description)
+    "C4c": ("C4c", {}, "C4c: single-image SGP 2048x2048, galaxies+stars, Airy PSF, b=20, Poisson, 200 iterations"),
+    "C4a": ("C4a", {}, "C4a: single-image SGP 4096x4096, galaxies+stars, Airy PSF, b=20, Poisson, 200 iterations"),
+    "C4b": ("C4b", {}, "C4b: multi-image SGP 3x2048x2048, rotated LBT PSFs, cluster+nebula, b_j=15, 200 iterations"),
+    "C1": ("C1", dict(max_iter=200, stop_rule=0), "C1: single-image SGP 512x512, galaxies+stars, Airy PSF, b=20, 200 iterations"),
+    "C0": ("C0", dict(), "C0: single-image SGP 256x256, 20 stars, Gaussian PSF, b=10, M=10, 100 iterations"),
+}
+
+
+def load_peaks():
+    f = ROOT / "MEASURED_PEAKS.json"
+    if f.exists():
+        try:
+            return float(json.loads(f.read_text())["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+        except Exception:
+            pass
+    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+def planes_per_launch(p: int, b_array: bool, masked: bool):
+    """algorithmic planes (n reals each) read + written per launch, SURVEY.md 8(d) schedule A / DESIGN.md section 6"""
+    ba = p if b_array else 0
+    m = 1 if masked else 0
+    return {
+        "K1_ratio_rowfft": 3 * p + ba, "K2_col_conjsum": 2 * p + 1, "K3_rowifft_grad_bb": 5 + m,
+        "K4_project_rowfft": 4 + m, "K5_col_mult": 2 * p + 1, "K6_rowifft_linesearch": 4 * p + ba, "K7_update": 3 + 3 * p,
+        "R1_rowfft": 2, "R2_col_mult": 2 * p + 1, "R3_rowifft_q_J": 3 * p + ba, "R4_ratio_rowfft": 3 * p + ba,
+        "R5_col_conjsum": 2 * p + 1, "R6_rowifft_update": 3 + m,
+    }
+
+
+class ClockSampler:
+    """nvidia-smi clocks and throttle reasons DURING the timed region (B200_PROFILING.md clocks line)"""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index, self.rows, self.proc = index, [], None
+
+    def __enter__(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                          "-lms", "100"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except Exception:
+            self.proc = None
+        return self
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append(line.strip())
+
+    def __exit__(self, *a):
+        if self.proc:
+            time.sleep(0.15)
+            self.proc.terminate()
+            try:
+                self.proc.wait(timeout=2)
+            except Exception:
+                self.proc.kill()
+
+    def summary(self):
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            c = [x.strip() for x in r.split(",")]
+            if len(c) < 7:
+                continue
+            try:
+                sm.append(float(c[0])); mx.append(float(c[1]))
+            except ValueError:
+                continue
+            for nm, v in zip(names, c[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(nm)
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        return {"sm_mhz": statistics.median(sm), "sm_max_mhz": max(mx), "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def make_workload(name: str, rank: int):
+    """rank r > 0 gets an independent replica: the same recipe drawn from another seed"""
+    from paper_1210_2258_b200 import synth
+    cfg, kw, desc = WORKLOADS[name]
+    if rank == 0:
+        return synth.make(cfg, **kw), desc
+    sidx = 100 * rank
+    if cfg == "C4c":
+        w = synth.c1_galaxies_airy(2048, seed_idx=6 + sidx, max_iter=200, stop_rule=0)
+    elif cfg == "C4a":
+        w = synth.c1_galaxies_airy(4096, seed_idx=4 + sidx, max_iter=200, stop_rule=0)
+    elif cfg == "C4b":
+        w = synth.c2_lbt_multi(2048, seed_idx=5 + sidx, max_iter=200)
+    elif cfg == "C1":
+        w = synth.c1_galaxies_airy(512, seed_idx=1 + sidx, **kw)
+    else:
+        w = synth.c0_stars_gaussian(256, seed_idx=sidx)
+    return w, desc
+
+
+def oracle_time(w, iters_a: int, iters_b: int):
+    """wall time of the oracle for iters_a and iters_b SGP iterations of workload w (fp64, OpenMP over the host cores)"""
+    import oracle
+    oo = oracle.default_options(**{**w["opts"], "max_iter": iters_a})
+    P = oracle.Problem(w["psf"], masked=w["S"] is not None, S=w["S"], sigma_R=oo.sigma_R)
+    ge = P.embed(w["g"]); be = [np.full((P.ny, P.nx), float(v)) for v in w["b"]]
+    out = []
+    for it in (iters_a, iters_b):
+        oo.max_iter = it
+        t0 = time.perf_counter()
+        _, r = P.sgp(ge, be, opts=oo)
+        out.append(time.perf_counter() - t0)
+        assert r.iterations == it
+    return out
+
+
+def run_reference(args):
+    """Reference arm of this tier: the CPU oracle as it stands, on the host cores; rank 0 only."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    cores = os.cpu_count() or 1
+    os.environ["OMP_NUM_THREADS"] = str(cores)
+    import oracle
+    w, desc = make_workload(args.workload, 0)
+    p = len(w["g"]); ny, nx = w["psf"][0].shape
+    m = args.ref_iters
+    oo = oracle.default_options(**{**w["opts"], "max_iter": m})
+    P = oracle.Problem(w["psf"], masked=w["S"] is not None, S=w["S"], sigma_R=oo.sigma_R)
+    ge = P.embed(w["g"]); be = [np.full((P.ny, P.nx), float(v)) for v in w["b"]]
+    fn = P.sgp if args.alg == "sgp" else P.rl
+    for _ in range(args.warmup):
+        fn(ge, be, opts=oo)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        _, r = fn(ge, be, opts=oo)
+    dt = time.perf_counter() - t0
+    value = m * args.steps / dt
+    sample = (f"each step = {m} {args.alg.upper()} iterations of {args.workload} ({p}x{ny}x{nx}, fp64) from the constant start, "
+              f"start-point phase (A f0, J0, adaptive bounds) inside the step; OpenMP over {cores} host threads")
+    line = {"impl": "reference", "metric": "SGP iterations/s" if args.alg == "sgp" else "RL iterations/s", "value": value,
+            "unit": "iterations/s", "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": 1e3 * dt / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64", "data": "synthetic", "gpixel_iter_per_s": value * ny * nx / 1e9,
+            "config": {"workload": desc, "iterations_per_step": m, "grid": [ny, nx], "images": p, "algorithm": args.alg},
+            "cpu_baseline": {"value": value, "unit": "iterations/s", "cores": cores, "kind": "oracle", "sample": sample},
+            "e2e": {"value": value, "unit": "iterations/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+    return 0
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    from paper_1210_2258_b200 import binding as B
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: there is no CPU fallback for the product path")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+    B.lib()   # fail loudly if the CUDA library is missing
+
+    w, desc = make_workload(args.workload, rank)
+    p = len(w["g"]); ny, nx = w["psf"][0].shape
+    npdt, tdt = (np.float32, torch.float32) if args.dtype == "f32" else (np.float64, torch.float64)
+    esz = np.dtype(npdt).itemsize
+    iters = int(w["opts"]["max_iter"])
+    okw = {**w["opts"], "stop_rule": 0}
+    if args.tile_cols: okw["tile_cols"] = args.tile_cols
+    if args.rows_per_block: okw["rows_per_block"] = args.rows_per_block
+    opts = B.default_options(**okw)
+    alg = B.ALG_SGP if args.alg == "sgp" else B.ALG_RL
+
+    to_dev = lambda a: torch.as_tensor(np.ascontiguousarray(a, dtype=npdt), device=dev)
+    psfs = [to_dev(k) for k in w["psf"]]
+    g = [to_dev(a) for a in w["g"]]
+    plan = B.Plan(psfs, S=w["S"], opts=opts)
+    f_out = torch.empty((ny, nx), dtype=tdt, device=dev)
+
+    def step():
+        _, r = plan.run(alg, g, w["b"], opts=opts, f_out=f_out, traces=False)
+        return r
+
+    def sync_all():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+            torch.cuda.synchronize()
+
+    for _ in range(max(args.warmup, 3)):
+        r = step()
+    assert r.iterations == iters, (r.iterations, iters)
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    launches = 0
+    backtracks = 0
+    loop_ms = 0.0
+    sync_all()
+    with ClockSampler(local) as clk:
+        ev0.record()
+        for _ in range(args.steps):
+            r = step()
+            launches += r.kernel_launches; backtracks += r.total_backtracks; loop_ms += r.loop_ms
+        ev1.record()
+        sync_all()
+    ms = ev0.elapsed_time(ev1)
+    if world > 1:
+        t = torch.tensor([ms], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+    total_iters = iters * args.steps * world
+    value = total_iters / (ms * 1e-3)
+    J_final = r.J0_final
+
+    # ---- instrumented pass: CUDA event pair around every launch of the same step (not part of `value`)
+    plan.set_profiling(True)
+    step()
+    rp = step()
+    kms = plan.kernel_ms()
+    plan.set_profiling(False)
+    planes = planes_per_launch(p, False, w["S"] is not None)
+    plane_bytes = ny * nx * esz
+    peak, peak_src = load_peaks()
+    per_kernel = {}
+    tot_ms = sum(v[0] for v in kms.values()) or 1.0
+    for name, (msum, cnt) in kms.items():
+        avg_us = 1e3 * msum / cnt
+        gbs = planes[name] * plane_bytes / (avg_us * 1e-6) / 1e9
+        per_kernel[name] = {"avg_us": round(avg_us, 2), "launches": cnt, "planes": planes[name], "GBps": round(gbs, 1),
+                            "frac": round(gbs / peak, 4), "share": round(msum / tot_ms, 4)}
+    dom = max(kms, key=lambda k: kms[k][0])
+    traffic = None
+    tf = ROOT / "profiles" / "traffic.json"
+    if tf.exists():
+        try:
+            traffic = json.loads(tf.read_text()).get(f"{args.workload}:{args.dtype}:{args.alg}", {}).get(dom)
+        except Exception:
+            traffic = None
+    iter_planes = (14 * p + 14 + (2 if w["S"] is not None else 0)) if args.alg == "sgp" else (
+        sum(planes[k] for k in planes if k.startswith("R")))
+    it_us = 1e3 * (loop_ms / args.steps) / iters          # loop only (library's own events), local rank
+    it_gbs = iter_planes * plane_bytes / (it_us * 1e-6) / 1e9
+    roofline = {"bound": "hbm", "kernel": dom, "achieved": per_kernel[dom]["GBps"], "peak": peak, "unit": "GB/s",
+                "frac": per_kernel[dom]["frac"], "traffic": traffic, "peak_source": peak_src,
+                "algorithmic_bytes_per_launch": planes[dom] * plane_bytes,
+                "iteration": {"planes": iter_planes, "bytes": iter_planes * plane_bytes, "us": round(it_us, 2),
+                              "GBps": round(it_gbs, 1), "frac": round(it_gbs / peak, 4),
+                              "backtracks_per_iteration": backtracks / max(1, iters * args.steps)},
+                "kernels": per_kernel}
+
+    # ---- e2e: host (pinned) buffers through the one-shot host entry points; copies inside the timed region
+    e2e = None
+    if not args.no_e2e:
+        pin = lambda a: torch.as_tensor(np.ascontiguousarray(a, dtype=npdt)).pin_memory().numpy()
+        hg = [pin(a) for a in w["g"]]; hk = [pin(a) for a in w["psf"]]
+        hf = torch.empty((ny, nx), dtype=tdt).pin_memory().numpy()
+
+        def e2e_step():
+            if w["S"] is not None:
+                return B._one_shot("sgp_boundary" if args.alg == "sgp" else "rl_boundary", hg, hk, w["b"], None, opts,
+                                   boundary=(w["S"][0], w["S"][1]), host=True, f_out=hf)[1]
+            if p == 1:
+                return (B.sgp_single if args.alg == "sgp" else B.rl_single)(hg[0], hk[0], w["b"][0], opts=opts, host=True, f_out=hf)[1]
+            return (B.sgp_multi if args.alg == "sgp" else B.rl_multi)(hg, hk, w["b"], opts=opts, host=True, f_out=hf)[1]
+
+        e2e_step()
+        sync_all()
+        n_e2e = max(1, min(args.steps, 5))
+        t0 = time.perf_counter()
+        for _ in range(n_e2e):
+            re = e2e_step()
+        torch.cuda.synchronize()
+        dt = time.perf_counter() - t0
+        if world > 1:
+            t = torch.tensor([dt], dtype=torch.float64, device=dev)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            dt = float(t.item())
+        sbytes = sum(a.nbytes for a in hg) + sum(a.nbytes for a in hk)
+        e2e = {"value": re.iterations * n_e2e * world / dt, "unit": "iterations/s", "h2d_bytes_per_step": sbytes,
+               "d2h_bytes_per_step": hf.nbytes, "steps": n_e2e, "ms_per_step": 1e3 * dt / n_e2e,
+               "api": "sgp_single_host" if p == 1 and w["S"] is None else ("sgp_boundary_host" if w["S"] is not None else "sgp_multi_host"),
+               "includes": "plan creation, workspace allocation, PSF transfer functions, H2D of g and PSF from pinned memory, "
+                           "all iterations, D2H of f"}
+
+    # ---- CPU baseline: the oracle on the host cores, bounded sample (rank 0, N = 1 only)
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu:
+        cores = os.cpu_count() or 1
+        os.environ["OMP_NUM_THREADS"] = str(cores)
+        ia, ib = 1, 1 + args.cpu_iters
+        ta, tb = oracle_time(w, ia, ib)
+        per_it = (tb - ta) / (ib - ia)
+        cpu = {"value": 1.0 / per_it, "unit": "iterations/s", "cores": cores, "kind": "oracle",
+               "sample": f"{args.workload} ({p}x{ny}x{nx}) fp64 oracle: (t({ib} it) - t({ia} it)) / {ib - ia}, start-point phase excluded; "
+                         f"t({ia})={ta:.2f}s t({ib})={tb:.2f}s; OpenMP over {cores} threads"}
+
+    if rank == 0:
+        line = {"metric": "SGP iterations/s" if args.alg == "sgp" else "RL iterations/s", "value": value, "unit": "iterations/s",
+                "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms / args.steps,
+                "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": args.dtype, "data": "synthetic",
+                "gpixel_iter_per_s": value * ny * nx / 1e9,
+                "config": {"workload": desc, "iterations_per_step": iters, "grid": [ny, nx], "images": p, "algorithm": args.alg,
+                           "parallelism": "replicas only" if world > 1 else "single GPU",
+                           "l2": f"no flush: per-iteration working set {(6 * p + 4) * plane_bytes / 1e6:.0f} MB "
+                                 f"({6 * p + 4} planes) vs 126 MB L2",
+                           "tile_cols": int(opts.tile_cols), "rows_per_block": int(opts.rows_per_block),
+                           "J0_final": J_final, "backtracks": backtracks // args.steps},
+                "clocks": clk.summary(), "e2e": e2e, "gpu_launches": launches, "roofline": roofline, "cpu_baseline": cpu}
+        print(json.dumps(line))
+    plan.close()
+    if world > 1:
+        dist.destroy_process_group()
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="C4c", choices=sorted(WORKLOADS))
+    ap.add_argument("--alg", default="sgp", choices=["sgp", "rl"])
+    ap.add_argument("--dtype", default="f32", choices=["f32", "f64"])
+    ap.add_argument("--tile-cols", type=int, default=0)
+    ap.add_argument("--rows-per-block", type=int, default=0)
+    ap.add_argument("--cpu-iters", type=int, default=5, help="oracle iterations timed for cpu_baseline")
+    ap.add_argument("--ref-iters", type=int, default=3, help="oracle iterations per step of --impl reference")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_ours(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

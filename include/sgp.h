@@ -126,6 +126,25 @@ typedef struct sgp_result {
 
 typedef struct sgp_plan sgp_plan;
 
+/* Kernel slots of the per-kernel timing (sgp_plan_set_profiling).  One SGP iteration is the seven launches
+ * K1..K7 (SURVEY.md 8(d) schedule A), one RL round the six launches R1..R6. */
+typedef enum {
+    SGP_PROF_K1 = 0,  /* a1: ratio g/(Af+b) fused into the forward row FFT, p images                          */
+    SGP_PROF_K2 = 1,  /* a2: column FFT -> sum_j conj(K^_j) x -> inverse column FFT                            */
+    SGP_PROF_K3 = 2,  /* a3+a5+a6: inverse row FFT -> gradient, BB dot products, step length                   */
+    SGP_PROF_K4 = 3,  /* a4+a7: scaling, projection, d, grad'd fused into the forward row FFT of d             */
+    SGP_PROF_K5 = 4,  /* a8: column FFT -> x K^_j -> p inverse column FFTs                                      */
+    SGP_PROF_K6 = 5,  /* a8+a9: inverse row FFTs -> u_j = A_j d, J(lambda = 1), Armijo test                     */
+    SGP_PROF_K7 = 6,  /* a9 backtracks + a10 update + a11 stopping rules                                        */
+    SGP_PROF_R1 = 7,  /* RL: forward row FFT of f                                                               */
+    SGP_PROF_R2 = 8,  /* RL: column pass x K^_j                                                                 */
+    SGP_PROF_R3 = 9,  /* RL: inverse row FFTs -> q_j = A_j f, J0(f), stopping rules                             */
+    SGP_PROF_R4 = 10, /* RL: ratio fused into the forward row FFTs                                              */
+    SGP_PROF_R5 = 11, /* RL: column pass sum_j conj(K^_j)                                                       */
+    SGP_PROF_R6 = 12, /* RL: inverse row FFT -> multiplicative update, Eq.1/13/21                               */
+    SGP_PROF_SLOTS = 13
+} sgp_prof_slot;
+
 void sgp_options_default(sgp_options *opt);
 void sgp_result_init(sgp_result *res);           /* zero everything, NULL traces */
 const char *sgp_strerror(int status);
@@ -210,6 +229,12 @@ int sgp_plan_get_mask(sgp_plan *plan, unsigned char *maskR_out, void *alpha_out,
  * in-run comparison with cuFFT.  sgp_plan_irfft2 is the inverse including the 1/(ny nx) factor. */
 int sgp_plan_rfft2(sgp_plan *plan, const void *x, void *spec_out, void *stream);
 int sgp_plan_irfft2(sgp_plan *plan, const void *spec_in, void *x_out, void *stream);
+/* Per-kernel device timing of the iteration loop.  on = 1: every launch of the following sgp_plan_run calls
+ * is bracketed by a CUDA event pair on `stream` (this costs a little throughput, so loop_ms of such a run is
+ * not a benchmark figure).  sgp_plan_get_kernel_ms returns, for the last run, the summed duration in ms and
+ * the number of launches of every slot: ms_sum and launches are HOST arrays of SGP_PROF_SLOTS entries. */
+int sgp_plan_set_profiling(sgp_plan *plan, int on);
+int sgp_plan_get_kernel_ms(sgp_plan *plan, double *ms_sum, long *launches);
 void sgp_plan_destroy(sgp_plan *plan);
 
 #ifdef __cplusplus

@@ -30,8 +30,10 @@ EXPORTS = [
     "sgp_single", "sgp_multi", "sgp_boundary", "rl_single", "rl_multi", "rl_boundary",
     "sgp_single_host", "sgp_multi_host", "sgp_boundary_host", "rl_single_host", "rl_multi_host", "rl_boundary_host",
     "sgp_plan_create", "sgp_plan_set_psf", "sgp_plan_run", "sgp_plan_apply_A", "sgp_plan_apply_AT", "sgp_plan_get_mask",
-    "sgp_plan_rfft2", "sgp_plan_irfft2", "sgp_plan_destroy",
+    "sgp_plan_rfft2", "sgp_plan_irfft2", "sgp_plan_set_profiling", "sgp_plan_get_kernel_ms", "sgp_plan_destroy",
 ]
+PROF_SLOTS = ["K1_ratio_rowfft", "K2_col_conjsum", "K3_rowifft_grad_bb", "K4_project_rowfft", "K5_col_mult", "K6_rowifft_linesearch",
+              "K7_update", "R1_rowfft", "R2_col_mult", "R3_rowifft_q_J", "R4_ratio_rowfft", "R5_col_conjsum", "R6_rowifft_update"]
 
 
 class Options(C.Structure):
@@ -263,6 +265,20 @@ class Plan:
     def rl(self, g, b, **kw):
         return self.run(ALG_RL, g, b, **kw)
 
+    def set_profiling(self, on: bool):
+        rc = lib().sgp_plan_set_profiling(self.h, int(bool(on)))
+        if rc != OK:
+            raise SgpError(rc, "sgp_plan_set_profiling")
+
+    def kernel_ms(self):
+        """{slot name: (summed ms, launches)} of the last profiled run"""
+        n = len(PROF_SLOTS)
+        ms, cnt = (C.c_double * n)(), (C.c_long * n)()
+        rc = lib().sgp_plan_get_kernel_ms(self.h, ms, cnt)
+        if rc != OK:
+            raise SgpError(rc, "sgp_plan_get_kernel_ms")
+        return {PROF_SLOTS[i]: (ms[i], cnt[i]) for i in range(n) if cnt[i] > 0}
+
     def apply_A(self, j, x):
         out = _torch().empty_like(x)
         rc = lib().sgp_plan_apply_A(self.h, int(j), _dev_ptr(x), _dev_ptr(out), _stream_ptr())
@@ -308,7 +324,7 @@ class Plan:
 
 # ---- one-shot entry points with the names of include/sgp.h ----------------------------------------
 
-def _one_shot(name, g, psf, b, f0, opts, boundary=None, single=False, host=False, check=True):
+def _one_shot(name, g, psf, b, f0, opts, boundary=None, single=False, host=False, check=True, f_out=None):
     """g, psf: lists of arrays (CUDA tensors, or numpy arrays when host=True); b: scalars or arrays."""
     torch = _torch() if not host else None
     p = len(g)
@@ -324,7 +340,9 @@ def _one_shot(name, g, psf, b, f0, opts, boundary=None, single=False, host=False
         b_is_arr = np.ndim(b[0]) != 0
         b = [np.ascontiguousarray(a, dtype=dt) for a in b] if b_is_arr else b
         f0 = np.ascontiguousarray(f0, dtype=dt) if f0 is not None else None
-        f_out = np.empty((ny, nx), dt)
+        if f_out is None:
+            f_out = np.empty((ny, nx), dt)
+        assert f_out.dtype == dt and f_out.shape == (ny, nx) and f_out.flags.c_contiguous
         maskR = np.empty((ny, nx), np.uint8) if boundary is not None else None
         stream = None
     else:
@@ -333,7 +351,9 @@ def _one_shot(name, g, psf, b, f0, opts, boundary=None, single=False, host=False
         ny, nx = psf[0].shape
         ptr, pp = _dev_ptr, _pp
         b_is_arr = torch.is_tensor(b[0])
-        f_out = torch.empty((ny, nx), dtype=tdt, device=g[0].device)
+        if f_out is None:
+            f_out = torch.empty((ny, nx), dtype=tdt, device=g[0].device)
+        _check_dev(f_out, (ny, nx), tdt, "f_out")
         maskR = torch.empty((ny, nx), dtype=torch.uint8, device=g[0].device) if boundary is not None else None
         stream = _stream_ptr()
     b_const = (C.c_double * p)(*([0.0] * p if b_is_arr else [float(v) for v in b]))
@@ -356,25 +376,25 @@ def _one_shot(name, g, psf, b, f0, opts, boundary=None, single=False, host=False
     return f_out, res
 
 
-def sgp_single(g, psf, b, f0=None, opts=None, host=False, check=True):
-    return _one_shot("sgp_single", [g], [psf], [b], f0, opts, single=True, host=host, check=check)
+def sgp_single(g, psf, b, f0=None, opts=None, host=False, check=True, f_out=None):
+    return _one_shot("sgp_single", [g], [psf], [b], f0, opts, single=True, host=host, check=check, f_out=f_out)
 
 
-def rl_single(g, psf, b, f0=None, opts=None, host=False, check=True):
-    return _one_shot("rl_single", [g], [psf], [b], f0, opts, single=True, host=host, check=check)
+def rl_single(g, psf, b, f0=None, opts=None, host=False, check=True, f_out=None):
+    return _one_shot("rl_single", [g], [psf], [b], f0, opts, single=True, host=host, check=check, f_out=f_out)
 
 
-def sgp_multi(g, psf, b, f0=None, opts=None, host=False, check=True):
-    return _one_shot("sgp_multi", g, psf, b, f0, opts, host=host, check=check)
+def sgp_multi(g, psf, b, f0=None, opts=None, host=False, check=True, f_out=None):
+    return _one_shot("sgp_multi", g, psf, b, f0, opts, host=host, check=check, f_out=f_out)
 
 
-def rl_multi(g, psf, b, f0=None, opts=None, host=False, check=True):
-    return _one_shot("rl_multi", g, psf, b, f0, opts, host=host, check=check)
+def rl_multi(g, psf, b, f0=None, opts=None, host=False, check=True, f_out=None):
+    return _one_shot("rl_multi", g, psf, b, f0, opts, host=host, check=check, f_out=f_out)
 
 
-def sgp_boundary(g, psf, b, oy, ox, f0=None, opts=None, host=False, check=True):
-    return _one_shot("sgp_boundary", g, psf, b, f0, opts, boundary=(oy, ox), host=host, check=check)
+def sgp_boundary(g, psf, b, oy, ox, f0=None, opts=None, host=False, check=True, f_out=None):
+    return _one_shot("sgp_boundary", g, psf, b, f0, opts, boundary=(oy, ox), host=host, check=check, f_out=f_out)
 
 
-def rl_boundary(g, psf, b, oy, ox, f0=None, opts=None, host=False, check=True):
-    return _one_shot("rl_boundary", g, psf, b, f0, opts, boundary=(oy, ox), host=host, check=check)
+def rl_boundary(g, psf, b, oy, ox, f0=None, opts=None, host=False, check=True, f_out=None):
+    return _one_shot("rl_boundary", g, psf, b, f0, opts, boundary=(oy, ox), host=host, check=check, f_out=f_out)

@@ -200,6 +200,19 @@ int sgp_plan_irfft2(sgp_plan *plan, const void *spec_in, void *x_out, void *stre
     return plan->impl->irfft2(spec_in, x_out, (cudaStream_t)stream);
 }
 
+int sgp_plan_set_profiling(sgp_plan *plan, int on)
+{
+    if (!plan) return SGP_ERR_ARG;
+    plan->impl->profiling = on != 0;
+    return SGP_OK;
+}
+int sgp_plan_get_kernel_ms(sgp_plan *plan, double *ms_sum, long *launches)
+{
+    if (!plan || !ms_sum || !launches) return SGP_ERR_ARG;
+    for (int i = 0; i < SGP_PROF_SLOTS; ++i) { ms_sum[i] = plan->impl->prof_ms[i]; launches[i] = plan->impl->prof_count[i]; }
+    return SGP_OK;
+}
+
 // ---- one-shot calls: create a plan, set the PSFs, run, destroy
 static int one_shot(int algorithm, int kind, int p, const void *const *g, const void *const *psf, const void *const *b_arr,
                     const double *b_const, int oy, int ox, int sy, int sx, int ny, int nx, const void *f0, void *f_out,

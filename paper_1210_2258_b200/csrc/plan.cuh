@@ -30,6 +30,9 @@ struct PlanBase {
     long nR = 0;
     size_t bytes_allocated = 0;
     long launches = 0;
+    bool profiling = false;
+    double prof_ms[SGP_PROF_SLOTS] = {0};
+    long prof_count[SGP_PROF_SLOTS] = {0};
     virtual ~PlanBase() {}
     virtual int init() = 0;
     virtual int set_psf(const void *const *psf, cudaStream_t st) = 0;

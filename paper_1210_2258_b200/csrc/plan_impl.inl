@@ -25,6 +25,12 @@ template <typename T> struct PlanImpl : PlanBase {
     int *trR = nullptr, *trB = nullptr;
     int trace_cap = 0;
     cudaEvent_t ev0 = nullptr, ev1 = nullptr, ev2 = nullptr;
+    // per-kernel timing (sgp_plan_set_profiling): one event pair per launch of the iteration loop
+    struct ProfRec { int slot; cudaEvent_t a, b; };
+    std::vector<ProfRec> prof_recs;
+    std::vector<cudaEvent_t> prof_pool;
+    size_t prof_used = 0;
+    int cur_slot = -1;
 
     ~PlanImpl() override
     {
@@ -33,6 +39,37 @@ template <typename T> struct PlanImpl : PlanBase {
         if (ev0) cudaEventDestroy(ev0);
         if (ev1) cudaEventDestroy(ev1);
         if (ev2) cudaEventDestroy(ev2);
+        for (cudaEvent_t e : prof_pool) cudaEventDestroy(e);
+    }
+    cudaEvent_t prof_event()
+    {
+        if (prof_used == prof_pool.size()) {
+            cudaEvent_t e = nullptr;
+            if (cudaEventCreate(&e) != cudaSuccess) return nullptr;
+            prof_pool.push_back(e);
+        }
+        return prof_pool[prof_used++];
+    }
+    // bracket the next launch with events when profiling is on and a slot is selected
+    struct ProfScope {
+        PlanImpl *P; cudaStream_t st; cudaEvent_t a = nullptr;
+        ProfScope(PlanImpl *P_, cudaStream_t st_) : P(P_), st(st_)
+        {
+            if (P->profiling && P->cur_slot >= 0 && (a = P->prof_event())) cudaEventRecord(a, st);
+        }
+        ~ProfScope()
+        {
+            if (a) { cudaEvent_t b = P->prof_event(); if (b) { cudaEventRecord(b, st); P->prof_recs.push_back({P->cur_slot, a, b}); } }
+        }
+    };
+    void prof_reset() { prof_recs.clear(); prof_used = 0; for (int i = 0; i < SGP_PROF_SLOTS; ++i) { prof_ms[i] = 0.0; prof_count[i] = 0; } }
+    void prof_collect()
+    {
+        for (const ProfRec &r : prof_recs) {
+            float ms = 0.f;
+            if (cudaEventElapsedTime(&ms, r.a, r.b) == cudaSuccess) { prof_ms[r.slot] += ms; prof_count[r.slot]++; }
+        }
+        prof_recs.clear(); prof_used = 0;
     }
     void free_trace()
     {
@@ -144,6 +181,7 @@ template <typename T> struct PlanImpl : PlanBase {
     }
     int launch_row(row_kernel_t<T> k, const RowParams<T> &P, int images, cudaStream_t st)
     {
+        ProfScope ps(this, st);
         k<<<dim3(nrb, images), row_threads, row_smem, st>>>(P);
         launches++;
         SGP_CUDA_TRY(cudaGetLastError());
@@ -159,6 +197,7 @@ template <typename T> struct PlanImpl : PlanBase {
     }
     int launch_col(col_kernel_t<T> k, const ColParams<T> &P, cudaStream_t st)
     {
+        ProfScope ps(this, st);
         k<<<ntiles, col_threads, col_smem, st>>>(P);
         launches++;
         SGP_CUDA_TRY(cudaGetLastError());

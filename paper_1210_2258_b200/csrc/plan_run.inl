@@ -47,30 +47,37 @@ int PlanImpl<T>::enqueue_sgp_iteration(const RowParams<T> &Pb, const DevOpts &o,
                                        int b_is_array, cudaStream_t st)
 {
     int rc;
+    cur_slot = SGP_PROF_K1;
     {   // K1 (a1)
         RowParams<T> P = Pb; P.mode = RF_RATIO; P.in0 = Gp; P.in1 = q; P.in2 = Bp;
         if ((rc = launch_row(k_rowf, P, p, st))) return rc;
     }
+    cur_slot = SGP_PROF_K2;
     {   // K2 (a2)
         ColParams<T> Q = col_params(); Q.check_status = 1;
         if ((rc = launch_col(k_conj, Q, st))) return rc;
     }
+    cur_slot = SGP_PROF_K3;
     {   // K3 (a3, a5, a6)
         RowParams<T> P = Pb; P.mode = RI_GRAD; P.in0 = f; P.in1 = d; P.out0 = grad; P.part = part_bb;
         if ((rc = launch_row(k_rowi, P, 1, st))) return rc;
     }
+    cur_slot = SGP_PROF_K4;
     {   // K4 (a4, a7)
         RowParams<T> P = Pb; P.mode = RF_PROJECT; P.in0 = f; P.in1 = grad; P.out0 = d; P.part = part_gd;
         if ((rc = launch_row(k_rowf, P, 1, st))) return rc;
     }
+    cur_slot = SGP_PROF_K5;
     {   // K5 (a8)
         ColParams<T> Q = col_params(); Q.check_status = 1;
         if ((rc = launch_col(k_mult, Q, st))) return rc;
     }
+    cur_slot = SGP_PROF_K6;
     {   // K6 (a8 tail, a9 at lambda = 1)
         RowParams<T> P = Pb; P.mode = RI_LS; P.in0 = Gp; P.in1 = q; P.in2 = Bp; P.out0 = u; P.part = part_J; P.part2 = part_gd;
         if ((rc = launch_row(k_rowi, P, p, st))) return rc;
     }
+    cur_slot = SGP_PROF_K7;
     {   // K7 (a9 backtracks, a10, a11)
         UpdParams<T> U;
         memset(&U, 0, sizeof(U));
@@ -78,9 +85,11 @@ int PlanImpl<T>::enqueue_sgp_iteration(const RowParams<T> &Pb, const DevOpts &o,
         U.plane = n; U.b_is_array = b_is_array; U.part = part_upd;
         for (int j = 0; j < p; ++j) U.bconst[j] = bconst[j];
         void *args[] = {(void *)&U};
+        ProfScope ps(this, st);
         SGP_CUDA_TRY(cudaLaunchCooperativeKernel((const void *)update_kernel<T>, dim3(upd_grid), dim3(256), args, 0, st));
         launches++;
     }
+    cur_slot = -1;
     return SGP_OK;
 }
 
@@ -92,12 +101,19 @@ int PlanImpl<T>::enqueue_rl_round(const DevOpts &o, const Trace &tr, const doubl
     RowParams<T> Pb = row_params(RF_PLAIN);
     Pb.o = o; Pb.tr = tr; Pb.check_status = 1; Pb.b_is_array = b_is_array;
     for (int j = 0; j < p; ++j) Pb.bconst[j] = bconst[j];
+    cur_slot = SGP_PROF_R1;
     { RowParams<T> P = Pb; P.mode = RF_PLAIN; P.in0 = f; P.maskmode = MM_NONE; if ((rc = launch_row(k_rowf, P, 1, st))) return rc; }
+    cur_slot = SGP_PROF_R2;
     { ColParams<T> Q = col_params(); Q.check_status = 1; if ((rc = launch_col(k_mult, Q, st))) return rc; }
+    cur_slot = SGP_PROF_R3;
     { RowParams<T> P = Pb; P.mode = RI_QJ; P.submode = QJ_RL; P.in0 = Gp; P.in2 = Bp; P.out0 = q; P.part = part_J; if ((rc = launch_row(k_rowi, P, p, st))) return rc; }
+    cur_slot = SGP_PROF_R4;
     { RowParams<T> P = Pb; P.mode = RF_RATIO; P.in0 = Gp; P.in1 = q; P.in2 = Bp; if ((rc = launch_row(k_rowf, P, p, st))) return rc; }
+    cur_slot = SGP_PROF_R5;
     { ColParams<T> Q = col_params(); Q.check_status = 1; if ((rc = launch_col(k_conj, Q, st))) return rc; }
+    cur_slot = SGP_PROF_R6;
     { RowParams<T> P = Pb; P.mode = RI_RLUPDATE; P.in0 = f; P.out0 = f; if ((rc = launch_row(k_rowi, P, 1, st))) return rc; }
+    cur_slot = -1;
     return SGP_OK;
 }
 
@@ -123,6 +139,7 @@ int PlanImpl<T>::run(int algorithm, const void *const *g, const void *const *b_a
         if (!arr) { if (!b_const) return SGP_ERR_ARG; bconst[j] = b_const[j]; }
     }
     const long launches0 = launches;
+    if (profiling) prof_reset();
 
     DevOpts o;
     memset(&o, 0, sizeof(o));
@@ -223,6 +240,7 @@ int PlanImpl<T>::run(int algorithm, const void *const *g, const void *const *b_a
         if (res->trace_backtracks) SGP_CUDA_TRY(cudaMemcpyAsync(res->trace_backtracks, trB, sizeof(int) * kdone, cudaMemcpyDeviceToHost, st));
     }
     SGP_CUDA_TRY(cudaStreamSynchronize(st));
+    if (profiling) prof_collect();
     float ms01 = 0.f, ms12 = 0.f;
     cudaEventElapsedTime(&ms01, ev0, ev1);
     cudaEventElapsedTime(&ms12, ev1, ev2);
