@@ -27,36 +27,42 @@ int validate_options(const sgp_options *o)
 static int floor_pow2(int v) { int r = 1; while (r * 2 <= v) r *= 2; return r; }
 static bool is_pow2(int v) { return v > 0 && (v & (v - 1)) == 0; }
 
+static int elems_per_thread(int L, int dtype, bool col)
+{
+    if (dtype == SGP_F64) return col ? fft_E_col<double>(L) : fft_E<double>(L);
+    return col ? fft_E_col<float>(L) : fft_E<float>(L);
+}
+static int pad_len(int L, int E) { return L + (L >> (E == 32 ? 5 : 4)); }
+
 // Spectrum tile width C (columns per CTA of the column kernel) and rows per CTA of the row kernels.
 int choose_tiles(int ny, int nx, int dtype, const sgp_options *opt, int *C_out, int *RB_out)
 {
     const int esz = dtype == SGP_F64 ? 16 : 8;                     // bytes per complex number
     const int Lr = nx / 2, Lc = ny;
-    const int Ec = (Lc % 5 == 0) ? 20 : (dtype == SGP_F64 ? 8 : 16);
-    const int Er = (Lr % 5 == 0) ? 20 : (dtype == SGP_F64 ? 8 : 16);
-    // column kernel: at most 512 threads and ~96 KB of shared memory per CTA
-    int C = floor_pow2(512 * Ec / Lc);
+    const int Ec = elems_per_thread(Lc, dtype, true), Er = elems_per_thread(Lr, dtype, false);
+    const int TFc = Lc / Ec, TFr = Lr / Er;
+    // column kernel: 256 threads per CTA when a thread holds 32 elements (two CTAs per SM), else up to 512;
+    // at most ~100 KB of shared memory per CTA
+    const int col_max = Ec == 32 ? 256 : 512;
+    int C = floor_pow2(col_max / TFc > 1 ? col_max / TFc : 1);
     if (C > 32) C = 32;
-    while (C > 1 && (size_t)C * (Lc + Lc / 16) * esz > 96 * 1024) C /= 2;
+    while (C > 1 && (size_t)C * pad_len(Lc, Ec) * esz > 100 * 1024) C /= 2;
     while (C > 1 && Lr % C != 0) C /= 2;
     if (opt && opt->tile_cols > 0) {
         if (!is_pow2(opt->tile_cols) || Lr % opt->tile_cols != 0) return SGP_ERR_ARG;
         C = opt->tile_cols;
     }
-    const int TFc = Lc / Ec;
-    if (C * TFc > 512 || (size_t)C * (Lc + Lc / 16) * esz > 227 * 1024) return SGP_ERR_ARG;
-    // row kernels: about 256 threads per CTA
-    const int TFr = Lr / Er;
+    if (C * TFc > col_max || (C * TFc) % 32 != 0 || (size_t)C * pad_len(Lc, Ec) * esz > 227 * 1024) return SGP_ERR_ARG;
+    // row kernels: 256 threads per CTA; rows whose threads span several warps use one named barrier each (ids 1..15)
     int RB = floor_pow2(256 / TFr > 1 ? 256 / TFr : 1);
     if (RB > 32) RB = 32;
-    while (RB > 1 && (size_t)RB * (Lr + Lr / 16 + 2) * esz > 96 * 1024) RB /= 2;
     if (opt && opt->rows_per_block > 0) {
         if (!is_pow2(opt->rows_per_block)) return SGP_ERR_ARG;
         RB = opt->rows_per_block;
     }
     while (RB > 1 && ny % RB != 0) RB /= 2;
-    if (RB * TFr > 512 || (size_t)RB * (Lr + Lr / 16 + 2) * esz > 227 * 1024) return SGP_ERR_ARG;
-    // the store mapping of the row kernels needs RB*C to divide the RB*Lr outputs of a CTA: true since C | Lr
+    if (RB * TFr > 256 || (RB * TFr) % 32 != 0 || (TFr > 32 && RB > 15)) return SGP_ERR_ARG;
+    if ((size_t)RB * pad_len(Lr, Er) * esz > 113 * 1024) return SGP_ERR_ARG;
     *C_out = C; *RB_out = RB;
     return SGP_OK;
 }

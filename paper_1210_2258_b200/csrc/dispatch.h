@@ -1,5 +1,5 @@
-// dispatch.h -- look-up of the kernel instantiations by FFT length (defined in inst_*.cu, one translation
-// unit per element type and kernel family so that they compile in parallel).
+// dispatch.h -- look-up of the kernel instantiations by FFT length and mode (defined in inst_*.cu, one
+// translation unit per element type and kernel family so that they compile in parallel).
 #pragma once
 #include "kernels.cuh"
 
@@ -9,8 +9,8 @@ template <typename T> using row_kernel_t = void (*)(const RowParams<T>);
 template <typename T> using col_kernel_t = void (*)(const ColParams<T>);
 
 // L = nx/2 (row kernels) or ny (column kernel); nullptr if the length is not supported
-template <typename T> row_kernel_t<T> get_row_fwd(int L);
-template <typename T> row_kernel_t<T> get_row_inv(int L);
+template <typename T> row_kernel_t<T> get_row_fwd(int L, int mode);
+template <typename T> row_kernel_t<T> get_row_inv(int L, int mode);
 template <typename T> col_kernel_t<T> get_col(int L, int mode, bool multi);
 
 // supported grid sizes (ny and nx independently)

@@ -1,0 +1,127 @@
+// ew.cuh -- parameter blocks of the hot-path kernels and the per-pixel arithmetic of the SGP / RL iteration
+// (DESIGN.md section 5).
+//
+// Data layout.  Real planes are row-major ny x nx.  A half spectrum of a real plane holds nx/2 complex
+// numbers per row: entry kx = 1..nx/2-1 is the DFT coefficient, entry 0 packs the two real coefficients
+// (kx = 0, kx = nx/2) as (re, im).  Spectra are stored COLUMN-TILE-MAJOR: tile = kx / C, and inside a tile
+// element (ky, kx % C) sits at ky*C + kx%C, so a CTA of the column kernel reads one contiguous chunk of
+// ny*C complex numbers.
+#pragma once
+#include <cooperative_groups.h>
+#include "fft_core.cuh"
+#include "sgp_dev.cuh"
+
+namespace sgpk {
+namespace cg = cooperative_groups;
+
+enum RowFwdMode { RF_PLAIN = 0, RF_SETUP = 1, RF_RATIO = 2, RF_PROJECT = 3, RF_NMODES = 4 };
+enum RowFwdSetup { RFS_PSF = 0, RFS_MASK_S = 1 };
+enum RowInvMode { RI_PLAIN = 0, RI_GRAD = 1, RI_LS = 2, RI_QJ = 3, RI_RLUPDATE = 4, RI_NMODES = 5 };
+enum RowInvPlain { RIP_STORE = 0, RIP_RLMINMAX = 1 };
+enum MaskMode { MM_NONE = 0, MM_S = 1, MM_R = 2 };
+enum QJSub { QJ_INIT = 0, QJ_RL = 1, QJ_PLAIN = 2 };
+enum Ticket { TK_GRAD = 0, TK_LS = 1, TK_QJ = 2, TK_MINMAX = 3, TK_BACKTRACK = 4 };
+
+template <typename T> struct RowParams {
+    Geom G;
+    DevOpts o;
+    Trace tr;
+    Ctrl *ct;
+    int submode, maskmode, b_is_array;
+    int lazy;                         // 1: SGP loop -- apply the pending update f += lambda d, q_j += lambda u_j on the fly
+    const T *in0, *in1, *in2, *in3;   // real planes; image j at + j*plane
+    T *out0, *out1;
+    cx<T> *spec;                      // spectrum of image j at + j*specplane
+    size_t plane, specplane;
+    const cx<T> *tw;                  // exp(-2 pi i k / (nx/2)), k < nx/2
+    const cx<T> *twh;                 // exp(-2 pi i k / nx),     k <= nx/2
+    const T *alphaR;                  // boundary problems: alpha on R, 0 outside R (Eq.19-20)
+    double *part, *part2;
+    double bconst[kMaxP];
+    int cy, cxs;                      // PSF centre (RFS_PSF)
+    int check_status;                 // 1: return immediately when ct->status != 0
+};
+
+template <typename T> struct ColParams {
+    Geom G;
+    Ctrl *ct;
+    const cx<T> *in;                  // spectrum of image j at + j*specplane
+    cx<T> *out;
+    const cx<T> *khat;                // tiled transfer function of image j at + j*specplane (scaled by 1/(ny nx))
+    const cx<T> *khatB;               // column-0 companion of image j at + j*ny
+    size_t specplane;
+    const cx<T> *tw;                  // exp(-2 pi i k / ny)
+    cx<T> *pack;                      // ny entries of scratch for the packed column of tile 0
+    int p;
+    int check_status;
+};
+
+// ---------------------------------------------------------------- elementwise pieces
+// One summand of Eq.2: g ln(g/y) + y - g with y = A f + b, evaluated without
+// cancellation (A17): g = 0 gives y; y <= 0 drops the log term.
+__device__ __forceinline__ double kl_term(double g, double y)
+{
+    if (!(g > 0.0)) return y;
+    if (!(y > 0.0)) return y - g;
+    double t = (y - g) / g;
+    return g * (t - log1p(t));
+}
+// float version: with u = (y-g)/(y+g), ln(y/g) = 2 atanh(u), hence
+//   g ln(g/y) + y - g = u [ (y-g) - 2 g u^2 (1/3 + u^2/5 + u^4/7 + ...) ]      (u^2 < 0.09: 9 terms, < 1 ulp)
+// and the plain form (y-g) - g log1p((y-g)/g) otherwise (no cancellation there).
+__device__ __forceinline__ float kl_term(float g, float y)
+{
+    if (!(g > 0.f)) return y;
+    if (!(y > 0.f)) return y - g;
+    const float dy = y - g;
+    const float u = __fdividef(dy, y + g);
+    const float w = u * u;
+    if (w < 0.09f) {
+        float S = fmaf(w, 1.f / 19.f, 1.f / 17.f);
+        S = fmaf(w, S, 1.f / 15.f);
+        S = fmaf(w, S, 1.f / 13.f);
+        S = fmaf(w, S, 1.f / 11.f);
+        S = fmaf(w, S, 1.f / 9.f);
+        S = fmaf(w, S, 1.f / 7.f);
+        S = fmaf(w, S, 1.f / 5.f);
+        S = fmaf(w, S, 1.f / 3.f);
+        return u * (dy - 2.f * g * w * S);
+    }
+    return dy - g * log1pf(dy / g);
+}
+// ratio g/(Af+b) of Eq.1/11; 0 where the denominator is <= 0 (A17)
+template <typename T> __device__ __forceinline__ T ratio_term(T g, T y) { return (y > (T)0) ? g / y : (T)0; }
+template <typename T> __device__ __forceinline__ T clipT(T f, T L1, T L2) { return fmin(L2, fmax(L1, f)); }
+
+template <typename T> __device__ __forceinline__ cx<T> ld2(const T *p) { return *reinterpret_cast<const cx<T> *>(p); }
+template <typename T> __device__ __forceinline__ void st2(T *p, cx<T> v) { *reinterpret_cast<cx<T> *>(p) = v; }
+
+// W = M_R / alpha (Eq.21/23) for the two pixels of a pair; unmasked: 1/p.  r0, r1 = pixel in R.
+template <typename T>
+__device__ __forceinline__ void weights(const Geom &G, const T *alphaR, size_t idx, T Wc, cx<T> &a2, cx<T> &w2, bool &r0, bool &r1)
+{
+    r0 = true; r1 = true;
+    w2 = mk<T>(Wc, Wc);
+    if (G.masked) {
+        a2 = ld2<T>(alphaR + idx);
+        r0 = a2.x > (T)0; r1 = a2.y > (T)0;
+        w2.x = r0 ? (T)1 / a2.x : (T)0; w2.y = r1 ? (T)1 / a2.y : (T)0;
+    }
+}
+
+// division that may be 2 ulp off in float (no slow path, no branch); exact in double
+__device__ __forceinline__ float fast_div(float a, float b) { return __fdividef(a, b); }
+__device__ __forceinline__ double fast_div(double a, double b) { return a / b; }
+
+// four consecutive pixels of a row
+template <typename T> struct alignas(16) Quad { T a[4]; };
+template <typename T> __device__ __forceinline__ Quad<T> ldq(const T *p) { return *reinterpret_cast<const Quad<T> *>(p); }
+template <typename T> __device__ __forceinline__ void stq(T *p, const Quad<T> &v) { *reinterpret_cast<Quad<T> *>(p) = v; }
+
+// address of spectrum entry (ky, kx) in the column-tile-major layout
+__device__ __forceinline__ size_t spec_index(const Geom &G, int ky, int kx)
+{
+    return ((size_t)(kx >> G.lc) * (size_t)G.ny + (size_t)ky) * (size_t)G.C + (size_t)(kx & (G.C - 1));
+}
+
+}  // namespace sgpk

@@ -67,6 +67,36 @@ template <int DIR, typename T, typename C> __device__ __forceinline__ void dft5(
     a2 = cadd(r2, iq2); a3 = csub(r2, iq2);
 }
 
+// cos / sin of 2 pi k / 32 from the quarter-wave table (folded to immediates once the callers are unrolled)
+__host__ __device__ constexpr double q32(int k)
+{
+    return k == 0 ? 1.0 : k == 1 ? 0.98078528040323043058 : k == 2 ? 0.92387953251128673848 : k == 3 ? 0.83146961230254523567
+         : k == 4 ? 0.70710678118654752440 : k == 5 ? 0.55557023301960217765 : k == 6 ? 0.38268343236508978178
+         : k == 7 ? 0.19509032201612824808 : 0.0;
+}
+__host__ __device__ constexpr double cos32(int k)
+{
+    k &= 31;
+    return k <= 8 ? q32(k) : k <= 16 ? -q32(16 - k) : k <= 24 ? -q32(k - 16) : q32(32 - k);
+}
+__host__ __device__ constexpr double sin32(int k) { return cos32(k + 24); }
+
+// 8-point DFT on references, natural order in and out
+template <int DIR, typename T, typename C>
+__device__ __forceinline__ void dft8r(C &a0, C &a1, C &a2, C &a3, C &a4, C &a5, C &a6, C &a7)
+{
+    const T h = (T)0.70710678118654752440;
+    dft4<DIR>(a0, a2, a4, a6);
+    dft4<DIR>(a1, a3, a5, a7);
+    a3 = tw_const<DIR>(a3, h, h);
+    a5 = mul_dir_i<DIR>(a5);
+    a7 = tw_const<DIR>(a7, -h, h);
+    dft2<DIR>(a0, a1); dft2<DIR>(a2, a3); dft2<DIR>(a4, a5); dft2<DIR>(a6, a7);
+    // position 2*s1 + s2 holds X[s1 + 4*s2]
+    C o1 = a2, o2 = a4, o3 = a6, o4 = a1, o5 = a3, o6 = a5, o7 = a7;
+    a1 = o1; a2 = o2; a3 = o3; a4 = o4; a5 = o5; a6 = o6; a7 = o7;
+}
+
 // In-register DFT of R points, a[r] -> a[s] (natural order).  Composite radices are Cooley-Tukey
 // products R = R1*R2 with input index r = R2*a + b and output index s = s1 + R1*s2.
 template <int R, int DIR, typename T, typename C> __device__ __forceinline__ void dft(C (&a)[R])
@@ -111,6 +141,30 @@ template <int R, int DIR, typename T, typename C> __device__ __forceinline__ voi
         for (int i = 0; i < 4; ++i)
 #pragma unroll
             for (int j = i + 1; j < 4; ++j) { C t = a[4 * i + j]; a[4 * i + j] = a[4 * j + i]; a[4 * j + i] = t; }
+    } else if constexpr (R == 32) {
+        // R1 = 4 (over a), R2 = 8 (b): r = 8a + b
+#pragma unroll
+        for (int b = 0; b < 8; ++b) dft4<DIR>(a[b], a[8 + b], a[16 + b], a[24 + b]);
+        // u[8*s1 + b] *= W32^(b*s1)
+#pragma unroll
+        for (int s1 = 1; s1 < 4; ++s1)
+#pragma unroll
+            for (int b = 1; b < 8; ++b) {
+                const int k = b * s1;
+                if (k == 8) a[8 * s1 + b] = mul_dir_i<DIR>(a[8 * s1 + b]);
+                else a[8 * s1 + b] = tw_const<DIR>(a[8 * s1 + b], (T)cos32(k), (T)sin32(k));
+            }
+#pragma unroll
+        for (int q = 0; q < 4; ++q)
+            dft8r<DIR, T>(a[8 * q], a[8 * q + 1], a[8 * q + 2], a[8 * q + 3], a[8 * q + 4], a[8 * q + 5], a[8 * q + 6], a[8 * q + 7]);
+        // position 8*s1 + s2 holds X[s1 + 4*s2]
+        C o[32];
+#pragma unroll
+        for (int q = 0; q < 4; ++q)
+#pragma unroll
+            for (int s2 = 0; s2 < 8; ++s2) o[q + 4 * s2] = a[8 * q + s2];
+#pragma unroll
+        for (int i = 0; i < 32; ++i) a[i] = o[i];
     } else if constexpr (R == 20) {
         // R1 = 4 (over a), R2 = 5 (b): r = 5a + b
 #pragma unroll
@@ -148,15 +202,34 @@ template <int R, int DIR, typename T, typename C> __device__ __forceinline__ voi
 }
 
 // ---------------------------------------------------------------- plans
-// Elements per thread: 16 (float, 2^k), 8 (double, 2^k), 20 (5*2^k).
+// Elements per thread: float 32 (L >= 512) or 16, double 8, 5*2^k lengths 20.
 template <typename T> __host__ __device__ constexpr int fft_E(int L)
 {
-    return (L % 5 == 0) ? 20 : (sizeof(T) == 8 ? 8 : 16);
+    return (L % 5 == 0) ? 20 : (sizeof(T) == 8 ? 8 : (L >= 512 ? 32 : 16));
+}
+// column kernel: a thread holds 32 elements only where that saves a pass (L = 512, 1024)
+#ifndef SGP_COL_E32_ALL
+#define SGP_COL_E32_ALL 0
+#endif
+#ifndef SGP_COL_E8_MIN
+#define SGP_COL_E8_MIN (1 << 30)
+#endif
+template <typename T> __host__ __device__ constexpr int fft_E_col(int L)
+{
+    if (sizeof(T) == 4 && L % 5 != 0 && L >= SGP_COL_E8_MIN) return 8;
+    return (L % 5 == 0) ? 20 : (sizeof(T) == 8 ? 8 : ((SGP_COL_E32_ALL ? L >= 512 : (L == 512 || L == 1024)) ? 32 : 16));
 }
 // radix of pass ip (0 = not a pass of this plan)
 __host__ __device__ constexpr int plan_radix(int L, int E, int ip)
 {
-    if (E == 16) {
+    if (E == 32) {
+        switch (L) {
+        case 512:  return ip == 0 ? 32 : ip == 1 ? 16 : 0;
+        case 1024: return ip <= 1 ? 32 : 0;
+        case 2048: return ip == 0 ? 32 : ip <= 2 ? 8 : 0;
+        case 4096: return ip == 0 ? 32 : ip == 1 ? 16 : ip == 2 ? 8 : 0;
+        }
+    } else if (E == 16) {
         switch (L) {
         case 16:   return ip == 0 ? 16 : 0;
         case 32:   return ip == 0 ? 16 : ip == 1 ? 2 : 0;
@@ -196,18 +269,34 @@ __host__ __device__ constexpr int plan_radix(int L, int E, int ip)
 }
 __host__ __device__ constexpr bool plan_ok(int L, int E) { return plan_radix(L, E, 0) != 0; }
 
-// shared-memory index padding: one extra slot every 16 keeps the stride-R stores of the first pass
-// and the reversed reads of the real<->complex untangling spread over the banks
-__host__ __device__ constexpr int fft_pad(int i) { return i + (i >> 4); }
-__host__ __device__ constexpr int fft_padded_len(int L) { return L + (L >> 4); }
+// shared-memory index padding: one extra slot every 2^PS elements (PS = 5 when the first pass is radix 32,
+// else 4) turns the stride-R stores of the first pass into an odd stride, and keeps the reversed reads of the
+// real<->complex untangling spread over the banks
+__host__ __device__ constexpr int pad_shift(int E) { return E == 32 ? 5 : 4; }
+template <int E> __host__ __device__ constexpr int fft_pad(int i) { return i + (i >> pad_shift(E)); }
+__host__ __device__ constexpr int fft_padded_len(int L, int E) { return L + (L >> pad_shift(E)); }
+
+// ---------------------------------------------------------------- synchronisation of the threads of one FFT
+// SyncBlock: all threads of the CTA (column kernel: the columns of a tile are interleaved over the warps).
+// SyncGroup<TF>: the TF threads of one row: __syncwarp when a warp holds whole rows, else a named barrier
+// (id 1 + row slot, TF threads), so that the rows of a CTA never wait for each other.
+struct SyncBlock { __device__ __forceinline__ void operator()() const { __syncthreads(); } };
+template <int TF> struct SyncGroup {
+    int id;
+    __device__ __forceinline__ void operator()() const
+    {
+        if constexpr (TF <= 32) __syncwarp();
+        else asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(TF) : "memory");
+    }
+};
 
 // All passes of one FFT.  sm points at element 0 of this FFT's shared-memory line; consecutive
 // elements are `cs` apart (1 for a row FFT; C for a column FFT stored as [element][column]).
 // tw[k] = exp(-2 pi i k / L).  Every exchange is bracketed sync / store / sync / load, so shared memory
 // the caller used before the call is safe to reuse, and on return nobody is writing it.
-template <typename T, int L, int E, int DIR, int IP, int NS>
+template <typename T, int L, int E, int DIR, int IP, int NS, typename SYNC>
 __device__ __forceinline__ void fft_passes(cx<T> (&v)[E], cx<T> *__restrict__ sm, const int cs, const int t,
-                                           const cx<T> *__restrict__ tw)
+                                           const cx<T> *__restrict__ tw, const SYNC &sync)
 {
     using C = cx<T>;
     constexpr int R = plan_radix(L, E, IP);
@@ -239,22 +328,22 @@ __device__ __forceinline__ void fft_passes(cx<T> (&v)[E], cx<T> *__restrict__ sm
         for (int s = 0; s < R; ++s) v[b + s * B] = a[s];
     }
     if constexpr (!LAST) {
-        __syncthreads();
+        sync();
 #pragma unroll
         for (int b = 0; b < B; ++b)
 #pragma unroll
-            for (int s = 0; s < R; ++s) sm[fft_pad(j0s[b] + s * NS) * cs] = v[b + s * B];
-        __syncthreads();
+            for (int s = 0; s < R; ++s) sm[fft_pad<E>(j0s[b] + s * NS) * cs] = v[b + s * B];
+        sync();
 #pragma unroll
-        for (int e = 0; e < E; ++e) v[e] = sm[fft_pad(t + TF * e) * cs];
-        fft_passes<T, L, E, DIR, IP + 1, NS * R>(v, sm, cs, t, tw);
+        for (int e = 0; e < E; ++e) v[e] = sm[fft_pad<E>(t + TF * e) * cs];
+        fft_passes<T, L, E, DIR, IP + 1, NS * R>(v, sm, cs, t, tw, sync);
     }
 }
 
-template <typename T, int L, int DIR>
-__device__ __forceinline__ void fft_block(cx<T> (&v)[fft_E<T>(L)], cx<T> *sm, int cs, int t, const cx<T> *tw)
+template <typename T, int L, int E, int DIR, typename SYNC>
+__device__ __forceinline__ void fft_block(cx<T> (&v)[E], cx<T> *sm, int cs, int t, const cx<T> *tw, const SYNC &sync)
 {
-    fft_passes<T, L, fft_E<T>(L), DIR, 0, 1>(v, sm, cs, t, tw);
+    fft_passes<T, L, E, DIR, 0, 1>(v, sm, cs, t, tw, sync);
 }
 
 }  // namespace sgpk

@@ -1,18 +1,34 @@
-// included by inst_row_f32.cu / inst_row_f64.cu with SGP_T defined
+// included by inst_row{f,i}_f32.cu / _f64.cu with SGP_T and SGP_ROW_FWD (1 = forward, 0 = inverse) defined
 #include "dispatch.h"
 namespace sgpk {
-#define SGP_ROW_CASE(LEN) case LEN: return row_fwd_kernel<SGP_T, LEN>;
-template <> row_kernel_t<SGP_T> get_row_fwd<SGP_T>(int L)
+#if SGP_ROW_FWD
+template <int L> static row_kernel_t<SGP_T> pick_rowf(int mode)
 {
-    switch (L) {
-        SGP_ROW_CASE(32) SGP_ROW_CASE(64) SGP_ROW_CASE(128) SGP_ROW_CASE(160) SGP_ROW_CASE(256) SGP_ROW_CASE(320)
-        SGP_ROW_CASE(512) SGP_ROW_CASE(640) SGP_ROW_CASE(1024) SGP_ROW_CASE(2048)
+    switch (mode) {
+    case RF_PLAIN: return row_fwd_kernel<SGP_T, L, RF_PLAIN>;
+    case RF_SETUP: return row_fwd_kernel<SGP_T, L, RF_SETUP>;
+    case RF_RATIO: return row_fwd_kernel<SGP_T, L, RF_RATIO>;
+    case RF_PROJECT: return row_fwd_kernel<SGP_T, L, RF_PROJECT>;
     default: return nullptr;
     }
 }
-#undef SGP_ROW_CASE
-#define SGP_ROW_CASE(LEN) case LEN: return row_inv_kernel<SGP_T, LEN>;
-template <> row_kernel_t<SGP_T> get_row_inv<SGP_T>(int L)
+#define SGP_ROW_CASE(LEN) case LEN: return pick_rowf<LEN>(mode);
+template <> row_kernel_t<SGP_T> get_row_fwd<SGP_T>(int L, int mode)
+#else
+template <int L> static row_kernel_t<SGP_T> pick_rowi(int mode)
+{
+    switch (mode) {
+    case RI_PLAIN: return row_inv_kernel<SGP_T, L, RI_PLAIN>;
+    case RI_GRAD: return row_inv_kernel<SGP_T, L, RI_GRAD>;
+    case RI_LS: return row_inv_kernel<SGP_T, L, RI_LS>;
+    case RI_QJ: return row_inv_kernel<SGP_T, L, RI_QJ>;
+    case RI_RLUPDATE: return row_inv_kernel<SGP_T, L, RI_RLUPDATE>;
+    default: return nullptr;
+    }
+}
+#define SGP_ROW_CASE(LEN) case LEN: return pick_rowi<LEN>(mode);
+template <> row_kernel_t<SGP_T> get_row_inv<SGP_T>(int L, int mode)
+#endif
 {
     switch (L) {
         SGP_ROW_CASE(32) SGP_ROW_CASE(64) SGP_ROW_CASE(128) SGP_ROW_CASE(160) SGP_ROW_CASE(256) SGP_ROW_CASE(320)

@@ -1,2 +1,3 @@
 #define SGP_T double
+#define SGP_ROW_FWD 0
 #include "inst_row.inl"

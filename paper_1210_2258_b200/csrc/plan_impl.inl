@@ -7,9 +7,9 @@ template <typename T> struct PlanImpl : PlanBase {
     using C = cx<T>;
     size_t n = 0, nspec = 0;       // reals per plane, complex numbers per half spectrum (= n/2)
     int Lr = 0, Lc = 0;            // FFT lengths: nx/2 (rows), ny (columns)
-    int row_threads = 0, col_threads = 0, nrb = 0, ntiles = 0, upd_grid = 0;
+    int row_threads = 0, col_threads = 0, nrb = 0, ntiles = 0, bt_grid = 0;
     size_t row_smem = 0, col_smem = 0;
-    row_kernel_t<T> k_rowf = nullptr, k_rowi = nullptr;
+    row_kernel_t<T> k_rowf[RF_NMODES] = {nullptr}, k_rowi[RI_NMODES] = {nullptr};
     col_kernel_t<T> k_colf = nullptr, k_conj = nullptr, k_mult = nullptr;
     // device memory
     std::vector<void *> allocs;
@@ -18,7 +18,7 @@ template <typename T> struct PlanImpl : PlanBase {
     T *Gp = nullptr, *Bp = nullptr, *q = nullptr, *u = nullptr, *f = nullptr, *grad = nullptr, *d = nullptr;
     T *alphaR = nullptr, *alpha = nullptr, *scratch = nullptr;
     unsigned char *MR = nullptr;
-    double *part_bb = nullptr, *part_gd = nullptr, *part_J = nullptr, *part_upd = nullptr, *part_misc = nullptr;
+    double *part_bb = nullptr, *part_gd = nullptr, *part_J = nullptr, *part_bt = nullptr, *part_misc = nullptr;
     Ctrl *ct = nullptr;
     // per-run trace buffers
     double *trJ = nullptr, *trA = nullptr, *trL = nullptr, *fA = nullptr, *fL = nullptr;
@@ -91,36 +91,39 @@ template <typename T> struct PlanImpl : PlanBase {
         n = (size_t)ny * nx; nspec = n / 2;
         Lr = nx / 2; Lc = ny;
         constexpr int dummy = 0; (void)dummy;
-        const int Er = fft_E<T>(Lr), Ec = fft_E<T>(Lc);
-        k_rowf = get_row_fwd<T>(Lr); k_rowi = get_row_inv<T>(Lr);
+        const int Er = fft_E<T>(Lr), Ec = fft_E_col<T>(Lc);
+        for (int m = 0; m < RF_NMODES; ++m) if (!(k_rowf[m] = get_row_fwd<T>(Lr, m))) return SGP_ERR_ARG;
+        for (int m = 0; m < RI_NMODES; ++m) if (!(k_rowi[m] = get_row_inv<T>(Lr, m))) return SGP_ERR_ARG;
         const bool multi = p > 1;
         k_colf = get_col<T>(Lc, CM_FWD, false); k_conj = get_col<T>(Lc, CM_CONJSUM, multi); k_mult = get_col<T>(Lc, CM_MULT, multi);
-        if (!k_rowf || !k_rowi || !k_colf || !k_conj || !k_mult) return SGP_ERR_ARG;
+        if (!k_colf || !k_conj || !k_mult) return SGP_ERR_ARG;
         int Cc = 0, RB = 0;
         int rc = choose_tiles(ny, nx, dtype, &opt, &Cc, &RB);
         if (rc) return rc;
-        G.C = Cc; G.RB = RB;
+        G.C = Cc; G.RB = RB; G.lc = 0; while ((1 << G.lc) < Cc) G.lc++;
         row_threads = RB * (Lr / Er);
         col_threads = Cc * (Lc / Ec);
         nrb = ny / RB; ntiles = Lr / Cc;
-        row_smem = (size_t)RB * row_stride(Lr) * sizeof(C);
-        col_smem = (size_t)Cc * fft_padded_len(Lc) * sizeof(C);
-        if (row_threads > 512 || col_threads > 512 || row_smem > 227 * 1024 || col_smem > 227 * 1024) return SGP_ERR_ARG;
-        SGP_CUDA_TRY(cudaFuncSetAttribute((const void *)k_rowf, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)row_smem));
-        SGP_CUDA_TRY(cudaFuncSetAttribute((const void *)k_rowi, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)row_smem));
+        row_smem = (size_t)RB * fft_padded_len(Lr, Er) * sizeof(C);
+        col_smem = (size_t)Cc * fft_padded_len(Lc, Ec) * sizeof(C);
+        if (row_threads > 256 || col_threads > 512 || row_smem > 227 * 1024 || col_smem > 227 * 1024) return SGP_ERR_ARG;
+        for (int m = 0; m < RF_NMODES; ++m)
+            SGP_CUDA_TRY(cudaFuncSetAttribute((const void *)k_rowf[m], cudaFuncAttributeMaxDynamicSharedMemorySize, (int)row_smem));
+        for (int m = 0; m < RI_NMODES; ++m)
+            SGP_CUDA_TRY(cudaFuncSetAttribute((const void *)k_rowi[m], cudaFuncAttributeMaxDynamicSharedMemorySize, (int)row_smem));
         SGP_CUDA_TRY(cudaFuncSetAttribute((const void *)k_colf, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)col_smem));
         SGP_CUDA_TRY(cudaFuncSetAttribute((const void *)k_conj, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)col_smem));
         SGP_CUDA_TRY(cudaFuncSetAttribute((const void *)k_mult, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)col_smem));
-        // cooperative grid of the update kernel
+        // cooperative grid of the backtracking kernel
         int dev = 0, nsm = 0, per_sm = 0;
         SGP_CUDA_TRY(cudaGetDevice(&dev));
         SGP_CUDA_TRY(cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev));
-        SGP_CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, update_kernel<T>, 256, 0));
+        SGP_CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, backtrack_kernel<T>, 256, 0));
         if (per_sm < 1) return SGP_ERR_CUDA;
         if (per_sm > 8) per_sm = 8;
-        upd_grid = nsm * per_sm;
+        bt_grid = nsm * per_sm;
         size_t want = (n / vec4_of<T>::N + 255) / 256;
-        if ((size_t)upd_grid > want) upd_grid = (int)(want < 1 ? 1 : want);
+        if ((size_t)bt_grid > want) bt_grid = (int)(want < 1 ? 1 : want);
 
         // twiddles, computed in double on the host
         std::vector<C> h;
@@ -159,7 +162,7 @@ template <typename T> struct PlanImpl : PlanBase {
         if ((rc = dalloc(&part_bb, (size_t)nrb * 4))) return rc;
         if ((rc = dalloc(&part_gd, (size_t)nrb))) return rc;
         if ((rc = dalloc(&part_J, (size_t)nrb * p * 2))) return rc;
-        if ((rc = dalloc(&part_upd, (size_t)upd_grid))) return rc;
+        if ((rc = dalloc(&part_bt, (size_t)bt_grid))) return rc;
         if ((rc = dalloc(&part_misc, (size_t)1024 * p))) return rc;
         if ((rc = dalloc(&ct, (size_t)1))) return rc;
         SGP_CUDA_TRY(cudaMemset(ct, 0, sizeof(Ctrl)));
@@ -170,11 +173,11 @@ template <typename T> struct PlanImpl : PlanBase {
     }
 
     // ------------------------------------------------------------------ launch helpers
-    RowParams<T> row_params(int mode) const
+    RowParams<T> row_params() const
     {
         RowParams<T> P;
         memset(&P, 0, sizeof(P));
-        P.G = G; P.ct = ct; P.mode = mode;
+        P.G = G; P.ct = ct;
         P.plane = n; P.specplane = nspec; P.spec = spec;
         P.tw = tw_r; P.twh = tw_h; P.alphaR = alphaR;
         return P;
@@ -219,10 +222,10 @@ template <typename T> struct PlanImpl : PlanBase {
             SGP_CUDA_TRY(cudaMemcpyAsync(&h, ct, sizeof(Ctrl), cudaMemcpyDeviceToHost, st));
             SGP_CUDA_TRY(cudaStreamSynchronize(st));
             if (!(h.psf_sum > 0.0) || !std::isfinite(h.psf_sum)) return SGP_ERR_PSF;       // PAPER.md:27 needs a positive volume
-            RowParams<T> P = row_params(RF_PSF);
-            P.in0 = (const T *)psf[j]; P.cy = cy; P.cxs = cxs;
+            RowParams<T> P = row_params();
+            P.submode = RFS_PSF; P.in0 = (const T *)psf[j]; P.cy = cy; P.cxs = cxs;
             P.spec = (C *)scratch;          // raw spectrum of this PSF
-            if ((rc = launch_row(k_rowf, P, 1, st))) return rc;
+            if ((rc = launch_row(k_rowf[RF_SETUP], P, 1, st))) return rc;
             ColParams<T> Q = col_params();
             Q.in = (const C *)scratch; Q.out = (C *)scratch;
             if ((rc = launch_col(k_colf, Q, st))) return rc;
@@ -233,16 +236,17 @@ template <typename T> struct PlanImpl : PlanBase {
         if (G.masked) {
             // alpha_j = A_j^T 1_S = IFFT2(conj K^_j FFT2(M_S)) (Eq.19 in reading A5), alpha = sum_j alpha_j, R by Eq.20
             for (int j = 0; j < p; ++j) {
-                RowParams<T> P = row_params(RF_MASK_S);
-                if ((rc = launch_row(k_rowf, P, 1, st))) return rc;
+                RowParams<T> P = row_params();
+                P.submode = RFS_MASK_S;
+                if ((rc = launch_row(k_rowf[RF_SETUP], P, 1, st))) return rc;
                 ColParams<T> Q = col_params();
                 Q.khat = khat + (size_t)j * nspec; Q.khatB = khatB + (size_t)j * ny; Q.p = 1;
                 col_kernel_t<T> k1 = get_col<T>(Lc, CM_CONJSUM, false);
                 SGP_CUDA_TRY(cudaFuncSetAttribute((const void *)k1, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)col_smem));
                 if ((rc = launch_col(k1, Q, st))) return rc;
-                RowParams<T> R = row_params(RI_PLAIN);
+                RowParams<T> R = row_params();
                 R.out0 = scratch; R.maskmode = MM_NONE;
-                if ((rc = launch_row(k_rowi, R, 1, st))) return rc;
+                if ((rc = launch_row(k_rowi[RI_PLAIN], R, 1, st))) return rc;
                 alpha_accum_kernel<T><<<ew_grid(n), 256, 0, st>>>(scratch, alpha, MR, n, opt.sigma_R, j == 0);
                 launches++;
             }
@@ -285,17 +289,17 @@ template <typename T> struct PlanImpl : PlanBase {
     {
         if (!psf_set || j < 0 || j >= p || !x || !out) return SGP_ERR_ARG;
         int rc;
-        RowParams<T> P = row_params(RF_PLAIN);
+        RowParams<T> P = row_params();
         P.in0 = (const T *)x; P.maskmode = transpose ? MM_S : MM_R;
-        if ((rc = launch_row(k_rowf, P, 1, st))) return rc;
+        if ((rc = launch_row(k_rowf[RF_PLAIN], P, 1, st))) return rc;
         ColParams<T> Q = col_params();
         Q.khat = khat + (size_t)j * nspec; Q.khatB = khatB + (size_t)j * ny; Q.p = 1;
         col_kernel_t<T> k1 = get_col<T>(Lc, transpose ? CM_CONJSUM : CM_MULT, false);
         SGP_CUDA_TRY(cudaFuncSetAttribute((const void *)k1, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)col_smem));
         if ((rc = launch_col(k1, Q, st))) return rc;
-        RowParams<T> R = row_params(RI_PLAIN);
+        RowParams<T> R = row_params();
         R.out0 = scratch; R.maskmode = transpose ? MM_R : MM_S;
-        if ((rc = launch_row(k_rowi, R, 1, st))) return rc;
+        if ((rc = launch_row(k_rowi[RI_PLAIN], R, 1, st))) return rc;
         SGP_CUDA_TRY(cudaMemcpyAsync(out, scratch, n * sizeof(T), cudaMemcpyDeviceToDevice, st));
         SGP_CUDA_TRY(cudaStreamSynchronize(st));
         return SGP_OK;
@@ -305,9 +309,9 @@ template <typename T> struct PlanImpl : PlanBase {
     {
         if (!x || !spec_out) return SGP_ERR_ARG;
         int rc;
-        RowParams<T> P = row_params(RF_PLAIN);
+        RowParams<T> P = row_params();
         P.in0 = (const T *)x;
-        if ((rc = launch_row(k_rowf, P, 1, st))) return rc;
+        if ((rc = launch_row(k_rowf[RF_PLAIN], P, 1, st))) return rc;
         ColParams<T> Q = col_params();
         if ((rc = launch_col(k_colf, Q, st))) return rc;
         spec_to_rfft2_kernel<T><<<ew_grid(n), 256, 0, st>>>(spec, (C *)spec_out, ny, nx, G.C);
@@ -327,9 +331,9 @@ template <typename T> struct PlanImpl : PlanBase {
         SGP_CUDA_TRY(cudaFuncSetAttribute((const void *)ki, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)col_smem));
         ColParams<T> Q = col_params();
         if ((rc = launch_col(ki, Q, st))) return rc;
-        RowParams<T> R = row_params(RI_PLAIN);
+        RowParams<T> R = row_params();
         R.out0 = (T *)x_out; R.maskmode = MM_NONE;
-        if ((rc = launch_row(k_rowi, R, 1, st))) return rc;
+        if ((rc = launch_row(k_rowi[RI_PLAIN], R, 1, st))) return rc;
         SGP_CUDA_TRY(cudaStreamSynchronize(st));
         return SGP_OK;
     }

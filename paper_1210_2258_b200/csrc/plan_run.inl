@@ -39,18 +39,19 @@ int PlanImpl<T>::ensure_trace(int max_iter, const sgp_result *res, Trace *tr, cu
     return SGP_OK;
 }
 
-// One SGP iteration = 7 launches (SURVEY.md 8(d) schedule A): K1 ratio + row FFT, K2 column pass with conj(K^) summed
-// over the images, K3 inverse rows + gradient + BB sums + step length, K4 projection + row FFT of d, K5 column pass
-// with K^_j, K6 inverse rows + u_j + J(lambda = 1) + Armijo test, K7 backtracks (elementwise) + update + book-keeping.
+// One SGP iteration = 7 launches: K1 lazy q update + ratio + row FFT, K2 column pass with conj(K^)
+// summed over the images, K3 inverse rows + lazy f update + gradient + BB sums + step length, K4 projection + row FFT
+// of d, K5 column pass with K^_j, K6 inverse rows + u_j + J(lambda = 1) + Armijo test + book-keeping, K7 backtracks
+// (elementwise; returns at once when lambda = 1 was accepted).
 template <typename T>
 int PlanImpl<T>::enqueue_sgp_iteration(const RowParams<T> &Pb, const DevOpts &o, const Trace &tr, const double *bconst,
                                        int b_is_array, cudaStream_t st)
 {
     int rc;
     cur_slot = SGP_PROF_K1;
-    {   // K1 (a1)
-        RowParams<T> P = Pb; P.mode = RF_RATIO; P.in0 = Gp; P.in1 = q; P.in2 = Bp;
-        if ((rc = launch_row(k_rowf, P, p, st))) return rc;
+    {   // K1 (a10 for q, a1)
+        RowParams<T> P = Pb; P.lazy = 1; P.in0 = Gp; P.in1 = q; P.in2 = Bp; P.in3 = u; P.out0 = q;
+        if ((rc = launch_row(k_rowf[RF_RATIO], P, p, st))) return rc;
     }
     cur_slot = SGP_PROF_K2;
     {   // K2 (a2)
@@ -58,14 +59,14 @@ int PlanImpl<T>::enqueue_sgp_iteration(const RowParams<T> &Pb, const DevOpts &o,
         if ((rc = launch_col(k_conj, Q, st))) return rc;
     }
     cur_slot = SGP_PROF_K3;
-    {   // K3 (a3, a5, a6)
-        RowParams<T> P = Pb; P.mode = RI_GRAD; P.in0 = f; P.in1 = d; P.out0 = grad; P.part = part_bb;
-        if ((rc = launch_row(k_rowi, P, 1, st))) return rc;
+    {   // K3 (a10 for f, a3, a5, a6)
+        RowParams<T> P = Pb; P.lazy = 1; P.in0 = f; P.in1 = d; P.out0 = grad; P.out1 = f; P.part = part_bb;
+        if ((rc = launch_row(k_rowi[RI_GRAD], P, 1, st))) return rc;
     }
     cur_slot = SGP_PROF_K4;
     {   // K4 (a4, a7)
-        RowParams<T> P = Pb; P.mode = RF_PROJECT; P.in0 = f; P.in1 = grad; P.out0 = d; P.part = part_gd;
-        if ((rc = launch_row(k_rowf, P, 1, st))) return rc;
+        RowParams<T> P = Pb; P.in0 = f; P.in1 = grad; P.out0 = d; P.part = part_gd;
+        if ((rc = launch_row(k_rowf[RF_PROJECT], P, 1, st))) return rc;
     }
     cur_slot = SGP_PROF_K5;
     {   // K5 (a8)
@@ -73,20 +74,20 @@ int PlanImpl<T>::enqueue_sgp_iteration(const RowParams<T> &Pb, const DevOpts &o,
         if ((rc = launch_col(k_mult, Q, st))) return rc;
     }
     cur_slot = SGP_PROF_K6;
-    {   // K6 (a8 tail, a9 at lambda = 1)
-        RowParams<T> P = Pb; P.mode = RI_LS; P.in0 = Gp; P.in1 = q; P.in2 = Bp; P.out0 = u; P.part = part_J; P.part2 = part_gd;
-        if ((rc = launch_row(k_rowi, P, p, st))) return rc;
+    {   // K6 (a8 tail, a9 at lambda = 1, a11)
+        RowParams<T> P = Pb; P.in0 = Gp; P.in1 = q; P.in2 = Bp; P.out0 = u; P.part = part_J; P.part2 = part_gd;
+        if ((rc = launch_row(k_rowi[RI_LS], P, p, st))) return rc;
     }
     cur_slot = SGP_PROF_K7;
-    {   // K7 (a9 backtracks, a10, a11)
-        UpdParams<T> U;
+    {   // K7 (a9 backtracks, a11)
+        BtParams<T> U;
         memset(&U, 0, sizeof(U));
-        U.G = G; U.o = o; U.tr = tr; U.ct = ct; U.f = f; U.d = d; U.q = q; U.u = u; U.g = Gp; U.b = Bp;
-        U.plane = n; U.b_is_array = b_is_array; U.part = part_upd;
+        U.G = G; U.o = o; U.tr = tr; U.ct = ct; U.q = q; U.u = u; U.g = Gp; U.b = Bp;
+        U.plane = n; U.b_is_array = b_is_array; U.part = part_bt;
         for (int j = 0; j < p; ++j) U.bconst[j] = bconst[j];
         void *args[] = {(void *)&U};
         ProfScope ps(this, st);
-        SGP_CUDA_TRY(cudaLaunchCooperativeKernel((const void *)update_kernel<T>, dim3(upd_grid), dim3(256), args, 0, st));
+        SGP_CUDA_TRY(cudaLaunchCooperativeKernel((const void *)backtrack_kernel<T>, dim3(bt_grid), dim3(256), args, 0, st));
         launches++;
     }
     cur_slot = -1;
@@ -98,21 +99,21 @@ template <typename T>
 int PlanImpl<T>::enqueue_rl_round(const DevOpts &o, const Trace &tr, const double *bconst, int b_is_array, cudaStream_t st)
 {
     int rc;
-    RowParams<T> Pb = row_params(RF_PLAIN);
+    RowParams<T> Pb = row_params();
     Pb.o = o; Pb.tr = tr; Pb.check_status = 1; Pb.b_is_array = b_is_array;
     for (int j = 0; j < p; ++j) Pb.bconst[j] = bconst[j];
     cur_slot = SGP_PROF_R1;
-    { RowParams<T> P = Pb; P.mode = RF_PLAIN; P.in0 = f; P.maskmode = MM_NONE; if ((rc = launch_row(k_rowf, P, 1, st))) return rc; }
+    { RowParams<T> P = Pb; P.in0 = f; P.maskmode = MM_NONE; if ((rc = launch_row(k_rowf[RF_PLAIN], P, 1, st))) return rc; }
     cur_slot = SGP_PROF_R2;
     { ColParams<T> Q = col_params(); Q.check_status = 1; if ((rc = launch_col(k_mult, Q, st))) return rc; }
     cur_slot = SGP_PROF_R3;
-    { RowParams<T> P = Pb; P.mode = RI_QJ; P.submode = QJ_RL; P.in0 = Gp; P.in2 = Bp; P.out0 = q; P.part = part_J; if ((rc = launch_row(k_rowi, P, p, st))) return rc; }
+    { RowParams<T> P = Pb; P.submode = QJ_RL; P.in0 = Gp; P.in2 = Bp; P.out0 = q; P.part = part_J; if ((rc = launch_row(k_rowi[RI_QJ], P, p, st))) return rc; }
     cur_slot = SGP_PROF_R4;
-    { RowParams<T> P = Pb; P.mode = RF_RATIO; P.in0 = Gp; P.in1 = q; P.in2 = Bp; if ((rc = launch_row(k_rowf, P, p, st))) return rc; }
+    { RowParams<T> P = Pb; P.in0 = Gp; P.in1 = q; P.in2 = Bp; if ((rc = launch_row(k_rowf[RF_RATIO], P, p, st))) return rc; }
     cur_slot = SGP_PROF_R5;
     { ColParams<T> Q = col_params(); Q.check_status = 1; if ((rc = launch_col(k_conj, Q, st))) return rc; }
     cur_slot = SGP_PROF_R6;
-    { RowParams<T> P = Pb; P.mode = RI_RLUPDATE; P.in0 = f; P.out0 = f; if ((rc = launch_row(k_rowi, P, 1, st))) return rc; }
+    { RowParams<T> P = Pb; P.in0 = f; P.out0 = f; if ((rc = launch_row(k_rowi[RI_RLUPDATE], P, 1, st))) return rc; }
     cur_slot = -1;
     return SGP_OK;
 }
@@ -172,19 +173,19 @@ int PlanImpl<T>::run(int algorithm, const void *const *g, const void *const *b_a
     launches++;
     SGP_CUDA_TRY(cudaGetLastError());
 
-    RowParams<T> Pb = row_params(RF_PLAIN);
+    RowParams<T> Pb = row_params();
     Pb.o = o; Pb.tr = tr; Pb.check_status = 1; Pb.b_is_array = b_is_array;
     for (int j = 0; j < p; ++j) Pb.bconst[j] = bconst[j];
 
     if (algorithm == SGP_ALG_SGP) {
-        { RowParams<T> P = Pb; P.mode = RF_PLAIN; P.in0 = f; if ((rc = launch_row(k_rowf, P, 1, st))) return rc; }
+        { RowParams<T> P = Pb; P.in0 = f; if ((rc = launch_row(k_rowf[RF_PLAIN], P, 1, st))) return rc; }
         { ColParams<T> Q = col_params(); Q.check_status = 1; if ((rc = launch_col(k_mult, Q, st))) return rc; }
-        { RowParams<T> P = Pb; P.mode = RI_QJ; P.submode = QJ_INIT; P.in0 = Gp; P.in2 = Bp; P.out0 = q; P.part = part_J;
-          if ((rc = launch_row(k_rowi, P, p, st))) return rc; }
+        { RowParams<T> P = Pb; P.submode = QJ_INIT; P.in0 = Gp; P.in2 = Bp; P.out0 = q; P.part = part_J;
+          if ((rc = launch_row(k_rowi[RI_QJ], P, p, st))) return rc; }
         if (ro.adaptive_L) {     // bounds from one RL step
-            { RowParams<T> P = Pb; P.mode = RF_RATIO; P.in0 = Gp; P.in1 = q; P.in2 = Bp; if ((rc = launch_row(k_rowf, P, p, st))) return rc; }
+            { RowParams<T> P = Pb; P.in0 = Gp; P.in1 = q; P.in2 = Bp; if ((rc = launch_row(k_rowf[RF_RATIO], P, p, st))) return rc; }
             { ColParams<T> Q = col_params(); Q.check_status = 1; if ((rc = launch_col(k_conj, Q, st))) return rc; }
-            { RowParams<T> P = Pb; P.mode = RI_RLMINMAX; P.in0 = f; P.part = part_J; if ((rc = launch_row(k_rowi, P, 1, st))) return rc; }
+            { RowParams<T> P = Pb; P.submode = RIP_RLMINMAX; P.in0 = f; P.part = part_J; if ((rc = launch_row(k_rowi[RI_PLAIN], P, 1, st))) return rc; }
         }
     }
     SGP_CUDA_TRY(cudaEventRecord(ev1, st));
@@ -228,7 +229,7 @@ int PlanImpl<T>::run(int algorithm, const void *const *g, const void *const *b_a
         }
     }
     SGP_CUDA_TRY(cudaEventRecord(ev2, st));
-    copy_plane_kernel<T><<<ew_grid(n), 256, 0, st>>>(f, (T *)f_out, n);
+    final_update_kernel<T><<<ew_grid(n), 256, 0, st>>>(f, d, (T *)f_out, n, ct);     // a10: the last accepted step, if still pending
     launches++;
     SGP_CUDA_TRY(cudaGetLastError());
     const int kdone = h.k;

@@ -1,0 +1,203 @@
+// row_epi.cuh -- elementwise epilogues of the inverse row kernel.  The transformed row w (2L reals) has been
+// parked in shared memory, so the registers of the FFT are free and the planes of the iteration are streamed
+// with 128-bit loads, four pixels per step and thread: x = 4 (t + TF it) .. + 3.
+#pragma once
+#include "ew.cuh"
+
+namespace sgpk {
+
+// quads loaded ahead of the first store of a batch
+template <typename T> __host__ __device__ constexpr int batch_len(int nit)
+{
+    return sizeof(T) == 8 ? (nit % 2 == 0 ? 2 : 1) : (nit % 4 == 0 ? 4 : (nit % 2 == 0 ? 2 : 1));
+}
+
+// M_S for the four pixels of a quad
+template <typename T>
+__device__ __forceinline__ void quad_in_S(const Geom &G, bool rowin, int x, bool (&s)[4])
+{
+#pragma unroll
+    for (int c = 0; c < 4; ++c) s[c] = rowin && (unsigned)(x + c - G.ox) < (unsigned)G.sx;
+}
+
+// a10 (lazy) + a3 + a5: f <- f + lambda d; grad = alpha - w on R (Eq.11/14/18); the four BB dot products with
+// s = lambda d, z = grad - grad_prev, D = (M_R/alpha) clip(f(k),L1,L2) (Eq.7-8).  s/D and z D are formed in T,
+// the products and sums in double.
+template <typename T, int L, int TF, bool MASKED>
+__device__ __forceinline__ void epi_grad(const RowParams<T> &P, const T *wrow, int t, size_t rowbase, double (&acc)[4])
+{
+    const Geom &G = P.G;
+    const int k = P.ct->k;
+    const T lam = (T)P.ct->lambda;
+    const T L1 = (T)P.ct->L1, L2 = (T)P.ct->L2;
+    const T pT = (T)G.p, Wc = (T)(1.0 / (double)G.p);
+    constexpr int NIT = (L / 2) / TF;
+    if (k == 0) {
+#pragma unroll 4
+        for (int it = 0; it < NIT; ++it) {
+            const int x = 4 * (t + TF * it);
+            const Quad<T> w4 = ldq<T>(wrow + x);
+            Quad<T> g4;
+            if constexpr (MASKED) {
+                const Quad<T> a4 = ldq<T>(P.alphaR + rowbase + x);
+#pragma unroll
+                for (int c = 0; c < 4; ++c) g4.a[c] = a4.a[c] > (T)0 ? a4.a[c] - w4.a[c] : (T)0;
+            } else {
+#pragma unroll
+                for (int c = 0; c < 4; ++c) g4.a[c] = pT - w4.a[c];
+            }
+            stq<T>(P.out0 + rowbase + x, g4);
+        }
+        return;
+    }
+    // loads of a batch are issued before its stores: the planes are updated in place, so the compiler must not be
+    // left to order them (it would serialise every load behind the previous store)
+    constexpr int U = batch_len<T>(NIT);
+    for (int it0 = 0; it0 < NIT; it0 += U) {
+        Quad<T> w4[U], f4[U], d4[U], go4[U], a4[U];
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            const int x = 4 * (t + TF * (it0 + u));
+            w4[u] = ldq<T>(wrow + x);
+            f4[u] = ldq<T>(P.in0 + rowbase + x);
+            d4[u] = ldq<T>(P.in1 + rowbase + x);
+            go4[u] = ldq<T>(P.out0 + rowbase + x);
+            if constexpr (MASKED) a4[u] = ldq<T>(P.alphaR + rowbase + x);
+        }
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            const int x = 4 * (t + TF * (it0 + u));
+            Quad<T> g4;
+#pragma unroll
+            for (int c = 0; c < 4; ++c) {
+                const T s = lam * d4[u].a[c];
+                const T fn = f4[u].a[c] + s;
+                f4[u].a[c] = fn;
+                bool inR = true;
+                T av = pT, wv = Wc;
+                if constexpr (MASKED) { av = a4[u].a[c]; inR = av > (T)0; wv = inR ? (T)1 / av : (T)0; }
+                const T gn = inR ? av - w4[u].a[c] : (T)0;
+                g4.a[c] = gn;
+                const T Di = wv * clipT<T>(fn, L1, L2);
+                const T zf = gn - go4[u].a[c];
+                const double si = inR ? (double)fast_div(s, Di) : 0.0, z = inR ? (double)zf : 0.0, zd = inR ? (double)(zf * Di) : 0.0;
+                acc[0] += si * si; acc[1] += si * z; acc[2] += (double)s * zd; acc[3] += zd * zd;
+            }
+            stq<T>(P.out1 + rowbase + x, f4[u]);
+            stq<T>(P.out0 + rowbase + x, g4);
+        }
+    }
+}
+
+// RI_LS (a8 tail + a9): u_j = A_j d on S; J(1) = sum kl(g_j, q_j + u_j + b_j).
+// RI_QJ: q_j = A_j f on S; J0(f) = sum kl(g_j, q_j + b_j) (Eq.2/12 over S, A12); QJ_PLAIN only stores.
+template <typename T, int L, int TF, bool WITH_Q>
+__device__ __forceinline__ void epi_kl(const RowParams<T> &P, const T *wrow, int t, int y, int j, size_t base, bool plain, double (&acc)[1])
+{
+    const Geom &G = P.G;
+    const T bc = (T)P.bconst[j];
+    const bool rowin = (unsigned)(y - G.oy) < (unsigned)G.sy;
+    constexpr int NIT = (L / 2) / TF;
+    constexpr int U = batch_len<T>(NIT);
+    const bool need = rowin && !plain;
+    for (int it0 = 0; it0 < NIT; it0 += U) {
+        Quad<T> w4[U], g4[U], q4[U], b4[U];
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            const int x = 4 * (t + TF * (it0 + u));
+            w4[u] = ldq<T>(wrow + x);
+            if (need) {
+                g4[u] = ldq<T>(P.in0 + base + x);
+                if constexpr (WITH_Q) q4[u] = ldq<T>(P.in1 + base + x);
+                if (P.b_is_array) b4[u] = ldq<T>(P.in2 + base + x);
+            }
+        }
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            const int x = 4 * (t + TF * (it0 + u));
+            bool s[4];
+            quad_in_S<T>(G, rowin, x, s);
+            Quad<T> u4;
+#pragma unroll
+            for (int c = 0; c < 4; ++c) u4.a[c] = s[c] ? w4[u].a[c] : (T)0;
+            stq<T>(P.out0 + base + x, u4);
+            if (need) {
+                T ksum = (T)0;
+#pragma unroll
+                for (int c = 0; c < 4; ++c) {
+                    T yv = u4.a[c];
+                    if constexpr (WITH_Q) yv += q4[u].a[c];
+                    const T bv = P.b_is_array ? b4[u].a[c] : bc;
+                    const T kv = kl_term(g4[u].a[c], (T)(yv + bv));
+                    ksum += s[c] ? kv : (T)0;
+                }
+                acc[0] += (double)ksum;
+            }
+        }
+    }
+}
+
+// plain store with the output mask of Eq.16 (M_S) or Eq.17 (M_R)
+template <typename T, int L, int TF>
+__device__ __forceinline__ void epi_store(const RowParams<T> &P, const T *wrow, int t, int y, size_t rowbase, size_t base)
+{
+    const Geom &G = P.G;
+    const bool rowin = (unsigned)(y - G.oy) < (unsigned)G.sy;
+    constexpr int NIT = (L / 2) / TF;
+#pragma unroll 4
+    for (int it = 0; it < NIT; ++it) {
+        const int x = 4 * (t + TF * it);
+        Quad<T> w4 = ldq<T>(wrow + x);
+        if (P.maskmode == MM_S) {
+            bool s[4];
+            quad_in_S<T>(G, rowin, x, s);
+#pragma unroll
+            for (int c = 0; c < 4; ++c) if (!s[c]) w4.a[c] = (T)0;
+        } else if (P.maskmode == MM_R && G.masked) {
+            const Quad<T> a4 = ldq<T>(P.alphaR + rowbase + x);
+#pragma unroll
+            for (int c = 0; c < 4; ++c) if (!(a4.a[c] > (T)0)) w4.a[c] = (T)0;
+        }
+        stq<T>(P.out0 + base + x, w4);
+    }
+}
+
+// y = (M_R/alpha) f w: one RL step (Eq.1/13/21).  STORE: write it (a12); else accumulate (-min positive, max) for
+// the adaptive bounds (A19).
+template <typename T, int L, int TF, bool STORE>
+__device__ __forceinline__ void epi_rl(const RowParams<T> &P, const T *wrow, int t, size_t rowbase, double (&acc)[2])
+{
+    const Geom &G = P.G;
+    const T Wc = (T)(1.0 / (double)G.p);
+    constexpr int NIT = (L / 2) / TF;
+    constexpr int U = batch_len<T>(NIT);
+    for (int it0 = 0; it0 < NIT; it0 += U) {
+        Quad<T> w4[U], f4[U], a4[U];
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            const int x = 4 * (t + TF * (it0 + u));
+            w4[u] = ldq<T>(wrow + x);
+            f4[u] = ldq<T>(P.in0 + rowbase + x);
+            if (G.masked) a4[u] = ldq<T>(P.alphaR + rowbase + x);
+        }
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            const int x = 4 * (t + TF * (it0 + u));
+            Quad<T> y4;
+#pragma unroll
+            for (int c = 0; c < 4; ++c) {
+                T wv = Wc;
+                if (G.masked) wv = a4[u].a[c] > (T)0 ? (T)1 / a4[u].a[c] : (T)0;
+                y4.a[c] = wv * f4[u].a[c] * w4[u].a[c];
+                if constexpr (!STORE) {
+                    const double yd = (double)y4.a[c];
+                    if (yd > 0.0) acc[0] = fmax(acc[0], -yd);
+                    acc[1] = fmax(acc[1], yd);
+                }
+            }
+            if constexpr (STORE) stq<T>(P.out0 + rowbase + x, y4);
+        }
+    }
+}
+
+}  // namespace sgpk

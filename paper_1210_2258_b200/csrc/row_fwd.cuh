@@ -1,0 +1,232 @@
+// row_fwd.cuh -- real rows -> half spectrum (row pass of FFT2), with the elementwise work of the iteration
+// fused into the load stage.
+//
+// One row is transformed by TF = L/E threads (a warp for the 2048-wide grid: L = 1024, E = 32, passes 32 x 32);
+// the threads of a row synchronise only among themselves (SyncGroup), so the rows of a CTA drift apart and
+// the loads of one row overlap the butterflies and stores of another.  grid = (ny/RB, images), block = RB*TF
+// threads, dynamic smem = RB * padded(L) complex.
+#pragma once
+#include "ew.cuh"
+
+namespace sgpk {
+
+// pairs loaded ahead of the first store of a batch in the load stage
+template <typename T> __host__ __device__ constexpr int fwd_batch(int E)
+{
+    return sizeof(T) == 8 ? (E % 4 == 0 ? 4 : 2) : (E % 8 == 0 ? 8 : 4);
+}
+
+// untangling of one (k, L-k) pair: a = Z[k], zb = Z[L-k], w = exp(-2 pi i k/nx):
+//   E = (a + conj zb)/2, O = -i (a - conj zb)/2:  X[k] = E + w O,  X[L-k] = conj(E - w O)
+template <typename T> __device__ __forceinline__ void untangle(cx<T> a, cx<T> zb, cx<T> w, cx<T> &xk, cx<T> &xlk)
+{
+    const cx<T> b = cconj(zb);
+    const cx<T> Ek = mk<T>((T)0.5 * (a.x + b.x), (T)0.5 * (a.y + b.y));
+    const cx<T> Dk = mk<T>((T)0.5 * (a.x - b.x), (T)0.5 * (a.y - b.y));
+    const cx<T> wo = cmul(w, mk<T>(Dk.y, -Dk.x));          // w * (-i Dk)
+    xk = cadd(Ek, wo);
+    xlk = cconj(csub(Ek, wo));
+}
+
+template <typename T, int L, int MODE>
+__global__ void __launch_bounds__(256, 2) row_fwd_kernel(const RowParams<T> P)
+{
+    using C = cx<T>;
+    constexpr int E = fft_E<T>(L);
+    constexpr int TF = L / E;
+    constexpr int RS = fft_padded_len(L, E);
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    C *sm = reinterpret_cast<C *>(smem_raw);
+    if (P.check_status && P.ct->status != 0) return;
+
+    const Geom &G = P.G;
+    const int tid = threadIdx.x;
+    const int row = tid / TF, t = tid - row * TF;
+    const int y = blockIdx.x * G.RB + row;
+    const int j = blockIdx.y;
+    constexpr int nx = 2 * L;
+    C v[E];
+    float accf = 0.f;
+    double acc[1] = {0.0};
+
+    // ---- load stage with the fused elementwise work
+    if constexpr (MODE == RF_PLAIN) {
+        // plain rows, optionally multiplied by M_S (input of A^T, Eq.17) or M_R (input of A, Eq.16)
+        const T *src = P.in0 + (size_t)j * P.plane + (size_t)y * nx;
+        const bool rowin = (unsigned)(y - G.oy) < (unsigned)G.sy;
+#pragma unroll
+        for (int e = 0; e < E; ++e) {
+            const int x0 = 2 * (t + TF * e);
+            C w2 = ld2<T>(src + x0);
+            if (P.maskmode == MM_S) {
+                if (!(rowin && (unsigned)(x0 - G.ox) < (unsigned)G.sx)) w2.x = (T)0;
+                if (!(rowin && (unsigned)(x0 + 1 - G.ox) < (unsigned)G.sx)) w2.y = (T)0;
+            } else if (P.maskmode == MM_R && G.masked) {
+                C a2 = ld2<T>(P.alphaR + (size_t)y * nx + x0);
+                if (!(a2.x > (T)0)) w2.x = (T)0;
+                if (!(a2.y > (T)0)) w2.y = (T)0;
+            }
+            v[e] = w2;
+        }
+    } else if constexpr (MODE == RF_SETUP) {
+        if (P.submode == RFS_PSF) {
+            // K_j normalised to unit volume and circularly shifted so that its centre sits at (0,0) (A18)
+            const T *src = P.in0 + (size_t)j * P.plane;
+            const T inv = (T)(1.0 / P.ct->psf_sum);
+            int ys = y + P.cy; if (ys >= G.ny) ys -= G.ny;
+#pragma unroll
+            for (int e = 0; e < E; ++e) {
+                int x0 = 2 * (t + TF * e) + P.cxs; if (x0 >= nx) x0 -= nx;
+                int x1 = x0 + 1; if (x1 >= nx) x1 -= nx;
+                v[e] = mk<T>(src[(size_t)ys * nx + x0] * inv, src[(size_t)ys * nx + x1] * inv);
+            }
+        } else {   // RFS_MASK_S
+#pragma unroll
+            for (int e = 0; e < E; ++e) {
+                int x0 = 2 * (t + TF * e);
+                v[e] = mk<T>(in_S(G, y, x0) ? (T)1 : (T)0, in_S(G, y, x0 + 1) ? (T)1 : (T)0);
+            }
+        }
+    } else if constexpr (MODE == RF_RATIO) {
+        // a10 (lazy): q_j <- q_j + lambda u_j of the step accepted last iteration; a1: r_j = g_j / (q_j + b_j) on S (Eq.11/14/18)
+        const size_t base = (size_t)j * P.plane + (size_t)y * nx;
+        const T bc = (T)P.bconst[j];
+        const bool rowin = (unsigned)(y - G.oy) < (unsigned)G.sy;
+        const bool pend = P.lazy && P.ct->pending;
+        const T lam = (T)P.ct->lambda;
+        // loads of a batch are issued before its stores (q is updated in place: the compiler would otherwise
+        // serialise every load behind the previous store)
+        constexpr int U = fwd_batch<T>(E);
+#pragma unroll
+        for (int e0 = 0; e0 < E; e0 += U) {
+            C g2[U], q2[U], u2[U], b2[U];
+            if (rowin) {
+#pragma unroll
+                for (int u = 0; u < U; ++u) {
+                    const int x0 = 2 * (t + TF * (e0 + u));
+                    g2[u] = ld2<T>(P.in0 + base + x0);
+                    q2[u] = ld2<T>(P.in1 + base + x0);
+                    if (pend) u2[u] = ld2<T>(P.in3 + base + x0);
+                    b2[u] = P.b_is_array ? ld2<T>(P.in2 + base + x0) : mk<T>(bc, bc);
+                }
+            }
+#pragma unroll
+            for (int u = 0; u < U; ++u) {
+                const int x0 = 2 * (t + TF * (e0 + u));
+                C r = mk<T>((T)0, (T)0);
+                if (rowin) {
+                    C qn = q2[u];
+                    if (pend) {
+                        qn.x = qn.x + lam * u2[u].x; qn.y = qn.y + lam * u2[u].y;
+                        st2<T>(P.out0 + base + x0, qn);
+                    }
+                    if ((unsigned)(x0 - G.ox) < (unsigned)G.sx)     r.x = ratio_term<T>(g2[u].x, qn.x + b2[u].x);
+                    if ((unsigned)(x0 + 1 - G.ox) < (unsigned)G.sx) r.y = ratio_term<T>(g2[u].y, qn.y + b2[u].y);
+                }
+                v[e0 + u] = r;
+            }
+        }
+    } else {   // RF_PROJECT
+        // a4 + a7: D = (M_R/alpha) clip(f,L1,L2) (Eq.10/23); y = P+(f - alpha_k D grad) (Eq.6); d = y - f; gd = grad'd
+        const size_t base = (size_t)y * nx;
+        const T alpha = (T)P.ct->alpha, L1 = (T)P.ct->L1, L2 = (T)P.ct->L2;
+        const T Wc = (T)(1.0 / (double)G.p);
+        constexpr int U = fwd_batch<T>(E);
+#pragma unroll
+        for (int e0 = 0; e0 < E; e0 += U) {
+            C f2[U], g2[U], a2[U];
+#pragma unroll
+            for (int u = 0; u < U; ++u) {
+                const int x0 = 2 * (t + TF * (e0 + u));
+                f2[u] = ld2<T>(P.in0 + base + x0);
+                g2[u] = ld2<T>(P.in1 + base + x0);
+                if (G.masked) a2[u] = ld2<T>(P.alphaR + base + x0);
+            }
+#pragma unroll
+            for (int u = 0; u < U; ++u) {
+                const int x0 = 2 * (t + TF * (e0 + u));
+                C w2 = mk<T>(Wc, Wc);
+                bool r0 = true, r1 = true;
+                if (G.masked) {
+                    r0 = a2[u].x > (T)0; r1 = a2[u].y > (T)0;
+                    w2.x = r0 ? (T)1 / a2[u].x : (T)0; w2.y = r1 ? (T)1 / a2[u].y : (T)0;
+                }
+                C d2;
+                {
+                    T D = w2.x * clipT<T>(f2[u].x, L1, L2);
+                    T yv = f2[u].x - alpha * D * g2[u].x;
+                    d2.x = r0 ? ((yv > (T)0 ? yv : (T)0) - f2[u].x) : (T)0;
+                    D = w2.y * clipT<T>(f2[u].y, L1, L2);
+                    yv = f2[u].y - alpha * D * g2[u].y;
+                    d2.y = r1 ? ((yv > (T)0 ? yv : (T)0) - f2[u].y) : (T)0;
+                }
+                if constexpr (sizeof(T) == 4) {
+                    accf += g2[u].x * d2.x + g2[u].y * d2.y;
+                    if (((e0 + u) & 3) == 3) { acc[0] += (double)accf; accf = 0.f; }
+                } else {
+                    acc[0] += (double)g2[u].x * (double)d2.x + (double)g2[u].y * (double)d2.y;
+                }
+                st2<T>(P.out0 + base + x0, d2);
+                v[e0 + u] = d2;
+            }
+        }
+        acc[0] += (double)accf;
+    }
+
+    // ---- complex FFT of length L = nx/2 over z[m] = x[2m] + i x[2m+1]
+    C *smrow = sm + row * RS;
+    const SyncGroup<TF> sync{1 + row};
+    fft_block<T, L, E, -1>(v, smrow, 1, t, P.tw, sync);
+    sync();
+#pragma unroll
+    for (int e = 0; e < E; ++e) smrow[fft_pad<E>(t + TF * e)] = v[e];
+    sync();
+
+    // ---- untangle the two interleaved real transforms, one (k, L-k) pair per step, and store tile-major:
+    //      E = (Z[k] + conj Z[L-k])/2, O = -i (Z[k] - conj Z[L-k])/2, w = exp(-2 pi i k/nx):
+    //      X[k] = E + w O,  X[L-k] = conj(E - w O);  entry 0 = (X[0], X[L]) packed;  X[L/2] = conj Z[L/2]
+    C *dst = P.spec + (size_t)j * P.specplane;
+    {   // i = 0
+        const C a = smrow[fft_pad<E>(t)];
+        if (t == 0) {
+            dst[spec_index(G, y, 0)] = mk<T>(a.x + a.y, a.x - a.y);
+            dst[spec_index(G, y, L / 2)] = cconj(smrow[fft_pad<E>(L / 2)]);
+        } else {
+            C xk, xlk;
+            untangle<T>(a, smrow[fft_pad<E>(L - t)], __ldg(&P.twh[t]), xk, xlk);
+            dst[spec_index(G, y, t)] = xk;
+            dst[spec_index(G, y, L - t)] = xlk;
+        }
+    }
+    if ((TF & (G.C - 1)) == 0) {
+        // TF is a multiple of the tile width: kx -> kx + TF moves TF/C tiles on, i.e. TF*ny elements
+        const size_t stride = (size_t)TF * (size_t)G.ny;
+        C *pa = dst + spec_index(G, y, t);
+        C *pb = dst + spec_index(G, y, L - TF - t) + stride;
+#pragma unroll
+        for (int i = 1; i < E / 2; ++i) {
+            const int k = t + TF * i;
+            C xk, xlk;
+            untangle<T>(smrow[fft_pad<E>(k)], smrow[fft_pad<E>(L - k)], __ldg(&P.twh[k]), xk, xlk);
+            pa[(size_t)i * stride] = xk;
+            *(pb - (size_t)i * stride) = xlk;
+        }
+    } else {
+#pragma unroll 4
+        for (int i = 1; i < E / 2; ++i) {
+            const int k = t + TF * i;
+            C xk, xlk;
+            untangle<T>(smrow[fft_pad<E>(k)], smrow[fft_pad<E>(L - k)], __ldg(&P.twh[k]), xk, xlk);
+            dst[spec_index(G, y, k)] = xk;
+            dst[spec_index(G, y, L - k)] = xlk;
+        }
+    }
+
+    if constexpr (MODE == RF_PROJECT) {
+        __shared__ double red[32];
+        block_reduce_sum<1>(acc, red);
+        if (tid == 0) P.part[blockIdx.x] = acc[0];
+    }
+}
+
+}  // namespace sgpk

@@ -27,7 +27,7 @@ struct Ctrl {
     int total_backtracks;
     int ring_len, ring_pos, nJ;
     int flag_data;         // set by the input-cleaning kernels: 1 = non-finite g, 2 = negative g (strict), 4 = negative f0
-    int pad0;
+    int pending;           // 1: the accepted step (lambda, d, u_j) has not been added to f, q_j yet (lazy update, a10)
     double alpha;          // alpha_k of the current iteration
     double lambda;         // accepted lambda of the last completed iteration (s(k-1) = lambda d)
     double alpha_prev, tau;
@@ -56,7 +56,8 @@ struct Geom {
     int oy, ox, sy, sx;    // S inside S-bar
     int masked;            // boundary-effect problem: alphaR plane present
     int p;
-    int C;                 // spectrum tile width (columns)
+    int C;                 // spectrum tile width (columns), a power of two
+    int lc;                // log2(C)
     int RB;                // rows per block in the row kernels
 };
 
@@ -131,6 +132,7 @@ __device__ inline void finish_iteration(Ctrl *ct, const DevOpts &o, const Trace 
     const double Jold = ct->J;
     ct->J = Jnew;
     ct->lambda = lambda;
+    ct->pending = 1;
     ct->Jhist[(k + 1) % o.armijo_memory] = Jnew;
     if (ct->nJ < o.armijo_memory) ct->nJ++;
     ct->k = k + 1;

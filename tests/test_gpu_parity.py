@@ -108,7 +108,9 @@ def long_run_tolerances(w, dt, tol, jtol, fo, ro, **optkw):
                 devs.append(oracle_run(w, np.float64, f0_scale=1.0 + 2.0 ** -53 * xi, **optkw))
             scale = 10.0
         df = max(rel_l2(f, fo) for f, _ in devs)
-        dj = max(abs(r.J0_final - ro.J0_final) / abs(ro.J0_final) for _, r in devs)
+        # largest deviation anywhere along the J0 trace: the deviation at the last iterate alone is a coin flip
+        dj = max(float(np.max(np.abs(np.asarray(r.J)[:n] - np.asarray(ro.J)[:n]) / np.abs(np.asarray(ro.J)[:n])))
+                 for _, r in devs for n in [min(len(r.J), len(ro.J))])
         _SENS_CACHE[key] = (scale * df, scale * dj)
     sf, sj = _SENS_CACHE[key]
     return max(tol, sf), max(jtol, sj)
@@ -233,8 +235,9 @@ def test_sgp_adaptive_bounds_and_discrepancy_stop_C1(dt, tol):
     ltol = 1e-3 if dt == np.float32 else 1e-9
     assert abs(rg.L1_used - ro.L1_used) <= ltol * ro.L1_used and abs(rg.L2_used - ro.L2_used) <= ltol * ro.L2_used
     if rg.iterations == ro.iterations:
-        assert rel_l2(fg, fo) < tol
-        assert abs(rg.J0_final - ro.J0_final) <= 1e-4 * abs(ro.J0_final)
+        ftol, jt = long_run_tolerances(w, dt, tol, 1e-4 if dt == np.float32 else 1e-12, fo, ro)
+        assert rel_l2(fg, fo) < ftol
+        assert abs(rg.J0_final - ro.J0_final) <= jt * abs(ro.J0_final)
     assert rg.discrepancy_final <= 1.0
 
 
