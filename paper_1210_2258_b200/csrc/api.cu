@@ -46,7 +46,7 @@ int choose_tiles(int ny, int nx, int dtype, const sgp_options *opt, int *C_out, 
     const int col_max = Ec == 32 ? 256 : 512;
     int C = floor_pow2(col_max / TFc > 1 ? col_max / TFc : 1);
     if (C > 32) C = 32;
-    while (C > 1 && (size_t)C * pad_len(Lc, Ec) * esz > 100 * 1024) C /= 2;
+    while (C > 1 && (size_t)C * pad_len(Lc, Ec) * esz > 72 * 1024) C /= 2;
     while (C > 1 && Lr % C != 0) C /= 2;
     if (opt && opt->tile_cols > 0) {
         if (!is_pow2(opt->tile_cols) || Lr % opt->tile_cols != 0) return SGP_ERR_ARG;

@@ -1,10 +1,13 @@
 // col.cuh -- column pass of FFT2 fused with the transfer-function product.
-// One CTA owns a tile of C adjacent columns of the half spectrum: forward column FFTs, pointwise product with
-// the transfer function(s) (conjugated and summed over the images for A^T), inverse column FFTs -- the spectrum
-// never leaves the registers between the three steps.
+// A tile of C adjacent columns of the half spectrum is handled by one CTA: forward column FFTs, pointwise product
+// with the transfer function(s) (conjugated and summed over the images for A^T), inverse column FFTs -- the
+// spectrum never leaves the registers between the three steps.
 //
-// grid = (nx/2)/C tiles, block = C * (L/E) threads (thread = (t, c), c fastest, so global accesses are
-// contiguous), dynamic smem = C * padded(L) complex.
+// The kernel is PERSISTENT: grid = min(tiles, SMs), CTA b works on tiles b, b + grid, ...; the spectrum and the
+// transfer-function tile of the next unit of work are copied global -> shared with cp.async while the current
+// one is transformed, so the only exposed load is the first.  block = C * (L/E) threads (thread = (t, c), c
+// fastest: global accesses are contiguous), dynamic smem = C * padded(L) complex (exchange buffer of the FFT
+// passes) + 2 tiles (landing zones of the asynchronous copies).
 //   CM_FWD / CM_INV: out = forward / unnormalised inverse column FFT of in (set-up of the transfer functions, rfft2 helpers)
 //   CM_CONJSUM: out = IFFTcol( sum_j conj(K^_j) o FFTcol(in_j) )         (a2: sum_j A_j^T r_j in Fourier space, Eq.17)
 //   CM_MULT   : out_j = IFFTcol( K^_j o FFTcol(in) ), j < p              (a8: A_j d, Eq.16)
@@ -18,46 +21,145 @@ namespace sgpk {
 
 enum ColMode { CM_FWD = 0, CM_CONJSUM = 1, CM_MULT = 2, CM_INV = 3 };
 
-__device__ __forceinline__ void prefetch_l2(const void *p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
+// asynchronous copy of one complex number global -> shared (LDGSTS), and the group bookkeeping around it
+template <typename C> __device__ __forceinline__ void cp_async_cx(C *smem_dst, const C *gmem_src)
+{
+    const unsigned int s = (unsigned int)__cvta_generic_to_shared(smem_dst);
+    if constexpr (sizeof(C) == 8) asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(s), "l"(gmem_src) : "memory");
+    else                          asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(s), "l"(gmem_src) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N> __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
+
+// per-CTA view of the work: tile it of this CTA starts at tile_of(it) in a spectrum plane
+template <typename T, int L, int E> struct ColCtx {
+    using C = cx<T>;
+    int tid, nthr, t, c, Cc;
+    size_t tile_len;
+    C *smc, *bufA, *bufB;
+    __device__ __forceinline__ size_t tile_of(int it) const { return (size_t)((int)blockIdx.x + it * (int)gridDim.x) * tile_len; }
+    // copies of this thread's own elements: what a thread reads back it has copied itself, so waiting for the
+    // copy group is all the synchronisation the landing zones need
+    __device__ __forceinline__ void fetch(C *buf, const C *src) const
+    {
+#pragma unroll
+        for (int e = 0; e < E; ++e) cp_async_cx<C>(buf + tid + e * nthr, src + tid + (size_t)e * nthr);
+    }
+};
+
+// product with the packed-column companion B (see the header): r[e] (+)= conj?(B) C~
+template <typename T, int L, int E, bool CONJ>
+__device__ __forceinline__ void packed_fix(cx<T> (&r)[E], volatile cx<T> *pack, const cx<T> *khatB, int t)
+{
+    using C = cx<T>;
+    constexpr int TF = L / E;
+#pragma unroll
+    for (int e = 0; e < E; ++e) {
+        const int ky = t + TF * e, kyn = ky == 0 ? 0 : L - ky;
+        C ct; ct.x = pack[kyn].x; ct.y = -pack[kyn].y;
+        r[e] = cadd(r[e], CONJ ? cmulc(ct, khatB[ky]) : cmul(ct, khatB[ky]));
+    }
+}
 
 template <typename T, int L, int MODE, bool MULTI>
-__global__ void __launch_bounds__(fft_E_col<T>(L) == 32 ? 256 : 512, ((fft_E_col<T>(L) == 32 && !MULTI) || (fft_E_col<T>(L) == 8 && sizeof(T) == 4)) ? 2 : 1) col_kernel(const ColParams<T> P)
+__global__ void __launch_bounds__(fft_E_col<T>(L) == 32 ? 256 : 512, 1) col_kernel(const ColParams<T> P)
 {
     using C = cx<T>;
     constexpr int E = fft_E_col<T>(L);
     constexpr int TF = L / E;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     C *sm = reinterpret_cast<C *>(smem_raw);
-    if (P.check_status && P.ct->status != 0) return;
+    pdl_trigger();
 
-    const int Cc = P.G.C;
-    const int tid = threadIdx.x, nthr = blockDim.x;
-    const int t = tid / Cc, c = tid - t * Cc;
-    const size_t tbase = (size_t)blockIdx.x * ((size_t)L * Cc) + tid;
-    C *smc = sm + c;
-    const bool packed = (blockIdx.x == 0);      // tile 0 holds the packed column
-    const bool pk = packed && c == 0;
+    ColCtx<T, L, E> X;
+    X.Cc = P.G.C; X.tid = threadIdx.x; X.nthr = blockDim.x;
+    X.t = X.tid / X.Cc; X.c = X.tid - X.t * X.Cc;
+    X.tile_len = (size_t)L * X.Cc;
+    X.smc = sm + X.c;
+    X.bufA = sm + (size_t)X.Cc * fft_padded_len(L, E);     // landing zone of the spectrum tile
+    X.bufB = X.bufA + X.tile_len;                          // landing zone of the transfer-function tile
+    const int tid = X.tid, nthr = X.nthr, t = X.t, Cc = X.Cc;
     volatile C *pack = P.pack;
     const SyncBlock sync;
+    const int ntiles = P.ntiles;
     C v[E];
 
     if constexpr (MODE == CM_FWD || MODE == CM_INV) {
+        pdl_wait();
+        for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
+            const size_t tbase = (size_t)tile * X.tile_len + tid;
 #pragma unroll
-        for (int e = 0; e < E; ++e) v[e] = P.in[tbase + (size_t)e * nthr];
-        fft_block<T, L, E, (MODE == CM_FWD ? -1 : +1)>(v, smc, Cc, t, P.tw, sync);
+            for (int e = 0; e < E; ++e) v[e] = P.in[tbase + (size_t)e * nthr];
+            fft_block<T, L, E, (MODE == CM_FWD ? -1 : +1)>(v, X.smc, Cc, t, P.tw, sync);
 #pragma unroll
-        for (int e = 0; e < E; ++e) P.out[tbase + (size_t)e * nthr] = v[e];
-    } else if constexpr (MODE == CM_CONJSUM) {
+            for (int e = 0; e < E; ++e) P.out[tbase + (size_t)e * nthr] = v[e];
+        }
+        return;
+    }
+    const int p = MULTI ? P.p : 1;
+    const int my_tiles = ((int)blockIdx.x < ntiles) ? (ntiles - 1 - (int)blockIdx.x) / (int)gridDim.x + 1 : 0;
+    if (my_tiles == 0) return;
+    // the transfer function does not depend on the previous kernel: its first tile is on its way before we wait
+    X.fetch(X.bufB, P.khat + X.tile_of(0)); cp_async_commit();
+    pdl_wait();
+    if (P.check_status && P.ct->status != 0) { cp_async_wait<0>(); return; }
+    X.fetch(X.bufA, P.in + X.tile_of(0)); cp_async_commit();
+
+    if constexpr (MODE == CM_CONJSUM) {
+        // unit of work u = it*p + j: spectrum and transfer function of image j on this CTA's it-th tile.
+        // Copy groups are committed in the order B(0) A(0) A(1) B(1) A(2) B(2) ..., one per unit and buffer (empty at
+        // the end), so after the first unit "all but the newest group" is always the one about to be read.
+        const int units = my_tiles * p;
         C acc[MULTI ? E : 1];
-        const int p = MULTI ? P.p : 1;
-        for (int j = 0; j < p; ++j) {
-            const C *src = P.in + (size_t)j * P.specplane;
-            const C *kh = P.khat + (size_t)j * P.specplane;
+        for (int it = 0; it < my_tiles; ++it) {
+            const bool packed = (blockIdx.x == 0 && it == 0);      // tile 0 holds the packed column
+            const bool pk = packed && X.c == 0;
+            for (int j = 0; j < p; ++j) {
+                const int u1 = it * p + j + 1, it1 = u1 / p, j1 = u1 - it1 * p;
+                if (u1 == 1) cp_async_wait<0>(); else cp_async_wait<1>();   // spectrum of this unit has landed
 #pragma unroll
-            for (int e = 0; e < E; ++e) v[e] = src[tbase + (size_t)e * nthr];
-            // the transfer function is needed only after the forward transform: start it on its way to L2 now
-            for (int e = (tid & 15); e < E; e += 16) prefetch_l2(kh + tbase - (tid & 15) + (size_t)e * nthr);
-            fft_block<T, L, E, -1>(v, smc, Cc, t, P.tw, sync);
+                for (int e = 0; e < E; ++e) v[e] = X.bufA[tid + e * nthr];
+                if (u1 < units) X.fetch(X.bufA, P.in + (size_t)j1 * P.specplane + X.tile_of(it1));
+                cp_async_commit();
+                fft_block<T, L, E, -1>(v, X.smc, Cc, t, P.tw, sync);
+                if (packed) {
+                    if (pk) {
+#pragma unroll
+                        for (int e = 0; e < E; ++e) { pack[t + TF * e].x = v[e].x; pack[t + TF * e].y = v[e].y; }
+                    }
+                    __syncthreads();
+                }
+                cp_async_wait<1>();                                 // transfer function of this unit has landed
+#pragma unroll
+                for (int e = 0; e < E; ++e) v[e] = cmulc(v[e], X.bufB[tid + e * nthr]);
+                if (u1 < units) X.fetch(X.bufB, P.khat + (size_t)j1 * P.specplane + X.tile_of(it1));
+                cp_async_commit();
+                if (pk) packed_fix<T, L, E, true>(v, pack, P.khatB + (size_t)j * L, t);
+                if constexpr (MULTI) {
+#pragma unroll
+                    for (int e = 0; e < E; ++e) acc[e] = (j == 0) ? v[e] : cadd(acc[e], v[e]);
+                    if (packed) __syncthreads();                    // pack[] is rewritten for the next image
+                }
+            }
+            if constexpr (MULTI) {
+#pragma unroll
+                for (int e = 0; e < E; ++e) v[e] = acc[e];
+            }
+            fft_block<T, L, E, +1>(v, X.smc, Cc, t, P.tw, sync);
+            C *dst = P.out + X.tile_of(it) + tid;
+#pragma unroll
+            for (int e = 0; e < E; ++e) dst[(size_t)e * nthr] = v[e];
+        }
+    } else {   // CM_MULT: groups B(0,0) A(0) A(1) B(0,1) .. B(0,p-1) B(1,0) A(2) ...
+        for (int it = 0; it < my_tiles; ++it) {
+            const bool packed = (blockIdx.x == 0 && it == 0);
+            const bool pk = packed && X.c == 0;
+            if (it == 0) cp_async_wait<0>(); else cp_async_wait<1>();   // spectrum of tile it has landed
+#pragma unroll
+            for (int e = 0; e < E; ++e) v[e] = X.bufA[tid + e * nthr];
+            if (it + 1 < my_tiles) X.fetch(X.bufA, P.in + X.tile_of(it + 1));
+            cp_async_commit();
+            fft_block<T, L, E, -1>(v, X.smc, Cc, t, P.tw, sync);
             if (packed) {
                 if (pk) {
 #pragma unroll
@@ -65,63 +167,23 @@ __global__ void __launch_bounds__(fft_E_col<T>(L) == 32 ? 256 : 512, ((fft_E_col
                 }
                 __syncthreads();
             }
+            for (int j = 0; j < p; ++j) {
+                C w[E];
+                if (j == 0) cp_async_wait<1>(); else cp_async_wait<0>();   // transfer function (it, j) has landed
 #pragma unroll
-            for (int e = 0; e < E; ++e) {
-                const C k = kh[tbase + (size_t)e * nthr];
-                const C r = cmulc(v[e], k);
-                if constexpr (MULTI) { if (j == 0) acc[e] = r; else acc[e] = cadd(acc[e], r); }
-                else v[e] = r;
+                for (int e = 0; e < E; ++e) w[e] = cmul(v[e], X.bufB[tid + e * nthr]);
+                if (j + 1 < p) X.fetch(X.bufB, P.khat + (size_t)(j + 1) * P.specplane + X.tile_of(it));
+                else if (it + 1 < my_tiles) X.fetch(X.bufB, P.khat + X.tile_of(it + 1));
+                cp_async_commit();
+                if (pk) packed_fix<T, L, E, false>(w, pack, P.khatB + (size_t)j * L, t);
+                fft_block<T, L, E, +1>(w, X.smc, Cc, t, P.tw, sync);
+                C *dst = P.out + (size_t)j * P.specplane + X.tile_of(it) + tid;
+#pragma unroll
+                for (int e = 0; e < E; ++e) dst[(size_t)e * nthr] = w[e];
             }
-            if (pk) {
-#pragma unroll
-                for (int e = 0; e < E; ++e) {
-                    const int ky = t + TF * e, kyn = ky == 0 ? 0 : L - ky;
-                    C ct; ct.x = pack[kyn].x; ct.y = -pack[kyn].y;
-                    const C r = cmulc(ct, P.khatB[(size_t)j * L + ky]);
-                    if constexpr (MULTI) acc[e] = cadd(acc[e], r); else v[e] = cadd(v[e], r);
-                }
-            }
-            if (packed && MULTI) __syncthreads();      // pack[] is rewritten for the next image
-        }
-        if constexpr (MULTI) {
-#pragma unroll
-            for (int e = 0; e < E; ++e) v[e] = acc[e];
-        }
-        fft_block<T, L, E, +1>(v, smc, Cc, t, P.tw, sync);
-#pragma unroll
-        for (int e = 0; e < E; ++e) P.out[tbase + (size_t)e * nthr] = v[e];
-    } else {   // CM_MULT
-#pragma unroll
-        for (int e = 0; e < E; ++e) v[e] = P.in[tbase + (size_t)e * nthr];
-        for (int e = (tid & 15); e < E; e += 16) prefetch_l2(P.khat + tbase - (tid & 15) + (size_t)e * nthr);
-        fft_block<T, L, E, -1>(v, smc, Cc, t, P.tw, sync);
-        if (packed) {
-            if (pk) {
-#pragma unroll
-                for (int e = 0; e < E; ++e) { pack[t + TF * e].x = v[e].x; pack[t + TF * e].y = v[e].y; }
-            }
-            __syncthreads();
-        }
-        const int p = MULTI ? P.p : 1;
-        for (int j = 0; j < p; ++j) {
-            const C *kh = P.khat + (size_t)j * P.specplane;
-            C w[E];
-#pragma unroll
-            for (int e = 0; e < E; ++e) w[e] = cmul(v[e], kh[tbase + (size_t)e * nthr]);
-            if (pk) {
-#pragma unroll
-                for (int e = 0; e < E; ++e) {
-                    const int ky = t + TF * e, kyn = ky == 0 ? 0 : L - ky;
-                    C ct; ct.x = pack[kyn].x; ct.y = -pack[kyn].y;
-                    w[e] = cadd(w[e], cmul(ct, P.khatB[(size_t)j * L + ky]));
-                }
-            }
-            fft_block<T, L, E, +1>(w, smc, Cc, t, P.tw, sync);
-            C *dst = P.out + (size_t)j * P.specplane;
-#pragma unroll
-            for (int e = 0; e < E; ++e) dst[tbase + (size_t)e * nthr] = w[e];
         }
     }
+    cp_async_wait<0>();
 }
 
 }  // namespace sgpk

@@ -53,6 +53,7 @@ template <typename T> struct ColParams {
     const cx<T> *tw;                  // exp(-2 pi i k / ny)
     cx<T> *pack;                      // ny entries of scratch for the packed column of tile 0
     int p;
+    int ntiles;                       // (nx/2)/C
     int check_status;
 };
 
@@ -89,6 +90,47 @@ __device__ __forceinline__ float kl_term(float g, float y)
     }
     return dy - g * log1pf(dy / g);
 }
+// Fast float path, valid for g > 0, y > 0, u^2 < 0.36 (y/g between 1/4 and 4: all but ~1e-4 of the pixels of a
+// Poisson image with a background of 10 counts or more): S(w) = (atanh(u)/u - 1)/w by a degree-7 polynomial fitted
+// on [0, 0.36] (max. relative error 9e-8 in float Horner arithmetic), u by the hardware reciprocal (1 ulp).
+__device__ __forceinline__ float kl_series(float g, float y, bool &ok)
+{
+    const float dy = y - g;
+    float r;
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(y + g));
+    const float u = dy * r;
+    const float w = u * u;
+    ok = (g > 0.f) && (y > 0.f) && (w < 0.36f);
+    float S = fmaf(w, 2.629362187e-01f, -8.657711682e-02f);
+    S = fmaf(w, S, 1.295689961e-01f);
+    S = fmaf(w, S, 8.138694077e-02f);
+    S = fmaf(w, S, 1.120216455e-01f);
+    S = fmaf(w, S, 1.428151035e-01f);
+    S = fmaf(w, S, 2.000007303e-01f);
+    S = fmaf(w, S, 3.333333313e-01f);
+    return u * fmaf(-2.f * g * w, S, dy);
+}
+// sum of kl_term over the pixels of a quad selected by s[]: straight-line code for the common case (so that the
+// compiler interleaves the four dependency chains), the general kl_term only where a pixel needs it
+__device__ __forceinline__ float kl_quad(const float (&g)[4], const float (&y)[4], const bool (&s)[4])
+{
+    float k[4]; bool ok[4];
+#pragma unroll
+    for (int c = 0; c < 4; ++c) k[c] = kl_series(g[c], y[c], ok[c]);
+    if (!((ok[0] || !s[0]) && (ok[1] || !s[1]) && (ok[2] || !s[2]) && (ok[3] || !s[3]))) {
+#pragma unroll
+        for (int c = 0; c < 4; ++c) if (s[c] && !ok[c]) k[c] = kl_term(g[c], y[c]);
+    }
+    return ((s[0] ? k[0] : 0.f) + (s[1] ? k[1] : 0.f)) + ((s[2] ? k[2] : 0.f) + (s[3] ? k[3] : 0.f));
+}
+__device__ __forceinline__ double kl_quad(const double (&g)[4], const double (&y)[4], const bool (&s)[4])
+{
+    double r = 0.0;
+#pragma unroll
+    for (int c = 0; c < 4; ++c) if (s[c]) r += kl_term(g[c], y[c]);
+    return r;
+}
+
 // ratio g/(Af+b) of Eq.1/11; 0 where the denominator is <= 0 (A17)
 template <typename T> __device__ __forceinline__ T ratio_term(T g, T y) { return (y > (T)0) ? g / y : (T)0; }
 template <typename T> __device__ __forceinline__ T clipT(T f, T L1, T L2) { return fmin(L2, fmax(L1, f)); }
@@ -107,6 +149,20 @@ __device__ __forceinline__ void weights(const Geom &G, const T *alphaR, size_t i
         r0 = a2.x > (T)0; r1 = a2.y > (T)0;
         w2.x = r0 ? (T)1 / a2.x : (T)0; w2.y = r1 ? (T)1 / a2.y : (T)0;
     }
+}
+
+// Programmatic dependent launch (sm_90+): pdl_trigger lets the next kernel of the stream be scheduled once every CTA
+// of this one has started, so that its CTAs fill the SMs as ours drain; pdl_wait blocks until the previous kernel
+// has completed and its writes are visible.  Both are no-ops in a launch without the attribute.
+__device__ __forceinline__ void pdl_trigger() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+
+__device__ __forceinline__ void prefetch_l2(const void *p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
+// start one row of a plane (len reals) on its way to L2; called by the TF threads of the row
+template <typename T> __device__ __forceinline__ void prefetch_row_l2(const T *row, int len, int t, int TF)
+{
+    constexpr int per_line = 128 / (int)sizeof(T);
+    for (int i = t * per_line; i < len; i += TF * per_line) prefetch_l2(row + i);
 }
 
 // division that may be 2 ulp off in float (no slow path, no branch); exact in double

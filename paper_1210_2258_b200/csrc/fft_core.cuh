@@ -269,6 +269,28 @@ __host__ __device__ constexpr int plan_radix(int L, int E, int ip)
 }
 __host__ __device__ constexpr bool plan_ok(int L, int E) { return plan_radix(L, E, 0) != 0; }
 
+// Twiddle tables.  Pass ip >= 1 of a plan (NS = product of the earlier radices, R = its radix) multiplies input r of
+// butterfly j by exp(-2 pi i r (j mod NS) / (NS R)).  The table of a pass is stored as [r-1][j mod NS], so that the
+// threads of a warp (consecutive j) read consecutive entries; the tables of the passes follow each other.
+__host__ __device__ constexpr int plan_ns(int L, int E, int ip)
+{
+    int ns = 1;
+    for (int i = 0; i < ip; ++i) ns *= plan_radix(L, E, i);
+    return ns;
+}
+__host__ __device__ constexpr int tw_offset(int L, int E, int ip)      // start of the table of pass ip (ip >= 1)
+{
+    int off = 0;
+    for (int i = 1; i < ip; ++i) off += (plan_radix(L, E, i) - 1) * plan_ns(L, E, i);
+    return off;
+}
+__host__ __device__ constexpr int tw_total(int L, int E)
+{
+    int ip = 1;
+    while (plan_radix(L, E, ip) != 0) ++ip;
+    return tw_offset(L, E, ip) > 0 ? tw_offset(L, E, ip) : 1;
+}
+
 // shared-memory index padding: one extra slot every 2^PS elements (PS = 5 when the first pass is radix 32,
 // else 4) turns the stride-R stores of the first pass into an odd stride, and keeps the reversed reads of the
 // real<->complex untangling spread over the banks
@@ -292,7 +314,7 @@ template <int TF> struct SyncGroup {
 
 // All passes of one FFT.  sm points at element 0 of this FFT's shared-memory line; consecutive
 // elements are `cs` apart (1 for a row FFT; C for a column FFT stored as [element][column]).
-// tw[k] = exp(-2 pi i k / L).  Every exchange is bracketed sync / store / sync / load, so shared memory
+// tw = the per-pass twiddle tables of this plan (see above).  Every exchange is bracketed sync / store / sync / load, so shared memory
 // the caller used before the call is safe to reuse, and on return nobody is writing it.
 template <typename T, int L, int E, int DIR, int IP, int NS, typename SYNC>
 __device__ __forceinline__ void fft_passes(cx<T> (&v)[E], cx<T> *__restrict__ sm, const int cs, const int t,
@@ -313,10 +335,10 @@ __device__ __forceinline__ void fft_passes(cx<T> (&v)[E], cx<T> *__restrict__ sm
         const int j = t + b * TF;
         if constexpr (NS > 1) {
             const int jm = j % NS;                       // NS is a compile-time constant
-            const int m = jm * (L / (NS * R));
+            const C *twp = tw + tw_offset(L, E, IP) + jm;
 #pragma unroll
             for (int r = 1; r < R; ++r) {
-                C w = __ldg(&tw[r * m]);
+                C w = __ldg(&twp[(r - 1) * NS]);
                 a[r] = (DIR < 0) ? cmul(a[r], w) : cmulc(a[r], w);
             }
             j0s[b] = (j / NS) * (NS * R) + jm;

@@ -3,6 +3,7 @@
 // virtual interface used by the C ABI (api.cu).
 #pragma once
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <cmath>
 #include <string>

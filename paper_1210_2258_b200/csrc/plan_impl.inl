@@ -7,7 +7,8 @@ template <typename T> struct PlanImpl : PlanBase {
     using C = cx<T>;
     size_t n = 0, nspec = 0;       // reals per plane, complex numbers per half spectrum (= n/2)
     int Lr = 0, Lc = 0;            // FFT lengths: nx/2 (rows), ny (columns)
-    int row_threads = 0, col_threads = 0, nrb = 0, ntiles = 0, bt_grid = 0;
+    bool use_pdl = true;
+    int row_threads = 0, col_threads = 0, nrb = 0, ntiles = 0, bt_grid = 0, nsm = 0, col_grid = 0;
     size_t row_smem = 0, col_smem = 0;
     row_kernel_t<T> k_rowf[RF_NMODES] = {nullptr}, k_rowi[RI_NMODES] = {nullptr};
     col_kernel_t<T> k_colf = nullptr, k_conj = nullptr, k_mult = nullptr;
@@ -89,6 +90,7 @@ template <typename T> struct PlanImpl : PlanBase {
     int init() override
     {
         n = (size_t)ny * nx; nspec = n / 2;
+        use_pdl = getenv("SGP_PDL") != nullptr;      // measured: no gain on B200 at 2048^2 (profiles/), off by default
         Lr = nx / 2; Lc = ny;
         constexpr int dummy = 0; (void)dummy;
         const int Er = fft_E<T>(Lr), Ec = fft_E_col<T>(Lc);
@@ -105,7 +107,7 @@ template <typename T> struct PlanImpl : PlanBase {
         col_threads = Cc * (Lc / Ec);
         nrb = ny / RB; ntiles = Lr / Cc;
         row_smem = (size_t)RB * fft_padded_len(Lr, Er) * sizeof(C);
-        col_smem = (size_t)Cc * fft_padded_len(Lc, Ec) * sizeof(C);
+        col_smem = ((size_t)Cc * fft_padded_len(Lc, Ec) + 2 * (size_t)Cc * Lc) * sizeof(C);
         if (row_threads > 256 || col_threads > 512 || row_smem > 227 * 1024 || col_smem > 227 * 1024) return SGP_ERR_ARG;
         for (int m = 0; m < RF_NMODES; ++m)
             SGP_CUDA_TRY(cudaFuncSetAttribute((const void *)k_rowf[m], cudaFuncAttributeMaxDynamicSharedMemorySize, (int)row_smem));
@@ -115,33 +117,48 @@ template <typename T> struct PlanImpl : PlanBase {
         SGP_CUDA_TRY(cudaFuncSetAttribute((const void *)k_conj, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)col_smem));
         SGP_CUDA_TRY(cudaFuncSetAttribute((const void *)k_mult, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)col_smem));
         // cooperative grid of the backtracking kernel
-        int dev = 0, nsm = 0, per_sm = 0;
+        int dev = 0, per_sm = 0;
         SGP_CUDA_TRY(cudaGetDevice(&dev));
         SGP_CUDA_TRY(cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev));
         SGP_CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, backtrack_kernel<T>, 256, 0));
         if (per_sm < 1) return SGP_ERR_CUDA;
         if (per_sm > 8) per_sm = 8;
         bt_grid = nsm * per_sm;
+        col_grid = (opt.use_graph & 2) ? (ntiles < nsm ? ntiles : nsm) : ntiles;   // experiment switch: persistent or one tile per CTA
         size_t want = (n / vec4_of<T>::N + 255) / 256;
         if ((size_t)bt_grid > want) bt_grid = (int)(want < 1 ? 1 : want);
 
         // twiddles, computed in double on the host
         std::vector<C> h;
-        auto upload = [&](C **dst, int len, int count, bool half) -> int {
+        auto upload = [&](C **dst, int len, int count) -> int {     // exp(-2 pi i k / len), k < count
             h.resize(count);
             for (int k = 0; k < count; ++k) {
                 double a = -2.0 * M_PI * (double)k / (double)len;
                 h[k].x = (T)cos(a); h[k].y = (T)sin(a);
             }
-            (void)half;
             int r = dalloc(dst, (size_t)count);
             if (r) return r;
             SGP_CUDA_TRY(cudaMemcpy(*dst, h.data(), sizeof(C) * count, cudaMemcpyHostToDevice));
             return SGP_OK;
         };
-        if ((rc = upload(&tw_r, Lr, Lr, false))) return rc;
-        if ((rc = upload(&tw_h, nx, Lr + 1, true))) return rc;
-        if ((rc = upload(&tw_c, Lc, Lc, false))) return rc;
+        auto upload_passes = [&](C **dst, int Lf, int Ef) -> int {  // per-pass tables [r-1][j mod NS] (fft_core.cuh)
+            h.assign((size_t)tw_total(Lf, Ef), C{(T)1, (T)0});
+            for (int ip = 1; plan_radix(Lf, Ef, ip) != 0; ++ip) {
+                const int R = plan_radix(Lf, Ef, ip), NS = plan_ns(Lf, Ef, ip), off = tw_offset(Lf, Ef, ip);
+                for (int r = 1; r < R; ++r)
+                    for (int jm = 0; jm < NS; ++jm) {
+                        double a = -2.0 * M_PI * (double)r * (double)jm / ((double)NS * (double)R);
+                        h[off + (r - 1) * NS + jm].x = (T)cos(a); h[off + (r - 1) * NS + jm].y = (T)sin(a);
+                    }
+            }
+            int r = dalloc(dst, h.size());
+            if (r) return r;
+            SGP_CUDA_TRY(cudaMemcpy(*dst, h.data(), sizeof(C) * h.size(), cudaMemcpyHostToDevice));
+            return SGP_OK;
+        };
+        if ((rc = upload_passes(&tw_r, Lr, Er))) return rc;
+        if ((rc = upload(&tw_h, nx, Lr + 1))) return rc;
+        if ((rc = upload_passes(&tw_c, Lc, Ec))) return rc;
         if ((rc = dalloc(&pack, (size_t)ny))) return rc;
         if ((rc = dalloc(&khat, nspec * p))) return rc;
         if ((rc = dalloc(&khatB, (size_t)ny * p))) return rc;
@@ -182,29 +199,38 @@ template <typename T> struct PlanImpl : PlanBase {
         P.tw = tw_r; P.twh = tw_h; P.alphaR = alphaR;
         return P;
     }
-    int launch_row(row_kernel_t<T> k, const RowParams<T> &P, int images, cudaStream_t st)
+    // launch with programmatic stream serialisation: the kernel may be scheduled while its predecessor drains and
+    // waits for it in pdl_wait() (ew.cuh)
+    template <typename K, typename PT>
+    int launch_pdl(K k, dim3 grid, int threads, size_t smem, const PT &P, cudaStream_t st)
     {
         ProfScope ps(this, st);
-        k<<<dim3(nrb, images), row_threads, row_smem, st>>>(P);
+        cudaLaunchConfig_t cfg;
+        memset(&cfg, 0, sizeof(cfg));
+        cfg.gridDim = grid; cfg.blockDim = dim3(threads); cfg.dynamicSmemBytes = smem; cfg.stream = st;
+        cudaLaunchAttribute at[1];
+        at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+        at[0].val.programmaticStreamSerializationAllowed = 1;
+        cfg.attrs = at; cfg.numAttrs = use_pdl ? 1 : 0;
+        SGP_CUDA_TRY(cudaLaunchKernelEx(&cfg, k, P));
         launches++;
-        SGP_CUDA_TRY(cudaGetLastError());
         return SGP_OK;
+    }
+    int launch_row(row_kernel_t<T> k, const RowParams<T> &P, int images, cudaStream_t st)
+    {
+        return launch_pdl(k, dim3(nrb, images), row_threads, row_smem, P, st);
     }
     ColParams<T> col_params() const
     {
         ColParams<T> P;
         memset(&P, 0, sizeof(P));
         P.G = G; P.ct = ct; P.in = spec; P.out = spec; P.khat = khat; P.khatB = khatB;
-        P.specplane = nspec; P.tw = tw_c; P.pack = pack; P.p = p;
+        P.specplane = nspec; P.tw = tw_c; P.pack = pack; P.p = p; P.ntiles = ntiles;
         return P;
     }
     int launch_col(col_kernel_t<T> k, const ColParams<T> &P, cudaStream_t st)
     {
-        ProfScope ps(this, st);
-        k<<<ntiles, col_threads, col_smem, st>>>(P);
-        launches++;
-        SGP_CUDA_TRY(cudaGetLastError());
-        return SGP_OK;
+        return launch_pdl(k, dim3(col_grid), col_threads, col_smem, P, st);
     }
     static int ew_grid(size_t count) { size_t b = (count + 255) / 256; return (int)(b > 1184 ? 1184 : (b < 1 ? 1 : b)); }
 

@@ -91,7 +91,7 @@ __device__ __forceinline__ void epi_grad(const RowParams<T> &P, const T *wrow, i
 
 // RI_LS (a8 tail + a9): u_j = A_j d on S; J(1) = sum kl(g_j, q_j + u_j + b_j).
 // RI_QJ: q_j = A_j f on S; J0(f) = sum kl(g_j, q_j + b_j) (Eq.2/12 over S, A12); QJ_PLAIN only stores.
-template <typename T, int L, int TF, bool WITH_Q>
+template <typename T, int L, int TF, bool WITH_Q, bool MASKED>
 __device__ __forceinline__ void epi_kl(const RowParams<T> &P, const T *wrow, int t, int y, int j, size_t base, bool plain, double (&acc)[1])
 {
     const Geom &G = P.G;
@@ -115,23 +115,21 @@ __device__ __forceinline__ void epi_kl(const RowParams<T> &P, const T *wrow, int
 #pragma unroll
         for (int u = 0; u < U; ++u) {
             const int x = 4 * (t + TF * (it0 + u));
-            bool s[4];
-            quad_in_S<T>(G, rowin, x, s);
+            bool s[4] = {true, true, true, true};      // without a boundary mask S is the whole grid
+            if constexpr (MASKED) quad_in_S<T>(G, rowin, x, s);
             Quad<T> u4;
 #pragma unroll
             for (int c = 0; c < 4; ++c) u4.a[c] = s[c] ? w4[u].a[c] : (T)0;
             stq<T>(P.out0 + base + x, u4);
             if (need) {
-                T ksum = (T)0;
+                T yv[4];
 #pragma unroll
                 for (int c = 0; c < 4; ++c) {
-                    T yv = u4.a[c];
-                    if constexpr (WITH_Q) yv += q4[u].a[c];
-                    const T bv = P.b_is_array ? b4[u].a[c] : bc;
-                    const T kv = kl_term(g4[u].a[c], (T)(yv + bv));
-                    ksum += s[c] ? kv : (T)0;
+                    yv[c] = u4.a[c];
+                    if constexpr (WITH_Q) yv[c] += q4[u].a[c];
+                    yv[c] += P.b_is_array ? b4[u].a[c] : bc;
                 }
-                acc[0] += (double)ksum;
+                acc[0] += (double)kl_quad(g4[u].a, yv, s);
             }
         }
     }

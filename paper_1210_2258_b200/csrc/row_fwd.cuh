@@ -37,6 +37,8 @@ __global__ void __launch_bounds__(256, 2) row_fwd_kernel(const RowParams<T> P)
     constexpr int RS = fft_padded_len(L, E);
     extern __shared__ __align__(16) unsigned char smem_raw[];
     C *sm = reinterpret_cast<C *>(smem_raw);
+    pdl_trigger();
+    pdl_wait();
     if (P.check_status && P.ct->status != 0) return;
 
     const Geom &G = P.G;

@@ -28,6 +28,8 @@ __global__ void __launch_bounds__(256, 2) row_inv_kernel(const RowParams<T> P)
     extern __shared__ __align__(16) unsigned char smem_raw[];
     __shared__ double red[kNQ * 32];
     C *sm = reinterpret_cast<C *>(smem_raw);
+    pdl_trigger();
+    pdl_wait();
     if (P.check_status && P.ct->status != 0) return;
 
     const Geom &G = P.G;
@@ -38,7 +40,6 @@ __global__ void __launch_bounds__(256, 2) row_inv_kernel(const RowParams<T> P)
     constexpr int nx = 2 * L;
     C *smrow = sm + row * RS;
     const SyncGroup<TF> sync{1 + row};
-
     // ---- tile-major spectrum -> re-tangled Z in shared memory, one (k, L-k) pair per step, k = t + TF i;
     //      Z[0] = (X0 + XL) + i (X0 - XL);  Z[L/2] = 2 conj X[L/2]
     {
@@ -142,7 +143,8 @@ __global__ void __launch_bounds__(256, 2) row_inv_kernel(const RowParams<T> P)
     } else if constexpr (MODE == RI_LS || MODE == RI_QJ) {
         const bool plain = (MODE == RI_QJ) && P.submode == QJ_PLAIN;
         double acc[1] = {0.0};
-        epi_kl<T, L, TF, MODE == RI_LS>(P, wrow, t, y, j, base, plain, acc);
+        if (G.masked) epi_kl<T, L, TF, MODE == RI_LS, true>(P, wrow, t, y, j, base, plain, acc);
+        else          epi_kl<T, L, TF, MODE == RI_LS, false>(P, wrow, t, y, j, base, plain, acc);
         if (plain) return;
         block_reduce_sum<1>(acc, red);
         const int tk = (MODE == RI_LS) ? TK_LS : TK_QJ;
