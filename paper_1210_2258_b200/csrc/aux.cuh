@@ -6,10 +6,12 @@
 namespace sgpk {
 
 // ---------------------------------------------------------------- a9 (backtracks) + a11
-// Cooperative kernel (all CTAs resident), launched every iteration; returns at once when lambda = 1 was accepted by
-// the RI_LS epilogue (the usual case).  Otherwise the Armijo loop lambda <- theta lambda runs
-// here: every trial is one elementwise pass over q_j + lambda u_j (no FFT), one grid-wide barrier, and the same
-// decision taken redundantly by every CTA.  The accepted step is NOT applied here: f + lambda d and q_j + lambda u_j
+// Launched every iteration; returns at once when lambda = 1 was accepted by the RI_LS epilogue (the usual case).
+// Otherwise the Armijo loop lambda <- theta lambda runs here: every trial is one elementwise
+// pass over q_j + lambda u_j (no FFT), one grid-wide barrier, and the same decision taken redundantly by every
+// CTA.  The grid is sized by the occupancy API so that all CTAs are resident together, and the barrier is a
+// sense-reversing counter in the control block: an ordinary launch, because the empty cooperative launches of the
+// usual case cost 7 us per iteration.  The accepted step is NOT applied here: f + lambda d and q_j + lambda u_j
 // are formed by the next iteration's kernels (lazy update) or by final_update_kernel.
 template <typename T> struct BtParams {
     Geom G;
@@ -26,6 +28,25 @@ template <typename T> struct BtParams {
 template <typename T> struct vec4_of;
 template <> struct vec4_of<float>  { using type = float4;  static constexpr int N = 4; };
 template <> struct vec4_of<double> { using type = double2; static constexpr int N = 2; };
+
+// all CTAs of the grid (resident together) meet here; bar[0] = arrival count, bar[1] = generation
+__device__ __forceinline__ void grid_barrier(unsigned int *bar)
+{
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        const unsigned int gen = atomicAdd(&bar[1], 0u);
+        __threadfence();
+        if (atomicAdd(&bar[0], 1u) == gridDim.x - 1) {
+            atomicExch(&bar[0], 0u);
+            __threadfence();
+            atomicAdd(&bar[1], 1u);
+        } else {
+            while (atomicAdd(&bar[1], 0u) == gen) __nanosleep(64);
+        }
+        __threadfence();
+    }
+    __syncthreads();
+}
 
 template <typename T>
 __global__ void __launch_bounds__(256) backtrack_kernel(const BtParams<T> P)
@@ -47,10 +68,10 @@ __global__ void __launch_bounds__(256) backtrack_kernel(const BtParams<T> P)
         const double fl = P.tr.force_lambda[k];
         if (isfinite(fl)) { forced = true; lambda = fl / P.o.theta; }
     }
+    grid_barrier(&ct->counter[6]);                             // every CTA has read the control block
     int nbt = 0;
     while (!accepted) {
         if (!forced && nbt >= P.o.max_backtracks) {            // A16
-            cg::this_grid().sync();                            // every CTA has read ct->status == 0 above
             if (blockIdx.x == 0 && threadIdx.x == 0) ct->status = SGP_ERR_LINESEARCH;
             return;
         }
@@ -79,8 +100,7 @@ __global__ void __launch_bounds__(256) backtrack_kernel(const BtParams<T> P)
         }
         block_reduce_sum<1>(acc, red);
         if (threadIdx.x == 0) P.part[blockIdx.x] = acc[0];
-        __threadfence();
-        cg::this_grid().sync();
+        grid_barrier(&ct->counter[6]);
         double tot[1] = {0.0};
         for (unsigned int bI = threadIdx.x; bI < gridDim.x; bI += blockDim.x) tot[0] += __ldcg(&P.part[bI]);
         block_reduce_sum<1>(tot, red);
@@ -88,7 +108,7 @@ __global__ void __launch_bounds__(256) backtrack_kernel(const BtParams<T> P)
         __syncthreads();
         Jnew = s_J;
         accepted = forced || (isfinite(Jnew) && Jnew <= Jref + P.o.beta * lambda * gd);
-        cg::this_grid().sync();     // partials may be overwritten by the next trial
+        grid_barrier(&ct->counter[6]);     // partials may be overwritten by the next trial
     }
     if (forced) nbt = 0;
     // ---- book-keeping by the last CTA to finish (every CTA has read the control block by now)

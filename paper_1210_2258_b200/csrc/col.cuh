@@ -102,8 +102,9 @@ __global__ void __launch_bounds__(fft_E_col<T>(L) == 32 ? 256 : 512, 1) col_kern
     // the transfer function does not depend on the previous kernel: its first tile is on its way before we wait
     X.fetch(X.bufB, P.khat + X.tile_of(0)); cp_async_commit();
     pdl_wait();
-    if (P.check_status && P.ct->status != 0) { cp_async_wait<0>(); return; }
+    const int stop = P.check_status ? P.ct->status : 0;      // tested after the copies have been issued
     X.fetch(X.bufA, P.in + X.tile_of(0)); cp_async_commit();
+    if (stop != 0) { cp_async_wait<0>(); return; }
 
     if constexpr (MODE == CM_CONJSUM) {
         // unit of work u = it*p + j: spectrum and transfer function of image j on this CTA's it-th tile.

@@ -116,13 +116,13 @@ template <typename T> struct PlanImpl : PlanBase {
         SGP_CUDA_TRY(cudaFuncSetAttribute((const void *)k_colf, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)col_smem));
         SGP_CUDA_TRY(cudaFuncSetAttribute((const void *)k_conj, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)col_smem));
         SGP_CUDA_TRY(cudaFuncSetAttribute((const void *)k_mult, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)col_smem));
-        // cooperative grid of the backtracking kernel
+        // grid of the backtracking kernel: all CTAs resident together (it synchronises grid-wide, aux.cuh)
         int dev = 0, per_sm = 0;
         SGP_CUDA_TRY(cudaGetDevice(&dev));
         SGP_CUDA_TRY(cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev));
         SGP_CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, backtrack_kernel<T>, 256, 0));
         if (per_sm < 1) return SGP_ERR_CUDA;
-        if (per_sm > 8) per_sm = 8;
+        if (per_sm > 4) per_sm = 4;
         bt_grid = nsm * per_sm;
         col_grid = (opt.use_graph & 2) ? (ntiles < nsm ? ntiles : nsm) : ntiles;   // experiment switch: persistent or one tile per CTA
         size_t want = (n / vec4_of<T>::N + 255) / 256;

@@ -85,10 +85,10 @@ int PlanImpl<T>::enqueue_sgp_iteration(const RowParams<T> &Pb, const DevOpts &o,
         U.G = G; U.o = o; U.tr = tr; U.ct = ct; U.q = q; U.u = u; U.g = Gp; U.b = Bp;
         U.plane = n; U.b_is_array = b_is_array; U.part = part_bt;
         for (int j = 0; j < p; ++j) U.bconst[j] = bconst[j];
-        void *args[] = {(void *)&U};
         ProfScope ps(this, st);
-        SGP_CUDA_TRY(cudaLaunchCooperativeKernel((const void *)backtrack_kernel<T>, dim3(bt_grid), dim3(256), args, 0, st));
+        backtrack_kernel<T><<<bt_grid, 256, 0, st>>>(U);
         launches++;
+        SGP_CUDA_TRY(cudaGetLastError());
     }
     cur_slot = -1;
     return SGP_OK;

@@ -39,7 +39,8 @@ __global__ void __launch_bounds__(256, 2) row_fwd_kernel(const RowParams<T> P)
     C *sm = reinterpret_cast<C *>(smem_raw);
     pdl_trigger();
     pdl_wait();
-    if (P.check_status && P.ct->status != 0) return;
+    // the stop flag is tested only before the first store, so that its load overlaps the loads of the row
+    const int stop = P.check_status ? P.ct->status : 0;
 
     const Geom &G = P.G;
     const int tid = threadIdx.x;
@@ -112,6 +113,7 @@ __global__ void __launch_bounds__(256, 2) row_fwd_kernel(const RowParams<T> P)
                     b2[u] = P.b_is_array ? ld2<T>(P.in2 + base + x0) : mk<T>(bc, bc);
                 }
             }
+            if (e0 == 0 && stop != 0) return;
 #pragma unroll
             for (int u = 0; u < U; ++u) {
                 const int x0 = 2 * (t + TF * (e0 + u));
@@ -144,6 +146,7 @@ __global__ void __launch_bounds__(256, 2) row_fwd_kernel(const RowParams<T> P)
                 g2[u] = ld2<T>(P.in1 + base + x0);
                 if (G.masked) a2[u] = ld2<T>(P.alphaR + base + x0);
             }
+            if (e0 == 0 && stop != 0) return;
 #pragma unroll
             for (int u = 0; u < U; ++u) {
                 const int x0 = 2 * (t + TF * (e0 + u));
@@ -175,6 +178,7 @@ __global__ void __launch_bounds__(256, 2) row_fwd_kernel(const RowParams<T> P)
         acc[0] += (double)accf;
     }
 
+    if (stop != 0) return;
     // ---- complex FFT of length L = nx/2 over z[m] = x[2m] + i x[2m+1]
     C *smrow = sm + row * RS;
     const SyncGroup<TF> sync{1 + row};

@@ -30,7 +30,8 @@ __global__ void __launch_bounds__(256, 2) row_inv_kernel(const RowParams<T> P)
     C *sm = reinterpret_cast<C *>(smem_raw);
     pdl_trigger();
     pdl_wait();
-    if (P.check_status && P.ct->status != 0) return;
+    // the stop flag is tested only after the loads of the spectrum have been issued (all stores come later)
+    const int stop = P.check_status ? P.ct->status : 0;
 
     const Geom &G = P.G;
     const int tid = threadIdx.x;
@@ -81,6 +82,7 @@ __global__ void __launch_bounds__(256, 2) row_inv_kernel(const RowParams<T> P)
             }
         }
     }
+    if (stop != 0) return;
     sync();
     {
         C v[E];
