@@ -60,13 +60,16 @@ def load_peaks():
     return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
 
 
-def planes_per_launch(p: int, b_array: bool, masked: bool):
-    """algorithmic planes (n reals each) read + written per launch, SURVEY.md 8(d) schedule A / DESIGN.md section 6"""
+def planes_per_launch(p: int, b_array: bool, masked: bool, backtracks_per_iter: float = 0.0):
+    """algorithmic planes (n reals each) read + written per launch of the kernels as built, DESIGN.md section 6.
+    K1 = g, q, u read; q, spectrum written (lazy a10 for q).  K3 = spectrum, f, d, grad read; f, grad written (lazy a10
+    for f).  K7 = q, u, g read once per Armijo trial (average over the launches of the run)."""
     ba = p if b_array else 0
     m = 1 if masked else 0
     return {
-        "K1_ratio_rowfft": 3 * p + ba, "K2_col_conjsum": 2 * p + 1, "K3_rowifft_grad_bb": 5 + m,
-        "K4_project_rowfft": 4 + m, "K5_col_mult": 2 * p + 1, "K6_rowifft_linesearch": 4 * p + ba, "K7_update": 3 + 3 * p,
+        "K1_ratio_rowfft": 5 * p + ba, "K2_col_conjsum": 2 * p + 1, "K3_rowifft_grad_bb": 6 + m,
+        "K4_project_rowfft": 4 + m, "K5_col_mult": 2 * p + 1, "K6_rowifft_linesearch": 4 * p + ba,
+        "K7_backtrack": (3 * p + ba) * backtracks_per_iter,
         "R1_rowfft": 2, "R2_col_mult": 2 * p + 1, "R3_rowifft_q_J": 3 * p + ba, "R4_ratio_rowfft": 3 * p + ba,
         "R5_col_conjsum": 2 * p + 1, "R6_rowifft_update": 3 + m,
     }
@@ -267,7 +270,8 @@ def run_ours(args):
     rp = step()
     kms = plan.kernel_ms()
     plan.set_profiling(False)
-    planes = planes_per_launch(p, False, w["S"] is not None)
+    bt_per_iter = rp.total_backtracks / max(1, rp.iterations)
+    planes = planes_per_launch(p, False, w["S"] is not None, bt_per_iter)
     plane_bytes = ny * nx * esz
     peak, peak_src = load_peaks()
     per_kernel = {}
@@ -275,7 +279,7 @@ def run_ours(args):
     for name, (msum, cnt) in kms.items():
         avg_us = 1e3 * msum / cnt
         gbs = planes[name] * plane_bytes / (avg_us * 1e-6) / 1e9
-        per_kernel[name] = {"avg_us": round(avg_us, 2), "launches": cnt, "planes": planes[name], "GBps": round(gbs, 1),
+        per_kernel[name] = {"avg_us": round(avg_us, 2), "launches": cnt, "planes": round(planes[name], 3), "GBps": round(gbs, 1),
                             "frac": round(gbs / peak, 4), "share": round(msum / tot_ms, 4)}
     dom = max(kms, key=lambda k: kms[k][0])
     traffic = None
@@ -285,8 +289,10 @@ def run_ours(args):
             traffic = json.loads(tf.read_text()).get(f"{args.workload}:{args.dtype}:{args.alg}", {}).get(dom)
         except Exception:
             traffic = None
+    # schedule A (14p + 14 planes, the primary denominator); the kernels as built move 13p + 12
     iter_planes = (14 * p + 14 + (2 if w["S"] is not None else 0)) if args.alg == "sgp" else (
         sum(planes[k] for k in planes if k.startswith("R")))
+    built_planes = sum(planes[k] for k in planes if k.startswith("K" if args.alg == "sgp" else "R"))
     it_us = 1e3 * (loop_ms / args.steps) / iters          # loop only (library's own events), local rank
     it_gbs = iter_planes * plane_bytes / (it_us * 1e-6) / 1e9
     roofline = {"bound": "hbm", "kernel": dom, "achieved": per_kernel[dom]["GBps"], "peak": peak, "unit": "GB/s",
@@ -294,6 +300,8 @@ def run_ours(args):
                 "algorithmic_bytes_per_launch": planes[dom] * plane_bytes,
                 "iteration": {"planes": iter_planes, "bytes": iter_planes * plane_bytes, "us": round(it_us, 2),
                               "GBps": round(it_gbs, 1), "frac": round(it_gbs / peak, 4),
+                              "planes_as_built": round(built_planes, 2),
+                              "frac_as_built": round(built_planes * plane_bytes / (it_us * 1e-6) / 1e9 / peak, 4),
                               "backtracks_per_iteration": backtracks / max(1, iters * args.steps)},
                 "kernels": per_kernel}
 

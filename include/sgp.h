@@ -129,13 +129,13 @@ typedef struct sgp_plan sgp_plan;
 /* Kernel slots of the per-kernel timing (sgp_plan_set_profiling).  One SGP iteration is the seven launches
  * K1..K7 (SURVEY.md 8(d) schedule A), one RL round the six launches R1..R6. */
 typedef enum {
-    SGP_PROF_K1 = 0,  /* a1: ratio g/(Af+b) fused into the forward row FFT, p images                          */
+    SGP_PROF_K1 = 0,  /* a10(q)+a1: lazy q_j += lambda u_j, ratio g/(Af+b) fused into the forward row FFT, p images */
     SGP_PROF_K2 = 1,  /* a2: column FFT -> sum_j conj(K^_j) x -> inverse column FFT                            */
-    SGP_PROF_K3 = 2,  /* a3+a5+a6: inverse row FFT -> gradient, BB dot products, step length                   */
+    SGP_PROF_K3 = 2,  /* a10(f)+a3+a5+a6: inverse row FFT -> lazy f += lambda d, gradient, BB sums, step length  */
     SGP_PROF_K4 = 3,  /* a4+a7: scaling, projection, d, grad'd fused into the forward row FFT of d             */
     SGP_PROF_K5 = 4,  /* a8: column FFT -> x K^_j -> p inverse column FFTs                                      */
-    SGP_PROF_K6 = 5,  /* a8+a9: inverse row FFTs -> u_j = A_j d, J(lambda = 1), Armijo test                     */
-    SGP_PROF_K7 = 6,  /* a9 backtracks + a10 update + a11 stopping rules                                        */
+    SGP_PROF_K6 = 5,  /* a8+a9+a11: inverse row FFTs -> u_j = A_j d, J(lambda = 1), Armijo test, book-keeping    */
+    SGP_PROF_K7 = 6,  /* a9 backtracks (elementwise; returns at once when lambda = 1 was accepted)                */
     SGP_PROF_R1 = 7,  /* RL: forward row FFT of f                                                               */
     SGP_PROF_R2 = 8,  /* RL: column pass x K^_j                                                                 */
     SGP_PROF_R3 = 9,  /* RL: inverse row FFTs -> q_j = A_j f, J0(f), stopping rules                             */

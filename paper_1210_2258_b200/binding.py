@@ -33,7 +33,7 @@ EXPORTS = [
     "sgp_plan_rfft2", "sgp_plan_irfft2", "sgp_plan_set_profiling", "sgp_plan_get_kernel_ms", "sgp_plan_destroy",
 ]
 PROF_SLOTS = ["K1_ratio_rowfft", "K2_col_conjsum", "K3_rowifft_grad_bb", "K4_project_rowfft", "K5_col_mult", "K6_rowifft_linesearch",
-              "K7_update", "R1_rowfft", "R2_col_mult", "R3_rowifft_q_J", "R4_ratio_rowfft", "R5_col_conjsum", "R6_rowifft_update"]
+              "K7_backtrack", "R1_rowfft", "R2_col_mult", "R3_rowifft_q_J", "R4_ratio_rowfft", "R5_col_conjsum", "R6_rowifft_update"]
 
 
 class Options(C.Structure):
