@@ -282,11 +282,14 @@ def run_ours(args):
         per_kernel[name] = {"avg_us": round(avg_us, 2), "launches": cnt, "planes": round(planes[name], 3), "GBps": round(gbs, 1),
                             "frac": round(gbs / peak, 4), "share": round(msum / tot_ms, 4)}
     dom = max(kms, key=lambda k: kms[k][0])
-    traffic = None
-    tf = ROOT / "profiles" / "traffic.json"
+    traffic = None          # DRAM read + write bytes of that kernel per launch, ncu --set full (profiles/traffic.md)
+    tf = ROOT / "profiles" / "traffic.csv"
     if tf.exists():
         try:
-            traffic = json.loads(tf.read_text()).get(f"{args.workload}:{args.dtype}:{args.alg}", {}).get(dom)
+            for line in tf.read_text().splitlines()[1:]:
+                wl, dt_, alg_, kern, nbytes = [c.strip() for c in line.split(",")]
+                if (wl, dt_, alg_, kern) == (args.workload, args.dtype, args.alg, dom):
+                    traffic = float(nbytes)
         except Exception:
             traffic = None
     # schedule A (14p + 14 planes, the primary denominator); the kernels as built move 13p + 12

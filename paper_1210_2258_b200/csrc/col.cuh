@@ -4,8 +4,8 @@
 // spectrum never leaves the registers between the three steps.
 //
 // The kernel is PERSISTENT: grid = min(tiles, SMs), CTA b works on tiles b, b + grid, ...; the spectrum and the
-// transfer-function tile of the next unit of work are copied global -> shared with cp.async while the current
-// one is transformed, so the only exposed load is the first.  block = C * (L/E) threads (thread = (t, c), c
+// transfer-function tile of the next unit of work are copied global -> shared by the TMA engine (cp.async.bulk)
+// while the current one is transformed, so the only exposed load is the first.  block = C * (L/E) threads (thread = (t, c), c
 // fastest: global accesses are contiguous), dynamic smem = C * padded(L) complex (exchange buffer of the FFT
 // passes) + 2 tiles (landing zones of the asynchronous copies).
 //   CM_FWD / CM_INV: out = forward / unnormalised inverse column FFT of in (set-up of the transfer functions, rfft2 helpers)
@@ -21,15 +21,27 @@ namespace sgpk {
 
 enum ColMode { CM_FWD = 0, CM_CONJSUM = 1, CM_MULT = 2, CM_INV = 3 };
 
-// asynchronous copy of one complex number global -> shared (LDGSTS), and the group bookkeeping around it
-template <typename C> __device__ __forceinline__ void cp_async_cx(C *smem_dst, const C *gmem_src)
+// Bulk asynchronous copy global -> shared by the TMA engine (cp.async.bulk, SASS UBLKCP): ONE instruction of one
+// thread moves a whole tile (contiguous in the tile-major layout); completion is signalled on an mbarrier.
+__device__ __forceinline__ unsigned int smem_u32(const void *p) { return (unsigned int)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(unsigned long long *bar, int count)
 {
-    const unsigned int s = (unsigned int)__cvta_generic_to_shared(smem_dst);
-    if constexpr (sizeof(C) == 8) asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(s), "l"(gmem_src) : "memory");
-    else                          asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(s), "l"(gmem_src) : "memory");
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
 }
-__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
-template <int N> __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
+__device__ __forceinline__ void bulk_load(void *smem_dst, const void *gmem_src, unsigned int bytes, unsigned long long *bar)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(smem_u32(smem_dst)), "l"(gmem_src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned long long *bar, unsigned int phase)
+{
+    unsigned int ok;
+    do {
+        asm volatile("{ .reg .pred p; mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2; selp.u32 %0, 1, 0, p; }"
+                     : "=r"(ok) : "r"(smem_u32(bar)), "r"(phase) : "memory");
+    } while (!ok);
+}
 
 // per-CTA view of the work: tile it of this CTA starts at tile_of(it) in a spectrum plane
 template <typename T, int L, int E> struct ColCtx {
@@ -38,13 +50,6 @@ template <typename T, int L, int E> struct ColCtx {
     size_t tile_len;
     C *smc, *bufA, *bufB;
     __device__ __forceinline__ size_t tile_of(int it) const { return (size_t)((int)blockIdx.x + it * (int)gridDim.x) * tile_len; }
-    // copies of this thread's own elements: what a thread reads back it has copied itself, so waiting for the
-    // copy group is all the synchronisation the landing zones need
-    __device__ __forceinline__ void fetch(C *buf, const C *src) const
-    {
-#pragma unroll
-        for (int e = 0; e < E; ++e) cp_async_cx<C>(buf + tid + e * nthr, src + tid + (size_t)e * nthr);
-    }
 };
 
 // product with the packed-column companion B (see the header): r[e] (+)= conj?(B) C~
@@ -99,17 +104,25 @@ __global__ void __launch_bounds__(fft_E_col<T>(L) == 32 ? 256 : 512, 1) col_kern
     const int p = MULTI ? P.p : 1;
     const int my_tiles = ((int)blockIdx.x < ntiles) ? (ntiles - 1 - (int)blockIdx.x) / (int)gridDim.x + 1 : 0;
     if (my_tiles == 0) return;
-    // the transfer function does not depend on the previous kernel: its first tile is on its way before we wait
-    X.fetch(X.bufB, P.khat + X.tile_of(0)); cp_async_commit();
+    // landing zones: bufA <- spectrum tile, bufB <- transfer-function tile, one mbarrier each.  Thread 0 issues the
+    // copies; a zone is re-filled only after a CTA barrier that follows the last read of it.
+    __shared__ unsigned long long bars[2];
+    const unsigned int tile_bytes = (unsigned int)(X.tile_len * sizeof(C));
+    unsigned int phA = 0, phB = 0;
+    if (tid == 0) {
+        mbar_init(&bars[0], 1); mbar_init(&bars[1], 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        // the transfer function does not depend on the previous kernel: it is on its way before we wait for that
+        bulk_load(X.bufB, P.khat + X.tile_of(0), tile_bytes, &bars[1]);
+    }
     pdl_wait();
-    const int stop = P.check_status ? P.ct->status : 0;      // tested after the copies have been issued
-    X.fetch(X.bufA, P.in + X.tile_of(0)); cp_async_commit();
-    if (stop != 0) { cp_async_wait<0>(); return; }
+    const int stop = P.check_status ? P.ct->status : 0;
+    if (tid == 0 && stop == 0) bulk_load(X.bufA, P.in + X.tile_of(0), tile_bytes, &bars[0]);
+    __syncthreads();                                            // barrier initialisation visible to all
+    if (stop != 0) { mbar_wait(&bars[1], 0); return; }
 
     if constexpr (MODE == CM_CONJSUM) {
-        // unit of work u = it*p + j: spectrum and transfer function of image j on this CTA's it-th tile.
-        // Copy groups are committed in the order B(0) A(0) A(1) B(1) A(2) B(2) ..., one per unit and buffer (empty at
-        // the end), so after the first unit "all but the newest group" is always the one about to be read.
+        // unit of work u = it*p + j: spectrum and transfer function of image j on this CTA's it-th tile
         const int units = my_tiles * p;
         C acc[MULTI ? E : 1];
         for (int it = 0; it < my_tiles; ++it) {
@@ -117,11 +130,13 @@ __global__ void __launch_bounds__(fft_E_col<T>(L) == 32 ? 256 : 512, 1) col_kern
             const bool pk = packed && X.c == 0;
             for (int j = 0; j < p; ++j) {
                 const int u1 = it * p + j + 1, it1 = u1 / p, j1 = u1 - it1 * p;
-                if (u1 == 1) cp_async_wait<0>(); else cp_async_wait<1>();   // spectrum of this unit has landed
+                mbar_wait(&bars[0], phA); phA ^= 1;                 // spectrum of this unit has landed
 #pragma unroll
                 for (int e = 0; e < E; ++e) v[e] = X.bufA[tid + e * nthr];
-                if (u1 < units) X.fetch(X.bufA, P.in + (size_t)j1 * P.specplane + X.tile_of(it1));
-                cp_async_commit();
+                if (u1 < units) {
+                    __syncthreads();
+                    if (tid == 0) bulk_load(X.bufA, P.in + (size_t)j1 * P.specplane + X.tile_of(it1), tile_bytes, &bars[0]);
+                }
                 fft_block<T, L, E, -1>(v, X.smc, Cc, t, P.tw, sync);
                 if (packed) {
                     if (pk) {
@@ -130,11 +145,13 @@ __global__ void __launch_bounds__(fft_E_col<T>(L) == 32 ? 256 : 512, 1) col_kern
                     }
                     __syncthreads();
                 }
-                cp_async_wait<1>();                                 // transfer function of this unit has landed
+                mbar_wait(&bars[1], phB); phB ^= 1;                 // transfer function of this unit has landed
 #pragma unroll
                 for (int e = 0; e < E; ++e) v[e] = cmulc(v[e], X.bufB[tid + e * nthr]);
-                if (u1 < units) X.fetch(X.bufB, P.khat + (size_t)j1 * P.specplane + X.tile_of(it1));
-                cp_async_commit();
+                if (u1 < units) {
+                    __syncthreads();
+                    if (tid == 0) bulk_load(X.bufB, P.khat + (size_t)j1 * P.specplane + X.tile_of(it1), tile_bytes, &bars[1]);
+                }
                 if (pk) packed_fix<T, L, E, true>(v, pack, P.khatB + (size_t)j * L, t);
                 if constexpr (MULTI) {
 #pragma unroll
@@ -151,15 +168,17 @@ __global__ void __launch_bounds__(fft_E_col<T>(L) == 32 ? 256 : 512, 1) col_kern
 #pragma unroll
             for (int e = 0; e < E; ++e) dst[(size_t)e * nthr] = v[e];
         }
-    } else {   // CM_MULT: groups B(0,0) A(0) A(1) B(0,1) .. B(0,p-1) B(1,0) A(2) ...
+    } else {   // CM_MULT
         for (int it = 0; it < my_tiles; ++it) {
             const bool packed = (blockIdx.x == 0 && it == 0);
             const bool pk = packed && X.c == 0;
-            if (it == 0) cp_async_wait<0>(); else cp_async_wait<1>();   // spectrum of tile it has landed
+            mbar_wait(&bars[0], phA); phA ^= 1;                     // spectrum of tile it has landed
 #pragma unroll
             for (int e = 0; e < E; ++e) v[e] = X.bufA[tid + e * nthr];
-            if (it + 1 < my_tiles) X.fetch(X.bufA, P.in + X.tile_of(it + 1));
-            cp_async_commit();
+            if (it + 1 < my_tiles) {
+                __syncthreads();
+                if (tid == 0) bulk_load(X.bufA, P.in + X.tile_of(it + 1), tile_bytes, &bars[0]);
+            }
             fft_block<T, L, E, -1>(v, X.smc, Cc, t, P.tw, sync);
             if (packed) {
                 if (pk) {
@@ -170,12 +189,16 @@ __global__ void __launch_bounds__(fft_E_col<T>(L) == 32 ? 256 : 512, 1) col_kern
             }
             for (int j = 0; j < p; ++j) {
                 C w[E];
-                if (j == 0) cp_async_wait<1>(); else cp_async_wait<0>();   // transfer function (it, j) has landed
+                mbar_wait(&bars[1], phB); phB ^= 1;                 // transfer function (it, j) has landed
 #pragma unroll
                 for (int e = 0; e < E; ++e) w[e] = cmul(v[e], X.bufB[tid + e * nthr]);
-                if (j + 1 < p) X.fetch(X.bufB, P.khat + (size_t)(j + 1) * P.specplane + X.tile_of(it));
-                else if (it + 1 < my_tiles) X.fetch(X.bufB, P.khat + X.tile_of(it + 1));
-                cp_async_commit();
+                if (j + 1 < p || it + 1 < my_tiles) {
+                    __syncthreads();
+                    if (tid == 0) {
+                        if (j + 1 < p) bulk_load(X.bufB, P.khat + (size_t)(j + 1) * P.specplane + X.tile_of(it), tile_bytes, &bars[1]);
+                        else           bulk_load(X.bufB, P.khat + X.tile_of(it + 1), tile_bytes, &bars[1]);
+                    }
+                }
                 if (pk) packed_fix<T, L, E, false>(w, pack, P.khatB + (size_t)j * L, t);
                 fft_block<T, L, E, +1>(w, X.smc, Cc, t, P.tw, sync);
                 C *dst = P.out + (size_t)j * P.specplane + X.tile_of(it) + tid;
@@ -184,7 +207,6 @@ __global__ void __launch_bounds__(fft_E_col<T>(L) == 32 ? 256 : 512, 1) col_kern
             }
         }
     }
-    cp_async_wait<0>();
 }
 
 }  // namespace sgpk
