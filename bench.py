@@ -221,6 +221,7 @@ def run_ours(args):
     okw = {**w["opts"], "stop_rule": 0}
     if args.tile_cols: okw["tile_cols"] = args.tile_cols
     if args.rows_per_block: okw["rows_per_block"] = args.rows_per_block
+    okw["use_graph"] = args.graph
     opts = B.default_options(**okw)
     alg = B.ALG_SGP if args.alg == "sgp" else B.ALG_RL
 
@@ -323,7 +324,7 @@ def run_ours(args):
                 return (B.sgp_single if args.alg == "sgp" else B.rl_single)(hg[0], hk[0], w["b"][0], opts=opts, host=True, f_out=hf)[1]
             return (B.sgp_multi if args.alg == "sgp" else B.rl_multi)(hg, hk, w["b"], opts=opts, host=True, f_out=hf)[1]
 
-        e2e_step()
+        e2e_step(); e2e_step()
         sync_all()
         n_e2e = max(1, min(args.steps, 5))
         t0 = time.perf_counter()
@@ -386,6 +387,7 @@ def main():
     ap.add_argument("--rows-per-block", type=int, default=0)
     ap.add_argument("--cpu-iters", type=int, default=5, help="oracle iterations timed for cpu_baseline")
     ap.add_argument("--ref-iters", type=int, default=3, help="oracle iterations per step of --impl reference")
+    ap.add_argument("--graph", type=int, default=1, help="1 = replay the iterations as CUDA graphs of 10 (default), 0 = plain launches")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     args = ap.parse_args()

@@ -100,7 +100,7 @@ typedef struct sgp_options {
     int backend;                                 /* sgp_backend */
     int tile_cols;                               /* tuning: spectrum tile width in columns (power of 2); 0 = auto */
     int rows_per_block;                          /* tuning: rows per CTA in the row-FFT kernels (power of 2); 0 = auto */
-    int use_graph;                               /* 1 = replay one iteration as a CUDA graph; 0 = plain stream launches */
+    int use_graph;                               /* 1 (default) = replay the iterations as CUDA graphs of 10; 0 = plain stream launches */
 } sgp_options;
 
 /* Result of a run.  The trace pointers are optional caller-allocated HOST arrays of max_iter+1 entries

@@ -26,6 +26,9 @@ template <typename T> struct PlanImpl : PlanBase {
     int *trR = nullptr, *trB = nullptr;
     int trace_cap = 0;
     cudaEvent_t ev0 = nullptr, ev1 = nullptr, ev2 = nullptr;
+    cudaStream_t cap_stream = nullptr;       // stream the iteration graph is captured on (use_graph)
+    cudaGraphExec_t gexec = nullptr;
+    long graph_launches = 0;                 // kernels in one replay of gexec
     // per-kernel timing (sgp_plan_set_profiling): one event pair per launch of the iteration loop
     struct ProfRec { int slot; cudaEvent_t a, b; };
     std::vector<ProfRec> prof_recs;
@@ -40,6 +43,8 @@ template <typename T> struct PlanImpl : PlanBase {
         if (ev0) cudaEventDestroy(ev0);
         if (ev1) cudaEventDestroy(ev1);
         if (ev2) cudaEventDestroy(ev2);
+        if (gexec) cudaGraphExecDestroy(gexec);
+        if (cap_stream) cudaStreamDestroy(cap_stream);
         for (cudaEvent_t e : prof_pool) cudaEventDestroy(e);
     }
     cudaEvent_t prof_event()
@@ -369,6 +374,8 @@ template <typename T> struct PlanImpl : PlanBase {
     int ensure_trace(int max_iter, const sgp_result *res, Trace *tr, cudaStream_t st);
     int enqueue_sgp_iteration(const RowParams<T> &Pbase, const DevOpts &o, const Trace &tr, const double *bconst, int b_is_array, cudaStream_t st);
     int enqueue_rl_round(const DevOpts &o, const Trace &tr, const double *bconst, int b_is_array, cudaStream_t st);
+    int enqueue_many(int algorithm, int count, const RowParams<T> &Pb, const DevOpts &o, const Trace &tr, const double *bconst,
+                     int b_is_array, cudaStream_t st);
 };
 
 }  // namespace sgpk

@@ -118,6 +118,42 @@ int PlanImpl<T>::enqueue_rl_round(const DevOpts &o, const Trace &tr, const doubl
     return SGP_OK;
 }
 
+// `count` iterations (SGP) or rounds (RL).  With opt.use_graph the launches of kGraphIters iterations are captured
+// once per run into a CUDA graph (on a stream of the plan: the caller's may be the legacy default stream, which
+// cannot be captured) and the graph is replayed; everything the kernels branch on lives in the control block, so
+// the launch parameters of all iterations are identical.
+template <typename T>
+int PlanImpl<T>::enqueue_many(int algorithm, int count, const RowParams<T> &Pb, const DevOpts &o, const Trace &tr,
+                              const double *bconst, int b_is_array, cudaStream_t st)
+{
+    int rc;
+    auto one = [&](cudaStream_t s) -> int {
+        return algorithm == SGP_ALG_SGP ? enqueue_sgp_iteration(Pb, o, tr, bconst, b_is_array, s)
+                                        : enqueue_rl_round(o, tr, bconst, b_is_array, s);
+    };
+    constexpr int kGraphIters = 10;
+    if ((opt.use_graph & 1) && !profiling && count >= kGraphIters) {
+        if (!gexec) {
+            if (!cap_stream) SGP_CUDA_TRY(cudaStreamCreateWithFlags(&cap_stream, cudaStreamNonBlocking));
+            cudaGraph_t g = nullptr;
+            const long l0 = launches;
+            SGP_CUDA_TRY(cudaStreamBeginCapture(cap_stream, cudaStreamCaptureModeThreadLocal));
+            rc = SGP_OK;
+            for (int i = 0; i < kGraphIters && !rc; ++i) rc = one(cap_stream);
+            cudaError_t e = cudaStreamEndCapture(cap_stream, &g);
+            graph_launches = launches - l0; launches = l0;
+            if (rc) { if (g) cudaGraphDestroy(g); return rc; }
+            SGP_CUDA_TRY(e);
+            e = cudaGraphInstantiate(&gexec, g, 0);
+            cudaGraphDestroy(g);
+            SGP_CUDA_TRY(e);
+        }
+        while (count >= kGraphIters) { SGP_CUDA_TRY(cudaGraphLaunch(gexec, st)); count -= kGraphIters; launches += graph_launches; }
+    }
+    for (int i = 0; i < count; ++i) if ((rc = one(st))) return rc;
+    return SGP_OK;
+}
+
 template <typename T>
 int PlanImpl<T>::run(int algorithm, const void *const *g, const void *const *b_arr, const double *b_const,
                      const void *f0, void *f_out, const sgp_options *ropt, sgp_result *res, cudaStream_t st)
@@ -206,8 +242,7 @@ int PlanImpl<T>::run(int algorithm, const void *const *g, const void *const *b_a
             while (status == 0) {
                 int todo = ro.max_iter - done; if (todo > chunk) todo = chunk;
                 if (todo < 1) { status = SGP_REASON_MAXIT; break; }
-                for (int i = 0; i < todo; ++i)
-                    if ((rc = enqueue_sgp_iteration(Pb, o, tr, bconst, b_is_array, st))) return rc;
+                if ((rc = enqueue_many(algorithm, todo, Pb, o, tr, bconst, b_is_array, st))) return rc;
                 SGP_CUDA_TRY(cudaMemcpyAsync(&h, ct, sizeof(Ctrl), cudaMemcpyDeviceToHost, st));
                 SGP_CUDA_TRY(cudaStreamSynchronize(st));
                 status = h.status; done = h.k;
@@ -218,8 +253,7 @@ int PlanImpl<T>::run(int algorithm, const void *const *g, const void *const *b_a
             int rounds = 0;     // round k evaluates J0(f(k)) and, unless a rule fires, makes update k+1
             while (status == 0) {
                 int todo = ro.max_iter + 1 - rounds; if (todo > chunk) todo = chunk; if (todo < 1) todo = 1;
-                for (int i = 0; i < todo; ++i)
-                    if ((rc = enqueue_rl_round(o, tr, bconst, b_is_array, st))) return rc;
+                if ((rc = enqueue_many(algorithm, todo, Pb, o, tr, bconst, b_is_array, st))) return rc;
                 rounds += todo;
                 SGP_CUDA_TRY(cudaMemcpyAsync(&h, ct, sizeof(Ctrl), cudaMemcpyDeviceToHost, st));
                 SGP_CUDA_TRY(cudaStreamSynchronize(st));
@@ -229,6 +263,7 @@ int PlanImpl<T>::run(int algorithm, const void *const *g, const void *const *b_a
         }
     }
     SGP_CUDA_TRY(cudaEventRecord(ev2, st));
+    if (gexec) { cudaGraphExecDestroy(gexec); gexec = nullptr; }      // the kernels it holds are already enqueued
     final_update_kernel<T><<<ew_grid(n), 256, 0, st>>>(f, d, (T *)f_out, n, ct);     // a10: the last accepted step, if still pending
     launches++;
     SGP_CUDA_TRY(cudaGetLastError());
