@@ -145,6 +145,23 @@ def make_workload(name: str, rank: int):
     return w, desc
 
 
+def max_over_ranks(x: float, world: int, device=None) -> float:
+    """the slowest rank's time: all-reduce MAX over the process group (NCCL on GPUs; gloo in the CPU tests)"""
+    if world <= 1:
+        return float(x)
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([x], dtype=torch.float64, device=device if device is not None else "cpu")
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_rate(ms_local: float, iters_per_step: int, steps: int, world: int, device=None) -> tuple:
+    """(iterations/s over all ranks, ms of the slowest rank): replicas only, every rank does iters_per_step x steps"""
+    ms = max_over_ranks(ms_local, world, device)
+    return iters_per_step * steps * world / (ms * 1e-3), ms
+
+
 def oracle_time(w, iters_a: int, iters_b: int):
     """wall time of the oracle for iters_a and iters_b SGP iterations of workload w (fp64, OpenMP over the host cores)"""
     import oracle
@@ -256,13 +273,7 @@ def run_ours(args):
             launches += r.kernel_launches; backtracks += r.total_backtracks; loop_ms += r.loop_ms
         ev1.record()
         sync_all()
-    ms = ev0.elapsed_time(ev1)
-    if world > 1:
-        t = torch.tensor([ms], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
-    total_iters = iters * args.steps * world
-    value = total_iters / (ms * 1e-3)
+    value, ms = whole_job_rate(ev0.elapsed_time(ev1), iters, args.steps, world, dev)
     J_final = r.J0_final
 
     # ---- instrumented pass: CUDA event pair around every launch of the same step (not part of `value`)
@@ -332,10 +343,7 @@ def run_ours(args):
             re = e2e_step()
         torch.cuda.synchronize()
         dt = time.perf_counter() - t0
-        if world > 1:
-            t = torch.tensor([dt], dtype=torch.float64, device=dev)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            dt = float(t.item())
+        dt = max_over_ranks(dt, world, dev)
         sbytes = sum(a.nbytes for a in hg) + sum(a.nbytes for a in hk)
         e2e = {"value": re.iterations * n_e2e * world / dt, "unit": "iterations/s", "h2d_bytes_per_step": sbytes,
                "d2h_bytes_per_step": hf.nbytes, "steps": n_e2e, "ms_per_step": 1e3 * dt / n_e2e,
