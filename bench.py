@@ -60,15 +60,19 @@ def load_peaks():
     return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
 
 
-def planes_per_launch(p: int, b_array: bool, masked: bool, backtracks_per_iter: float = 0.0):
+def planes_per_launch(p: int, b_array: bool, masked: bool, backtracks_per_iter: float = 0.0, fused: bool = True):
     """algorithmic planes (n reals each) read + written per launch of the kernels as built, DESIGN.md section 6.
-    K1 = g, q, u read; q, spectrum written (lazy a10 for q).  K3 = spectrum, f, d, grad read; f, grad written (lazy a10
-    for f).  K7 = q, u, g read once per Armijo trial (average over the launches of the run)."""
+    K6 (fused line search) = spectrum, q, g read; u, q(k+1), ratio spectrum written.  K1 = g, q, u read; q, spectrum
+    written: it returns at once unless the previous iteration backtracked (average over the launches of the run, the
+    share of such iterations bounded by backtracks per iteration).  K3 = spectrum, f, d, grad read; f, grad written
+    (lazy a10 for f).  K7 = q, u, g read once per Armijo trial (average over the launches of the run)."""
     ba = p if b_array else 0
     m = 1 if masked else 0
+    k1 = (5 * p + ba) * (min(1.0, backtracks_per_iter) if fused else 1.0)
+    k6 = (6 * p + ba) if fused else (4 * p + ba)
     return {
-        "K1_ratio_rowfft": 5 * p + ba, "K2_col_conjsum": 2 * p + 1, "K3_rowifft_grad_bb": 6 + m,
-        "K4_project_rowfft": 4 + m, "K5_col_mult": 2 * p + 1, "K6_rowifft_linesearch": 4 * p + ba,
+        "K1_ratio_rowfft": k1, "K2_col_conjsum": 2 * p + 1, "K3_rowifft_grad_bb": 6 + m,
+        "K4_project_rowfft": 4 + m, "K5_col_mult": 2 * p + 1, "K6_rowifft_linesearch": k6,
         "K7_backtrack": (3 * p + ba) * backtracks_per_iter,
         "R1_rowfft": 2, "R2_col_mult": 2 * p + 1, "R3_rowifft_q_J": 3 * p + ba, "R4_ratio_rowfft": 3 * p + ba,
         "R5_col_conjsum": 2 * p + 1, "R6_rowifft_update": 3 + m,
@@ -160,6 +164,99 @@ def whole_job_rate(ms_local: float, iters_per_step: int, steps: int, world: int,
     """(iterations/s over all ranks, ms of the slowest rank): replicas only, every rank does iters_per_step x steps"""
     ms = max_over_ranks(ms_local, world, device)
     return iters_per_step * steps * world / (ms * 1e-3), ms
+
+
+def cufft_compare(w, dev, tdt, iters: int, warm: int = 5):
+    """In-run comparison baseline named by north_star: the same SGP iteration (Alg.1, step lengths
+    PAPER.md:130-155) written the way the paper's own GPU code is organised (one library call per
+    vector operation, the host decides every branch), with cuFFT (torch.fft) for the 2p + 2 transforms and torch
+    elementwise / reduction kernels for the rest.  Periodic (unmasked) workloads only.  Returns iterations/s over
+    `iters` iterations after `warm` untimed ones, and J0 for a sanity comparison with the library's trace."""
+    import torch
+    fft = torch.fft
+    o = w["opts"]
+    p = len(w["g"]); ny, nx = w["psf"][0].shape
+    g = [torch.as_tensor(np.ascontiguousarray(a), device=dev).to(tdt).clamp_(min=0) for a in w["g"]]
+    b = [float(x) for x in w["b"]]
+    K = []
+    for k in w["psf"]:
+        kk = torch.as_tensor(np.ascontiguousarray(k), device=dev).to(torch.float64)
+        K.append(fft.rfft2(fft.ifftshift(kk / kk.sum()).to(tdt)))
+    dsum = lambda x: float(x.sum(dtype=torch.float64).item())
+    A = lambda F, j: fft.irfft2(K[j] * F, s=(ny, nx))
+    def kl(gj, y):
+        return torch.where(gj > 0, gj * torch.log(gj / y) + y - gj, y)
+    def J0(q, lam=None, u=None):
+        return sum(dsum(kl(g[j], (q[j] if u is None else q[j] + lam * u[j]) + b[j])) for j in range(p))
+    def AT_ratio(q):
+        F = None
+        for j in range(p):
+            t = torch.conj(K[j]) * fft.rfft2(g[j] / (q[j] + b[j]))
+            F = t if F is None else F + t
+        return fft.irfft2(F, s=(ny, nx))
+    c0 = max(0.0, sum(dsum(g[j] - b[j]) for j in range(p)) / (p * ny * nx))
+    f = torch.full((ny, nx), c0, dtype=tdt, device=dev)
+    Ff = fft.rfft2(f)
+    q = [A(Ff, j) for j in range(p)]
+    J = J0(q)
+    L1, L2 = float(o.get("L1", 1e-10)), float(o.get("L2", 1e10))
+    if o.get("adaptive_L", 1):
+        y = f * AT_ratio(q) / p
+        ymin, ymax = float(y[y > 0].min().item()), float(y.max().item())
+        L1, L2 = (ymin / 10, ymax * 10) if ymax / ymin < 50 else (ymin, ymax)
+    beta, theta = float(o.get("beta", 1e-4)), float(o.get("theta", 0.4))
+    amin, amax, alpha_prev, tau = 1e-5, 1e5, 1.3, 0.5
+    m_alpha, M = int(o.get("m_alpha", 3)), int(o.get("armijo_memory", 1))
+    ring, Jhist = [], [J]
+    f_prev = grad_prev = None
+    on_gpu = torch.device(dev).type == "cuda"
+    if on_gpu:
+        ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    for k in range(warm + iters):
+        if k == warm:
+            if on_gpu:
+                torch.cuda.synchronize(); ev0.record()
+            else:
+                t0 = time.perf_counter()
+        grad = p - AT_ratio(q)
+        D = f.clamp(L1, L2) / p
+        if k == 0:
+            alpha = 1.3
+        else:
+            s_, z_ = f - f_prev, grad - grad_prev
+            a_, c_, e_, h_ = dsum(s_ * s_ / (D * D)), dsum(s_ * z_ / D), dsum(s_ * z_ * D), dsum(z_ * z_ * D * D)
+            a1 = min(10 * alpha_prev, amax) if c_ <= 0 else min(amax, max(amin, a_ / c_))
+            a2 = min(10 * alpha_prev, amax) if e_ <= 0 else min(amax, max(amin, e_ / h_))
+            ring = (ring + [a2])[-m_alpha:]
+            if k <= 20 or a2 / a1 <= tau:
+                alpha = min(ring)
+                if k > 20: tau *= 0.9
+            else:
+                alpha = a1; tau *= 1.1
+            alpha_prev = alpha
+        d = (f - alpha * D * grad).clamp_(min=0) - f
+        gd = dsum(grad * d)
+        Fd = fft.rfft2(d)
+        u = [A(Fd, j) for j in range(p)]
+        lam, Jref = 1.0, max(Jhist[-M:])
+        for _ in range(30):
+            Jn = J0(q, lam, u)
+            if np.isfinite(Jn) and Jn <= Jref + beta * lam * gd:
+                break
+            lam *= theta
+        f_prev, grad_prev = f, grad
+        f = f + lam * d
+        q = [q[j] + lam * u[j] for j in range(p)]
+        J = Jn; Jhist.append(J)
+    if on_gpu:
+        ev1.record(); torch.cuda.synchronize()
+        ms = ev0.elapsed_time(ev1)
+    else:
+        ms = 1e3 * (time.perf_counter() - t0)
+    return {"value": iters / (ms * 1e-3), "unit": "iterations/s", "iterations": iters, "warmup_iterations": warm,
+            "J0_after": warm + iters, "J0": J,
+            "impl": "torch.fft (cuFFT) rfft2/irfft2 + torch elementwise and reduction kernels, scalar logic on the host "
+                    "(the organisation of the paper's GPUlib code, PAPER.md:302-310); comparison baseline only"}
 
 
 def oracle_time(w, iters_a: int, iters_b: int):
@@ -283,7 +380,7 @@ def run_ours(args):
     kms = plan.kernel_ms()
     plan.set_profiling(False)
     bt_per_iter = rp.total_backtracks / max(1, rp.iterations)
-    planes = planes_per_launch(p, False, w["S"] is not None, bt_per_iter)
+    planes = planes_per_launch(p, False, w["S"] is not None, bt_per_iter, fused=bool(rp.fused_linesearch))
     plane_bytes = ny * nx * esz
     peak, peak_src = load_peaks()
     per_kernel = {}
@@ -304,7 +401,7 @@ def run_ours(args):
                     traffic = float(nbytes)
         except Exception:
             traffic = None
-    # schedule A (14p + 14 planes, the primary denominator); the kernels as built move 13p + 12
+    # schedule A (14p + 14 planes, the primary denominator); the kernels as built move 10p + 12 (+ 5p + 3p per backtracked iteration)
     iter_planes = (14 * p + 14 + (2 if w["S"] is not None else 0)) if args.alg == "sgp" else (
         sum(planes[k] for k in planes if k.startswith("R")))
     built_planes = sum(planes[k] for k in planes if k.startswith("K" if args.alg == "sgp" else "R"))
@@ -363,6 +460,15 @@ def run_ours(args):
                "sample": f"{args.workload} ({p}x{ny}x{nx}) fp64 oracle: (t({ib} it) - t({ia} it)) / {ib - ia}, start-point phase excluded; "
                          f"t({ia})={ta:.2f}s t({ib})={tb:.2f}s; OpenMP over {cores} threads"}
 
+    # ---- in-run comparison: the same iteration on cuFFT + torch kernels (north_star: "cuFFT ... in-run comparison baseline")
+    cufft = None
+    if rank == 0 and world == 1 and args.alg == "sgp" and w["S"] is None and not args.no_cufft:
+        try:
+            cufft = cufft_compare(w, dev, tdt, args.cufft_iters)
+            cufft["speedup_of_this_library"] = value / cufft["value"]
+        except Exception as e:      # a comparison leg must never take the bench line down
+            cufft = {"error": f"{type(e).__name__}: {e}"}
+
     if rank == 0:
         line = {"metric": "SGP iterations/s" if args.alg == "sgp" else "RL iterations/s", "value": value, "unit": "iterations/s",
                 "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms / args.steps,
@@ -373,8 +479,10 @@ def run_ours(args):
                            "l2": f"no flush: per-iteration working set {(6 * p + 4) * plane_bytes / 1e6:.0f} MB "
                                  f"({6 * p + 4} planes) vs 126 MB L2",
                            "tile_cols": int(opts.tile_cols), "rows_per_block": int(opts.rows_per_block),
-                           "J0_final": J_final, "backtracks": backtracks // args.steps},
-                "clocks": clk.summary(), "e2e": e2e, "gpu_launches": launches, "roofline": roofline, "cpu_baseline": cpu}
+                           "J0_final": J_final, "backtracks": backtracks // args.steps,
+                           "fused_linesearch": int(r.fused_linesearch)},
+                "clocks": clk.summary(), "e2e": e2e, "gpu_launches": launches, "roofline": roofline, "cpu_baseline": cpu,
+                "cufft_compare": cufft}
         print(json.dumps(line))
     plan.close()
     if world > 1:
@@ -395,9 +503,11 @@ def main():
     ap.add_argument("--rows-per-block", type=int, default=0)
     ap.add_argument("--cpu-iters", type=int, default=5, help="oracle iterations timed for cpu_baseline")
     ap.add_argument("--ref-iters", type=int, default=3, help="oracle iterations per step of --impl reference")
-    ap.add_argument("--graph", type=int, default=1, help="1 = replay the iterations as CUDA graphs of 10 (default), 0 = plain launches")
+    ap.add_argument("--graph", type=int, default=1, help="1 = replay the iterations as CUDA graphs of 10 (default), 0 = plain launches; +4 / +8 = force the separate / fused line-search kernel (experiment)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
+    ap.add_argument("--no-cufft", action="store_true", help="skip the cuFFT + torch comparison leg")
+    ap.add_argument("--cufft-iters", type=int, default=40, help="iterations timed by the cuFFT comparison leg")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)

@@ -100,7 +100,9 @@ typedef struct sgp_options {
     int backend;                                 /* sgp_backend */
     int tile_cols;                               /* tuning: spectrum tile width in columns (power of 2); 0 = auto */
     int rows_per_block;                          /* tuning: rows per CTA in the row-FFT kernels (power of 2); 0 = auto */
-    int use_graph;                               /* 1 (default) = replay the iterations as CUDA graphs of 10; 0 = plain stream launches */
+    int use_graph;                               /* bit 0 (default 1) = replay the iterations as CUDA graphs of 10, else plain stream launches;
+                                                    experiment switches: bit 1 = persistent column kernel, bit 2 / bit 3 = force the
+                                                    separate / the fused line-search kernel (default: chosen by working set vs L2) */
 } sgp_options;
 
 /* Result of a run.  The trace pointers are optional caller-allocated HOST arrays of max_iter+1 entries
@@ -119,6 +121,7 @@ typedef struct sgp_result {
     long n_fft2;                /* 2-D transforms executed inside the iteration loop (2p+2 per iteration) */
     double setup_ms, loop_ms;   /* device time of the start-point phase and of the iteration loop (CUDA events) */
     long kernel_launches;       /* kernels of this library launched by the call */
+    int fused_linesearch;       /* 1: the run used the fused line-search + ratio kernel (chosen by working set vs L2) */
     double *trace_J, *trace_alpha, *trace_lambda;
     int *trace_rule, *trace_backtracks;
     const double *force_alpha, *force_lambda;

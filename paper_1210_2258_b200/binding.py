@@ -56,6 +56,7 @@ class _Result(C.Structure):
         ("discrepancy_final", C.c_double), ("total_backtracks", C.c_int),
         ("L1_used", C.c_double), ("L2_used", C.c_double), ("n_fft2", C.c_long),
         ("setup_ms", C.c_double), ("loop_ms", C.c_double), ("kernel_launches", C.c_long),
+        ("fused_linesearch", C.c_int),
         ("trace_J", C.POINTER(C.c_double)), ("trace_alpha", C.POINTER(C.c_double)),
         ("trace_lambda", C.POINTER(C.c_double)), ("trace_rule", C.POINTER(C.c_int)),
         ("trace_backtracks", C.POINTER(C.c_int)),
@@ -136,6 +137,7 @@ class Result:
         self.n_fft2 = raw.n_fft2
         self.setup_ms, self.loop_ms = raw.setup_ms, raw.loop_ms
         self.kernel_launches = raw.kernel_launches
+        self.fused_linesearch = raw.fused_linesearch
         k = self.iterations
         self.J = tr["J"][: k + 1].copy()
         self.alpha = tr["alpha"][:k].copy()

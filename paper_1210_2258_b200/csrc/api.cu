@@ -72,7 +72,7 @@ size_t workspace_bytes(int kind, int p, int ny, int nx, int dtype)
     if (p < 1 || p > SGP_MAX_IMAGES || !size_supported(ny) || !size_supported(nx)) return 0;
     const size_t r = dtype == SGP_F64 ? 8 : 4;
     const size_t n = (size_t)ny * nx;
-    size_t planes = 6 * (size_t)p + 4;                 // khat, spec, g, b, q, u per image; f, grad, d, scratch
+    size_t planes = 7 * (size_t)p + 4;                 // khat, spec, g, b, q (two buffers), u per image; f, grad, d, scratch
     size_t b = planes * n * r;
     if (kind == SGP_KIND_BOUNDARY) b += 2 * n * r + n;
     b += ((size_t)nx + 1 + 2 * (size_t)ny + (size_t)ny * p) * 2 * r;   // twiddles, pack line, khatB

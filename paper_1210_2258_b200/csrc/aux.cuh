@@ -12,14 +12,14 @@ namespace sgpk {
 // CTA.  The grid is sized by the occupancy API so that all CTAs are resident together, and the barrier is a
 // sense-reversing counter in the control block: an ordinary launch, because the empty cooperative launches of the
 // usual case cost 7 us per iteration.  The accepted step is NOT applied here: f + lambda d and q_j + lambda u_j
-// are formed by the next iteration's kernels (lazy update) or by final_update_kernel.
+// are formed by the next iteration's kernels (K1 in repair mode, Ctrl::need_k1 = 2; K3) or by final_update_kernel.
 template <typename T> struct BtParams {
     Geom G;
     DevOpts o;
     Trace tr;
     Ctrl *ct;
-    const T *q, *u, *g, *b;                      // image j at + j*plane
-    size_t plane;
+    const T *q, *u, *g, *b;                      // image j at + j*plane; q: buffer Ctrl::qsel at + qsel*qbuf
+    size_t plane, qbuf;
     int b_is_array;
     double bconst[kMaxP];
     double *part;                                // gridDim.x doubles
@@ -61,6 +61,7 @@ __global__ void __launch_bounds__(256) backtrack_kernel(const BtParams<T> P)
     const size_t n = (size_t)G.ny * G.nx, nv = n / VN;
     const size_t gtid = (size_t)blockIdx.x * blockDim.x + threadIdx.x, gstride = (size_t)gridDim.x * blockDim.x;
     const int k = ct->k;
+    const T *qcur = P.q + (size_t)ct->qsel * P.qbuf;           // A_j f(k): the buffer the line-search kernel read
     const double Jref = ct->Jref, gd = ct->gd;
     double lambda = 1.0, Jnew = ct->Jtrial;
     bool accepted = false, forced = false;
@@ -80,7 +81,7 @@ __global__ void __launch_bounds__(256) backtrack_kernel(const BtParams<T> P)
         const T lam = (T)lambda;
         double acc[1] = {0.0};
         for (int j = 0; j < G.p; ++j) {
-            const T *q = P.q + (size_t)j * P.plane, *u = P.u + (size_t)j * P.plane, *g = P.g + (size_t)j * P.plane;
+            const T *q = qcur + (size_t)j * P.plane, *u = P.u + (size_t)j * P.plane, *g = P.g + (size_t)j * P.plane;
             const T *b = P.b_is_array ? P.b + (size_t)j * P.plane : nullptr;
             const T bc = (T)P.bconst[j];
             for (size_t i = gtid; i < nv; i += gstride) {
@@ -115,7 +116,7 @@ __global__ void __launch_bounds__(256) backtrack_kernel(const BtParams<T> P)
     if (threadIdx.x == 0) {
         __threadfence();
         unsigned int tk = atomicAdd(&ct->counter[TK_BACKTRACK], 1u);
-        if (tk == gridDim.x - 1) { ct->counter[TK_BACKTRACK] = 0; finish_iteration(ct, P.o, P.tr, lambda, Jnew, nbt); }
+        if (tk == gridDim.x - 1) { ct->counter[TK_BACKTRACK] = 0; finish_iteration(ct, P.o, P.tr, lambda, Jnew, nbt, 2); }
     }
 }
 

@@ -23,6 +23,7 @@ template <int L> static row_kernel_t<SGP_T> pick_rowi(int mode)
     case RI_LS: return row_inv_kernel<SGP_T, L, RI_LS>;
     case RI_QJ: return row_inv_kernel<SGP_T, L, RI_QJ>;
     case RI_RLUPDATE: return row_inv_kernel<SGP_T, L, RI_RLUPDATE>;
+    case RI_LSF: return row_inv_kernel<SGP_T, L, RI_LSF>;
     default: return nullptr;
     }
 }

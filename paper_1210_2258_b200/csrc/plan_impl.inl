@@ -8,6 +8,7 @@ template <typename T> struct PlanImpl : PlanBase {
     size_t n = 0, nspec = 0;       // reals per plane, complex numbers per half spectrum (= n/2)
     int Lr = 0, Lc = 0;            // FFT lengths: nx/2 (rows), ny (columns)
     bool use_pdl = true;
+    bool fuse_ls = true;           // line-search kernel fused with the next iteration's ratio + row FFT (row_inv RI_LSF)
     int row_threads = 0, col_threads = 0, nrb = 0, ntiles = 0, bt_grid = 0, nsm = 0, col_grid = 0;
     size_t row_smem = 0, col_smem = 0;
     row_kernel_t<T> k_rowf[RF_NMODES] = {nullptr}, k_rowi[RI_NMODES] = {nullptr};
@@ -129,6 +130,18 @@ template <typename T> struct PlanImpl : PlanBase {
         if (per_sm < 1) return SGP_ERR_CUDA;
         if (per_sm > 4) per_sm = 4;
         bt_grid = nsm * per_sm;
+        // Fused or separate line-search / ratio kernels.  Separate, the ratio kernel re-reads g_j, q_j, u_j right after the
+        // line-search kernel touched them: free while those 3p planes stay in L2 (2048^2 fp32 single image: 50 MB of
+        // 126 MB; measured 7700 vs 7240 it/s), a second trip to HBM once they do not (3 x 2048^2, 4096^2, fp64: fused is
+        // 3.5-4.5 % faster).  Small grids are latency-bound and gain from the launch the fused form saves.
+        {
+            int l2 = 0;
+            SGP_CUDA_TRY(cudaDeviceGetAttribute(&l2, cudaDevAttrL2CacheSize, dev));
+            const size_t handoff = 3 * (size_t)p * n * sizeof(T);
+            fuse_ls = handoff > (size_t)l2 / 2 || handoff < (size_t)l2 / 8;
+            if (opt.use_graph & 4) fuse_ls = false;      // experiment switches
+            if (opt.use_graph & 8) fuse_ls = true;
+        }
         col_grid = (opt.use_graph & 2) ? (ntiles < nsm ? ntiles : nsm) : ntiles;   // experiment switch: persistent or one tile per CTA
         size_t want = (n / vec4_of<T>::N + 255) / 256;
         if ((size_t)bt_grid > want) bt_grid = (int)(want < 1 ? 1 : want);
@@ -170,7 +183,7 @@ template <typename T> struct PlanImpl : PlanBase {
         if ((rc = dalloc(&spec, nspec * p))) return rc;
         if ((rc = dalloc(&Gp, n * p))) return rc;
         if ((rc = dalloc(&Bp, n * p))) return rc;
-        if ((rc = dalloc(&q, n * p))) return rc;
+        if ((rc = dalloc(&q, 2 * n * p))) return rc;          // double-buffered (Ctrl::qsel)
         if ((rc = dalloc(&u, n * p))) return rc;
         if ((rc = dalloc(&f, n))) return rc;
         if ((rc = dalloc(&grad, n))) return rc;
@@ -200,7 +213,7 @@ template <typename T> struct PlanImpl : PlanBase {
         RowParams<T> P;
         memset(&P, 0, sizeof(P));
         P.G = G; P.ct = ct;
-        P.plane = n; P.specplane = nspec; P.spec = spec;
+        P.plane = n; P.specplane = nspec; P.spec = spec; P.qbuf = n * (size_t)p;
         P.tw = tw_r; P.twh = tw_h; P.alphaR = alphaR;
         return P;
     }

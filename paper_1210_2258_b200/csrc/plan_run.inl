@@ -76,14 +76,14 @@ int PlanImpl<T>::enqueue_sgp_iteration(const RowParams<T> &Pb, const DevOpts &o,
     cur_slot = SGP_PROF_K6;
     {   // K6 (a8 tail, a9 at lambda = 1, a11)
         RowParams<T> P = Pb; P.in0 = Gp; P.in1 = q; P.in2 = Bp; P.out0 = u; P.part = part_J; P.part2 = part_gd;
-        if ((rc = launch_row(k_rowi[RI_LS], P, p, st))) return rc;
+        if ((rc = launch_row(k_rowi[fuse_ls ? RI_LSF : RI_LS], P, p, st))) return rc;
     }
     cur_slot = SGP_PROF_K7;
     {   // K7 (a9 backtracks, a11)
         BtParams<T> U;
         memset(&U, 0, sizeof(U));
         U.G = G; U.o = o; U.tr = tr; U.ct = ct; U.q = q; U.u = u; U.g = Gp; U.b = Bp;
-        U.plane = n; U.b_is_array = b_is_array; U.part = part_bt;
+        U.plane = n; U.qbuf = n * (size_t)p; U.b_is_array = b_is_array; U.part = part_bt;
         for (int j = 0; j < p; ++j) U.bconst[j] = bconst[j];
         ProfScope ps(this, st);
         backtrack_kernel<T><<<bt_grid, 256, 0, st>>>(U);
@@ -194,7 +194,9 @@ int PlanImpl<T>::run(int algorithm, const void *const *g, const void *const *b_a
     Ctrl h;
     memset(&h, 0, sizeof(h));
     h.alpha_prev = ro.alpha0; h.tau = ro.tau1; h.L1 = ro.L1; h.L2 = ro.L2; h.lambda = 1.0;
+    h.qsel = 0; h.need_k1 = 1;
     SGP_CUDA_TRY(cudaMemcpyAsync(ct, &h, sizeof(Ctrl), cudaMemcpyHostToDevice, st));
+    SGP_CUDA_TRY(cudaMemsetAsync(q + n * (size_t)p, 0, sizeof(T) * n * (size_t)p, st));     // second q buffer: zero outside S
     const int eg = ew_grid(n) > 1024 ? 1024 : ew_grid(n);
     for (int j = 0; j < p; ++j) {
         embed_inputs_kernel<T><<<eg, 256, 0, st>>>((const T *)g[j], b_is_array ? (const T *)b_arr[j] : nullptr, Gp + (size_t)j * n,
@@ -290,6 +292,7 @@ int PlanImpl<T>::run(int algorithm, const void *const *g, const void *const *b_a
     res->n_fft2 = fft2;
     res->setup_ms = ms01; res->loop_ms = ms12;
     res->kernel_launches = launches - launches0;
+    res->fused_linesearch = (algorithm == SGP_ALG_SGP && fuse_ls) ? 1 : 0;
     return status < 0 ? status : SGP_OK;
 }
 

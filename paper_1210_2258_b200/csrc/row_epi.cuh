@@ -91,8 +91,13 @@ __device__ __forceinline__ void epi_grad(const RowParams<T> &P, const T *wrow, i
 
 // RI_LS (a8 tail + a9): u_j = A_j d on S; J(1) = sum kl(g_j, q_j + u_j + b_j).
 // RI_QJ: q_j = A_j f on S; J0(f) = sum kl(g_j, q_j + b_j) (Eq.2/12 over S, A12); QJ_PLAIN only stores.
-template <typename T, int L, int TF, bool WITH_Q, bool MASKED>
-__device__ __forceinline__ void epi_kl(const RowParams<T> &P, const T *wrow, int t, int y, int j, size_t base, bool plain, double (&acc)[1])
+// SPEC (RI_LSF): besides u_j and J(1), the step lambda = 1 is applied speculatively: q_j + u_j goes to the other q
+// buffer (qout) and the ratio r_j = g_j / (q_j + u_j + b_j) of the NEXT iteration (a1) replaces the row in shared
+// memory (wmut), from where the caller transforms it -- if the Armijo test then accepts lambda = 1 (the usual
+// case) the next iteration needs no ratio kernel at all.
+template <typename T, int L, int TF, bool WITH_Q, bool MASKED, bool SPEC>
+__device__ __forceinline__ void epi_kl(const RowParams<T> &P, const T *wrow, T *wmut, const T *qin, T *qout, int t, int y, int j,
+                                       size_t base, bool plain, double (&acc)[1])
 {
     const Geom &G = P.G;
     const T bc = (T)P.bconst[j];
@@ -108,7 +113,7 @@ __device__ __forceinline__ void epi_kl(const RowParams<T> &P, const T *wrow, int
             w4[u] = ldq<T>(wrow + x);
             if (need) {
                 g4[u] = ldq<T>(P.in0 + base + x);
-                if constexpr (WITH_Q) q4[u] = ldq<T>(P.in1 + base + x);
+                if constexpr (WITH_Q) q4[u] = ldq<T>(qin + base + x);
                 if (P.b_is_array) b4[u] = ldq<T>(P.in2 + base + x);
             }
         }
@@ -121,16 +126,31 @@ __device__ __forceinline__ void epi_kl(const RowParams<T> &P, const T *wrow, int
 #pragma unroll
             for (int c = 0; c < 4; ++c) u4.a[c] = s[c] ? w4[u].a[c] : (T)0;
             stq<T>(P.out0 + base + x, u4);
+            Quad<T> r4;
+#pragma unroll
+            for (int c = 0; c < 4; ++c) r4.a[c] = (T)0;
             if (need) {
                 T yv[4];
 #pragma unroll
                 for (int c = 0; c < 4; ++c) {
                     yv[c] = u4.a[c];
                     if constexpr (WITH_Q) yv[c] += q4[u].a[c];
-                    yv[c] += P.b_is_array ? b4[u].a[c] : bc;
                 }
+                if constexpr (SPEC) {
+                    Quad<T> q1;
+#pragma unroll
+                    for (int c = 0; c < 4; ++c) q1.a[c] = yv[c];
+                    stq<T>(qout + base + x, q1);
+                }
+#pragma unroll
+                for (int c = 0; c < 4; ++c) yv[c] += P.b_is_array ? b4[u].a[c] : bc;
                 acc[0] += (double)kl_quad(g4[u].a, yv, s);
+                if constexpr (SPEC) {
+#pragma unroll
+                    for (int c = 0; c < 4; ++c) r4.a[c] = s[c] ? ratio_term(g4[u].a[c], yv[c]) : (T)0;
+                }
             }
+            if constexpr (SPEC) stq<T>(wmut + x, r4);
         }
     }
 }

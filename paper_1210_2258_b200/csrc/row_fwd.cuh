@@ -28,6 +28,64 @@ template <typename T> __device__ __forceinline__ void untangle(cx<T> a, cx<T> zb
     xlk = cconj(csub(Ek, wo));
 }
 
+// Forward transform of one row held as v[e] = (x[2m], x[2m+1]), m = t + TF e, by the TF threads of the row, and
+// store of its half spectrum (tile-major).  Shared by the forward row kernel and the fused line-search kernel.
+template <typename T, int L, typename SYNC>
+__device__ __forceinline__ void fwd_fft_store(cx<T> (&v)[fft_E<T>(L)], cx<T> *smrow, const int t, const SYNC &sync,
+                                              const RowParams<T> &P, const int y, const int j)
+{
+    using C = cx<T>;
+    constexpr int E = fft_E<T>(L);
+    constexpr int TF = L / E;
+    const Geom &G = P.G;
+    // ---- complex FFT of length L = nx/2 over z[m] = x[2m] + i x[2m+1]
+    fft_block<T, L, E, -1>(v, smrow, 1, t, P.tw, sync);
+    sync();
+#pragma unroll
+    for (int e = 0; e < E; ++e) smrow[fft_pad<E>(t + TF * e)] = v[e];
+    sync();
+
+    // ---- untangle the two interleaved real transforms, one (k, L-k) pair per step, and store tile-major:
+    //      E = (Z[k] + conj Z[L-k])/2, O = -i (Z[k] - conj Z[L-k])/2, w = exp(-2 pi i k/nx):
+    //      X[k] = E + w O,  X[L-k] = conj(E - w O);  entry 0 = (X[0], X[L]) packed;  X[L/2] = conj Z[L/2]
+    C *dst = P.spec + (size_t)j * P.specplane;
+    {   // i = 0
+        const C a = smrow[fft_pad<E>(t)];
+        if (t == 0) {
+            dst[spec_index(G, y, 0)] = mk<T>(a.x + a.y, a.x - a.y);
+            dst[spec_index(G, y, L / 2)] = cconj(smrow[fft_pad<E>(L / 2)]);
+        } else {
+            C xk, xlk;
+            untangle<T>(a, smrow[fft_pad<E>(L - t)], __ldg(&P.twh[t]), xk, xlk);
+            dst[spec_index(G, y, t)] = xk;
+            dst[spec_index(G, y, L - t)] = xlk;
+        }
+    }
+    if ((TF & (G.C - 1)) == 0) {
+        // TF is a multiple of the tile width: kx -> kx + TF moves TF/C tiles on, i.e. TF*ny elements
+        const size_t stride = (size_t)TF * (size_t)G.ny;
+        C *pa = dst + spec_index(G, y, t);
+        C *pb = dst + spec_index(G, y, L - TF - t) + stride;
+#pragma unroll
+        for (int i = 1; i < E / 2; ++i) {
+            const int k = t + TF * i;
+            C xk, xlk;
+            untangle<T>(smrow[fft_pad<E>(k)], smrow[fft_pad<E>(L - k)], __ldg(&P.twh[k]), xk, xlk);
+            pa[(size_t)i * stride] = xk;
+            *(pb - (size_t)i * stride) = xlk;
+        }
+    } else {
+#pragma unroll 4
+        for (int i = 1; i < E / 2; ++i) {
+            const int k = t + TF * i;
+            C xk, xlk;
+            untangle<T>(smrow[fft_pad<E>(k)], smrow[fft_pad<E>(L - k)], __ldg(&P.twh[k]), xk, xlk);
+            dst[spec_index(G, y, k)] = xk;
+            dst[spec_index(G, y, L - k)] = xlk;
+        }
+    }
+}
+
 template <typename T, int L, int MODE>
 __global__ void __launch_bounds__(256, 2) row_fwd_kernel(const RowParams<T> P)
 {
@@ -91,11 +149,18 @@ __global__ void __launch_bounds__(256, 2) row_fwd_kernel(const RowParams<T> P)
             }
         }
     } else if constexpr (MODE == RF_RATIO) {
-        // a10 (lazy): q_j <- q_j + lambda u_j of the step accepted last iteration; a1: r_j = g_j / (q_j + b_j) on S (Eq.11/14/18)
+        // a1: r_j = g_j / (q_j + b_j) on S (Eq.11/14/18).  In the SGP loop (lazy) the q planes are double-buffered and
+        // Ctrl::need_k1 says what is left to do: 0 = nothing (the fused line-search kernel accepted lambda = 1 and has
+        // already formed q(k+1), the ratio and this very spectrum), 1 = ratio of the current q (first iteration),
+        // 2 = a10 after a backtrack: q(k+1) = q(k) + lambda u_j into the other buffer, then the ratio.
         const size_t base = (size_t)j * P.plane + (size_t)y * nx;
         const T bc = (T)P.bconst[j];
         const bool rowin = (unsigned)(y - G.oy) < (unsigned)G.sy;
-        const bool pend = P.lazy && P.ct->pending;
+        int todo = 1, sel = 0;
+        if (P.lazy) { todo = P.ct->need_k1; if (todo == 0) return; sel = P.ct->qsel; }
+        const bool pend = todo == 2;
+        const T *qsrc = P.in1 + (size_t)(pend ? sel ^ 1 : sel) * P.qbuf;
+        T *qdst = P.out0 + (size_t)sel * P.qbuf;
         const T lam = (T)P.ct->lambda;
         // loads of a batch are issued before its stores (q is updated in place: the compiler would otherwise
         // serialise every load behind the previous store)
@@ -108,7 +173,7 @@ __global__ void __launch_bounds__(256, 2) row_fwd_kernel(const RowParams<T> P)
                 for (int u = 0; u < U; ++u) {
                     const int x0 = 2 * (t + TF * (e0 + u));
                     g2[u] = ld2<T>(P.in0 + base + x0);
-                    q2[u] = ld2<T>(P.in1 + base + x0);
+                    q2[u] = ld2<T>(qsrc + base + x0);
                     if (pend) u2[u] = ld2<T>(P.in3 + base + x0);
                     b2[u] = P.b_is_array ? ld2<T>(P.in2 + base + x0) : mk<T>(bc, bc);
                 }
@@ -122,10 +187,10 @@ __global__ void __launch_bounds__(256, 2) row_fwd_kernel(const RowParams<T> P)
                     C qn = q2[u];
                     if (pend) {
                         qn.x = qn.x + lam * u2[u].x; qn.y = qn.y + lam * u2[u].y;
-                        st2<T>(P.out0 + base + x0, qn);
+                        st2<T>(qdst + base + x0, qn);
                     }
-                    if ((unsigned)(x0 - G.ox) < (unsigned)G.sx)     r.x = ratio_term<T>(g2[u].x, qn.x + b2[u].x);
-                    if ((unsigned)(x0 + 1 - G.ox) < (unsigned)G.sx) r.y = ratio_term<T>(g2[u].y, qn.y + b2[u].y);
+                    if ((unsigned)(x0 - G.ox) < (unsigned)G.sx)     r.x = ratio_term(g2[u].x, qn.x + b2[u].x);
+                    if ((unsigned)(x0 + 1 - G.ox) < (unsigned)G.sx) r.y = ratio_term(g2[u].y, qn.y + b2[u].y);
                 }
                 v[e0 + u] = r;
             }
@@ -179,54 +244,9 @@ __global__ void __launch_bounds__(256, 2) row_fwd_kernel(const RowParams<T> P)
     }
 
     if (stop != 0) return;
-    // ---- complex FFT of length L = nx/2 over z[m] = x[2m] + i x[2m+1]
     C *smrow = sm + row * RS;
     const SyncGroup<TF> sync{1 + row};
-    fft_block<T, L, E, -1>(v, smrow, 1, t, P.tw, sync);
-    sync();
-#pragma unroll
-    for (int e = 0; e < E; ++e) smrow[fft_pad<E>(t + TF * e)] = v[e];
-    sync();
-
-    // ---- untangle the two interleaved real transforms, one (k, L-k) pair per step, and store tile-major:
-    //      E = (Z[k] + conj Z[L-k])/2, O = -i (Z[k] - conj Z[L-k])/2, w = exp(-2 pi i k/nx):
-    //      X[k] = E + w O,  X[L-k] = conj(E - w O);  entry 0 = (X[0], X[L]) packed;  X[L/2] = conj Z[L/2]
-    C *dst = P.spec + (size_t)j * P.specplane;
-    {   // i = 0
-        const C a = smrow[fft_pad<E>(t)];
-        if (t == 0) {
-            dst[spec_index(G, y, 0)] = mk<T>(a.x + a.y, a.x - a.y);
-            dst[spec_index(G, y, L / 2)] = cconj(smrow[fft_pad<E>(L / 2)]);
-        } else {
-            C xk, xlk;
-            untangle<T>(a, smrow[fft_pad<E>(L - t)], __ldg(&P.twh[t]), xk, xlk);
-            dst[spec_index(G, y, t)] = xk;
-            dst[spec_index(G, y, L - t)] = xlk;
-        }
-    }
-    if ((TF & (G.C - 1)) == 0) {
-        // TF is a multiple of the tile width: kx -> kx + TF moves TF/C tiles on, i.e. TF*ny elements
-        const size_t stride = (size_t)TF * (size_t)G.ny;
-        C *pa = dst + spec_index(G, y, t);
-        C *pb = dst + spec_index(G, y, L - TF - t) + stride;
-#pragma unroll
-        for (int i = 1; i < E / 2; ++i) {
-            const int k = t + TF * i;
-            C xk, xlk;
-            untangle<T>(smrow[fft_pad<E>(k)], smrow[fft_pad<E>(L - k)], __ldg(&P.twh[k]), xk, xlk);
-            pa[(size_t)i * stride] = xk;
-            *(pb - (size_t)i * stride) = xlk;
-        }
-    } else {
-#pragma unroll 4
-        for (int i = 1; i < E / 2; ++i) {
-            const int k = t + TF * i;
-            C xk, xlk;
-            untangle<T>(smrow[fft_pad<E>(k)], smrow[fft_pad<E>(L - k)], __ldg(&P.twh[k]), xk, xlk);
-            dst[spec_index(G, y, k)] = xk;
-            dst[spec_index(G, y, L - k)] = xlk;
-        }
-    }
+    fwd_fft_store<T, L>(v, smrow, t, sync, P, y, j);
 
     if constexpr (MODE == RF_PROJECT) {
         __shared__ double red[32];

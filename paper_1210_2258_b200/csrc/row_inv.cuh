@@ -4,6 +4,7 @@
 // Same thread organisation as row_fwd.cuh: the TF threads of a row synchronise only among themselves.
 #pragma once
 #include "row_epi.cuh"
+#include "row_fwd.cuh"
 
 namespace sgpk {
 
@@ -142,19 +143,25 @@ __global__ void __launch_bounds__(256, 2) row_inv_kernel(const RowParams<T> P)
             final_sum<4>(acc, P.part, nblk, red);
             if (tid == 0) { P.ct->pending = 0; bb_step(P.ct, P.o, P.tr, acc[0], acc[1], acc[2], acc[3]); }   // a6
         }
-    } else if constexpr (MODE == RI_LS || MODE == RI_QJ) {
+    } else if constexpr (MODE == RI_LS || MODE == RI_QJ || MODE == RI_LSF) {
+        constexpr bool LS = (MODE == RI_LS || MODE == RI_LSF), SPEC = (MODE == RI_LSF);
         const bool plain = (MODE == RI_QJ) && P.submode == QJ_PLAIN;
         double acc[1] = {0.0};
-        if (G.masked) epi_kl<T, L, TF, MODE == RI_LS, true>(P, wrow, t, y, j, base, plain, acc);
-        else          epi_kl<T, L, TF, MODE == RI_LS, false>(P, wrow, t, y, j, base, plain, acc);
+        // SGP loop: q is double-buffered; this kernel reads buffer qsel and (SPEC) writes q + u into the other one
+        const int sel = LS ? P.ct->qsel : 0;
+        const T *qin = P.in1 + (size_t)sel * P.qbuf;
+        T *qout = SPEC ? const_cast<T *>(P.in1) + (size_t)(sel ^ 1) * P.qbuf : nullptr;
+        T *wmut = reinterpret_cast<T *>(smrow);
+        if (G.masked) epi_kl<T, L, TF, LS, true, SPEC>(P, wrow, wmut, qin, qout, t, y, j, base, plain, acc);
+        else          epi_kl<T, L, TF, LS, false, SPEC>(P, wrow, wmut, qin, qout, t, y, j, base, plain, acc);
         if (plain) return;
         block_reduce_sum<1>(acc, red);
-        const int tk = (MODE == RI_LS) ? TK_LS : TK_QJ;
+        const int tk = LS ? TK_LS : TK_QJ;
         if (publish_partials<1>(acc, P.part, bid, nblk, &P.ct->counter[tk])) {
             final_sum<1>(acc, P.part, nblk, red);
             const double J = acc[0];
             Ctrl *ct = P.ct;
-            if constexpr (MODE == RI_LS) {
+            if constexpr (LS) {
                 double gd[1];
                 final_sum<1>(gd, P.part2, gridDim.x, red);     // grad'd partials of the projection kernel
                 if (tid == 0) {
@@ -167,7 +174,9 @@ __global__ void __launch_bounds__(256, 2) row_inv_kernel(const RowParams<T> P)
                         if (isfinite(fl)) acc1 = (fl == 1.0) ? 1 : 0;
                     }
                     ct->accepted = acc1;
-                    if (acc1) finish_iteration(ct, P.o, P.tr, 1.0, J, 0);   // a10 (book-keeping; the update itself is lazy), a11
+                    // a10 (book-keeping; f is updated lazily by K3), a11.  SPEC: q(k+1) and the ratio spectrum are
+                    // already in place, so the ratio kernel of the next iteration has nothing to do.
+                    if (acc1) finish_iteration(ct, P.o, P.tr, 1.0, J, 0, SPEC ? 0 : 2);
                 }
             } else if (tid == 0) {
                 if (P.submode == QJ_INIT) {
@@ -186,6 +195,15 @@ __global__ void __launch_bounds__(256, 2) row_inv_kernel(const RowParams<T> P)
                     }
                 }
             }
+        }
+        if constexpr (SPEC) {
+            // a1 of the next iteration, speculating on lambda = 1: forward row transform of the ratio parked in shared
+            // memory by the epilogue; the spectrum row this warp read at the top is overwritten in place
+            C v[E];
+            sync();
+#pragma unroll
+            for (int e = 0; e < E; ++e) v[e] = smrow[t + TF * e];
+            fwd_fft_store<T, L>(v, smrow, t, sync, P, y, j);
         }
     } else {   // RI_RLUPDATE, a12: f <- (M_R/alpha) o f o sum_j A_j^T(g_j/(A_j f + b_j))   (Eq.1/13/21)
         double dummy[2];

@@ -27,7 +27,10 @@ struct Ctrl {
     int total_backtracks;
     int ring_len, ring_pos, nJ;
     int flag_data;         // set by the input-cleaning kernels: 1 = non-finite g, 2 = negative g (strict), 4 = negative f0
-    int pending;           // 1: the accepted step (lambda, d, u_j) has not been added to f, q_j yet (lazy update, a10)
+    int pending;           // 1: the accepted step (lambda, d) has not been added to f yet (lazy update, a10)
+    int qsel;              // which of the two q buffers holds A_j f(k): toggled by every finished iteration
+    int need_k1;           // what the ratio kernel K1 has to do: 0 = nothing (the line-search kernel already formed q(k+1), the
+                           // ratio and its row FFT at lambda = 1), 1 = ratio of the current q, 2 = q <- q + lambda u first
     double alpha;          // alpha_k of the current iteration
     double lambda;         // accepted lambda of the last completed iteration (s(k-1) = lambda d)
     double alpha_prev, tau;
@@ -120,7 +123,7 @@ __device__ inline int stop_test(const DevOpts &o, int k_done, double Jnew, doubl
 }
 
 // book-keeping after an accepted step f(k+1) = f(k) + lambda d (Alg.1 step 6), one thread
-__device__ inline void finish_iteration(Ctrl *ct, const DevOpts &o, const Trace &tr, double lambda, double Jnew, int nbt)
+__device__ inline void finish_iteration(Ctrl *ct, const DevOpts &o, const Trace &tr, double lambda, double Jnew, int nbt, int need_k1)
 {
     const int k = ct->k;
     if (tr.alpha) tr.alpha[k] = ct->alpha;
@@ -133,6 +136,8 @@ __device__ inline void finish_iteration(Ctrl *ct, const DevOpts &o, const Trace 
     ct->J = Jnew;
     ct->lambda = lambda;
     ct->pending = 1;
+    ct->qsel ^= 1;
+    ct->need_k1 = need_k1;
     ct->Jhist[(k + 1) % o.armijo_memory] = Jnew;
     if (ct->nJ < o.armijo_memory) ct->nJ++;
     ct->k = k + 1;
