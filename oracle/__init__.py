@@ -319,6 +319,10 @@ class Problem:
     def rl(self, g, b, f0=None, opts=None, **kw):
         return self._run(self.L.oracle_rl_run, g, b, f0, opts or default_options(), **kw)
 
+    def osem(self, g, b, f0=None, opts=None, **kw):
+        """Algorithm 2 (Eq.15 / Eq.22): max_iter cycles over the images; J0 only at the final iterate"""
+        return self._run(self.L.oracle_osem_run, g, b, f0, opts or default_options(), **kw)
+
 
 # ---- paper-level entry points (same argument lists as the CUDA library, host arrays) ----
 
@@ -374,6 +378,17 @@ def sgp_multi(g, psf, b, f0=None, opts=None, dtype=np.float64):
 def rl_multi(g, psf, b, f0=None, opts=None, dtype=np.float64):
     ny, nx = np.shape(g[0])
     return _entry("oracle_rl_multi", len(g), g, psf, b, f0, ny, nx, opts or default_options(), dtype)
+
+
+def osem_multi(g, psf, b, f0=None, opts=None, dtype=np.float64):
+    ny, nx = np.shape(g[0])
+    return _entry("oracle_osem_multi", len(g), g, psf, b, f0, ny, nx, opts or default_options(), dtype)
+
+
+def osem_boundary(g, psf, b, oy, ox, f0=None, opts=None, dtype=np.float64):
+    sy, sx = np.shape(g[0]); ny, nx = np.shape(psf[0])
+    return _entry("oracle_osem_boundary", len(g), g, psf, b, f0, ny, nx, opts or default_options(), dtype,
+                  boundary=(oy, ox, sy, sx))
 
 
 def sgp_boundary(g, psf, b, oy, ox, f0=None, opts=None, dtype=np.float64):

@@ -805,6 +805,65 @@ done:
 }
 
 /* ------------------------------------------------------------------------------------
+ * OSEM, Algorithm 2: h(0) = f(k); for j = 1..p
+ *   h(j) = h(j-1) o A_j^T( g_j / (A_j h(j-1) + b_j) )                         Eq.15
+ * and with boundary-effect correction
+ *   h(j) = (M_R / alpha_j) o h(j-1) o A_j^T( g_j / (A_j h(j-1) + b_j) )       Eq.22
+ * f(k+1) = h(p).  alpha_j = A_j^T 1_S (Eq.19 in reading A5; == 1 analytically when unmasked,
+ * the PSFs having unit volume).  4p transforms per iteration.  The paper stops
+ * OSEM by the reconstruction error only (needs the true object: out of scope), so the run is
+ * max_iter cycles; J0(f) of Eq.12 is evaluated once, at the final iterate.
+ * ------------------------------------------------------------------------------------ */
+int oracle_osem_run(const oracle_problem *P, const oreal *const *g_in, const oreal *const *b,
+                    const oreal *f0, const oracle_options *o, oracle_result *res, oreal *f_out)
+{
+    if (!P || !g_in || !b || !res || !f_out) return ORACLE_ERR_ARG;
+    int rc = check_options(o);
+    if (rc) return rc;
+    const int p = P->p;
+    const size_t n = P->n;
+    oreal **g = alloc_planes(p, n), **q = alloc_planes(p, n), **aj = alloc_planes(p, n);
+    oreal *h = (oreal *)calloc(n, sizeof(oreal)), *w = (oreal *)calloc(n, sizeof(oreal));
+    oreal *r = (oreal *)calloc(n, sizeof(oreal));
+    if (!g || !q || !aj || !h || !w || !r) { rc = ORACLE_ERR_ALLOC; goto done; }
+    rc = clean_data(P, g_in, o->strict, g);                           if (rc) goto done;
+    rc = make_start(P, (const oreal *const *)g, b, f0, o->init, h);   if (rc) goto done;
+    for (int j = 0; j < p; ++j) {                                     /* alpha_j on R, 0 elsewhere */
+        if (P->masked) {
+            for (size_t i = 0; i < n; ++i) r[i] = P->MS[i] ? (oreal)1 : (oreal)0;
+            rc = oracle_apply_AT(P, j, r, aj[j]);                     if (rc) goto done;
+        } else {
+            for (size_t i = 0; i < n; ++i) aj[j][i] = (oreal)1;
+        }
+    }
+    res->iterations = 0; res->stop_reason = 0; res->total_backtracks = 0;
+    res->L1_used = 0; res->L2_used = 0;
+    long fft0 = g_fft2_count;
+    for (int k = 0; k < o->max_iter; ++k) {
+        for (int j = 0; j < p; ++j) {
+            rc = oracle_apply_A(P, j, h, q[j]);                       if (rc) goto done;
+            for (size_t i = 0; i < n; ++i) r[i] = P->MS[i] ? ratio_term(g[j][i], q[j][i] + b[j][i]) : (oreal)0;
+            rc = oracle_apply_AT(P, j, r, w);                         if (rc) goto done;
+            for (size_t i = 0; i < n; ++i) h[i] = P->MR[i] ? h[i] * w[i] / aj[j][i] : (oreal)0;
+        }
+        res->iterations = k + 1;
+    }
+    res->n_fft2 = g_fft2_count - fft0;
+    res->stop_reason = ORACLE_REASON_MAXIT;
+    rc = oracle_all_A(P, h, q);                                       if (rc) goto done;
+    {
+        double J = oracle_J0(P, (const oreal *const *)q, (const oreal *const *)g, b);
+        res->J0_final = J;
+        res->discrepancy_final = 2.0 * J / ((double)p * (double)P->nS);
+        rc = isfinite(J) ? ORACLE_OK : ORACLE_ERR_NONFINITE;
+    }
+done:
+    if (h) memcpy(f_out, h, sizeof(oreal) * n);
+    free_planes(g, p); free_planes(q, p); free_planes(aj, p); free(h); free(w); free(r);
+    return rc;
+}
+
+/* ------------------------------------------------------------------------------------
  * Paper-level entry points: marshal (g, K, b, f0) onto the S-bar grid and run.
  * ------------------------------------------------------------------------------------ */
 typedef int (*run_fn)(const oracle_problem *, const oreal *const *, const oreal *const *,
@@ -890,5 +949,22 @@ int oracle_rl_boundary(int p, const oreal *const *g, const oreal *const *psf,
                        oracle_result *res)
 {
     return run_generic(oracle_rl_run, p, g, psf, b_arr, b_const, 1, oy, ox, sy, sx, ny, nx, f0, f_out,
+                       maskR_out, dtype, o, res);
+}
+int oracle_osem_multi(int p, const oreal *const *g, const oreal *const *psf,
+                      const oreal *const *b_arr, const double *b_const, const oreal *f0,
+                      oreal *f_out, int ny, int nx, int dtype, const oracle_options *o,
+                      oracle_result *res)
+{
+    return run_generic(oracle_osem_run, p, g, psf, b_arr, b_const, 0, 0, 0, ny, nx, ny, nx, f0, f_out,
+                       NULL, dtype, o, res);
+}
+int oracle_osem_boundary(int p, const oreal *const *g, const oreal *const *psf,
+                         const oreal *const *b_arr, const double *b_const, int oy, int ox, int sy,
+                         int sx, int ny, int nx, const oreal *f0, oreal *f_out,
+                         unsigned char *maskR_out, int dtype, const oracle_options *o,
+                         oracle_result *res)
+{
+    return run_generic(oracle_osem_run, p, g, psf, b_arr, b_const, 1, oy, ox, sy, sx, ny, nx, f0, f_out,
                        maskR_out, dtype, o, res);
 }

@@ -138,6 +138,9 @@ int oracle_sgp_run(const oracle_problem *P, const oreal *const *g, const oreal *
                    const oreal *f0, const oracle_options *o, oracle_result *res, oreal *f_out);
 int oracle_rl_run(const oracle_problem *P, const oreal *const *g, const oreal *const *b,
                   const oreal *f0, const oracle_options *o, oracle_result *res, oreal *f_out);
+/* OSEM, Algorithm 2 / Eq.15 / Eq.22: max_iter cycles over the p images; J0 evaluated at the end only */
+int oracle_osem_run(const oracle_problem *P, const oreal *const *g, const oreal *const *b,
+                    const oreal *f0, const oracle_options *o, oracle_result *res, oreal *f_out);
 
 /* ---- the paper-level entry points (SURVEY.md 8(b) signatures, host pointers) ---- */
 int oracle_sgp_single(const oreal *g, const oreal *psf, const oreal *b_arr, double b_const,
@@ -165,6 +168,16 @@ int oracle_rl_boundary(int p, const oreal *const *g, const oreal *const *psf,
                        int sx, int ny, int nx, const oreal *f0, oreal *f_out,
                        unsigned char *maskR_out, int dtype, const oracle_options *o,
                        oracle_result *res);
+
+int oracle_osem_multi(int p, const oreal *const *g, const oreal *const *psf,
+                      const oreal *const *b_arr, const double *b_const, const oreal *f0,
+                      oreal *f_out, int ny, int nx, int dtype, const oracle_options *o,
+                      oracle_result *res);
+int oracle_osem_boundary(int p, const oreal *const *g, const oreal *const *psf,
+                         const oreal *const *b_arr, const double *b_const, int oy, int ox, int sy,
+                         int sx, int ny, int nx, const oreal *f0, oreal *f_out,
+                         unsigned char *maskR_out, int dtype, const oracle_options *o,
+                         oracle_result *res);
 
 #ifdef __cplusplus
 }

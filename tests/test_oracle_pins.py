@@ -528,6 +528,85 @@ def test_P11_fft_count(p):
 
 
 # ---------------------------------------------------------------------------------- entry points
+# ---------------------------------------------------------------------------------- P12 (OSEM, Algorithm 2)
+def _dense_operator(k, ny, nx, MS, MR):
+    """the matrix of A_j written out from Eq.16: A[m, n] = M_S(m) K_j(m - n) M_R(n), K_j normalised, periodic, centre at ny/2, nx/2"""
+    K0 = np.fft.ifftshift(k / k.sum())
+    A = np.zeros((ny * nx, ny * nx))
+    for my, mx in itertools.product(range(ny), range(nx)):
+        if not MS[my, mx]:
+            continue
+        for qy, qx in itertools.product(range(ny), range(nx)):
+            if MR[qy, qx]:
+                A[my * nx + mx, qy * nx + qx] = K0[(my - qy) % ny, (mx - qx) % nx]
+    return A
+
+
+@pytest.mark.parametrize("p,masked,S", [(2, False, None), (3, False, None), (2, True, (1, 2, 6, 5))])
+def test_P12_osem_cycle_is_eq15_eq22_written_out_with_dense_matrices(p, masked, S):
+    """PAPER.md:178-191 (Algorithm 2, Eq.15) and :246 (Eq.22): the cycle over the images written with dense matrices
+    built from the definition of A_j (Eq.16), its transpose, and alpha_j = A_j^T 1_S: h <- (M_R/alpha_j) h o A_j^T(g_j/(A_j h + b_j)),
+    j = 1..p in this order, each sub-step seeing the previous one's h."""
+    rng = np.random.default_rng(120 + p)
+    ny, nx = 8, 7
+    P, g, b, truth, MS = _tiny_problem(ny, nx, p, masked, rng, S=S)
+    info = P.info()
+    MR = info["MR"].astype(bool)
+    f0 = (1.0 + 20 * rng.random((ny, nx))) * MR
+    K = 3
+    f_or, res = P.osem(g, b, f0, oracle.default_options(max_iter=K, init=oracle.INIT_USER))
+    mats = [_dense_operator(k, ny, nx, MS, MR) for k in P.psfs] if hasattr(P, "psfs") else None
+    if mats is None:
+        pytest.skip("Problem does not keep its PSFs")
+    h = f0.ravel().copy()
+    ones_S = MS.ravel().astype(float)
+    for _ in range(K):
+        for j in range(p):
+            A = mats[j]
+            aj = A.T @ ones_S
+            r = np.where(MS.ravel() > 0, g[j].ravel() / (A @ h + b[j].ravel()), 0.0)
+            h = np.where(MR.ravel(), h * (A.T @ r) / np.where(MR.ravel(), aj, 1.0), 0.0)
+    assert np.abs(f_or.ravel() - h).max() <= 1e-11 * np.abs(h).max()
+    assert res.iterations == K and res.n_fft2 == 4 * p * K          # "4p FFTs" per OSEM iteration, PAPER.md:208
+    # the order of the cycle matters (so the pin would catch a reversed or simultaneous update)
+    h2 = f0.ravel().copy()
+    for _ in range(K):
+        for j in reversed(range(p)):
+            A = mats[j]
+            aj = A.T @ ones_S
+            r = np.where(MS.ravel() > 0, g[j].ravel() / (A @ h2 + b[j].ravel()), 0.0)
+            h2 = np.where(MR.ravel(), h2 * (A.T @ r) / np.where(MR.ravel(), aj, 1.0), 0.0)
+    assert np.abs(h2 - h).max() > 1e-6 * np.abs(h).max()
+    # J0 reported at the final iterate is Eq.12 there
+    q = [mats[j] @ h for j in range(p)]
+    J = sum(float(np.sum(np.where(MS.ravel() > 0, np.where(g[j].ravel() > 0, g[j].ravel() * np.log(np.where(g[j].ravel() > 0, g[j].ravel(), 1.0) / (q[j] + b[j].ravel())), 0.0) + q[j] + b[j].ravel() - g[j].ravel(), 0.0))) for j in range(p))
+    assert abs(res.J0_final - J) <= 1e-10 * abs(J)
+
+
+@pytest.mark.parametrize("masked,S", [(False, None), (True, (2, 2, 8, 8))])
+def test_P12_osem_with_one_image_is_RL_and_substeps_conserve_flux(masked, S):
+    """p = 1: Algorithm 2 is Eq.1 / Eq.21.  b = 0: every sub-step j conserves sum_R alpha_j h(j) = sum_S g_j
+    (the argument of PAPER.md:33 applied to image j), so after a full cycle the flux is that of the LAST image."""
+    rng = np.random.default_rng(12)
+    P, g, b, truth, MS = _tiny_problem(12, 12, 1, masked, rng, S=S)
+    o = oracle.default_options(max_iter=5)
+    f_rl, r_rl = P.rl(g, b, opts=o)
+    f_os, r_os = P.osem(g, b, opts=o)
+    assert np.abs(f_rl - f_os).max() <= 1e-13 * np.abs(f_rl).max() and abs(r_os.J0_final - r_rl.J0_final) <= 1e-12 * r_rl.J0_final
+    p = 3
+    psfs = [_rand_psf(12, 12, rng, 1.0 + 0.5 * j) for j in range(p)]
+    P3 = oracle.Problem(psfs, masked=masked, S=S, sigma_R=0.02)
+    oy, ox, sy, sx = P3.S
+    M = np.zeros((12, 12)); M[oy:oy + sy, ox:ox + sx] = 1
+    g3 = [rng.poisson(20 + 60 * (j + 1) * rng.random((12, 12))) * M for j in range(p)]
+    b0 = [np.zeros((12, 12)) for _ in range(p)]
+    f, _ = P3.osem(g3, b0, opts=oracle.default_options(max_iter=4))
+    alpha_last = P3.AT(p - 1, M)
+    assert np.isclose((alpha_last * f).sum(), g3[-1].sum(), rtol=1e-12)
+    assert not np.isclose((alpha_last * f).sum(), g3[0].sum(), rtol=1e-3)
+    assert np.all(f >= 0)
+
+
 def test_entry_points_match_problem_api():
     w = synth.c3_boundary(24, 32, n_stars=30)
     o = oracle.default_options(max_iter=15)
