@@ -60,7 +60,7 @@ typedef enum { SGP_FFT_NATIVE = 0, SGP_FFT_CUFFT = 1 } sgp_backend;
 /* problem kind of a plan */
 typedef enum { SGP_KIND_SINGLE = 0, SGP_KIND_MULTI = 1, SGP_KIND_BOUNDARY = 2 } sgp_kind;
 /* algorithm run by sgp_plan_run */
-typedef enum { SGP_ALG_SGP = 0, SGP_ALG_RL = 1 } sgp_algorithm;
+typedef enum { SGP_ALG_SGP = 0, SGP_ALG_RL = 1, SGP_ALG_OSEM = 2 } sgp_algorithm;
 
 typedef enum {
     SGP_OK = 0,
@@ -185,6 +185,19 @@ int rl_boundary(int p, const void *const *g, const void *const *psf, const void 
                 const double *b_const, int oy, int ox, int sy, int sx, int ny, int nx,
                 const void *f0, void *f_out, unsigned char *maskR_out, int dtype,
                 const sgp_options *opt, sgp_result *res, void *stream);
+/* OSEM, Algorithm 2 of the paper: one iteration is a cycle over the p images,
+ *   h <- h o A_j^T( g_j / (A_j h + b_j) ), j = 1..p (Eq.15);  boundary form: h <- (M_R/alpha_j) o h o ... (Eq.22),
+ * 4p two-dimensional FFTs per iteration, on the kernels of rl_*.  Same arguments as rl_multi /
+ * rl_boundary (device pointers).  opt->max_iter cycles are run: stop_rule must be SGP_STOP_MAXIT (the paper stops
+ * OSEM by the reconstruction error, which needs the true object), else SGP_ERR_UNSUPPORTED.  J0 (Eq.12) is evaluated
+ * once, at the final iterate (res->J0_final); no per-iteration traces.  (sgp_plan_run takes SGP_ALG_OSEM as well.) */
+int osem_multi(int p, const void *const *g, const void *const *psf, const void *const *b_arr,
+               const double *b_const, const void *f0, void *f_out, int ny, int nx, int dtype,
+               const sgp_options *opt, sgp_result *res, void *stream);
+int osem_boundary(int p, const void *const *g, const void *const *psf, const void *const *b_arr,
+                  const double *b_const, int oy, int ox, int sy, int sx, int ny, int nx,
+                  const void *f0, void *f_out, unsigned char *maskR_out, int dtype,
+                  const sgp_options *opt, sgp_result *res, void *stream);
 
 /* ---- the same six calls with HOST pointers (copies inside the call; what bench.py times as e2e) -- */
 int sgp_single_host(const void *g, const void *psf, const void *b_arr, double b_const, const void *f0,

@@ -21,13 +21,14 @@ STOP_MAXIT, STOP_RELJ, STOP_DISCREPANCY = 0, 1, 2
 INIT_USER, INIT_CONST, INIT_ZERO, INIT_G = 0, 1, 2, 3
 PSF_CENTER, PSF_CORNER = 0, 1
 KIND_SINGLE, KIND_MULTI, KIND_BOUNDARY = 0, 1, 2
-ALG_SGP, ALG_RL = 0, 1
+ALG_SGP, ALG_RL, ALG_OSEM = 0, 1, 2
 OK, ERR_ARG, ERR_PSF, ERR_DATA, ERR_ALLOC, ERR_CUDA, ERR_LINESEARCH, ERR_NONFINITE, ERR_UNSUPPORTED = 0, -1, -2, -3, -4, -5, -6, -7, -8
 REASON = {0: "none", 1: "maxit", 2: "relJ", 3: "discrepancy"}
 
 EXPORTS = [
     "sgp_options_default", "sgp_result_init", "sgp_strerror", "sgp_version", "sgp_last_cuda_error", "sgp_workspace_bytes",
     "sgp_single", "sgp_multi", "sgp_boundary", "rl_single", "rl_multi", "rl_boundary",
+    "osem_multi", "osem_boundary",
     "sgp_single_host", "sgp_multi_host", "sgp_boundary_host", "rl_single_host", "rl_multi_host", "rl_boundary_host",
     "sgp_plan_create", "sgp_plan_set_psf", "sgp_plan_run", "sgp_plan_apply_A", "sgp_plan_apply_AT", "sgp_plan_get_mask",
     "sgp_plan_rfft2", "sgp_plan_irfft2", "sgp_plan_set_profiling", "sgp_plan_get_kernel_ms", "sgp_plan_destroy",
@@ -267,6 +268,9 @@ class Plan:
     def rl(self, g, b, **kw):
         return self.run(ALG_RL, g, b, **kw)
 
+    def osem(self, g, b, **kw):
+        return self.run(ALG_OSEM, g, b, **kw)
+
     def set_profiling(self, on: bool):
         rc = lib().sgp_plan_set_profiling(self.h, int(bool(on)))
         if rc != OK:
@@ -400,3 +404,11 @@ def sgp_boundary(g, psf, b, oy, ox, f0=None, opts=None, host=False, check=True, 
 
 def rl_boundary(g, psf, b, oy, ox, f0=None, opts=None, host=False, check=True, f_out=None):
     return _one_shot("rl_boundary", g, psf, b, f0, opts, boundary=(oy, ox), host=host, check=check, f_out=f_out)
+
+
+def osem_multi(g, psf, b, f0=None, opts=None, check=True, f_out=None):
+    return _one_shot("osem_multi", g, psf, b, f0, opts, check=check, f_out=f_out)
+
+
+def osem_boundary(g, psf, b, oy, ox, f0=None, opts=None, check=True, f_out=None):
+    return _one_shot("osem_boundary", g, psf, b, f0, opts, boundary=(oy, ox), check=check, f_out=f_out)

@@ -74,7 +74,7 @@ size_t workspace_bytes(int kind, int p, int ny, int nx, int dtype)
     const size_t n = (size_t)ny * nx;
     size_t planes = 7 * (size_t)p + 4;                 // khat, spec, g, b, q (two buffers), u per image; f, grad, d, scratch
     size_t b = planes * n * r;
-    if (kind == SGP_KIND_BOUNDARY) b += 2 * n * r + n;
+    if (kind == SGP_KIND_BOUNDARY) b += (2 + (size_t)p) * n * r + n;     // alphaR, alpha, alpha_j on R (OSEM, Eq.22), M_R
     b += ((size_t)nx + 1 + 2 * (size_t)ny + (size_t)ny * p) * 2 * r;   // twiddles, pack line, khatB
     b += (size_t)(ny * (6 + 2 * p) + 1024 * p + 2048) * sizeof(double) + sizeof(Ctrl);
     return b;
@@ -274,6 +274,18 @@ int rl_boundary(int p, const void *const *g, const void *const *psf, const void 
                 int dtype, const sgp_options *opt, sgp_result *res, void *stream)
 {
     return one_shot(SGP_ALG_RL, SGP_KIND_BOUNDARY, p, g, psf, b_arr, b_const, oy, ox, sy, sx, ny, nx, f0, f_out, maskR_out, dtype, opt, res, stream);
+}
+
+int osem_multi(int p, const void *const *g, const void *const *psf, const void *const *b_arr, const double *b_const,
+               const void *f0, void *f_out, int ny, int nx, int dtype, const sgp_options *opt, sgp_result *res, void *stream)
+{
+    return one_shot(SGP_ALG_OSEM, SGP_KIND_MULTI, p, g, psf, b_arr, b_const, 0, 0, ny, nx, ny, nx, f0, f_out, nullptr, dtype, opt, res, stream);
+}
+int osem_boundary(int p, const void *const *g, const void *const *psf, const void *const *b_arr, const double *b_const,
+                  int oy, int ox, int sy, int sx, int ny, int nx, const void *f0, void *f_out, unsigned char *maskR_out,
+                  int dtype, const sgp_options *opt, sgp_result *res, void *stream)
+{
+    return one_shot(SGP_ALG_OSEM, SGP_KIND_BOUNDARY, p, g, psf, b_arr, b_const, oy, ox, sy, sx, ny, nx, f0, f_out, maskR_out, dtype, opt, res, stream);
 }
 
 // ---- host-pointer variants: stage through device buffers (pinned staging is the caller's choice)

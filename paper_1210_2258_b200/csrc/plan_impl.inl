@@ -13,12 +13,14 @@ template <typename T> struct PlanImpl : PlanBase {
     size_t row_smem = 0, col_smem = 0;
     row_kernel_t<T> k_rowf[RF_NMODES] = {nullptr}, k_rowi[RI_NMODES] = {nullptr};
     col_kernel_t<T> k_colf = nullptr, k_conj = nullptr, k_mult = nullptr;
+    col_kernel_t<T> k_conj1 = nullptr, k_mult1 = nullptr;      // single-image forms (OSEM sub-steps, A_j / A_j^T alone)
     // device memory
     std::vector<void *> allocs;
     C *tw_r = nullptr, *tw_h = nullptr, *tw_c = nullptr, *pack = nullptr;
     C *khat = nullptr, *khatB = nullptr, *spec = nullptr;
     T *Gp = nullptr, *Bp = nullptr, *q = nullptr, *u = nullptr, *f = nullptr, *grad = nullptr, *d = nullptr;
     T *alphaR = nullptr, *alpha = nullptr, *scratch = nullptr;
+    T *alphaJ = nullptr;           // boundary problems: alpha_j on R, 0 elsewhere, p planes (OSEM, Eq.22)
     unsigned char *MR = nullptr;
     double *part_bb = nullptr, *part_gd = nullptr, *part_J = nullptr, *part_bt = nullptr, *part_misc = nullptr;
     Ctrl *ct = nullptr;
@@ -104,7 +106,8 @@ template <typename T> struct PlanImpl : PlanBase {
         for (int m = 0; m < RI_NMODES; ++m) if (!(k_rowi[m] = get_row_inv<T>(Lr, m))) return SGP_ERR_ARG;
         const bool multi = p > 1;
         k_colf = get_col<T>(Lc, CM_FWD, false); k_conj = get_col<T>(Lc, CM_CONJSUM, multi); k_mult = get_col<T>(Lc, CM_MULT, multi);
-        if (!k_colf || !k_conj || !k_mult) return SGP_ERR_ARG;
+        k_conj1 = get_col<T>(Lc, CM_CONJSUM, false); k_mult1 = get_col<T>(Lc, CM_MULT, false);
+        if (!k_colf || !k_conj || !k_mult || !k_conj1 || !k_mult1) return SGP_ERR_ARG;
         int Cc = 0, RB = 0;
         int rc = choose_tiles(ny, nx, dtype, &opt, &Cc, &RB);
         if (rc) return rc;
@@ -122,6 +125,8 @@ template <typename T> struct PlanImpl : PlanBase {
         SGP_CUDA_TRY(cudaFuncSetAttribute((const void *)k_colf, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)col_smem));
         SGP_CUDA_TRY(cudaFuncSetAttribute((const void *)k_conj, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)col_smem));
         SGP_CUDA_TRY(cudaFuncSetAttribute((const void *)k_mult, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)col_smem));
+        SGP_CUDA_TRY(cudaFuncSetAttribute((const void *)k_conj1, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)col_smem));
+        SGP_CUDA_TRY(cudaFuncSetAttribute((const void *)k_mult1, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)col_smem));
         // grid of the backtracking kernel: all CTAs resident together (it synchronises grid-wide, aux.cuh)
         int dev = 0, per_sm = 0;
         SGP_CUDA_TRY(cudaGetDevice(&dev));
@@ -193,6 +198,7 @@ template <typename T> struct PlanImpl : PlanBase {
             if ((rc = dalloc(&alphaR, n))) return rc;
             if ((rc = dalloc(&alpha, n))) return rc;
             if ((rc = dalloc(&MR, n))) return rc;
+            if ((rc = dalloc(&alphaJ, n * p))) return rc;
         }
         if ((rc = dalloc(&part_bb, (size_t)nrb * 4))) return rc;
         if ((rc = dalloc(&part_gd, (size_t)nrb))) return rc;
@@ -293,9 +299,14 @@ template <typename T> struct PlanImpl : PlanBase {
                 if ((rc = launch_row(k_rowi[RI_PLAIN], R, 1, st))) return rc;
                 alpha_accum_kernel<T><<<ew_grid(n), 256, 0, st>>>(scratch, alpha, MR, n, opt.sigma_R, j == 0);
                 launches++;
+                SGP_CUDA_TRY(cudaMemcpyAsync(alphaJ + (size_t)j * n, scratch, n * sizeof(T), cudaMemcpyDeviceToDevice, st));
             }
             alpha_finish_kernel<T><<<ew_grid(n), 256, 0, st>>>(alpha, MR, alphaR, n);
             launches++;
+            for (int j = 0; j < p; ++j) {     // alpha_j restricted to R (R needs all the alpha_j, Eq.20), in place
+                alpha_finish_kernel<T><<<ew_grid(n), 256, 0, st>>>(alphaJ + (size_t)j * n, MR, alphaJ + (size_t)j * n, n);
+                launches++;
+            }
             SGP_CUDA_TRY(cudaGetLastError());
             std::vector<unsigned char> hm(n);
             SGP_CUDA_TRY(cudaMemcpyAsync(hm.data(), MR, n, cudaMemcpyDeviceToHost, st));
@@ -387,6 +398,7 @@ template <typename T> struct PlanImpl : PlanBase {
     int ensure_trace(int max_iter, const sgp_result *res, Trace *tr, cudaStream_t st);
     int enqueue_sgp_iteration(const RowParams<T> &Pbase, const DevOpts &o, const Trace &tr, const double *bconst, int b_is_array, cudaStream_t st);
     int enqueue_rl_round(const DevOpts &o, const Trace &tr, const double *bconst, int b_is_array, cudaStream_t st);
+    int enqueue_osem_cycle(const DevOpts &o, const Trace &tr, const double *bconst, int b_is_array, cudaStream_t st);
     int enqueue_many(int algorithm, int count, const RowParams<T> &Pb, const DevOpts &o, const Trace &tr, const double *bconst,
                      int b_is_array, cudaStream_t st);
 };

@@ -118,7 +118,42 @@ int PlanImpl<T>::enqueue_rl_round(const DevOpts &o, const Trace &tr, const doubl
     return SGP_OK;
 }
 
-// `count` iterations (SGP) or rounds (RL).  With opt.use_graph the launches of kGraphIters iterations are captured
+// One OSEM iteration (Algorithm 2): for j = 1..p, h <- (M_R/alpha_j) o h o A_j^T(g_j / (A_j h + b_j))
+// (Eq.15; Eq.22 with boundary-effect correction): the six launches of an RL round restricted to image j -- the
+// single-image column kernels with K^_j, scaling 1 instead of 1/p (Geom::p = 1), alpha_j on R in place of alpha.
+// 4p two-dimensional FFTs.  h lives in f.
+template <typename T>
+int PlanImpl<T>::enqueue_osem_cycle(const DevOpts &o, const Trace &tr, const double *bconst, int b_is_array, cudaStream_t st)
+{
+    int rc;
+    RowParams<T> Pb = row_params();
+    Pb.o = o; Pb.tr = tr; Pb.check_status = 1; Pb.b_is_array = b_is_array;
+    Pb.G.p = 1;
+    for (int j = 0; j < p; ++j) {
+        const size_t off = (size_t)j * n;
+        Pb.bconst[0] = bconst[j];
+        Pb.alphaR = G.masked ? alphaJ + off : nullptr;
+        ColParams<T> Qb = col_params();
+        Qb.check_status = 1; Qb.p = 1; Qb.khat = khat + (size_t)j * nspec; Qb.khatB = khatB + (size_t)j * ny;
+        cur_slot = SGP_PROF_R1;
+        { RowParams<T> P = Pb; P.in0 = f; P.maskmode = MM_NONE; if ((rc = launch_row(k_rowf[RF_PLAIN], P, 1, st))) return rc; }
+        cur_slot = SGP_PROF_R2;
+        if ((rc = launch_col(k_mult1, Qb, st))) return rc;
+        cur_slot = SGP_PROF_R3;
+        { RowParams<T> P = Pb; P.submode = QJ_PLAIN; P.in0 = Gp + off; P.in2 = Bp + off; P.out0 = q + off; P.part = part_J;
+          if ((rc = launch_row(k_rowi[RI_QJ], P, 1, st))) return rc; }
+        cur_slot = SGP_PROF_R4;
+        { RowParams<T> P = Pb; P.in0 = Gp + off; P.in1 = q + off; P.in2 = Bp + off; if ((rc = launch_row(k_rowf[RF_RATIO], P, 1, st))) return rc; }
+        cur_slot = SGP_PROF_R5;
+        if ((rc = launch_col(k_conj1, Qb, st))) return rc;
+        cur_slot = SGP_PROF_R6;
+        { RowParams<T> P = Pb; P.in0 = f; P.out0 = f; if ((rc = launch_row(k_rowi[RI_RLUPDATE], P, 1, st))) return rc; }
+    }
+    cur_slot = -1;
+    return SGP_OK;
+}
+
+// `count` iterations (SGP), rounds (RL) or cycles (OSEM).  With opt.use_graph the launches of kGraphIters iterations are captured
 // once per run into a CUDA graph (on a stream of the plan: the caller's may be the legacy default stream, which
 // cannot be captured) and the graph is replayed; everything the kernels branch on lives in the control block, so
 // the launch parameters of all iterations are identical.
@@ -129,7 +164,8 @@ int PlanImpl<T>::enqueue_many(int algorithm, int count, const RowParams<T> &Pb, 
     int rc;
     auto one = [&](cudaStream_t s) -> int {
         return algorithm == SGP_ALG_SGP ? enqueue_sgp_iteration(Pb, o, tr, bconst, b_is_array, s)
-                                        : enqueue_rl_round(o, tr, bconst, b_is_array, s);
+             : algorithm == SGP_ALG_RL  ? enqueue_rl_round(o, tr, bconst, b_is_array, s)
+                                        : enqueue_osem_cycle(o, tr, bconst, b_is_array, s);
     };
     constexpr int kGraphIters = 10;
     if ((opt.use_graph & 1) && !profiling && count >= kGraphIters) {
@@ -160,11 +196,12 @@ int PlanImpl<T>::run(int algorithm, const void *const *g, const void *const *b_a
 {
     if (!psf_set || !g || !f_out || !res) return SGP_ERR_ARG;
     if (!b_arr && !b_const) return SGP_ERR_ARG;
-    if (algorithm != SGP_ALG_SGP && algorithm != SGP_ALG_RL) return SGP_ERR_ARG;
+    if (algorithm != SGP_ALG_SGP && algorithm != SGP_ALG_RL && algorithm != SGP_ALG_OSEM) return SGP_ERR_ARG;
     sgp_options ro = ropt ? *ropt : opt;
     int rc = validate_options(&ro);
     if (rc) return rc;
     if (ro.refresh_every != 0) return SGP_ERR_UNSUPPORTED;
+    if (algorithm == SGP_ALG_OSEM && ro.stop_rule != SGP_STOP_MAXIT) return SGP_ERR_UNSUPPORTED;   // include/sgp.h: osem_*
     if (ro.init == SGP_INIT_USER && !f0) return SGP_ERR_ARG;
     for (int j = 0; j < p; ++j) if (!g[j]) return SGP_ERR_ARG;
     int b_is_array = 0;
@@ -251,6 +288,31 @@ int PlanImpl<T>::run(int algorithm, const void *const *g, const void *const *b_a
                 if (status == 0 && done >= ro.max_iter) status = SGP_REASON_MAXIT;   // not reachable: the device sets it
             }
             fft2 = (long)h.k * (2 * p + 2);
+        } else if (algorithm == SGP_ALG_OSEM) {
+            // max_iter cycles, then J0 (Eq.12) at the final iterate: q_j = A_j f for all j, as in the start-point phase
+            int done = 0;
+            while (status == 0 && done < ro.max_iter) {
+                int todo = ro.max_iter - done; if (todo > chunk) todo = chunk;
+                if ((rc = enqueue_many(algorithm, todo, Pb, o, tr, bconst, b_is_array, st))) return rc;
+                done += todo;
+                SGP_CUDA_TRY(cudaMemcpyAsync(&h, ct, sizeof(Ctrl), cudaMemcpyDeviceToHost, st));
+                SGP_CUDA_TRY(cudaStreamSynchronize(st));
+                status = h.status;
+            }
+            fft2 = (long)done * 4 * p;
+            if (status == 0) {
+                Trace t0 = tr; t0.J = nullptr;
+                RowParams<T> Pj = Pb; Pj.tr = t0;
+                { RowParams<T> P = Pj; P.in0 = f; if ((rc = launch_row(k_rowf[RF_PLAIN], P, 1, st))) return rc; }
+                { ColParams<T> Q = col_params(); Q.check_status = 1; if ((rc = launch_col(k_mult, Q, st))) return rc; }
+                { RowParams<T> P = Pj; P.submode = QJ_INIT; P.in0 = Gp; P.in2 = Bp; P.out0 = q; P.part = part_J;
+                  if ((rc = launch_row(k_rowi[RI_QJ], P, p, st))) return rc; }
+                SGP_CUDA_TRY(cudaMemcpyAsync(&h, ct, sizeof(Ctrl), cudaMemcpyDeviceToHost, st));
+                SGP_CUDA_TRY(cudaStreamSynchronize(st));
+                status = h.status;
+                h.k = done;
+                if (status == 0) status = SGP_REASON_MAXIT;
+            }
         } else {
             int rounds = 0;     // round k evaluates J0(f(k)) and, unless a rule fires, makes update k+1
             while (status == 0) {

@@ -445,3 +445,51 @@ def test_full_size_workloads_match_the_oracle(cfg, iters, force):
     assert np.max(np.abs(rg.J - np.asarray(ro.J)) / np.abs(np.asarray(ro.J))) <= 1e-4
     assert np.array_equal(rg.backtracks, np.asarray(ro.backtracks)[:iters])
     assert (fg >= 0).all()
+
+
+# ---------------------------------------------------------------- OSEM (Algorithm 2)
+@pytest.mark.parametrize("dt,tol", [(np.float32, 1e-4), (np.float64, 1e-11)])
+@pytest.mark.parametrize("cfg,kw", [("C2", {"n": 128}), ("C2", {"n": 256, "p": 2}), ("C3", {"s": 256, "sbar": 320, "n_stars": 150, "fwhm": 64.0})])
+def test_osem_parity(cfg, kw, dt, tol):
+    """OSEM cycles (Eq.15; Eq.22 with the boundary weights M_R/alpha_j) against the oracle: 12 cycles, graph replay
+    of 10 plus 2 plain; whole image and J0 at the final iterate.  Multiplicative updates: no branch, tight tolerance."""
+    _need_gpu()
+    w = synth.make(cfg, **kw)
+    if cfg == "C3":       # a second, different PSF so that the cycle has more than one image also with masks
+        w2 = synth.make(cfg, **{**kw, "seed_idx": 13, "fwhm": 40.0})
+        w["psf"] = [w["psf"][0], w2["psf"][0]]; w["g"] = [w["g"][0], w2["g"][0]]; w["b"] = [w["b"][0], w2["b"][0]]
+    iters = 12
+    plan, o = gpu_plan(w, dt, max_iter=iters, stop_rule=0)
+    g = [dev(a, dt) for a in w["g"]]
+    fg, rg = plan.osem(g, w["b"], opts=o)
+    torch.cuda.synchronize()
+    plan.close()
+    oo = oracle_opts(w, max_iter=iters, stop_rule=0)
+    P = oracle_problem(w, oo)
+    ge = P.embed(w["g"]); be = [np.full((P.ny, P.nx), float(v)) for v in w["b"]]
+    fo, ro = P.osem(ge, be, opts=oo)
+    assert rg.iterations == ro.iterations == iters and rg.stop_reason == 1
+    assert rg.n_fft2 == ro.n_fft2 == 4 * len(w["g"]) * iters
+    if dt == np.float32:
+        # fp32 tolerance from the arithmetic (DESIGN.md 3a): 3 x the deviation of the oracle's own float build over the
+        # same 12 p multiplicative updates (the boundary weights 1/alpha_j, alpha_j >= sigma_R, amplify rounding near the rim of R)
+        P32 = oracle.Problem(w["psf"], masked=w["S"] is not None, S=w["S"], sigma_R=oo.sigma_R, dtype=np.float32)
+        f32, _ = P32.osem(P32.embed(w["g"]), [np.full((P.ny, P.nx), float(v)) for v in w["b"]], opts=oo)
+        tol = max(tol, 3.0 * rel_l2(f32, fo))
+    assert rel_l2(fg.cpu().numpy(), fo) <= tol
+    assert abs(rg.J0_final - ro.J0_final) <= max(tol, 1e-6 if dt == np.float32 else 0) * abs(ro.J0_final)
+    assert (fg >= 0).all()
+
+
+def test_osem_one_shot_and_unsupported_stop_rule():
+    _need_gpu()
+    w = synth.make("C2", n=128)
+    g = [dev(a, np.float32) for a in w["g"]]; k = [dev(a, np.float32) for a in w["psf"]]
+    o = B.default_options(**{**w["opts"], "max_iter": 5, "stop_rule": 0})
+    f1, r1 = B.osem_multi(g, k, w["b"], opts=o)
+    plan, _ = gpu_plan(w, np.float32, max_iter=5, stop_rule=0)
+    f2, r2 = plan.osem(g, w["b"], opts=o)
+    plan.close()
+    assert torch.equal(f1, f2) and r1.J0_final == r2.J0_final and r1.iterations == 5
+    _, r = B.osem_multi(g, k, w["b"], opts=B.default_options(**{**w["opts"], "max_iter": 5, "stop_rule": 2}), check=False)
+    assert r.rc == B.ERR_UNSUPPORTED
