@@ -289,22 +289,30 @@ int osem_boundary(int p, const void *const *g, const void *const *psf, const voi
 }
 
 // ---- host-pointer variants: stage through device buffers (pinned staging is the caller's choice)
-struct DevBufs {
-    std::vector<void *> bufs;
-    ~DevBufs() { for (void *b : bufs) cudaFree(b); }
-    int up(const void *host, size_t bytes, cudaStream_t st, void **dev)
+struct DevBufs {      // one device allocation, carved into 256-byte aligned pieces
+    unsigned char *base = nullptr;
+    size_t cap = 0, used = 0;
+    ~DevBufs() { cudaFree(base); }
+    static size_t al(size_t b) { return (b + 255) & ~(size_t)255; }
+    int reserve(size_t bytes)
     {
-        *dev = nullptr;
-        if (!host) return SGP_OK;
-        SGP_CUDA_TRY(cudaMalloc(dev, bytes));
-        bufs.push_back(*dev);
-        SGP_CUDA_TRY(cudaMemcpyAsync(*dev, host, bytes, cudaMemcpyHostToDevice, st));
+        SGP_CUDA_TRY(cudaMalloc((void **)&base, bytes ? bytes : 256));
+        cap = bytes;
         return SGP_OK;
     }
     int blank(size_t bytes, void **dev)
     {
-        SGP_CUDA_TRY(cudaMalloc(dev, bytes));
-        bufs.push_back(*dev);
+        if (used + al(bytes) > cap) return SGP_ERR_ALLOC;
+        *dev = base + used; used += al(bytes);
+        return SGP_OK;
+    }
+    int up(const void *host, size_t bytes, cudaStream_t st, void **dev)
+    {
+        *dev = nullptr;
+        if (!host) return SGP_OK;
+        int rc = blank(bytes, dev);
+        if (rc) return rc;
+        SGP_CUDA_TRY(cudaMemcpyAsync(*dev, host, bytes, cudaMemcpyHostToDevice, st));
         return SGP_OK;
     }
 };
@@ -323,6 +331,7 @@ static int host_shot(int algorithm, int kind, int p, const void *const *g, const
     const void *dg[SGP_MAX_IMAGES], *dk[SGP_MAX_IMAGES], *db[SGP_MAX_IMAGES];
     int rc;
     bool have_b = false;
+    if ((rc = D.reserve((size_t)p * (2 * DevBufs::al(sb) + DevBufs::al(nb)) + 2 * DevBufs::al(nb) + DevBufs::al((size_t)ny * nx)))) return rc;
     for (int j = 0; j < p; ++j) {
         if (!g[j] || !psf[j]) return SGP_ERR_ARG;
         void *t;

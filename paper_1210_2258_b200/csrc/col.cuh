@@ -209,4 +209,70 @@ __global__ void __launch_bounds__(fft_E_col<T>(L) == 32 ? 256 : 512, 1) col_kern
     }
 }
 
+// ---------------------------------------------------------------------------------------------------------------
+// Second form of the column pass for single-image problems (CM_CONJSUM / CM_MULT with p = 1), float:
+// 32 elements per thread (passes 32 x 8 x 8 at L = 2048), 256 threads per CTA, and only ONE shared-memory buffer --
+// the landing zone of the spectrum tile is the exchange buffer of the FFT passes, the transfer function comes
+// straight from global memory (L2-resident: it is read twice per iteration) into the registers.  68 KB and 128
+// registers per CTA, so TWO CTAs share an SM: the whole grid (256 tiles at 2048^2) is resident at once instead of
+// 1.73 waves of one 200 KB CTA per SM, and one CTA's loads and stores overlap the other's butterflies.
+template <typename T, int L, int MODE>
+__global__ void __launch_bounds__(256, 2) col2_kernel(const ColParams<T> P)
+{
+    using C = cx<T>;
+    static_assert(MODE == CM_CONJSUM || MODE == CM_MULT, "col2_kernel: product modes only");
+    constexpr int E = 32;
+    constexpr int TF = L / E;
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    C *sm = reinterpret_cast<C *>(smem_raw);
+    __shared__ unsigned long long bar;
+    constexpr int Cc = 256 / TF, nthr = 256;                    // tile width fixed by the block size (the host checks G.C)
+    const int tid = threadIdx.x;
+    const int t = tid / Cc, c = tid - t * Cc;
+    constexpr size_t tile_len = (size_t)L * Cc;
+    const size_t tbase = (size_t)blockIdx.x * tile_len;
+    const unsigned int tile_bytes = (unsigned int)(tile_len * sizeof(C));
+    const int stop = P.check_status ? P.ct->status : 0;
+    if (stop != 0) return;
+    if (tid == 0) {
+        mbar_init(&bar, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        bulk_load(sm, P.in + tbase, tile_bytes, &bar);
+        // the transfer-function tile is wanted after the forward transform: start it on its way to L2 now (in the SGP
+        // loop the planes touched since its last use have pushed it out to HBM)
+        asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(P.khat + tbase), "r"(tile_bytes) : "memory");
+    }
+    __syncthreads();                                            // barrier initialisation visible to all
+    const SyncBlock sync;
+    const bool packed = blockIdx.x == 0;                        // tile 0 holds the packed column (kx = 0 and nx/2)
+    const bool pk = packed && c == 0;
+    volatile C *pack = P.pack;
+    C v[E];
+    mbar_wait(&bar, 0);
+#pragma unroll
+    for (int e = 0; e < E; ++e) v[e] = sm[tid + e * nthr];
+    fft_block<T, L, E, -1>(v, sm + c, Cc, t, P.tw, sync);       // its first exchange starts with a barrier: the tile has been read
+    if (packed) {
+        if (pk) {
+#pragma unroll
+            for (int e = 0; e < E; ++e) { pack[t + TF * e].x = v[e].x; pack[t + TF * e].y = v[e].y; }
+        }
+        __syncthreads();
+    }
+    const C *kh = P.khat + tbase + tid;
+#pragma unroll
+    for (int e0 = 0; e0 < E; e0 += 8) {
+        C k[8];
+#pragma unroll
+        for (int u = 0; u < 8; ++u) k[u] = __ldg(&kh[(size_t)(e0 + u) * nthr]);
+#pragma unroll
+        for (int u = 0; u < 8; ++u) v[e0 + u] = (MODE == CM_CONJSUM) ? cmulc(v[e0 + u], k[u]) : cmul(v[e0 + u], k[u]);
+    }
+    if (pk) packed_fix<T, L, E, MODE == CM_CONJSUM>(v, pack, P.khatB, t);
+    fft_block<T, L, E, +1>(v, sm + c, Cc, t, P.tw, sync);
+    C *dst = P.out + tbase + tid;
+#pragma unroll
+    for (int e = 0; e < E; ++e) dst[(size_t)e * nthr] = v[e];
+}
+
 }  // namespace sgpk

@@ -12,6 +12,8 @@ template <typename T> using col_kernel_t = void (*)(const ColParams<T>);
 template <typename T> row_kernel_t<T> get_row_fwd(int L, int mode);
 template <typename T> row_kernel_t<T> get_row_inv(int L, int mode);
 template <typename T> col_kernel_t<T> get_col(int L, int mode, bool multi);
+// two-CTAs-per-SM form of the single-image product modes (col.cuh: col2_kernel); nullptr where it does not exist
+template <typename T> col_kernel_t<T> get_col2(int L, int mode);
 
 // supported grid sizes (ny and nx independently)
 inline bool size_supported(int n)

@@ -24,4 +24,21 @@ template <> col_kernel_t<SGP_T> get_col<SGP_T>(int L, int mode, bool multi)
     default: return nullptr;
     }
 }
+template <int L> static col_kernel_t<SGP_T> pick_col2(int mode)
+{
+    if constexpr (sizeof(SGP_T) == 4) {
+        if (mode == CM_CONJSUM) return col2_kernel<SGP_T, L, CM_CONJSUM>;
+        if (mode == CM_MULT) return col2_kernel<SGP_T, L, CM_MULT>;
+    }
+    return nullptr;
+}
+template <> col_kernel_t<SGP_T> get_col2<SGP_T>(int L, int mode)
+{
+    switch (L) {
+    case 1024: return pick_col2<1024>(mode);
+    case 2048: return pick_col2<2048>(mode);
+    case 4096: return pick_col2<4096>(mode);
+    default: return nullptr;
+    }
+}
 }  // namespace sgpk

@@ -13,7 +13,12 @@ template <typename T> struct PlanImpl : PlanBase {
     size_t row_smem = 0, col_smem = 0;
     row_kernel_t<T> k_rowf[RF_NMODES] = {nullptr}, k_rowi[RI_NMODES] = {nullptr};
     col_kernel_t<T> k_colf = nullptr, k_conj = nullptr, k_mult = nullptr;
-    col_kernel_t<T> k_conj1 = nullptr, k_mult1 = nullptr;      // single-image forms (OSEM sub-steps, A_j / A_j^T alone)
+    col_kernel_t<T> k_conj1 = nullptr, k_mult1 = nullptr;
+    bool col2 = false;             // single-image product kernels also exist in their two-CTAs-per-SM form (col2_kernel)
+    col_kernel_t<T> k_conj2 = nullptr, k_mult2 = nullptr;
+    col_kernel_t<T> k_conj_run = nullptr, k_mult_run = nullptr;   // the pair the current run uses
+    int col2_threads = 0; size_t col2_smem = 0;
+    C *tw_c2 = nullptr;            // pass tables of the 32-elements-per-thread column plan      // single-image forms (OSEM sub-steps, A_j / A_j^T alone)
     // device memory
     std::vector<void *> allocs;
     C *tw_r = nullptr, *tw_h = nullptr, *tw_c = nullptr, *pack = nullptr;
@@ -82,16 +87,34 @@ template <typename T> struct PlanImpl : PlanBase {
     }
     void free_trace()
     {
-        cudaFree(trJ); cudaFree(trA); cudaFree(trL); cudaFree(fA); cudaFree(fL); cudaFree(trR); cudaFree(trB);
+        cudaFree(trJ);      // one block: trJ, trA, trL, fA, fL, trR, trB
         trJ = trA = trL = fA = fL = nullptr; trR = trB = nullptr; trace_cap = 0;
     }
+    // The workspace is ONE device allocation (a cudaMalloc / cudaFree pair costs ~0.5 ms and synchronises the device:
+    // two dozen of them were a third of a one-shot call): dalloc() only records a request, commit_allocs() allocates
+    // the arena, hands out 256-byte aligned pieces and performs the deferred table uploads.
+    struct Req { void **ptr; size_t bytes; };
+    struct Upload { void **ptr; std::vector<unsigned char> data; };
+    std::vector<Req> reqs;
+    std::vector<Upload> uploads;
     template <typename U> int dalloc(U **ptr, size_t count)
     {
+        reqs.push_back({reinterpret_cast<void **>(ptr), count * sizeof(U)});
+        return SGP_OK;
+    }
+    int commit_allocs()
+    {
+        size_t total = 0;
+        for (const Req &r : reqs) total += (r.bytes + 255) & ~(size_t)255;
         void *raw = nullptr;
-        SGP_CUDA_TRY(cudaMalloc(&raw, count * sizeof(U)));
+        SGP_CUDA_TRY(cudaMalloc(&raw, total ? total : 256));
         allocs.push_back(raw);
-        bytes_allocated += count * sizeof(U);
-        *ptr = static_cast<U *>(raw);
+        bytes_allocated += total;
+        size_t off = 0;
+        for (const Req &r : reqs) { *r.ptr = static_cast<unsigned char *>(raw) + off; off += (r.bytes + 255) & ~(size_t)255; }
+        reqs.clear();
+        for (const Upload &u : uploads) SGP_CUDA_TRY(cudaMemcpy(*u.ptr, u.data.data(), u.data.size(), cudaMemcpyHostToDevice));
+        uploads.clear();
         return SGP_OK;
     }
 
@@ -161,7 +184,8 @@ template <typename T> struct PlanImpl : PlanBase {
             }
             int r = dalloc(dst, (size_t)count);
             if (r) return r;
-            SGP_CUDA_TRY(cudaMemcpy(*dst, h.data(), sizeof(C) * count, cudaMemcpyHostToDevice));
+            const unsigned char *b = reinterpret_cast<const unsigned char *>(h.data());
+            uploads.push_back({reinterpret_cast<void **>(dst), std::vector<unsigned char>(b, b + sizeof(C) * count)});
             return SGP_OK;
         };
         auto upload_passes = [&](C **dst, int Lf, int Ef) -> int {  // per-pass tables [r-1][j mod NS] (fft_core.cuh)
@@ -176,12 +200,26 @@ template <typename T> struct PlanImpl : PlanBase {
             }
             int r = dalloc(dst, h.size());
             if (r) return r;
-            SGP_CUDA_TRY(cudaMemcpy(*dst, h.data(), sizeof(C) * h.size(), cudaMemcpyHostToDevice));
+            const unsigned char *b = reinterpret_cast<const unsigned char *>(h.data());
+            uploads.push_back({reinterpret_cast<void **>(dst), std::vector<unsigned char>(b, b + sizeof(C) * h.size())});
             return SGP_OK;
         };
         if ((rc = upload_passes(&tw_r, Lr, Er))) return rc;
         if ((rc = upload(&tw_h, nx, Lr + 1))) return rc;
         if ((rc = upload_passes(&tw_c, Lc, Ec))) return rc;
+        // single-image product passes: the two-CTAs-per-SM kernel where it exists (float, 256 threads at this tile width);
+        // run() decides per algorithm whether to use it
+        k_conj_run = k_conj; k_mult_run = k_mult;
+        if (p == 1 && !(opt.use_graph & 16) && plan_ok(Lc, 32) && Cc * (Lc / 32) == 256) {
+            col_kernel_t<T> c2 = get_col2<T>(Lc, CM_CONJSUM), m2 = get_col2<T>(Lc, CM_MULT);
+            const size_t sm2 = (size_t)Cc * fft_padded_len(Lc, 32) * sizeof(C);
+            if (c2 && m2 && sm2 <= 113 * 1024) {
+                SGP_CUDA_TRY(cudaFuncSetAttribute((const void *)c2, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm2));
+                SGP_CUDA_TRY(cudaFuncSetAttribute((const void *)m2, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm2));
+                if ((rc = upload_passes(&tw_c2, Lc, 32))) return rc;
+                k_conj2 = c2; k_mult2 = m2; col2 = true; col2_threads = 256; col2_smem = sm2;
+            }
+        }
         if ((rc = dalloc(&pack, (size_t)ny))) return rc;
         if ((rc = dalloc(&khat, nspec * p))) return rc;
         if ((rc = dalloc(&khatB, (size_t)ny * p))) return rc;
@@ -206,6 +244,7 @@ template <typename T> struct PlanImpl : PlanBase {
         if ((rc = dalloc(&part_bt, (size_t)bt_grid))) return rc;
         if ((rc = dalloc(&part_misc, (size_t)1024 * p))) return rc;
         if ((rc = dalloc(&ct, (size_t)1))) return rc;
+        if ((rc = commit_allocs())) return rc;
         SGP_CUDA_TRY(cudaMemset(ct, 0, sizeof(Ctrl)));
         SGP_CUDA_TRY(cudaEventCreate(&ev0));
         SGP_CUDA_TRY(cudaEventCreate(&ev1));
@@ -254,6 +293,10 @@ template <typename T> struct PlanImpl : PlanBase {
     }
     int launch_col(col_kernel_t<T> k, const ColParams<T> &P, cudaStream_t st)
     {
+        if (col2 && (k == k_conj2 || k == k_mult2)) {     // one tile per CTA, its own pass tables
+            ColParams<T> Q = P; Q.tw = tw_c2;
+            return launch_pdl(k, dim3(ntiles), col2_threads, col2_smem, Q, st);
+        }
         return launch_pdl(k, dim3(col_grid), col_threads, col_smem, P, st);
     }
     static int ew_grid(size_t count) { size_t b = (count + 255) / 256; return (int)(b > 1184 ? 1184 : (b < 1 ? 1 : b)); }

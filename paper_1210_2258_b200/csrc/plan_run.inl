@@ -12,20 +12,13 @@ int PlanImpl<T>::ensure_trace(int max_iter, const sgp_result *res, Trace *tr, cu
     const int need = max_iter + 1;
     if (need > trace_cap) {
         free_trace();
-        SGP_CUDA_TRY(cudaMalloc((void **)&trJ, sizeof(double) * need));
-        SGP_CUDA_TRY(cudaMalloc((void **)&trA, sizeof(double) * need));
-        SGP_CUDA_TRY(cudaMalloc((void **)&trL, sizeof(double) * need));
-        SGP_CUDA_TRY(cudaMalloc((void **)&fA, sizeof(double) * need));
-        SGP_CUDA_TRY(cudaMalloc((void **)&fL, sizeof(double) * need));
-        SGP_CUDA_TRY(cudaMalloc((void **)&trR, sizeof(int) * need));
-        SGP_CUDA_TRY(cudaMalloc((void **)&trB, sizeof(int) * need));
-        trace_cap = need;
+        const size_t cap = ((size_t)need + 1) & ~(size_t)1;     // even: the int arrays stay 8-byte aligned
+        SGP_CUDA_TRY(cudaMalloc((void **)&trJ, (5 * sizeof(double) + 2 * sizeof(int)) * cap));      // one block
+        trA = trJ + cap; trL = trA + cap; fA = trL + cap; fL = fA + cap;
+        trR = reinterpret_cast<int *>(fL + cap); trB = trR + cap;
+        trace_cap = (int)cap;
     }
-    SGP_CUDA_TRY(cudaMemsetAsync(trJ, 0, sizeof(double) * need, st));
-    SGP_CUDA_TRY(cudaMemsetAsync(trA, 0, sizeof(double) * need, st));
-    SGP_CUDA_TRY(cudaMemsetAsync(trL, 0, sizeof(double) * need, st));
-    SGP_CUDA_TRY(cudaMemsetAsync(trR, 0, sizeof(int) * need, st));
-    SGP_CUDA_TRY(cudaMemsetAsync(trB, 0, sizeof(int) * need, st));
+    SGP_CUDA_TRY(cudaMemsetAsync(trJ, 0, (5 * sizeof(double) + 2 * sizeof(int)) * (size_t)trace_cap, st));
     tr->J = trJ; tr->alpha = trA; tr->lambda = trL; tr->rule = trR; tr->backtracks = trB;
     tr->force_alpha = nullptr; tr->force_lambda = nullptr;
     if (res->force_alpha && max_iter > 0) {
@@ -56,7 +49,7 @@ int PlanImpl<T>::enqueue_sgp_iteration(const RowParams<T> &Pb, const DevOpts &o,
     cur_slot = SGP_PROF_K2;
     {   // K2 (a2)
         ColParams<T> Q = col_params(); Q.check_status = 1;
-        if ((rc = launch_col(k_conj, Q, st))) return rc;
+        if ((rc = launch_col(k_conj_run, Q, st))) return rc;
     }
     cur_slot = SGP_PROF_K3;
     {   // K3 (a10 for f, a3, a5, a6)
@@ -71,7 +64,7 @@ int PlanImpl<T>::enqueue_sgp_iteration(const RowParams<T> &Pb, const DevOpts &o,
     cur_slot = SGP_PROF_K5;
     {   // K5 (a8)
         ColParams<T> Q = col_params(); Q.check_status = 1;
-        if ((rc = launch_col(k_mult, Q, st))) return rc;
+        if ((rc = launch_col(k_mult_run, Q, st))) return rc;
     }
     cur_slot = SGP_PROF_K6;
     {   // K6 (a8 tail, a9 at lambda = 1, a11)
@@ -105,13 +98,13 @@ int PlanImpl<T>::enqueue_rl_round(const DevOpts &o, const Trace &tr, const doubl
     cur_slot = SGP_PROF_R1;
     { RowParams<T> P = Pb; P.in0 = f; P.maskmode = MM_NONE; if ((rc = launch_row(k_rowf[RF_PLAIN], P, 1, st))) return rc; }
     cur_slot = SGP_PROF_R2;
-    { ColParams<T> Q = col_params(); Q.check_status = 1; if ((rc = launch_col(k_mult, Q, st))) return rc; }
+    { ColParams<T> Q = col_params(); Q.check_status = 1; if ((rc = launch_col(k_mult_run, Q, st))) return rc; }
     cur_slot = SGP_PROF_R3;
     { RowParams<T> P = Pb; P.submode = QJ_RL; P.in0 = Gp; P.in2 = Bp; P.out0 = q; P.part = part_J; if ((rc = launch_row(k_rowi[RI_QJ], P, p, st))) return rc; }
     cur_slot = SGP_PROF_R4;
     { RowParams<T> P = Pb; P.in0 = Gp; P.in1 = q; P.in2 = Bp; if ((rc = launch_row(k_rowf[RF_RATIO], P, p, st))) return rc; }
     cur_slot = SGP_PROF_R5;
-    { ColParams<T> Q = col_params(); Q.check_status = 1; if ((rc = launch_col(k_conj, Q, st))) return rc; }
+    { ColParams<T> Q = col_params(); Q.check_status = 1; if ((rc = launch_col(k_conj_run, Q, st))) return rc; }
     cur_slot = SGP_PROF_R6;
     { RowParams<T> P = Pb; P.in0 = f; P.out0 = f; if ((rc = launch_row(k_rowi[RI_RLUPDATE], P, 1, st))) return rc; }
     cur_slot = -1;
@@ -214,6 +207,15 @@ int PlanImpl<T>::run(int algorithm, const void *const *g, const void *const *b_a
     }
     const long launches0 = launches;
     if (profiling) prof_reset();
+    // Column product kernels of this run.  The two-CTAs-per-SM form (col2_kernel) is 25-30 % faster where the tiles
+    // make several waves (4096^2: 82 -> 59 us) and 8 % faster in the RL / OSEM loops at 2048^2 (25 -> 23 us); in the
+    // SGP loop at 2048^2 its single wave (all CTAs load, transform and store in phase) is slower (31 vs 27 us behind
+    // the ratio kernel's write-backs), so the one-CTA form with the TMA-staged transfer function stays there.
+    {
+        const bool use2 = col2 && (algorithm != SGP_ALG_SGP || ntiles > 2 * nsm);
+        k_conj_run = use2 ? k_conj2 : k_conj;
+        k_mult_run = use2 ? k_mult2 : k_mult;
+    }
 
     DevOpts o;
     memset(&o, 0, sizeof(o));
@@ -254,12 +256,12 @@ int PlanImpl<T>::run(int algorithm, const void *const *g, const void *const *b_a
 
     if (algorithm == SGP_ALG_SGP) {
         { RowParams<T> P = Pb; P.in0 = f; if ((rc = launch_row(k_rowf[RF_PLAIN], P, 1, st))) return rc; }
-        { ColParams<T> Q = col_params(); Q.check_status = 1; if ((rc = launch_col(k_mult, Q, st))) return rc; }
+        { ColParams<T> Q = col_params(); Q.check_status = 1; if ((rc = launch_col(k_mult_run, Q, st))) return rc; }
         { RowParams<T> P = Pb; P.submode = QJ_INIT; P.in0 = Gp; P.in2 = Bp; P.out0 = q; P.part = part_J;
           if ((rc = launch_row(k_rowi[RI_QJ], P, p, st))) return rc; }
         if (ro.adaptive_L) {     // bounds from one RL step
             { RowParams<T> P = Pb; P.in0 = Gp; P.in1 = q; P.in2 = Bp; if ((rc = launch_row(k_rowf[RF_RATIO], P, p, st))) return rc; }
-            { ColParams<T> Q = col_params(); Q.check_status = 1; if ((rc = launch_col(k_conj, Q, st))) return rc; }
+            { ColParams<T> Q = col_params(); Q.check_status = 1; if ((rc = launch_col(k_conj_run, Q, st))) return rc; }
             { RowParams<T> P = Pb; P.submode = RIP_RLMINMAX; P.in0 = f; P.part = part_J; if ((rc = launch_row(k_rowi[RI_PLAIN], P, 1, st))) return rc; }
         }
     }
@@ -304,7 +306,7 @@ int PlanImpl<T>::run(int algorithm, const void *const *g, const void *const *b_a
                 Trace t0 = tr; t0.J = nullptr;
                 RowParams<T> Pj = Pb; Pj.tr = t0;
                 { RowParams<T> P = Pj; P.in0 = f; if ((rc = launch_row(k_rowf[RF_PLAIN], P, 1, st))) return rc; }
-                { ColParams<T> Q = col_params(); Q.check_status = 1; if ((rc = launch_col(k_mult, Q, st))) return rc; }
+                { ColParams<T> Q = col_params(); Q.check_status = 1; if ((rc = launch_col(k_mult_run, Q, st))) return rc; }
                 { RowParams<T> P = Pj; P.submode = QJ_INIT; P.in0 = Gp; P.in2 = Bp; P.out0 = q; P.part = part_J;
                   if ((rc = launch_row(k_rowi[RI_QJ], P, p, st))) return rc; }
                 SGP_CUDA_TRY(cudaMemcpyAsync(&h, ct, sizeof(Ctrl), cudaMemcpyDeviceToHost, st));
