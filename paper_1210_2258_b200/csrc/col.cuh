@@ -66,8 +66,19 @@ __device__ __forceinline__ void packed_fix(cx<T> (&r)[E], volatile cx<T> *pack, 
     }
 }
 
-template <typename T, int L, int MODE, bool MULTI>
-__global__ void __launch_bounds__(fft_E_col<T>(L) == 32 ? 256 : 512, 1) col_kernel(const ColParams<T> P)
+// tile width the host chooses by default (api.cu: choose_tiles) for this element type and length: with it known at
+// compile time the shared-memory addresses of the exchanges are immediates (no spills, fewer integer instructions)
+template <typename T> __host__ __device__ constexpr int col_default_C(int L)
+{
+    const int E = fft_E_col<T>(L), TF = L / E, col_max = E == 32 ? 256 : 512;
+    int C = 1;
+    while (2 * C <= (col_max / TF > 1 ? col_max / TF : 1) && 2 * C <= 32) C *= 2;
+    while (C > 1 && (size_t)C * fft_padded_len(L, E) * sizeof(cx<T>) > 72 * 1024) C /= 2;
+    return C;
+}
+
+template <typename T, int L, int MODE, bool MULTI, int CT>
+__device__ __forceinline__ void col_body(const ColParams<T> &P)
 {
     using C = cx<T>;
     constexpr int E = fft_E_col<T>(L);
@@ -77,7 +88,7 @@ __global__ void __launch_bounds__(fft_E_col<T>(L) == 32 ? 256 : 512, 1) col_kern
     pdl_trigger();
 
     ColCtx<T, L, E> X;
-    X.Cc = P.G.C; X.tid = threadIdx.x; X.nthr = blockDim.x;
+    X.Cc = CT > 0 ? CT : P.G.C; X.tid = threadIdx.x; X.nthr = CT > 0 ? CT * TF : (int)blockDim.x;
     X.t = X.tid / X.Cc; X.c = X.tid - X.t * X.Cc;
     X.tile_len = (size_t)L * X.Cc;
     X.smc = sm + X.c;
@@ -207,6 +218,13 @@ __global__ void __launch_bounds__(fft_E_col<T>(L) == 32 ? 256 : 512, 1) col_kern
             }
         }
     }
+}
+
+// CT = 0: tile width from P.G.C; CT > 0: compiled for that width (the host launches it only when G.C == CT)
+template <typename T, int L, int MODE, bool MULTI, int CT = 0>
+__global__ void __launch_bounds__(fft_E_col<T>(L) == 32 ? 256 : 512, 1) col_kernel(const ColParams<T> P)
+{
+    col_body<T, L, MODE, MULTI, CT>(P);
 }
 
 // ---------------------------------------------------------------------------------------------------------------

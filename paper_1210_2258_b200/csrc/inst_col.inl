@@ -1,26 +1,29 @@
 // included by inst_col_f32.cu / inst_col_f64.cu with SGP_T defined
 #include "dispatch.h"
 namespace sgpk {
-template <int L> static col_kernel_t<SGP_T> pick_col(int mode, bool multi)
+template <int L> static col_kernel_t<SGP_T> pick_col(int mode, bool multi, int tile_cols)
 {
+    constexpr int CD = col_default_C<SGP_T>(L);
+    if (tile_cols == CD && mode == CM_CONJSUM) return multi ? col_kernel<SGP_T, L, CM_CONJSUM, true, CD> : col_kernel<SGP_T, L, CM_CONJSUM, false, CD>;
+    if (tile_cols == CD && mode == CM_MULT) return multi ? col_kernel<SGP_T, L, CM_MULT, true, CD> : col_kernel<SGP_T, L, CM_MULT, false, CD>;
     if (mode == CM_FWD) return col_kernel<SGP_T, L, CM_FWD, false>;
     if (mode == CM_INV) return col_kernel<SGP_T, L, CM_INV, false>;
     if (mode == CM_CONJSUM) return multi ? col_kernel<SGP_T, L, CM_CONJSUM, true> : col_kernel<SGP_T, L, CM_CONJSUM, false>;
     return multi ? col_kernel<SGP_T, L, CM_MULT, true> : col_kernel<SGP_T, L, CM_MULT, false>;
 }
-template <> col_kernel_t<SGP_T> get_col<SGP_T>(int L, int mode, bool multi)
+template <> col_kernel_t<SGP_T> get_col<SGP_T>(int L, int mode, bool multi, int tile_cols)
 {
     switch (L) {
-    case 64: return pick_col<64>(mode, multi);
-    case 128: return pick_col<128>(mode, multi);
-    case 256: return pick_col<256>(mode, multi);
-    case 320: return pick_col<320>(mode, multi);
-    case 512: return pick_col<512>(mode, multi);
-    case 640: return pick_col<640>(mode, multi);
-    case 1024: return pick_col<1024>(mode, multi);
-    case 1280: return pick_col<1280>(mode, multi);
-    case 2048: return pick_col<2048>(mode, multi);
-    case 4096: return pick_col<4096>(mode, multi);
+    case 64: return pick_col<64>(mode, multi, tile_cols);
+    case 128: return pick_col<128>(mode, multi, tile_cols);
+    case 256: return pick_col<256>(mode, multi, tile_cols);
+    case 320: return pick_col<320>(mode, multi, tile_cols);
+    case 512: return pick_col<512>(mode, multi, tile_cols);
+    case 640: return pick_col<640>(mode, multi, tile_cols);
+    case 1024: return pick_col<1024>(mode, multi, tile_cols);
+    case 1280: return pick_col<1280>(mode, multi, tile_cols);
+    case 2048: return pick_col<2048>(mode, multi, tile_cols);
+    case 4096: return pick_col<4096>(mode, multi, tile_cols);
     default: return nullptr;
     }
 }

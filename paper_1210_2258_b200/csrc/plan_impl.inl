@@ -127,13 +127,13 @@ template <typename T> struct PlanImpl : PlanBase {
         const int Er = fft_E<T>(Lr), Ec = fft_E_col<T>(Lc);
         for (int m = 0; m < RF_NMODES; ++m) if (!(k_rowf[m] = get_row_fwd<T>(Lr, m))) return SGP_ERR_ARG;
         for (int m = 0; m < RI_NMODES; ++m) if (!(k_rowi[m] = get_row_inv<T>(Lr, m))) return SGP_ERR_ARG;
-        const bool multi = p > 1;
-        k_colf = get_col<T>(Lc, CM_FWD, false); k_conj = get_col<T>(Lc, CM_CONJSUM, multi); k_mult = get_col<T>(Lc, CM_MULT, multi);
-        k_conj1 = get_col<T>(Lc, CM_CONJSUM, false); k_mult1 = get_col<T>(Lc, CM_MULT, false);
-        if (!k_colf || !k_conj || !k_mult || !k_conj1 || !k_mult1) return SGP_ERR_ARG;
         int Cc = 0, RB = 0;
         int rc = choose_tiles(ny, nx, dtype, &opt, &Cc, &RB);
         if (rc) return rc;
+        const bool multi = p > 1;
+        k_colf = get_col<T>(Lc, CM_FWD, false); k_conj = get_col<T>(Lc, CM_CONJSUM, multi, Cc); k_mult = get_col<T>(Lc, CM_MULT, multi, Cc);
+        k_conj1 = get_col<T>(Lc, CM_CONJSUM, false, Cc); k_mult1 = get_col<T>(Lc, CM_MULT, false, Cc);
+        if (!k_colf || !k_conj || !k_mult || !k_conj1 || !k_mult1) return SGP_ERR_ARG;
         G.C = Cc; G.RB = RB; G.lc = 0; while ((1 << G.lc) < Cc) G.lc++;
         row_threads = RB * (Lr / Er);
         col_threads = Cc * (Lc / Ec);
