@@ -21,8 +21,9 @@ __device__ __forceinline__ void quad_in_S(const Geom &G, bool rowin, int x, bool
 }
 
 // a10 (lazy) + a3 + a5: f <- f + lambda d; grad = alpha - w on R (Eq.11/14/18); the four BB dot products with
-// s = lambda d, z = grad - grad_prev, D = (M_R/alpha) clip(f(k),L1,L2) (Eq.7-8).  s/D and z D are formed in T,
-// the products and sums in double.
+// s = lambda d, z = grad - grad_prev, D = (M_R/alpha) clip(f(k),L1,L2) (Eq.7-8).  s/D and z D are formed in T; float:
+// the four products of a pixel are summed over its quad in float (fma) and each quad sum is added to a double
+// accumulator (6 instructions per pixel less than converting every factor); double: everything in double.
 template <typename T, int L, int TF, bool MASKED>
 __device__ __forceinline__ void epi_grad(const RowParams<T> &P, const T *wrow, int t, size_t rowbase, double (&acc)[4])
 {
@@ -68,6 +69,7 @@ __device__ __forceinline__ void epi_grad(const RowParams<T> &P, const T *wrow, i
         for (int u = 0; u < U; ++u) {
             const int x = 4 * (t + TF * (it0 + u));
             Quad<T> g4;
+            T pq[4] = {(T)0, (T)0, (T)0, (T)0};     // the four sums over this quad, in T; added to the double accumulators once per quad
 #pragma unroll
             for (int c = 0; c < 4; ++c) {
                 const T s = lam * d4[u].a[c];
@@ -80,8 +82,17 @@ __device__ __forceinline__ void epi_grad(const RowParams<T> &P, const T *wrow, i
                 g4.a[c] = gn;
                 const T Di = wv * clipT<T>(fn, L1, L2);
                 const T zf = gn - go4[u].a[c];
-                const double si = inR ? (double)fast_div(s, Di) : 0.0, z = inR ? (double)zf : 0.0, zd = inR ? (double)(zf * Di) : 0.0;
-                acc[0] += si * si; acc[1] += si * z; acc[2] += (double)s * zd; acc[3] += zd * zd;
+                if constexpr (sizeof(T) == 8) {
+                    const double si = inR ? fast_div(s, Di) : 0.0, z = inR ? zf : 0.0, zd = inR ? zf * Di : 0.0;
+                    acc[0] += si * si; acc[1] += si * z; acc[2] += s * zd; acc[3] += zd * zd;
+                } else {
+                    const T si = inR ? fast_div(s, Di) : (T)0, z = inR ? zf : (T)0, zd = inR ? zf * Di : (T)0;
+                    pq[0] = fmaf(si, si, pq[0]); pq[1] = fmaf(si, z, pq[1]); pq[2] = fmaf(s, zd, pq[2]); pq[3] = fmaf(zd, zd, pq[3]);
+                }
+            }
+            if constexpr (sizeof(T) == 4) {
+#pragma unroll
+                for (int k4 = 0; k4 < 4; ++k4) acc[k4] += (double)pq[k4];
             }
             stq<T>(P.out1 + rowbase + x, f4[u]);
             stq<T>(P.out0 + rowbase + x, g4);
