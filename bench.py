@@ -476,8 +476,8 @@ def run_ours(args):
                 "gpixel_iter_per_s": value * ny * nx / 1e9,
                 "config": {"workload": desc, "iterations_per_step": iters, "grid": [ny, nx], "images": p, "algorithm": args.alg,
                            "parallelism": "replicas only" if world > 1 else "single GPU",
-                           "l2": f"no flush: per-iteration working set {(6 * p + 4) * plane_bytes / 1e6:.0f} MB "
-                                 f"({6 * p + 4} planes) vs 126 MB L2",
+                           "l2": f"no flush: per-iteration working set {(7 * p + 4) * plane_bytes / 1e6:.0f} MB "
+                                 f"({7 * p + 4} planes) vs 126 MB L2",
                            "tile_cols": int(opts.tile_cols), "rows_per_block": int(opts.rows_per_block),
                            "J0_final": J_final, "backtracks": backtracks // args.steps,
                            "fused_linesearch": int(r.fused_linesearch)},
