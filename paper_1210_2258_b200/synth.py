@@ -158,6 +158,18 @@ def c0_stars_gaussian(n=256, seed_idx=0):
     return dict(name=f"C0_{n}", seed=BASE_SEED + seed_idx, g=[g], psf=[psf], b=[b], truth=truth, S=None, opts=opts)
 
 
+def c0_rect(ny=128, nx=320, seed_idx=7, n_stars=20):
+    """the C0 recipe on a rectangular ny x nx grid (ragged shapes for the parity tests: ny != nx, radix-5 lengths)"""
+    rng = _rng(seed_idx, ny * 4096 + nx)
+    truth = _add_stars(np.zeros((ny, nx)), rng, n_stars)
+    psf = psf_gaussian(ny, nx, 2.0)
+    b = 10.0
+    g = _poisson(rng, _circ_conv(psf, truth) + b)
+    opts = dict(L1=1e-10, L2=1e10, adaptive_L=0, m_alpha=3, armijo_memory=10, beta=1e-4, theta=0.4,
+                max_iter=100, stop_rule=0)
+    return dict(name=f"C0_{ny}x{nx}", seed=BASE_SEED + seed_idx, g=[g], psf=[psf], b=[b], truth=truth, S=None, opts=opts)
+
+
 def c1_galaxies_airy(n=512, seed_idx=1, max_iter=1000, stop_rule=2):
     """C1 (and C4a at n=4096, C4c at n=2048): galaxies + stars, Airy PSF, b = 20"""
     rng = _rng(seed_idx, n)
@@ -205,7 +217,7 @@ def c4c(n=2048):
     w = c1_galaxies_airy(n, seed_idx=6, max_iter=200, stop_rule=0); w["name"] = f"C4c_{n}"; return w
 
 
-CONFIGS = {"C0": c0_stars_gaussian, "C1": c1_galaxies_airy, "C2": c2_lbt_multi, "C3": c3_boundary,
+CONFIGS = {"C0": c0_stars_gaussian, "C0r": c0_rect, "C1": c1_galaxies_airy, "C2": c2_lbt_multi, "C3": c3_boundary,
            "C4a": c4a, "C4b": c4b, "C4c": c4c}
 
 

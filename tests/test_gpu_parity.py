@@ -493,3 +493,27 @@ def test_osem_one_shot_and_unsupported_stop_rule():
     assert torch.equal(f1, f2) and r1.J0_final == r2.J0_final and r1.iterations == 5
     _, r = B.osem_multi(g, k, w["b"], opts=B.default_options(**{**w["opts"], "max_iter": 5, "stop_rule": 2}), check=False)
     assert r.rc == B.ERR_UNSUPPORTED
+
+
+# ---------------------------------------------------------------- ragged shapes: ny != nx, radix-5 lengths, the smallest grid
+@pytest.mark.parametrize("dt,tol", [(np.float32, 1e-3), (np.float64, 1e-10)])
+@pytest.mark.parametrize("ny,nx", [(128, 320), (640, 64), (64, 64), (1280, 256)])
+def test_sgp_and_rl_on_rectangular_grids(ny, nx, dt, tol):
+    """row length and column length differ (row kernels of length nx/2, column kernel of length ny, spectrum tiles of
+    ny x C): one SGP iteration at north_star's 1e-5, 25 iterations at the precision-derived tolerance (the star-field
+    recipe with L = 1e10 amplifies rounding fastest), 15 RL steps (no branches: tight)."""
+    _need_gpu()
+    w = synth.make("C0r", ny=ny, nx=nx)
+    f1, r1, fo1, ro1 = run_both(w, dt, max_iter=1)
+    assert rel_l2(f1, fo1) <= (1e-5 if dt == np.float32 else 1e-12)
+    assert abs(r1.J0_final - ro1.J0_final) <= (1e-6 if dt == np.float32 else 1e-13) * abs(ro1.J0_final)
+    fg, rg, fo, ro = run_both(w, dt, max_iter=25)
+    ftol, jt = long_run_tolerances(w, dt, tol, 1e-4 if dt == np.float32 else 1e-11, fo, ro, max_iter=25)
+    assert rg.iterations == ro.iterations == 25
+    assert rel_l2(fg, fo) <= ftol
+    assert np.max(np.abs(rg.J - np.asarray(ro.J)) / np.abs(np.asarray(ro.J))) <= jt
+    if dt == np.float64:
+        assert np.array_equal(rg.backtracks, np.asarray(ro.backtracks)[:25])
+    assert (fg >= 0).all()
+    fg, rg, fo, ro = run_both(w, dt, alg="rl", max_iter=15)
+    assert rel_l2(fg, fo) <= (1e-4 if dt == np.float32 else 1e-11)
