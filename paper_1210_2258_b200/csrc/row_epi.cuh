@@ -12,6 +12,16 @@ template <typename T> __host__ __device__ constexpr int batch_len(int nit)
     return sizeof(T) == 8 ? (nit % 2 == 0 ? 2 : 1) : (nit % 4 == 0 ? 4 : (nit % 2 == 0 ? 2 : 1));
 }
 
+// quads of g and q loaded ahead in epi_kl.  Measured at 2048^2 (K6, us): 2 quads 30.6, 4 quads 29.8, 8 quads 36.3 (3 x 2048^2:
+// 101 / 99 / 130) -- longer batches do not hide more latency, they delay the first KL evaluation of every warp
+#ifndef SGP_KL_BATCH
+#define SGP_KL_BATCH 4
+#endif
+template <typename T> __host__ __device__ constexpr int batch_len_kl(int nit)
+{
+    return (sizeof(T) == 4 && nit % SGP_KL_BATCH == 0) ? SGP_KL_BATCH : batch_len<T>(nit);
+}
+
 // M_S for the four pixels of a quad
 template <typename T>
 __device__ __forceinline__ void quad_in_S(const Geom &G, bool rowin, int x, bool (&s)[4])
@@ -114,14 +124,13 @@ __device__ __forceinline__ void epi_kl(const RowParams<T> &P, const T *wrow, T *
     const T bc = (T)P.bconst[j];
     const bool rowin = (unsigned)(y - G.oy) < (unsigned)G.sy;
     constexpr int NIT = (L / 2) / TF;
-    constexpr int U = batch_len<T>(NIT);
+    constexpr int U = batch_len_kl<T>(NIT);
     const bool need = rowin && !plain;
     for (int it0 = 0; it0 < NIT; it0 += U) {
-        Quad<T> w4[U], g4[U], q4[U], b4[U];
+        Quad<T> g4[U], q4[U], b4[U];
 #pragma unroll
         for (int u = 0; u < U; ++u) {
             const int x = 4 * (t + TF * (it0 + u));
-            w4[u] = ldq<T>(wrow + x);
             if (need) {
                 g4[u] = ldq<T>(P.in0 + base + x);
                 if constexpr (WITH_Q) q4[u] = ldq<T>(qin + base + x);
@@ -133,9 +142,10 @@ __device__ __forceinline__ void epi_kl(const RowParams<T> &P, const T *wrow, T *
             const int x = 4 * (t + TF * (it0 + u));
             bool s[4] = {true, true, true, true};      // without a boundary mask S is the whole grid
             if constexpr (MASKED) quad_in_S<T>(G, rowin, x, s);
+            const Quad<T> w4 = ldq<T>(wrow + x);          // the row itself sits in shared memory: fetched when used
             Quad<T> u4;
 #pragma unroll
-            for (int c = 0; c < 4; ++c) u4.a[c] = s[c] ? w4[u].a[c] : (T)0;
+            for (int c = 0; c < 4; ++c) u4.a[c] = s[c] ? w4.a[c] : (T)0;
             stq<T>(P.out0 + base + x, u4);
             Quad<T> r4;
 #pragma unroll
