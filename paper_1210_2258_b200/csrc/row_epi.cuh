@@ -65,11 +65,10 @@ __device__ __forceinline__ void epi_grad(const RowParams<T> &P, const T *wrow, i
     // left to order them (it would serialise every load behind the previous store)
     constexpr int U = batch_len<T>(NIT);
     for (int it0 = 0; it0 < NIT; it0 += U) {
-        Quad<T> w4[U], f4[U], d4[U], go4[U], a4[U];
+        Quad<T> f4[U], d4[U], go4[U], a4[U];
 #pragma unroll
         for (int u = 0; u < U; ++u) {
             const int x = 4 * (t + TF * (it0 + u));
-            w4[u] = ldq<T>(wrow + x);
             f4[u] = ldq<T>(P.in0 + rowbase + x);
             d4[u] = ldq<T>(P.in1 + rowbase + x);
             go4[u] = ldq<T>(P.out0 + rowbase + x);
@@ -78,6 +77,7 @@ __device__ __forceinline__ void epi_grad(const RowParams<T> &P, const T *wrow, i
 #pragma unroll
         for (int u = 0; u < U; ++u) {
             const int x = 4 * (t + TF * (it0 + u));
+            const Quad<T> w4 = ldq<T>(wrow + x);          // shared memory: fetched when used
             Quad<T> g4;
             T pq[4] = {(T)0, (T)0, (T)0, (T)0};     // the four sums over this quad, in T; added to the double accumulators once per quad
 #pragma unroll
@@ -88,7 +88,7 @@ __device__ __forceinline__ void epi_grad(const RowParams<T> &P, const T *wrow, i
                 bool inR = true;
                 T av = pT, wv = Wc;
                 if constexpr (MASKED) { av = a4[u].a[c]; inR = av > (T)0; wv = inR ? (T)1 / av : (T)0; }
-                const T gn = inR ? av - w4[u].a[c] : (T)0;
+                const T gn = inR ? av - w4.a[c] : (T)0;
                 g4.a[c] = gn;
                 const T Di = wv * clipT<T>(fn, L1, L2);
                 const T zf = gn - go4[u].a[c];
