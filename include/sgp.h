@@ -103,7 +103,8 @@ typedef struct sgp_options {
     int use_graph;                               /* bit 0 (default 1) = replay the iterations as CUDA graphs of 10, else plain stream launches;
                                                     experiment switches: bit 1 = persistent column kernel, bit 2 / bit 3 = force the
                                                     separate / the fused line-search kernel (default: chosen by working set vs L2),
-                                                    bit 4 = never use the two-CTAs-per-SM column kernel */
+                                                    bit 4 = never use the two-CTAs-per-SM column kernel, bit 5 = fork the backtracking /
+                                                    ratio tail inside the graph */
 } sgp_options;
 
 /* Result of a run.  The trace pointers are optional caller-allocated HOST arrays of max_iter+1 entries

@@ -35,6 +35,8 @@ template <typename T> struct PlanImpl : PlanBase {
     int trace_cap = 0;
     cudaEvent_t ev0 = nullptr, ev1 = nullptr, ev2 = nullptr;
     cudaStream_t cap_stream = nullptr;       // stream the iteration graph is captured on (use_graph)
+    cudaStream_t cap_stream2 = nullptr;      // side branch of the graph: backtracking kernel + ratio kernel in repair mode
+    cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
     cudaGraphExec_t gexec = nullptr;
     long graph_launches = 0;                 // kernels in one replay of gexec
     // per-kernel timing (sgp_plan_set_profiling): one event pair per launch of the iteration loop
@@ -53,6 +55,9 @@ template <typename T> struct PlanImpl : PlanBase {
         if (ev2) cudaEventDestroy(ev2);
         if (gexec) cudaGraphExecDestroy(gexec);
         if (cap_stream) cudaStreamDestroy(cap_stream);
+        if (cap_stream2) cudaStreamDestroy(cap_stream2);
+        if (ev_fork) cudaEventDestroy(ev_fork);
+        if (ev_join) cudaEventDestroy(ev_join);
         for (cudaEvent_t e : prof_pool) cudaEventDestroy(e);
     }
     cudaEvent_t prof_event()
@@ -440,6 +445,8 @@ template <typename T> struct PlanImpl : PlanBase {
             const void *f0, void *f_out, const sgp_options *ropt, sgp_result *res, cudaStream_t st) override;
     int ensure_trace(int max_iter, const sgp_result *res, Trace *tr, cudaStream_t st);
     int enqueue_sgp_iteration(const RowParams<T> &Pbase, const DevOpts &o, const Trace &tr, const double *bconst, int b_is_array, cudaStream_t st);
+    int enqueue_ratio(const RowParams<T> &Pbase, int lazy, cudaStream_t st);
+    int enqueue_backtrack(const DevOpts &o, const Trace &tr, const double *bconst, int b_is_array, cudaStream_t st);
     int enqueue_rl_round(const DevOpts &o, const Trace &tr, const double *bconst, int b_is_array, cudaStream_t st);
     int enqueue_osem_cycle(const DevOpts &o, const Trace &tr, const double *bconst, int b_is_array, cudaStream_t st);
     int enqueue_many(int algorithm, int count, const RowParams<T> &Pb, const DevOpts &o, const Trace &tr, const double *bconst,

@@ -32,20 +32,50 @@ int PlanImpl<T>::ensure_trace(int max_iter, const sgp_result *res, Trace *tr, cu
     return SGP_OK;
 }
 
-// One SGP iteration = 7 launches: K1 lazy q update + ratio + row FFT, K2 column pass with conj(K^)
-// summed over the images, K3 inverse rows + lazy f update + gradient + BB sums + step length, K4 projection + row FFT
-// of d, K5 column pass with K^_j, K6 inverse rows + u_j + J(lambda = 1) + Armijo test + book-keeping, K7 backtracks
-// (elementwise; returns at once when lambda = 1 was accepted).
+// One SGP iteration: K2 column pass with conj(K^) summed over the images, K3 inverse rows + lazy
+// f update + gradient + BB sums + step length, K4 projection + row FFT of d, K5 column pass with K^_j, K6 inverse rows +
+// u_j + J(lambda = 1) + Armijo test + book-keeping (fused form: also q(k+1), the ratio and its row FFT), then the tail
+// K7 backtracks (elementwise; returns at once when lambda = 1 was accepted) and K1 = ratio + row FFT of iteration k + 1.
+// The ratio kernel of the FIRST iteration is enqueued by run() before the loop.
+//
+// Experiment (opt.use_graph bit 5, off by default): inside a captured graph the tail becomes a fork -- K1 in its
+// "lambda = 1 accepted" instance BESIDE K7 -> K1 in its repair instance, the next K2 joining both -- which takes the two
+// kernels that usually return at once off the critical path.  Measured: the fork / join edges cost more than the
+// 2.7 us they hide (C4c 7660 vs 8110 it/s, C0 14.6 vs 17.3 kit/s), so the tail stays in stream order.
+template <typename T>
+int PlanImpl<T>::enqueue_ratio(const RowParams<T> &Pb, int lazy, cudaStream_t st)
+{
+    cur_slot = SGP_PROF_K1;
+    RowParams<T> P = Pb; P.lazy = lazy; P.in0 = Gp; P.in1 = q; P.in2 = Bp; P.in3 = u; P.out0 = q;
+    int rc = launch_row(k_rowf[RF_RATIO], P, p, st);
+    cur_slot = -1;
+    return rc;
+}
+
+template <typename T>
+int PlanImpl<T>::enqueue_backtrack(const DevOpts &o, const Trace &tr, const double *bconst, int b_is_array, cudaStream_t st)
+{
+    cur_slot = SGP_PROF_K7;
+    {
+        BtParams<T> U;
+        memset(&U, 0, sizeof(U));
+        U.G = G; U.o = o; U.tr = tr; U.ct = ct; U.q = q; U.u = u; U.g = Gp; U.b = Bp;
+        U.plane = n; U.qbuf = n * (size_t)p; U.b_is_array = b_is_array; U.part = part_bt;
+        for (int j = 0; j < p; ++j) U.bconst[j] = bconst[j];
+        ProfScope ps(this, st);
+        backtrack_kernel<T><<<bt_grid, 256, 0, st>>>(U);
+        launches++;
+        SGP_CUDA_TRY(cudaGetLastError());
+    }
+    cur_slot = -1;
+    return SGP_OK;
+}
+
 template <typename T>
 int PlanImpl<T>::enqueue_sgp_iteration(const RowParams<T> &Pb, const DevOpts &o, const Trace &tr, const double *bconst,
                                        int b_is_array, cudaStream_t st)
 {
     int rc;
-    cur_slot = SGP_PROF_K1;
-    {   // K1 (a10 for q, a1)
-        RowParams<T> P = Pb; P.lazy = 1; P.in0 = Gp; P.in1 = q; P.in2 = Bp; P.in3 = u; P.out0 = q;
-        if ((rc = launch_row(k_rowf[RF_RATIO], P, p, st))) return rc;
-    }
     cur_slot = SGP_PROF_K2;
     {   // K2 (a2)
         ColParams<T> Q = col_params(); Q.check_status = 1;
@@ -71,19 +101,20 @@ int PlanImpl<T>::enqueue_sgp_iteration(const RowParams<T> &Pb, const DevOpts &o,
         RowParams<T> P = Pb; P.in0 = Gp; P.in1 = q; P.in2 = Bp; P.out0 = u; P.part = part_J; P.part2 = part_gd;
         if ((rc = launch_row(k_rowi[fuse_ls ? RI_LSF : RI_LS], P, p, st))) return rc;
     }
-    cur_slot = SGP_PROF_K7;
-    {   // K7 (a9 backtracks, a11)
-        BtParams<T> U;
-        memset(&U, 0, sizeof(U));
-        U.G = G; U.o = o; U.tr = tr; U.ct = ct; U.q = q; U.u = u; U.g = Gp; U.b = Bp;
-        U.plane = n; U.qbuf = n * (size_t)p; U.b_is_array = b_is_array; U.part = part_bt;
-        for (int j = 0; j < p; ++j) U.bconst[j] = bconst[j];
-        ProfScope ps(this, st);
-        backtrack_kernel<T><<<bt_grid, 256, 0, st>>>(U);
-        launches++;
-        SGP_CUDA_TRY(cudaGetLastError());
-    }
     cur_slot = -1;
+    // ---- tail: K7 (a9 backtracks, a11) and K1 of the next iteration (a10 for q, a1)
+    if (st == cap_stream && cap_stream2 && (opt.use_graph & 32)) {
+        SGP_CUDA_TRY(cudaEventRecord(ev_fork, st));
+        SGP_CUDA_TRY(cudaStreamWaitEvent(cap_stream2, ev_fork, 0));
+        if ((rc = enqueue_backtrack(o, tr, bconst, b_is_array, cap_stream2))) return rc;
+        if ((rc = enqueue_ratio(Pb, 2, cap_stream2))) return rc;
+        SGP_CUDA_TRY(cudaEventRecord(ev_join, cap_stream2));
+        if ((rc = enqueue_ratio(Pb, 1, st))) return rc;
+        SGP_CUDA_TRY(cudaStreamWaitEvent(st, ev_join, 0));
+    } else {
+        if ((rc = enqueue_backtrack(o, tr, bconst, b_is_array, st))) return rc;
+        if ((rc = enqueue_ratio(Pb, 3, st))) return rc;
+    }
     return SGP_OK;
 }
 
@@ -164,6 +195,9 @@ int PlanImpl<T>::enqueue_many(int algorithm, int count, const RowParams<T> &Pb, 
     if ((opt.use_graph & 1) && !profiling && count >= kGraphIters) {
         if (!gexec) {
             if (!cap_stream) SGP_CUDA_TRY(cudaStreamCreateWithFlags(&cap_stream, cudaStreamNonBlocking));
+            if (!cap_stream2) SGP_CUDA_TRY(cudaStreamCreateWithFlags(&cap_stream2, cudaStreamNonBlocking));
+            if (!ev_fork) SGP_CUDA_TRY(cudaEventCreateWithFlags(&ev_fork, cudaEventDisableTiming));
+            if (!ev_join) SGP_CUDA_TRY(cudaEventCreateWithFlags(&ev_join, cudaEventDisableTiming));
             cudaGraph_t g = nullptr;
             const long l0 = launches;
             SGP_CUDA_TRY(cudaStreamBeginCapture(cap_stream, cudaStreamCaptureModeThreadLocal));
@@ -233,7 +267,7 @@ int PlanImpl<T>::run(int algorithm, const void *const *g, const void *const *b_a
     Ctrl h;
     memset(&h, 0, sizeof(h));
     h.alpha_prev = ro.alpha0; h.tau = ro.tau1; h.L1 = ro.L1; h.L2 = ro.L2; h.lambda = 1.0;
-    h.qsel = 0; h.need_k1 = 1;
+    h.qsel = 0; h.need_k1 = 1; h.accepted = 1;
     SGP_CUDA_TRY(cudaMemcpyAsync(ct, &h, sizeof(Ctrl), cudaMemcpyHostToDevice, st));
     SGP_CUDA_TRY(cudaMemsetAsync(q + n * (size_t)p, 0, sizeof(T) * n * (size_t)p, st));     // second q buffer: zero outside S
     const int eg = ew_grid(n) > 1024 ? 1024 : ew_grid(n);
@@ -279,6 +313,7 @@ int PlanImpl<T>::run(int algorithm, const void *const *g, const void *const *b_a
         int chunk = ro.check_every > 0 ? ro.check_every : (ro.stop_rule == SGP_STOP_MAXIT ? 200 : 20);
         if (algorithm == SGP_ALG_SGP) {
             if (ro.max_iter == 0) status = SGP_REASON_MAXIT;
+            else if ((rc = enqueue_ratio(Pb, 3, st))) return rc;        // K1 of iteration 0; every iteration enqueues the next one's
             int done = 0;
             while (status == 0) {
                 int todo = ro.max_iter - done; if (todo > chunk) todo = chunk;

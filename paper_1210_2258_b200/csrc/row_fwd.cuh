@@ -157,7 +157,17 @@ __global__ void __launch_bounds__(256, 2) row_fwd_kernel(const RowParams<T> P)
         const T bc = (T)P.bconst[j];
         const bool rowin = (unsigned)(y - G.oy) < (unsigned)G.sy;
         int todo = 1, sel = 0;
-        if (P.lazy) { todo = P.ct->need_k1; if (todo == 0) return; sel = P.ct->qsel; }
+        if (P.lazy) {
+            // Two instances of this kernel follow the line-search kernel (plan_run.inl): lazy = 1 runs BESIDE the
+            // backtracking kernel and works only if lambda = 1 was accepted (Ctrl::accepted is written by the line-search
+            // kernel alone, so it is stable here; nothing else of the control block is read before this test, because the
+            // backtracking kernel rewrites it when it has work); lazy = 2 runs BEHIND the backtracking kernel and works
+            // only if that had to find lambda < 1; lazy = 3 (plain stream order) takes either case.
+            const int acc = P.ct->accepted;
+            if ((P.lazy == 1 && acc == 0) || (P.lazy == 2 && acc != 0)) return;
+            if (P.ct->status != 0) return;
+            todo = P.ct->need_k1; if (todo == 0) return; sel = P.ct->qsel;
+        }
         const bool pend = todo == 2;
         const T *qsrc = P.in1 + (size_t)(pend ? sel ^ 1 : sel) * P.qbuf;
         T *qdst = P.out0 + (size_t)sel * P.qbuf;
