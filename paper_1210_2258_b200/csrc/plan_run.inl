@@ -242,11 +242,10 @@ int PlanImpl<T>::run(int algorithm, const void *const *g, const void *const *b_a
     const long launches0 = launches;
     if (profiling) prof_reset();
     // Column product kernels of this run.  The two-CTAs-per-SM form (col2_kernel) is 25-30 % faster where the tiles
-    // make several waves (4096^2: 82 -> 59 us) and 8 % faster in the RL / OSEM loops at 2048^2 (25 -> 23 us); in the
-    // SGP loop at 2048^2 its single wave (all CTAs load, transform and store in phase) is slower (31 vs 27 us behind
-    // the ratio kernel's write-backs), so the one-CTA form with the TMA-staged transfer function stays there.
+    // make several waves (4096^2: 82 -> 58 us per pass); at 2048^2 its single wave (all CTAs load, transform and store
+    // in phase) loses to the one-CTA form with the TMA-staged transfer function (SGP: 31 vs 23 us; RL: 24 vs 21 us).
     {
-        const bool use2 = col2 && (algorithm != SGP_ALG_SGP || ntiles > 2 * nsm);
+        const bool use2 = col2 && ntiles > 2 * nsm;
         k_conj_run = use2 ? k_conj2 : k_conj;
         k_mult_run = use2 ? k_mult2 : k_mult;
     }
