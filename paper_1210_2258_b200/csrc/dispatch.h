@@ -9,8 +9,8 @@ template <typename T> using row_kernel_t = void (*)(const RowParams<T>);
 template <typename T> using col_kernel_t = void (*)(const ColParams<T>);
 
 // L = nx/2 (row kernels) or ny (column kernel); nullptr if the length is not supported
-template <typename T> row_kernel_t<T> get_row_fwd(int L, int mode);
-template <typename T> row_kernel_t<T> get_row_inv(int L, int mode);
+template <typename T> row_kernel_t<T> get_row_fwd(int L, int mode, bool masked);
+template <typename T> row_kernel_t<T> get_row_inv(int L, int mode, bool masked);
 // tile_cols: the plan's tile width; the product modes have a variant compiled for the default width (col.cuh)
 template <typename T> col_kernel_t<T> get_col(int L, int mode, bool multi, int tile_cols = 0);
 // two-CTAs-per-SM form of the single-image product modes (col.cuh: col2_kernel); nullptr where it does not exist

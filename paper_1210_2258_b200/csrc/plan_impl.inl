@@ -130,8 +130,8 @@ template <typename T> struct PlanImpl : PlanBase {
         Lr = nx / 2; Lc = ny;
         constexpr int dummy = 0; (void)dummy;
         const int Er = fft_E<T>(Lr), Ec = fft_E_col<T>(Lc);
-        for (int m = 0; m < RF_NMODES; ++m) if (!(k_rowf[m] = get_row_fwd<T>(Lr, m))) return SGP_ERR_ARG;
-        for (int m = 0; m < RI_NMODES; ++m) if (!(k_rowi[m] = get_row_inv<T>(Lr, m))) return SGP_ERR_ARG;
+        for (int m = 0; m < RF_NMODES; ++m) if (!(k_rowf[m] = get_row_fwd<T>(Lr, m, G.masked != 0))) return SGP_ERR_ARG;
+        for (int m = 0; m < RI_NMODES; ++m) if (!(k_rowi[m] = get_row_inv<T>(Lr, m, G.masked != 0))) return SGP_ERR_ARG;
         int Cc = 0, RB = 0;
         int rc = choose_tiles(ny, nx, dtype, &opt, &Cc, &RB);
         if (rc) return rc;

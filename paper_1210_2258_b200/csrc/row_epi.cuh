@@ -177,7 +177,7 @@ __device__ __forceinline__ void epi_kl(const RowParams<T> &P, const T *wrow, T *
 }
 
 // plain store with the output mask of Eq.16 (M_S) or Eq.17 (M_R)
-template <typename T, int L, int TF>
+template <typename T, int L, int TF, bool MK>
 __device__ __forceinline__ void epi_store(const RowParams<T> &P, const T *wrow, int t, int y, size_t rowbase, size_t base)
 {
     const Geom &G = P.G;
@@ -192,7 +192,7 @@ __device__ __forceinline__ void epi_store(const RowParams<T> &P, const T *wrow, 
             quad_in_S<T>(G, rowin, x, s);
 #pragma unroll
             for (int c = 0; c < 4; ++c) if (!s[c]) w4.a[c] = (T)0;
-        } else if (P.maskmode == MM_R && G.masked) {
+        } else if (P.maskmode == MM_R && MK) {
             const Quad<T> a4 = ldq<T>(P.alphaR + rowbase + x);
 #pragma unroll
             for (int c = 0; c < 4; ++c) if (!(a4.a[c] > (T)0)) w4.a[c] = (T)0;
@@ -203,7 +203,7 @@ __device__ __forceinline__ void epi_store(const RowParams<T> &P, const T *wrow, 
 
 // y = (M_R/alpha) f w: one RL step (Eq.1/13/21).  STORE: write it (a12); else accumulate (-min positive, max) for
 // the adaptive bounds (A19).
-template <typename T, int L, int TF, bool STORE>
+template <typename T, int L, int TF, bool STORE, bool MK>
 __device__ __forceinline__ void epi_rl(const RowParams<T> &P, const T *wrow, int t, size_t rowbase, double (&acc)[2])
 {
     const Geom &G = P.G;
@@ -217,7 +217,7 @@ __device__ __forceinline__ void epi_rl(const RowParams<T> &P, const T *wrow, int
             const int x = 4 * (t + TF * (it0 + u));
             w4[u] = ldq<T>(wrow + x);
             f4[u] = ldq<T>(P.in0 + rowbase + x);
-            if (G.masked) a4[u] = ldq<T>(P.alphaR + rowbase + x);
+            if (MK) a4[u] = ldq<T>(P.alphaR + rowbase + x);
         }
 #pragma unroll
         for (int u = 0; u < U; ++u) {
@@ -226,7 +226,7 @@ __device__ __forceinline__ void epi_rl(const RowParams<T> &P, const T *wrow, int
 #pragma unroll
             for (int c = 0; c < 4; ++c) {
                 T wv = Wc;
-                if (G.masked) wv = a4[u].a[c] > (T)0 ? (T)1 / a4[u].a[c] : (T)0;
+                if (MK) wv = a4[u].a[c] > (T)0 ? (T)1 / a4[u].a[c] : (T)0;
                 y4.a[c] = wv * f4[u].a[c] * w4[u].a[c];
                 if constexpr (!STORE) {
                     const double yd = (double)y4.a[c];

@@ -86,7 +86,9 @@ __device__ __forceinline__ void fwd_fft_store(cx<T> (&v)[fft_E<T>(L)], cx<T> *sm
     }
 }
 
-template <typename T, int L, int MODE>
+// MK: the plan has a boundary mask (alphaR plane present); a template parameter so that the unmasked kernels carry none of
+// the mask branches (their registers and instructions cost 1.2-2.3 us per row kernel at 2048^2)
+template <typename T, int L, int MODE, bool MK>
 __global__ void __launch_bounds__(256, 2) row_fwd_kernel(const RowParams<T> P)
 {
     using C = cx<T>;
@@ -122,7 +124,7 @@ __global__ void __launch_bounds__(256, 2) row_fwd_kernel(const RowParams<T> P)
             if (P.maskmode == MM_S) {
                 if (!(rowin && (unsigned)(x0 - G.ox) < (unsigned)G.sx)) w2.x = (T)0;
                 if (!(rowin && (unsigned)(x0 + 1 - G.ox) < (unsigned)G.sx)) w2.y = (T)0;
-            } else if (P.maskmode == MM_R && G.masked) {
+            } else if (P.maskmode == MM_R && MK) {
                 C a2 = ld2<T>(P.alphaR + (size_t)y * nx + x0);
                 if (!(a2.x > (T)0)) w2.x = (T)0;
                 if (!(a2.y > (T)0)) w2.y = (T)0;
@@ -236,7 +238,7 @@ __global__ void __launch_bounds__(256, 2) row_fwd_kernel(const RowParams<T> P)
 #pragma unroll
         for (int e0 = 0; e0 < E; e0 += U) {
             C a2[U];
-            if (G.masked) {
+            if (MK) {
 #pragma unroll
                 for (int u = 0; u < U; ++u) a2[u] = ld2<T>(P.alphaR + base + 2 * (t + TF * (e0 + u)));
             }
@@ -246,7 +248,7 @@ __global__ void __launch_bounds__(256, 2) row_fwd_kernel(const RowParams<T> P)
                 const C f2 = frow[t + TF * (e0 + u)], g2 = v[e0 + u];
                 C w2 = mk<T>(Wc, Wc);
                 bool r0 = true, r1 = true;
-                if (G.masked) {
+                if (MK) {
                     r0 = a2[u].x > (T)0; r1 = a2[u].y > (T)0;
                     w2.x = r0 ? (T)1 / a2[u].x : (T)0; w2.y = r1 ? (T)1 / a2[u].y : (T)0;
                 }

@@ -19,7 +19,7 @@ template <typename T> __device__ __forceinline__ void retangle(cx<T> a, cx<T> xb
     zlk = cconj(csub(Sk, Tm));
 }
 
-template <typename T, int L, int MODE>
+template <typename T, int L, int MODE, bool MK>
 __global__ void __launch_bounds__(256, 2) row_inv_kernel(const RowParams<T> P)
 {
     using C = cx<T>;
@@ -105,11 +105,11 @@ __global__ void __launch_bounds__(256, 2) row_inv_kernel(const RowParams<T> P)
 
     if constexpr (MODE == RI_PLAIN) {
         if (P.submode == RIP_STORE) {
-            epi_store<T, L, TF>(P, wrow, t, y, rowbase, base);
+            epi_store<T, L, TF, MK>(P, wrow, t, y, rowbase, base);
         } else {
             // RIP_RLMINMAX: adaptive bounds from one RL step (A19)
             double acc[2] = {-INFINITY, -INFINITY};   // (-min positive, max)
-            epi_rl<T, L, TF, false>(P, wrow, t, rowbase, acc);
+            epi_rl<T, L, TF, false, MK>(P, wrow, t, rowbase, acc);
             // max-reduction over the block (fixed tree)
             const int lane = tid & 31, wid = tid >> 5, nw = (blockDim.x + 31) >> 5;
 #pragma unroll
@@ -136,8 +136,7 @@ __global__ void __launch_bounds__(256, 2) row_inv_kernel(const RowParams<T> P)
         }
     } else if constexpr (MODE == RI_GRAD) {
         double acc[4] = {0.0, 0.0, 0.0, 0.0};
-        if (G.masked) epi_grad<T, L, TF, true>(P, wrow, t, rowbase, acc);
-        else          epi_grad<T, L, TF, false>(P, wrow, t, rowbase, acc);
+        epi_grad<T, L, TF, MK>(P, wrow, t, rowbase, acc);
         block_reduce_sum<4>(acc, red);
         if (publish_partials<4>(acc, P.part, bid, nblk, &P.ct->counter[TK_GRAD])) {
             final_sum<4>(acc, P.part, nblk, red);
@@ -152,8 +151,7 @@ __global__ void __launch_bounds__(256, 2) row_inv_kernel(const RowParams<T> P)
         const T *qin = P.in1 + (size_t)sel * P.qbuf;
         T *qout = SPEC ? const_cast<T *>(P.in1) + (size_t)(sel ^ 1) * P.qbuf : nullptr;
         T *wmut = reinterpret_cast<T *>(smrow);
-        if (G.masked) epi_kl<T, L, TF, LS, true, SPEC>(P, wrow, wmut, qin, qout, t, y, j, base, plain, acc);
-        else          epi_kl<T, L, TF, LS, false, SPEC>(P, wrow, wmut, qin, qout, t, y, j, base, plain, acc);
+        epi_kl<T, L, TF, LS, MK, SPEC>(P, wrow, wmut, qin, qout, t, y, j, base, plain, acc);
         if (plain) return;
         block_reduce_sum<1>(acc, red);
         const int tk = LS ? TK_LS : TK_QJ;
@@ -207,7 +205,7 @@ __global__ void __launch_bounds__(256, 2) row_inv_kernel(const RowParams<T> P)
         }
     } else {   // RI_RLUPDATE, a12: f <- (M_R/alpha) o f o sum_j A_j^T(g_j/(A_j f + b_j))   (Eq.1/13/21)
         double dummy[2];
-        epi_rl<T, L, TF, true>(P, wrow, t, rowbase, dummy);
+        epi_rl<T, L, TF, true, MK>(P, wrow, t, rowbase, dummy);
     }
 }
 
