@@ -84,17 +84,45 @@ __global__ void __launch_bounds__(256) backtrack_kernel(const BtParams<T> P)
             const T *q = qcur + (size_t)j * P.plane, *u = P.u + (size_t)j * P.plane, *g = P.g + (size_t)j * P.plane;
             const T *b = P.b_is_array ? P.b + (size_t)j * P.plane : nullptr;
             const T bc = (T)P.bconst[j];
-            for (size_t i = gtid; i < nv; i += gstride) {
-                const size_t i0 = i * VN;
-                const int y = (int)(i0 / G.nx), x = (int)(i0 - (size_t)y * G.nx);
-                if ((unsigned)(y - G.oy) >= (unsigned)G.sy) continue;
-                V q4 = reinterpret_cast<const V *>(q)[i], u4 = reinterpret_cast<const V *>(u)[i], g4 = reinterpret_cast<const V *>(g)[i];
-                const T *qa = reinterpret_cast<const T *>(&q4), *ua = reinterpret_cast<const T *>(&u4), *ga = reinterpret_cast<const T *>(&g4);
+            // four vectors per thread and step, all loads issued before the first use (the trial is one pass over three
+            // planes: what counts is how many bytes each thread has in flight)
+            constexpr int UN = 4;
+            for (size_t i0 = gtid; i0 < nv; i0 += UN * gstride) {
+                V q4[UN], u4[UN], g4[UN];
+                bool ok[UN];
 #pragma unroll
-                for (int c = 0; c < VN; ++c) {
-                    if ((unsigned)(x + c - G.ox) < (unsigned)G.sx) {
-                        const T bb = b ? b[i0 + c] : bc;
-                        acc[0] += (double)kl_term(ga[c], (T)((T)(qa[c] + lam * ua[c]) + bb));
+                for (int k4 = 0; k4 < UN; ++k4) {
+                    const size_t i = i0 + (size_t)k4 * gstride;
+                    ok[k4] = i < nv;
+                    if (ok[k4]) {
+                        q4[k4] = reinterpret_cast<const V *>(q)[i]; u4[k4] = reinterpret_cast<const V *>(u)[i];
+                        g4[k4] = reinterpret_cast<const V *>(g)[i];
+                    }
+                }
+#pragma unroll
+                for (int k4 = 0; k4 < UN; ++k4) {
+                    if (!ok[k4]) continue;
+                    const size_t e0 = (i0 + (size_t)k4 * gstride) * VN;
+                    const int y = (int)(e0 / G.nx), x = (int)(e0 - (size_t)y * G.nx);
+                    if ((unsigned)(y - G.oy) >= (unsigned)G.sy) continue;
+                    const T *qa = reinterpret_cast<const T *>(&q4[k4]), *ua = reinterpret_cast<const T *>(&u4[k4]), *ga = reinterpret_cast<const T *>(&g4[k4]);
+                    if constexpr (VN == 4) {
+                        T yv[4], gv[4]; bool s[4];
+#pragma unroll
+                        for (int c = 0; c < 4; ++c) {
+                            s[c] = (unsigned)(x + c - G.ox) < (unsigned)G.sx;
+                            const T bb = b ? b[e0 + c] : bc;
+                            yv[c] = (T)((T)(qa[c] + lam * ua[c]) + bb); gv[c] = ga[c];
+                        }
+                        acc[0] += (double)kl_quad(gv, yv, s);
+                    } else {
+#pragma unroll
+                        for (int c = 0; c < VN; ++c) {
+                            if ((unsigned)(x + c - G.ox) < (unsigned)G.sx) {
+                                const T bb = b ? b[e0 + c] : bc;
+                                acc[0] += (double)kl_term(ga[c], (T)((T)(qa[c] + lam * ua[c]) + bb));
+                            }
+                        }
                     }
                 }
             }
