@@ -60,6 +60,7 @@ typedef struct {
     int init;
     int refresh_every;      /* A21: 0 = never recompute A f from f */
     int strict;             /* A17: 1 = negative g is an error instead of being clamped */
+    double rl_relax;        /* Eq.3: exponent of the multiplicative relaxation of RL; 1 = plain RL */
 } oracle_options;
 
 typedef struct {
