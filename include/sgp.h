@@ -105,6 +105,8 @@ typedef struct sgp_options {
                                                     separate / the fused line-search kernel (default: chosen by working set vs L2),
                                                     bit 4 = never use the two-CTAs-per-SM column kernel, bit 5 = fork the backtracking /
                                                     ratio tail inside the graph */
+    double rl_relax;                             /* rl_* only: exponent of the multiplicative relaxation, Eq.3:
+                                                    f <- f o (W o sum_j A_j^T(g_j/(A_j f + b_j)))^rl_relax; 1 (default) = plain RL */
 } sgp_options;
 
 /* Result of a run.  The trace pointers are optional caller-allocated HOST arrays of max_iter+1 entries

@@ -803,7 +803,7 @@ int oracle_rl_run(const oracle_problem *P, const oreal *const *g_in, const oreal
                     r[j][i2] = P->MS[i2] ? ratio_term(g[j][i2], q[j][i2] + b[j][i2]) : (oreal)0;
             rc = oracle_sum_AT(P, (const oreal *const *)r, w);
             if (rc) goto done;
-            for (size_t i2 = 0; i2 < n; ++i2) f[i2] = f[i2] * (oreal)pow((double)(P->W[i2] * w[i2]), o->rl_relax);
+            for (size_t i2 = 0; i2 < n; ++i2) f[i2] = f[i2] * (oreal)pow(fmax(0.0, (double)(P->W[i2] * w[i2])), o->rl_relax);   /* base >= 0 up to FFT round-off */
         }
     }
     res->n_fft2 = g_fft2_count - fft0;

@@ -257,6 +257,7 @@ int PlanImpl<T>::run(int algorithm, const void *const *g, const void *const *b_a
     o.armijo_memory = ro.armijo_memory; o.max_iter = ro.max_iter; o.stop_rule = ro.stop_rule;
     o.max_backtracks = ro.max_backtracks; o.adaptive_L = ro.adaptive_L; o.p = p;
     o.nS_total = (double)p * (double)G.sy * (double)G.sx;
+    o.rl_relax = algorithm == SGP_ALG_RL ? ro.rl_relax : 1.0;      // Eq.3 is a variant of RL (Eq.1/13/21) only
 
     Trace tr;
     if ((rc = ensure_trace(ro.max_iter, res, &tr, st))) return rc;

@@ -208,6 +208,8 @@ __device__ __forceinline__ void epi_rl(const RowParams<T> &P, const T *wrow, int
 {
     const Geom &G = P.G;
     const T Wc = (T)(1.0 / (double)G.p);
+    const bool relax = P.o.rl_relax != 1.0;          // multiplicative relaxation of RL, Eq.3
+    const T rx = (T)P.o.rl_relax;
     constexpr int NIT = (L / 2) / TF;
     constexpr int U = batch_len<T>(NIT);
     for (int it0 = 0; it0 < NIT; it0 += U) {
@@ -228,6 +230,7 @@ __device__ __forceinline__ void epi_rl(const RowParams<T> &P, const T *wrow, int
                 T wv = Wc;
                 if (MK) wv = a4[u].a[c] > (T)0 ? (T)1 / a4[u].a[c] : (T)0;
                 y4.a[c] = wv * f4[u].a[c] * w4[u].a[c];
+                if (STORE && relax) y4.a[c] = f4[u].a[c] * pow(fmax(wv * w4[u].a[c], (T)0), rx);      // Eq.3
                 if constexpr (!STORE) {
                     const double yd = (double)y4.a[c];
                     if (yd > 0.0) acc[0] = fmax(acc[0], -yd);
