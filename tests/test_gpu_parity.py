@@ -539,3 +539,29 @@ def test_rl_multiplicative_relaxation_parity(cfg, dt, tol):
     f1, _ = plan.rl(g, w["b"], opts=o)
     plan.close()
     assert np.array_equal(f1.cpu().numpy(), fp)
+
+
+# ---------------------------------------------------------------- the start points of PAPER.md:260-267
+@pytest.mark.parametrize("dt,tol", [(np.float32, 1e-4), (np.float64, 1e-10)])
+@pytest.mark.parametrize("cfg", ["C0", "C2", "C3"])
+def test_start_points_noisy_image_and_null_image(cfg, dt, tol):
+    """init = G: the noisy image g (g_1 for several images, restricted to R with boundary correction); init = ZERO:
+    the null image.  10 SGP iterations (and 5 RL steps from g) against the oracle from the same start."""
+    _need_gpu()
+    w = {"C0": lambda: synth.make("C0", n=128), "C2": lambda: synth.make("C2", n=128),
+         "C3": lambda: synth.make("C3", s=256, sbar=320, n_stars=150, max_iter=60, fwhm=64.0)}[cfg]()
+    # the null image needs fixed scaling bounds (the adaptive rule of PAPER.md:273-275 has no positive value to start from),
+    # and bounds large enough for the first steps to change J0 by more than the fp32 noise of its evaluation
+    for init, iters, extra in ((B.INIT_G, 10, {}), (B.INIT_ZERO, 5, {"adaptive_L": 0, "L1": 1e-3, "L2": 1e10})):
+        fg, rg, fo, ro = run_both(w, dt, max_iter=iters, stop_rule=0, init=init, **extra)
+        assert rg.iterations == ro.iterations == iters
+        assert rel_l2(fg, fo) <= tol * (10 if dt == np.float32 else 1)
+        assert abs(rg.J[0] - ro.J[0]) <= (1e-6 if dt == np.float32 else 1e-12) * abs(ro.J[0])      # J0 at the start point itself
+        assert abs(rg.J0_final - ro.J0_final) <= (1e-4 if dt == np.float32 else 1e-11) * abs(ro.J0_final)
+    if cfg != "C0":      # with the adaptive bounds the null image is rejected, not silently accepted
+        plan, o = gpu_plan(w, dt, max_iter=3, stop_rule=0, init=B.INIT_ZERO)
+        _, r = plan.sgp([dev(a, dt) for a in w["g"]], w["b"], opts=o, check=False)
+        plan.close()
+        assert r.rc == B.ERR_DATA
+    fg, rg, fo, ro = run_both(w, dt, alg="rl", max_iter=5, stop_rule=0, init=B.INIT_G)
+    assert rel_l2(fg, fo) <= tol
