@@ -50,7 +50,7 @@ class Options(C.Structure):
         ("L1", C.c_double), ("L2", C.c_double), ("adaptive_L", C.c_int),
         ("max_iter", C.c_int), ("stop_rule", C.c_int), ("tol", C.c_double), ("disc_threshold", C.c_double),
         ("sigma_R", C.c_double), ("max_backtracks", C.c_int), ("psf_origin", C.c_int), ("init", C.c_int),
-        ("refresh_every", C.c_int), ("strict", C.c_int), ("rl_relax", C.c_double),
+        ("refresh_every", C.c_int), ("strict", C.c_int), ("rl_relax", C.c_double), ("rl_linear", C.c_double),
     ]
 
 

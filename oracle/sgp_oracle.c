@@ -498,7 +498,7 @@ void oracle_options_default(oracle_options *o)
     o->max_iter = 100; o->stop_rule = ORACLE_STOP_MAXIT; o->tol = 1e-5;
     o->disc_threshold = 1.0; o->sigma_R = 1e-2; o->max_backtracks = 30;
     o->psf_origin = ORACLE_PSF_CENTER; o->init = ORACLE_INIT_CONST;
-    o->refresh_every = 0; o->strict = 0; o->rl_relax = 1.0;
+    o->refresh_every = 0; o->strict = 0; o->rl_relax = 1.0; o->rl_linear = 1.0;
 }
 
 void oracle_bb_init(oracle_bb_state *s, const oracle_options *o)
@@ -581,6 +581,8 @@ static int make_start(const oracle_problem *P, const oreal *const *g, const orea
 static int check_options(const oracle_options *o)
 {
     if (o && !(o->rl_relax > 0.0)) return ORACLE_ERR_ARG;
+    if (o && !(o->rl_linear > 0.0)) return ORACLE_ERR_ARG;
+    if (o && o->rl_relax != 1.0 && o->rl_linear != 1.0) return ORACLE_ERR_ARG;      /* Eq.3 and Eq.4 are alternatives */
     if (!o) return ORACLE_ERR_ARG;
     if (!(o->beta > 0 && o->beta < 1 && o->theta > 0 && o->theta < 1)) return ORACLE_ERR_ARG;
     if (!(o->alpha_min > 0 && o->alpha_min < o->alpha_max)) return ORACLE_ERR_ARG;
@@ -792,7 +794,18 @@ int oracle_rl_run(const oracle_problem *P, const oreal *const *g_in, const oreal
         res->iterations = k;
         res->stop_reason = stop_test(o, P, k, J, Jold, k > 0);
         if (res->stop_reason) break;
-        if (o->rl_relax == 1.0) {
+        if (o->rl_linear != 1.0) {
+            /* linear relaxation, Eq.4 (Adorf et al.): f(k+1) = f(k) - lambda_k f(k) o (1 - A^T g/(Af+b)), here with a
+               constant lambda_k = rl_linear; for p images / boundary correction the subtracted array is f o (1 - W o sum_j
+               A_j^T(...)), i.e. f minus the RL step of Eq.13 / Eq.21 (reading A25).  No projection: Eq.4 has none. */
+            for (int j = 0; j < p; ++j)
+                for (size_t i2 = 0; i2 < n; ++i2)
+                    r[j][i2] = P->MS[i2] ? ratio_term(g[j][i2], q[j][i2] + b[j][i2]) : (oreal)0;
+            rc = oracle_sum_AT(P, (const oreal *const *)r, w);
+            if (rc) goto done;
+            for (size_t i2 = 0; i2 < n; ++i2)
+                f[i2] = f[i2] - (oreal)o->rl_linear * (f[i2] * ((oreal)1 - P->W[i2] * w[i2]));
+        } else if (o->rl_relax == 1.0) {
             rc = rl_update_from_q(P, f, q, (const oreal *const *)g, b, r, w, f);
             if (rc) goto done;
         } else {
