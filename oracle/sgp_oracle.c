@@ -797,14 +797,17 @@ int oracle_rl_run(const oracle_problem *P, const oreal *const *g_in, const oreal
         if (o->rl_linear != 1.0) {
             /* linear relaxation, Eq.4 (Adorf et al.): f(k+1) = f(k) - lambda_k f(k) o (1 - A^T g/(Af+b)), here with a
                constant lambda_k = rl_linear; for p images / boundary correction the subtracted array is f o (1 - W o sum_j
-               A_j^T(...)), i.e. f minus the RL step of Eq.13 / Eq.21 (reading A25).  No projection: Eq.4 has none. */
+               A_j^T(...)), i.e. f minus the RL step of Eq.13 / Eq.21, and the result is projected on f >= 0 (reading A25). */
             for (int j = 0; j < p; ++j)
                 for (size_t i2 = 0; i2 < n; ++i2)
                     r[j][i2] = P->MS[i2] ? ratio_term(g[j][i2], q[j][i2] + b[j][i2]) : (oreal)0;
             rc = oracle_sum_AT(P, (const oreal *const *)r, w);
             if (rc) goto done;
             for (size_t i2 = 0; i2 < n; ++i2)
-                f[i2] = f[i2] - (oreal)o->rl_linear * (f[i2] * ((oreal)1 - P->W[i2] * w[i2]));
+            {
+                oreal y = f[i2] - (oreal)o->rl_linear * (f[i2] * ((oreal)1 - P->W[i2] * w[i2]));
+                f[i2] = y > (oreal)0 ? y : (oreal)0;       /* the non-negativity constraint of the paper, reading A25 */
+            }
         } else if (o->rl_relax == 1.0) {
             rc = rl_update_from_q(P, f, q, (const oreal *const *)g, b, r, w, f);
             if (rc) goto done;

@@ -61,7 +61,7 @@ typedef struct {
     int refresh_every;      /* A21: 0 = never recompute A f from f */
     int strict;             /* A17: 1 = negative g is an error instead of being clamped */
     double rl_relax;        /* Eq.3: exponent of the multiplicative relaxation of RL; 1 = plain RL */
-    double rl_linear;       /* Eq.4: constant lambda_k of the linear relaxation of RL; 1 = plain RL (reading A25) */
+    double rl_linear;       /* Eq.4: constant lambda_k of the linear relaxation of RL; result projected on f >= 0; 1 = plain RL (reading A25) */
 } oracle_options;
 
 typedef struct {

@@ -646,7 +646,8 @@ def test_P14_linear_relaxation_is_eq4(p, masked, S):
     """PAPER.md:50, Eq.4: f(k+1) = f(k) - lambda f(k) o (1 - A^T g/(A f(k) + b)) written out with the operators of
     Eq.16/17 (constant lambda_k, reading A25; for p images / boundary correction the bracket holds the RL factor of
     Eq.13 / Eq.21); lambda = 1 is RL itself; one step is the point (1 - lambda) f + lambda f_RL on the
-    line through f and the RL step ("a line search along this descent direction"); the flux invariant of
+    line through f and the RL step ("a line search along this descent direction"), projected on f >= 0
+    (the paper's constraint); the flux invariant of
     RL survives for p = 1 unmasked (sum f(k+1) = sum(g - b) whenever sum f(k) is); the true object of a noiseless
     problem is a fixed point; J0 after a few relaxed steps is below plain RL."""
     rng = np.random.default_rng(140 + p)
@@ -658,7 +659,7 @@ def test_P14_linear_relaxation_is_eq4(p, masked, S):
     f = f0.copy()
     for _ in range(K):
         w = sum(P.AT(j, np.where(P.A(j, f) + b[j] > 0, g[j] / (P.A(j, f) + b[j]), 0.0)) for j in range(P.p))
-        f = f - lam * f * (1.0 - info["W"] * w)
+        f = np.maximum(0.0, f - lam * f * (1.0 - info["W"] * w))      # projected on f >= 0 (reading A25)
     assert np.abs(f_or - f).max() <= 1e-12 * np.abs(f).max()
     f1, _ = P.rl(g, b, f0, oracle.default_options(max_iter=K, init=oracle.INIT_USER, rl_linear=1.0))
     f2, _ = P.rl(g, b, f0, oracle.default_options(max_iter=K, init=oracle.INIT_USER))
@@ -666,14 +667,19 @@ def test_P14_linear_relaxation_is_eq4(p, masked, S):
     # one step lies on the line through f0 and the plain RL step
     fl, _ = P.rl(g, b, f0, oracle.default_options(max_iter=1, init=oracle.INIT_USER, rl_linear=lam))
     fr, _ = P.rl(g, b, f0, oracle.default_options(max_iter=1, init=oracle.INIT_USER))
-    assert np.abs(fl - ((1 - lam) * f0 + lam * fr)).max() <= 1e-12 * np.abs(fr).max()
+    assert np.abs(fl - np.maximum(0.0, (1 - lam) * f0 + lam * fr)).max() <= 1e-12 * np.abs(fr).max()
     assert np.abs(fl - fr).max() > 1e-3 * np.abs(fr).max()                    # and is not the RL step itself
     if p == 1 and not masked:
         # flux: sum f_RL = sum g f/(Af+b) A1 ... for b = 0 and a unit-volume PSF sum f_RL = sum g; the relaxed step keeps
         # (1 - lam) sum f0 + lam sum g
         g0 = [P.A(0, truth)]
         fz, _ = P.rl(g0, [np.zeros_like(truth)], f0, oracle.default_options(max_iter=1, init=oracle.INIT_USER, rl_linear=lam))
-        assert abs(fz.sum() - ((1 - lam) * f0.sum() + lam * g0[0].sum())) <= 1e-11 * g0[0].sum()
+        if fz[f0 > 0].min() > 0:      # no pixel was projected
+            assert abs(fz.sum() - ((1 - lam) * f0.sum() + lam * g0[0].sum())) <= 1e-11 * g0[0].sum()
+        # a start point far above the data: the unprojected step (1 - lam) f + lam f_RL is negative there, the result is 0
+        fbig = f0.copy(); fbig[3, 4] = 1e6
+        fc, _ = P.rl(g, b, fbig, oracle.default_options(max_iter=1, init=oracle.INIT_USER, rl_linear=lam))
+        assert fc[3, 4] == 0.0 and fc.min() == 0.0
     # fixed point: noiseless data g_j = A_j truth + b
     gq = [q + b[j] for j, q in enumerate(P.all_A(truth))]
     ft, _ = P.rl(gq, b, truth, oracle.default_options(max_iter=3, init=oracle.INIT_USER, rl_linear=lam))
