@@ -107,6 +107,9 @@ typedef struct sgp_options {
                                                     ratio tail inside the graph */
     double rl_relax;                             /* rl_* only: exponent of the multiplicative relaxation, Eq.3:
                                                     f <- f o (W o sum_j A_j^T(g_j/(A_j f + b_j)))^rl_relax; 1 (default) = plain RL */
+    double rl_linear;                            /* rl_* only: constant lambda_k of the linear relaxation, Eq.4:
+                                                    f <- max(0, f - rl_linear f o (1 - W o sum_j A_j^T(g_j/(A_j f + b_j)))), the max being the paper's
+                                                    non-negativity constraint (DESIGN reading A25); 1 (default) = plain RL; rl_relax and rl_linear both != 1 is SGP_ERR_ARG */
 } sgp_options;
 
 /* Result of a run.  The trace pointers are optional caller-allocated HOST arrays of max_iter+1 entries

@@ -47,7 +47,7 @@ class Options(C.Structure):
         ("max_iter", C.c_int), ("stop_rule", C.c_int), ("tol", C.c_double), ("disc_threshold", C.c_double),
         ("sigma_R", C.c_double), ("max_backtracks", C.c_int), ("psf_origin", C.c_int), ("init", C.c_int),
         ("refresh_every", C.c_int), ("strict", C.c_int), ("check_every", C.c_int), ("backend", C.c_int),
-        ("tile_cols", C.c_int), ("rows_per_block", C.c_int), ("use_graph", C.c_int), ("rl_relax", C.c_double),
+        ("tile_cols", C.c_int), ("rows_per_block", C.c_int), ("use_graph", C.c_int), ("rl_relax", C.c_double), ("rl_linear", C.c_double),
     ]
 
 

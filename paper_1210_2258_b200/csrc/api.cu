@@ -21,7 +21,8 @@ int validate_options(const sgp_options *o)
     if (o->psf_origin != SGP_PSF_CENTER && o->psf_origin != SGP_PSF_CORNER) return SGP_ERR_ARG;
     if (o->check_every < 0 || o->refresh_every < 0) return SGP_ERR_ARG;
     if (o->backend != SGP_FFT_NATIVE && o->backend != SGP_FFT_CUFFT) return SGP_ERR_ARG;
-    if (!(o->rl_relax > 0.0)) return SGP_ERR_ARG;
+    if (!(o->rl_relax > 0.0) || !(o->rl_linear > 0.0)) return SGP_ERR_ARG;
+    if (o->rl_relax != 1.0 && o->rl_linear != 1.0) return SGP_ERR_ARG;      // Eq.3 and Eq.4 are alternatives
     return SGP_OK;
 }
 
@@ -103,7 +104,7 @@ void sgp_options_default(sgp_options *o)
     o->disc_threshold = 1.0; o->sigma_R = 1e-2; o->max_backtracks = 30;
     o->psf_origin = SGP_PSF_CENTER; o->init = SGP_INIT_CONST;
     o->refresh_every = 0; o->strict = 0; o->check_every = 0;
-    o->backend = SGP_FFT_NATIVE; o->tile_cols = 0; o->rows_per_block = 0; o->use_graph = 1; o->rl_relax = 1.0;
+    o->backend = SGP_FFT_NATIVE; o->tile_cols = 0; o->rows_per_block = 0; o->use_graph = 1; o->rl_relax = 1.0; o->rl_linear = 1.0;
 }
 
 void sgp_result_init(sgp_result *r) { if (r) memset(r, 0, sizeof(*r)); }

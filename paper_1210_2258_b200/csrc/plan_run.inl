@@ -258,6 +258,7 @@ int PlanImpl<T>::run(int algorithm, const void *const *g, const void *const *b_a
     o.max_backtracks = ro.max_backtracks; o.adaptive_L = ro.adaptive_L; o.p = p;
     o.nS_total = (double)p * (double)G.sy * (double)G.sx;
     o.rl_relax = algorithm == SGP_ALG_RL ? ro.rl_relax : 1.0;      // Eq.3 is a variant of RL (Eq.1/13/21) only
+    o.rl_linear = algorithm == SGP_ALG_RL ? ro.rl_linear : 1.0;    // and so is Eq.4
 
     Trace tr;
     if ((rc = ensure_trace(ro.max_iter, res, &tr, st))) return rc;

@@ -210,6 +210,8 @@ __device__ __forceinline__ void epi_rl(const RowParams<T> &P, const T *wrow, int
     const T Wc = (T)(1.0 / (double)G.p);
     const bool relax = P.o.rl_relax != 1.0;          // multiplicative relaxation of RL, Eq.3
     const T rx = (T)P.o.rl_relax;
+    const bool lin = P.o.rl_linear != 1.0;           // linear relaxation of RL, Eq.4
+    const T lam = (T)P.o.rl_linear;
     constexpr int NIT = (L / 2) / TF;
     constexpr int U = batch_len<T>(NIT);
     for (int it0 = 0; it0 < NIT; it0 += U) {
@@ -231,6 +233,7 @@ __device__ __forceinline__ void epi_rl(const RowParams<T> &P, const T *wrow, int
                 if (MK) wv = a4[u].a[c] > (T)0 ? (T)1 / a4[u].a[c] : (T)0;
                 y4.a[c] = wv * f4[u].a[c] * w4[u].a[c];
                 if (STORE && relax) y4.a[c] = f4[u].a[c] * pow(fmax(wv * w4[u].a[c], (T)0), rx);      // Eq.3
+                if (STORE && lin) y4.a[c] = fmax(f4[u].a[c] - lam * (f4[u].a[c] * ((T)1 - wv * w4[u].a[c])), (T)0);   // Eq.4, projected on f >= 0 (A25)
                 if constexpr (!STORE) {
                     const double yd = (double)y4.a[c];
                     if (yd > 0.0) acc[0] = fmax(acc[0], -yd);

@@ -17,6 +17,7 @@ struct DevOpts {
     int m_alpha, alt_start, armijo_memory, max_iter, stop_rule, max_backtracks, adaptive_L, p;
     double nS_total;   // p * #S, the denominator of Eq.26
     double rl_relax;   // RL: exponent of the multiplicative relaxation, Eq.3; 1 = plain RL
+    double rl_linear;  // RL: constant lambda_k of the linear relaxation, Eq.4; 1 = plain RL
 };
 
 // one per plan, in device memory; written only by single threads of "last block" epilogues

@@ -541,6 +541,29 @@ def test_rl_multiplicative_relaxation_parity(cfg, dt, tol):
     assert np.array_equal(f1.cpu().numpy(), fp)
 
 
+# ---------------------------------------------------------------- linear relaxation of RL (Eq.4)
+@pytest.mark.parametrize("dt,tol", [(np.float32, 2e-4), (np.float64, 1e-11)])
+@pytest.mark.parametrize("cfg", ["C0", "C2", "C3"])
+def test_rl_linear_relaxation_parity(cfg, dt, tol):
+    """f <- f - 1.4 f o (1 - W o sum_j A_j^T(g_j/(A_j f + b_j))) (Eq.4, constant lambda_k: reading A25) for
+    20 steps against the oracle; with lambda = 1 the option leaves plain RL bit-for-bit unchanged; Eq.3 and Eq.4 together
+    are refused."""
+    _need_gpu()
+    w = {"C0": lambda: synth.make("C0", n=128), "C2": lambda: synth.make("C2", n=128),
+         "C3": lambda: synth.make("C3", s=256, sbar=320, n_stars=150, max_iter=60, fwhm=64.0)}[cfg]()
+    fg, rg, fo, ro = run_both(w, dt, alg="rl", max_iter=20, stop_rule=0, rl_linear=1.4)
+    assert rg.iterations == ro.iterations == 20
+    assert rel_l2(fg, fo) <= tol
+    assert abs(rg.J0_final - ro.J0_final) <= max(tol, 1e-6 if dt == np.float32 else 0) * abs(ro.J0_final)
+    fp, rp, fo1, ro1 = run_both(w, dt, alg="rl", max_iter=20, stop_rule=0)
+    assert ro.J0_final < ro1.J0_final and rg.J0_final < rp.J0_final          # the relaxed iteration is ahead of plain RL
+    plan, o = gpu_plan(w, dt, max_iter=20, stop_rule=0, rl_linear=1.0)
+    g = [dev(a, dt) for a in w["g"]]
+    f1, _ = plan.rl(g, w["b"], opts=o)
+    plan.close()
+    assert np.array_equal(f1.cpu().numpy(), fp)
+
+
 # ---------------------------------------------------------------- the start points of PAPER.md:260-267
 @pytest.mark.parametrize("dt,tol", [(np.float32, 1e-4), (np.float64, 1e-10)])
 @pytest.mark.parametrize("cfg", ["C0", "C2", "C3"])

@@ -49,6 +49,7 @@ def test_option_defaults_are_the_papers(lib):
     assert o.armijo_memory == 1                    # monotone line search
     assert o.adaptive_L == 1
     assert o.disc_threshold == 1.0 and o.max_backtracks == 30 and o.sigma_R == 1e-2      # readings A7, A16, A13
+    assert o.rl_relax == 1.0 and o.rl_linear == 1.0        # plain RL (Eq.1) unless Eq.3 / Eq.4 is asked for
 
 
 def test_strings_and_workspace(lib):
@@ -86,6 +87,10 @@ def test_plan_create_rejects_bad_arguments_before_touching_the_device(lib):
     bad = B.default_options(); bad.theta = 1.5
     assert create(B.KIND_SINGLE, 1, 256, 256, opt=bad) == B.ERR_ARG
     bad = B.default_options(); bad.adaptive_L = 0; bad.L1 = 2.0; bad.L2 = 1.0
+    assert create(B.KIND_SINGLE, 1, 256, 256, opt=bad) == B.ERR_ARG
+    bad = B.default_options(); bad.rl_linear = 0.0                    # Eq.4: lambda_k > 0
+    assert create(B.KIND_SINGLE, 1, 256, 256, opt=bad) == B.ERR_ARG
+    bad = B.default_options(); bad.rl_linear = 1.2; bad.rl_relax = 1.2   # Eq.3 and Eq.4 are alternatives
     assert create(B.KIND_SINGLE, 1, 256, 256, opt=bad) == B.ERR_ARG
     assert plan.value is None
 
