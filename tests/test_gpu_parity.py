@@ -447,6 +447,19 @@ def test_full_size_workloads_match_the_oracle(cfg, iters, force):
     assert (fg >= 0).all()
 
 
+@pytest.mark.parametrize("kw", [{}, {"rl_relax": 1.5}, {"rl_linear": 1.4}], ids=["rl", "eq3", "eq4"])
+def test_full_size_rl_and_its_relaxations_match_the_oracle(kw):
+    """Richardson-Lucy (Eq.1) and its relaxations (Eq.3, Eq.4) at 2048^2 fp32 in the configuration `bench.py --alg rl`
+    times (CUDA-graph replay of 10 steps plus 2 plain): whole image and J0 trace against the fp64 oracle."""
+    _need_gpu()
+    w = synth.make("C4c")
+    fg, rg, fo, ro = run_both(w, np.float32, alg="rl", max_iter=12, stop_rule=0, **kw)
+    assert rg.iterations == ro.iterations == 12
+    assert rel_l2(fg, fo) <= 1e-4
+    assert np.max(np.abs(rg.J - np.asarray(ro.J)) / np.abs(np.asarray(ro.J))) <= 1e-5
+    assert (fg >= 0).all()
+
+
 # ---------------------------------------------------------------- OSEM (Algorithm 2, SURVEY.md 8(f) item 1)
 @pytest.mark.parametrize("dt,tol", [(np.float32, 1e-4), (np.float64, 1e-11)])
 @pytest.mark.parametrize("cfg,kw", [("C2", {"n": 128}), ("C2", {"n": 256, "p": 2}), ("C3", {"s": 256, "sbar": 320, "n_stars": 150, "fwhm": 64.0})])
