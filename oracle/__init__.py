@@ -21,10 +21,10 @@ _HDR = _HERE / "sgp_oracle.h"
 _LIBS = {np.dtype(np.float64): _HERE / "liboracle_f64.so", np.dtype(np.float32): _HERE / "liboracle_f32.so"}
 _loaded: dict = {}
 
-STOP_MAXIT, STOP_RELJ, STOP_DISCREPANCY = 0, 1, 2
-INIT_USER, INIT_CONST, INIT_ZERO, INIT_G = 0, 1, 2, 3
+STOP_MAXIT, STOP_RELJ, STOP_DISCREPANCY, STOP_MINERR = 0, 1, 2, 3
+INIT_USER, INIT_CONST, INIT_ZERO, INIT_G, INIT_CONST_SMOOTH = 0, 1, 2, 3, 4
 PSF_CENTER, PSF_CORNER = 0, 1
-REASON = {1: "maxit", 2: "relJ", 3: "discrepancy"}
+REASON = {1: "maxit", 2: "relJ", 3: "discrepancy", 4: "minerr"}
 ERR_LINESEARCH = -6
 
 
@@ -51,6 +51,7 @@ class Options(C.Structure):
         ("max_iter", C.c_int), ("stop_rule", C.c_int), ("tol", C.c_double), ("disc_threshold", C.c_double),
         ("sigma_R", C.c_double), ("max_backtracks", C.c_int), ("psf_origin", C.c_int), ("init", C.c_int),
         ("refresh_every", C.c_int), ("strict", C.c_int), ("rl_relax", C.c_double), ("rl_linear", C.c_double),
+        ("flux_constraint", C.c_int), ("flux_value", C.c_double), ("init_sigma", C.c_double),
     ]
 
 
@@ -63,6 +64,7 @@ class _Result(C.Structure):
         ("trace_lambda", C.POINTER(C.c_double)), ("trace_rule", C.POINTER(C.c_int)),
         ("trace_backtracks", C.POINTER(C.c_int)),
         ("force_alpha", C.POINTER(C.c_double)), ("force_lambda", C.POINTER(C.c_double)),
+        ("truth", C.c_void_p), ("trace_err", C.POINTER(C.c_double)), ("err_final", C.c_double),
     ]
 
 
@@ -80,6 +82,7 @@ def lib(dtype=np.float64) -> C.CDLL:
         L = C.CDLL(str(_LIBS[dt]))
         L.oracle_J0.restype = C.c_double
         L.oracle_bb_next.restype = C.c_double
+        L.oracle_rel_error.restype = C.c_double
         L.oracle_problem_create.restype = C.c_void_p
         L.oracle_options_default.restype = None
         L.oracle_bb_init.restype = None
@@ -157,6 +160,22 @@ def adaptive_bounds(y, dtype=np.float64):
     return L1.value, L2.value
 
 
+def project_flux(x, D, c, dtype=np.float64):
+    """(y, mu): projection on {y >= 0, sum y = c} in the metric D^-1 (oracle_project_flux)"""
+    dt = np.dtype(dtype)
+    x, D = _arr(x, dt), _arr(D, dt)
+    y = np.empty_like(x)
+    mu = C.c_double()
+    _check(lib(dt).oracle_project_flux(C.c_long(x.size), _ptr(x), _ptr(D), C.c_double(c), _ptr(y), C.byref(mu)), "project_flux")
+    return y, mu.value
+
+
+def rel_error(f, truth, dtype=np.float64):
+    dt = np.dtype(dtype)
+    f, truth = _arr(f, dt), _arr(truth, dt)
+    return lib(dt).oracle_rel_error(C.c_long(f.size), _ptr(f), _ptr(truth))
+
+
 class BB:
     """The step-length state machine of PAPER.md:130-155 (oracle_bb_init / oracle_bb_next)."""
 
@@ -187,13 +206,16 @@ class Result:
         self.lam = traces["lambda"][:k].copy()
         self.rule = traces["rule"][:k].copy()
         self.backtracks = traces["backtracks"][:k].copy()
+        self.err_final = raw.err_final
+        self.err = traces["err"][: k + 2].copy()      # rho(0..k) and, for a MINERR stop, the discarded rho(k+1)
 
 
-def _make_result(max_iter, force_alpha=None, force_lambda=None):
+def _make_result(max_iter, force_alpha=None, force_lambda=None, truth=None, dt=np.float64):
     n = max_iter + 1
     tr = {"J": np.zeros(n), "alpha": np.zeros(n), "lambda": np.zeros(n),
-          "rule": np.zeros(n, np.int32), "backtracks": np.zeros(n, np.int32)}
+          "rule": np.zeros(n, np.int32), "backtracks": np.zeros(n, np.int32), "err": np.full(n + 1, np.nan)}
     raw = _Result()
+    raw.trace_err = tr["err"].ctypes.data_as(C.POINTER(C.c_double))
     raw.trace_J = tr["J"].ctypes.data_as(C.POINTER(C.c_double))
     raw.trace_alpha = tr["alpha"].ctypes.data_as(C.POINTER(C.c_double))
     raw.trace_lambda = tr["lambda"].ctypes.data_as(C.POINTER(C.c_double))
@@ -206,6 +228,10 @@ def _make_result(max_iter, force_alpha=None, force_lambda=None):
             a[: len(arr)] = np.asarray(arr, dtype=np.float64)[: len(a)]
             keep.append(a)
             setattr(raw, name, a.ctypes.data_as(C.POINTER(C.c_double)))
+    if truth is not None:
+        t = _arr(truth, dt)
+        keep.append(t)
+        raw.truth = t.ctypes.data
     return raw, tr, keep
 
 
@@ -301,10 +327,10 @@ class Problem:
         _check(self.L.oracle_scaling(self.h, _ptr(f), C.c_double(L1), C.c_double(L2), _ptr(out)), "scaling")
         return out
 
-    def _run(self, fn, g, b, f0, opts, force_alpha=None, force_lambda=None, check=True):
+    def _run(self, fn, g, b, f0, opts, force_alpha=None, force_lambda=None, check=True, truth=None):
         g, b = self._planes(g), self._planes(b)
         f0a = _arr(f0, self.dt) if f0 is not None else None
-        raw, tr, keep = _make_result(opts.max_iter, force_alpha, force_lambda)
+        raw, tr, keep = _make_result(opts.max_iter, force_alpha, force_lambda, truth, self.dt)
         f_out = np.empty((self.ny, self.nx), self.dt)
         rc = fn(self.h, _pp(g), _pp(b), _ptr(f0a) if f0a is not None else None, C.byref(opts), C.byref(raw), _ptr(f_out))
         if check:
@@ -406,3 +432,46 @@ def rl_boundary(g, psf, b, oy, ox, f0=None, opts=None, dtype=np.float64):
 def set_threads(n: int) -> None:
     """OpenMP thread count for the oracle's FFT loops (takes effect before the library is first loaded)."""
     os.environ["OMP_NUM_THREADS"] = str(int(n))
+
+
+# ---- mosaic of sub-domain reconstructions with boundary-effect correction (PAPER.md:385-389, :530; pin P19) ----
+
+def mosaic_layout(Ny, Nx, ty, tx, sy, sx, ny, nx):
+    """The paper's procedure: the Ny x Nx image is partitioned into ty x tx partially overlapping
+    sy x sx sub-images; each is merged by zero padding into an ny x nx array (S centred in S-bar: reading A29); from
+    each reconstruction the (Ny/ty) x (Nx/tx) non-overlapping part is extracted.  Sub-image t starts at
+    clamp(t*N/T - (s - N/T)/2, 0, N - s) (256 -> four 160^2 sub-images at offsets 0 and 96, 128^2 parts extracted).
+    Returns one dict per tile: img = (y, x) offset of the sub-image in the image, S = (oy, ox, sy, sx) in S-bar,
+    out = (y0, x0, hy, hx) the part of the mosaic it fills (image coordinates), src = (y, x) of that part in S-bar."""
+    assert Ny % ty == 0 and Nx % tx == 0 and sy >= Ny // ty and sx >= Nx // tx and sy <= min(Ny, ny) and sx <= min(Nx, nx)
+    hy, hx = Ny // ty, Nx // tx
+    oy, ox = (ny - sy) // 2, (nx - sx) // 2
+    tiles = []
+    for iy in range(ty):
+        y_img = min(max(iy * hy - (sy - hy) // 2, 0), Ny - sy)
+        for ix in range(tx):
+            x_img = min(max(ix * hx - (sx - hx) // 2, 0), Nx - sx)
+            tiles.append({"img": (y_img, x_img), "S": (oy, ox, sy, sx), "out": (iy * hy, ix * hx, hy, hx),
+                          "src": (iy * hy - y_img + oy, ix * hx - x_img + ox)})
+    return tiles
+
+
+def mosaic(alg, g, psf, b, ty, tx, sub, opts=None, dtype=np.float64):
+    """alg in {"sgp", "rl", "osem"}; g: p images (Ny x Nx); psf: p PSFs (ny x nx, the S-bar grid of every sub-problem);
+    b: p background constants.  Every sub-domain is reconstructed independently by the boundary-effect-corrected
+    method (Eq.16-23) and the non-overlapping parts are put together.  Returns (mosaic Ny x Nx, [Result per tile])."""
+    opts = opts or default_options()
+    Ny, Nx = np.shape(g[0]); ny, nx = np.shape(psf[0])
+    fn = {"sgp": sgp_boundary, "rl": rl_boundary, "osem": osem_boundary}[alg]
+    out = np.zeros((Ny, Nx), np.dtype(dtype))
+    results = []
+    for t in mosaic_layout(Ny, Nx, ty, tx, sub[0], sub[1], ny, nx):
+        yi, xi = t["img"]; oy, ox, sy, sx = t["S"]
+        gs = [np.ascontiguousarray(a[yi:yi + sy, xi:xi + sx]) for a in g]
+        f, r = fn(gs, psf, b, oy, ox, None, opts, dtype)
+        if r.rc != 0:
+            raise OracleError(r.rc, "mosaic tile")
+        y0, x0, hy, hx = t["out"]; ys, xs = t["src"]
+        out[y0:y0 + hy, x0:x0 + hx] = f[ys:ys + hy, xs:xs + hx]
+        results.append(r)
+    return out, results

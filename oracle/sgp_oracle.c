@@ -7,7 +7,9 @@
  * spectra (no half-spectrum tricks), every operator and every step of Algorithm 1 in
  * the paper's order.  No blocking, no fusion.  Shares nothing with the CUDA library.
  *
- * Pins (tests/test_oracle_*.py, run with -m "not gpu"): P1..P11 of SURVEY.md 8(c).
+ * Pins (tests/test_oracle_*.py, run with -m "not gpu"): P1..P11 of SURVEY.md 8(c), P12-P14 (OSEM, Eq.3, Eq.4),
+ * P15 (start points, data cleaning, refresh_every), P16 (flux-constrained projection), P17 (Eq.25 stop),
+ * P18 (Gaussian-smoothed constant start), P19 (mosaic of sub-domain reconstructions, oracle/__init__.py).
  * Parity unpinned (oracle and GPU library merely share the option):
  *   A7 (disc_threshold = 1), A9 (off-by-one of "first 20 iterations"), A13 (sigma_R),
  *   A14 (which mean the constant start uses), A16 (backtrack cap).
@@ -483,6 +485,67 @@ int oracle_adaptive_bounds(long n, const oreal *y, double *L1, double *L2)
     return ORACLE_OK;
 }
 
+/* Projection on the set { y >= 0, sum_i y_i = c } in the norm induced by D^-1 -- the "additional flux
+   constraint" of Bonettini et al. (2009) that the paper mentions and does not use (reading A26).
+   KKT conditions of  min sum_i (y_i - x_i)^2 / (2 D_i)  s.t. y >= 0, sum y = c:
+       y_i = max(0, x_i - mu D_i),   mu such that  h(mu) = sum_i max(0, x_i - mu D_i) = c.
+   h is continuous, piecewise linear and non-increasing in mu with break points t_i = x_i / D_i.  The root is found
+   exactly: sort the break points in decreasing order; with the m largest active, h(mu) = SX_m - mu SD_m, so the
+   candidate mu_m = (SX_m - c) / SD_m is the root iff t_(m) > mu_m >= t_(m+1).  Entries with D_i = 0 (pixels outside
+   R, Eq.23) cannot move: y_i = 0 there. */
+typedef struct { double t; long i; } brk_t;
+static int brk_cmp(const void *a, const void *b)
+{
+    double ta = ((const brk_t *)a)->t, tb = ((const brk_t *)b)->t;
+    if (ta > tb) return -1;
+    if (ta < tb) return 1;
+    long ia = ((const brk_t *)a)->i, ib = ((const brk_t *)b)->i;
+    return ia < ib ? -1 : (ia > ib ? 1 : 0);
+}
+int oracle_project_flux(long n, const oreal *x, const oreal *D, double c, oreal *y, double *mu_out)
+{
+    if (n < 1 || !x || !D || !y || !(c >= 0.0)) return ORACLE_ERR_ARG;
+    brk_t *bk = (brk_t *)malloc(sizeof(brk_t) * (size_t)n);
+    if (!bk) return ORACLE_ERR_ALLOC;
+    long m = 0;
+    for (long i = 0; i < n; ++i)
+        if (D[i] > 0) { bk[m].t = (double)x[i] / (double)D[i]; bk[m].i = i; m++; }
+    if (m == 0) { free(bk); return ORACLE_ERR_DATA; }
+    qsort(bk, (size_t)m, sizeof(brk_t), brk_cmp);
+    double SX = 0.0, SD = 0.0, mu = 0.0;
+    int found = 0;
+    for (long k = 0; k < m; ++k) {
+        SX += (double)x[bk[k].i]; SD += (double)D[bk[k].i];
+        double cand = (SX - c) / SD;
+        double tnext = (k + 1 < m) ? bk[k + 1].t : -INFINITY;
+        if (cand < bk[k].t && cand >= tnext) { mu = cand; found = 1; break; }
+    }
+    if (!found) {
+        /* c = 0 with all x <= 0 etc.: the largest break point makes every entry inactive, h = 0 */
+        if (c == 0.0) { mu = bk[0].t; found = 1; }
+    }
+    free(bk);
+    if (!found) return ORACLE_ERR_DATA;
+    for (long i = 0; i < n; ++i) {
+        if (!(D[i] > 0)) { y[i] = 0; continue; }
+        oreal v = x[i] - (oreal)mu * D[i];
+        y[i] = v > 0 ? v : (oreal)0;
+    }
+    if (mu_out) *mu_out = mu;
+    return ORACLE_OK;
+}
+
+/* rho = ||f - f~||_2 / ||f~||_2, Eq.25 with the l2 norm the paper's code uses */
+double oracle_rel_error(long n, const oreal *f, const oreal *truth)
+{
+    double num = 0.0, den = 0.0;
+    for (long i = 0; i < n; ++i) {
+        double e = (double)f[i] - (double)truth[i];
+        num += e * e; den += (double)truth[i] * (double)truth[i];
+    }
+    return sqrt(num) / sqrt(den);
+}
+
 /* ------------------------------------------------------------------------------------
  * Step-length selection.
  * ------------------------------------------------------------------------------------ */
@@ -499,6 +562,7 @@ void oracle_options_default(oracle_options *o)
     o->disc_threshold = 1.0; o->sigma_R = 1e-2; o->max_backtracks = 30;
     o->psf_origin = ORACLE_PSF_CENTER; o->init = ORACLE_INIT_CONST;
     o->refresh_every = 0; o->strict = 0; o->rl_relax = 1.0; o->rl_linear = 1.0;
+    o->flux_constraint = 0; o->flux_value = 0.0; o->init_sigma = 2.0;
 }
 
 void oracle_bb_init(oracle_bb_state *s, const oracle_options *o)
@@ -545,7 +609,7 @@ double oracle_bb_next(oracle_bb_state *s, const oracle_options *o, int k, double
  * Start point, PAPER.md:260-267 (readings A11, A14)
  * ------------------------------------------------------------------------------------ */
 static int make_start(const oracle_problem *P, const oreal *const *g, const oreal *const *b,
-                      const oreal *f0, int init, oreal *f)
+                      const oreal *f0, int init, double init_sigma, oreal *f)
 {
     size_t n = P->n;
     switch (init) {
@@ -556,7 +620,8 @@ static int make_start(const oracle_problem *P, const oreal *const *g, const orea
             f[i] = P->MR[i] ? f0[i] : (oreal)0;
         }
         break;
-    case ORACLE_INIT_CONST: {
+    case ORACLE_INIT_CONST:
+    case ORACLE_INIT_CONST_SMOOTH: {
         /* c = max(0, (1/p) sum_j mean_S(g_j - b_j)), placed on R */
         double s = 0.0;
         for (int j = 0; j < P->p; ++j)
@@ -565,6 +630,32 @@ static int make_start(const oracle_problem *P, const oreal *const *g, const orea
         double c = s / ((double)P->p * (double)P->nS);
         if (c < 0.0) c = 0.0;
         for (size_t i = 0; i < n; ++i) f[i] = P->MR[i] ? (oreal)c : (oreal)0;
+        if (init == ORACLE_INIT_CONST_SMOOTH) {
+            /* "the constant image will be convolved with a Gaussian to avoid the presence of sharp edges"
+               (reading A28): f0 = M_R o max(0, G_sigma * (c M_R)), G_sigma the periodic Gaussian
+               of standard deviation init_sigma pixels on the S-bar grid, unit sum, centred on pixel (0,0) */
+            if (!(init_sigma > 0.0)) return ORACLE_ERR_ARG;
+            ocplx *G = (ocplx *)malloc(sizeof(ocplx) * n), *t = (ocplx *)malloc(sizeof(ocplx) * n);
+            if (!G || !t) { free(G); free(t); return ORACLE_ERR_ALLOC; }
+            double sum = 0.0;
+            for (int y = 0; y < P->ny; ++y)
+                for (int x = 0; x < P->nx; ++x) {
+                    double dy = y <= P->ny / 2 ? y : y - P->ny, dx = x <= P->nx / 2 ? x : x - P->nx;
+                    sum += exp(-(dy * dy + dx * dx) / (2.0 * init_sigma * init_sigma));
+                }
+            for (int y = 0; y < P->ny; ++y)
+                for (int x = 0; x < P->nx; ++x) {
+                    double dy = y <= P->ny / 2 ? y : y - P->ny, dx = x <= P->nx / 2 ? x : x - P->nx;
+                    G[(size_t)y * P->nx + x] = (oreal)(exp(-(dy * dy + dx * dx) / (2.0 * init_sigma * init_sigma)) / sum);
+                }
+            for (size_t i = 0; i < n; ++i) t[i] = f[i];
+            int rc = fft2_inplace(P->ny, P->nx, -1, G);
+            if (!rc) rc = fft2_inplace(P->ny, P->nx, -1, t);
+            if (!rc) { for (size_t i = 0; i < n; ++i) t[i] *= G[i]; rc = fft2_inplace(P->ny, P->nx, +1, t); }
+            if (!rc) for (size_t i = 0; i < n; ++i) { oreal v = (oreal)creal(t[i]); f[i] = (P->MR[i] && v > 0) ? v : (oreal)0; }
+            free(G); free(t);
+            if (rc) return rc;
+        }
         break; }
     case ORACLE_INIT_ZERO:
         for (size_t i = 0; i < n; ++i) f[i] = 0;
@@ -589,6 +680,8 @@ static int check_options(const oracle_options *o)
     if (o->m_alpha < 1 || o->m_alpha > 16 || o->armijo_memory < 1 || o->max_iter < 0) return ORACLE_ERR_ARG;
     if (!o->adaptive_L && !(o->L1 > 0 && o->L1 < o->L2)) return ORACLE_ERR_ARG;
     if (o->max_backtracks < 0) return ORACLE_ERR_ARG;
+    if (o->stop_rule < ORACLE_STOP_MAXIT || o->stop_rule > ORACLE_STOP_MINERR) return ORACLE_ERR_ARG;
+    if (o->init == ORACLE_INIT_CONST_SMOOTH && !(o->init_sigma > 0.0)) return ORACLE_ERR_ARG;
     return ORACLE_OK;
 }
 
@@ -639,10 +732,37 @@ int oracle_sgp_run(const oracle_problem *P, const oreal *const *g_in, const orea
     if (!g || !q || !u || !r || !f || !fprev || !grad || !gprev || !D || !y || !d || !Jhist) { rc = ORACLE_ERR_ALLOC; goto done; }
 
     rc = clean_data(P, g_in, o->strict, g);                     if (rc) goto done;
-    rc = make_start(P, (const oreal *const *)g, b, f0, o->init, f);   if (rc) goto done;
+    rc = make_start(P, (const oreal *const *)g, b, f0, o->init, o->init_sigma, f);   if (rc) goto done;
+    /* flux constraint (reading A26): c = the background-subtracted flux of the data, averaged over the images */
+    double flux_c = o->flux_value;
+    if (o->flux_constraint && !(flux_c > 0.0)) {
+        double sfl = 0.0;
+        for (int j = 0; j < p; ++j)
+            for (size_t i = 0; i < n; ++i)
+                if (P->MS[i]) sfl += (double)g[j][i] - (double)b[j][i];
+        flux_c = sfl / (double)p;
+        if (flux_c < 0.0) flux_c = 0.0;
+    }
+    if (o->flux_constraint) {
+        /* SGP needs a feasible f(0) (Bonettini et al. 2009: f(0) in Omega; d = P(f - alpha D grad) - f is a descent
+           direction only from a feasible f): the start point is rescaled to the flux c, the null image becomes the
+           constant c / #R on R (reading A26) */
+        double s0 = 0.0;
+        for (size_t i = 0; i < n; ++i) s0 += (double)f[i];
+        if (!(flux_c > 0.0)) { rc = ORACLE_ERR_DATA; goto done; }
+        for (size_t i = 0; i < n; ++i)
+            f[i] = s0 > 0.0 ? (oreal)((double)f[i] * (flux_c / s0)) : (P->MR[i] ? (oreal)(flux_c / (double)P->nR) : (oreal)0);
+    }
     rc = oracle_all_A(P, f, q);                                 if (rc) goto done;   /* q_j = A_j f(0) */
     double J = oracle_J0(P, (const oreal *const *)q, (const oreal *const *)g, b);
     if (!isfinite(J)) { rc = ORACLE_ERR_NONFINITE; goto done; }
+
+    /* Eq.25 (reading A27): rho(k) = ||f(k) - f~|| / ||f~||; with ORACLE_STOP_MINERR the run stops at the first k whose
+       step would increase rho ("reaches a minimum value"), that step is discarded and f(k) returned */
+    const oreal *truth = (const oreal *)res->truth;
+    if (o->stop_rule == ORACLE_STOP_MINERR && !truth) { rc = ORACLE_ERR_ARG; goto done; }
+    double rho = truth ? oracle_rel_error((long)n, f, truth) : 0.0;
+    if (truth && res->trace_err) res->trace_err[0] = rho;
 
     double L1 = o->L1, L2 = o->L2;
     if (o->adaptive_L) {
@@ -691,6 +811,12 @@ int oracle_sgp_run(const oracle_problem *P, const oreal *const *g_in, const orea
         }
         if (res->force_alpha && isfinite(res->force_alpha[k])) { alpha = res->force_alpha[k]; bb.alpha_prev = alpha; }
         /* step 4: y = P+(f - alpha D grad); d = y - f; gd = grad' d   (Alg.1 steps 2-3) */
+        if (o->flux_constraint) {
+            /* projection on { y >= 0, sum y = c } in the metric D^-1 (Bonettini et al. 2009) */
+            for (size_t i = 0; i < n; ++i) y[i] = f[i] - (oreal)alpha * D[i] * grad[i];
+            rc = oracle_project_flux((long)n, y, D, flux_c, y, NULL);
+            if (rc) goto done;
+        } else
         oracle_project((long)n, f, grad, D, alpha, y);
         double gd = 0.0;
         for (size_t i = 0; i < n; ++i) {
@@ -726,6 +852,15 @@ int oracle_sgp_run(const oracle_problem *P, const oreal *const *g_in, const orea
                 nb++;
             }
         }
+        /* Eq.25: error of the candidate f(k) + lambda d; an increase stops the run BEFORE the step is taken (A27) */
+        double rho_new = 0.0;
+        if (truth) {
+            for (size_t i = 0; i < n; ++i) y[i] = f[i] + (oreal)lambda * d[i];
+            rho_new = oracle_rel_error((long)n, y, truth);
+            if (res->trace_err) res->trace_err[k + 1] = rho_new;
+            if (o->stop_rule == ORACLE_STOP_MINERR && rho_new > rho) { res->stop_reason = ORACLE_REASON_MINERR; break; }
+            rho = rho_new;
+        }
         /* step 7: f(k+1) = f(k) + lambda d (Alg.1 step 6); q_j <- q_j + lambda u_j (A21) */
         for (size_t i = 0; i < n; ++i) {
             fprev[i] = f[i]; gprev[i] = grad[i];
@@ -756,6 +891,7 @@ int oracle_sgp_run(const oracle_problem *P, const oreal *const *g_in, const orea
     res->n_fft2 = g_fft2_count - fft0;
     res->J0_final = J;
     res->discrepancy_final = 2.0 * J / ((double)p * (double)P->nS);
+    res->err_final = rho;
     rc = ORACLE_OK;
 done:
     if (f) memcpy(f_out, f, sizeof(oreal) * n);     /* on error: the last accepted iterate */
@@ -777,14 +913,21 @@ int oracle_rl_run(const oracle_problem *P, const oreal *const *g_in, const oreal
     const int p = P->p;
     const size_t n = P->n;
     oreal **g = alloc_planes(p, n), **q = alloc_planes(p, n), **r = alloc_planes(p, n);
-    oreal *f = (oreal *)calloc(n, sizeof(oreal)), *w = (oreal *)calloc(n, sizeof(oreal));
+    oreal *f = (oreal *)calloc(n, sizeof(oreal)), *w = (oreal *)calloc(n, sizeof(oreal)), *fn = NULL;
     if (!g || !q || !r || !f || !w) { rc = ORACLE_ERR_ALLOC; goto done; }
     rc = clean_data(P, g_in, o->strict, g);                           if (rc) goto done;
-    rc = make_start(P, (const oreal *const *)g, b, f0, o->init, f);   if (rc) goto done;
+    rc = make_start(P, (const oreal *const *)g, b, f0, o->init, o->init_sigma, f);   if (rc) goto done;
     res->iterations = 0; res->stop_reason = 0; res->total_backtracks = 0;
     res->L1_used = 0; res->L2_used = 0;
     long fft0 = g_fft2_count;
     double J = 0.0, Jold = 0.0;
+    /* Eq.25 (reading A27), as in oracle_sgp_run: an update that would increase rho is not taken */
+    const oreal *truth = (const oreal *)res->truth;
+    if (o->stop_rule == ORACLE_STOP_MINERR && !truth) { rc = ORACLE_ERR_ARG; goto done; }
+    double rho = truth ? oracle_rel_error((long)n, f, truth) : 0.0;
+    if (truth && res->trace_err) res->trace_err[0] = rho;
+    fn = (oreal *)calloc(n, sizeof(oreal));
+    if (!fn) { rc = ORACLE_ERR_ALLOC; goto done; }
     for (int k = 0;; ++k) {
         rc = oracle_all_A(P, f, q);                                   if (rc) goto done;
         Jold = J;
@@ -806,10 +949,10 @@ int oracle_rl_run(const oracle_problem *P, const oreal *const *g_in, const oreal
             for (size_t i2 = 0; i2 < n; ++i2)
             {
                 oreal y = f[i2] - (oreal)o->rl_linear * (f[i2] * ((oreal)1 - P->W[i2] * w[i2]));
-                f[i2] = y > (oreal)0 ? y : (oreal)0;       /* the non-negativity constraint of the paper, reading A25 */
+                fn[i2] = y > (oreal)0 ? y : (oreal)0;      /* the non-negativity constraint of the paper, reading A25 */
             }
         } else if (o->rl_relax == 1.0) {
-            rc = rl_update_from_q(P, f, q, (const oreal *const *)g, b, r, w, f);
+            rc = rl_update_from_q(P, f, q, (const oreal *const *)g, b, r, w, fn);
             if (rc) goto done;
         } else {
             /* multiplicative relaxation, Eq.3 (Llacer & Nunez): f(k+1) = f(k) o (A^T g/(Af+b))^alpha;
@@ -819,16 +962,24 @@ int oracle_rl_run(const oracle_problem *P, const oreal *const *g_in, const oreal
                     r[j][i2] = P->MS[i2] ? ratio_term(g[j][i2], q[j][i2] + b[j][i2]) : (oreal)0;
             rc = oracle_sum_AT(P, (const oreal *const *)r, w);
             if (rc) goto done;
-            for (size_t i2 = 0; i2 < n; ++i2) f[i2] = f[i2] * (oreal)pow(fmax(0.0, (double)(P->W[i2] * w[i2])), o->rl_relax);   /* base >= 0 up to FFT round-off */
+            for (size_t i2 = 0; i2 < n; ++i2) fn[i2] = f[i2] * (oreal)pow(fmax(0.0, (double)(P->W[i2] * w[i2])), o->rl_relax);   /* base >= 0 up to FFT round-off */
         }
+        if (truth) {
+            double rho_new = oracle_rel_error((long)n, fn, truth);
+            if (res->trace_err) res->trace_err[k + 1] = rho_new;
+            if (o->stop_rule == ORACLE_STOP_MINERR && rho_new > rho) { res->stop_reason = ORACLE_REASON_MINERR; break; }
+            rho = rho_new;
+        }
+        memcpy(f, fn, sizeof(oreal) * n);
     }
     res->n_fft2 = g_fft2_count - fft0;
     res->J0_final = J;
     res->discrepancy_final = 2.0 * J / ((double)p * (double)P->nS);
+    res->err_final = rho;
     rc = ORACLE_OK;
 done:
     if (f) memcpy(f_out, f, sizeof(oreal) * n);
-    free_planes(g, p); free_planes(q, p); free_planes(r, p); free(f); free(w);
+    free_planes(g, p); free_planes(q, p); free_planes(r, p); free(f); free(w); free(fn);
     return rc;
 }
 
@@ -852,10 +1003,10 @@ int oracle_osem_run(const oracle_problem *P, const oreal *const *g_in, const ore
     const size_t n = P->n;
     oreal **g = alloc_planes(p, n), **q = alloc_planes(p, n), **aj = alloc_planes(p, n);
     oreal *h = (oreal *)calloc(n, sizeof(oreal)), *w = (oreal *)calloc(n, sizeof(oreal));
-    oreal *r = (oreal *)calloc(n, sizeof(oreal));
+    oreal *r = (oreal *)calloc(n, sizeof(oreal)), *hk = NULL;
     if (!g || !q || !aj || !h || !w || !r) { rc = ORACLE_ERR_ALLOC; goto done; }
     rc = clean_data(P, g_in, o->strict, g);                           if (rc) goto done;
-    rc = make_start(P, (const oreal *const *)g, b, f0, o->init, h);   if (rc) goto done;
+    rc = make_start(P, (const oreal *const *)g, b, f0, o->init, o->init_sigma, h);   if (rc) goto done;
     for (int j = 0; j < p; ++j) {                                     /* alpha_j on R, 0 elsewhere */
         if (P->masked) {
             for (size_t i = 0; i < n; ++i) r[i] = P->MS[i] ? (oreal)1 : (oreal)0;
@@ -867,17 +1018,36 @@ int oracle_osem_run(const oracle_problem *P, const oreal *const *g_in, const ore
     res->iterations = 0; res->stop_reason = 0; res->total_backtracks = 0;
     res->L1_used = 0; res->L2_used = 0;
     long fft0 = g_fft2_count;
+    /* Eq.25 (reading A27), per cycle: the paper stops OSEM (and RL, SGP) at the minimum r.m.s. error in its diffuse-object experiments */
+    const oreal *truth = (const oreal *)res->truth;
+    if (o->stop_rule == ORACLE_STOP_MINERR && !truth) { rc = ORACLE_ERR_ARG; goto done; }
+    double rho = truth ? oracle_rel_error((long)n, h, truth) : 0.0;
+    if (truth && res->trace_err) res->trace_err[0] = rho;
+    hk = (oreal *)calloc(n, sizeof(oreal));
+    if (!hk) { rc = ORACLE_ERR_ALLOC; goto done; }
     for (int k = 0; k < o->max_iter; ++k) {
+        memcpy(hk, h, sizeof(oreal) * n);                             /* f(k), restored if the cycle is discarded */
         for (int j = 0; j < p; ++j) {
             rc = oracle_apply_A(P, j, h, q[j]);                       if (rc) goto done;
             for (size_t i = 0; i < n; ++i) r[i] = P->MS[i] ? ratio_term(g[j][i], q[j][i] + b[j][i]) : (oreal)0;
             rc = oracle_apply_AT(P, j, r, w);                         if (rc) goto done;
             for (size_t i = 0; i < n; ++i) h[i] = P->MR[i] ? h[i] * w[i] / aj[j][i] : (oreal)0;
         }
+        if (truth) {
+            double rho_new = oracle_rel_error((long)n, h, truth);
+            if (res->trace_err) res->trace_err[k + 1] = rho_new;
+            if (o->stop_rule == ORACLE_STOP_MINERR && rho_new > rho) {
+                memcpy(h, hk, sizeof(oreal) * n);
+                res->stop_reason = ORACLE_REASON_MINERR;
+                break;
+            }
+            rho = rho_new;
+        }
         res->iterations = k + 1;
     }
     res->n_fft2 = g_fft2_count - fft0;
-    res->stop_reason = ORACLE_REASON_MAXIT;
+    if (!res->stop_reason) res->stop_reason = ORACLE_REASON_MAXIT;
+    res->err_final = rho;
     rc = oracle_all_A(P, h, q);                                       if (rc) goto done;
     {
         double J = oracle_J0(P, (const oreal *const *)q, (const oreal *const *)g, b);
@@ -887,7 +1057,7 @@ int oracle_osem_run(const oracle_problem *P, const oreal *const *g_in, const ore
     }
 done:
     if (h) memcpy(f_out, h, sizeof(oreal) * n);
-    free_planes(g, p); free_planes(q, p); free_planes(aj, p); free(h); free(w); free(r);
+    free_planes(g, p); free_planes(q, p); free_planes(aj, p); free(h); free(w); free(r); free(hk);
     return rc;
 }
 

@@ -28,13 +28,15 @@ typedef double oreal;
 #endif
 
 /* stopping rules, PAPER.md:279-298 (Sect. 3.3).  max_iter is always an additional cap. */
-enum { ORACLE_STOP_MAXIT = 0, ORACLE_STOP_RELJ = 1, ORACLE_STOP_DISCREPANCY = 2 };
+enum { ORACLE_STOP_MAXIT = 0, ORACLE_STOP_RELJ = 1, ORACLE_STOP_DISCREPANCY = 2,
+       ORACLE_STOP_MINERR = 3 /* Eq.25: needs oracle_result.truth (reading A27) */ };
 /* initial guess, PAPER.md:260-267 (Sect. 3.1) */
-enum { ORACLE_INIT_USER = 0, ORACLE_INIT_CONST = 1, ORACLE_INIT_ZERO = 2, ORACLE_INIT_G = 3 };
+enum { ORACLE_INIT_USER = 0, ORACLE_INIT_CONST = 1, ORACLE_INIT_ZERO = 2, ORACLE_INIT_G = 3,
+       ORACLE_INIT_CONST_SMOOTH = 4 /* the constant image convolved with a Gaussian, PAPER.md:264 (reading A28) */ };
 /* where the PSF centre sits in the input array (reading A18) */
 enum { ORACLE_PSF_CENTER = 0, ORACLE_PSF_CORNER = 1 };
 /* stop_reason values in oracle_result (>0) and error codes (<0) */
-enum { ORACLE_REASON_MAXIT = 1, ORACLE_REASON_RELJ = 2, ORACLE_REASON_DISCREPANCY = 3 };
+enum { ORACLE_REASON_MAXIT = 1, ORACLE_REASON_RELJ = 2, ORACLE_REASON_DISCREPANCY = 3, ORACLE_REASON_MINERR = 4 };
 enum { ORACLE_OK = 0, ORACLE_ERR_ARG = -1, ORACLE_ERR_PSF = -2, ORACLE_ERR_DATA = -3,
        ORACLE_ERR_ALLOC = -4, ORACLE_ERR_LINESEARCH = -6, ORACLE_ERR_NONFINITE = -7 };
 
@@ -62,6 +64,9 @@ typedef struct {
     int strict;             /* A17: 1 = negative g is an error instead of being clamped */
     double rl_relax;        /* Eq.3: exponent of the multiplicative relaxation of RL; 1 = plain RL */
     double rl_linear;       /* Eq.4: constant lambda_k of the linear relaxation of RL; result projected on f >= 0; 1 = plain RL (reading A25) */
+    int flux_constraint;    /* 1: SGP projects on { f >= 0, sum_R f = c } (Bonettini et al. 2009; reading A26) */
+    double flux_value;      /* c; <= 0: c = (1/p) sum_j sum_S (g_j - b_j), clipped at 0 ("background-subtracted flux") */
+    double init_sigma;      /* ORACLE_INIT_CONST_SMOOTH: standard deviation of the Gaussian in pixels (reading A28) */
 } oracle_options;
 
 typedef struct {
@@ -81,6 +86,12 @@ typedef struct {
        (length max_iter) instead of the BB rules / the Armijo loop -- pin P4 and the replay
        mode of SURVEY.md section 7. */
     const double *force_alpha, *force_lambda;
+    /* Eq.25: truth = the object f~ on the S-bar grid (ny*nx oreal values, input, may be NULL);
+       trace_err[k] = ||f(k) - f~||_2 / ||f~||_2, k = 0..iterations (+1 entry for the discarded step of
+       ORACLE_STOP_MINERR), optional, length max_iter + 2; err_final = the value at the returned iterate. */
+    const void *truth;
+    double *trace_err;
+    double err_final;
 } oracle_result;
 
 void oracle_options_default(oracle_options *o);
@@ -119,6 +130,12 @@ int oracle_scaling(const oracle_problem *P, const oreal *f, double L1, double L2
 int oracle_project(long n, const oreal *f, const oreal *grad, const oreal *D, double alpha,
                    oreal *y);                                                     /* Eq.6 */
 int oracle_adaptive_bounds(long n, const oreal *y, double *L1, double *L2);
+/* Projection on { y >= 0, sum y = c } in the metric of D^-1 (Bonettini et al. 2009, cited PAPER.md:60, :68):
+   y = argmin sum_i (y_i - x_i)^2 / D_i  =>  y_i = max(0, x_i - mu D_i) with mu the root of sum_i y_i = c, found exactly
+   by sorting the break points x_i / D_i.  Entries with D_i = 0 (outside R) are fixed at y_i = 0.  *mu (may be NULL). */
+int oracle_project_flux(long n, const oreal *x, const oreal *D, double c, oreal *y, double *mu);
+/* relative reconstruction error of Eq.25 in the l2 norm over the whole grid */
+double oracle_rel_error(long n, const oreal *f, const oreal *truth);
 
 /* BB step-length state machine */
 typedef struct {
