@@ -74,8 +74,10 @@ def planes_per_launch(p: int, b_array: bool, masked: bool, backtracks_per_iter: 
         "K1_ratio_rowfft": k1, "K2_col_conjsum": 2 * p + 1, "K3_rowifft_grad_bb": 6 + m,
         "K4_project_rowfft": 4 + m, "K5_col_mult": 2 * p + 1, "K6_rowifft_linesearch": k6,
         "K7_backtrack": (3 * p + ba) * backtracks_per_iter,
+        # RL on the schedule of SURVEY.md 8(d) (7p + 6 planes): R3 = row C2R -> J0 -> ratio -> row R2C (spectrum_j, g_j read;
+        # ratio spectrum_j written), R6 = row C2R -> update -> row R2C (spectrum, f read; f, spectrum written); R1 runs once per run
         "R1_rowfft": 2, "R2_col_mult": 2 * p + 1, "R3_rowifft_q_J": 3 * p + ba, "R4_ratio_rowfft": 3 * p + ba,
-        "R5_col_conjsum": 2 * p + 1, "R6_rowifft_update": 3 + m,
+        "R5_col_conjsum": 2 * p + 1, "R6_rowifft_update": 4 + m,
     }
 
 
@@ -275,6 +277,25 @@ def oracle_time(w, iters_a: int, iters_b: int):
     return out
 
 
+def oracle_time_single_thread(workload: str):
+    """(seconds per SGP iteration, sample text) of the oracle on ONE host thread: t(1 iteration) - t(0 iterations) of the
+    same workload, in a child process (the OpenMP thread count is fixed when the oracle library is loaded)"""
+    code = ("import sys, time, json, numpy as np; sys.path.insert(0, %r)\n"
+            "import oracle; from bench import make_workload\n"
+            "w, _ = make_workload(%r, 0)\n"
+            "oo = oracle.default_options(**{**w['opts'], 'max_iter': 0})\n"
+            "P = oracle.Problem(w['psf'], masked=w['S'] is not None, S=w['S'], sigma_R=oo.sigma_R)\n"
+            "ge = P.embed(w['g']); be = [np.full((P.ny, P.nx), float(v)) for v in w['b']]\n"
+            "t = []\n"
+            "for it in (0, 1):\n"
+            "    oo.max_iter = it; t0 = time.perf_counter(); P.sgp(ge, be, opts=oo); t.append(time.perf_counter() - t0)\n"
+            "print(json.dumps(t))\n") % (str(ROOT), workload)
+    env = {**os.environ, "OMP_NUM_THREADS": "1"}
+    r = subprocess.run([sys.executable, "-c", code], capture_output=True, text=True, env=env, timeout=600)
+    t0, t1 = json.loads(r.stdout.strip().splitlines()[-1])
+    return t1 - t0, f"t(1 it) - t(0 it) = {t1:.2f}s - {t0:.2f}s, one thread"
+
+
 def run_reference(args):
     """Reference arm of this tier: the CPU oracle as it stands, on the host cores; rank 0 only."""
     rank = int(os.environ.get("RANK", "0"))
@@ -311,6 +332,44 @@ def run_reference(args):
     return 0
 
 
+def measure_other(name: str, alg_name: str, steps: int, dev, peak: float):
+    """device-timed throughput of another workload of BASELINE.json configs[4] (north_star's target names 3 x 2048^2
+    beside 2048^2; RL is timed separately): `steps` reconstructions after 3 warm-up ones, CUDA events on the launching
+    stream; fractions of the roofline on SURVEY.md 8(d)'s bytes (SGP: schedule A, 14p + 14 planes; RL: 7p + 6)."""
+    import torch
+    from paper_1210_2258_b200 import binding as B
+    w, desc = make_workload(name, 0)
+    p = len(w["g"]); ny, nx = w["psf"][0].shape
+    to_dev = lambda a: torch.as_tensor(np.ascontiguousarray(a, dtype=np.float32), device=dev)
+    opts = B.default_options(**{**w["opts"], "stop_rule": 0})
+    plan = B.Plan([to_dev(k) for k in w["psf"]], S=w["S"], opts=opts)
+    g = [to_dev(a) for a in w["g"]]
+    f_out = torch.empty((ny, nx), dtype=torch.float32, device=dev)
+    alg = B.ALG_SGP if alg_name == "sgp" else B.ALG_RL
+    for _ in range(3):
+        _, r = plan.run(alg, g, w["b"], opts=opts, f_out=f_out, traces=False)
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize(); ev0.record()
+    loop_ms = 0.0
+    for _ in range(steps):
+        _, r = plan.run(alg, g, w["b"], opts=opts, f_out=f_out, traces=False)
+        loop_ms += r.loop_ms
+    ev1.record(); torch.cuda.synchronize()
+    ms = ev0.elapsed_time(ev1)
+    plan.close()
+    iters = r.iterations
+    masked = 1 if w["S"] is not None else 0
+    planes = (14 * p + 14 + 2 * masked) if alg_name == "sgp" else (7 * p + 6 + masked)
+    it_us = 1e3 * (loop_ms / steps) / iters
+    gbs = planes * ny * nx * 4 / (it_us * 1e-6) / 1e9
+    return {"workload": desc, "algorithm": alg_name, "dtype": "f32", "value": iters * steps / (ms * 1e-3), "unit": "iterations/s",
+            "steps": steps, "iterations_per_step": iters, "ms_per_step": ms / steps, "iteration_us": round(it_us, 2),
+            "planes": planes, "schedule": "SURVEY 8(d) schedule A (14p+14)" if alg_name == "sgp" else "SURVEY 8(d) RL schedule (7p+6)",
+            "GBps": round(gbs, 1), "frac": round(gbs / peak, 4), "frac_nominal_8TBs": round(gbs / 8000.0, 4),
+            "gpixel_iter_per_s": iters * steps / (ms * 1e-3) * ny * nx / 1e9, "backtracks_per_iteration": r.total_backtracks / max(1, iters),
+            "fused_linesearch": int(r.fused_linesearch)}
+
+
 def run_ours(args):
     import torch
     import torch.distributed as dist
@@ -319,6 +378,9 @@ def run_ours(args):
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
+    if args.gpus != world:
+        raise SystemExit(f"--gpus {args.gpus} but WORLD_SIZE={world}: launch N > 1 as `python -m torch.distributed.run --nnodes=1 "
+                         f"--nproc-per-node N --master-addr 127.0.0.1 bench.py --gpus N ...` (one rank per GPU)")
     if not torch.cuda.is_available():
         raise RuntimeError("bench.py needs a CUDA device: there is no CPU fallback for the product path")
     torch.cuda.set_device(local)
@@ -392,6 +454,7 @@ def run_ours(args):
                             "frac": round(gbs / peak, 4), "share": round(msum / tot_ms, 4)}
     dom = max(kms, key=lambda k: kms[k][0])
     traffic = None          # DRAM read + write bytes of that kernel per launch, ncu --set full (profiles/traffic.md)
+    traffic_source = None
     tf = ROOT / "profiles" / "traffic.csv"
     if tf.exists():
         try:
@@ -399,19 +462,33 @@ def run_ours(args):
                 wl, dt_, alg_, kern, nbytes = [c.strip() for c in line.split(",")]
                 if (wl, dt_, alg_, kern) == (args.workload, args.dtype, args.alg, dom):
                     traffic = float(nbytes)
+                    traffic_source = ("NOT measured in this run (ncu cannot run inside it): profiles/traffic.csv, written from the "
+                                      "ncu --set full capture named in profiles/traffic.md (another box of the same pool, cold cache)")
         except Exception:
             traffic = None
     # schedule A (14p + 14 planes, the primary denominator); the kernels as built move 10p + 12 (+ 5p + 3p per backtracked iteration)
     iter_planes = (14 * p + 14 + (2 if w["S"] is not None else 0)) if args.alg == "sgp" else (
-        sum(planes[k] for k in planes if k.startswith("R")))
-    built_planes = sum(planes[k] for k in planes if k.startswith("K" if args.alg == "sgp" else "R"))
+        7 * p + 6 + (1 if w["S"] is not None else 0))
+    built_planes = sum(planes[k] for k in planes if k.startswith("K")) if args.alg == "sgp" else (
+        sum(planes[k] for k in kms if k.startswith("R") and k != "R1_rowfft"))
     it_us = 1e3 * (loop_ms / args.steps) / iters          # loop only (library's own events), local rank
     it_gbs = iter_planes * plane_bytes / (it_us * 1e-6) / 1e9
+    # the event pairs of the instrumented pass serialise the launches (no graph replay, no overlap of one kernel's tail with
+    # the next one's head), so the kernel times add up to more than the iteration: `us_in_iteration` apportions the
+    # un-instrumented iteration time by the measured shares, and those do add up to iteration.us
+    sum_us = sum(v["avg_us"] * v["launches"] for v in per_kernel.values()) / max(1, iters)
+    for v in per_kernel.values():
+        v["us_in_iteration"] = round(v["share"] * it_us, 2)
+        v["frac_nominal_8TBs"] = round(v["GBps"] / 8000.0, 4)
     roofline = {"bound": "hbm", "kernel": dom, "achieved": per_kernel[dom]["GBps"], "peak": peak, "unit": "GB/s",
-                "frac": per_kernel[dom]["frac"], "traffic": traffic, "peak_source": peak_src,
+                "frac": per_kernel[dom]["frac"], "frac_nominal_8TBs": round(per_kernel[dom]["GBps"] / 8000.0, 4),
+                "traffic": traffic, "traffic_source": traffic_source, "peak_source": peak_src,
+                "note": "2048^2 single image: the 10-plane working set largely stays in the 126 MB L2, the kernels are latency / "
+                        "issue-bound, not HBM-bound (DESIGN.md section 6); `frac` divides ALGORITHMIC bytes by time",
+                "sum_of_kernel_us_instrumented": round(sum_us, 2),
                 "algorithmic_bytes_per_launch": planes[dom] * plane_bytes,
                 "iteration": {"planes": iter_planes, "bytes": iter_planes * plane_bytes, "us": round(it_us, 2),
-                              "GBps": round(it_gbs, 1), "frac": round(it_gbs / peak, 4),
+                              "GBps": round(it_gbs, 1), "frac": round(it_gbs / peak, 4), "frac_nominal_8TBs": round(it_gbs / 8000.0, 4),
                               "planes_as_built": round(built_planes, 2),
                               "frac_as_built": round(built_planes * plane_bytes / (it_us * 1e-6) / 1e9 / peak, 4),
                               "backtracks_per_iteration": backtracks / max(1, iters * args.steps)},
@@ -459,6 +536,12 @@ def run_ours(args):
         cpu = {"value": 1.0 / per_it, "unit": "iterations/s", "cores": cores, "kind": "oracle",
                "sample": f"{args.workload} ({p}x{ny}x{nx}) fp64 oracle: (t({ib} it) - t({ia} it)) / {ib - ia}, start-point phase excluded; "
                          f"t({ia})={ta:.2f}s t({ib})={tb:.2f}s; OpenMP over {cores} threads"}
+        if not args.no_cpu_single:
+            try:        # SURVEY.md 8(d) "Timing the oracle beside it": (i) single thread and (ii) all cores
+                st, stxt = oracle_time_single_thread(args.workload)
+                cpu["single_thread"] = {"value": 1.0 / st, "unit": "iterations/s", "cores": 1, "sample": stxt}
+            except Exception as e:
+                cpu["single_thread"] = {"error": f"{type(e).__name__}: {e}"}
 
     # ---- in-run comparison: the same iteration on cuFFT + torch kernels (north_star: "cuFFT ... in-run comparison baseline")
     cufft = None
@@ -468,6 +551,16 @@ def run_ours(args):
             cufft["speedup_of_this_library"] = value / cufft["value"]
         except Exception as e:      # a comparison leg must never take the bench line down
             cufft = {"error": f"{type(e).__name__}: {e}"}
+
+    # ---- the other workloads of BASELINE.json configs[4] (north_star's target names 3 x 2048^2 as well; RL timed separately)
+    others = None
+    if rank == 0 and world == 1 and not args.no_others and args.workload == "C4c" and args.alg == "sgp" and args.dtype == "f32":
+        others = []
+        for nm, al in (("C4b", "sgp"), ("C4c", "rl"), ("C4b", "rl")):
+            try:
+                others.append(measure_other(nm, al, max(2, min(args.steps, 3)), dev, peak))
+            except Exception as e:
+                others.append({"workload": nm, "algorithm": al, "error": f"{type(e).__name__}: {e}"})
 
     if rank == 0:
         line = {"metric": "SGP iterations/s" if args.alg == "sgp" else "RL iterations/s", "value": value, "unit": "iterations/s",
@@ -482,7 +575,7 @@ def run_ours(args):
                            "J0_final": J_final, "backtracks": backtracks // args.steps,
                            "fused_linesearch": int(r.fused_linesearch)},
                 "clocks": clk.summary(), "e2e": e2e, "gpu_launches": launches, "roofline": roofline, "cpu_baseline": cpu,
-                "cufft_compare": cufft}
+                "cufft_compare": cufft, "other_workloads": others}
         print(json.dumps(line))
     plan.close()
     if world > 1:
@@ -506,6 +599,8 @@ def main():
     ap.add_argument("--graph", type=int, default=1, help="1 = replay the iterations as CUDA graphs of 10 (default), 0 = plain launches; +4 / +8 = force the separate / fused line-search kernel (experiment)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
+    ap.add_argument("--no-cpu-single", action="store_true", help="skip the single-thread timing of the oracle")
+    ap.add_argument("--no-others", action="store_true", help="skip the C4b / RL lines of other_workloads")
     ap.add_argument("--no-cufft", action="store_true", help="skip the cuFFT + torch comparison leg")
     ap.add_argument("--cufft-iters", type=int, default=40, help="iterations timed by the cuFFT comparison leg")
     args = ap.parse_args()

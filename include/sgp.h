@@ -31,8 +31,9 @@
  *   - Errors: every entry point returns 0 (SGP_OK) or a negative sgp_status.  Nothing is printed, no
  *     exception crosses the ABI.  After an error inside the iteration f_out holds the last accepted
  *     iterate.  sgp_last_cuda_error() gives the text of the last CUDA error seen by this thread.
- *   - Grid sizes: the native FFT supports ny, nx in {64,128,256,320,512,640,1024,1280,2048,4096};
- *     any other size returns SGP_ERR_ARG.
+ *   - Grid sizes: ny, nx (independently) of the form 2^a 5^b within 64...4096 that are a power of two or a multiple of
+ *     40: 64 80 128 160 200 256 320 400 512 640 800 1000 1024 1280 1600 2000 2048 2560 3200 4000 4096; any other size
+ *     returns SGP_ERR_ARG (500, 625, 1250, 2500, 3125 have no radix plan; pad the grid).
  *   - A plan is not thread-safe; different plans may be used from different threads.
  */
 #ifndef SGP_B200_H
@@ -50,13 +51,13 @@ extern "C" {
 
 typedef enum { SGP_F32 = 0, SGP_F64 = 1 } sgp_dtype;
 /* stopping rules, PAPER.md:279-298 (Sect.3.3); max_iter is always an additional cap */
-typedef enum { SGP_STOP_MAXIT = 0, SGP_STOP_RELJ = 1, SGP_STOP_DISCREPANCY = 2 } sgp_stop;
+typedef enum { SGP_STOP_MAXIT = 0, SGP_STOP_RELJ = 1, SGP_STOP_DISCREPANCY = 2,
+               SGP_STOP_MINERR = 3 /* Eq.25: needs sgp_result.truth; DESIGN reading A27 */ } sgp_stop;
 /* initial guess, PAPER.md:260-267 (Sect.3.1) */
-typedef enum { SGP_INIT_USER = 0, SGP_INIT_CONST = 1, SGP_INIT_ZERO = 2, SGP_INIT_G = 3 } sgp_init;
+typedef enum { SGP_INIT_USER = 0, SGP_INIT_CONST = 1, SGP_INIT_ZERO = 2, SGP_INIT_G = 3,
+               SGP_INIT_CONST_SMOOTH = 4 /* the constant image convolved with a Gaussian (reading A28) */ } sgp_init;
 /* where the PSF centre sits in the input array (A18) */
 typedef enum { SGP_PSF_CENTER = 0, SGP_PSF_CORNER = 1 } sgp_psf_origin;
-/* FFT backend: the library's own kernels, or cuFFT as the in-run comparison baseline */
-typedef enum { SGP_FFT_NATIVE = 0, SGP_FFT_CUFFT = 1 } sgp_backend;
 /* problem kind of a plan */
 typedef enum { SGP_KIND_SINGLE = 0, SGP_KIND_MULTI = 1, SGP_KIND_BOUNDARY = 2 } sgp_kind;
 /* algorithm run by sgp_plan_run */
@@ -75,7 +76,8 @@ typedef enum {
 } sgp_status;
 
 /* stop_reason values in sgp_result */
-typedef enum { SGP_REASON_NONE = 0, SGP_REASON_MAXIT = 1, SGP_REASON_RELJ = 2, SGP_REASON_DISCREPANCY = 3 } sgp_reason;
+typedef enum { SGP_REASON_NONE = 0, SGP_REASON_MAXIT = 1, SGP_REASON_RELJ = 2, SGP_REASON_DISCREPANCY = 3,
+               SGP_REASON_MINERR = 4 } sgp_reason;
 
 /* Options; sgp_options_default() fills the paper's values. */
 typedef struct sgp_options {
@@ -94,28 +96,33 @@ typedef struct sgp_options {
     int max_backtracks;                          /* A16 */
     int psf_origin;                              /* sgp_psf_origin */
     int init;                                    /* sgp_init */
-    int refresh_every;                           /* A21: recompute A f from f every n iterations; 0 = never */
+    int refresh_every;                           /* A21 (sgp_* only): recompute A_j f and J0 from f after every n-th iteration; 0 = never */
     int strict;                                  /* A17: 1 = negative g is SGP_ERR_DATA instead of being clamped to 0 */
     int check_every;                             /* iterations enqueued between two host reads of the device status; 0 = auto */
-    int backend;                                 /* sgp_backend */
     int tile_cols;                               /* tuning: spectrum tile width in columns (power of 2); 0 = auto */
     int rows_per_block;                          /* tuning: rows per CTA in the row-FFT kernels (power of 2); 0 = auto */
-    int use_graph;                               /* bit 0 (default 1) = replay the iterations as CUDA graphs of 10, else plain stream launches;
-                                                    experiment switches: bit 1 = persistent column kernel, bit 2 / bit 3 = force the
-                                                    separate / the fused line-search kernel (default: chosen by working set vs L2),
-                                                    bit 4 = never use the two-CTAs-per-SM column kernel, bit 5 = fork the backtracking /
-                                                    ratio tail inside the graph */
+    int use_graph;                               /* bit 0 (default 1) = replay the iterations as CUDA graphs of 10 (kept across runs of a plan), else
+                                                    plain stream launches; the only bit that may differ per run.  Experiment switches (plan level):
+                                                    bit 1 = persistent column kernel, bit 2 / bit 3 = force the separate / the fused line-search
+                                                    kernel (default: chosen by working set vs L2), bit 4 = never use the two-CTAs-per-SM column
+                                                    kernel, bit 6 = RL / OSEM on the six separate launches of round 1 instead of the fused four */
     double rl_relax;                             /* rl_* only: exponent of the multiplicative relaxation, Eq.3:
                                                     f <- f o (W o sum_j A_j^T(g_j/(A_j f + b_j)))^rl_relax; 1 (default) = plain RL */
     double rl_linear;                            /* rl_* only: constant lambda_k of the linear relaxation, Eq.4:
                                                     f <- max(0, f - rl_linear f o (1 - W o sum_j A_j^T(g_j/(A_j f + b_j)))), the max being the paper's
                                                     non-negativity constraint (DESIGN reading A25); 1 (default) = plain RL; rl_relax and rl_linear both != 1 is SGP_ERR_ARG */
+    int flux_constraint;                         /* sgp_* only: 1 = project on { f >= 0, sum_R f = c } in the metric D^-1 (Bonettini et al. 2009, cited
+                                                    PAPER.md:60, :68; the paper itself uses f >= 0 only): y_i = max(0, x_i - mu D_i), mu by Newton steps on
+                                                    the piecewise-linear equation sum y = c, each one reduction over f and the gradient, no FFT.  f(0) is
+                                                    rescaled to the flux c (DESIGN reading A26).  0 (default) = off */
+    double flux_value;                           /* c; <= 0 (default): c = (1/p) sum_j sum_S (g_j - b_j), clipped at 0 */
+    double init_sigma;                           /* SGP_INIT_CONST_SMOOTH: standard deviation of the Gaussian in pixels (default 2) */
 } sgp_options;
 
 /* Result of a run.  The trace pointers are optional caller-allocated HOST arrays of max_iter+1 entries
  * (NULL = not wanted): trace_J[k] = J0(f(k)) for k = 0..iterations; trace_alpha[k], trace_lambda[k],
  * trace_rule[k] (0 = alpha0, 1 = BB1, 2 = Eq.9 minimum of BB2), trace_backtracks[k] describe the step
- * f(k) -> f(k+1).  RL fills trace_J only.
+ * f(k) -> f(k+1).  RL fills trace_J only; OSEM evaluates J0 at the final iterate only (J0_final) and leaves trace_J zero.
  * force_alpha / force_lambda (HOST arrays of max_iter doubles, NaN = not forced, NULL = off) are a
  * TEST-ONLY replay mode: alpha_k / lambda_k are taken from them instead of the BB rules / Armijo loop. */
 typedef struct sgp_result {
@@ -125,13 +132,23 @@ typedef struct sgp_result {
     double discrepancy_final;   /* 2 J0 / (p #S), Eq.26 */
     int total_backtracks;
     double L1_used, L2_used;
-    long n_fft2;                /* 2-D transforms executed inside the iteration loop (2p+2 per iteration) */
+    long n_fft2;                /* 2-D transforms executed inside the iteration loop, COUNTED on the device by the column passes
+                                   (2p+2 per SGP iteration and RL step, 4p per OSEM cycle, p+1 per refresh) */
     double setup_ms, loop_ms;   /* device time of the start-point phase and of the iteration loop (CUDA events) */
     long kernel_launches;       /* kernels of this library launched by the call */
     int fused_linesearch;       /* 1: the run used the fused line-search + ratio kernel (chosen by working set vs L2) */
+    int status;                 /* sgp_status of THIS problem (batched runs return the first error; every problem reports its own here) */
     double *trace_J, *trace_alpha, *trace_lambda;
     int *trace_rule, *trace_backtracks;
     const double *force_alpha, *force_lambda;
+    /* Eq.25: truth = the object f~ used to generate the data, a DEVICE array ny x nx in the dtype of the call
+     * (input; NULL = not given).  When given, trace_err[k] = ||f(k) - f~||_2 / ||f~||_2 for k = 0..iterations (optional HOST array
+     * of max_iter + 2 doubles; entry iterations + 1 holds the error of the discarded step after a SGP_STOP_MINERR stop) and
+     * err_final = the error of the returned iterate.  SGP_STOP_MINERR stops at the first k whose next step would increase the
+     * error and returns f(k) (sgp_* and rl_*; DESIGN reading A27). */
+    const void *truth;
+    double *trace_err;
+    double err_final;
 } sgp_result;
 
 typedef struct sgp_plan sgp_plan;
@@ -160,8 +177,10 @@ void sgp_result_init(sgp_result *res);           /* zero everything, NULL traces
 const char *sgp_strerror(int status);
 const char *sgp_version(void);
 const char *sgp_last_cuda_error(void);
-/* bytes of device workspace a plan of this shape allocates (0 for unsupported arguments) */
+/* upper bound of the device workspace a plan of this shape allocates at creation (0 for unsupported arguments); the
+ * per-run trace block (56 bytes per iteration of max_iter) comes on top.  sgp_plan_workspace_bytes: what a plan did allocate. */
 size_t sgp_workspace_bytes(int kind, int p, int ny, int nx, int dtype);
+size_t sgp_plan_workspace_bytes(const sgp_plan *plan);
 
 /* ---- one-shot entry points: DEVICE pointers ------------------------------------------------------
  * g: detected image(s), psf: PSF(s) on the object grid (any positive scale; normalised to unit sum
@@ -206,7 +225,7 @@ int osem_boundary(int p, const void *const *g, const void *const *psf, const voi
                   const void *f0, void *f_out, unsigned char *maskR_out, int dtype,
                   const sgp_options *opt, sgp_result *res, void *stream);
 
-/* ---- the same six calls with HOST pointers (copies inside the call; what bench.py times as e2e) -- */
+/* ---- the same calls with HOST pointers (copies inside the call; what bench.py times as e2e) -- */
 int sgp_single_host(const void *g, const void *psf, const void *b_arr, double b_const, const void *f0,
                     void *f_out, int ny, int nx, int dtype, const sgp_options *opt, sgp_result *res,
                     void *stream);
@@ -228,6 +247,13 @@ int rl_boundary_host(int p, const void *const *g, const void *const *psf, const 
                      const void *f0, void *f_out, unsigned char *maskR_out, int dtype,
                      const sgp_options *opt, sgp_result *res, void *stream);
 
+int osem_multi_host(int p, const void *const *g, const void *const *psf, const void *const *b_arr, const double *b_const,
+                    const void *f0, void *f_out, int ny, int nx, int dtype, const sgp_options *opt, sgp_result *res,
+                    void *stream);
+int osem_boundary_host(int p, const void *const *g, const void *const *psf, const void *const *b_arr, const double *b_const,
+                       int oy, int ox, int sy, int sx, int ny, int nx, const void *f0, void *f_out,
+                       unsigned char *maskR_out, int dtype, const sgp_options *opt, sgp_result *res, void *stream);
+
 /* ---- plan form: set-up once (workspace, twiddles, transfer functions, boundary weights), run many -- */
 /* kind SINGLE requires p = 1; for SINGLE / MULTI the (oy,ox,sy,sx) arguments are ignored (S = S-bar). */
 int sgp_plan_create(sgp_plan **plan, int kind, int p, int ny, int nx, int oy, int ox, int sy, int sx,
@@ -237,10 +263,36 @@ int sgp_plan_create(sgp_plan **plan, int kind, int p, int ny, int nx, int oy, in
 int sgp_plan_set_psf(sgp_plan *plan, const void *const *psf, void *stream);
 /* One reconstruction.  g, b_arr: HOST arrays of p DEVICE pointers (sy x sx each; b_arr or its entries may
  * be NULL -> b_const[j]).  algorithm: sgp_algorithm.  opt (may be NULL = the plan's options) replaces the
- * run-time options (everything except backend, tile_cols, rows_per_block, sigma_R, psf_origin). */
+ * run-time options; the plan-level fields (tile_cols, rows_per_block, sigma_R, psf_origin, use_graph bits > 0) must
+ * equal the plan's, else SGP_ERR_ARG. */
 int sgp_plan_run(sgp_plan *plan, int algorithm, const void *const *g, const void *const *b_arr,
                  const double *b_const, const void *f0, void *f_out, const sgp_options *opt,
                  sgp_result *res, void *stream);
+/* Batched plan: nb problems of the SAME geometry, dtype and PSFs solved at once -- the sub-domains of a
+ * mosaic, or a stack of frames from one instrument.  Every kernel of the iteration is launched once
+ * for all problems; each problem keeps its own step lengths, line search and stopping test.  g, b_arr, b_const: nb * p
+ * entries, problem-major (problem i, image j at i * p + j); f0 (may be NULL unless init = USER), f_out, res: nb entries.
+ * Not available in batched runs (SGP_ERR_UNSUPPORTED): flux_constraint, refresh_every, SGP_STOP_MINERR, the smoothed start
+ * with boundary correction, forced step lengths.  A plan created with nb = 1 is an ordinary plan. */
+int sgp_plan_create_batched(sgp_plan **plan, int nb, int kind, int p, int ny, int nx, int oy, int ox, int sy, int sx,
+                            int dtype, const sgp_options *opt);
+int sgp_plan_run_batched(sgp_plan *plan, int algorithm, const void *const *g, const void *const *b_arr,
+                         const double *b_const, const void *const *f0, void *const *f_out, const sgp_options *opt,
+                         sgp_result *res, void *stream);
+/* Mosaic of sub-domain reconstructions with boundary-effect correction ("the 256 x 256 ... images are
+ * partitioned into four partially overlapping 160 x 160 subdomains. Each ... is merged, by zero-padding, in a 256 x 256 array
+ * ... From the four reconstructions 128 x 128, nonoverlapping images are extracted and the complete reconstructed image is
+ * formed as a mosaic of them").  g[j]: the p detected images, Ny x Nx; psf[j]: ny x nx, the S-bar grid of every sub-problem;
+ * the image is cut into ty x tx sub-images of sy x sx pixels (sub-image t starts at clamp(t N/T - (s - N/T)/2, 0, N - s)), each
+ * placed in the centre of S-bar (DESIGN reading A29) and reconstructed by `algorithm` with Eq.16-23 -- all ty * tx at once, as
+ * one batched plan -- and the (Ny/ty) x (Nx/tx) parts are put together in f_out (Ny x Nx).  res: ty * tx entries, row-major
+ * over the tiles.  DEVICE pointers; the _host variant takes HOST pointers and copies inside the call. */
+int sgp_mosaic(int algorithm, int p, const void *const *g, const void *const *psf, const double *b_const, int Ny, int Nx,
+               int ty, int tx, int sy, int sx, int ny, int nx, void *f_out, int dtype, const sgp_options *opt,
+               sgp_result *res, void *stream);
+int sgp_mosaic_host(int algorithm, int p, const void *const *g, const void *const *psf, const double *b_const, int Ny, int Nx,
+                    int ty, int tx, int sy, int sx, int ny, int nx, void *f_out, int dtype, const sgp_options *opt,
+                    sgp_result *res, void *stream);
 /* Operators of the plan, for callers and tests: out = A_j x (Eq.16) / out = A_j^T y (Eq.17),
  * all ny x nx DEVICE arrays on the S-bar grid. */
 int sgp_plan_apply_A(sgp_plan *plan, int j, const void *x, void *out, void *stream);

@@ -14,23 +14,26 @@ import numpy as np
 
 _PKG = Path(__file__).resolve().parent
 _CSRC = _PKG / "csrc"
-LIB_PATH = _PKG / "libsgp_b200.so"
+import os as _os
+# SGP_B200_LIB: developer override (e.g. the FAST=1 build of csrc/Makefile); the product library is libsgp_b200.so
+LIB_PATH = Path(_os.environ["SGP_B200_LIB"]).resolve() if _os.environ.get("SGP_B200_LIB") else _PKG / "libsgp_b200.so"
 
 F32, F64 = 0, 1
-STOP_MAXIT, STOP_RELJ, STOP_DISCREPANCY = 0, 1, 2
-INIT_USER, INIT_CONST, INIT_ZERO, INIT_G = 0, 1, 2, 3
+STOP_MAXIT, STOP_RELJ, STOP_DISCREPANCY, STOP_MINERR = 0, 1, 2, 3
+INIT_USER, INIT_CONST, INIT_ZERO, INIT_G, INIT_CONST_SMOOTH = 0, 1, 2, 3, 4
 PSF_CENTER, PSF_CORNER = 0, 1
 KIND_SINGLE, KIND_MULTI, KIND_BOUNDARY = 0, 1, 2
 ALG_SGP, ALG_RL, ALG_OSEM = 0, 1, 2
 OK, ERR_ARG, ERR_PSF, ERR_DATA, ERR_ALLOC, ERR_CUDA, ERR_LINESEARCH, ERR_NONFINITE, ERR_UNSUPPORTED = 0, -1, -2, -3, -4, -5, -6, -7, -8
-REASON = {0: "none", 1: "maxit", 2: "relJ", 3: "discrepancy"}
+REASON = {0: "none", 1: "maxit", 2: "relJ", 3: "discrepancy", 4: "minerr"}
 
 EXPORTS = [
-    "sgp_options_default", "sgp_result_init", "sgp_strerror", "sgp_version", "sgp_last_cuda_error", "sgp_workspace_bytes",
+    "sgp_options_default", "sgp_result_init", "sgp_strerror", "sgp_version", "sgp_last_cuda_error", "sgp_workspace_bytes", "sgp_plan_workspace_bytes",
     "sgp_single", "sgp_multi", "sgp_boundary", "rl_single", "rl_multi", "rl_boundary",
     "osem_multi", "osem_boundary",
     "sgp_single_host", "sgp_multi_host", "sgp_boundary_host", "rl_single_host", "rl_multi_host", "rl_boundary_host",
-    "sgp_plan_create", "sgp_plan_set_psf", "sgp_plan_run", "sgp_plan_apply_A", "sgp_plan_apply_AT", "sgp_plan_get_mask",
+    "osem_multi_host", "osem_boundary_host",
+    "sgp_plan_create", "sgp_plan_create_batched", "sgp_plan_run_batched", "sgp_mosaic", "sgp_mosaic_host", "sgp_plan_set_psf", "sgp_plan_run", "sgp_plan_apply_A", "sgp_plan_apply_AT", "sgp_plan_get_mask",
     "sgp_plan_rfft2", "sgp_plan_irfft2", "sgp_plan_set_profiling", "sgp_plan_get_kernel_ms", "sgp_plan_destroy",
 ]
 PROF_SLOTS = ["K1_ratio_rowfft", "K2_col_conjsum", "K3_rowifft_grad_bb", "K4_project_rowfft", "K5_col_mult", "K6_rowifft_linesearch",
@@ -46,8 +49,9 @@ class Options(C.Structure):
         ("L1", C.c_double), ("L2", C.c_double), ("adaptive_L", C.c_int),
         ("max_iter", C.c_int), ("stop_rule", C.c_int), ("tol", C.c_double), ("disc_threshold", C.c_double),
         ("sigma_R", C.c_double), ("max_backtracks", C.c_int), ("psf_origin", C.c_int), ("init", C.c_int),
-        ("refresh_every", C.c_int), ("strict", C.c_int), ("check_every", C.c_int), ("backend", C.c_int),
+        ("refresh_every", C.c_int), ("strict", C.c_int), ("check_every", C.c_int),
         ("tile_cols", C.c_int), ("rows_per_block", C.c_int), ("use_graph", C.c_int), ("rl_relax", C.c_double), ("rl_linear", C.c_double),
+        ("flux_constraint", C.c_int), ("flux_value", C.c_double), ("init_sigma", C.c_double),
     ]
 
 
@@ -57,11 +61,12 @@ class _Result(C.Structure):
         ("discrepancy_final", C.c_double), ("total_backtracks", C.c_int),
         ("L1_used", C.c_double), ("L2_used", C.c_double), ("n_fft2", C.c_long),
         ("setup_ms", C.c_double), ("loop_ms", C.c_double), ("kernel_launches", C.c_long),
-        ("fused_linesearch", C.c_int),
+        ("fused_linesearch", C.c_int), ("status", C.c_int),
         ("trace_J", C.POINTER(C.c_double)), ("trace_alpha", C.POINTER(C.c_double)),
         ("trace_lambda", C.POINTER(C.c_double)), ("trace_rule", C.POINTER(C.c_int)),
         ("trace_backtracks", C.POINTER(C.c_int)),
         ("force_alpha", C.POINTER(C.c_double)), ("force_lambda", C.POINTER(C.c_double)),
+        ("truth", C.c_void_p), ("trace_err", C.POINTER(C.c_double)), ("err_final", C.c_double),
     ]
 
 
@@ -97,6 +102,8 @@ def lib() -> C.CDLL:
         L.sgp_version.restype = C.c_char_p
         L.sgp_last_cuda_error.restype = C.c_char_p
         L.sgp_workspace_bytes.restype = C.c_size_t
+        L.sgp_plan_workspace_bytes.restype = C.c_size_t
+        L.sgp_plan_workspace_bytes.argtypes = [C.c_void_p]
         L.sgp_options_default.restype = None
         L.sgp_result_init.restype = None
         L.sgp_plan_destroy.restype = None
@@ -145,13 +152,15 @@ class Result:
         self.lam = tr["lambda"][:k].copy()
         self.rule = tr["rule"][:k].copy()
         self.backtracks = tr["backtracks"][:k].copy()
+        self.err = tr["err"][: k + 2].copy()
+        self.err_final = raw.err_final
         self.maskR = None
 
 
-def _make_result(max_iter, force_alpha=None, force_lambda=None, traces=True):
+def _make_result(max_iter, force_alpha=None, force_lambda=None, traces=True, truth=None):
     n = max_iter + 1
     tr = {"J": np.zeros(n), "alpha": np.zeros(n), "lambda": np.zeros(n),
-          "rule": np.zeros(n, np.int32), "backtracks": np.zeros(n, np.int32)}
+          "rule": np.zeros(n, np.int32), "backtracks": np.zeros(n, np.int32), "err": np.full(n + 1, np.nan)}
     raw = _Result()
     lib().sgp_result_init(C.byref(raw))
     if traces:
@@ -167,6 +176,10 @@ def _make_result(max_iter, force_alpha=None, force_lambda=None, traces=True):
             a[: len(arr)] = np.asarray(arr, dtype=np.float64)[: len(a)]
             keep.append(a)
             setattr(raw, name, a.ctypes.data_as(C.POINTER(C.c_double)))
+    if truth is not None:          # Eq.25: a CUDA tensor holding the true object
+        raw.truth = truth.data_ptr()
+        raw.trace_err = tr["err"].ctypes.data_as(C.POINTER(C.c_double))
+        keep.append(truth)
     return raw, tr, keep
 
 
@@ -237,7 +250,7 @@ class Plan:
             pass
 
     def run(self, algorithm, g, b, f0=None, opts: Options | None = None, f_out=None, force_alpha=None, force_lambda=None,
-            traces=True, check=True):
+            traces=True, check=True, truth=None):
         """g: list of p CUDA tensors (sy x sx); b: list of p scalars or p CUDA tensors."""
         torch = _torch()
         o = opts or self.opts
@@ -254,7 +267,8 @@ class Plan:
         _check_dev(f0, (self.ny, self.nx), self.tdt, "f0")
         if f_out is None:
             f_out = torch.empty((self.ny, self.nx), dtype=self.tdt, device=g[0].device)
-        raw, tr, keep = _make_result(o.max_iter, force_alpha, force_lambda, traces)
+        _check_dev(truth, (self.ny, self.nx), self.tdt, "truth")
+        raw, tr, keep = _make_result(o.max_iter, force_alpha, force_lambda, traces, truth)
         rc = lib().sgp_plan_run(self.h, int(algorithm), _pp(g), b_arr, b_const, _dev_ptr(f0), _dev_ptr(f_out), C.byref(o),
                                 C.byref(raw), _stream_ptr())
         res = Result(raw, tr, rc)
@@ -270,6 +284,9 @@ class Plan:
 
     def osem(self, g, b, **kw):
         return self.run(ALG_OSEM, g, b, **kw)
+
+    def workspace_bytes(self) -> int:
+        return int(lib().sgp_plan_workspace_bytes(self.h))
 
     def set_profiling(self, on: bool):
         rc = lib().sgp_plan_set_profiling(self.h, int(bool(on)))
@@ -406,9 +423,106 @@ def rl_boundary(g, psf, b, oy, ox, f0=None, opts=None, host=False, check=True, f
     return _one_shot("rl_boundary", g, psf, b, f0, opts, boundary=(oy, ox), host=host, check=check, f_out=f_out)
 
 
-def osem_multi(g, psf, b, f0=None, opts=None, check=True, f_out=None):
-    return _one_shot("osem_multi", g, psf, b, f0, opts, check=check, f_out=f_out)
+def osem_multi(g, psf, b, f0=None, opts=None, host=False, check=True, f_out=None):
+    return _one_shot("osem_multi", g, psf, b, f0, opts, host=host, check=check, f_out=f_out)
 
 
-def osem_boundary(g, psf, b, oy, ox, f0=None, opts=None, check=True, f_out=None):
-    return _one_shot("osem_boundary", g, psf, b, f0, opts, boundary=(oy, ox), check=check, f_out=f_out)
+def osem_boundary(g, psf, b, oy, ox, f0=None, opts=None, host=False, check=True, f_out=None):
+    return _one_shot("osem_boundary", g, psf, b, f0, opts, boundary=(oy, ox), host=host, check=check, f_out=f_out)
+
+
+# ---- batched plans and the mosaic driver ------------------------------------
+
+class BatchedPlan(Plan):
+    """sgp_plan_create_batched: nb problems of one geometry and one set of PSFs, every kernel launched once for all of them"""
+
+    def __init__(self, nb, psfs, S=None, opts: Options | None = None):
+        torch = _torch()
+        self.nb = int(nb)
+        self.p = len(psfs)
+        self.ny, self.nx = psfs[0].shape
+        self.tdt = psfs[0].dtype
+        self.code = F32 if self.tdt == torch.float32 else F64
+        self.opts = opts or default_options()
+        self.S = S
+        kind = KIND_BOUNDARY if S is not None else (KIND_SINGLE if self.p == 1 else KIND_MULTI)
+        oy, ox, sy, sx = S if S is not None else (0, 0, self.ny, self.nx)
+        self.sy, self.sx = sy, sx
+        self.h = C.c_void_p()
+        rc = lib().sgp_plan_create_batched(C.byref(self.h), self.nb, kind, self.p, self.ny, self.nx, oy, ox, sy, sx, self.code, C.byref(self.opts))
+        if rc != OK:
+            self.h = None
+            raise SgpError(rc, "sgp_plan_create_batched")
+        for k in psfs:
+            _check_dev(k, (self.ny, self.nx), self.tdt, "psf")
+        self._psfs = psfs
+        rc = lib().sgp_plan_set_psf(self.h, _pp(psfs), _stream_ptr())
+        if rc != OK:
+            raise SgpError(rc, "sgp_plan_set_psf")
+
+    def run_batched(self, algorithm, g, b, f0=None, opts: Options | None = None, check=True):
+        """g: nb lists of p CUDA tensors; b: nb lists of p scalars.  Returns ([f_out per problem], [Result per problem])."""
+        torch = _torch()
+        o = opts or self.opts
+        flat_g = [t for prob in g for t in prob]
+        for t in flat_g:
+            _check_dev(t, (self.sy, self.sx), self.tdt, "g")
+        n = self.nb * self.p
+        b_const = (C.c_double * n)(*[float(v) for prob in b for v in prob])
+        f_out = [torch.empty((self.ny, self.nx), dtype=self.tdt, device=flat_g[0].device) for _ in range(self.nb)]
+        raws = (_Result * self.nb)()
+        trs = []
+        for i in range(self.nb):
+            lib().sgp_result_init(C.byref(raws[i]))
+            tr = {"J": np.zeros(o.max_iter + 1), "alpha": np.zeros(o.max_iter + 1), "lambda": np.zeros(o.max_iter + 1),
+                  "rule": np.zeros(o.max_iter + 1, np.int32), "backtracks": np.zeros(o.max_iter + 1, np.int32), "err": np.full(o.max_iter + 2, np.nan)}
+            raws[i].trace_J = tr["J"].ctypes.data_as(C.POINTER(C.c_double))
+            raws[i].trace_alpha = tr["alpha"].ctypes.data_as(C.POINTER(C.c_double))
+            raws[i].trace_lambda = tr["lambda"].ctypes.data_as(C.POINTER(C.c_double))
+            raws[i].trace_rule = tr["rule"].ctypes.data_as(C.POINTER(C.c_int))
+            raws[i].trace_backtracks = tr["backtracks"].ctypes.data_as(C.POINTER(C.c_int))
+            trs.append(tr)
+        rc = lib().sgp_plan_run_batched(self.h, int(algorithm), _pp(flat_g), None, b_const, _pp(f0) if f0 is not None else None,
+                                        _pp(f_out), C.byref(o), raws, _stream_ptr())
+        res = [Result(raws[i], trs[i], raws[i].status) for i in range(self.nb)]
+        if check and rc != OK:
+            raise SgpError(rc, "sgp_plan_run_batched")
+        return f_out, res
+
+
+def mosaic(algorithm, g, psf, b, ty, tx, sub, opts=None, host=False, check=True):
+    """sgp_mosaic / sgp_mosaic_host: g: p images (Ny x Nx); psf: p PSFs (ny x nx); b: p constants; sub = (sy, sx).
+    Returns (mosaic Ny x Nx, [Result per tile])."""
+    o = opts or default_options()
+    p = len(g)
+    nb = ty * tx
+    if host:
+        dt = np.dtype(g[0].dtype)
+        code = _dtype_code(dt)
+        g = [np.ascontiguousarray(a, dtype=dt) for a in g]; psf = [np.ascontiguousarray(a, dtype=dt) for a in psf]
+        Ny, Nx = g[0].shape; ny, nx = psf[0].shape
+        f_out = np.empty((Ny, Nx), dt)
+        pp = lambda arrs: (C.c_void_p * len(arrs))(*[a.ctypes.data for a in arrs])
+        fptr, stream, fn = C.c_void_p(f_out.ctypes.data), None, lib().sgp_mosaic_host
+    else:
+        torch = _torch()
+        tdt = g[0].dtype
+        code = F32 if tdt == torch.float32 else F64
+        Ny, Nx = g[0].shape; ny, nx = psf[0].shape
+        f_out = torch.empty((Ny, Nx), dtype=tdt, device=g[0].device)
+        pp, fptr, stream, fn = _pp, _dev_ptr(f_out), _stream_ptr(), lib().sgp_mosaic
+    b_const = (C.c_double * p)(*[float(v) for v in b])
+    raws = (_Result * nb)()
+    trs = []
+    for i in range(nb):
+        lib().sgp_result_init(C.byref(raws[i]))
+        tr = {"J": np.zeros(o.max_iter + 1), "alpha": np.zeros(o.max_iter + 1), "lambda": np.zeros(o.max_iter + 1),
+              "rule": np.zeros(o.max_iter + 1, np.int32), "backtracks": np.zeros(o.max_iter + 1, np.int32), "err": np.full(o.max_iter + 2, np.nan)}
+        raws[i].trace_J = tr["J"].ctypes.data_as(C.POINTER(C.c_double))
+        trs.append(tr)
+    rc = fn(int(algorithm), p, pp(g), pp(psf), b_const, Ny, Nx, int(ty), int(tx), int(sub[0]), int(sub[1]), ny, nx, fptr, code,
+            C.byref(o), raws, stream)
+    res = [Result(raws[i], trs[i], raws[i].status) for i in range(nb)]
+    if check and rc != OK:
+        raise SgpError(rc, "sgp_mosaic")
+    return f_out, res

@@ -16,11 +16,12 @@ int validate_options(const sgp_options *o)
     if (o->armijo_memory < 1 || o->armijo_memory > SGP_MAX_ARMIJO_MEMORY) return SGP_ERR_ARG;
     if (o->max_iter < 0 || o->max_backtracks < 0 || o->alt_start < 0) return SGP_ERR_ARG;
     if (!o->adaptive_L && !(o->L1 > 0 && o->L1 < o->L2)) return SGP_ERR_ARG;
-    if (o->stop_rule < SGP_STOP_MAXIT || o->stop_rule > SGP_STOP_DISCREPANCY) return SGP_ERR_ARG;
-    if (o->init < SGP_INIT_USER || o->init > SGP_INIT_G) return SGP_ERR_ARG;
+    if (o->stop_rule < SGP_STOP_MAXIT || o->stop_rule > SGP_STOP_MINERR) return SGP_ERR_ARG;
+    if (o->init < SGP_INIT_USER || o->init > SGP_INIT_CONST_SMOOTH) return SGP_ERR_ARG;
+    if (o->init == SGP_INIT_CONST_SMOOTH && !(o->init_sigma > 0.0)) return SGP_ERR_ARG;
+    if (o->flux_constraint != 0 && o->flux_constraint != 1) return SGP_ERR_ARG;
     if (o->psf_origin != SGP_PSF_CENTER && o->psf_origin != SGP_PSF_CORNER) return SGP_ERR_ARG;
     if (o->check_every < 0 || o->refresh_every < 0) return SGP_ERR_ARG;
-    if (o->backend != SGP_FFT_NATIVE && o->backend != SGP_FFT_CUFFT) return SGP_ERR_ARG;
     if (!(o->rl_relax > 0.0) || !(o->rl_linear > 0.0)) return SGP_ERR_ARG;
     if (o->rl_relax != 1.0 && o->rl_linear != 1.0) return SGP_ERR_ARG;      // Eq.3 and Eq.4 are alternatives
     return SGP_OK;
@@ -35,6 +36,7 @@ static int elems_per_thread(int L, int dtype, bool col)
     return col ? fft_E_col<float>(L) : fft_E<float>(L);
 }
 static int pad_len(int L, int E) { return L + (L >> (E == 32 ? 5 : 4)); }
+static int row_len(int L, int E) { return (pad_len(L, E) + 1) & ~1; }      // fft_core.cuh: row_stride
 
 // Spectrum tile width C (columns per CTA of the column kernel) and rows per CTA of the row kernels.
 int choose_tiles(int ny, int nx, int dtype, const sgp_options *opt, int *C_out, int *RB_out)
@@ -54,17 +56,24 @@ int choose_tiles(int ny, int nx, int dtype, const sgp_options *opt, int *C_out, 
         if (!is_pow2(opt->tile_cols) || Lr % opt->tile_cols != 0) return SGP_ERR_ARG;
         C = opt->tile_cols;
     }
-    if (C * TFc > col_max || (C * TFc) % 32 != 0 || (size_t)C * pad_len(Lc, Ec) * esz > 227 * 1024) return SGP_ERR_ARG;
-    // row kernels: 256 threads per CTA; rows whose threads span several warps use one named barrier each (ids 1..15)
-    int RB = floor_pow2(256 / TFr > 1 ? 256 / TFr : 1);
+    if (C * TFc > col_max || (size_t)C * pad_len(Lc, Ec) * esz > 227 * 1024) return SGP_ERR_ARG;
+    if (((size_t)C * pad_len(Lc, Ec) * esz) % 16 != 0) return SGP_ERR_ARG;        // the landing zones of the bulk copies follow the exchange buffer
+    // row kernels: 256 threads per CTA; rows whose threads span several warps use one named barrier each (ids 1..15);
+    // the 5-smooth lengths pad a row's thread group to a synchronisable size (fft_core.cuh: group_threads)
+    const int TFg = group_threads(TFr);
+    int RB = floor_pow2(256 / TFg > 1 ? 256 / TFg : 1);
     if (RB > 32) RB = 32;
     if (opt && opt->rows_per_block > 0) {
         if (!is_pow2(opt->rows_per_block)) return SGP_ERR_ARG;
         RB = opt->rows_per_block;
     }
     while (RB > 1 && ny % RB != 0) RB /= 2;
-    if (RB * TFr > 256 || (RB * TFr) % 32 != 0 || (TFr > 32 && RB > 15)) return SGP_ERR_ARG;
-    if ((size_t)RB * pad_len(Lr, Er) * esz > 113 * 1024) return SGP_ERR_ARG;
+    if (RB * TFg > 256 || (RB * TFg) % 32 != 0 || (TFg > 32 && RB > 15)) return SGP_ERR_ARG;
+    {   // rows + the shared-memory copies of the twiddle tables (row_fwd.cuh) must leave room for two CTAs per SM
+        const size_t tables = dtype == SGP_F64 ? row_table_entries<double>(Lr) : row_table_entries<float>(Lr);
+        while (RB > 1 && ((size_t)RB * row_len(Lr, Er) + tables) * esz > 113 * 1024 && (RB / 2) * TFg % 32 == 0) RB /= 2;
+        if (((size_t)RB * row_len(Lr, Er) + tables) * esz > 113 * 1024) return SGP_ERR_ARG;
+    }
     *C_out = C; *RB_out = RB;
     return SGP_OK;
 }
@@ -77,8 +86,12 @@ size_t workspace_bytes(int kind, int p, int ny, int nx, int dtype)
     size_t planes = 7 * (size_t)p + 4;                 // khat, spec, g, b, q (two buffers), u per image; f, grad, d, scratch
     size_t b = planes * n * r;
     if (kind == SGP_KIND_BOUNDARY) b += (2 + (size_t)p) * n * r + n;     // alphaR, alpha, alpha_j on R (OSEM, Eq.22), M_R
-    b += ((size_t)nx + 1 + 2 * (size_t)ny + (size_t)ny * p) * 2 * r;   // twiddles, pack line, khatB
-    b += (size_t)(ny * (6 + 2 * p) + 1024 * p + 2048) * sizeof(double) + sizeof(Ctrl);
+    // twiddle tables (row passes, real<->complex, two column plans), pack line, companion lines of the transfer functions
+    b += ((size_t)nx * 2 + 3 * (size_t)ny + (size_t)ny * (p + 1) + 64) * 2 * r;
+    // per-CTA partial sums (one row of the grid per CTA at worst), per-chunk partials of the backtracking / flux kernels, set-up partials
+    b += ((size_t)ny * (6 + 2 * p) + 2 * (n * p / 4096 + 2) + 1024 * (size_t)p + 2 * 1184 + 4096) * sizeof(double);
+    b += sizeof(Ctrl) + 2048 /* BtInfo */ + 2 * 96 * sizeof(unsigned int);
+    b += 64 * 256;                                     // every piece is rounded up to 256 bytes
     return b;
 }
 
@@ -104,7 +117,8 @@ void sgp_options_default(sgp_options *o)
     o->disc_threshold = 1.0; o->sigma_R = 1e-2; o->max_backtracks = 30;
     o->psf_origin = SGP_PSF_CENTER; o->init = SGP_INIT_CONST;
     o->refresh_every = 0; o->strict = 0; o->check_every = 0;
-    o->backend = SGP_FFT_NATIVE; o->tile_cols = 0; o->rows_per_block = 0; o->use_graph = 1; o->rl_relax = 1.0; o->rl_linear = 1.0;
+    o->flux_constraint = 0; o->flux_value = 0.0; o->init_sigma = 2.0;
+    o->tile_cols = 0; o->rows_per_block = 0; o->use_graph = 1; o->rl_relax = 1.0; o->rl_linear = 1.0;
 }
 
 void sgp_result_init(sgp_result *r) { if (r) memset(r, 0, sizeof(*r)); }
@@ -129,17 +143,24 @@ const char *sgp_version(void) { return "sgp-b200 0.1.0 (sm_100a)"; }
 const char *sgp_last_cuda_error(void) { return g_last_cuda_error.c_str(); }
 
 size_t sgp_workspace_bytes(int kind, int p, int ny, int nx, int dtype) { return workspace_bytes(kind, p, ny, nx, dtype); }
+size_t sgp_plan_workspace_bytes(const sgp_plan *plan);
 
 int sgp_plan_create(sgp_plan **plan, int kind, int p, int ny, int nx, int oy, int ox, int sy, int sx, int dtype,
                     const sgp_options *opt)
 {
+    return sgp_plan_create_batched(plan, 1, kind, p, ny, nx, oy, ox, sy, sx, dtype, opt);
+}
+
+int sgp_plan_create_batched(sgp_plan **plan, int nb, int kind, int p, int ny, int nx, int oy, int ox, int sy, int sx, int dtype,
+                            const sgp_options *opt)
+{
     if (!plan) return SGP_ERR_ARG;
+    if (nb < 1 || nb > 65535) { *plan = nullptr; return SGP_ERR_ARG; }
     *plan = nullptr;
     sgp_options o;
     if (opt) o = *opt; else sgp_options_default(&o);
     int rc = validate_options(&o);
     if (rc) return rc;
-    if (o.backend != SGP_FFT_NATIVE) return SGP_ERR_UNSUPPORTED;
     if (dtype != SGP_F32 && dtype != SGP_F64) return SGP_ERR_ARG;
     if (kind < SGP_KIND_SINGLE || kind > SGP_KIND_BOUNDARY) return SGP_ERR_ARG;
     if (p < 1 || p > SGP_MAX_IMAGES || (kind == SGP_KIND_SINGLE && p != 1)) return SGP_ERR_ARG;
@@ -150,7 +171,7 @@ int sgp_plan_create(sgp_plan **plan, int kind, int p, int ny, int nx, int oy, in
     } else { oy = 0; ox = 0; sy = ny; sx = nx; }
     PlanBase *b = dtype == SGP_F32 ? make_plan_f32() : make_plan_f64();
     if (!b) return SGP_ERR_ALLOC;
-    b->kind = kind; b->p = p; b->ny = ny; b->nx = nx; b->dtype = dtype; b->opt = o;
+    b->kind = kind; b->p = p; b->ny = ny; b->nx = nx; b->dtype = dtype; b->opt = o; b->nb = nb;
     b->G.ny = ny; b->G.nx = nx; b->G.oy = oy; b->G.ox = ox; b->G.sy = sy; b->G.sx = sx;
     b->G.masked = kind == SGP_KIND_BOUNDARY ? 1 : 0; b->G.p = p;
     rc = b->init();
@@ -161,6 +182,8 @@ int sgp_plan_create(sgp_plan **plan, int kind, int p, int ny, int nx, int oy, in
     *plan = pl;
     return SGP_OK;
 }
+
+size_t sgp_plan_workspace_bytes(const sgp_plan *plan) { return plan ? plan->impl->bytes_allocated : 0; }
 
 void sgp_plan_destroy(sgp_plan *plan)
 {
@@ -180,6 +203,13 @@ int sgp_plan_run(sgp_plan *plan, int algorithm, const void *const *g, const void
 {
     if (!plan) return SGP_ERR_ARG;
     return plan->impl->run(algorithm, g, b_arr, b_const, f0, f_out, opt, res, (cudaStream_t)stream);
+}
+
+int sgp_plan_run_batched(sgp_plan *plan, int algorithm, const void *const *g, const void *const *b_arr, const double *b_const,
+                         const void *const *f0, void *const *f_out, const sgp_options *opt, sgp_result *res, void *stream)
+{
+    if (!plan) return SGP_ERR_ARG;
+    return plan->impl->run_batched(algorithm, g, b_arr, b_const, f0, f_out, opt, res, (cudaStream_t)stream);
 }
 
 int sgp_plan_apply_A(sgp_plan *plan, int j, const void *x, void *out, void *stream)
@@ -380,6 +410,17 @@ int rl_multi_host(int p, const void *const *g, const void *const *psf, const voi
 {
     return host_shot(SGP_ALG_RL, SGP_KIND_MULTI, p, g, psf, b_arr, b_const, 0, 0, ny, nx, ny, nx, f0, f_out, nullptr, dtype, opt, res, stream);
 }
+int osem_multi_host(int p, const void *const *g, const void *const *psf, const void *const *b_arr, const double *b_const,
+                    const void *f0, void *f_out, int ny, int nx, int dtype, const sgp_options *opt, sgp_result *res, void *stream)
+{
+    return host_shot(SGP_ALG_OSEM, SGP_KIND_MULTI, p, g, psf, b_arr, b_const, 0, 0, ny, nx, ny, nx, f0, f_out, nullptr, dtype, opt, res, stream);
+}
+int osem_boundary_host(int p, const void *const *g, const void *const *psf, const void *const *b_arr, const double *b_const,
+                       int oy, int ox, int sy, int sx, int ny, int nx, const void *f0, void *f_out, unsigned char *maskR_out,
+                       int dtype, const sgp_options *opt, sgp_result *res, void *stream)
+{
+    return host_shot(SGP_ALG_OSEM, SGP_KIND_BOUNDARY, p, g, psf, b_arr, b_const, oy, ox, sy, sx, ny, nx, f0, f_out, maskR_out, dtype, opt, res, stream);
+}
 int sgp_boundary_host(int p, const void *const *g, const void *const *psf, const void *const *b_arr, const double *b_const,
                       int oy, int ox, int sy, int sx, int ny, int nx, const void *f0, void *f_out, unsigned char *maskR_out,
                       int dtype, const sgp_options *opt, sgp_result *res, void *stream)
@@ -391,6 +432,87 @@ int rl_boundary_host(int p, const void *const *g, const void *const *psf, const 
                      int dtype, const sgp_options *opt, sgp_result *res, void *stream)
 {
     return host_shot(SGP_ALG_RL, SGP_KIND_BOUNDARY, p, g, psf, b_arr, b_const, oy, ox, sy, sx, ny, nx, f0, f_out, maskR_out, dtype, opt, res, stream);
+}
+
+// ---- mosaic of sub-domain reconstructions: one batched boundary plan over the ty x tx sub-images
+static int mosaic_start(int t, int N, int T, int s) { int h = N / T, o = t * h - (s - h) / 2; return o < 0 ? 0 : (o > N - s ? N - s : o); }
+
+int sgp_mosaic(int algorithm, int p, const void *const *g, const void *const *psf, const double *b_const, int Ny, int Nx,
+               int ty, int tx, int sy, int sx, int ny, int nx, void *f_out, int dtype, const sgp_options *opt,
+               sgp_result *res, void *stream)
+{
+    if (!g || !psf || !b_const || !f_out || !opt || !res || p < 1 || p > SGP_MAX_IMAGES) return SGP_ERR_ARG;
+    if (dtype != SGP_F32 && dtype != SGP_F64) return SGP_ERR_ARG;
+    if (ty < 1 || tx < 1 || Ny % ty || Nx % tx || sy < Ny / ty || sx < Nx / tx || sy > Ny || sx > Nx || sy > ny || sx > nx) return SGP_ERR_ARG;
+    cudaStream_t st = (cudaStream_t)stream;
+    const size_t r = dtype == SGP_F64 ? 8 : 4;
+    const int nb = ty * tx, hy = Ny / ty, hx = Nx / tx, oy = (ny - sy) / 2, ox = (nx - sx) / 2;
+    sgp_plan *pl = nullptr;
+    int rc = sgp_plan_create_batched(&pl, nb, SGP_KIND_BOUNDARY, p, ny, nx, oy, ox, sy, sx, dtype, opt);
+    if (rc) return rc;
+    DevBufs D;       // the sub-images (contiguous sy x sx copies of windows of g_j) and the nb reconstructions
+    const size_t sb = (size_t)sy * sx * r, nbytes = (size_t)ny * nx * r;
+    std::vector<const void *> gs((size_t)nb * p);
+    std::vector<void *> fo((size_t)nb);
+    std::vector<double> bc((size_t)nb * p);
+    rc = D.reserve((size_t)nb * p * DevBufs::al(sb) + (size_t)nb * DevBufs::al(nbytes));
+    for (int t = 0; t < nb && !rc; ++t) {
+        const int yi = mosaic_start(t / tx, Ny, ty, sy), xi = mosaic_start(t % tx, Nx, tx, sx);
+        for (int j = 0; j < p && !rc; ++j) {
+            void *sub = nullptr;
+            if (!g[j]) { rc = SGP_ERR_ARG; break; }
+            rc = D.blank(sb, &sub);
+            if (rc) break;
+            const unsigned char *src = static_cast<const unsigned char *>(g[j]) + ((size_t)yi * Nx + xi) * r;
+            if (cudaMemcpy2DAsync(sub, (size_t)sx * r, src, (size_t)Nx * r, (size_t)sx * r, (size_t)sy, cudaMemcpyDeviceToDevice, st) != cudaSuccess) rc = SGP_ERR_CUDA;
+            gs[(size_t)t * p + j] = sub; bc[(size_t)t * p + j] = b_const[j];
+        }
+        if (!rc) rc = D.blank(nbytes, &fo[t]);
+    }
+    if (!rc) rc = sgp_plan_set_psf(pl, psf, stream);
+    if (!rc) rc = sgp_plan_run_batched(pl, algorithm, gs.data(), nullptr, bc.data(), nullptr, fo.data(), opt, res, stream);
+    if (rc == SGP_OK || rc == SGP_ERR_LINESEARCH) {
+        for (int t = 0; t < nb; ++t) {
+            const int iy = t / tx, ix = t % tx;
+            const int yi = mosaic_start(iy, Ny, ty, sy), xi = mosaic_start(ix, Nx, tx, sx);
+            const int ys = iy * hy - yi + oy, xs = ix * hx - xi + ox;        // the non-overlapping part inside S-bar
+            const unsigned char *src = static_cast<const unsigned char *>(fo[t]) + ((size_t)ys * nx + xs) * r;
+            unsigned char *dst = static_cast<unsigned char *>(f_out) + ((size_t)iy * hy * Nx + (size_t)ix * hx) * r;
+            if (cudaMemcpy2DAsync(dst, (size_t)Nx * r, src, (size_t)nx * r, (size_t)hx * r, (size_t)hy, cudaMemcpyDeviceToDevice, st) != cudaSuccess && !rc) rc = SGP_ERR_CUDA;
+        }
+        if (cudaStreamSynchronize(st) != cudaSuccess && !rc) rc = SGP_ERR_CUDA;
+    }
+    sgp_plan_destroy(pl);
+    return rc;
+}
+
+int sgp_mosaic_host(int algorithm, int p, const void *const *g, const void *const *psf, const double *b_const, int Ny, int Nx,
+                    int ty, int tx, int sy, int sx, int ny, int nx, void *f_out, int dtype, const sgp_options *opt,
+                    sgp_result *res, void *stream)
+{
+    if (!g || !psf || !f_out || p < 1 || p > SGP_MAX_IMAGES || Ny < 1 || Nx < 1 || ny < 1 || nx < 1) return SGP_ERR_ARG;
+    if (dtype != SGP_F32 && dtype != SGP_F64) return SGP_ERR_ARG;
+    cudaStream_t st = (cudaStream_t)stream;
+    const size_t r = dtype == SGP_F64 ? 8 : 4;
+    const size_t ib = (size_t)Ny * Nx * r, kb = (size_t)ny * nx * r;
+    DevBufs D;
+    int rc = D.reserve((size_t)p * (DevBufs::al(ib) + DevBufs::al(kb)) + DevBufs::al(ib));
+    if (rc) return rc;
+    const void *dg[SGP_MAX_IMAGES], *dk[SGP_MAX_IMAGES];
+    for (int j = 0; j < p; ++j) {
+        if (!g[j] || !psf[j]) return SGP_ERR_ARG;
+        void *t;
+        if ((rc = D.up(g[j], ib, st, &t))) return rc; dg[j] = t;
+        if ((rc = D.up(psf[j], kb, st, &t))) return rc; dk[j] = t;
+    }
+    void *dout = nullptr;
+    if ((rc = D.blank(ib, &dout))) return rc;
+    rc = sgp_mosaic(algorithm, p, dg, dk, b_const, Ny, Nx, ty, tx, sy, sx, ny, nx, dout, dtype, opt, res, stream);
+    if (rc == SGP_OK || rc == SGP_ERR_LINESEARCH) {
+        SGP_CUDA_TRY(cudaMemcpyAsync(f_out, dout, ib, cudaMemcpyDeviceToHost, st));
+        SGP_CUDA_TRY(cudaStreamSynchronize(st));
+    }
+    return rc;
 }
 
 }  // extern "C"

@@ -6,145 +6,171 @@
 namespace sgpk {
 
 // ---------------------------------------------------------------- a9 (backtracks) + a11
-// Launched every iteration; returns at once when lambda = 1 was accepted by the RI_LS epilogue (the usual case).
-// Otherwise the Armijo loop lambda <- theta lambda runs here: every trial is one elementwise
-// pass over q_j + lambda u_j (no FFT), one grid-wide barrier, and the same decision taken redundantly by every
-// CTA.  The grid is sized by the occupancy API so that all CTAs are resident together, and the barrier is a
-// sense-reversing counter in the control block: an ordinary launch, because the empty cooperative launches of the
-// usual case cost 7 us per iteration.  The accepted step is NOT applied here: f + lambda d and q_j + lambda u_j
-// are formed by the next iteration's kernels (K1 in repair mode, Ctrl::need_k1 = 2; K3) or by final_update_kernel.
-template <typename T> struct BtParams {
-    Geom G;
-    DevOpts o;
-    Trace tr;
-    Ctrl *ct;
-    const T *q, *u, *g, *b;                      // image j at + j*plane; q: buffer Ctrl::qsel at + qsel*qbuf
-    size_t plane, qbuf;
-    int b_is_array;
-    double bconst[kMaxP];
-    double *part;                                // gridDim.x doubles
-};
-
+// The Armijo loop lambda <- theta lambda for the iterations whose lambda = 1 was rejected by the
+// line-search kernel.  Every trial is one elementwise pass over q_j + lambda u_j (no FFT).  It runs as a PROLOGUE of the
+// ratio kernel K1 (row_fwd.cuh), which follows the line-search kernel anyway: there is no kernel of its own and, when
+// lambda = 1 was accepted (the usual case), no work at all.
+//
+// Grid-wide coordination WITHOUT assuming that the CTAs of the grid are resident together (round 1 used a spinning
+// grid barrier, which hangs when another plan or an SM-limited context keeps part of the grid from being scheduled):
+// a trial is cut into `nchunks` fixed chunks of pixels; CTAs draw tickets T = 0, 1, 2, ... from one counter, ticket T
+// being chunk T % nchunks of trial T / nchunks.  A CTA holding a ticket of trial t waits until trials < t are decided
+// -- it waits only for chunks that are held by RUNNING CTAs (tickets are handed out in order), so it always makes
+// progress; CTAs scheduled late find the decision taken and leave.  The CTA that finishes the last chunk of a trial
+// sums the per-chunk partials in a fixed order (runs are deterministic whatever CTA did which chunk) and takes the
+// decision: accept (book-keeping by finish_iteration), give up (A16) or open the next trial.
 template <typename T> struct vec4_of;
 template <> struct vec4_of<float>  { using type = float4;  static constexpr int N = 4; };
 template <> struct vec4_of<double> { using type = double2; static constexpr int N = 2; };
 
-// all CTAs of the grid (resident together) meet here; bar[0] = arrival count, bar[1] = generation
-__device__ __forceinline__ void grid_barrier(unsigned int *bar)
-{
-    __syncthreads();
-    if (threadIdx.x == 0) {
-        const unsigned int gen = atomicAdd(&bar[1], 0u);
-        __threadfence();
-        if (atomicAdd(&bar[0], 1u) == gridDim.x - 1) {
-            atomicExch(&bar[0], 0u);
-            __threadfence();
-            atomicAdd(&bar[1], 1u);
-        } else {
-            while (atomicAdd(&bar[1], 0u) == gen) __nanosleep(64);
-        }
-        __threadfence();
-    }
-    __syncthreads();
-}
+constexpr int kBtVecPerThread = 4;                                   // vectors per thread and chunk
+template <typename T> __host__ __device__ constexpr size_t bt_chunk_elems() { return (size_t)256 * kBtVecPerThread * vec4_of<T>::N; }
 
+__device__ __forceinline__ unsigned int ld_volatile_u32(const unsigned int *p) { return *reinterpret_cast<const volatile unsigned int *>(p); }
+
+// The arguments live in a block in DEVICE memory (BtInfo, written by run() before the loop) and the function is NOT
+// inlined: compiled into the ratio kernel -- or called with arguments that take the address of the kernel's parameter
+// block -- it costs that kernel 7 us per launch at 2048^2 whether it runs or not (measured: 26.4 vs 19.0 us).
+template <typename T> struct BtInfo {
+    Geom G; DevOpts o; Trace tr; Ctrl *ct;
+    const T *q, *u, *g, *b;                      // p contiguous planes each; q: buffer Ctrl::qsel at + qsel*qbuf
+    size_t qbuf;
+    int b_is_array;
+    unsigned int nchunks;                        // chunks per trial, ~ one per CTA of the ratio kernel
+    unsigned int chunk_batches;                  // batches (of 256 x kBtVecPerThread vectors) per chunk
+    double bconst[kMaxP];
+    double *part;                                // nchunks doubles
+    unsigned int *sync;                          // the counters, one 128-byte line each (kBtNext ...): tickets and polls do not share a line with each other or with Ctrl
+};
+enum BtSyncSlot { kBtNext = 0, kBtDone = 32, kBtDecided = 64, kBtFinal = 65, kBtSyncWords = 96 };
+// Called by ALL threads of a CTA (blockDim.x <= 256).
 template <typename T>
-__global__ void __launch_bounds__(256) backtrack_kernel(const BtParams<T> P)
+__device__ __noinline__ void backtrack_rounds(const BtInfo<T> *__restrict__ I)
 {
+    __shared__ double red[32];
+    const BtInfo<T> &P = *I;
     using V = typename vec4_of<T>::type;
     constexpr int VN = vec4_of<T>::N;
-    __shared__ double red[32];
-    __shared__ double s_J;
+    __shared__ unsigned int s_ticket;
+    __shared__ int s_state;
     Ctrl *ct = P.ct;
-    if (ct->status != 0 || ct->accepted != 0) return;
     const Geom &G = P.G;
-    const size_t n = (size_t)G.ny * G.nx, nv = n / VN;
-    const size_t gtid = (size_t)blockIdx.x * blockDim.x + threadIdx.x, gstride = (size_t)gridDim.x * blockDim.x;
+    const int tid = threadIdx.x, nthr = blockDim.x;
+    const size_t n = (size_t)G.ny * G.nx, ntot = n * (size_t)G.p;
+    // everything the trials need is read BEFORE the first ticket is drawn (see the header)
     const int k = ct->k;
-    const T *qcur = P.q + (size_t)ct->qsel * P.qbuf;           // A_j f(k): the buffer the line-search kernel read
+    const T *qcur = P.q + (size_t)ct->qsel * P.qbuf;
     const double Jref = ct->Jref, gd = ct->gd;
-    double lambda = 1.0, Jnew = ct->Jtrial;
-    bool accepted = false, forced = false;
+    double forced_lambda = 0.0;
+    bool forced = false;
     if (P.tr.force_lambda) {
         const double fl = P.tr.force_lambda[k];
-        if (isfinite(fl)) { forced = true; lambda = fl / P.o.theta; }
+        if (isfinite(fl)) { forced = true; forced_lambda = fl; }
     }
-    grid_barrier(&ct->counter[6]);                             // every CTA has read the control block
-    int nbt = 0;
-    while (!accepted) {
-        if (!forced && nbt >= P.o.max_backtracks) {            // A16
-            if (blockIdx.x == 0 && threadIdx.x == 0) ct->status = SGP_ERR_LINESEARCH;
-            return;
+    __threadfence();
+    for (;;) {
+        if (tid == 0) s_ticket = atomicAdd(&P.sync[kBtNext], 1u);
+        __syncthreads();
+        const unsigned int ticket = s_ticket;
+        const unsigned int nchunks = P.nchunks;
+        const unsigned int trial = ticket / nchunks, chunk = ticket - trial * nchunks;
+        if (tid == 0) {
+            int st = 0;                                               // 0 = go, 1 = decision already taken
+            for (;;) {
+                if (ld_volatile_u32(&P.sync[kBtFinal]) != 0u) { st = 1; break; }
+                if (ld_volatile_u32(&P.sync[kBtDecided]) >= trial) break;
+                __nanosleep(300);
+            }
+            __threadfence();
+            s_state = st;
         }
-        lambda *= P.o.theta;
-        nbt++;
+        __syncthreads();
+        if (s_state != 0) return;
+        double lambda = 1.0;
+        for (unsigned int i = 0; i <= trial; ++i) lambda *= P.o.theta;       // PAPER.md:124, the oracle's own sequence of products
+        if (forced) lambda = forced_lambda;
         const T lam = (T)lambda;
+        // ---- this chunk of J(lambda) = sum_j sum_S kl(g_j, q_j + lambda u_j + b_j)
         double acc[1] = {0.0};
-        for (int j = 0; j < G.p; ++j) {
-            const T *q = qcur + (size_t)j * P.plane, *u = P.u + (size_t)j * P.plane, *g = P.g + (size_t)j * P.plane;
-            const T *b = P.b_is_array ? P.b + (size_t)j * P.plane : nullptr;
-            const T bc = (T)P.bconst[j];
-            // four vectors per thread and step, all loads issued before the first use (the trial is one pass over three
-            // planes: what counts is how many bytes each thread has in flight)
-            constexpr int UN = 4;
-            for (size_t i0 = gtid; i0 < nv; i0 += UN * gstride) {
-                V q4[UN], u4[UN], g4[UN];
-                bool ok[UN];
+        const int CHV = 256 * kBtVecPerThread * (int)P.chunk_batches; // vectors per chunk
+        const size_t e_begin = (size_t)chunk * (size_t)CHV * VN;
+        // kBtVecPerThread vectors per thread and step, all loads issued before the first use
+        for (int v0 = tid; v0 < CHV; v0 += nthr * kBtVecPerThread) {
+            V q4[kBtVecPerThread], u4[kBtVecPerThread], g4[kBtVecPerThread];
+            bool ok[kBtVecPerThread];
 #pragma unroll
-                for (int k4 = 0; k4 < UN; ++k4) {
-                    const size_t i = i0 + (size_t)k4 * gstride;
-                    ok[k4] = i < nv;
-                    if (ok[k4]) {
-                        q4[k4] = reinterpret_cast<const V *>(q)[i]; u4[k4] = reinterpret_cast<const V *>(u)[i];
-                        g4[k4] = reinterpret_cast<const V *>(g)[i];
-                    }
+            for (int v = 0; v < kBtVecPerThread; ++v) {
+                const int vi = v0 + v * nthr;
+                const size_t e0 = e_begin + (size_t)vi * VN;
+                ok[v] = vi < CHV && e0 < ntot;
+                if (ok[v]) {
+                    q4[v] = *reinterpret_cast<const V *>(qcur + e0); u4[v] = *reinterpret_cast<const V *>(P.u + e0);
+                    g4[v] = *reinterpret_cast<const V *>(P.g + e0);
                 }
+            }
 #pragma unroll
-                for (int k4 = 0; k4 < UN; ++k4) {
-                    if (!ok[k4]) continue;
-                    const size_t e0 = (i0 + (size_t)k4 * gstride) * VN;
-                    const int y = (int)(e0 / G.nx), x = (int)(e0 - (size_t)y * G.nx);
-                    if ((unsigned)(y - G.oy) >= (unsigned)G.sy) continue;
-                    const T *qa = reinterpret_cast<const T *>(&q4[k4]), *ua = reinterpret_cast<const T *>(&u4[k4]), *ga = reinterpret_cast<const T *>(&g4[k4]);
-                    if constexpr (VN == 4) {
-                        T yv[4], gv[4]; bool s[4];
+            for (int v = 0; v < kBtVecPerThread; ++v) {
+                if (!ok[v]) continue;
+                const size_t e0 = e_begin + (size_t)(v0 + v * nthr) * VN;
+                const int j = (int)(e0 / n);
+                const size_t ip = e0 - (size_t)j * n;
+                const int y = (int)(ip / G.nx), x = (int)(ip - (size_t)y * G.nx);
+                if ((unsigned)(y - G.oy) >= (unsigned)G.sy) continue;
+                const T bc = (T)P.bconst[j];
+                const T *qa = reinterpret_cast<const T *>(&q4[v]), *ua = reinterpret_cast<const T *>(&u4[v]), *ga = reinterpret_cast<const T *>(&g4[v]);
+                if constexpr (VN == 4) {
+                    T yv[4], gv[4]; bool s[4];
 #pragma unroll
-                        for (int c = 0; c < 4; ++c) {
-                            s[c] = (unsigned)(x + c - G.ox) < (unsigned)G.sx;
-                            const T bb = b ? b[e0 + c] : bc;
-                            yv[c] = (T)((T)(qa[c] + lam * ua[c]) + bb); gv[c] = ga[c];
-                        }
-                        acc[0] += (double)kl_quad(gv, yv, s);
-                    } else {
+                    for (int c = 0; c < 4; ++c) {
+                        s[c] = (unsigned)(x + c - G.ox) < (unsigned)G.sx;
+                        const T bb = P.b_is_array ? P.b[e0 + c] : bc;
+                        yv[c] = (T)((T)(qa[c] + lam * ua[c]) + bb); gv[c] = ga[c];
+                    }
+                    acc[0] += (double)kl_quad(gv, yv, s);
+                } else {
 #pragma unroll
-                        for (int c = 0; c < VN; ++c) {
-                            if ((unsigned)(x + c - G.ox) < (unsigned)G.sx) {
-                                const T bb = b ? b[e0 + c] : bc;
-                                acc[0] += (double)kl_term(ga[c], (T)((T)(qa[c] + lam * ua[c]) + bb));
-                            }
+                    for (int c = 0; c < VN; ++c) {
+                        if ((unsigned)(x + c - G.ox) < (unsigned)G.sx) {
+                            const T bb = P.b_is_array ? P.b[e0 + c] : bc;
+                            acc[0] += (double)kl_term(ga[c], (T)((T)(qa[c] + lam * ua[c]) + bb));
                         }
                     }
                 }
             }
         }
         block_reduce_sum<1>(acc, red);
-        if (threadIdx.x == 0) P.part[blockIdx.x] = acc[0];
-        grid_barrier(&ct->counter[6]);
-        double tot[1] = {0.0};
-        for (unsigned int bI = threadIdx.x; bI < gridDim.x; bI += blockDim.x) tot[0] += __ldcg(&P.part[bI]);
-        block_reduce_sum<1>(tot, red);
-        if (threadIdx.x == 0) s_J = tot[0];
+        __shared__ int s_last;
+        if (tid == 0) {
+            P.part[chunk] = acc[0];
+            __threadfence();
+            s_last = (atomicAdd(&P.sync[kBtDone], 1u) == nchunks - 1) ? 1 : 0;
+        }
         __syncthreads();
-        Jnew = s_J;
-        accepted = forced || (isfinite(Jnew) && Jnew <= Jref + P.o.beta * lambda * gd);
-        grid_barrier(&ct->counter[6]);     // partials may be overwritten by the next trial
-    }
-    if (forced) nbt = 0;
-    // ---- book-keeping by the last CTA to finish (every CTA has read the control block by now)
-    if (threadIdx.x == 0) {
-        __threadfence();
-        unsigned int tk = atomicAdd(&ct->counter[TK_BACKTRACK], 1u);
-        if (tk == gridDim.x - 1) { ct->counter[TK_BACKTRACK] = 0; finish_iteration(ct, P.o, P.tr, lambda, Jnew, nbt, 2); }
+        if (s_last) {                                                 // this CTA closes the trial
+            __threadfence();
+            double tot[1] = {0.0};
+            for (unsigned int c = tid; c < nchunks; c += nthr) tot[0] += __ldcg(&P.part[c]);
+            block_reduce_sum<1>(tot, red);
+            if (tid == 0) {
+                const double Jnew = tot[0];
+                const int nbt = (int)trial + 1;
+                const bool accepted = forced || (isfinite(Jnew) && Jnew <= Jref + P.o.beta * lambda * gd);
+                P.sync[kBtDone] = 0;
+                if (accepted) {
+                    finish_iteration(ct, P.o, P.tr, lambda, Jnew, forced ? 0 : nbt, 2);
+                    __threadfence();
+                    *reinterpret_cast<volatile unsigned int *>(&P.sync[kBtFinal]) = 1u;
+                } else if (nbt >= P.o.max_backtracks) {                // A16
+                    ct->status = SGP_ERR_LINESEARCH;
+                    __threadfence();
+                    *reinterpret_cast<volatile unsigned int *>(&P.sync[kBtFinal]) = 1u;
+                } else {
+                    __threadfence();
+                    *reinterpret_cast<volatile unsigned int *>(&P.sync[kBtDecided]) = trial + 1u;
+                }
+            }
+            __syncthreads();
+        }
     }
 }
 
@@ -230,14 +256,17 @@ __global__ void embed_inputs_kernel(const T *g, const T *b, T *G_out, T *B_out, 
     if (threadIdx.x == 0) part[blockIdx.x] = acc[0];
 }
 
-// c = max(0, (1/p) sum_j mean_S (g_j - b_j)) (A14); single thread, partials in fixed order
-template <typename T> __global__ void const_start_kernel(const double *part, int nparts, double denom, Ctrl *ct)
+// c = max(0, (1/p) sum_j mean_S (g_j - b_j)) (A14); single thread, partials in fixed order.  Also the flux of the
+// flux-constrained projection (A26): flux_value if > 0, else max(0, (1/p) sum_j sum_S (g_j - b_j)).
+template <typename T> __global__ void const_start_kernel(const double *part, int nparts, double denom, int p, double flux_value, Ctrl *ct)
 {
     if (threadIdx.x == 0 && blockIdx.x == 0) {
         double s = 0.0;
         for (int i = 0; i < nparts; ++i) s += part[i];
         double c = s / denom;
         ct->c0 = c < 0.0 ? 0.0 : c;
+        double fc = flux_value > 0.0 ? flux_value : s / (double)p;
+        ct->flux_c = fc < 0.0 ? 0.0 : fc;
     }
 }
 

@@ -13,13 +13,26 @@
 //   CM_MULT   : out_j = IFFTcol( K^_j o FFTcol(in) ), j < p              (a8: A_j d, Eq.16)
 // Column 0 of tile 0 carries the packed pair (kx = 0, kx = nx/2): with C~[ky] = conj(C[-ky]) the product is
 //   C'[ky] = A[ky] C[ky] + B[ky] C~[ky],  A = (K0 + KM)/2 (stored in column 0 of khat), B = (K0 - KM)/2 (khatB).
-// The partner values C[-ky] of that one column go through a small global scratch line (P.pack, L entries).
+// The partner values C[-ky] of that one column go through a small global scratch line (pack, L entries).
 #pragma once
 #include "ew.cuh"
 
 namespace sgpk {
 
 enum ColMode { CM_FWD = 0, CM_CONJSUM = 1, CM_MULT = 2, CM_INV = 3 };
+
+#ifndef SGP_COL_SPLIT
+#define SGP_COL_SPLIT 0     // measured at 2048^2 (round 2): K2 / K5 27.9 / 24.9 us split against 23.0 / 21.1 us as one group -- off
+#endif
+// all threads of the CTA, or the N threads of one column group (named barrier `id`)
+template <bool GROUP, int N> struct ColSync {
+    int id;
+    __device__ __forceinline__ void operator()() const
+    {
+        if constexpr (GROUP) asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(N) : "memory");
+        else __syncthreads();
+    }
+};
 
 // Bulk asynchronous copy global -> shared by the TMA engine (cp.async.bulk, SASS UBLKCP): ONE instruction of one
 // thread moves a whole tile (contiguous in the tile-major layout); completion is signalled on an mbarrier.
@@ -77,15 +90,29 @@ template <typename T> __host__ __device__ constexpr int col_default_C(int L)
     return C;
 }
 
+// the pass tables join the exchange buffer and the landing zones in shared memory where all of it fits (fft_core.cuh)
+template <typename T> __host__ __device__ constexpr bool col_tw_in_smem(int L, int Cc)
+{
+    const int E = fft_E_col<T>(L);
+    return SGP_TW_SMEM && Cc > 0 &&
+           ((size_t)Cc * fft_padded_len(L, E) + 2 * (size_t)Cc * L + (size_t)tw_total(L, E)) * sizeof(cx<T>) <= (size_t)227 * 1024;
+}
+
 template <typename T, int L, int MODE, bool MULTI, int CT>
 __device__ __forceinline__ void col_body(const ColParams<T> &P)
 {
     using C = cx<T>;
     constexpr int E = fft_E_col<T>(L);
     constexpr int TF = L / E;
+    constexpr bool TWS = (MODE == CM_CONJSUM || MODE == CM_MULT) && col_tw_in_smem<T>(L, CT);
     extern __shared__ __align__(16) unsigned char smem_raw[];
     C *sm = reinterpret_cast<C *>(smem_raw);
     pdl_trigger();
+    // batched plans: problem blockIdx.z works on its own spectra, scratch line and control block (ew.cuh: bshift)
+    const size_t boff = (size_t)blockIdx.z * P.slab;
+    const C *Pin = bshift(P.in, boff);
+    C *Pout = bshift(P.out, boff);
+    Ctrl *Pct = bshift(P.ct, boff);
 
     ColCtx<T, L, E> X;
     X.Cc = CT > 0 ? CT : P.G.C; X.tid = threadIdx.x; X.nthr = CT > 0 ? CT * TF : (int)blockDim.x;
@@ -94,8 +121,8 @@ __device__ __forceinline__ void col_body(const ColParams<T> &P)
     X.smc = sm + X.c;
     X.bufA = sm + (size_t)X.Cc * fft_padded_len(L, E);     // landing zone of the spectrum tile
     X.bufB = X.bufA + X.tile_len;                          // landing zone of the transfer-function tile
-    const int tid = X.tid, nthr = X.nthr, t = X.t, Cc = X.Cc;
-    volatile C *pack = P.pack;
+    const int tid = X.tid, nthr = X.nthr, Cc = X.Cc;
+    volatile C *pack = bshift(P.pack, boff);
     const SyncBlock sync;
     const int ntiles = P.ntiles;
     C v[E];
@@ -105,13 +132,26 @@ __device__ __forceinline__ void col_body(const ColParams<T> &P)
         for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
             const size_t tbase = (size_t)tile * X.tile_len + tid;
 #pragma unroll
-            for (int e = 0; e < E; ++e) v[e] = P.in[tbase + (size_t)e * nthr];
-            fft_block<T, L, E, (MODE == CM_FWD ? -1 : +1)>(v, X.smc, Cc, t, P.tw, sync);
+            for (int e = 0; e < E; ++e) v[e] = Pin[tbase + (size_t)e * nthr];
+            fft_block<T, L, E, (MODE == CM_FWD ? -1 : +1)>(v, X.smc, Cc, X.t, P.tw, sync);
 #pragma unroll
-            for (int e = 0; e < E; ++e) P.out[tbase + (size_t)e * nthr] = v[e];
+            for (int e = 0; e < E; ++e) Pout[tbase + (size_t)e * nthr] = v[e];
         }
         return;
     }
+    // SPLIT (SGP_COL_SPLIT, product modes compiled for their tile width): the CTA works as TWO groups of CT/2 columns, each with its
+    // own exchange buffer and its own named barrier.  The passes of a column FFT alternate between butterflies (FMA pipe) and
+    // exchanges (shared-memory pipe) with a barrier in between, so with ONE group per SM the two pipes are never busy together;
+    // two groups drift apart and overlap one's exchange with the other's butterflies.
+    constexpr bool SPLIT = SGP_COL_SPLIT && CT >= 2 && ((CT / 2) * TF) % 32 == 0;
+    constexpr int Cg = SPLIT ? CT / 2 : 1, GN = Cg * TF;
+    const int grp = SPLIT ? tid / GN : 0, lt = SPLIT ? tid - grp * GN : tid;
+    const int t = SPLIT ? lt / Cg : X.t;
+    const int cloc = SPLIT ? grp * Cg + (lt - t * Cg) : X.c;          // column of this thread inside the tile
+    const int lin = SPLIT ? t * CT + cloc : tid;                        // its element of "row" t of the tile (+ e * nthr for the others)
+    C *smc = SPLIT ? sm + (size_t)grp * Cg * fft_padded_len(L, E) + (lt - t * Cg) : X.smc;
+    const int cs = SPLIT ? Cg : Cc;
+    const ColSync<SPLIT, GN> gsync{1 + grp};
     const int p = MULTI ? P.p : 1;
     const int my_tiles = ((int)blockIdx.x < ntiles) ? (ntiles - 1 - (int)blockIdx.x) / (int)gridDim.x + 1 : 0;
     if (my_tiles == 0) return;
@@ -127,10 +167,15 @@ __device__ __forceinline__ void col_body(const ColParams<T> &P)
         bulk_load(X.bufB, P.khat + X.tile_of(0), tile_bytes, &bars[1]);
     }
     pdl_wait();
-    const int stop = P.check_status ? P.ct->status : 0;
-    if (tid == 0 && stop == 0) bulk_load(X.bufA, P.in + X.tile_of(0), tile_bytes, &bars[0]);
-    __syncthreads();                                            // barrier initialisation visible to all
+    // check_status = 2: an instance of the refresh round (A21), which runs only after every n-th iteration
+    const int stop = P.check_status ? (Pct->status != 0 || (P.check_status == 2 && Pct->refresh_due == 0)) : 0;
+    if (tid == 0 && stop == 0) bulk_load(X.bufA, Pin + X.tile_of(0), tile_bytes, &bars[0]);
+    C *tw_s = X.bufB + X.tile_len;
+    if constexpr (TWS) { if (stop == 0) copy_table_to_smem(tw_s, P.tw, tw_total(L, E), tid, nthr); }
+    const C *tw = TWS ? tw_s : P.tw;
+    __syncthreads();                                            // barrier initialisation (and the tables) visible to all
     if (stop != 0) { mbar_wait(&bars[1], 0); return; }
+    if (P.count_fft && blockIdx.x == 0 && tid == 0) atomicAdd(&Pct->nfft, (unsigned long long)(p + 1));   // p + 1 two-dimensional transforms pass through this launch
 
     if constexpr (MODE == CM_CONJSUM) {
         // unit of work u = it*p + j: spectrum and transfer function of image j on this CTA's it-th tile
@@ -138,17 +183,17 @@ __device__ __forceinline__ void col_body(const ColParams<T> &P)
         C acc[MULTI ? E : 1];
         for (int it = 0; it < my_tiles; ++it) {
             const bool packed = (blockIdx.x == 0 && it == 0);      // tile 0 holds the packed column
-            const bool pk = packed && X.c == 0;
+            const bool pk = packed && cloc == 0;
             for (int j = 0; j < p; ++j) {
                 const int u1 = it * p + j + 1, it1 = u1 / p, j1 = u1 - it1 * p;
                 mbar_wait(&bars[0], phA); phA ^= 1;                 // spectrum of this unit has landed
 #pragma unroll
-                for (int e = 0; e < E; ++e) v[e] = X.bufA[tid + e * nthr];
+                for (int e = 0; e < E; ++e) v[e] = X.bufA[lin + e * nthr];
                 if (u1 < units) {
                     __syncthreads();
-                    if (tid == 0) bulk_load(X.bufA, P.in + (size_t)j1 * P.specplane + X.tile_of(it1), tile_bytes, &bars[0]);
+                    if (tid == 0) bulk_load(X.bufA, Pin + (size_t)j1 * P.specplane + X.tile_of(it1), tile_bytes, &bars[0]);
                 }
-                fft_block<T, L, E, -1>(v, X.smc, Cc, t, P.tw, sync);
+                fft_block<T, L, E, -1, TWS>(v, smc, cs, t, tw, gsync);
                 if (packed) {
                     if (pk) {
 #pragma unroll
@@ -158,7 +203,7 @@ __device__ __forceinline__ void col_body(const ColParams<T> &P)
                 }
                 mbar_wait(&bars[1], phB); phB ^= 1;                 // transfer function of this unit has landed
 #pragma unroll
-                for (int e = 0; e < E; ++e) v[e] = cmulc(v[e], X.bufB[tid + e * nthr]);
+                for (int e = 0; e < E; ++e) v[e] = cmulc(v[e], X.bufB[lin + e * nthr]);
                 if (u1 < units) {
                     __syncthreads();
                     if (tid == 0) bulk_load(X.bufB, P.khat + (size_t)j1 * P.specplane + X.tile_of(it1), tile_bytes, &bars[1]);
@@ -174,23 +219,23 @@ __device__ __forceinline__ void col_body(const ColParams<T> &P)
 #pragma unroll
                 for (int e = 0; e < E; ++e) v[e] = acc[e];
             }
-            fft_block<T, L, E, +1>(v, X.smc, Cc, t, P.tw, sync);
-            C *dst = P.out + X.tile_of(it) + tid;
+            fft_block<T, L, E, +1, TWS>(v, smc, cs, t, tw, gsync);
+            C *dst = Pout + X.tile_of(it) + lin;
 #pragma unroll
             for (int e = 0; e < E; ++e) dst[(size_t)e * nthr] = v[e];
         }
     } else {   // CM_MULT
         for (int it = 0; it < my_tiles; ++it) {
             const bool packed = (blockIdx.x == 0 && it == 0);
-            const bool pk = packed && X.c == 0;
+            const bool pk = packed && cloc == 0;
             mbar_wait(&bars[0], phA); phA ^= 1;                     // spectrum of tile it has landed
 #pragma unroll
-            for (int e = 0; e < E; ++e) v[e] = X.bufA[tid + e * nthr];
+            for (int e = 0; e < E; ++e) v[e] = X.bufA[lin + e * nthr];
             if (it + 1 < my_tiles) {
                 __syncthreads();
-                if (tid == 0) bulk_load(X.bufA, P.in + X.tile_of(it + 1), tile_bytes, &bars[0]);
+                if (tid == 0) bulk_load(X.bufA, Pin + X.tile_of(it + 1), tile_bytes, &bars[0]);
             }
-            fft_block<T, L, E, -1>(v, X.smc, Cc, t, P.tw, sync);
+            fft_block<T, L, E, -1, TWS>(v, smc, cs, t, tw, gsync);
             if (packed) {
                 if (pk) {
 #pragma unroll
@@ -202,7 +247,7 @@ __device__ __forceinline__ void col_body(const ColParams<T> &P)
                 C w[E];
                 mbar_wait(&bars[1], phB); phB ^= 1;                 // transfer function (it, j) has landed
 #pragma unroll
-                for (int e = 0; e < E; ++e) w[e] = cmul(v[e], X.bufB[tid + e * nthr]);
+                for (int e = 0; e < E; ++e) w[e] = cmul(v[e], X.bufB[lin + e * nthr]);
                 if (j + 1 < p || it + 1 < my_tiles) {
                     __syncthreads();
                     if (tid == 0) {
@@ -211,8 +256,8 @@ __device__ __forceinline__ void col_body(const ColParams<T> &P)
                     }
                 }
                 if (pk) packed_fix<T, L, E, false>(w, pack, P.khatB + (size_t)j * L, t);
-                fft_block<T, L, E, +1>(w, X.smc, Cc, t, P.tw, sync);
-                C *dst = P.out + (size_t)j * P.specplane + X.tile_of(it) + tid;
+                fft_block<T, L, E, +1, TWS>(w, smc, cs, t, tw, gsync);
+                C *dst = Pout + (size_t)j * P.specplane + X.tile_of(it) + lin;
 #pragma unroll
                 for (int e = 0; e < E; ++e) dst[(size_t)e * nthr] = w[e];
             }
@@ -250,26 +295,35 @@ __global__ void __launch_bounds__(256, 2) col2_kernel(const ColParams<T> P)
     constexpr size_t tile_len = (size_t)L * Cc;
     const size_t tbase = (size_t)blockIdx.x * tile_len;
     const unsigned int tile_bytes = (unsigned int)(tile_len * sizeof(C));
-    const int stop = P.check_status ? P.ct->status : 0;
+    const size_t boff = (size_t)blockIdx.z * P.slab;
+    const C *Pin = bshift(P.in, boff);
+    C *Pout = bshift(P.out, boff);
+    Ctrl *Pct = bshift(P.ct, boff);
+    const int stop = P.check_status ? (Pct->status != 0 || (P.check_status == 2 && Pct->refresh_due == 0)) : 0;
     if (stop != 0) return;
+    if (P.count_fft && blockIdx.x == 0 && tid == 0) atomicAdd(&Pct->nfft, 2ull);
     if (tid == 0) {
         mbar_init(&bar, 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-        bulk_load(sm, P.in + tbase, tile_bytes, &bar);
+        bulk_load(sm, Pin + tbase, tile_bytes, &bar);
         // the transfer-function tile is wanted after the forward transform: start it on its way to L2 now (in the SGP
         // loop the planes touched since its last use have pushed it out to HBM)
         asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(P.khat + tbase), "r"(tile_bytes) : "memory");
     }
-    __syncthreads();                                            // barrier initialisation visible to all
+    constexpr bool TWS = SGP_TW_SMEM != 0;
+    C *tw_s = sm + (size_t)Cc * fft_padded_len(L, E);
+    if constexpr (TWS) copy_table_to_smem(tw_s, P.tw, tw_total(L, E), tid, nthr);
+    const C *tw = TWS ? tw_s : P.tw;
+    __syncthreads();                                            // barrier initialisation (and the tables) visible to all
     const SyncBlock sync;
     const bool packed = blockIdx.x == 0;                        // tile 0 holds the packed column (kx = 0 and nx/2)
     const bool pk = packed && c == 0;
-    volatile C *pack = P.pack;
+    volatile C *pack = bshift(P.pack, boff);
     C v[E];
     mbar_wait(&bar, 0);
 #pragma unroll
     for (int e = 0; e < E; ++e) v[e] = sm[tid + e * nthr];
-    fft_block<T, L, E, -1>(v, sm + c, Cc, t, P.tw, sync);       // its first exchange starts with a barrier: the tile has been read
+    fft_block<T, L, E, -1, TWS>(v, sm + c, Cc, t, tw, sync);    // its first exchange starts with a barrier: the tile has been read
     if (packed) {
         if (pk) {
 #pragma unroll
@@ -287,8 +341,8 @@ __global__ void __launch_bounds__(256, 2) col2_kernel(const ColParams<T> P)
         for (int u = 0; u < 8; ++u) v[e0 + u] = (MODE == CM_CONJSUM) ? cmulc(v[e0 + u], k[u]) : cmul(v[e0 + u], k[u]);
     }
     if (pk) packed_fix<T, L, E, MODE == CM_CONJSUM>(v, pack, P.khatB, t);
-    fft_block<T, L, E, +1>(v, sm + c, Cc, t, P.tw, sync);
-    C *dst = P.out + tbase + tid;
+    fft_block<T, L, E, +1, TWS>(v, sm + c, Cc, t, tw, sync);
+    C *dst = Pout + tbase + tid;
 #pragma unroll
     for (int e = 0; e < E; ++e) dst[(size_t)e * nthr] = v[e];
 }

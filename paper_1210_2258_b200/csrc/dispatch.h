@@ -20,7 +20,10 @@ template <typename T> col_kernel_t<T> get_col2(int L, int mode);
 inline bool size_supported(int n)
 {
     switch (n) {
-    case 64: case 128: case 256: case 320: case 512: case 640: case 1024: case 1280: case 2048: case 4096: return true;
+    case 64: case 128: case 256: case 512: case 1024: case 2048: case 4096:                                  // 2^a
+    case 80: case 160: case 200: case 320: case 400: case 640: case 800: case 1000: case 1280: case 1600:    // 2^a 5^b, multiples of 40
+    case 2000: case 2560: case 3200: case 4000:
+        return true;
     default: return false;
     }
 }

@@ -8,6 +8,7 @@
 // ny*C complex numbers.
 #pragma once
 #include <cooperative_groups.h>
+#include <type_traits>
 #include "fft_core.cuh"
 #include "sgp_dev.cuh"
 
@@ -16,11 +17,11 @@ namespace cg = cooperative_groups;
 
 enum RowFwdMode { RF_PLAIN = 0, RF_SETUP = 1, RF_RATIO = 2, RF_PROJECT = 3, RF_NMODES = 4 };
 enum RowFwdSetup { RFS_PSF = 0, RFS_MASK_S = 1 };
-enum RowInvMode { RI_PLAIN = 0, RI_GRAD = 1, RI_LS = 2, RI_QJ = 3, RI_RLUPDATE = 4, RI_LSF = 5, RI_NMODES = 6 };
-enum RowInvPlain { RIP_STORE = 0, RIP_RLMINMAX = 1 };
+enum RowInvMode { RI_PLAIN = 0, RI_GRAD = 1, RI_LS = 2, RI_QJ = 3, RI_RLUPDATE = 4, RI_LSF = 5, RI_QJF = 6, RI_RLUPF = 7, RI_NMODES = 8 };
+enum RowInvPlain { RIP_STORE = 0, RIP_RLMINMAX = 1, RIP_STORE_POS = 2 };
 enum MaskMode { MM_NONE = 0, MM_S = 1, MM_R = 2 };
-enum QJSub { QJ_INIT = 0, QJ_RL = 1, QJ_PLAIN = 2 };
-enum Ticket { TK_GRAD = 0, TK_LS = 1, TK_QJ = 2, TK_MINMAX = 3, TK_BACKTRACK = 4 };
+enum QJSub { QJ_INIT = 0, QJ_RL = 1, QJ_PLAIN = 2, QJ_REFRESH = 3 };
+enum Ticket { TK_GRAD = 0, TK_LS = 1, TK_QJ = 2, TK_MINMAX = 3, TK_BACKTRACK = 4, TK_ERR = 5 };
 
 template <typename T> struct RowParams {
     Geom G;
@@ -41,7 +42,45 @@ template <typename T> struct RowParams {
     double bconst[kMaxP];
     int cy, cxs;                      // PSF centre (RFS_PSF)
     int check_status;                 // 1: return immediately when ct->status != 0
+    unsigned int *btsync;             // K6: counters of the Armijo backtracking to re-arm (aux.cuh)
+    const void *btinfo;               // K1 in the SGP loop: BtInfo<T> block in device memory (aux.cuh: Armijo backtracking)
+    size_t slab, tr_slab;             // batched plans: bytes between the per-problem arrays / trace blocks of consecutive problems
 };
+
+// Batched plans (sgp_plan_create_batched; PAPER.md:385-389 solves four sub-domain problems): problem
+// b = blockIdx.z.  Every per-problem array of problem b lies `slab` bytes behind the one of problem b - 1 (one slab per
+// problem, identical layout); twiddle tables, transfer functions and boundary weights are shared.  The kernels work on
+// this per-problem view of the pointers of the parameter block; slab = 0 and gridDim.z = 1 for an ordinary plan.
+template <typename U> __device__ __forceinline__ U *bshift(U *p, size_t off)
+{
+    return p ? reinterpret_cast<U *>(reinterpret_cast<unsigned char *>(const_cast<typename std::remove_const<U>::type *>(p)) + off) : p;
+}
+template <typename T> struct RowPtrs {
+    const T *in0, *in1, *in2, *in3;
+    T *out0, *out1;
+    cx<T> *spec;
+    double *part, *part2;
+    Ctrl *ct;
+    Trace tr;
+    unsigned int *btsync;
+    const void *btinfo;
+    bool act;                         // false in the padding lanes of a thread group (fft_core.cuh: group_threads): no global stores
+};
+template <typename T> __device__ __forceinline__ RowPtrs<T> row_ptrs(const RowParams<T> &P)
+{
+    const size_t off = (size_t)blockIdx.z * P.slab, toff = (size_t)blockIdx.z * P.tr_slab;
+    RowPtrs<T> X;
+    X.in0 = bshift(P.in0, off); X.in1 = bshift(P.in1, off); X.in2 = bshift(P.in2, off); X.in3 = bshift(P.in3, off);
+    X.out0 = bshift(P.out0, off); X.out1 = bshift(P.out1, off); X.spec = bshift(P.spec, off);
+    X.part = bshift(P.part, off); X.part2 = bshift(P.part2, off); X.ct = bshift(P.ct, off);
+    X.btsync = bshift(P.btsync, off); X.btinfo = bshift(P.btinfo, off);
+    X.tr.J = bshift(P.tr.J, toff); X.tr.alpha = bshift(P.tr.alpha, toff); X.tr.lambda = bshift(P.tr.lambda, toff);
+    X.tr.rule = bshift(P.tr.rule, toff); X.tr.backtracks = bshift(P.tr.backtracks, toff);
+    X.tr.force_alpha = bshift(P.tr.force_alpha, toff); X.tr.force_lambda = bshift(P.tr.force_lambda, toff);
+    X.tr.err = bshift(P.tr.err, toff);
+    X.act = true;
+    return X;
+}
 
 template <typename T> struct ColParams {
     Geom G;
@@ -56,6 +95,8 @@ template <typename T> struct ColParams {
     int p;
     int ntiles;                       // (nx/2)/C
     int check_status;
+    int count_fft;                    // 1: add the p + 1 two-dimensional transforms of this pass to Ctrl::nfft
+    size_t slab;                      // batched plans: bytes between the per-problem arrays (in, out, pack, ct) of consecutive problems
 };
 
 // ---------------------------------------------------------------- elementwise pieces
@@ -68,6 +109,7 @@ __device__ __forceinline__ double kl_term(double g, double y)
     double t = (y - g) / g;
     return g * (t - log1p(t));
 }
+__device__ __forceinline__ float fast_rcp_f(float y) { float r; asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(y)); return r; }
 // float version: with u = (y-g)/(y+g), ln(y/g) = 2 atanh(u), hence
 //   g ln(g/y) + y - g = u [ (y-g) - 2 g u^2 (1/3 + u^2/5 + u^4/7 + ...) ]      (u^2 < 0.09: 9 terms, < 1 ulp)
 // and the plain form (y-g) - g log1p((y-g)/g) otherwise (no cancellation there).
@@ -111,8 +153,23 @@ __device__ __forceinline__ float kl_series(float g, float y, bool &ok)
     S = fmaf(w, S, 3.333333313e-01f);
     return u * fmaf(-2.f * g * w, S, dy);
 }
+// Pixels outside the range of kl_series: for y/g < 1/4 or > 4 the two terms of (y - g) - g ln(y/g) do not cancel (the
+// result is >= 0.16 g), so the logarithm may come from the hardware lg2 (relative error 2^-22 outside (1/2, 2)): 4
+// instructions instead of the ~60 of a division and log1pf -- a rejected Armijo trial, where most pixels overshoot,
+// ran 3-4 times longer than an accepted one.  g = 0 gives y; y <= 0 drops the log term (A17).
+__device__ __forceinline__ float kl_far(float g, float y)
+{
+    if (!(g > 0.f)) return y;
+    if (!(y > 0.f)) return y - g;
+    float rg, lr;
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(rg) : "f"(g));
+    asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(lr) : "f"(y * rg));
+    const float w = (y - g) * fast_rcp_f(y + g);
+    if (w * w < 0.36f) return kl_term(g, y);          // denormal / overflow corner cases of the fast test: the exact form
+    return fmaf(-0.69314718055994530942f * g, lr, y - g);
+}
 // sum of kl_term over the pixels of a quad selected by s[]: straight-line code for the common case (so that the
-// compiler interleaves the four dependency chains), the general kl_term only where a pixel needs it
+// compiler interleaves the four dependency chains), the far-range form only where a pixel needs it
 __device__ __forceinline__ float kl_quad(const float (&g)[4], const float (&y)[4], const bool (&s)[4])
 {
     float k[4]; bool ok[4];
@@ -120,7 +177,7 @@ __device__ __forceinline__ float kl_quad(const float (&g)[4], const float (&y)[4
     for (int c = 0; c < 4; ++c) k[c] = kl_series(g[c], y[c], ok[c]);
     if (!((ok[0] || !s[0]) && (ok[1] || !s[1]) && (ok[2] || !s[2]) && (ok[3] || !s[3]))) {
 #pragma unroll
-        for (int c = 0; c < 4; ++c) if (s[c] && !ok[c]) k[c] = kl_term(g[c], y[c]);
+        for (int c = 0; c < 4; ++c) if (s[c] && !ok[c]) k[c] = kl_far(g[c], y[c]);
     }
     return ((s[0] ? k[0] : 0.f) + (s[1] ? k[1] : 0.f)) + ((s[2] ? k[2] : 0.f) + (s[3] ? k[3] : 0.f));
 }
@@ -143,6 +200,7 @@ template <typename T> __device__ __forceinline__ T clipT(T f, T L1, T L2) { retu
 
 template <typename T> __device__ __forceinline__ cx<T> ld2(const T *p) { return *reinterpret_cast<const cx<T> *>(p); }
 template <typename T> __device__ __forceinline__ void st2(T *p, cx<T> v) { *reinterpret_cast<cx<T> *>(p) = v; }
+template <typename T> __device__ __forceinline__ void st2_if(bool act, T *p, cx<T> v) { if (act) *reinterpret_cast<cx<T> *>(p) = v; }
 
 // W = M_R / alpha (Eq.21/23) for the two pixels of a pair; unmasked: 1/p.  r0, r1 = pixel in R.
 template <typename T>
@@ -179,6 +237,7 @@ __device__ __forceinline__ double fast_div(double a, double b) { return a / b; }
 template <typename T> struct alignas(16) Quad { T a[4]; };
 template <typename T> __device__ __forceinline__ Quad<T> ldq(const T *p) { return *reinterpret_cast<const Quad<T> *>(p); }
 template <typename T> __device__ __forceinline__ void stq(T *p, const Quad<T> &v) { *reinterpret_cast<Quad<T> *>(p) = v; }
+template <typename T> __device__ __forceinline__ void stq_if(bool act, T *p, const Quad<T> &v) { if (act) *reinterpret_cast<Quad<T> *>(p) = v; }
 
 // address of spectrum entry (ky, kx) in the column-tile-major layout
 __device__ __forceinline__ size_t spec_index(const Geom &G, int ky, int kx)

@@ -165,6 +165,27 @@ template <int R, int DIR, typename T, typename C> __device__ __forceinline__ voi
             for (int s2 = 0; s2 < 8; ++s2) o[q + 4 * s2] = a[8 * q + s2];
 #pragma unroll
         for (int i = 0; i < 32; ++i) a[i] = o[i];
+    } else if constexpr (R == 10) {
+        // R1 = 2 (over a), R2 = 5 (b): r = 5a + b
+        const T C1 = (T)0.80901699437494742410, S1 = (T)0.58778525229247312917;   // (cos, sin)(2 pi / 10)
+        const T C2 = (T)0.30901699437494742410, S2 = (T)0.95105651629515357212;   // k = 2
+#pragma unroll
+        for (int b = 0; b < 5; ++b) dft2<DIR>(a[b], a[5 + b]);
+        // u[5*s1 + b] *= W10^(b*s1), s1 = 1
+        a[6] = tw_const<DIR>(a[6], C1, S1);
+        a[7] = tw_const<DIR>(a[7], C2, S2);
+        a[8] = tw_const<DIR>(a[8], -C2, S2);        // k = 3: cos(108deg), sin(108deg)
+        a[9] = tw_const<DIR>(a[9], -C1, S1);        // k = 4: cos(144deg), sin(144deg)
+#pragma unroll
+        for (int q = 0; q < 2; ++q) dft5<DIR, T>(a[5 * q], a[5 * q + 1], a[5 * q + 2], a[5 * q + 3], a[5 * q + 4]);
+        // position 5*s1 + s2 holds X[s1 + 2*s2]
+        C o[10];
+#pragma unroll
+        for (int q = 0; q < 2; ++q)
+#pragma unroll
+            for (int s2 = 0; s2 < 5; ++s2) o[q + 2 * s2] = a[5 * q + s2];
+#pragma unroll
+        for (int i = 0; i < 10; ++i) a[i] = o[i];
     } else if constexpr (R == 20) {
         // R1 = 4 (over a), R2 = 5 (b): r = 5a + b
 #pragma unroll
@@ -263,6 +284,18 @@ __host__ __device__ constexpr int plan_radix(int L, int E, int ip)
         case 320:  return ip == 0 ? 20 : ip <= 2 ? 4 : 0;
         case 640:  return ip == 0 ? 20 : ip <= 2 ? 4 : ip == 3 ? 2 : 0;
         case 1280: return ip == 0 ? 20 : ip <= 3 ? 4 : 0;
+        // the other 2^a 5^b lengths: radix 20 first, then 20 / 10 / 5 / 4 / 2
+        case 100:  return ip == 0 ? 20 : ip == 1 ? 5 : 0;
+        case 200:  return ip == 0 ? 20 : ip == 1 ? 10 : 0;
+        case 400:  return ip <= 1 ? 20 : 0;
+        case 500:  return ip == 0 ? 20 : ip <= 2 ? 5 : 0;
+        case 800:  return ip <= 1 ? 20 : ip == 2 ? 2 : 0;
+        case 1000: return ip == 0 ? 20 : ip == 1 ? 10 : ip == 2 ? 5 : 0;
+        case 1600: return ip <= 1 ? 20 : ip == 2 ? 4 : 0;
+        case 2000: return ip <= 1 ? 20 : ip == 2 ? 5 : 0;
+        case 2560: return ip == 0 ? 20 : ip <= 3 ? 4 : ip == 4 ? 2 : 0;
+        case 3200: return ip <= 1 ? 20 : ip == 2 ? 4 : ip == 3 ? 2 : 0;
+        case 4000: return ip <= 1 ? 20 : ip == 2 ? 10 : 0;
         }
     }
     return 0;
@@ -297,6 +330,19 @@ __host__ __device__ constexpr int tw_total(int L, int E)
 __host__ __device__ constexpr int pad_shift(int E) { return E == 32 ? 5 : 4; }
 template <int E> __host__ __device__ constexpr int fft_pad(int i) { return i + (i >> pad_shift(E)); }
 __host__ __device__ constexpr int fft_padded_len(int L, int E) { return L + (L >> pad_shift(E)); }
+// distance between the lines of two rows of a row-kernel CTA: even, so that every line starts on a 16-byte boundary (128-bit
+// accesses of the epilogues, cp.async) also where the padded length is odd (L = 80, 400, 500, 2000)
+__host__ __device__ constexpr int row_stride(int L, int E) { return (fft_padded_len(L, E) + 1) & ~1; }
+
+// Threads that work on one row FFT of TF = L/E lanes.  A group must be synchronisable on its own: within a warp (a power
+// of two <= 32) or whole warps (named barrier), so for the 5-smooth lengths (TF = 5, 10, 25, 40, 50, 100, ...) the group is
+// padded to TFP threads; the lanes t >= TF repeat lane TF - 1 (same loads, same shared-memory traffic), take part in the
+// barriers, and neither store to global memory nor contribute to a reduction.
+__host__ __device__ constexpr int group_threads(int TF)
+{
+    if (TF <= 32) { int p = 1; while (p < TF) p *= 2; return p; }
+    return (TF + 31) / 32 * 32;
+}
 
 // ---------------------------------------------------------------- synchronisation of the threads of one FFT
 // SyncBlock: all threads of the CTA (column kernel: the columns of a tile are interleaved over the warps).
@@ -316,7 +362,8 @@ template <int TF> struct SyncGroup {
 // elements are `cs` apart (1 for a row FFT; C for a column FFT stored as [element][column]).
 // tw = the per-pass twiddle tables of this plan (see above).  Every exchange is bracketed sync / store / sync / load, so shared memory
 // the caller used before the call is safe to reuse, and on return nobody is writing it.
-template <typename T, int L, int E, int DIR, int IP, int NS, typename SYNC>
+// TWS: the tables sit in shared memory (copied there by the caller), else in global memory (read-only path)
+template <typename T, int L, int E, int DIR, int IP, int NS, bool TWS, typename SYNC>
 __device__ __forceinline__ void fft_passes(cx<T> (&v)[E], cx<T> *__restrict__ sm, const int cs, const int t,
                                            const cx<T> *__restrict__ tw, const SYNC &sync)
 {
@@ -338,7 +385,7 @@ __device__ __forceinline__ void fft_passes(cx<T> (&v)[E], cx<T> *__restrict__ sm
             const C *twp = tw + tw_offset(L, E, IP) + jm;
 #pragma unroll
             for (int r = 1; r < R; ++r) {
-                C w = __ldg(&twp[(r - 1) * NS]);
+                C w = TWS ? twp[(r - 1) * NS] : __ldg(&twp[(r - 1) * NS]);
                 a[r] = (DIR < 0) ? cmul(a[r], w) : cmulc(a[r], w);
             }
             j0s[b] = (j / NS) * (NS * R) + jm;
@@ -358,14 +405,27 @@ __device__ __forceinline__ void fft_passes(cx<T> (&v)[E], cx<T> *__restrict__ sm
         sync();
 #pragma unroll
         for (int e = 0; e < E; ++e) v[e] = sm[fft_pad<E>(t + TF * e) * cs];
-        fft_passes<T, L, E, DIR, IP + 1, NS * R>(v, sm, cs, t, tw, sync);
+        fft_passes<T, L, E, DIR, IP + 1, NS * R, TWS>(v, sm, cs, t, tw, sync);
     }
 }
 
-template <typename T, int L, int E, int DIR, typename SYNC>
+template <typename T, int L, int E, int DIR, bool TWS = false, typename SYNC>
 __device__ __forceinline__ void fft_block(cx<T> (&v)[E], cx<T> *sm, int cs, int t, const cx<T> *tw, const SYNC &sync)
 {
-    fft_passes<T, L, E, DIR, 0, 1>(v, sm, cs, t, tw, sync);
+    fft_passes<T, L, E, DIR, 0, 1, TWS>(v, sm, cs, t, tw, sync);
+}
+
+// Twiddle tables in shared memory.  The pass tables of a transform are read (R - 1)/R times per element and pass -- as
+// often as the exchange buffer -- and as global loads they miss a good part of the time in what the shared-memory
+// carve-out leaves of the L1 (ncu, 2048^2: 28 % of the column kernel's twiddle sectors, 200 KB carve-out), each miss a trip
+// to L2 that the 4 warps per scheduler cannot hide: "long scoreboard" was the top stall of every FFT kernel.
+#ifndef SGP_TW_SMEM
+#define SGP_TW_SMEM 0      // measured at 2048^2 (round 2): every FFT kernel 0.5-2 us SLOWER with the tables in shared memory -- off
+#endif
+template <typename C>
+__device__ __forceinline__ void copy_table_to_smem(C *dst, const C *__restrict__ src, int count, int tid, int nthr)
+{
+    for (int i = tid; i < count; i += nthr) dst[i] = __ldg(&src[i]);
 }
 
 }  // namespace sgpk

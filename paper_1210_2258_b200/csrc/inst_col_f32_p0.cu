@@ -1,0 +1,5 @@
+#define SGP_T float
+#define SGP_COL_PART 0
+#define SGP_COL_FN get_col_f32_p0
+#define SGP_COL2_FN get_col2_f32
+#include "inst_col.inl"

@@ -1,0 +1,5 @@
+#define SGP_T double
+#define SGP_ROW_FWD 0
+#define SGP_ROW_PART 1
+#define SGP_ROW_FN get_rowi_f64_p1
+#include "inst_row.inl"

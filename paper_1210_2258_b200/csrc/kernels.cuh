@@ -6,3 +6,4 @@
 #include "row_inv.cuh"
 #include "col.cuh"
 #include "aux.cuh"
+#include "extra.cuh"

@@ -8,6 +8,7 @@
 #include <cmath>
 #include <string>
 #include <vector>
+#include <type_traits>
 #include "dispatch.h"
 
 namespace sgpk {
@@ -25,6 +26,7 @@ extern thread_local std::string g_last_cuda_error;
 
 struct PlanBase {
     int kind = 0, p = 1, ny = 0, nx = 0, dtype = 0;
+    int nb = 1;                    // problems of a batched plan (sgp_plan_create_batched); 1 = an ordinary plan
     Geom G{};
     sgp_options opt{};
     bool psf_set = false;
@@ -39,6 +41,8 @@ struct PlanBase {
     virtual int set_psf(const void *const *psf, cudaStream_t st) = 0;
     virtual int run(int algorithm, const void *const *g, const void *const *b_arr, const double *b_const,
                     const void *f0, void *f_out, const sgp_options *opt, sgp_result *res, cudaStream_t st) = 0;
+    virtual int run_batched(int algorithm, const void *const *g, const void *const *b_arr, const double *b_const,
+                            const void *const *f0, void *const *f_out, const sgp_options *opt, sgp_result *res, cudaStream_t st) = 0;
     virtual int apply(bool transpose, int j, const void *x, void *out, cudaStream_t st) = 0;
     virtual int get_mask(unsigned char *maskR_out, void *alpha_out, long *nR_out, cudaStream_t st) = 0;
     virtual int rfft2(const void *x, void *spec_out, cudaStream_t st) = 0;

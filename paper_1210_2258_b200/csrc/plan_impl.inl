@@ -6,10 +6,13 @@ namespace sgpk {
 template <typename T> struct PlanImpl : PlanBase {
     using C = cx<T>;
     size_t n = 0, nspec = 0;       // reals per plane, complex numbers per half spectrum (= n/2)
+    int lnb = 1;                   // problems per launch: nb inside run_batched, 1 in the set-up paths (which work on shared buffers)
+    size_t slab = 0, tr_slab = 0;  // batched plans: bytes between the per-problem arrays / the trace blocks of consecutive problems
     int Lr = 0, Lc = 0;            // FFT lengths: nx/2 (rows), ny (columns)
     bool use_pdl = true;
     bool fuse_ls = true;           // line-search kernel fused with the next iteration's ratio + row FFT (row_inv RI_LSF)
-    int row_threads = 0, col_threads = 0, nrb = 0, ntiles = 0, bt_grid = 0, nsm = 0, col_grid = 0;
+    int row_threads = 0, col_threads = 0, nrb = 0, ntiles = 0, nsm = 0, col_grid = 0;
+    size_t bt_chunks = 0, bt_batches = 1;   // chunks per Armijo trial and batches per chunk (aux.cuh: backtrack_rounds)
     size_t row_smem = 0, col_smem = 0;
     row_kernel_t<T> k_rowf[RF_NMODES] = {nullptr}, k_rowi[RI_NMODES] = {nullptr};
     col_kernel_t<T> k_colf = nullptr, k_conj = nullptr, k_mult = nullptr;
@@ -29,15 +32,25 @@ template <typename T> struct PlanImpl : PlanBase {
     unsigned char *MR = nullptr;
     double *part_bb = nullptr, *part_gd = nullptr, *part_J = nullptr, *part_bt = nullptr, *part_misc = nullptr;
     Ctrl *ct = nullptr;
+    BtInfo<T> *btinfo = nullptr;
+    unsigned int *btsync = nullptr, *fxsync = nullptr;
+    double *part_fx = nullptr, *part_err = nullptr;
+    size_t fx_chunks = 0, fx_batches = 1;
+    C *khatB_tmp = nullptr;        // companion line of the Gaussian's transfer function (smoothed constant start)
     // per-run trace buffers
-    double *trJ = nullptr, *trA = nullptr, *trL = nullptr, *fA = nullptr, *fL = nullptr;
+    double *trJ = nullptr, *trA = nullptr, *trL = nullptr, *fA = nullptr, *fL = nullptr, *trE = nullptr;
     int *trR = nullptr, *trB = nullptr;
     int trace_cap = 0;
     cudaEvent_t ev0 = nullptr, ev1 = nullptr, ev2 = nullptr;
     cudaStream_t cap_stream = nullptr;       // stream the iteration graph is captured on (use_graph)
-    cudaStream_t cap_stream2 = nullptr;      // side branch of the graph: backtracking kernel + ratio kernel in repair mode
-    cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
-    cudaGraphExec_t gexec = nullptr;
+    cudaGraphExec_t gexec = nullptr;         // kept across run() calls, re-captured when gsig changes
+    struct GraphSig {                        // everything the captured launches carry by value
+        int algorithm, b_is_array; DevOpts o; Trace tr; double bconst[kMaxP];
+        bool fuse_ls, rl_fused; const void *k_conj, *k_mult, *truth;
+    } gsig;
+    const void *run_truth = nullptr;         // Eq.25: the true object of the current run (device pointer)
+    bool run_graph = true;                   // this run replays graphs (per-run use_graph bit 0)
+    bool rl_fused = true;                    // RL / OSEM on the four-launch schedule, else six launches
     long graph_launches = 0;                 // kernels in one replay of gexec
     // per-kernel timing (sgp_plan_set_profiling): one event pair per launch of the iteration loop
     struct ProfRec { int slot; cudaEvent_t a, b; };
@@ -55,9 +68,6 @@ template <typename T> struct PlanImpl : PlanBase {
         if (ev2) cudaEventDestroy(ev2);
         if (gexec) cudaGraphExecDestroy(gexec);
         if (cap_stream) cudaStreamDestroy(cap_stream);
-        if (cap_stream2) cudaStreamDestroy(cap_stream2);
-        if (ev_fork) cudaEventDestroy(ev_fork);
-        if (ev_join) cudaEventDestroy(ev_join);
         for (cudaEvent_t e : prof_pool) cudaEventDestroy(e);
     }
     cudaEvent_t prof_event()
@@ -93,7 +103,7 @@ template <typename T> struct PlanImpl : PlanBase {
     void free_trace()
     {
         cudaFree(trJ);      // one block: trJ, trA, trL, fA, fL, trR, trB
-        trJ = trA = trL = fA = fL = nullptr; trR = trB = nullptr; trace_cap = 0;
+        trJ = trA = trL = fA = fL = trE = nullptr; trR = trB = nullptr; trace_cap = 0;
     }
     // The workspace is ONE device allocation (a cudaMalloc / cudaFree pair costs ~0.5 ms and synchronises the device:
     // two dozen of them were a third of a one-shot call): dalloc() only records a request, commit_allocs() allocates
@@ -107,6 +117,17 @@ template <typename T> struct PlanImpl : PlanBase {
         reqs.push_back({reinterpret_cast<void **>(ptr), count * sizeof(U)});
         return SGP_OK;
     }
+    // per-problem arrays: one slab per problem (nb of them, identical layout); *ptr is problem 0's copy
+    std::vector<Req> reqs_pp;
+    template <typename U> int dalloc_pp(U **ptr, size_t count)
+    {
+        reqs_pp.push_back({reinterpret_cast<void **>(ptr), count * sizeof(U)});
+        return SGP_OK;
+    }
+    template <typename U> static U *bshift_host(U *ptr, size_t off)
+    {
+        return ptr ? reinterpret_cast<U *>(reinterpret_cast<unsigned char *>(const_cast<typename std::remove_const<U>::type *>(ptr)) + off) : ptr;
+    }
     int commit_allocs()
     {
         size_t total = 0;
@@ -118,6 +139,16 @@ template <typename T> struct PlanImpl : PlanBase {
         size_t off = 0;
         for (const Req &r : reqs) { *r.ptr = static_cast<unsigned char *>(raw) + off; off += (r.bytes + 255) & ~(size_t)255; }
         reqs.clear();
+        size_t per = 0;
+        for (const Req &r : reqs_pp) per += (r.bytes + 255) & ~(size_t)255;
+        void *raw_pp = nullptr;
+        SGP_CUDA_TRY(cudaMalloc(&raw_pp, per * (size_t)nb ? per * (size_t)nb : 256));
+        allocs.push_back(raw_pp);
+        bytes_allocated += per * (size_t)nb;
+        off = 0;
+        for (const Req &r : reqs_pp) { *r.ptr = static_cast<unsigned char *>(raw_pp) + off; off += (r.bytes + 255) & ~(size_t)255; }
+        reqs_pp.clear();
+        slab = nb > 1 ? per : 0;
         for (const Upload &u : uploads) SGP_CUDA_TRY(cudaMemcpy(*u.ptr, u.data.data(), u.data.size(), cudaMemcpyHostToDevice));
         uploads.clear();
         return SGP_OK;
@@ -140,11 +171,12 @@ template <typename T> struct PlanImpl : PlanBase {
         k_conj1 = get_col<T>(Lc, CM_CONJSUM, false, Cc); k_mult1 = get_col<T>(Lc, CM_MULT, false, Cc);
         if (!k_colf || !k_conj || !k_mult || !k_conj1 || !k_mult1) return SGP_ERR_ARG;
         G.C = Cc; G.RB = RB; G.lc = 0; while ((1 << G.lc) < Cc) G.lc++;
-        row_threads = RB * (Lr / Er);
+        row_threads = RB * group_threads(Lr / Er);
         col_threads = Cc * (Lc / Ec);
         nrb = ny / RB; ntiles = Lr / Cc;
-        row_smem = (size_t)RB * fft_padded_len(Lr, Er) * sizeof(C);
+        row_smem = ((size_t)RB * row_stride(Lr, Er) + row_table_entries<T>(Lr)) * sizeof(C);     // rows + twiddle tables (row_fwd.cuh)
         col_smem = ((size_t)Cc * fft_padded_len(Lc, Ec) + 2 * (size_t)Cc * Lc) * sizeof(C);
+        if (col_tw_in_smem<T>(Lc, Cc)) col_smem += (size_t)tw_total(Lc, Ec) * sizeof(C);      // pass tables in shared memory (col.cuh)
         if (row_threads > 256 || col_threads > 512 || row_smem > 227 * 1024 || col_smem > 227 * 1024) return SGP_ERR_ARG;
         for (int m = 0; m < RF_NMODES; ++m)
             SGP_CUDA_TRY(cudaFuncSetAttribute((const void *)k_rowf[m], cudaFuncAttributeMaxDynamicSharedMemorySize, (int)row_smem));
@@ -155,14 +187,9 @@ template <typename T> struct PlanImpl : PlanBase {
         SGP_CUDA_TRY(cudaFuncSetAttribute((const void *)k_mult, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)col_smem));
         SGP_CUDA_TRY(cudaFuncSetAttribute((const void *)k_conj1, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)col_smem));
         SGP_CUDA_TRY(cudaFuncSetAttribute((const void *)k_mult1, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)col_smem));
-        // grid of the backtracking kernel: all CTAs resident together (it synchronises grid-wide, aux.cuh)
-        int dev = 0, per_sm = 0;
+        int dev = 0;
         SGP_CUDA_TRY(cudaGetDevice(&dev));
         SGP_CUDA_TRY(cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev));
-        SGP_CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, backtrack_kernel<T>, 256, 0));
-        if (per_sm < 1) return SGP_ERR_CUDA;
-        if (per_sm > 4) per_sm = 4;
-        bt_grid = nsm * per_sm;
         // Fused or separate line-search / ratio kernels.  Separate, the ratio kernel re-reads g_j, q_j, u_j right after the
         // line-search kernel touched them: free while those 3p planes stay in L2 (2048^2 fp32 single image: 50 MB of
         // 126 MB; measured 7700 vs 7240 it/s), a second trip to HBM once they do not (3 x 2048^2, 4096^2, fp64: fused is
@@ -176,8 +203,6 @@ template <typename T> struct PlanImpl : PlanBase {
             if (opt.use_graph & 8) fuse_ls = true;
         }
         col_grid = (opt.use_graph & 2) ? (ntiles < nsm ? ntiles : nsm) : ntiles;   // experiment switch: persistent or one tile per CTA
-        size_t want = (n / vec4_of<T>::N + 255) / 256;
-        if ((size_t)bt_grid > want) bt_grid = (int)(want < 1 ? 1 : want);
 
         // twiddles, computed in double on the host
         std::vector<C> h;
@@ -187,7 +212,7 @@ template <typename T> struct PlanImpl : PlanBase {
                 double a = -2.0 * M_PI * (double)k / (double)len;
                 h[k].x = (T)cos(a); h[k].y = (T)sin(a);
             }
-            int r = dalloc(dst, (size_t)count);
+            int r = dalloc(dst, (size_t)count + 2);      // + padding: the kernels copy the tables in 16-byte pieces
             if (r) return r;
             const unsigned char *b = reinterpret_cast<const unsigned char *>(h.data());
             uploads.push_back({reinterpret_cast<void **>(dst), std::vector<unsigned char>(b, b + sizeof(C) * count)});
@@ -203,7 +228,7 @@ template <typename T> struct PlanImpl : PlanBase {
                         h[off + (r - 1) * NS + jm].x = (T)cos(a); h[off + (r - 1) * NS + jm].y = (T)sin(a);
                     }
             }
-            int r = dalloc(dst, h.size());
+            int r = dalloc(dst, h.size() + 2);
             if (r) return r;
             const unsigned char *b = reinterpret_cast<const unsigned char *>(h.data());
             uploads.push_back({reinterpret_cast<void **>(dst), std::vector<unsigned char>(b, b + sizeof(C) * h.size())});
@@ -217,7 +242,7 @@ template <typename T> struct PlanImpl : PlanBase {
         k_conj_run = k_conj; k_mult_run = k_mult;
         if (p == 1 && !(opt.use_graph & 16) && plan_ok(Lc, 32) && Cc * (Lc / 32) == 256) {
             col_kernel_t<T> c2 = get_col2<T>(Lc, CM_CONJSUM), m2 = get_col2<T>(Lc, CM_MULT);
-            const size_t sm2 = (size_t)Cc * fft_padded_len(Lc, 32) * sizeof(C);
+            const size_t sm2 = ((size_t)Cc * fft_padded_len(Lc, 32) + (SGP_TW_SMEM ? (size_t)tw_total(Lc, 32) : 0)) * sizeof(C);
             if (c2 && m2 && sm2 <= 113 * 1024) {
                 SGP_CUDA_TRY(cudaFuncSetAttribute((const void *)c2, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm2));
                 SGP_CUDA_TRY(cudaFuncSetAttribute((const void *)m2, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm2));
@@ -225,17 +250,17 @@ template <typename T> struct PlanImpl : PlanBase {
                 k_conj2 = c2; k_mult2 = m2; col2 = true; col2_threads = 256; col2_smem = sm2;
             }
         }
-        if ((rc = dalloc(&pack, (size_t)ny))) return rc;
+        if ((rc = dalloc_pp(&pack, (size_t)ny))) return rc;
         if ((rc = dalloc(&khat, nspec * p))) return rc;
         if ((rc = dalloc(&khatB, (size_t)ny * p))) return rc;
-        if ((rc = dalloc(&spec, nspec * p))) return rc;
-        if ((rc = dalloc(&Gp, n * p))) return rc;
-        if ((rc = dalloc(&Bp, n * p))) return rc;
-        if ((rc = dalloc(&q, 2 * n * p))) return rc;          // double-buffered (Ctrl::qsel)
-        if ((rc = dalloc(&u, n * p))) return rc;
-        if ((rc = dalloc(&f, n))) return rc;
-        if ((rc = dalloc(&grad, n))) return rc;
-        if ((rc = dalloc(&d, n))) return rc;
+        if ((rc = dalloc_pp(&spec, nspec * p))) return rc;
+        if ((rc = dalloc_pp(&Gp, n * p))) return rc;
+        if ((rc = dalloc_pp(&Bp, n * p))) return rc;
+        if ((rc = dalloc_pp(&q, 2 * n * p))) return rc;          // double-buffered (Ctrl::qsel)
+        if ((rc = dalloc_pp(&u, n * p))) return rc;
+        if ((rc = dalloc_pp(&f, n))) return rc;
+        if ((rc = dalloc_pp(&grad, n))) return rc;
+        if ((rc = dalloc_pp(&d, n))) return rc;
         if ((rc = dalloc(&scratch, n))) return rc;
         if (G.masked) {
             if ((rc = dalloc(&alphaR, n))) return rc;
@@ -243,14 +268,32 @@ template <typename T> struct PlanImpl : PlanBase {
             if ((rc = dalloc(&MR, n))) return rc;
             if ((rc = dalloc(&alphaJ, n * p))) return rc;
         }
-        if ((rc = dalloc(&part_bb, (size_t)nrb * 4))) return rc;
-        if ((rc = dalloc(&part_gd, (size_t)nrb))) return rc;
-        if ((rc = dalloc(&part_J, (size_t)nrb * p * 2))) return rc;
-        if ((rc = dalloc(&part_bt, (size_t)bt_grid))) return rc;
-        if ((rc = dalloc(&part_misc, (size_t)1024 * p))) return rc;
-        if ((rc = dalloc(&ct, (size_t)1))) return rc;
+        if ((rc = dalloc_pp(&part_bb, (size_t)nrb * 4))) return rc;
+        if ((rc = dalloc_pp(&part_gd, (size_t)nrb))) return rc;
+        if ((rc = dalloc_pp(&part_J, (size_t)nrb * p * 2))) return rc;
+        {   // one chunk per CTA of the ratio kernel (grid nrb x p), in whole batches
+            const size_t batch = bt_chunk_elems<T>(), total = (size_t)p * n, ctas = (size_t)nrb * p;
+            bt_batches = (total + batch * ctas - 1) / (batch * ctas);
+            if (bt_batches < 1) bt_batches = 1;
+            bt_chunks = (total + batch * bt_batches - 1) / (batch * bt_batches);
+        }
+        if ((rc = dalloc_pp(&part_bt, bt_chunks))) return rc;
+        if ((rc = dalloc_pp(&part_misc, (size_t)1024 * p))) return rc;
+        if ((rc = dalloc_pp(&ct, (size_t)1))) return rc;
+        if ((rc = dalloc_pp(&btinfo, (size_t)1))) return rc;
+        if ((rc = dalloc_pp(&btsync, (size_t)kBtSyncWords))) return rc;
+        if ((rc = dalloc(&fxsync, (size_t)kBtSyncWords))) return rc;
+        {   // flux-constrained projection (extra.cuh): about two chunks per SM and Newton step
+            const size_t batch = bt_chunk_elems<T>(), ctas = 2 * (size_t)nsm;
+            fx_batches = (n + batch * ctas - 1) / (batch * ctas);
+            if (fx_batches < 1) fx_batches = 1;
+            fx_chunks = (n + batch * fx_batches - 1) / (batch * fx_batches);
+        }
+        if ((rc = dalloc(&part_fx, 3 * fx_chunks))) return rc;
+        if ((rc = dalloc(&part_err, (size_t)2 * 1184))) return rc;
+        if ((rc = dalloc(&khatB_tmp, (size_t)ny))) return rc;
         if ((rc = commit_allocs())) return rc;
-        SGP_CUDA_TRY(cudaMemset(ct, 0, sizeof(Ctrl)));
+        for (int b = 0; b < nb; ++b) SGP_CUDA_TRY(cudaMemset(bshift_host(ct, (size_t)b * slab), 0, sizeof(Ctrl)));
         SGP_CUDA_TRY(cudaEventCreate(&ev0));
         SGP_CUDA_TRY(cudaEventCreate(&ev1));
         SGP_CUDA_TRY(cudaEventCreate(&ev2));
@@ -264,7 +307,7 @@ template <typename T> struct PlanImpl : PlanBase {
         memset(&P, 0, sizeof(P));
         P.G = G; P.ct = ct;
         P.plane = n; P.specplane = nspec; P.spec = spec; P.qbuf = n * (size_t)p;
-        P.tw = tw_r; P.twh = tw_h; P.alphaR = alphaR;
+        P.tw = tw_r; P.twh = tw_h; P.alphaR = alphaR; P.slab = lnb > 1 ? slab : 0; P.tr_slab = lnb > 1 ? tr_slab : 0;
         return P;
     }
     // launch with programmatic stream serialisation: the kernel may be scheduled while its predecessor drains and
@@ -286,23 +329,23 @@ template <typename T> struct PlanImpl : PlanBase {
     }
     int launch_row(row_kernel_t<T> k, const RowParams<T> &P, int images, cudaStream_t st)
     {
-        return launch_pdl(k, dim3(nrb, images), row_threads, row_smem, P, st);
+        return launch_pdl(k, dim3(nrb, images, lnb), row_threads, row_smem, P, st);
     }
     ColParams<T> col_params() const
     {
         ColParams<T> P;
         memset(&P, 0, sizeof(P));
         P.G = G; P.ct = ct; P.in = spec; P.out = spec; P.khat = khat; P.khatB = khatB;
-        P.specplane = nspec; P.tw = tw_c; P.pack = pack; P.p = p; P.ntiles = ntiles;
+        P.specplane = nspec; P.tw = tw_c; P.pack = pack; P.p = p; P.ntiles = ntiles; P.slab = lnb > 1 ? slab : 0;
         return P;
     }
     int launch_col(col_kernel_t<T> k, const ColParams<T> &P, cudaStream_t st)
     {
         if (col2 && (k == k_conj2 || k == k_mult2)) {     // one tile per CTA, its own pass tables
             ColParams<T> Q = P; Q.tw = tw_c2;
-            return launch_pdl(k, dim3(ntiles), col2_threads, col2_smem, Q, st);
+            return launch_pdl(k, dim3(ntiles, 1, lnb), col2_threads, col2_smem, Q, st);
         }
-        return launch_pdl(k, dim3(col_grid), col_threads, col_smem, P, st);
+        return launch_pdl(k, dim3(col_grid, 1, lnb), col_threads, col_smem, P, st);
     }
     static int ew_grid(size_t count) { size_t b = (count + 255) / 256; return (int)(b > 1184 ? 1184 : (b < 1 ? 1 : b)); }
 
@@ -443,10 +486,11 @@ template <typename T> struct PlanImpl : PlanBase {
 
     int run(int algorithm, const void *const *g, const void *const *b_arr, const double *b_const,
             const void *f0, void *f_out, const sgp_options *ropt, sgp_result *res, cudaStream_t st) override;
+    int run_batched(int algorithm, const void *const *g, const void *const *b_arr, const double *b_const,
+                    const void *const *f0, void *const *f_out, const sgp_options *ropt, sgp_result *res, cudaStream_t st) override;
     int ensure_trace(int max_iter, const sgp_result *res, Trace *tr, cudaStream_t st);
     int enqueue_sgp_iteration(const RowParams<T> &Pbase, const DevOpts &o, const Trace &tr, const double *bconst, int b_is_array, cudaStream_t st);
     int enqueue_ratio(const RowParams<T> &Pbase, int lazy, cudaStream_t st);
-    int enqueue_backtrack(const DevOpts &o, const Trace &tr, const double *bconst, int b_is_array, cudaStream_t st);
     int enqueue_rl_round(const DevOpts &o, const Trace &tr, const double *bconst, int b_is_array, cudaStream_t st);
     int enqueue_osem_cycle(const DevOpts &o, const Trace &tr, const double *bconst, int b_is_array, cudaStream_t st);
     int enqueue_many(int algorithm, int count, const RowParams<T> &Pb, const DevOpts &o, const Trace &tr, const double *bconst,

@@ -35,12 +35,13 @@ __device__ __forceinline__ void quad_in_S(const Geom &G, bool rowin, int x, bool
 // the four products of a pixel are summed over its quad in float (fma) and each quad sum is added to a double
 // accumulator (6 instructions per pixel less than converting every factor); double: everything in double.
 template <typename T, int L, int TF, bool MASKED>
-__device__ __forceinline__ void epi_grad(const RowParams<T> &P, const T *wrow, int t, size_t rowbase, double (&acc)[4])
+__device__ __forceinline__ void epi_grad(const RowParams<T> &P, const RowPtrs<T> &X, const T *wrow, int t, size_t rowbase, double (&acc)[4])
 {
     const Geom &G = P.G;
-    const int k = P.ct->k;
-    const T lam = (T)P.ct->lambda;
-    const T L1 = (T)P.ct->L1, L2 = (T)P.ct->L2;
+    const int k = X.ct->k;
+    const bool pend = X.ct->pending != 0;          // 0 after a refresh round (A21), which has already applied the step
+    const T lam = (T)X.ct->lambda;
+    const T L1 = (T)X.ct->L1, L2 = (T)X.ct->L2;
     const T pT = (T)G.p, Wc = (T)(1.0 / (double)G.p);
     constexpr int NIT = (L / 2) / TF;
     if (k == 0) {
@@ -57,7 +58,7 @@ __device__ __forceinline__ void epi_grad(const RowParams<T> &P, const T *wrow, i
 #pragma unroll
                 for (int c = 0; c < 4; ++c) g4.a[c] = pT - w4.a[c];
             }
-            stq<T>(P.out0 + rowbase + x, g4);
+            stq_if<T>(X.act, X.out0 + rowbase + x, g4);
         }
         return;
     }
@@ -69,9 +70,9 @@ __device__ __forceinline__ void epi_grad(const RowParams<T> &P, const T *wrow, i
 #pragma unroll
         for (int u = 0; u < U; ++u) {
             const int x = 4 * (t + TF * (it0 + u));
-            f4[u] = ldq<T>(P.in0 + rowbase + x);
-            d4[u] = ldq<T>(P.in1 + rowbase + x);
-            go4[u] = ldq<T>(P.out0 + rowbase + x);
+            f4[u] = ldq<T>(X.in0 + rowbase + x);
+            d4[u] = ldq<T>(X.in1 + rowbase + x);
+            go4[u] = ldq<T>(X.out0 + rowbase + x);
             if constexpr (MASKED) a4[u] = ldq<T>(P.alphaR + rowbase + x);
         }
 #pragma unroll
@@ -83,7 +84,7 @@ __device__ __forceinline__ void epi_grad(const RowParams<T> &P, const T *wrow, i
 #pragma unroll
             for (int c = 0; c < 4; ++c) {
                 const T s = lam * d4[u].a[c];
-                const T fn = f4[u].a[c] + s;
+                const T fn = pend ? f4[u].a[c] + s : f4[u].a[c];
                 f4[u].a[c] = fn;
                 bool inR = true;
                 T av = pT, wv = Wc;
@@ -104,37 +105,39 @@ __device__ __forceinline__ void epi_grad(const RowParams<T> &P, const T *wrow, i
 #pragma unroll
                 for (int k4 = 0; k4 < 4; ++k4) acc[k4] += (double)pq[k4];
             }
-            stq<T>(P.out1 + rowbase + x, f4[u]);
-            stq<T>(P.out0 + rowbase + x, g4);
+            stq_if<T>(X.act, X.out1 + rowbase + x, f4[u]);
+            stq_if<T>(X.act, X.out0 + rowbase + x, g4);
         }
     }
 }
 
 // RI_LS (a8 tail + a9): u_j = A_j d on S; J(1) = sum kl(g_j, q_j + u_j + b_j).
 // RI_QJ: q_j = A_j f on S; J0(f) = sum kl(g_j, q_j + b_j) (Eq.2/12 over S, A12); QJ_PLAIN only stores.
-// SPEC (RI_LSF): besides u_j and J(1), the step lambda = 1 is applied speculatively: q_j + u_j goes to the other q
-// buffer (qout) and the ratio r_j = g_j / (q_j + u_j + b_j) of the NEXT iteration (a1) replaces the row in shared
-// memory (wmut), from where the caller transforms it -- if the Armijo test then accepts lambda = 1 (the usual
-// case) the next iteration needs no ratio kernel at all.
-template <typename T, int L, int TF, bool WITH_Q, bool MASKED, bool SPEC>
-__device__ __forceinline__ void epi_kl(const RowParams<T> &P, const T *wrow, T *wmut, const T *qin, T *qout, int t, int y, int j,
+// RATIO: besides that, the ratio r_j = g_j / (y_j + b_j) of the step that follows (a1) replaces the row in shared memory
+// (wmut), from where the caller transforms it:
+//   RI_LSF (WITH_Q, STORE_ROW, STORE_Q): the step lambda = 1 is applied speculatively -- q_j + u_j goes to the other q
+//     buffer (qout); if the Armijo test then accepts lambda = 1 (the usual case) the next iteration needs no ratio kernel;
+//   RI_QJF (RL / OSEM, SURVEY.md 8(d) "RL schedule": row C2R -> ratio -> row R2C in one kernel): A_j f is used for J0 and
+//     the ratio and never stored.
+template <typename T, int L, int TF, bool WITH_Q, bool MASKED, bool RATIO, bool STORE_ROW, bool STORE_Q>
+__device__ __forceinline__ void epi_kl(const RowParams<T> &P, const RowPtrs<T> &X, const T *wrow, T *wmut, const T *qin, T *qout, T *rowout, int t, int y, int j,
                                        size_t base, bool plain, double (&acc)[1])
 {
     const Geom &G = P.G;
-    const T bc = (T)P.bconst[j];
+    const T bc = (T)(P.slab ? X.ct->bconst[j] : P.bconst[j]);
     const bool rowin = (unsigned)(y - G.oy) < (unsigned)G.sy;
     constexpr int NIT = (L / 2) / TF;
     constexpr int U = batch_len_kl<T>(NIT);
-    const bool need = rowin && !plain;
+    const bool need = rowin && (!plain || RATIO);
     for (int it0 = 0; it0 < NIT; it0 += U) {
         Quad<T> g4[U], q4[U], b4[U];
 #pragma unroll
         for (int u = 0; u < U; ++u) {
             const int x = 4 * (t + TF * (it0 + u));
             if (need) {
-                g4[u] = ldq<T>(P.in0 + base + x);
+                g4[u] = ldq<T>(X.in0 + base + x);
                 if constexpr (WITH_Q) q4[u] = ldq<T>(qin + base + x);
-                if (P.b_is_array) b4[u] = ldq<T>(P.in2 + base + x);
+                if (P.b_is_array) b4[u] = ldq<T>(X.in2 + base + x);
             }
         }
 #pragma unroll
@@ -146,7 +149,7 @@ __device__ __forceinline__ void epi_kl(const RowParams<T> &P, const T *wrow, T *
             Quad<T> u4;
 #pragma unroll
             for (int c = 0; c < 4; ++c) u4.a[c] = s[c] ? w4.a[c] : (T)0;
-            stq<T>(P.out0 + base + x, u4);
+            if constexpr (STORE_ROW) stq_if<T>(X.act, rowout + base + x, u4);
             Quad<T> r4;
 #pragma unroll
             for (int c = 0; c < 4; ++c) r4.a[c] = (T)0;
@@ -157,28 +160,28 @@ __device__ __forceinline__ void epi_kl(const RowParams<T> &P, const T *wrow, T *
                     yv[c] = u4.a[c];
                     if constexpr (WITH_Q) yv[c] += q4[u].a[c];
                 }
-                if constexpr (SPEC) {
+                if constexpr (STORE_Q) {
                     Quad<T> q1;
 #pragma unroll
                     for (int c = 0; c < 4; ++c) q1.a[c] = yv[c];
-                    stq<T>(qout + base + x, q1);
+                    stq_if<T>(X.act, qout + base + x, q1);
                 }
 #pragma unroll
                 for (int c = 0; c < 4; ++c) yv[c] += P.b_is_array ? b4[u].a[c] : bc;
-                acc[0] += (double)kl_quad(g4[u].a, yv, s);
-                if constexpr (SPEC) {
+                if (!plain) acc[0] += (double)kl_quad(g4[u].a, yv, s);
+                if constexpr (RATIO) {
 #pragma unroll
                     for (int c = 0; c < 4; ++c) r4.a[c] = s[c] ? ratio_term(g4[u].a[c], yv[c]) : (T)0;
                 }
             }
-            if constexpr (SPEC) stq<T>(wmut + x, r4);
+            if constexpr (RATIO) stq<T>(wmut + x, r4);
         }
     }
 }
 
 // plain store with the output mask of Eq.16 (M_S) or Eq.17 (M_R)
 template <typename T, int L, int TF, bool MK>
-__device__ __forceinline__ void epi_store(const RowParams<T> &P, const T *wrow, int t, int y, size_t rowbase, size_t base)
+__device__ __forceinline__ void epi_store(const RowParams<T> &P, const RowPtrs<T> &X, const T *wrow, int t, int y, size_t rowbase, size_t base)
 {
     const Geom &G = P.G;
     const bool rowin = (unsigned)(y - G.oy) < (unsigned)G.sy;
@@ -197,14 +200,20 @@ __device__ __forceinline__ void epi_store(const RowParams<T> &P, const T *wrow, 
 #pragma unroll
             for (int c = 0; c < 4; ++c) if (!(a4.a[c] > (T)0)) w4.a[c] = (T)0;
         }
-        stq<T>(P.out0 + base + x, w4);
+        if (P.submode == RIP_STORE_POS) {
+#pragma unroll
+            for (int c = 0; c < 4; ++c) w4.a[c] = w4.a[c] > (T)0 ? w4.a[c] : (T)0;
+        }
+        stq_if<T>(X.act, X.out0 + base + x, w4);
     }
 }
 
 // y = (M_R/alpha) f w: one RL step (Eq.1/13/21).  STORE: write it (a12); else accumulate (-min positive, max) for
 // the adaptive bounds (A19).
-template <typename T, int L, int TF, bool STORE, bool MK>
-__device__ __forceinline__ void epi_rl(const RowParams<T> &P, const T *wrow, int t, size_t rowbase, double (&acc)[2])
+// FUSE (RI_RLUPF, SURVEY.md 8(d) "RL schedule": row C2R -> f update -> row R2C of the new f in one kernel): the new f also
+// replaces the row in shared memory (wmut), from where the caller transforms it for the next round.
+template <typename T, int L, int TF, bool STORE, bool MK, bool FUSE = false>
+__device__ __forceinline__ void epi_rl(const RowParams<T> &P, const RowPtrs<T> &X, const T *wrow, int t, size_t rowbase, double (&acc)[2], T *wmut = nullptr)
 {
     const Geom &G = P.G;
     const T Wc = (T)(1.0 / (double)G.p);
@@ -220,7 +229,7 @@ __device__ __forceinline__ void epi_rl(const RowParams<T> &P, const T *wrow, int
         for (int u = 0; u < U; ++u) {
             const int x = 4 * (t + TF * (it0 + u));
             w4[u] = ldq<T>(wrow + x);
-            f4[u] = ldq<T>(P.in0 + rowbase + x);
+            f4[u] = ldq<T>(X.in0 + rowbase + x);
             if (MK) a4[u] = ldq<T>(P.alphaR + rowbase + x);
         }
 #pragma unroll
@@ -240,7 +249,8 @@ __device__ __forceinline__ void epi_rl(const RowParams<T> &P, const T *wrow, int
                     acc[1] = fmax(acc[1], yd);
                 }
             }
-            if constexpr (STORE) stq<T>(P.out0 + rowbase + x, y4);
+            if constexpr (STORE) stq_if<T>(X.act, X.out0 + rowbase + x, y4);
+            if constexpr (FUSE) stq<T>(wmut + x, y4);
         }
     }
 }

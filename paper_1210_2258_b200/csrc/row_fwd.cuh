@@ -7,6 +7,7 @@
 // threads, dynamic smem = RB * padded(L) complex.
 #pragma once
 #include "ew.cuh"
+#include "aux.cuh"
 
 namespace sgpk {
 
@@ -14,6 +15,35 @@ namespace sgpk {
 template <typename T> __host__ __device__ constexpr int fwd_batch(int E)
 {
     return sizeof(T) == 8 ? (E % 4 == 0 ? 4 : 2) : (E % 8 == 0 ? 8 : 4);
+}
+
+// Shared-memory copies of the twiddle tables of a row kernel (fft_core.cuh: SGP_TW_SMEM), behind the rows' lines:
+// the pass tables of the length-L complex FFT and exp(-2 pi i k/nx), k <= L/2, of the real<->complex step.  The copy is
+// asynchronous (cp.async, 16 bytes per request, no registers): issued at the start of the kernel, awaited before the
+// first use.  Counts are rounded up to even numbers (the device tables are allocated with that padding).
+__host__ __device__ constexpr int even_up(int n) { return (n + 1) & ~1; }
+template <typename T> __host__ __device__ constexpr size_t row_table_entries(int L)
+{
+    return SGP_TW_SMEM ? (size_t)even_up(tw_total(L, fft_E<T>(L))) + (size_t)even_up(L / 2 + 1) : 0;
+}
+template <typename T, int L>
+__device__ __forceinline__ void row_tables_issue(cx<T> *tw_s, const RowParams<T> &P, int tid, int nthr)
+{
+    constexpr int E = fft_E<T>(L);
+    constexpr int N1 = even_up(tw_total(L, E)), N2 = even_up(L / 2 + 1);
+    constexpr int per16 = 16 / (int)sizeof(cx<T>);               // complex numbers per 16-byte request: 2 (float) or 1 (double)
+    const unsigned int s1 = (unsigned int)__cvta_generic_to_shared(tw_s), s2 = (unsigned int)__cvta_generic_to_shared(tw_s + N1);
+    for (int i = tid; i < N1 / per16; i += nthr)
+        asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"(s1 + 16u * i), "l"(reinterpret_cast<const char *>(P.tw) + 16 * (size_t)i) : "memory");
+    for (int i = tid; i < N2 / per16; i += nthr)
+        asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"(s2 + 16u * i), "l"(reinterpret_cast<const char *>(P.twh) + 16 * (size_t)i) : "memory");
+    asm volatile("cp.async.commit_group;" ::: "memory");
+}
+// all threads of the CTA: the tables have landed and are visible
+__device__ __forceinline__ void row_tables_wait()
+{
+    asm volatile("cp.async.wait_all;" ::: "memory");
+    __syncthreads();
 }
 
 // untangling of one (k, L-k) pair: a = Z[k], zb = Z[L-k], w = exp(-2 pi i k/nx):
@@ -30,16 +60,17 @@ template <typename T> __device__ __forceinline__ void untangle(cx<T> a, cx<T> zb
 
 // Forward transform of one row held as v[e] = (x[2m], x[2m+1]), m = t + TF e, by the TF threads of the row, and
 // store of its half spectrum (tile-major).  Shared by the forward row kernel and the fused line-search kernel.
-template <typename T, int L, typename SYNC>
+// tw / twh: the tables, in shared memory when TWS
+template <typename T, int L, bool TWS, typename SYNC>
 __device__ __forceinline__ void fwd_fft_store(cx<T> (&v)[fft_E<T>(L)], cx<T> *smrow, const int t, const SYNC &sync,
-                                              const RowParams<T> &P, const int y, const int j)
+                                              const RowParams<T> &P, const RowPtrs<T> &X, const int y, const int j, const cx<T> *tw, const cx<T> *twh)
 {
     using C = cx<T>;
     constexpr int E = fft_E<T>(L);
     constexpr int TF = L / E;
     const Geom &G = P.G;
     // ---- complex FFT of length L = nx/2 over z[m] = x[2m] + i x[2m+1]
-    fft_block<T, L, E, -1>(v, smrow, 1, t, P.tw, sync);
+    fft_block<T, L, E, -1, TWS>(v, smrow, 1, t, tw, sync);
     sync();
 #pragma unroll
     for (int e = 0; e < E; ++e) smrow[fft_pad<E>(t + TF * e)] = v[e];
@@ -48,17 +79,15 @@ __device__ __forceinline__ void fwd_fft_store(cx<T> (&v)[fft_E<T>(L)], cx<T> *sm
     // ---- untangle the two interleaved real transforms, one (k, L-k) pair per step, and store tile-major:
     //      E = (Z[k] + conj Z[L-k])/2, O = -i (Z[k] - conj Z[L-k])/2, w = exp(-2 pi i k/nx):
     //      X[k] = E + w O,  X[L-k] = conj(E - w O);  entry 0 = (X[0], X[L]) packed;  X[L/2] = conj Z[L/2]
-    C *dst = P.spec + (size_t)j * P.specplane;
+    C *dst = X.spec + (size_t)j * P.specplane;
     {   // i = 0
         const C a = smrow[fft_pad<E>(t)];
         if (t == 0) {
-            dst[spec_index(G, y, 0)] = mk<T>(a.x + a.y, a.x - a.y);
-            dst[spec_index(G, y, L / 2)] = cconj(smrow[fft_pad<E>(L / 2)]);
+            if (X.act) { dst[spec_index(G, y, 0)] = mk<T>(a.x + a.y, a.x - a.y); dst[spec_index(G, y, L / 2)] = cconj(smrow[fft_pad<E>(L / 2)]); }
         } else {
             C xk, xlk;
-            untangle<T>(a, smrow[fft_pad<E>(L - t)], __ldg(&P.twh[t]), xk, xlk);
-            dst[spec_index(G, y, t)] = xk;
-            dst[spec_index(G, y, L - t)] = xlk;
+            untangle<T>(a, smrow[fft_pad<E>(L - t)], TWS ? twh[t] : __ldg(&twh[t]), xk, xlk);
+            if (X.act) { dst[spec_index(G, y, t)] = xk; dst[spec_index(G, y, L - t)] = xlk; }
         }
     }
     if ((TF & (G.C - 1)) == 0) {
@@ -70,18 +99,16 @@ __device__ __forceinline__ void fwd_fft_store(cx<T> (&v)[fft_E<T>(L)], cx<T> *sm
         for (int i = 1; i < E / 2; ++i) {
             const int k = t + TF * i;
             C xk, xlk;
-            untangle<T>(smrow[fft_pad<E>(k)], smrow[fft_pad<E>(L - k)], __ldg(&P.twh[k]), xk, xlk);
-            pa[(size_t)i * stride] = xk;
-            *(pb - (size_t)i * stride) = xlk;
+            untangle<T>(smrow[fft_pad<E>(k)], smrow[fft_pad<E>(L - k)], TWS ? twh[k] : __ldg(&twh[k]), xk, xlk);
+            if (X.act) { pa[(size_t)i * stride] = xk; *(pb - (size_t)i * stride) = xlk; }
         }
     } else {
 #pragma unroll 4
         for (int i = 1; i < E / 2; ++i) {
             const int k = t + TF * i;
             C xk, xlk;
-            untangle<T>(smrow[fft_pad<E>(k)], smrow[fft_pad<E>(L - k)], __ldg(&P.twh[k]), xk, xlk);
-            dst[spec_index(G, y, k)] = xk;
-            dst[spec_index(G, y, L - k)] = xlk;
+            untangle<T>(smrow[fft_pad<E>(k)], smrow[fft_pad<E>(L - k)], TWS ? twh[k] : __ldg(&twh[k]), xk, xlk);
+            if (X.act) { dst[spec_index(G, y, k)] = xk; dst[spec_index(G, y, L - k)] = xlk; }
         }
     }
 }
@@ -94,28 +121,37 @@ __global__ void __launch_bounds__(256, 2) row_fwd_kernel(const RowParams<T> P)
     using C = cx<T>;
     constexpr int E = fft_E<T>(L);
     constexpr int TF = L / E;
-    constexpr int RS = fft_padded_len(L, E);
+    constexpr int RS = row_stride(L, E);
     extern __shared__ __align__(16) unsigned char smem_raw[];
     C *sm = reinterpret_cast<C *>(smem_raw);
     pdl_trigger();
     pdl_wait();
+    RowPtrs<T> X = row_ptrs(P);                                  // this problem's arrays (batched plans: blockIdx.z)
     // the stop flag is tested only before the first store, so that its load overlaps the loads of the row
-    const int stop = P.check_status ? P.ct->status : 0;
+    const int stop = P.check_status ? X.ct->status : 0;
 
     const Geom &G = P.G;
     const int tid = threadIdx.x;
-    const int row = tid / TF, t = tid - row * TF;
+    constexpr int TFP = group_threads(TF);                       // threads per row incl. padding lanes (5-smooth lengths)
+    const int row = tid / TFP, traw = tid - row * TFP;
+    const bool act = TFP == TF ? true : traw < TF;
+    const int t = TFP == TF ? traw : (traw < TF ? traw : TF - 1);
+    X.act = act;
     const int y = blockIdx.x * G.RB + row;
     const int j = blockIdx.y;
     constexpr int nx = 2 * L;
     C v[E];
     float accf = 0.f;
     double acc[1] = {0.0};
+    constexpr bool TWS = SGP_TW_SMEM != 0;
+    C *tw_s = sm + (size_t)G.RB * RS;                            // shared-memory copies of the twiddle tables, behind the rows
+    if constexpr (TWS && MODE != RF_RATIO) row_tables_issue<T, L>(tw_s, P, tid, (int)blockDim.x);
 
     // ---- load stage with the fused elementwise work
     if constexpr (MODE == RF_PLAIN) {
+        if (P.lazy == 4 && X.ct->refresh_due == 0) return;          // refresh round (A21): only after every n-th iteration
         // plain rows, optionally multiplied by M_S (input of A^T, Eq.17) or M_R (input of A, Eq.16)
-        const T *src = P.in0 + (size_t)j * P.plane + (size_t)y * nx;
+        const T *src = X.in0 + (size_t)j * P.plane + (size_t)y * nx;
         const bool rowin = (unsigned)(y - G.oy) < (unsigned)G.sy;
 #pragma unroll
         for (int e = 0; e < E; ++e) {
@@ -134,8 +170,8 @@ __global__ void __launch_bounds__(256, 2) row_fwd_kernel(const RowParams<T> P)
     } else if constexpr (MODE == RF_SETUP) {
         if (P.submode == RFS_PSF) {
             // K_j normalised to unit volume and circularly shifted so that its centre sits at (0,0) (A18)
-            const T *src = P.in0 + (size_t)j * P.plane;
-            const T inv = (T)(1.0 / P.ct->psf_sum);
+            const T *src = X.in0 + (size_t)j * P.plane;
+            const T inv = (T)(1.0 / X.ct->psf_sum);
             int ys = y + P.cy; if (ys >= G.ny) ys -= G.ny;
 #pragma unroll
             for (int e = 0; e < E; ++e) {
@@ -156,24 +192,28 @@ __global__ void __launch_bounds__(256, 2) row_fwd_kernel(const RowParams<T> P)
         // already formed q(k+1), the ratio and this very spectrum), 1 = ratio of the current q (first iteration),
         // 2 = a10 after a backtrack: q(k+1) = q(k) + lambda u_j into the other buffer, then the ratio.
         const size_t base = (size_t)j * P.plane + (size_t)y * nx;
-        const T bc = (T)P.bconst[j];
+        const T bc = (T)(P.slab ? X.ct->bconst[j] : P.bconst[j]);      // batched plans: per-problem backgrounds live in the control block
         const bool rowin = (unsigned)(y - G.oy) < (unsigned)G.sy;
         int todo = 1, sel = 0;
+        T lam = (T)1;
         if (P.lazy) {
-            // Two instances of this kernel follow the line-search kernel (plan_run.inl): lazy = 1 runs BESIDE the
-            // backtracking kernel and works only if lambda = 1 was accepted (Ctrl::accepted is written by the line-search
-            // kernel alone, so it is stable here; nothing else of the control block is read before this test, because the
-            // backtracking kernel rewrites it when it has work); lazy = 2 runs BEHIND the backtracking kernel and works
-            // only if that had to find lambda < 1; lazy = 3 (plain stream order) takes either case.
-            const int acc = P.ct->accepted;
-            if ((P.lazy == 1 && acc == 0) || (P.lazy == 2 && acc != 0)) return;
-            if (P.ct->status != 0) return;
-            todo = P.ct->need_k1; if (todo == 0) return; sel = P.ct->qsel;
+            // SGP loop.  This kernel follows the line-search kernel K6.  If K6 rejected lambda = 1, the Armijo backtracking
+            // (a9 for lambda < 1, elementwise on q_j + lambda u_j) runs here first, by all CTAs of the grid
+            // (aux.cuh: backtrack_rounds); it ends with the book-keeping of the accepted step (finish_iteration).
+            Ctrl *ct = X.ct;
+            if (ct->status != 0) return;
+#ifndef SGP_NO_BT
+            if (P.lazy == 1 && ct->accepted == 0) backtrack_rounds<T>(static_cast<const BtInfo<T> *>(X.btinfo));
+#endif
+            // the control block as the accepted step left it (written by another CTA: read past the L1)
+            if (__ldcg(&ct->status) != 0) return;
+            todo = __ldcg(&ct->need_k1); if (todo == 0) return; sel = __ldcg(&ct->qsel);
+            lam = (T)__ldcg(&ct->lambda);
         }
+        if constexpr (TWS) row_tables_issue<T, L>(tw_s, P, tid, (int)blockDim.x);      // after the early returns above
         const bool pend = todo == 2;
-        const T *qsrc = P.in1 + (size_t)(pend ? sel ^ 1 : sel) * P.qbuf;
-        T *qdst = P.out0 + (size_t)sel * P.qbuf;
-        const T lam = (T)P.ct->lambda;
+        const T *qsrc = X.in1 + (size_t)(pend ? sel ^ 1 : sel) * P.qbuf;
+        T *qdst = X.out0 + (size_t)sel * P.qbuf;
         // loads of a batch are issued before its stores (q is updated in place: the compiler would otherwise
         // serialise every load behind the previous store)
         constexpr int U = fwd_batch<T>(E);
@@ -184,10 +224,10 @@ __global__ void __launch_bounds__(256, 2) row_fwd_kernel(const RowParams<T> P)
 #pragma unroll
                 for (int u = 0; u < U; ++u) {
                     const int x0 = 2 * (t + TF * (e0 + u));
-                    g2[u] = ld2<T>(P.in0 + base + x0);
+                    g2[u] = ld2<T>(X.in0 + base + x0);
                     q2[u] = ld2<T>(qsrc + base + x0);
-                    if (pend) u2[u] = ld2<T>(P.in3 + base + x0);
-                    b2[u] = P.b_is_array ? ld2<T>(P.in2 + base + x0) : mk<T>(bc, bc);
+                    if (pend) u2[u] = ld2<T>(X.in3 + base + x0);
+                    b2[u] = P.b_is_array ? ld2<T>(X.in2 + base + x0) : mk<T>(bc, bc);
                 }
             }
             if (e0 == 0 && stop != 0) return;
@@ -199,7 +239,7 @@ __global__ void __launch_bounds__(256, 2) row_fwd_kernel(const RowParams<T> P)
                     C qn = q2[u];
                     if (pend) {
                         qn.x = qn.x + lam * u2[u].x; qn.y = qn.y + lam * u2[u].y;
-                        st2<T>(qdst + base + x0, qn);
+                        st2_if<T>(X.act, qdst + base + x0, qn);
                     }
                     if ((unsigned)(x0 - G.ox) < (unsigned)G.sx)     r.x = ratio_term(g2[u].x, qn.x + b2[u].x);
                     if ((unsigned)(x0 + 1 - G.ox) < (unsigned)G.sx) r.y = ratio_term(g2[u].y, qn.y + b2[u].y);
@@ -218,7 +258,7 @@ __global__ void __launch_bounds__(256, 2) row_fwd_kernel(const RowParams<T> P)
         {
             constexpr int CH = (int)(L * sizeof(C) / 16) / TF;    // 16-byte chunks per thread
             const unsigned int sdst = (unsigned int)__cvta_generic_to_shared(frow);
-            const char *gsrc = reinterpret_cast<const char *>(P.in0 + base);
+            const char *gsrc = reinterpret_cast<const char *>(X.in0 + base);
 #pragma unroll
             for (int i = 0; i < CH; ++i) {
                 const int ch = t + TF * i;
@@ -227,11 +267,13 @@ __global__ void __launch_bounds__(256, 2) row_fwd_kernel(const RowParams<T> P)
             asm volatile("cp.async.commit_group;" ::: "memory");
         }
 #pragma unroll
-        for (int e = 0; e < E; ++e) v[e] = ld2<T>(P.in1 + base + 2 * (t + TF * e));
-        const T alpha = (T)P.ct->alpha, L1 = (T)P.ct->L1, L2 = (T)P.ct->L2;
+        for (int e = 0; e < E; ++e) v[e] = ld2<T>(X.in1 + base + 2 * (t + TF * e));
+        const T alpha = (T)X.ct->alpha, L1 = (T)X.ct->L1, L2 = (T)X.ct->L2;
         const T Wc = (T)(1.0 / (double)G.p);
+        // flux-constrained projection (Bonettini et al. 2009): y = max(0, x - mu D), mu from flux_mu_kernel
+        const T mu = P.o.flux_constraint ? (T)X.ct->mu : (T)0;
         asm volatile("cp.async.wait_group 0;" ::: "memory");
-        const SyncGroup<TF> rsync{1 + row};
+        const SyncGroup<TFP> rsync{1 + row};
         rsync();                                                  // the copies of all threads of the row have landed
         if (stop != 0) return;
         constexpr int U = fwd_batch<T>(E);
@@ -256,9 +298,11 @@ __global__ void __launch_bounds__(256, 2) row_fwd_kernel(const RowParams<T> P)
                 {
                     T D = w2.x * clipT<T>(f2.x, L1, L2);
                     T yv = f2.x - alpha * D * g2.x;
+                    if (P.o.flux_constraint) yv = yv - mu * D;
                     d2.x = r0 ? ((yv > (T)0 ? yv : (T)0) - f2.x) : (T)0;
                     D = w2.y * clipT<T>(f2.y, L1, L2);
                     yv = f2.y - alpha * D * g2.y;
+                    if (P.o.flux_constraint) yv = yv - mu * D;
                     d2.y = r1 ? ((yv > (T)0 ? yv : (T)0) - f2.y) : (T)0;
                 }
                 if constexpr (sizeof(T) == 4) {
@@ -267,22 +311,24 @@ __global__ void __launch_bounds__(256, 2) row_fwd_kernel(const RowParams<T> P)
                 } else {
                     acc[0] += (double)g2.x * (double)d2.x + (double)g2.y * (double)d2.y;
                 }
-                st2<T>(P.out0 + base + x0, d2);
+                st2_if<T>(X.act, X.out0 + base + x0, d2);
                 v[e0 + u] = d2;
             }
         }
         acc[0] += (double)accf;
+        if (!act) acc[0] = 0.0;                                   // padding lanes repeat lane TF - 1: not twice in the sum
     }
 
     if (stop != 0) return;
     C *smrow = sm + row * RS;
-    const SyncGroup<TF> sync{1 + row};
-    fwd_fft_store<T, L>(v, smrow, t, sync, P, y, j);
+    const SyncGroup<TFP> sync{1 + row};
+    if constexpr (TWS) row_tables_wait();
+    fwd_fft_store<T, L, TWS>(v, smrow, t, sync, P, X, y, j, TWS ? tw_s : P.tw, TWS ? tw_s + even_up(tw_total(L, E)) : P.twh);
 
     if constexpr (MODE == RF_PROJECT) {
         __shared__ double red[32];
         block_reduce_sum<1>(acc, red);
-        if (tid == 0) P.part[blockIdx.x] = acc[0];
+        if (tid == 0) X.part[blockIdx.x] = acc[0];
     }
 }
 

@@ -25,27 +25,39 @@ __global__ void __launch_bounds__(256, 2) row_inv_kernel(const RowParams<T> P)
     using C = cx<T>;
     constexpr int E = fft_E<T>(L);
     constexpr int TF = L / E;
-    constexpr int RS = fft_padded_len(L, E);
+    constexpr int RS = row_stride(L, E);
     extern __shared__ __align__(16) unsigned char smem_raw[];
     __shared__ double red[kNQ * 32];
     C *sm = reinterpret_cast<C *>(smem_raw);
     pdl_trigger();
     pdl_wait();
+    RowPtrs<T> X = row_ptrs(P);                                  // this problem's arrays (batched plans: blockIdx.z)
     // the stop flag is tested only after the loads of the spectrum have been issued (all stores come later)
-    const int stop = P.check_status ? P.ct->status : 0;
+    const int stop = P.check_status ? X.ct->status : 0;
+    if constexpr (MODE == RI_QJ) { if (P.submode == QJ_REFRESH && X.ct->refresh_due == 0) return; }      // A21: only after every n-th iteration
 
     const Geom &G = P.G;
     const int tid = threadIdx.x;
-    const int row = tid / TF, t = tid - row * TF;
+    constexpr int TFP = group_threads(TF);                       // threads per row incl. padding lanes (5-smooth lengths)
+    const int row = tid / TFP, traw = tid - row * TFP;
+    const bool act = TFP == TF ? true : traw < TF;
+    const int t = TFP == TF ? traw : (traw < TF ? traw : TF - 1);
+    X.act = act;
     const int y = blockIdx.x * G.RB + row;
     const int j = blockIdx.y;
     constexpr int nx = 2 * L;
     C *smrow = sm + row * RS;
-    const SyncGroup<TF> sync{1 + row};
+    const SyncGroup<TFP> sync{1 + row};
+    // twiddle tables in shared memory (row_fwd.cuh): wanted from the inverse transform on; the re-tangling below, which
+    // starts at once, reads exp(-2 pi i k/nx) from global memory
+    constexpr bool TWS = SGP_TW_SMEM != 0;
+    C *tw_s = sm + (size_t)G.RB * RS;
+    const C *tw = TWS ? tw_s : P.tw, *twh = TWS ? tw_s + even_up(tw_total(L, E)) : P.twh;
+    if constexpr (TWS) { if (stop == 0) row_tables_issue<T, L>(tw_s, P, tid, (int)blockDim.x); }
     // ---- tile-major spectrum -> re-tangled Z in shared memory, one (k, L-k) pair per step, k = t + TF i;
     //      Z[0] = (X0 + XL) + i (X0 - XL);  Z[L/2] = 2 conj X[L/2]
     {
-        const C *src = P.spec + (size_t)j * P.specplane;
+        const C *src = X.spec + (size_t)j * P.specplane;
         {   // i = 0
             const C a = src[spec_index(G, y, t)];
             if (t == 0) {
@@ -84,12 +96,12 @@ __global__ void __launch_bounds__(256, 2) row_inv_kernel(const RowParams<T> P)
         }
     }
     if (stop != 0) return;
-    sync();
+    if constexpr (TWS) row_tables_wait(); else sync();
     {
         C v[E];
 #pragma unroll
         for (int e = 0; e < E; ++e) v[e] = smrow[fft_pad<E>(t + TF * e)];
-        fft_block<T, L, E, +1>(v, smrow, 1, t, P.tw, sync);
+        fft_block<T, L, E, +1, TWS>(v, smrow, 1, t, tw, sync);
         // park the row (w(y, 2m), w(y, 2m+1)), m = t + TF e, in natural order (no padding) for the epilogue
         sync();
 #pragma unroll
@@ -104,12 +116,12 @@ __global__ void __launch_bounds__(256, 2) row_inv_kernel(const RowParams<T> P)
     const int bid = blockIdx.y * gridDim.x + blockIdx.x;
 
     if constexpr (MODE == RI_PLAIN) {
-        if (P.submode == RIP_STORE) {
-            epi_store<T, L, TF, MK>(P, wrow, t, y, rowbase, base);
+        if (P.submode == RIP_STORE || P.submode == RIP_STORE_POS) {
+            epi_store<T, L, TF, MK>(P, X, wrow, t, y, rowbase, base);
         } else {
             // RIP_RLMINMAX: adaptive bounds from one RL step (A19)
             double acc[2] = {-INFINITY, -INFINITY};   // (-min positive, max)
-            epi_rl<T, L, TF, false, MK>(P, wrow, t, rowbase, acc);
+            epi_rl<T, L, TF, false, MK>(P, X, wrow, t, rowbase, acc);
             // max-reduction over the block (fixed tree)
             const int lane = tid & 31, wid = tid >> 5, nw = (blockDim.x + 31) >> 5;
 #pragma unroll
@@ -123,69 +135,87 @@ __global__ void __launch_bounds__(256, 2) row_inv_kernel(const RowParams<T> P)
                 for (int q = 0; q < 2; ++q) { double m = red[q * 32]; for (int w = 1; w < nw; ++w) m = fmax(m, red[q * 32 + w]); acc[q] = m; }
             }
             __syncthreads();
-            if (publish_partials<2>(acc, P.part, bid, nblk, &P.ct->counter[TK_MINMAX])) {
+            if (publish_partials<2>(acc, X.part, bid, nblk, &X.ct->counter[TK_MINMAX])) {
                 if (tid == 0) {
                     double mn = -INFINITY, mx = -INFINITY;
-                    for (unsigned int b = 0; b < nblk; ++b) { mn = fmax(mn, __ldcg(&P.part[2 * b])); mx = fmax(mx, __ldcg(&P.part[2 * b + 1])); }
+                    for (unsigned int b = 0; b < nblk; ++b) { mn = fmax(mn, __ldcg(&X.part[2 * b])); mx = fmax(mx, __ldcg(&X.part[2 * b + 1])); }
                     const double ymin = -mn, ymax = mx;
-                    if (!(ymin < INFINITY) || !(ymax > 0.0)) P.ct->status = SGP_ERR_DATA;
-                    else if (ymax / ymin < 50.0) { P.ct->L1 = ymin / 10.0; P.ct->L2 = ymax * 10.0; }
-                    else                         { P.ct->L1 = ymin;        P.ct->L2 = ymax; }
+                    if (!(ymin < INFINITY) || !(ymax > 0.0)) X.ct->status = SGP_ERR_DATA;
+                    else if (ymax / ymin < 50.0) { X.ct->L1 = ymin / 10.0; X.ct->L2 = ymax * 10.0; }
+                    else                         { X.ct->L1 = ymin;        X.ct->L2 = ymax; }
                 }
             }
         }
     } else if constexpr (MODE == RI_GRAD) {
         double acc[4] = {0.0, 0.0, 0.0, 0.0};
-        epi_grad<T, L, TF, MK>(P, wrow, t, rowbase, acc);
+        epi_grad<T, L, TF, MK>(P, X, wrow, t, rowbase, acc);
+        if (!act) { acc[0] = 0.0; acc[1] = 0.0; acc[2] = 0.0; acc[3] = 0.0; }     // padding lanes repeat lane TF - 1
         block_reduce_sum<4>(acc, red);
-        if (publish_partials<4>(acc, P.part, bid, nblk, &P.ct->counter[TK_GRAD])) {
-            final_sum<4>(acc, P.part, nblk, red);
-            if (tid == 0) { P.ct->pending = 0; bb_step(P.ct, P.o, P.tr, acc[0], acc[1], acc[2], acc[3]); }   // a6
+        if (publish_partials<4>(acc, X.part, bid, nblk, &X.ct->counter[TK_GRAD])) {
+            final_sum<4>(acc, X.part, nblk, red);
+            if (tid == 0) { X.ct->pending = 0; bb_step(X.ct, P.o, X.tr, acc[0], acc[1], acc[2], acc[3]); }   // a6
         }
-    } else if constexpr (MODE == RI_LS || MODE == RI_QJ || MODE == RI_LSF) {
+    } else if constexpr (MODE == RI_LS || MODE == RI_QJ || MODE == RI_LSF || MODE == RI_QJF) {
         constexpr bool LS = (MODE == RI_LS || MODE == RI_LSF), SPEC = (MODE == RI_LSF);
-        const bool plain = (MODE == RI_QJ) && P.submode == QJ_PLAIN;
+        constexpr bool RATIO = (MODE == RI_LSF || MODE == RI_QJF);
+        const bool plain = (MODE == RI_QJ || MODE == RI_QJF) && P.submode == QJ_PLAIN;
         double acc[1] = {0.0};
         // SGP loop: q is double-buffered; this kernel reads buffer qsel and (SPEC) writes q + u into the other one
-        const int sel = LS ? P.ct->qsel : 0;
-        const T *qin = P.in1 + (size_t)sel * P.qbuf;
-        T *qout = SPEC ? const_cast<T *>(P.in1) + (size_t)(sel ^ 1) * P.qbuf : nullptr;
+        const int sel = LS ? X.ct->qsel : 0;
+        const T *qin = X.in1 + (size_t)sel * P.qbuf;
+        T *qout = SPEC ? const_cast<T *>(X.in1) + (size_t)(sel ^ 1) * P.qbuf : nullptr;
         T *wmut = reinterpret_cast<T *>(smrow);
-        epi_kl<T, L, TF, LS, MK, SPEC>(P, wrow, wmut, qin, qout, t, y, j, base, plain, acc);
-        if (plain) return;
+        // where the row itself goes: u_j (SGP), q_j (set-up, RL); the refresh round (A21) rewrites the current q buffer
+        T *rowout = X.out0;
+        if (MODE == RI_QJ && P.submode == QJ_REFRESH) rowout += (size_t)X.ct->qsel * P.qbuf;
+        epi_kl<T, L, TF, LS, MK, RATIO, MODE != RI_QJF, SPEC>(P, X, wrow, wmut, qin, qout, rowout, t, y, j, base, plain, acc);
+        if (!act) acc[0] = 0.0;                                    // padding lanes repeat lane TF - 1
+        if (!plain) {
         block_reduce_sum<1>(acc, red);
         const int tk = LS ? TK_LS : TK_QJ;
-        if (publish_partials<1>(acc, P.part, bid, nblk, &P.ct->counter[tk])) {
-            final_sum<1>(acc, P.part, nblk, red);
+        if (publish_partials<1>(acc, X.part, bid, nblk, &X.ct->counter[tk])) {
+            final_sum<1>(acc, X.part, nblk, red);
             const double J = acc[0];
-            Ctrl *ct = P.ct;
+            Ctrl *ct = X.ct;
             if constexpr (LS) {
                 double gd[1];
-                final_sum<1>(gd, P.part2, gridDim.x, red);     // grad'd partials of the projection kernel
+                final_sum<1>(gd, X.part2, gridDim.x, red);     // grad'd partials of the projection kernel
                 if (tid == 0) {
                     // Alg.1 step 5 at lambda = 1: J(f + d) <= J_ref + beta * 1 * grad'd
                     const double Jref = armijo_ref(ct);
                     ct->gd = gd[0]; ct->Jref = Jref; ct->Jtrial = J;
                     int acc1 = (isfinite(J) && J <= Jref + P.o.beta * gd[0]) ? 1 : 0;
-                    if (P.tr.force_lambda) {
-                        const double fl = P.tr.force_lambda[ct->k];
+                    if (X.tr.force_lambda) {
+                        const double fl = X.tr.force_lambda[ct->k];
                         if (isfinite(fl)) acc1 = (fl == 1.0) ? 1 : 0;
                     }
                     ct->accepted = acc1;
+                    // re-arm the backtracking prologue of the ratio kernel that follows (aux.cuh: backtrack_rounds)
+                    if (X.btsync) { X.btsync[kBtNext] = 0; X.btsync[kBtDone] = 0; X.btsync[kBtDecided] = 0; X.btsync[kBtFinal] = 0; }
+                    if (!acc1 && P.o.max_backtracks < 1 && !X.tr.force_lambda) { ct->status = SGP_ERR_LINESEARCH; ct->accepted = 1; }   // A16
                     // a10 (book-keeping; f is updated lazily by K3), a11.  SPEC: q(k+1) and the ratio spectrum are
                     // already in place, so the ratio kernel of the next iteration has nothing to do.
-                    if (acc1) finish_iteration(ct, P.o, P.tr, 1.0, J, 0, SPEC ? 0 : 2);
+                    if (acc1) finish_iteration(ct, P.o, X.tr, 1.0, J, 0, SPEC ? 0 : 2);
                 }
             } else if (tid == 0) {
                 if (P.submode == QJ_INIT) {
                     ct->J = J; ct->Jhist[0] = J; ct->nJ = 1;
-                    if (P.tr.J) P.tr.J[0] = J;
+                    if (X.tr.J) X.tr.J[0] = J;
                     if (!isfinite(J)) ct->status = SGP_ERR_NONFINITE;
+                } else if (P.submode == QJ_REFRESH) {
+                    // A21: J0(f(k)) recomputed from f replaces the value carried by q + lambda u; the stopping rules that
+                    // finish_iteration left to this kernel
+                    const int k = ct->k;
+                    ct->J = J; ct->Jhist[k % P.o.armijo_memory] = J;
+                    if (X.tr.J) X.tr.J[k] = J;
+                    ct->refresh_due = 0;
+                    if (!isfinite(J)) ct->status = SGP_ERR_NONFINITE;
+                    else { int r = stop_test(P.o, k, J, ct->Jprev, true); if (r) ct->status = r; }
                 } else {   // QJ_RL: J0(f(k)) and the stopping rules before the k-th RL update
                     const int k = ct->k;
                     const double Jold = ct->J;
                     ct->J = J;
-                    if (P.tr.J) P.tr.J[k] = J;
+                    if (X.tr.J) X.tr.J[k] = J;
                     if (!isfinite(J)) ct->status = SGP_ERR_NONFINITE;
                     else {
                         int r = stop_test(P.o, k, J, Jold, k > 0);
@@ -194,18 +224,27 @@ __global__ void __launch_bounds__(256, 2) row_inv_kernel(const RowParams<T> P)
                 }
             }
         }
-        if constexpr (SPEC) {
-            // a1 of the next iteration, speculating on lambda = 1: forward row transform of the ratio parked in shared
+        }   // !plain
+        if constexpr (RATIO) {
+            // a1 of the next step (SGP: speculating on lambda = 1): forward row transform of the ratio parked in shared
             // memory by the epilogue; the spectrum row this warp read at the top is overwritten in place
             C v[E];
             sync();
 #pragma unroll
             for (int e = 0; e < E; ++e) v[e] = smrow[t + TF * e];
-            fwd_fft_store<T, L>(v, smrow, t, sync, P, y, j);
+            fwd_fft_store<T, L, TWS>(v, smrow, t, sync, P, X, y, j, tw, twh);
         }
-    } else {   // RI_RLUPDATE, a12: f <- (M_R/alpha) o f o sum_j A_j^T(g_j/(A_j f + b_j))   (Eq.1/13/21)
+    } else if constexpr (MODE == RI_RLUPDATE) {   // a12: f <- (M_R/alpha) o f o sum_j A_j^T(g_j/(A_j f + b_j))   (Eq.1/13/21)
         double dummy[2];
-        epi_rl<T, L, TF, true, MK>(P, wrow, t, rowbase, dummy);
+        epi_rl<T, L, TF, true, MK>(P, X, wrow, t, rowbase, dummy);
+    } else {   // RI_RLUPF: a12 and the forward row transform of the new f (the first pass of A_j f of the next round)
+        double dummy[2];
+        epi_rl<T, L, TF, true, MK, true>(P, X, wrow, t, rowbase, dummy, reinterpret_cast<T *>(smrow));
+        C v[E];
+        sync();
+#pragma unroll
+        for (int e = 0; e < E; ++e) v[e] = smrow[t + TF * e];
+        fwd_fft_store<T, L, TWS>(v, smrow, t, sync, P, X, y, 0, tw, twh);
     }
 }
 

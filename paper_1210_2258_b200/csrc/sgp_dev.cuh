@@ -15,6 +15,8 @@ constexpr int kNQ = 4;            // partial sums per block (max over the kernel
 struct DevOpts {
     double beta, theta, alpha0, alpha_min, alpha_max, tol, disc_threshold;
     int m_alpha, alt_start, armijo_memory, max_iter, stop_rule, max_backtracks, adaptive_L, p;
+    int flux_constraint;       // 1: projection on { f >= 0, sum f = c } (extra.cuh)
+    int refresh_every;         // A21: recompute A f from f after every n-th iteration (0 = never)
     double nS_total;   // p * #S, the denominator of Eq.26
     double rl_relax;   // RL: exponent of the multiplicative relaxation, Eq.3; 1 = plain RL
     double rl_linear;  // RL: constant lambda_k of the linear relaxation, Eq.4; 1 = plain RL
@@ -46,6 +48,19 @@ struct Ctrl {
     double ring[SGP_MAX_MALPHA];
     double Jhist[SGP_MAX_ARMIJO_MEMORY];
     unsigned int counter[8];   // "last block done" tickets, one per kernel family
+    unsigned long long nfft;   // 2-D transforms executed by the column kernels since the run started (n_fft2)
+    double Jprev;              // J0(f(k-1)): restored when the Eq.25 rule discards the last step
+    int nbt_last;              // backtracks of the last accepted step (same purpose)
+    double err, err_trial;     // Eq.25: rho(k) of the current iterate / of the candidate f(k) + lambda d
+    double flux_c, mu;         // flux constraint: c and the multiplier of the current projection
+    int refresh_due;           // 1: the step just accepted is followed by a recomputation of A f (refresh_every)
+    int need_k1_next;          // refresh round: what the second instance of the ratio kernel has to do
+    int err_pending;           // Eq.25: the error of the step just accepted has not been evaluated yet
+    int commit;                // RL with the Eq.25 rule: adopt the candidate update
+    int flux_rounds;           // Newton steps of the last flux-constrained projection
+    double flux_cnt;           // active pixels of the previous Newton step
+    double tmp_sum;            // scratch of the set-up kernels
+    double bconst[SGP_MAX_IMAGES];   // batched plans: the background constants of this problem
 };
 
 // optional per-iteration traces (device arrays of max_iter+1 entries) and forced steps (test-only)
@@ -53,6 +68,7 @@ struct Trace {
     double *J, *alpha, *lambda;
     int *rule, *backtracks;
     const double *force_alpha, *force_lambda;
+    double *err;               // Eq.25: rho(k), max_iter + 2 entries (nullptr without a true object)
 };
 
 // geometry shared by all kernels of a plan
@@ -134,7 +150,9 @@ __device__ inline void finish_iteration(Ctrl *ct, const DevOpts &o, const Trace 
     if (tr.backtracks) tr.backtracks[k] = nbt;
     if (tr.J) tr.J[k + 1] = Jnew;
     ct->total_backtracks += nbt;
+    ct->nbt_last = nbt;
     const double Jold = ct->J;
+    ct->Jprev = Jold;
     ct->J = Jnew;
     ct->lambda = lambda;
     ct->pending = 1;
@@ -143,6 +161,10 @@ __device__ inline void finish_iteration(Ctrl *ct, const DevOpts &o, const Trace 
     ct->Jhist[(k + 1) % o.armijo_memory] = Jnew;
     if (ct->nJ < o.armijo_memory) ct->nJ++;
     ct->k = k + 1;
+    ct->err_pending = 1;
+    // A21: after every refresh_every-th iteration A_j f and J0 are recomputed from f; the stopping rules then see the
+    // recomputed J0 (extra.cuh / row_inv.cuh QJ_REFRESH), so the test is left to that kernel
+    if (o.refresh_every > 0 && (k + 1) % o.refresh_every == 0) { ct->refresh_due = 1; return; }
     int r = stop_test(o, k + 1, Jnew, Jold, true);
     if (r) ct->status = r;
 }

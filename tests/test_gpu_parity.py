@@ -52,7 +52,7 @@ def gpu_plan(w, dt, **optkw):
 
 def oracle_opts(w, **optkw):
     kw = {**w["opts"], **optkw}
-    kw = {k: v for k, v in kw.items() if k not in ("check_every", "tile_cols", "rows_per_block", "use_graph", "backend")}
+    kw = {k: v for k, v in kw.items() if k not in ("check_every", "tile_cols", "rows_per_block", "use_graph")}
     return oracle.default_options(**kw)
 
 
