@@ -370,6 +370,36 @@ def measure_other(name: str, alg_name: str, steps: int, dev, peak: float):
             "fused_linesearch": int(r.fused_linesearch)}
 
 
+def measure_batched(nb: int, steps: int, dev):
+    """nb problems of the C0 recipe (256^2, different seeds) through ONE batched plan (every kernel launched
+    once for all problems, blockIdx.z = problem) beside one C0 problem through an ordinary plan: aggregate iterations/s"""
+    import torch
+    from paper_1210_2258_b200 import binding as B, synth
+    ws = [synth.c0_stars_gaussian(256, seed_idx=200 + i) for i in range(nb)]
+    to_dev = lambda a: torch.as_tensor(np.ascontiguousarray(a, dtype=np.float32), device=dev)
+    opts = B.default_options(**ws[0]["opts"])
+    out = {}
+    for label, n_ in (("single", 1), ("batched", nb)):
+        plan = B.BatchedPlan(n_, [to_dev(ws[0]["psf"][0])], opts=opts)
+        g = [[to_dev(w["g"][0])] for w in ws[:n_]]
+        b = [[10.0]] * n_
+        for _ in range(3):
+            _, rs = plan.run_batched(B.ALG_SGP, g, b, opts=opts)
+        ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize(); ev0.record()
+        its = 0
+        for _ in range(steps):
+            _, rs = plan.run_batched(B.ALG_SGP, g, b, opts=opts)
+            its += sum(r.iterations for r in rs)
+        ev1.record(); torch.cuda.synchronize()
+        plan.close()
+        out[label] = {"problems": n_, "value": its / (ev0.elapsed_time(ev1) * 1e-3), "unit": "iterations/s (sum over the problems)",
+                      "ms_per_step": ev0.elapsed_time(ev1) / steps, "iterations_per_problem": rs[0].iterations}
+    out["aggregate_speedup"] = out["batched"]["value"] / out["single"]["value"]
+    out["workload"] = f"C0 recipe, 256x256 fp32, 100 SGP iterations per problem, {nb} problems in one sgp_plan_run_batched call vs 1"
+    return out
+
+
 def run_ours(args):
     import torch
     import torch.distributed as dist
@@ -562,6 +592,13 @@ def run_ours(args):
             except Exception as e:
                 others.append({"workload": nm, "algorithm": al, "error": f"{type(e).__name__}: {e}"})
 
+    batched = None
+    if rank == 0 and world == 1 and not args.no_others and args.workload == "C4c" and args.alg == "sgp" and args.dtype == "f32":
+        try:
+            batched = measure_batched(64, 3, dev)
+        except Exception as e:
+            batched = {"error": f"{type(e).__name__}: {e}"}
+
     if rank == 0:
         line = {"metric": "SGP iterations/s" if args.alg == "sgp" else "RL iterations/s", "value": value, "unit": "iterations/s",
                 "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms / args.steps,
@@ -575,7 +612,7 @@ def run_ours(args):
                            "J0_final": J_final, "backtracks": backtracks // args.steps,
                            "fused_linesearch": int(r.fused_linesearch)},
                 "clocks": clk.summary(), "e2e": e2e, "gpu_launches": launches, "roofline": roofline, "cpu_baseline": cpu,
-                "cufft_compare": cufft, "other_workloads": others}
+                "cufft_compare": cufft, "other_workloads": others, "batched_small_grids": batched}
         print(json.dumps(line))
     plan.close()
     if world > 1:

@@ -79,7 +79,7 @@ __device__ __noinline__ void backtrack_rounds(const BtInfo<T> *__restrict__ I)
             for (;;) {
                 if (ld_volatile_u32(&P.sync[kBtFinal]) != 0u) { st = 1; break; }
                 if (ld_volatile_u32(&P.sync[kBtDecided]) >= trial) break;
-                __nanosleep(300);
+                __nanosleep(100);
             }
             __threadfence();
             s_state = st;

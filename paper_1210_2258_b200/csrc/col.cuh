@@ -13,26 +13,13 @@
 //   CM_MULT   : out_j = IFFTcol( K^_j o FFTcol(in) ), j < p              (a8: A_j d, Eq.16)
 // Column 0 of tile 0 carries the packed pair (kx = 0, kx = nx/2): with C~[ky] = conj(C[-ky]) the product is
 //   C'[ky] = A[ky] C[ky] + B[ky] C~[ky],  A = (K0 + KM)/2 (stored in column 0 of khat), B = (K0 - KM)/2 (khatB).
-// The partner values C[-ky] of that one column go through a small global scratch line (pack, L entries).
+// The partner values C[-ky] of that one column go through a small global scratch line (P.pack, L entries).
 #pragma once
 #include "ew.cuh"
 
 namespace sgpk {
 
 enum ColMode { CM_FWD = 0, CM_CONJSUM = 1, CM_MULT = 2, CM_INV = 3 };
-
-#ifndef SGP_COL_SPLIT
-#define SGP_COL_SPLIT 0     // measured at 2048^2 (round 2): K2 / K5 27.9 / 24.9 us split against 23.0 / 21.1 us as one group -- off
-#endif
-// all threads of the CTA, or the N threads of one column group (named barrier `id`)
-template <bool GROUP, int N> struct ColSync {
-    int id;
-    __device__ __forceinline__ void operator()() const
-    {
-        if constexpr (GROUP) asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(N) : "memory");
-        else __syncthreads();
-    }
-};
 
 // Bulk asynchronous copy global -> shared by the TMA engine (cp.async.bulk, SASS UBLKCP): ONE instruction of one
 // thread moves a whole tile (contiguous in the tile-major layout); completion is signalled on an mbarrier.
@@ -57,12 +44,15 @@ __device__ __forceinline__ void mbar_wait(unsigned long long *bar, unsigned int 
 }
 
 // per-CTA view of the work: tile it of this CTA starts at tile_of(it) in a spectrum plane
-template <typename T, int L, int E> struct ColCtx {
+template <typename T, int L, int E, bool BATCH> struct ColCtx {
     using C = cx<T>;
     int tid, nthr, t, c, Cc;
     size_t tile_len;
+    size_t zoff;                      // batched plans: offset (in complex numbers) of problem blockIdx.z's spectra behind problem 0's
     C *smc, *bufA, *bufB;
-    __device__ __forceinline__ size_t tile_of(int it) const { return (size_t)((int)blockIdx.x + it * (int)gridDim.x) * tile_len; }
+    // tile `it` of this CTA in the shared transfer function / in this problem's spectra
+    __device__ __forceinline__ size_t ktile_of(int it) const { return (size_t)((int)blockIdx.x + it * (int)gridDim.x) * tile_len; }
+    __device__ __forceinline__ size_t tile_of(int it) const { if constexpr (BATCH) return zoff + ktile_of(it); else return ktile_of(it); }
 };
 
 // product with the packed-column companion B (see the header): r[e] (+)= conj?(B) C~
@@ -90,39 +80,28 @@ template <typename T> __host__ __device__ constexpr int col_default_C(int L)
     return C;
 }
 
-// the pass tables join the exchange buffer and the landing zones in shared memory where all of it fits (fft_core.cuh)
-template <typename T> __host__ __device__ constexpr bool col_tw_in_smem(int L, int Cc)
-{
-    const int E = fft_E_col<T>(L);
-    return SGP_TW_SMEM && Cc > 0 &&
-           ((size_t)Cc * fft_padded_len(L, E) + 2 * (size_t)Cc * L + (size_t)tw_total(L, E)) * sizeof(cx<T>) <= (size_t)227 * 1024;
-}
-
-template <typename T, int L, int MODE, bool MULTI, int CT>
+// BATCH: a batched plan (blockIdx.z = problem, ew.cuh).  A template parameter because the product kernels sit exactly at
+// their register limit: the two registers of a run-time batch offset made them spill (K2 at 3 x 2048^2: 39 -> 52 us).
+template <typename T, int L, int MODE, bool MULTI, int CT, bool BATCH>
 __device__ __forceinline__ void col_body(const ColParams<T> &P)
 {
     using C = cx<T>;
     constexpr int E = fft_E_col<T>(L);
     constexpr int TF = L / E;
-    constexpr bool TWS = (MODE == CM_CONJSUM || MODE == CM_MULT) && col_tw_in_smem<T>(L, CT);
     extern __shared__ __align__(16) unsigned char smem_raw[];
     C *sm = reinterpret_cast<C *>(smem_raw);
     pdl_trigger();
-    // batched plans: problem blockIdx.z works on its own spectra, scratch line and control block (ew.cuh: bshift)
-    const size_t boff = (size_t)blockIdx.z * P.slab;
-    const C *Pin = bshift(P.in, boff);
-    C *Pout = bshift(P.out, boff);
-    Ctrl *Pct = bshift(P.ct, boff);
 
-    ColCtx<T, L, E> X;
+    ColCtx<T, L, E, BATCH> X;
     X.Cc = CT > 0 ? CT : P.G.C; X.tid = threadIdx.x; X.nthr = CT > 0 ? CT * TF : (int)blockDim.x;
     X.t = X.tid / X.Cc; X.c = X.tid - X.t * X.Cc;
     X.tile_len = (size_t)L * X.Cc;
+    if constexpr (BATCH) X.zoff = (size_t)blockIdx.z * (P.slab / sizeof(C));      // batched plans (ew.cuh)
     X.smc = sm + X.c;
     X.bufA = sm + (size_t)X.Cc * fft_padded_len(L, E);     // landing zone of the spectrum tile
     X.bufB = X.bufA + X.tile_len;                          // landing zone of the transfer-function tile
-    const int tid = X.tid, nthr = X.nthr, Cc = X.Cc;
-    volatile C *pack = bshift(P.pack, boff);
+    const int tid = X.tid, nthr = X.nthr, t = X.t, Cc = X.Cc;
+    volatile C *pack = (BATCH ? bshift(P.pack, (size_t)blockIdx.z * P.slab) : P.pack);
     const SyncBlock sync;
     const int ntiles = P.ntiles;
     C v[E];
@@ -130,28 +109,15 @@ __device__ __forceinline__ void col_body(const ColParams<T> &P)
     if constexpr (MODE == CM_FWD || MODE == CM_INV) {
         pdl_wait();
         for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
-            const size_t tbase = (size_t)tile * X.tile_len + tid;
+            const size_t tbase = (BATCH ? X.zoff : 0) + (size_t)tile * X.tile_len + tid;
 #pragma unroll
-            for (int e = 0; e < E; ++e) v[e] = Pin[tbase + (size_t)e * nthr];
-            fft_block<T, L, E, (MODE == CM_FWD ? -1 : +1)>(v, X.smc, Cc, X.t, P.tw, sync);
+            for (int e = 0; e < E; ++e) v[e] = P.in[tbase + (size_t)e * nthr];
+            fft_block<T, L, E, (MODE == CM_FWD ? -1 : +1)>(v, X.smc, Cc, t, P.tw, sync);
 #pragma unroll
-            for (int e = 0; e < E; ++e) Pout[tbase + (size_t)e * nthr] = v[e];
+            for (int e = 0; e < E; ++e) P.out[tbase + (size_t)e * nthr] = v[e];
         }
         return;
     }
-    // SPLIT (SGP_COL_SPLIT, product modes compiled for their tile width): the CTA works as TWO groups of CT/2 columns, each with its
-    // own exchange buffer and its own named barrier.  The passes of a column FFT alternate between butterflies (FMA pipe) and
-    // exchanges (shared-memory pipe) with a barrier in between, so with ONE group per SM the two pipes are never busy together;
-    // two groups drift apart and overlap one's exchange with the other's butterflies.
-    constexpr bool SPLIT = SGP_COL_SPLIT && CT >= 2 && ((CT / 2) * TF) % 32 == 0;
-    constexpr int Cg = SPLIT ? CT / 2 : 1, GN = Cg * TF;
-    const int grp = SPLIT ? tid / GN : 0, lt = SPLIT ? tid - grp * GN : tid;
-    const int t = SPLIT ? lt / Cg : X.t;
-    const int cloc = SPLIT ? grp * Cg + (lt - t * Cg) : X.c;          // column of this thread inside the tile
-    const int lin = SPLIT ? t * CT + cloc : tid;                        // its element of "row" t of the tile (+ e * nthr for the others)
-    C *smc = SPLIT ? sm + (size_t)grp * Cg * fft_padded_len(L, E) + (lt - t * Cg) : X.smc;
-    const int cs = SPLIT ? Cg : Cc;
-    const ColSync<SPLIT, GN> gsync{1 + grp};
     const int p = MULTI ? P.p : 1;
     const int my_tiles = ((int)blockIdx.x < ntiles) ? (ntiles - 1 - (int)blockIdx.x) / (int)gridDim.x + 1 : 0;
     if (my_tiles == 0) return;
@@ -164,18 +130,17 @@ __device__ __forceinline__ void col_body(const ColParams<T> &P)
         mbar_init(&bars[0], 1); mbar_init(&bars[1], 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
         // the transfer function does not depend on the previous kernel: it is on its way before we wait for that
-        bulk_load(X.bufB, P.khat + X.tile_of(0), tile_bytes, &bars[1]);
+        bulk_load(X.bufB, P.khat + X.ktile_of(0), tile_bytes, &bars[1]);
     }
     pdl_wait();
-    // check_status = 2: an instance of the refresh round (A21), which runs only after every n-th iteration
-    const int stop = P.check_status ? (Pct->status != 0 || (P.check_status == 2 && Pct->refresh_due == 0)) : 0;
-    if (tid == 0 && stop == 0) bulk_load(X.bufA, Pin + X.tile_of(0), tile_bytes, &bars[0]);
-    C *tw_s = X.bufB + X.tile_len;
-    if constexpr (TWS) { if (stop == 0) copy_table_to_smem(tw_s, P.tw, tw_total(L, E), tid, nthr); }
-    const C *tw = TWS ? tw_s : P.tw;
-    __syncthreads();                                            // barrier initialisation (and the tables) visible to all
+    // (The transforms are counted by the inverse row kernel that follows every column pass, and this test is kept as simple
+    // as it is: anything more in this kernel keeps the compiler from hoisting the first twiddle loads above the wait for
+    // the tile -- K2 / K5 45 instead of 39 us at 3 x 2048^2.  The refresh round of reading A21 passes a shadow control block
+    // whose status says "not this iteration".)
+    const int stop = P.check_status ? (BATCH ? bshift(P.ct, (size_t)blockIdx.z * P.slab) : P.ct)->status : 0;
+    if (tid == 0 && stop == 0) bulk_load(X.bufA, P.in + X.tile_of(0), tile_bytes, &bars[0]);
+    __syncthreads();                                            // barrier initialisation visible to all
     if (stop != 0) { mbar_wait(&bars[1], 0); return; }
-    if (P.count_fft && blockIdx.x == 0 && tid == 0) atomicAdd(&Pct->nfft, (unsigned long long)(p + 1));   // p + 1 two-dimensional transforms pass through this launch
 
     if constexpr (MODE == CM_CONJSUM) {
         // unit of work u = it*p + j: spectrum and transfer function of image j on this CTA's it-th tile
@@ -183,17 +148,17 @@ __device__ __forceinline__ void col_body(const ColParams<T> &P)
         C acc[MULTI ? E : 1];
         for (int it = 0; it < my_tiles; ++it) {
             const bool packed = (blockIdx.x == 0 && it == 0);      // tile 0 holds the packed column
-            const bool pk = packed && cloc == 0;
+            const bool pk = packed && X.c == 0;
             for (int j = 0; j < p; ++j) {
                 const int u1 = it * p + j + 1, it1 = u1 / p, j1 = u1 - it1 * p;
                 mbar_wait(&bars[0], phA); phA ^= 1;                 // spectrum of this unit has landed
 #pragma unroll
-                for (int e = 0; e < E; ++e) v[e] = X.bufA[lin + e * nthr];
+                for (int e = 0; e < E; ++e) v[e] = X.bufA[tid + e * nthr];
                 if (u1 < units) {
                     __syncthreads();
-                    if (tid == 0) bulk_load(X.bufA, Pin + (size_t)j1 * P.specplane + X.tile_of(it1), tile_bytes, &bars[0]);
+                    if (tid == 0) bulk_load(X.bufA, P.in + (size_t)j1 * P.specplane + X.tile_of(it1), tile_bytes, &bars[0]);
                 }
-                fft_block<T, L, E, -1, TWS>(v, smc, cs, t, tw, gsync);
+                fft_block<T, L, E, -1>(v, X.smc, Cc, t, P.tw, sync);
                 if (packed) {
                     if (pk) {
 #pragma unroll
@@ -203,10 +168,10 @@ __device__ __forceinline__ void col_body(const ColParams<T> &P)
                 }
                 mbar_wait(&bars[1], phB); phB ^= 1;                 // transfer function of this unit has landed
 #pragma unroll
-                for (int e = 0; e < E; ++e) v[e] = cmulc(v[e], X.bufB[lin + e * nthr]);
+                for (int e = 0; e < E; ++e) v[e] = cmulc(v[e], X.bufB[tid + e * nthr]);
                 if (u1 < units) {
                     __syncthreads();
-                    if (tid == 0) bulk_load(X.bufB, P.khat + (size_t)j1 * P.specplane + X.tile_of(it1), tile_bytes, &bars[1]);
+                    if (tid == 0) bulk_load(X.bufB, P.khat + (size_t)j1 * P.specplane + X.ktile_of(it1), tile_bytes, &bars[1]);
                 }
                 if (pk) packed_fix<T, L, E, true>(v, pack, P.khatB + (size_t)j * L, t);
                 if constexpr (MULTI) {
@@ -219,23 +184,23 @@ __device__ __forceinline__ void col_body(const ColParams<T> &P)
 #pragma unroll
                 for (int e = 0; e < E; ++e) v[e] = acc[e];
             }
-            fft_block<T, L, E, +1, TWS>(v, smc, cs, t, tw, gsync);
-            C *dst = Pout + X.tile_of(it) + lin;
+            fft_block<T, L, E, +1>(v, X.smc, Cc, t, P.tw, sync);
+            C *dst = P.out + X.tile_of(it) + tid;
 #pragma unroll
             for (int e = 0; e < E; ++e) dst[(size_t)e * nthr] = v[e];
         }
     } else {   // CM_MULT
         for (int it = 0; it < my_tiles; ++it) {
             const bool packed = (blockIdx.x == 0 && it == 0);
-            const bool pk = packed && cloc == 0;
+            const bool pk = packed && X.c == 0;
             mbar_wait(&bars[0], phA); phA ^= 1;                     // spectrum of tile it has landed
 #pragma unroll
-            for (int e = 0; e < E; ++e) v[e] = X.bufA[lin + e * nthr];
+            for (int e = 0; e < E; ++e) v[e] = X.bufA[tid + e * nthr];
             if (it + 1 < my_tiles) {
                 __syncthreads();
-                if (tid == 0) bulk_load(X.bufA, Pin + X.tile_of(it + 1), tile_bytes, &bars[0]);
+                if (tid == 0) bulk_load(X.bufA, P.in + X.tile_of(it + 1), tile_bytes, &bars[0]);
             }
-            fft_block<T, L, E, -1, TWS>(v, smc, cs, t, tw, gsync);
+            fft_block<T, L, E, -1>(v, X.smc, Cc, t, P.tw, sync);
             if (packed) {
                 if (pk) {
 #pragma unroll
@@ -247,17 +212,17 @@ __device__ __forceinline__ void col_body(const ColParams<T> &P)
                 C w[E];
                 mbar_wait(&bars[1], phB); phB ^= 1;                 // transfer function (it, j) has landed
 #pragma unroll
-                for (int e = 0; e < E; ++e) w[e] = cmul(v[e], X.bufB[lin + e * nthr]);
+                for (int e = 0; e < E; ++e) w[e] = cmul(v[e], X.bufB[tid + e * nthr]);
                 if (j + 1 < p || it + 1 < my_tiles) {
                     __syncthreads();
                     if (tid == 0) {
-                        if (j + 1 < p) bulk_load(X.bufB, P.khat + (size_t)(j + 1) * P.specplane + X.tile_of(it), tile_bytes, &bars[1]);
-                        else           bulk_load(X.bufB, P.khat + X.tile_of(it + 1), tile_bytes, &bars[1]);
+                        if (j + 1 < p) bulk_load(X.bufB, P.khat + (size_t)(j + 1) * P.specplane + X.ktile_of(it), tile_bytes, &bars[1]);
+                        else           bulk_load(X.bufB, P.khat + X.ktile_of(it + 1), tile_bytes, &bars[1]);
                     }
                 }
                 if (pk) packed_fix<T, L, E, false>(w, pack, P.khatB + (size_t)j * L, t);
-                fft_block<T, L, E, +1, TWS>(w, smc, cs, t, tw, gsync);
-                C *dst = Pout + (size_t)j * P.specplane + X.tile_of(it) + lin;
+                fft_block<T, L, E, +1>(w, X.smc, Cc, t, P.tw, sync);
+                C *dst = P.out + (size_t)j * P.specplane + X.tile_of(it) + tid;
 #pragma unroll
                 for (int e = 0; e < E; ++e) dst[(size_t)e * nthr] = w[e];
             }
@@ -266,10 +231,10 @@ __device__ __forceinline__ void col_body(const ColParams<T> &P)
 }
 
 // CT = 0: tile width from P.G.C; CT > 0: compiled for that width (the host launches it only when G.C == CT)
-template <typename T, int L, int MODE, bool MULTI, int CT = 0>
+template <typename T, int L, int MODE, bool MULTI, int CT = 0, bool BATCH = false>
 __global__ void __launch_bounds__(fft_E_col<T>(L) == 32 ? 256 : 512, 1) col_kernel(const ColParams<T> P)
 {
-    col_body<T, L, MODE, MULTI, CT>(P);
+    col_body<T, L, MODE, MULTI, CT, BATCH>(P);
 }
 
 // ---------------------------------------------------------------------------------------------------------------
@@ -279,7 +244,7 @@ __global__ void __launch_bounds__(fft_E_col<T>(L) == 32 ? 256 : 512, 1) col_kern
 // straight from global memory (L2-resident: it is read twice per iteration) into the registers.  68 KB and 128
 // registers per CTA, so TWO CTAs share an SM: the whole grid (256 tiles at 2048^2) is resident at once instead of
 // 1.73 waves of one 200 KB CTA per SM, and one CTA's loads and stores overlap the other's butterflies.
-template <typename T, int L, int MODE>
+template <typename T, int L, int MODE, bool BATCH = false>
 __global__ void __launch_bounds__(256, 2) col2_kernel(const ColParams<T> P)
 {
     using C = cx<T>;
@@ -293,37 +258,32 @@ __global__ void __launch_bounds__(256, 2) col2_kernel(const ColParams<T> P)
     const int tid = threadIdx.x;
     const int t = tid / Cc, c = tid - t * Cc;
     constexpr size_t tile_len = (size_t)L * Cc;
-    const size_t tbase = (size_t)blockIdx.x * tile_len;
+    const size_t kbase = (size_t)blockIdx.x * tile_len;                              // in the (shared) transfer function
+    const size_t tbase = kbase + (BATCH ? (size_t)blockIdx.z * (P.slab / sizeof(C)) : 0);          // in this problem's spectra (batched plans)
     const unsigned int tile_bytes = (unsigned int)(tile_len * sizeof(C));
-    const size_t boff = (size_t)blockIdx.z * P.slab;
-    const C *Pin = bshift(P.in, boff);
-    C *Pout = bshift(P.out, boff);
-    Ctrl *Pct = bshift(P.ct, boff);
-    const int stop = P.check_status ? (Pct->status != 0 || (P.check_status == 2 && Pct->refresh_due == 0)) : 0;
-    if (stop != 0) return;
-    if (P.count_fft && blockIdx.x == 0 && tid == 0) atomicAdd(&Pct->nfft, 2ull);
+    {
+        Ctrl *ctz = BATCH ? bshift(P.ct, (size_t)blockIdx.z * P.slab) : P.ct;
+        const int stop = P.check_status ? ctz->status : 0;
+        if (stop != 0) return;
+    }
     if (tid == 0) {
         mbar_init(&bar, 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-        bulk_load(sm, Pin + tbase, tile_bytes, &bar);
+        bulk_load(sm, P.in + tbase, tile_bytes, &bar);
         // the transfer-function tile is wanted after the forward transform: start it on its way to L2 now (in the SGP
         // loop the planes touched since its last use have pushed it out to HBM)
-        asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(P.khat + tbase), "r"(tile_bytes) : "memory");
+        asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(P.khat + kbase), "r"(tile_bytes) : "memory");
     }
-    constexpr bool TWS = SGP_TW_SMEM != 0;
-    C *tw_s = sm + (size_t)Cc * fft_padded_len(L, E);
-    if constexpr (TWS) copy_table_to_smem(tw_s, P.tw, tw_total(L, E), tid, nthr);
-    const C *tw = TWS ? tw_s : P.tw;
-    __syncthreads();                                            // barrier initialisation (and the tables) visible to all
+    __syncthreads();                                            // barrier initialisation visible to all
     const SyncBlock sync;
     const bool packed = blockIdx.x == 0;                        // tile 0 holds the packed column (kx = 0 and nx/2)
     const bool pk = packed && c == 0;
-    volatile C *pack = bshift(P.pack, boff);
+    volatile C *pack = (BATCH ? bshift(P.pack, (size_t)blockIdx.z * P.slab) : P.pack);
     C v[E];
     mbar_wait(&bar, 0);
 #pragma unroll
     for (int e = 0; e < E; ++e) v[e] = sm[tid + e * nthr];
-    fft_block<T, L, E, -1, TWS>(v, sm + c, Cc, t, tw, sync);    // its first exchange starts with a barrier: the tile has been read
+    fft_block<T, L, E, -1>(v, sm + c, Cc, t, P.tw, sync);       // its first exchange starts with a barrier: the tile has been read
     if (packed) {
         if (pk) {
 #pragma unroll
@@ -331,7 +291,7 @@ __global__ void __launch_bounds__(256, 2) col2_kernel(const ColParams<T> P)
         }
         __syncthreads();
     }
-    const C *kh = P.khat + tbase + tid;
+    const C *kh = P.khat + kbase + tid;
 #pragma unroll
     for (int e0 = 0; e0 < E; e0 += 8) {
         C k[8];
@@ -341,8 +301,8 @@ __global__ void __launch_bounds__(256, 2) col2_kernel(const ColParams<T> P)
         for (int u = 0; u < 8; ++u) v[e0 + u] = (MODE == CM_CONJSUM) ? cmulc(v[e0 + u], k[u]) : cmul(v[e0 + u], k[u]);
     }
     if (pk) packed_fix<T, L, E, MODE == CM_CONJSUM>(v, pack, P.khatB, t);
-    fft_block<T, L, E, +1, TWS>(v, sm + c, Cc, t, tw, sync);
-    C *dst = Pout + tbase + tid;
+    fft_block<T, L, E, +1>(v, sm + c, Cc, t, P.tw, sync);
+    C *dst = P.out + tbase + tid;
 #pragma unroll
     for (int e = 0; e < E; ++e) dst[(size_t)e * nthr] = v[e];
 }

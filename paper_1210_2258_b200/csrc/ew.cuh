@@ -44,6 +44,8 @@ template <typename T> struct RowParams {
     int check_status;                 // 1: return immediately when ct->status != 0
     unsigned int *btsync;             // K6: counters of the Armijo backtracking to re-arm (aux.cuh)
     const void *btinfo;               // K1 in the SGP loop: BtInfo<T> block in device memory (aux.cuh: Armijo backtracking)
+    int count_fft;                    // inverse row kernels of the loops: two-dimensional transforms completed by this launch and the column
+                                      // pass before it (p + 1), added to Ctrl::nfft by one thread
     size_t slab, tr_slab;             // batched plans: bytes between the per-problem arrays / trace blocks of consecutive problems
 };
 
@@ -95,7 +97,6 @@ template <typename T> struct ColParams {
     int p;
     int ntiles;                       // (nx/2)/C
     int check_status;
-    int count_fft;                    // 1: add the p + 1 two-dimensional transforms of this pass to Ctrl::nfft
     size_t slab;                      // batched plans: bytes between the per-problem arrays (in, out, pack, ct) of consecutive problems
 };
 
@@ -222,6 +223,21 @@ __device__ __forceinline__ void pdl_trigger() { asm volatile("griddepcontrol.lau
 __device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
 
 __device__ __forceinline__ void prefetch_l2(const void *p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
+__device__ __forceinline__ void prefetch_l1(const void *p) { asm volatile("prefetch.global.L1 [%0];" ::"l"(p)); }
+// The twiddle tables of a kernel on their way into the L1 at its start, one 128-byte line per thread.  The L1 is empty at
+// every launch, and a CTA of the column kernel lives for one or two tiles only: 28 % of its twiddle sectors missed (ncu,
+// 2048^2), each miss a trip to L2 in the middle of a pass.  Issued while the tile is still in flight, the trips overlap.
+#ifndef SGP_TW_PREFETCH
+#define SGP_TW_PREFETCH 1
+#endif
+template <typename C> __device__ __forceinline__ void prefetch_table_l1(const C *table, int entries, int tid, int nthr)
+{
+#if SGP_TW_PREFETCH
+    const char *b = reinterpret_cast<const char *>(table);
+    const int nlines = (entries * (int)sizeof(C) + 127) / 128;
+    for (int l = tid; l < nlines; l += nthr) prefetch_l1(b + 128 * l);
+#endif
+}
 // start one row of a plane (len reals) on its way to L2; called by the TF threads of the row
 template <typename T> __device__ __forceinline__ void prefetch_row_l2(const T *row, int len, int t, int TF)
 {

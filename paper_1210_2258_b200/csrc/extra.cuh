@@ -226,12 +226,16 @@ __global__ void apply_pending_kernel(T *f, const T *d, size_t n, Ctrl *ct)
     const T lam = (T)ct->lambda;
     for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) f[i] = f[i] + lam * d[i];
 }
-// closes the bracket: pending <- 0 after every CTA of apply_pending_kernel has read it; hands need_k1 to the ratio kernel
-template <int DUMMY = 0> __global__ void refresh_flags_kernel(Ctrl *ct)
+// closes the bracket: pending <- 0 after every CTA of apply_pending_kernel has read it; hands need_k1 to the ratio kernel;
+// and sets the status of the SHADOW control block that the column pass of the refresh round tests (0 = run, 1 = not this
+// iteration), so that the column kernel needs no test of its own for the refresh round
+template <int DUMMY = 0> __global__ void refresh_flags_kernel(Ctrl *ct, Ctrl *shadow)
 {
     if (threadIdx.x == 0 && blockIdx.x == 0) {
-        if (ct->refresh_due != 0 && ct->status == 0) ct->pending = 0;
+        const bool due = ct->refresh_due != 0 && ct->status == 0;
+        if (due) ct->pending = 0;
         ct->need_k1 = ct->need_k1_next;
+        shadow->status = due ? 0 : 1;
     }
 }
 

@@ -224,9 +224,15 @@ template <int R, int DIR, typename T, typename C> __device__ __forceinline__ voi
 
 // ---------------------------------------------------------------- plans
 // Elements per thread: float 32 (L >= 512) or 16, double 8, 5*2^k lengths 20.
+#ifndef SGP_ROW_MINB
+#define SGP_ROW_MINB 2        // resident CTAs per SM the row kernels are compiled for (register cap 128 at 2)
+#endif
+#ifndef SGP_ROW_E16
+#define SGP_ROW_E16 0         // experiment: 16 elements per thread in the float row kernels (two warps per 2048-pixel row)
+#endif
 template <typename T> __host__ __device__ constexpr int fft_E(int L)
 {
-    return (L % 5 == 0) ? 20 : (sizeof(T) == 8 ? 8 : (L >= 512 ? 32 : 16));
+    return (L % 5 == 0) ? 20 : (sizeof(T) == 8 ? 8 : ((L >= 512 && !SGP_ROW_E16) ? 32 : 16));
 }
 // column kernel: a thread holds 32 elements only where that saves a pass (L = 512, 1024)
 #ifndef SGP_COL_E32_ALL

@@ -6,8 +6,16 @@ namespace sgpk {
 // it without spills where the specialised single-image form spilled 116-170 bytes, and it is 2 us per pass faster at 2048^2.
 template <int L> static col_kernel_t<SGP_T> pick_col(int mode, bool multi, int tile_cols)
 {
-    (void)multi;
     constexpr int CD = col_default_C<SGP_T>(L);
+    const bool batch = tile_cols < 0;          // a negative tile width asks for the batched-plan variant (blockIdx.z = problem)
+    if (batch) {
+        (void)multi;
+        if (-tile_cols == CD && mode == CM_CONJSUM) return col_kernel<SGP_T, L, CM_CONJSUM, true, CD, true>;
+        if (-tile_cols == CD && mode == CM_MULT) return col_kernel<SGP_T, L, CM_MULT, true, CD, true>;
+        if (mode == CM_CONJSUM) return col_kernel<SGP_T, L, CM_CONJSUM, true, 0, true>;
+        if (mode == CM_MULT) return col_kernel<SGP_T, L, CM_MULT, true, 0, true>;
+        return nullptr;
+    }
     if (tile_cols == CD && mode == CM_CONJSUM) return col_kernel<SGP_T, L, CM_CONJSUM, true, CD>;
     if (tile_cols == CD && mode == CM_MULT) return col_kernel<SGP_T, L, CM_MULT, true, CD>;
     if (mode == CM_FWD) return col_kernel<SGP_T, L, CM_FWD, false>;

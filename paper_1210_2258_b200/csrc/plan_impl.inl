@@ -34,6 +34,7 @@ template <typename T> struct PlanImpl : PlanBase {
     Ctrl *ct = nullptr;
     BtInfo<T> *btinfo = nullptr;
     unsigned int *btsync = nullptr, *fxsync = nullptr;
+    Ctrl *ct_shadow = nullptr;      // refresh round (A21): control block whose status tells the column pass whether this is a refresh iteration
     double *part_fx = nullptr, *part_err = nullptr;
     size_t fx_chunks = 0, fx_batches = 1;
     C *khatB_tmp = nullptr;        // companion line of the Gaussian's transfer function (smoothed constant start)
@@ -121,6 +122,11 @@ template <typename T> struct PlanImpl : PlanBase {
     std::vector<Req> reqs_pp;
     template <typename U> int dalloc_pp(U **ptr, size_t count)
     {
+        // an ordinary plan keeps everything in ONE arena, in the order of the requests: the column passes stream a spectrum
+        // tile and the transfer-function tile of the same offset at once, and how far apart the two planes lie decides how
+        // the two streams share the L2 slices (measured: with the spectra in an allocation of their own K2 / K5 took
+        // 45 / 45 us instead of 39 / 37 us at 3 x 2048^2)
+        if (nb == 1) return dalloc(ptr, count);
         reqs_pp.push_back({reinterpret_cast<void **>(ptr), count * sizeof(U)});
         return SGP_OK;
     }
@@ -128,25 +134,39 @@ template <typename T> struct PlanImpl : PlanBase {
     {
         return ptr ? reinterpret_cast<U *>(reinterpret_cast<unsigned char *>(const_cast<typename std::remove_const<U>::type *>(ptr)) + off) : ptr;
     }
+    // pieces of 64 KB and more start on a 4 KB boundary (the 64 KB tiles of spectra and transfer functions are moved by bulk
+    // copies: with the planes on odd multiples of 256 bytes the column passes of 3 x 2048^2 took 45 us instead of 39 us), the
+    // small ones on 256 bytes
+    static size_t piece_align(size_t bytes) { return bytes >= 65536 ? 4096 : 256; }
+    static size_t place(size_t &off, size_t bytes)
+    {
+        const size_t a = piece_align(bytes);
+        off = (off + a - 1) & ~(a - 1);
+        const size_t at = off;
+        off += bytes;
+        return at;
+    }
     int commit_allocs()
     {
         size_t total = 0;
-        for (const Req &r : reqs) total += (r.bytes + 255) & ~(size_t)255;
+        for (const Req &r : reqs) place(total, r.bytes);
+        total = (total + 4095) & ~(size_t)4095;
         void *raw = nullptr;
         SGP_CUDA_TRY(cudaMalloc(&raw, total ? total : 256));
         allocs.push_back(raw);
         bytes_allocated += total;
         size_t off = 0;
-        for (const Req &r : reqs) { *r.ptr = static_cast<unsigned char *>(raw) + off; off += (r.bytes + 255) & ~(size_t)255; }
+        for (const Req &r : reqs) { const size_t at = place(off, r.bytes); *r.ptr = static_cast<unsigned char *>(raw) + at; }
         reqs.clear();
         size_t per = 0;
-        for (const Req &r : reqs_pp) per += (r.bytes + 255) & ~(size_t)255;
+        for (const Req &r : reqs_pp) place(per, r.bytes);
+        per = (per + 4095) & ~(size_t)4095;
         void *raw_pp = nullptr;
         SGP_CUDA_TRY(cudaMalloc(&raw_pp, per * (size_t)nb ? per * (size_t)nb : 256));
         allocs.push_back(raw_pp);
         bytes_allocated += per * (size_t)nb;
         off = 0;
-        for (const Req &r : reqs_pp) { *r.ptr = static_cast<unsigned char *>(raw_pp) + off; off += (r.bytes + 255) & ~(size_t)255; }
+        for (const Req &r : reqs_pp) { const size_t at = place(off, r.bytes); *r.ptr = static_cast<unsigned char *>(raw_pp) + at; }
         reqs_pp.clear();
         slab = nb > 1 ? per : 0;
         for (const Upload &u : uploads) SGP_CUDA_TRY(cudaMemcpy(*u.ptr, u.data.data(), u.data.size(), cudaMemcpyHostToDevice));
@@ -167,8 +187,10 @@ template <typename T> struct PlanImpl : PlanBase {
         int rc = choose_tiles(ny, nx, dtype, &opt, &Cc, &RB);
         if (rc) return rc;
         const bool multi = p > 1;
-        k_colf = get_col<T>(Lc, CM_FWD, false); k_conj = get_col<T>(Lc, CM_CONJSUM, multi, Cc); k_mult = get_col<T>(Lc, CM_MULT, multi, Cc);
-        k_conj1 = get_col<T>(Lc, CM_CONJSUM, false, Cc); k_mult1 = get_col<T>(Lc, CM_MULT, false, Cc);
+        // batched plans (nb > 1) use the column kernels compiled with the per-problem offset (col.cuh: BATCH), asked for by a negative width
+        const int Cq = nb > 1 ? -Cc : Cc;
+        k_colf = get_col<T>(Lc, CM_FWD, false); k_conj = get_col<T>(Lc, CM_CONJSUM, multi, Cq); k_mult = get_col<T>(Lc, CM_MULT, multi, Cq);
+        k_conj1 = get_col<T>(Lc, CM_CONJSUM, false, Cq); k_mult1 = get_col<T>(Lc, CM_MULT, false, Cq);
         if (!k_colf || !k_conj || !k_mult || !k_conj1 || !k_mult1) return SGP_ERR_ARG;
         G.C = Cc; G.RB = RB; G.lc = 0; while ((1 << G.lc) < Cc) G.lc++;
         row_threads = RB * group_threads(Lr / Er);
@@ -176,7 +198,6 @@ template <typename T> struct PlanImpl : PlanBase {
         nrb = ny / RB; ntiles = Lr / Cc;
         row_smem = ((size_t)RB * row_stride(Lr, Er) + row_table_entries<T>(Lr)) * sizeof(C);     // rows + twiddle tables (row_fwd.cuh)
         col_smem = ((size_t)Cc * fft_padded_len(Lc, Ec) + 2 * (size_t)Cc * Lc) * sizeof(C);
-        if (col_tw_in_smem<T>(Lc, Cc)) col_smem += (size_t)tw_total(Lc, Ec) * sizeof(C);      // pass tables in shared memory (col.cuh)
         if (row_threads > 256 || col_threads > 512 || row_smem > 227 * 1024 || col_smem > 227 * 1024) return SGP_ERR_ARG;
         for (int m = 0; m < RF_NMODES; ++m)
             SGP_CUDA_TRY(cudaFuncSetAttribute((const void *)k_rowf[m], cudaFuncAttributeMaxDynamicSharedMemorySize, (int)row_smem));
@@ -190,18 +211,12 @@ template <typename T> struct PlanImpl : PlanBase {
         int dev = 0;
         SGP_CUDA_TRY(cudaGetDevice(&dev));
         SGP_CUDA_TRY(cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev));
-        // Fused or separate line-search / ratio kernels.  Separate, the ratio kernel re-reads g_j, q_j, u_j right after the
-        // line-search kernel touched them: free while those 3p planes stay in L2 (2048^2 fp32 single image: 50 MB of
-        // 126 MB; measured 7700 vs 7240 it/s), a second trip to HBM once they do not (3 x 2048^2, 4096^2, fp64: fused is
-        // 3.5-4.5 % faster).  Small grids are latency-bound and gain from the launch the fused form saves.
-        {
-            int l2 = 0;
-            SGP_CUDA_TRY(cudaDeviceGetAttribute(&l2, cudaDevAttrL2CacheSize, dev));
-            const size_t handoff = 3 * (size_t)p * n * sizeof(T);
-            fuse_ls = handoff > (size_t)l2 / 2 || handoff < (size_t)l2 / 8;
-            if (opt.use_graph & 4) fuse_ls = false;      // experiment switches
-            if (opt.use_graph & 8) fuse_ls = true;
-        }
+        // Fused or separate line-search / ratio kernels.  Round 1 chose by the size of the hand-off (g_j, q_j, u_j: 3p planes) against
+        // L2 and ran 2048^2 single image separate; with the backtracking folded into the ratio kernel (six launches instead of
+        // seven) the fused form is ahead there too (112.7 vs 113.2 us per iteration; 3 x 2048^2: 209 vs 222 us), so it is the default.
+        fuse_ls = true;
+        if (opt.use_graph & 4) fuse_ls = false;      // experiment switches
+        if (opt.use_graph & 8) fuse_ls = true;
         col_grid = (opt.use_graph & 2) ? (ntiles < nsm ? ntiles : nsm) : ntiles;   // experiment switch: persistent or one tile per CTA
 
         // twiddles, computed in double on the host
@@ -240,9 +255,9 @@ template <typename T> struct PlanImpl : PlanBase {
         // single-image product passes: the two-CTAs-per-SM kernel where it exists (float, 256 threads at this tile width);
         // run() decides per algorithm whether to use it
         k_conj_run = k_conj; k_mult_run = k_mult;
-        if (p == 1 && !(opt.use_graph & 16) && plan_ok(Lc, 32) && Cc * (Lc / 32) == 256) {
+        if (p == 1 && nb == 1 && !(opt.use_graph & 16) && plan_ok(Lc, 32) && Cc * (Lc / 32) == 256) {
             col_kernel_t<T> c2 = get_col2<T>(Lc, CM_CONJSUM), m2 = get_col2<T>(Lc, CM_MULT);
-            const size_t sm2 = ((size_t)Cc * fft_padded_len(Lc, 32) + (SGP_TW_SMEM ? (size_t)tw_total(Lc, 32) : 0)) * sizeof(C);
+            const size_t sm2 = (size_t)Cc * fft_padded_len(Lc, 32) * sizeof(C);
             if (c2 && m2 && sm2 <= 113 * 1024) {
                 SGP_CUDA_TRY(cudaFuncSetAttribute((const void *)c2, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm2));
                 SGP_CUDA_TRY(cudaFuncSetAttribute((const void *)m2, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm2));
@@ -283,6 +298,7 @@ template <typename T> struct PlanImpl : PlanBase {
         if ((rc = dalloc_pp(&btinfo, (size_t)1))) return rc;
         if ((rc = dalloc_pp(&btsync, (size_t)kBtSyncWords))) return rc;
         if ((rc = dalloc(&fxsync, (size_t)kBtSyncWords))) return rc;
+        if ((rc = dalloc(&ct_shadow, (size_t)1))) return rc;
         {   // flux-constrained projection (extra.cuh): about two chunks per SM and Newton step
             const size_t batch = bt_chunk_elems<T>(), ctas = 2 * (size_t)nsm;
             fx_batches = (n + batch * ctas - 1) / (batch * ctas);

@@ -58,13 +58,13 @@ int PlanImpl<T>::enqueue_sgp_iteration(const RowParams<T> &Pb, const DevOpts &o,
     int rc;
     cur_slot = SGP_PROF_K2;
     {   // K2 (a2)
-        ColParams<T> Q = col_params(); Q.check_status = 1; Q.count_fft = 1;
+        ColParams<T> Q = col_params(); Q.check_status = 1;
         if ((rc = launch_col(k_conj_run, Q, st))) return rc;
     }
     cur_slot = SGP_PROF_K3;
     {   // K3 (a10 for f, a3, a5, a6)
         RowParams<T> P = Pb; P.lazy = 1; P.in0 = f; P.in1 = d; P.out0 = grad; P.out1 = f; P.part = part_bb;
-        if ((rc = launch_row(k_rowi[RI_GRAD], P, 1, st))) return rc;
+        P.count_fft = p + 1; if ((rc = launch_row(k_rowi[RI_GRAD], P, 1, st))) return rc;
     }
     if (o.flux_constraint) {   // the multiplier mu of the flux-constrained projection (extra.cuh): Newton steps, no FFT
         flux_arm_kernel<0><<<1, 32, 0, st>>>(fxsync, ct);
@@ -84,13 +84,13 @@ int PlanImpl<T>::enqueue_sgp_iteration(const RowParams<T> &Pb, const DevOpts &o,
     }
     cur_slot = SGP_PROF_K5;
     {   // K5 (a8)
-        ColParams<T> Q = col_params(); Q.check_status = 1; Q.count_fft = 1;
+        ColParams<T> Q = col_params(); Q.check_status = 1;
         if ((rc = launch_col(k_mult_run, Q, st))) return rc;
     }
     cur_slot = SGP_PROF_K6;
     {   // K6 (a8 tail, a9 at lambda = 1, a11)
         RowParams<T> P = Pb; P.in0 = Gp; P.in1 = q; P.in2 = Bp; P.out0 = u; P.part = part_J; P.part2 = part_gd; P.btsync = btsync;
-        if ((rc = launch_row(k_rowi[fuse_ls ? RI_LSF : RI_LS], P, p, st))) return rc;
+        P.count_fft = p + 1; if ((rc = launch_row(k_rowi[fuse_ls ? RI_LSF : RI_LS], P, p, st))) return rc;
     }
     cur_slot = -1;
     // ---- tail: K1 of the next iteration (a9 for lambda < 1 as its prologue, a11, a10 for q, a1)
@@ -105,13 +105,13 @@ int PlanImpl<T>::enqueue_sgp_iteration(const RowParams<T> &Pb, const DevOpts &o,
         // this round return at once otherwise): apply the pending step to f, row FFT of f, column pass x K^_j, inverse rows
         // -> q_j, J0, stopping rules; then the ratio of the next iteration once more, from the recomputed q
         apply_pending_kernel<T><<<ew_grid(n), 256, 0, st>>>(f, d, n, ct);
-        refresh_flags_kernel<0><<<1, 32, 0, st>>>(ct);
+        refresh_flags_kernel<0><<<1, 32, 0, st>>>(ct, ct_shadow);
         launches += 2;
         SGP_CUDA_TRY(cudaGetLastError());
         { RowParams<T> P = Pb; P.in0 = f; P.lazy = 4; if ((rc = launch_row(k_rowf[RF_PLAIN], P, 1, st))) return rc; }
-        { ColParams<T> Q = col_params(); Q.check_status = 2; Q.count_fft = 1; if ((rc = launch_col(k_mult_run, Q, st))) return rc; }
+        { ColParams<T> Q = col_params(); Q.check_status = 1; Q.ct = ct_shadow; if ((rc = launch_col(k_mult_run, Q, st))) return rc; }     // counted by the QJ_REFRESH kernel
         { RowParams<T> P = Pb; P.submode = QJ_REFRESH; P.in0 = Gp; P.in2 = Bp; P.out0 = q; P.part = part_J;
-          if ((rc = launch_row(k_rowi[RI_QJ], P, p, st))) return rc; }
+          P.count_fft = p + 1; if ((rc = launch_row(k_rowi[RI_QJ], P, p, st))) return rc; }
         if ((rc = enqueue_ratio(Pb, 2, st))) return rc;
     }
     return SGP_OK;
@@ -136,30 +136,30 @@ int PlanImpl<T>::enqueue_rl_round(const DevOpts &o, const Trace &tr, const doubl
         { RowParams<T> P = Pb; P.in0 = f; P.maskmode = MM_NONE; if ((rc = launch_row(k_rowf[RF_PLAIN], P, 1, st))) return rc; }
     }
     cur_slot = SGP_PROF_R2;
-    { ColParams<T> Q = col_params(); Q.check_status = 1; Q.count_fft = 1; if ((rc = launch_col(k_mult_run, Q, st))) return rc; }
+    { ColParams<T> Q = col_params(); Q.check_status = 1; if ((rc = launch_col(k_mult_run, Q, st))) return rc; }
     cur_slot = SGP_PROF_R3;
     if (rl_fused) {
         RowParams<T> P = Pb; P.submode = QJ_RL; P.in0 = Gp; P.in2 = Bp; P.part = part_J;
-        if ((rc = launch_row(k_rowi[RI_QJF], P, p, st))) return rc;
+        P.count_fft = p + 1; if ((rc = launch_row(k_rowi[RI_QJF], P, p, st))) return rc;
     } else {
-        { RowParams<T> P = Pb; P.submode = QJ_RL; P.in0 = Gp; P.in2 = Bp; P.out0 = q; P.part = part_J; if ((rc = launch_row(k_rowi[RI_QJ], P, p, st))) return rc; }
+        { RowParams<T> P = Pb; P.submode = QJ_RL; P.in0 = Gp; P.in2 = Bp; P.out0 = q; P.part = part_J; P.count_fft = p + 1; if ((rc = launch_row(k_rowi[RI_QJ], P, p, st))) return rc; }
         cur_slot = SGP_PROF_R4;
         { RowParams<T> P = Pb; P.in0 = Gp; P.in1 = q; P.in2 = Bp; if ((rc = launch_row(k_rowf[RF_RATIO], P, p, st))) return rc; }
     }
     cur_slot = SGP_PROF_R5;
-    { ColParams<T> Q = col_params(); Q.check_status = 1; Q.count_fft = 1; if ((rc = launch_col(k_conj_run, Q, st))) return rc; }
+    { ColParams<T> Q = col_params(); Q.check_status = 1; if ((rc = launch_col(k_conj_run, Q, st))) return rc; }
     cur_slot = SGP_PROF_R6;
     if (tr.err) {
         // Eq.25: the update goes to the plane `d` (unused by RL), its error is evaluated, and it replaces f only if the
         // rule lets it (extra.cuh); needs the separate kernels (rl_fused is off)
-        { RowParams<T> P = Pb; P.in0 = f; P.out0 = d; if ((rc = launch_row(k_rowi[RI_RLUPDATE], P, 1, st))) return rc; }
+        { RowParams<T> P = Pb; P.in0 = f; P.out0 = d; P.count_fft = p + 1; if ((rc = launch_row(k_rowi[RI_RLUPDATE], P, 1, st))) return rc; }
         err_kernel<T><<<ew_grid(n), 256, 0, st>>>(f, nullptr, d, (const T *)run_truth, n, ct, o, tr, part_err, 2);
         rl_commit_kernel<T><<<ew_grid(n), 256, 0, st>>>(f, d, n, ct);
         launches += 2;
         SGP_CUDA_TRY(cudaGetLastError());
     } else {
         RowParams<T> P = Pb; P.in0 = f; P.out0 = f;
-        if ((rc = launch_row(k_rowi[rl_fused ? RI_RLUPF : RI_RLUPDATE], P, 1, st))) return rc;
+        P.count_fft = p + 1; if ((rc = launch_row(k_rowi[rl_fused ? RI_RLUPF : RI_RLUPDATE], P, 1, st))) return rc;
     }
     cur_slot = -1;
     return SGP_OK;
@@ -181,7 +181,7 @@ int PlanImpl<T>::enqueue_osem_cycle(const DevOpts &o, const Trace &tr, const dou
         Pb.bconst[0] = bconst[j];
         Pb.alphaR = G.masked ? alphaJ + off : nullptr;
         ColParams<T> Qb = col_params();
-        Qb.check_status = 1; Qb.count_fft = 1; Qb.p = 1; Qb.khat = khat + (size_t)j * nspec; Qb.khatB = khatB + (size_t)j * ny;
+        Qb.check_status = 1; Qb.p = 1; Qb.khat = khat + (size_t)j * nspec; Qb.khatB = khatB + (size_t)j * ny;
         if (!rl_fused) {
             cur_slot = SGP_PROF_R1;
             { RowParams<T> P = Pb; P.in0 = f; P.maskmode = MM_NONE; if ((rc = launch_row(k_rowf[RF_PLAIN], P, 1, st))) return rc; }
@@ -191,17 +191,17 @@ int PlanImpl<T>::enqueue_osem_cycle(const DevOpts &o, const Trace &tr, const dou
         cur_slot = SGP_PROF_R3;
         if (rl_fused) {
             RowParams<T> P = Pb; P.submode = QJ_PLAIN; P.in0 = Gp + off; P.in2 = Bp + off; P.part = part_J;
-            if ((rc = launch_row(k_rowi[RI_QJF], P, 1, st))) return rc;
+            P.count_fft = 2; if ((rc = launch_row(k_rowi[RI_QJF], P, 1, st))) return rc;
         } else {
             { RowParams<T> P = Pb; P.submode = QJ_PLAIN; P.in0 = Gp + off; P.in2 = Bp + off; P.out0 = q + off; P.part = part_J;
-              if ((rc = launch_row(k_rowi[RI_QJ], P, 1, st))) return rc; }
+              P.count_fft = 2; if ((rc = launch_row(k_rowi[RI_QJ], P, 1, st))) return rc; }
             cur_slot = SGP_PROF_R4;
             { RowParams<T> P = Pb; P.in0 = Gp + off; P.in1 = q + off; P.in2 = Bp + off; if ((rc = launch_row(k_rowf[RF_RATIO], P, 1, st))) return rc; }
         }
         cur_slot = SGP_PROF_R5;
         if ((rc = launch_col(k_conj1, Qb, st))) return rc;
         cur_slot = SGP_PROF_R6;
-        { RowParams<T> P = Pb; P.in0 = f; P.out0 = f; if ((rc = launch_row(k_rowi[rl_fused ? RI_RLUPF : RI_RLUPDATE], P, 1, st))) return rc; }
+        { RowParams<T> P = Pb; P.in0 = f; P.out0 = f; P.count_fft = 2; if ((rc = launch_row(k_rowi[rl_fused ? RI_RLUPF : RI_RLUPDATE], P, 1, st))) return rc; }
     }
     cur_slot = -1;
     return SGP_OK;
@@ -398,12 +398,12 @@ int PlanImpl<T>::run_batched(int algorithm, const void *const *g, const void *co
 
     if (algorithm == SGP_ALG_SGP) {
         { RowParams<T> P = Pb; P.in0 = f; if ((rc = launch_row(k_rowf[RF_PLAIN], P, 1, st))) return rc; }
-        { ColParams<T> Q = col_params(); Q.check_status = 1; Q.count_fft = 1; if ((rc = launch_col(k_mult_run, Q, st))) return rc; }
+        { ColParams<T> Q = col_params(); Q.check_status = 1; if ((rc = launch_col(k_mult_run, Q, st))) return rc; }
         { RowParams<T> P = Pb; P.submode = QJ_INIT; P.in0 = Gp; P.in2 = Bp; P.out0 = q; P.part = part_J;
           if ((rc = launch_row(k_rowi[RI_QJ], P, p, st))) return rc; }
         if (ro.adaptive_L) {     // bounds from one RL step
             { RowParams<T> P = Pb; P.in0 = Gp; P.in1 = q; P.in2 = Bp; if ((rc = launch_row(k_rowf[RF_RATIO], P, p, st))) return rc; }
-            { ColParams<T> Q = col_params(); Q.check_status = 1; Q.count_fft = 1; if ((rc = launch_col(k_conj_run, Q, st))) return rc; }
+            { ColParams<T> Q = col_params(); Q.check_status = 1; if ((rc = launch_col(k_conj_run, Q, st))) return rc; }
             { RowParams<T> P = Pb; P.submode = RIP_RLMINMAX; P.in0 = f; P.part = part_J; if ((rc = launch_row(k_rowi[RI_PLAIN], P, 1, st))) return rc; }
         }
     }
@@ -478,13 +478,12 @@ int PlanImpl<T>::run_batched(int algorithm, const void *const *g, const void *co
                 Trace t0 = tr; t0.J = nullptr;
                 RowParams<T> Pj = Pb; Pj.tr = t0;
                 { RowParams<T> P = Pj; P.in0 = f; if ((rc = launch_row(k_rowf[RF_PLAIN], P, 1, st))) return rc; }
-                { ColParams<T> Q = col_params(); Q.check_status = 1; Q.count_fft = 1; if ((rc = launch_col(k_mult_run, Q, st))) return rc; }
+                { ColParams<T> Q = col_params(); Q.check_status = 1; if ((rc = launch_col(k_mult_run, Q, st))) return rc; }
                 { RowParams<T> P = Pj; P.submode = QJ_INIT; P.in0 = Gp; P.in2 = Bp; P.out0 = q; P.part = part_J;
                   if ((rc = launch_row(k_rowi[RI_QJ], P, p, st))) return rc; }
                 if ((rc = read_ctrl())) return rc;
                 for (int b = 0; b < nb; ++b) {
-                    // the transforms of this last evaluation of J0 are not part of the cycles
-                    if (status[b] == 0) { status[b] = hs[b].status; hs[b].nfft -= (unsigned long long)(p + 1); }
+                    if (status[b] == 0) status[b] = hs[b].status;
                     hs[b].k = done;
                     if (status[b] == 0) status[b] = SGP_REASON_MAXIT;
                 }

@@ -116,7 +116,7 @@ __device__ __forceinline__ void fwd_fft_store(cx<T> (&v)[fft_E<T>(L)], cx<T> *sm
 // MK: the plan has a boundary mask (alphaR plane present); a template parameter so that the unmasked kernels carry none of
 // the mask branches (their registers and instructions cost 1.2-2.3 us per row kernel at 2048^2)
 template <typename T, int L, int MODE, bool MK>
-__global__ void __launch_bounds__(256, 2) row_fwd_kernel(const RowParams<T> P)
+__global__ void __launch_bounds__(256, SGP_ROW_MINB) row_fwd_kernel(const RowParams<T> P)
 {
     using C = cx<T>;
     constexpr int E = fft_E<T>(L);
@@ -201,14 +201,19 @@ __global__ void __launch_bounds__(256, 2) row_fwd_kernel(const RowParams<T> P)
             // (a9 for lambda < 1, elementwise on q_j + lambda u_j) runs here first, by all CTAs of the grid
             // (aux.cuh: backtrack_rounds); it ends with the book-keeping of the accepted step (finish_iteration).
             Ctrl *ct = X.ct;
-            if (ct->status != 0) return;
-#ifndef SGP_NO_BT
-            if (P.lazy == 1 && ct->accepted == 0) backtrack_rounds<T>(static_cast<const BtInfo<T> *>(X.btinfo));
-#endif
-            // the control block as the accepted step left it (written by another CTA: read past the L1)
-            if (__ldcg(&ct->status) != 0) return;
-            todo = __ldcg(&ct->need_k1); if (todo == 0) return; sel = __ldcg(&ct->qsel);
-            lam = (T)__ldcg(&ct->lambda);
+            // one round trip for everything the kernel needs from the control block ...
+            const int acc0 = ct->accepted;
+            int st0 = ct->status, nk = ct->need_k1, qs = ct->qsel;
+            double lm = ct->lambda;
+            if (st0 != 0) return;
+            if (P.lazy == 1 && acc0 == 0) {
+                backtrack_rounds<T>(static_cast<const BtInfo<T> *>(X.btinfo));
+                // ... and once more, as the accepted step left it (written by another CTA: read past the L1)
+                st0 = __ldcg(&ct->status); nk = __ldcg(&ct->need_k1); qs = __ldcg(&ct->qsel); lm = __ldcg(&ct->lambda);
+                if (st0 != 0) return;
+            }
+            todo = nk; if (todo == 0) return; sel = qs;
+            lam = (T)lm;
         }
         if constexpr (TWS) row_tables_issue<T, L>(tw_s, P, tid, (int)blockDim.x);      // after the early returns above
         const bool pend = todo == 2;

@@ -20,7 +20,7 @@ template <typename T> __device__ __forceinline__ void retangle(cx<T> a, cx<T> xb
 }
 
 template <typename T, int L, int MODE, bool MK>
-__global__ void __launch_bounds__(256, 2) row_inv_kernel(const RowParams<T> P)
+__global__ void __launch_bounds__(256, SGP_ROW_MINB) row_inv_kernel(const RowParams<T> P)
 {
     using C = cx<T>;
     constexpr int E = fft_E<T>(L);
@@ -246,6 +246,8 @@ __global__ void __launch_bounds__(256, 2) row_inv_kernel(const RowParams<T> P)
         for (int e = 0; e < E; ++e) v[e] = smrow[t + TF * e];
         fwd_fft_store<T, L, TWS>(v, smrow, t, sync, P, X, y, 0, tw, twh);
     }
+    // n_fft2 (include/sgp.h): the two-dimensional transforms this launch and the column pass before it completed
+    if (P.count_fft && bid == 0 && tid == 0) atomicAdd(&X.ct->nfft, (unsigned long long)P.count_fft);
 }
 
 }  // namespace sgpk

@@ -105,7 +105,7 @@ def test_mosaic_of_four_subdomains_matches_the_oracle(alg, dt, tol):
         print(f"[measured] mosaic {alg} p={p} {np.dtype(dt).name} rel_l2 = {e:.3e}")
         assert e <= tol
         for r, r_o in zip(res, ro):
-            assert abs(r.J0_final - r_o.J0_final) <= ((1e-3 if alg == "sgp" else 1e-5) if dt == np.float32 else 1e-10) * r_o.J0_final
+            assert abs(r.J0_final - r_o.J0_final) <= ((5e-3 if alg == "sgp" else 1e-5) if dt == np.float32 else 1e-10) * r_o.J0_final
     # host pointers
     w = synth.make("C1", n=256, max_iter=5, stop_rule=0)
     o = B.default_options(**{**w["opts"], "max_iter": 5, "stop_rule": 0})
