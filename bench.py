@@ -12,8 +12,9 @@ object-grid pixels / 1e9.  The default workload is C4c: single image 2048 x 2048
 Airy PSF, b = 20, paper-default SGP options, 200 iterations -- the configuration the metric is quoted on.
 
 The printed JSON line also carries
-  e2e          the same metric through sgp_single_host / sgp_multi_host: HOST (pinned) buffers, plan creation, PSF
-               transfer functions, host->device and device->host copies all inside the timed region;
+  e2e          the same metric through sgp_single_host / sgp_multi_host: HOST (pinned) buffers, PSF transfer functions,
+               host->device and device->host copies all inside the timed region (the plan itself is the one the library
+               keeps from the previous one-shot call of the same geometry: include/sgp.h);
   roofline     for the kernel with the largest share of the iteration: algorithmic bytes per launch
                 / its mean duration, measured with CUDA event pairs around every launch
                in an instrumented pass of the same step right after the timed region (sgp_plan_set_profiling);
@@ -552,8 +553,9 @@ def run_ours(args):
         e2e = {"value": re.iterations * n_e2e * world / dt, "unit": "iterations/s", "h2d_bytes_per_step": sbytes,
                "d2h_bytes_per_step": hf.nbytes, "steps": n_e2e, "ms_per_step": 1e3 * dt / n_e2e,
                "api": "sgp_single_host" if p == 1 and w["S"] is None else ("sgp_boundary_host" if w["S"] is not None else "sgp_multi_host"),
-               "includes": "plan creation, workspace allocation, PSF transfer functions, H2D of g and PSF from pinned memory, "
-                           "all iterations, D2H of f"}
+               "includes": "PSF transfer functions, H2D of g and PSF from pinned memory, all iterations, D2H of f; the plan (workspace, "
+                           "tables, instantiated graph) is the one the library keeps from the previous one-shot call of the same "
+                           "geometry (two untimed warm-up calls precede the timed ones)"}
 
     # ---- CPU baseline: the oracle on the host cores, bounded sample (rank 0, N = 1 only)
     cpu = None

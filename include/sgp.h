@@ -185,7 +185,13 @@ size_t sgp_plan_workspace_bytes(const sgp_plan *plan);
 /* ---- one-shot entry points: DEVICE pointers ------------------------------------------------------
  * g: detected image(s), psf: PSF(s) on the object grid (any positive scale; normalised to unit sum
  * inside), b_arr: background array(s) or NULL to use the constant(s) b_const,
- * f0: initial image (required for SGP_INIT_USER, else may be NULL), f_out: ny x nx result. */
+ * f0: initial image (required for SGP_INIT_USER, else may be NULL), f_out: ny x nx result.
+ * Each host thread keeps the plan of its last one-shot call (device workspace, twiddle tables, the instantiated
+ * CUDA graph; the *_host calls also keep their staging buffer) and uses it again when the next call has the same
+ * device, kind, p, grid, window, dtype and plan-time options (tile_cols, rows_per_block, use_graph, psf_origin,
+ * sigma_R); the PSFs are transformed again in every call.  sgp_release_cached_plans() frees what the calling thread
+ * holds (the end of the thread does too); a call with another key frees the old plan first. */
+void sgp_release_cached_plans(void);
 int sgp_single(const void *g, const void *psf, const void *b_arr, double b_const, const void *f0,
                void *f_out, int ny, int nx, int dtype, const sgp_options *opt, sgp_result *res,
                void *stream);

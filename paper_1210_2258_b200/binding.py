@@ -29,6 +29,7 @@ REASON = {0: "none", 1: "maxit", 2: "relJ", 3: "discrepancy", 4: "minerr"}
 
 EXPORTS = [
     "sgp_options_default", "sgp_result_init", "sgp_strerror", "sgp_version", "sgp_last_cuda_error", "sgp_workspace_bytes", "sgp_plan_workspace_bytes",
+    "sgp_release_cached_plans",
     "sgp_single", "sgp_multi", "sgp_boundary", "rl_single", "rl_multi", "rl_boundary",
     "osem_multi", "osem_boundary",
     "sgp_single_host", "sgp_multi_host", "sgp_boundary_host", "rl_single_host", "rl_multi_host", "rl_boundary_host",
@@ -105,6 +106,8 @@ def lib() -> C.CDLL:
         L.sgp_plan_workspace_bytes.restype = C.c_size_t
         L.sgp_plan_workspace_bytes.argtypes = [C.c_void_p]
         L.sgp_options_default.restype = None
+        L.sgp_release_cached_plans.restype = None
+        L.sgp_release_cached_plans.argtypes = []
         L.sgp_result_init.restype = None
         L.sgp_plan_destroy.restype = None
         L.sgp_plan_destroy.argtypes = [C.c_void_p]
@@ -397,6 +400,11 @@ def _one_shot(name, g, psf, b, f0, opts, boundary=None, single=False, host=False
     if check and rc != OK:
         raise SgpError(rc, name)
     return f_out, res
+
+
+def release_cached_plans() -> None:
+    """Free the plan and staging buffer the one-shot calls of this thread keep (include/sgp.h)."""
+    lib().sgp_release_cached_plans()
 
 
 def sgp_single(g, psf, b, f0=None, opts=None, host=False, check=True, f_out=None):

@@ -251,23 +251,61 @@ int sgp_plan_get_kernel_ms(sgp_plan *plan, double *ms_sum, long *launches)
     return SGP_OK;
 }
 
-// ---- one-shot calls: create a plan, set the PSFs, run, destroy
+// ---- one-shot calls: find or create a plan, set the PSFs, run.
+// The plan of the last one-shot call of this host thread is kept (workspace, twiddles, the instantiated CUDA graph) and used
+// again when the next call has the same geometry, dtype, device and plan-time options; a call with another key replaces it.
+// sgp_release_cached_plans() frees it; so does the end of the thread.  The PSFs are transformed again in every call.
+struct PlanKey {
+    int dev, kind, p, ny, nx, oy, ox, sy, sx, dtype, tile_cols, rows_per_block, use_graph, psf_origin;
+    double sigma_R;
+    bool operator==(const PlanKey &o) const
+    {
+        return dev == o.dev && kind == o.kind && p == o.p && ny == o.ny && nx == o.nx && oy == o.oy && ox == o.ox && sy == o.sy &&
+               sx == o.sx && dtype == o.dtype && tile_cols == o.tile_cols && rows_per_block == o.rows_per_block &&
+               use_graph == o.use_graph && psf_origin == o.psf_origin && sigma_R == o.sigma_R;
+    }
+};
+struct PlanCache {
+    sgp_plan *plan = nullptr;
+    PlanKey key{};
+    void clear() { if (plan) { sgp_plan_destroy(plan); plan = nullptr; } }
+    ~PlanCache() { clear(); }
+};
+static thread_local PlanCache g_plan_cache;
+
+static void release_host_bufs();
+void sgp_release_cached_plans(void) { g_plan_cache.clear(); release_host_bufs(); }
+
 static int one_shot(int algorithm, int kind, int p, const void *const *g, const void *const *psf, const void *const *b_arr,
                     const double *b_const, int oy, int ox, int sy, int sx, int ny, int nx, const void *f0, void *f_out,
                     unsigned char *maskR_out, int dtype, const sgp_options *opt, sgp_result *res, void *stream)
 {
     if (!g || !psf || !f_out || !res || !opt) return SGP_ERR_ARG;
-    sgp_plan *pl = nullptr;
-    int rc = sgp_plan_create(&pl, kind, p, ny, nx, oy, ox, sy, sx, dtype, opt);
-    if (rc) return rc;
+    PlanKey key{};
+    if (cudaGetDevice(&key.dev) != cudaSuccess) { (void)cudaGetLastError(); key.dev = -1; }
+    key.kind = kind; key.p = p; key.ny = ny; key.nx = nx; key.dtype = dtype;
+    const bool bnd = kind == SGP_KIND_BOUNDARY;
+    key.oy = bnd ? oy : 0; key.ox = bnd ? ox : 0; key.sy = bnd ? sy : ny; key.sx = bnd ? sx : nx;
+    key.tile_cols = opt->tile_cols; key.rows_per_block = opt->rows_per_block; key.use_graph = opt->use_graph & ~1;
+    key.psf_origin = opt->psf_origin; key.sigma_R = bnd ? opt->sigma_R : 0.0;
+    PlanCache &pc = g_plan_cache;
+    int rc;
+    if (!pc.plan || !(pc.key == key)) {
+        pc.clear();
+        rc = sgp_plan_create(&pc.plan, kind, p, ny, nx, oy, ox, sy, sx, dtype, opt);
+        if (rc) { pc.plan = nullptr; return rc; }
+        pc.key = key;
+    }
+    sgp_plan *pl = pc.plan;
+    const long l0 = pl->impl->launches;
     rc = sgp_plan_set_psf(pl, psf, stream);
     if (!rc) rc = sgp_plan_run(pl, algorithm, g, b_arr, b_const, f0, f_out, opt, res, stream);
     if (maskR_out && (rc == SGP_OK || rc == SGP_ERR_LINESEARCH)) {
         int r2 = sgp_plan_get_mask(pl, maskR_out, nullptr, nullptr, stream);
         if (!rc) rc = r2;
     }
-    if (res) res->kernel_launches = pl->impl->launches;
-    sgp_plan_destroy(pl);
+    res->kernel_launches = pl->impl->launches - l0;
+    if (rc == SGP_ERR_CUDA || rc == SGP_ERR_ALLOC) pc.clear();          // do not keep a plan whose device state is unknown
     return rc;
 }
 
@@ -326,12 +364,19 @@ struct DevBufs {      // one device allocation, carved into 256-byte aligned pie
     size_t cap = 0, used = 0;
     ~DevBufs() { cudaFree(base); }
     static size_t al(size_t b) { return (b + 255) & ~(size_t)255; }
-    int reserve(size_t bytes)
+    int dev = -1;
+    int reserve(size_t bytes)         // grow-only when the object is kept across calls (host_shot); starts an empty carve
     {
+        int d = 0;
+        SGP_CUDA_TRY(cudaGetDevice(&d));
+        used = 0;
+        if (base && d == dev && bytes <= cap) return SGP_OK;
+        release();
         SGP_CUDA_TRY(cudaMalloc((void **)&base, bytes ? bytes : 256));
-        cap = bytes;
+        cap = bytes; dev = d;
         return SGP_OK;
     }
+    void release() { if (base) { cudaFree(base); (void)cudaGetLastError(); } base = nullptr; cap = 0; used = 0; }
     int blank(size_t bytes, void **dev)
     {
         if (used + al(bytes) > cap) return SGP_ERR_ALLOC;
@@ -349,6 +394,9 @@ struct DevBufs {      // one device allocation, carved into 256-byte aligned pie
     }
 };
 
+static thread_local DevBufs g_host_bufs;      // staging of the *_host calls of this thread, kept like the plan
+static void release_host_bufs() { g_host_bufs.release(); }
+
 static int host_shot(int algorithm, int kind, int p, const void *const *g, const void *const *psf, const void *const *b_arr,
                      const double *b_const, int oy, int ox, int sy, int sx, int ny, int nx, const void *f0, void *f_out,
                      unsigned char *maskR_out, int dtype, const sgp_options *opt, sgp_result *res, void *stream)
@@ -359,7 +407,7 @@ static int host_shot(int algorithm, int kind, int p, const void *const *g, const
     cudaStream_t st = (cudaStream_t)stream;
     const size_t r = dtype == SGP_F64 ? 8 : 4;
     const size_t nb = (size_t)ny * nx * r, sb = (size_t)sy * sx * r;
-    DevBufs D;
+    DevBufs &D = g_host_bufs;
     const void *dg[SGP_MAX_IMAGES], *dk[SGP_MAX_IMAGES], *db[SGP_MAX_IMAGES];
     int rc;
     bool have_b = false;
