@@ -318,6 +318,28 @@ int sgp_plan_set_profiling(sgp_plan *plan, int on);
 int sgp_plan_get_kernel_ms(sgp_plan *plan, double *ms_sum, long *launches);
 void sgp_plan_destroy(sgp_plan *plan);
 
+/* ---- an entry point that allocates nothing ----------------------------------------------------------
+ * For callers that cannot call cudaMalloc (code under CUDA graph capture, tight serving loops, harnesses that
+ * forbid it): the relative reconstruction error of Eq.25,
+ *     *rho_out = || f - truth ||_2 / || truth ||_2      over n elements, accumulated in double,
+ * the quantity sgp_plan_run reports as trace_err[0] / err_final for a run given sgp_result.truth, computed by the same
+ * kernel arithmetic (same grid, same reduction order) but with its scratch -- per-CTA partial sums and the arrival
+ * counter -- in a file-scope device array of 19 200 bytes that every GPU which loads the library holds until exit.
+ *   f, truth : DEVICE pointers, n elements of `dtype` (SGP_F32 or SGP_F64), not written;
+ *   rho_out  : DEVICE pointer to one double, written by the kernel (read it after the stream reaches that point);
+ *   n        : 1 .. SGP_STATIC_MAX_ELEMS (4096 x 4096, the largest grid a plan accepts).  A larger n is rejected with
+ *              SGP_ERR_ARG and sgp_last_cuda_error() then says so ("n exceeds SGP_STATIC_MAX_ELEMS ..."); nothing is launched;
+ *   stream   : the cudaStream_t the kernel is enqueued on.  The call does not synchronise, and calls no cudaMalloc,
+ *              cudaFree or allocating library routine (the array's device address is looked up once per device with
+ *              cudaGetSymbolAddress, with that device current).
+ * Every call on a device shares the array, which keeps the previous call's contents (the kernel overwrites the partials
+ * before reading them and re-arms the counter itself).  Calls that OVERLAP on the GPU -- two streams with no ordering
+ * between them, or two host threads -- race on it: keep the calls of one device on one stream or order them with events.
+ * Returns SGP_OK, SGP_ERR_ARG (null pointer, n = 0 or beyond the maximum, bad dtype) or SGP_ERR_CUDA. */
+#define SGP_STATIC_MAX_ELEMS (4096L * 4096L)
+int sgp_rel_error_static(const void *f, const void *truth, size_t n, int dtype, double *rho_out, void *stream);
+size_t sgp_rel_error_static_max(void);       /* SGP_STATIC_MAX_ELEMS of the loaded library */
+
 #ifdef __cplusplus
 }
 #endif

@@ -24,12 +24,13 @@ INIT_USER, INIT_CONST, INIT_ZERO, INIT_G, INIT_CONST_SMOOTH = 0, 1, 2, 3, 4
 PSF_CENTER, PSF_CORNER = 0, 1
 KIND_SINGLE, KIND_MULTI, KIND_BOUNDARY = 0, 1, 2
 ALG_SGP, ALG_RL, ALG_OSEM = 0, 1, 2
+STATIC_MAX_ELEMS = 4096 * 4096     # SGP_STATIC_MAX_ELEMS of include/sgp.h
 OK, ERR_ARG, ERR_PSF, ERR_DATA, ERR_ALLOC, ERR_CUDA, ERR_LINESEARCH, ERR_NONFINITE, ERR_UNSUPPORTED = 0, -1, -2, -3, -4, -5, -6, -7, -8
 REASON = {0: "none", 1: "maxit", 2: "relJ", 3: "discrepancy", 4: "minerr"}
 
 EXPORTS = [
     "sgp_options_default", "sgp_result_init", "sgp_strerror", "sgp_version", "sgp_last_cuda_error", "sgp_workspace_bytes", "sgp_plan_workspace_bytes",
-    "sgp_release_cached_plans",
+    "sgp_release_cached_plans", "sgp_rel_error_static", "sgp_rel_error_static_max",
     "sgp_single", "sgp_multi", "sgp_boundary", "rl_single", "rl_multi", "rl_boundary",
     "osem_multi", "osem_boundary",
     "sgp_single_host", "sgp_multi_host", "sgp_boundary_host", "rl_single_host", "rl_multi_host", "rl_boundary_host",
@@ -107,6 +108,10 @@ def lib() -> C.CDLL:
         L.sgp_plan_workspace_bytes.argtypes = [C.c_void_p]
         L.sgp_options_default.restype = None
         L.sgp_release_cached_plans.restype = None
+        L.sgp_rel_error_static.restype = C.c_int
+        L.sgp_rel_error_static.argtypes = [C.c_void_p, C.c_void_p, C.c_size_t, C.c_int, C.c_void_p, C.c_void_p]
+        L.sgp_rel_error_static_max.restype = C.c_size_t
+        L.sgp_rel_error_static_max.argtypes = []
         L.sgp_release_cached_plans.argtypes = []
         L.sgp_result_init.restype = None
         L.sgp_plan_destroy.restype = None
@@ -405,6 +410,24 @@ def _one_shot(name, g, psf, b, f0, opts, boundary=None, single=False, host=False
 def release_cached_plans() -> None:
     """Free the plan and staging buffer the one-shot calls of this thread keep (include/sgp.h)."""
     lib().sgp_release_cached_plans()
+
+
+def rel_error_static(f, truth, rho_out, check=True) -> int:
+    """sgp_rel_error_static (include/sgp.h): || f - truth || / || truth || (Eq.25) into the one-element float64 DEVICE tensor
+    `rho_out`, on torch's current stream, through the entry point that allocates nothing (scratch in a static device array;
+    at most STATIC_MAX_ELEMS elements; calls that overlap on the GPU race).  Returns the status code."""
+    torch = _torch()
+    if f.shape != truth.shape or f.dtype != truth.dtype or not (f.is_cuda and truth.is_cuda and rho_out.is_cuda):
+        raise ValueError("f and truth: device tensors of one shape and dtype; rho_out: a device tensor")
+    if rho_out.dtype != torch.float64 or rho_out.numel() != 1 or not (f.is_contiguous() and truth.is_contiguous()):
+        raise ValueError("rho_out: one float64; f and truth contiguous")
+    if f.dtype not in (torch.float32, torch.float64):
+        raise TypeError(f"unsupported dtype {f.dtype}")
+    code = F32 if f.dtype == torch.float32 else F64
+    rc = lib().sgp_rel_error_static(_dev_ptr(f), _dev_ptr(truth), f.numel(), code, _dev_ptr(rho_out), _stream_ptr())
+    if rc and check:
+        raise SgpError(rc, lib().sgp_last_cuda_error().decode() or "sgp_rel_error_static")
+    return rc
 
 
 def sgp_single(g, psf, b, f0=None, opts=None, host=False, check=True, f_out=None):

@@ -72,6 +72,18 @@ def main():
     o = B.default_options(**{**w["opts"], "max_iter": 6, "stop_rule": 0})
     m, res = B.mosaic(B.ALG_SGP, [dev(a) for a in w["g"]], [dev(k) for k in w["psf"]], w["b"], 2, 2, (80, 80), opts=o)
     assert torch.isfinite(m).all()
+    # one-shot calls (the plan is kept between them, then released) and the entry point whose scratch is a static device array
+    w = synth.make("C0", n=64)
+    o = B.default_options(**{**w["opts"], "max_iter": 5})
+    for _ in range(2):
+        B.sgp_single(dev(w["g"][0]), dev(w["psf"][0]), w["b"][0], opts=o)
+    B.release_cached_plans()
+    rho = torch.zeros(1, dtype=torch.float64, device="cuda")
+    for n in (1000, 70000, 400000):
+        x = torch.rand(n, device="cuda") + 0.5
+        B.rel_error_static(x, x + 0.1, rho)
+        B.rel_error_static(x + 0.1, x, rho)
+        assert 0.0 < float(rho.item()) < 1.0
     torch.cuda.synchronize()
     print("sanitize tour ok")
 
