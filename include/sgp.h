@@ -100,7 +100,9 @@ typedef struct sgp_options {
     int strict;                                  /* A17: 1 = negative g is SGP_ERR_DATA instead of being clamped to 0 */
     int check_every;                             /* iterations enqueued between two host reads of the device status; 0 = auto */
     int tile_cols;                               /* tuning: spectrum tile width in columns (power of 2); 0 = auto */
-    int rows_per_block;                          /* tuning: rows per CTA in the row-FFT kernels (power of 2); 0 = auto */
+    int rows_per_block;                          /* tuning: rows per CTA in the row-FFT kernels (power of 2); 0 = auto (depends on the grid and, for small
+                                                    grids, on the number of problems of a batched plan; reductions are summed per CTA, so two plans agree
+                                                    bit for bit only with equal rows_per_block) */
     int use_graph;                               /* bit 0 (default 1) = replay the iterations as CUDA graphs of 10 (kept across runs of a plan), else
                                                     plain stream launches; the only bit that may differ per run.  Experiment switches (plan level):
                                                     bit 1 = persistent column kernel, bit 2 / bit 3 = force the separate / the fused line-search

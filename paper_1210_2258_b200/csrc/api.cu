@@ -39,7 +39,7 @@ static int pad_len(int L, int E) { return L + (L >> (E == 32 ? 5 : 4)); }
 static int row_len(int L, int E) { return (pad_len(L, E) + 1) & ~1; }      // fft_core.cuh: row_stride
 
 // Spectrum tile width C (columns per CTA of the column kernel) and rows per CTA of the row kernels.
-int choose_tiles(int ny, int nx, int dtype, const sgp_options *opt, int *C_out, int *RB_out)
+int choose_tiles(int ny, int nx, int dtype, const sgp_options *opt, int *C_out, int *RB_out, int nb)
 {
     const int esz = dtype == SGP_F64 ? 16 : 8;                     // bytes per complex number
     const int Lr = nx / 2, Lc = ny;
@@ -52,6 +52,10 @@ int choose_tiles(int ny, int nx, int dtype, const sgp_options *opt, int *C_out, 
     if (C > 32) C = 32;
     while (C > 1 && (size_t)C * pad_len(Lc, Ec) * esz > 72 * 1024) C /= 2;
     while (C > 1 && Lr % C != 0) C /= 2;
+    // small grids: at least 32 tiles as long as a tile keeps 8 columns (full 64-byte pieces of a spectrum row in fp32) -- a 256^2
+    // problem on 4 CTAs of 32 columns is latency-bound on 4 of 148 SMs (measured, 256^2: K2 / K5 14.9 / 14.2 -> 10.8 / 10.7 us;
+    // same rule in col.cuh: col_default_C, for square grids)
+    while (C > 8 && Lr / C < 32) C /= 2;
     if (opt && opt->tile_cols > 0) {
         if (!is_pow2(opt->tile_cols) || Lr % opt->tile_cols != 0) return SGP_ERR_ARG;
         C = opt->tile_cols;
@@ -63,6 +67,11 @@ int choose_tiles(int ny, int nx, int dtype, const sgp_options *opt, int *C_out, 
     const int TFg = group_threads(TFr);
     int RB = floor_pow2(256 / TFg > 1 ? 256 / TFg : 1);
     if (RB > 32) RB = 32;
+    // small grids: enough row CTAs for two per SM (148 SMs) over all nb problems, as long as a CTA keeps 8 rows (one 256^2 problem:
+    // 8 CTAs of 32 rows -> 32 of 8, with the tile rule above 19.7 -> 27.6 kit/s; 512^2: 18.3 -> 22.8 kit/s); a batched plan of 64
+    // problems fills the GPU through blockIdx.z and keeps the larger CTAs (RB = 8 there: -6 %).  Sums are per CTA, so a batched and an
+    // ordinary plan agree bit for bit only when their rows_per_block are equal (set it explicitly where that matters).
+    while (RB > 8 && (long long)nb * (ny / RB) < 296 && ((RB / 2) * TFg) % 32 == 0) RB /= 2;
     if (opt && opt->rows_per_block > 0) {
         if (!is_pow2(opt->rows_per_block)) return SGP_ERR_ARG;
         RB = opt->rows_per_block;

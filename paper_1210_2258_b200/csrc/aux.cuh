@@ -187,6 +187,27 @@ __global__ void final_update_kernel(const T *f, const T *d, T *f_out, size_t n, 
     }
 }
 
+// addresses of the caller's arrays of a batched run (see embed_inputs_batched_kernel below)
+struct BatchTab {
+    const void *const *g, *const *b, *const *f0;
+    void *const *f_out;
+};
+template <typename T>
+__global__ void final_update_batched_kernel(BatchTab tab, const T *f, const T *d, size_t n, const Ctrl *ct, size_t slab)
+{
+    const size_t off = (size_t)blockIdx.z * slab;
+    const Ctrl *ctz = bshift(ct, off);
+    const T *fz = bshift(f, off), *dz = bshift(d, off);
+    T *f_out = (T *)tab.f_out[blockIdx.z];
+    const bool pend = ctz->pending != 0;
+    const T lam = (T)ctz->lambda;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
+        T v = fz[i];
+        if (pend) v = v + lam * dz[i];
+        f_out[i] = v;
+    }
+}
+
 // ---------------------------------------------------------------- set-up and marshalling kernels (not on the hot path)
 // sum of a plane (PSF volume) with a non-finite check -> ct->psf_sum; single CTA
 template <typename T>
@@ -230,8 +251,8 @@ __global__ void khat_fixup_kernel(const cx<T> *raw, cx<T> *khat, cx<T> *khatB, i
 // g_j, b_j (sy x sx, caller's arrays) -> S-bar planes; negative g clamped to 0 (A17) or flagged (strict);
 // also sum_S (g - b) for the constant start (A14), accumulated per block into part[] (deterministic final sum later)
 template <typename T>
-__global__ void embed_inputs_kernel(const T *g, const T *b, T *G_out, T *B_out, Geom Gm, double bconst, int strict,
-                                    Ctrl *ct, double *part)
+__device__ __forceinline__ void embed_inputs_body(const T *g, const T *b, T *G_out, T *B_out, const Geom &Gm, double bconst, int strict,
+                                                  Ctrl *ct, double *part)
 {
     __shared__ double red[32];
     const size_t n = (size_t)Gm.ny * Gm.nx;
@@ -255,6 +276,27 @@ __global__ void embed_inputs_kernel(const T *g, const T *b, T *G_out, T *B_out, 
     block_reduce_sum<1>(acc, red);
     if (threadIdx.x == 0) part[blockIdx.x] = acc[0];
 }
+template <typename T>
+__global__ void embed_inputs_kernel(const T *g, const T *b, T *G_out, T *B_out, Geom Gm, double bconst, int strict,
+                                    Ctrl *ct, double *part)
+{
+    embed_inputs_body<T>(g, b, G_out, B_out, Gm, bconst, strict, ct, part);
+}
+
+// Batched plans (sgp_plan_run_batched): the set-up kernels of ALL problems in one launch each, blockIdx.z = problem (and
+// blockIdx.y = image where there is one).  The caller's arrays are separate allocations, so their addresses come from a table in
+// device memory: [g: nb*p][b: nb*p][f0: nb][f_out: nb]; the plan's own per-problem arrays are `slab` bytes apart (ew.cuh).
+template <typename T>
+__global__ void embed_inputs_batched_kernel(BatchTab tab, T *Gp, T *Bp, Geom Gm, int p, int b_is_array, int strict,
+                                            Ctrl *ct, double *part_misc, size_t slab)
+{
+    const int j = blockIdx.y, z = blockIdx.z;
+    const size_t n = (size_t)Gm.ny * Gm.nx, off = (size_t)z * slab;
+    Ctrl *ctz = bshift(ct, off);
+    embed_inputs_body<T>((const T *)tab.g[z * p + j], b_is_array ? (const T *)tab.b[z * p + j] : nullptr, bshift(Gp, off) + (size_t)j * n,
+                         b_is_array ? bshift(Bp, off) + (size_t)j * n : nullptr, Gm, ctz->bconst[j], strict, ctz,
+                         bshift(part_misc, off) + (size_t)j * 1024);
+}
 
 // c = max(0, (1/p) sum_j mean_S (g_j - b_j)) (A14); single thread, partials in fixed order.  Also the flux of the
 // flux-constrained projection (A26): flux_value if > 0, else max(0, (1/p) sum_j sum_S (g_j - b_j)).
@@ -270,9 +312,24 @@ template <typename T> __global__ void const_start_kernel(const double *part, int
     }
 }
 
+template <typename T> __global__ void const_start_batched_kernel(const double *part_misc, int nparts, double denom, int p, double flux_value, Ctrl *ct, size_t slab)
+{
+    if (threadIdx.x == 0 && blockIdx.x == 0) {
+        const size_t off = (size_t)blockIdx.z * slab;
+        const double *part = bshift(part_misc, off);
+        Ctrl *ctz = bshift(ct, off);
+        double s = 0.0;
+        for (int i = 0; i < nparts; ++i) s += part[i];
+        double c = s / denom;
+        ctz->c0 = c < 0.0 ? 0.0 : c;
+        double fc = flux_value > 0.0 ? flux_value : s / (double)p;
+        ctz->flux_c = fc < 0.0 ? 0.0 : fc;
+    }
+}
+
 // start point f(0): user image / constant / zero / g_1, restricted to R (A11)
 template <typename T>
-__global__ void start_point_kernel(T *f, const T *f0, const T *g0, const T *alphaR, Geom Gm, int init, Ctrl *ct)
+__device__ __forceinline__ void start_point_body(T *f, const T *f0, const T *g0, const T *alphaR, const Geom &Gm, int init, Ctrl *ct)
 {
     const size_t n = (size_t)Gm.ny * Gm.nx;
     int flag = 0;
@@ -290,6 +347,17 @@ __global__ void start_point_kernel(T *f, const T *f0, const T *g0, const T *alph
         f[i] = v;
     }
     if (flag) atomicOr(&ct->flag_data, flag);
+}
+template <typename T>
+__global__ void start_point_kernel(T *f, const T *f0, const T *g0, const T *alphaR, Geom Gm, int init, Ctrl *ct)
+{
+    start_point_body<T>(f, f0, g0, alphaR, Gm, init, ct);
+}
+template <typename T>
+__global__ void start_point_batched_kernel(BatchTab tab, T *f, const T *Gp, const T *alphaR, Geom Gm, int init, Ctrl *ct, size_t slab)
+{
+    const size_t off = (size_t)blockIdx.z * slab;
+    start_point_body<T>(bshift(f, off), init == SGP_INIT_USER ? (const T *)tab.f0[blockIdx.z] : nullptr, bshift(Gp, off), alphaR, Gm, init, bshift(ct, off));
 }
 
 // boundary weights (Eq.19-20): alpha += alpha_j; M_R &= (alpha_j >= sigma)

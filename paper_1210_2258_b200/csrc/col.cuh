@@ -77,6 +77,7 @@ template <typename T> __host__ __device__ constexpr int col_default_C(int L)
     int C = 1;
     while (2 * C <= (col_max / TF > 1 ? col_max / TF : 1) && 2 * C <= 32) C *= 2;
     while (C > 1 && (size_t)C * fft_padded_len(L, E) * sizeof(cx<T>) > 72 * 1024) C /= 2;
+    while (C > 8 && (L / 2) / C < 32) C /= 2;          // small grids (api.cu: choose_tiles), assuming nx = ny
     return C;
 }
 

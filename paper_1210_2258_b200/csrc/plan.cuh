@@ -50,7 +50,7 @@ struct PlanBase {
 };
 
 int validate_options(const sgp_options *o);
-int choose_tiles(int ny, int nx, int dtype, const sgp_options *opt, int *C, int *RB);
+int choose_tiles(int ny, int nx, int dtype, const sgp_options *opt, int *C, int *RB, int nb = 1);
 size_t workspace_bytes(int kind, int p, int ny, int nx, int dtype);
 PlanBase *make_plan_f32();
 PlanBase *make_plan_f64();

@@ -38,6 +38,7 @@ template <typename T> struct PlanImpl : PlanBase {
     double *part_fx = nullptr, *part_err = nullptr;
     size_t fx_chunks = 0, fx_batches = 1;
     C *khatB_tmp = nullptr;        // companion line of the Gaussian's transfer function (smoothed constant start)
+    const void **ptrtab = nullptr;  // batched plans: addresses of the caller's arrays of a run (aux.cuh: BatchTab), 2 nb p + 2 nb entries
     // per-run trace buffers
     double *trJ = nullptr, *trA = nullptr, *trL = nullptr, *fA = nullptr, *fL = nullptr, *trE = nullptr;
     int *trR = nullptr, *trB = nullptr;
@@ -184,7 +185,7 @@ template <typename T> struct PlanImpl : PlanBase {
         for (int m = 0; m < RF_NMODES; ++m) if (!(k_rowf[m] = get_row_fwd<T>(Lr, m, G.masked != 0))) return SGP_ERR_ARG;
         for (int m = 0; m < RI_NMODES; ++m) if (!(k_rowi[m] = get_row_inv<T>(Lr, m, G.masked != 0))) return SGP_ERR_ARG;
         int Cc = 0, RB = 0;
-        int rc = choose_tiles(ny, nx, dtype, &opt, &Cc, &RB);
+        int rc = choose_tiles(ny, nx, dtype, &opt, &Cc, &RB, nb);
         if (rc) return rc;
         const bool multi = p > 1;
         // batched plans (nb > 1) use the column kernels compiled with the per-problem offset (col.cuh: BATCH), asked for by a negative width
@@ -308,6 +309,7 @@ template <typename T> struct PlanImpl : PlanBase {
         if ((rc = dalloc(&part_fx, 3 * fx_chunks))) return rc;
         if ((rc = dalloc(&part_err, (size_t)2 * 1184))) return rc;
         if ((rc = dalloc(&khatB_tmp, (size_t)ny))) return rc;
+        if (nb > 1 && (rc = dalloc(&ptrtab, (size_t)2 * nb * p + 2 * (size_t)nb))) return rc;
         if ((rc = commit_allocs())) return rc;
         for (int b = 0; b < nb; ++b) SGP_CUDA_TRY(cudaMemset(bshift_host(ct, (size_t)b * slab), 0, sizeof(Ctrl)));
         SGP_CUDA_TRY(cudaEventCreate(&ev0));

@@ -344,7 +344,33 @@ int PlanImpl<T>::run_batched(int algorithm, const void *const *g, const void *co
         h.alpha_prev = ro.alpha0; h.tau = ro.tau1; h.L1 = ro.L1; h.L2 = ro.L2; h.lambda = 1.0;
         h.qsel = 0; h.need_k1 = 1; h.accepted = 1;
         for (int j = 0; j < p; ++j) h.bconst[j] = bconst_all[(size_t)b * kMaxP + j];
-        SGP_CUDA_TRY(cudaMemcpyAsync(pp(ct, b), &h, sizeof(Ctrl), cudaMemcpyHostToDevice, st));
+    }
+    BatchTab tab;
+    memset(&tab, 0, sizeof(tab));
+    if (nb > 1) {
+        // Batched plans: one copy, one memset and one launch per set-up step for ALL problems (blockIdx.z = problem), not one per
+        // problem -- with 64 problems of 256^2 the per-problem form spent 5.3 ms in ~600 small copies and launches, as much as
+        // 30 of the 100 iterations that followed.  The addresses of the caller's arrays go to the device as one table.
+        std::vector<const void *> th((size_t)2 * nb * p + 2 * (size_t)nb, nullptr);
+        for (int i = 0; i < nb * p; ++i) { th[i] = g[i]; th[(size_t)nb * p + i] = b_is_array ? b_arr[i] : nullptr; }
+        for (int b = 0; b < nb; ++b) { th[(size_t)2 * nb * p + b] = f0 ? f0[b] : nullptr; th[(size_t)2 * nb * p + nb + b] = f_out[b]; }
+        SGP_CUDA_TRY(cudaMemcpyAsync(ptrtab, th.data(), th.size() * sizeof(void *), cudaMemcpyHostToDevice, st));
+        tab.g = ptrtab; tab.b = ptrtab + (size_t)nb * p; tab.f0 = ptrtab + (size_t)2 * nb * p;
+        tab.f_out = (void *const *)(ptrtab + (size_t)2 * nb * p + nb);
+        SGP_CUDA_TRY(cudaMemcpy2DAsync(ct, slab, hs.data(), sizeof(Ctrl), sizeof(Ctrl), (size_t)nb, cudaMemcpyHostToDevice, st));
+        SGP_CUDA_TRY(cudaMemset2DAsync(q + n * (size_t)p, slab, 0, sizeof(T) * n * (size_t)p, (size_t)nb, st));     // second q buffers: zero outside S
+        embed_inputs_batched_kernel<T><<<dim3(eg, p, nb), 256, 0, st>>>(tab, Gp, b_is_array ? Bp : nullptr, G, p, b_is_array, ro.strict, ct, part_misc, slab);
+        launches++;
+        if (eg < 1024)
+            for (int j = 0; j < p; ++j)
+                SGP_CUDA_TRY(cudaMemset2DAsync(part_misc + (size_t)j * 1024 + eg, slab, 0, sizeof(double) * (1024 - eg), (size_t)nb, st));
+        const_start_batched_kernel<T><<<dim3(1, 1, nb), 32, 0, st>>>(part_misc, 1024 * p, o.nS_total, p, ro.flux_value, ct, slab);
+        launches++;
+        start_point_batched_kernel<T><<<dim3(ew_grid(n), 1, nb), 256, 0, st>>>(tab, f, Gp, alphaR, G, ro.init == SGP_INIT_CONST_SMOOTH ? SGP_INIT_CONST : ro.init, ct, slab);
+        launches++;
+    } else {
+        const int b = 0;
+        SGP_CUDA_TRY(cudaMemcpyAsync(pp(ct, b), &hs[b], sizeof(Ctrl), cudaMemcpyHostToDevice, st));
         SGP_CUDA_TRY(cudaMemsetAsync(pp(q, b) + n * (size_t)p, 0, sizeof(T) * n * (size_t)p, st));     // second q buffer: zero outside S
         for (int j = 0; j < p; ++j) {
             embed_inputs_kernel<T><<<eg, 256, 0, st>>>((const T *)g[b * p + j], b_is_array ? (const T *)b_arr[b * p + j] : nullptr,
@@ -428,8 +454,9 @@ int PlanImpl<T>::run_batched(int algorithm, const void *const *g, const void *co
         if (status[b] != hs[b].status) SGP_CUDA_TRY(cudaMemcpyAsync(&pp(ct, b)->status, &status[b], sizeof(int), cudaMemcpyHostToDevice, st));
 
     if (algorithm == SGP_ALG_SGP) {     // arguments of the Armijo backtracking (aux.cuh), read from device memory
+        std::vector<BtInfo<T>> bis((size_t)nb);
         for (int b = 0; b < nb; ++b) {
-            BtInfo<T> bi;
+            BtInfo<T> &bi = bis[b];
             memset(&bi, 0, sizeof(bi));
             bi.G = G; bi.o = o; bi.ct = pp(ct, b); bi.q = pp(q, b); bi.u = pp(u, b); bi.g = pp(Gp, b); bi.b = pp(Bp, b); bi.qbuf = n * (size_t)p;
             bi.tr = tr;
@@ -439,8 +466,9 @@ int PlanImpl<T>::run_batched(int algorithm, const void *const *g, const void *co
             bi.b_is_array = b_is_array; bi.nchunks = (unsigned int)bt_chunks; bi.chunk_batches = (unsigned int)bt_batches;
             bi.part = pp(part_bt, b); bi.sync = pp(btsync, b);
             for (int j = 0; j < p; ++j) bi.bconst[j] = bconst_all[(size_t)b * kMaxP + j];
-            SGP_CUDA_TRY(cudaMemcpyAsync(pp(btinfo, b), &bi, sizeof(bi), cudaMemcpyHostToDevice, st));
         }
+        // all blocks in one strided copy
+        SGP_CUDA_TRY(cudaMemcpy2DAsync(btinfo, slab ? slab : sizeof(BtInfo<T>), bis.data(), sizeof(BtInfo<T>), sizeof(BtInfo<T>), (size_t)nb, cudaMemcpyHostToDevice, st));
     }
     // ---- iteration loop
     if (any_running()) {
@@ -504,12 +532,36 @@ int PlanImpl<T>::run_batched(int algorithm, const void *const *g, const void *co
         }
     }
     SGP_CUDA_TRY(cudaEventRecord(ev2, st));
-    for (int b = 0; b < nb; ++b) {
-        final_update_kernel<T><<<ew_grid(n), 256, 0, st>>>(pp(f, b), pp(d, b), (T *)f_out[b], n, pp(ct, b));     // a10: the last accepted step, if still pending
+    if (nb > 1) {
+        final_update_batched_kernel<T><<<dim3(ew_grid(n), 1, nb), 256, 0, st>>>(tab, f, d, n, ct, slab);     // a10: the last accepted step, if still pending
+        launches++;
+    } else {
+        final_update_kernel<T><<<ew_grid(n), 256, 0, st>>>(f, d, (T *)f_out[0], n, ct);
         launches++;
     }
     SGP_CUDA_TRY(cudaGetLastError());
-    for (int b = 0; b < nb; ++b) {
+    // traces: batched plans bring every trace array of all problems to the host in ONE strided copy and hand the rows out from there
+    int kmax = 0;
+    for (int b = 0; b < nb; ++b) if (hs[b].k > kmax) kmax = hs[b].k;
+    struct TraceCopy { void *dev; size_t elem; int extra; bool any; std::vector<unsigned char> host; };
+    TraceCopy tcs[6] = {{trJ, sizeof(double), 1, false, {}}, {tr.err ? trE : nullptr, sizeof(double), 2, false, {}}, {trA, sizeof(double), 0, false, {}},
+                        {trL, sizeof(double), 0, false, {}}, {trR, sizeof(int), 0, false, {}}, {trB, sizeof(int), 0, false, {}}};
+    auto wanted = [&](const sgp_result &R, int i) -> void * {
+        switch (i) { case 0: return R.trace_J; case 1: return R.trace_err; case 2: return R.trace_alpha; case 3: return R.trace_lambda;
+                     case 4: return R.trace_rule; default: return R.trace_backtracks; }
+    };
+    if (nb > 1) {
+        for (int i = 0; i < 6; ++i) {
+            TraceCopy &t = tcs[i];
+            if (!t.dev) continue;
+            for (int b = 0; b < nb; ++b) if (wanted(res[b], i) && hs[b].k + t.extra > 0) t.any = true;
+            if (!t.any) continue;
+            const size_t width = t.elem * (size_t)(kmax + t.extra);
+            t.host.resize(width * (size_t)nb);
+            SGP_CUDA_TRY(cudaMemcpy2DAsync(t.host.data(), width, t.dev, tr_slab, width, (size_t)nb, cudaMemcpyDeviceToHost, st));
+        }
+    } else {
+        const int b = 0;
         const int kdone = hs[b].k;
         const size_t to = (size_t)b * tr_slab;
         sgp_result &R = res[b];
@@ -523,6 +575,18 @@ int PlanImpl<T>::run_batched(int algorithm, const void *const *g, const void *co
         }
     }
     SGP_CUDA_TRY(cudaStreamSynchronize(st));
+    if (nb > 1) {
+        for (int i = 0; i < 6; ++i) {
+            const TraceCopy &t = tcs[i];
+            if (!t.any) continue;
+            const size_t width = t.elem * (size_t)(kmax + t.extra);
+            for (int b = 0; b < nb; ++b) {
+                void *dst = wanted(res[b], i);
+                const int cnt = hs[b].k + t.extra;
+                if (dst && cnt > 0) memcpy(dst, t.host.data() + (size_t)b * width, t.elem * (size_t)cnt);
+            }
+        }
+    }
     if (profiling) prof_collect();
     float ms01 = 0.f, ms12 = 0.f;
     cudaEventElapsedTime(&ms01, ev0, ev1);
