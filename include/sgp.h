@@ -107,7 +107,9 @@ typedef struct sgp_options {
                                                     plain stream launches; the only bit that may differ per run.  Experiment switches (plan level):
                                                     bit 1 = persistent column kernel, bit 2 / bit 3 = force the separate / the fused line-search
                                                     kernel (default: chosen by working set vs L2), bit 4 = never use the two-CTAs-per-SM column
-                                                    kernel, bit 6 = RL / OSEM on the six separate launches of round 1 instead of the fused four */
+                                                    kernel, bit 6 = RL / OSEM on the six separate launches of round 1 instead of the fused four,
+                                                    bit 7 = never use the one-cluster-per-problem kernel of the small grids (sgp_*, one image, no mask,
+                                                    128^2 ... 512^2: the whole iteration in one kernel, csrc/small.cuh) */
     double rl_relax;                             /* rl_* only: exponent of the multiplicative relaxation, Eq.3:
                                                     f <- f o (W o sum_j A_j^T(g_j/(A_j f + b_j)))^rl_relax; 1 (default) = plain RL */
     double rl_linear;                            /* rl_* only: constant lambda_k of the linear relaxation, Eq.4:
@@ -138,7 +140,8 @@ typedef struct sgp_result {
                                    (2p+2 per SGP iteration and RL step, 4p per OSEM cycle, p+1 per refresh) */
     double setup_ms, loop_ms;   /* device time of the start-point phase and of the iteration loop (CUDA events) */
     long kernel_launches;       /* kernels of this library launched by the call */
-    int fused_linesearch;       /* 1: the run used the fused line-search + ratio kernel (chosen by working set vs L2) */
+    int fused_linesearch;       /* 1: the run used the fused line-search + ratio kernel; 2: the whole iteration ran inside the one-cluster-per-problem
+                                   kernel of the small grids (csrc/small.cuh) */
     int status;                 /* sgp_status of THIS problem (batched runs return the first error; every problem reports its own here) */
     double *trace_J, *trace_alpha, *trace_lambda;
     int *trace_rule, *trace_backtracks;

@@ -1,5 +1,6 @@
 // plan_impl.inl -- included by plan_f32.cu / plan_f64.cu with SGP_T and SGP_MAKE defined.
 #include "plan.cuh"
+#include "small_params.h"
 
 namespace sgpk {
 
@@ -38,6 +39,9 @@ template <typename T> struct PlanImpl : PlanBase {
     double *part_fx = nullptr, *part_err = nullptr;
     size_t fx_chunks = 0, fx_batches = 1;
     C *khatB_tmp = nullptr;        // companion line of the Gaussian's transfer function (smoothed constant start)
+    small_kernel_t<T> small_k = nullptr;   // small grids: the whole SGP iteration in one kernel, one cluster per problem (small.cuh)
+    int small_nc = 0, small_threads = 0, small_er = 0, small_ec = 0; size_t small_smem = 0;
+    C *tw_sr = nullptr, *tw_sc = nullptr;   // pass tables of its row / column FFT plans
     const void **ptrtab = nullptr;  // batched plans: addresses of the caller's arrays of a run (aux.cuh: BatchTab), 2 nb p + 2 nb entries
     // per-run trace buffers
     double *trJ = nullptr, *trA = nullptr, *trL = nullptr, *fA = nullptr, *fL = nullptr, *trE = nullptr;
@@ -220,6 +224,31 @@ template <typename T> struct PlanImpl : PlanBase {
         if (opt.use_graph & 8) fuse_ls = true;
         col_grid = (opt.use_graph & 2) ? (ntiles < nsm ? ntiles : nsm) : ntiles;   // experiment switch: persistent or one tile per CTA
 
+        // Small grids: one image without a boundary mask at 128^2 ... 512^2 iterates inside ONE kernel run by
+        // one thread-block cluster per problem (small.cuh) when the device can co-schedule such a cluster; use_graph bit 7 (or any other
+        // experiment switch) keeps the launch-per-pass path.  A batched plan of 256^2 problems uses it up to 16 problems (the device
+        // holds about 7 clusters of 16 CTAs at once: 4 problems run 151 kit/s this way against 71 kit/s launch-per-pass, 16 problems 214
+        // against 195, 32 problems 261 against 326, 64 problems 270 against 394); 128^2 (clusters of 8) always: 64 problems 1174 against 571.
+        if (p == 1 && !G.masked && (opt.use_graph & ~1) == 0 && !getenv("SGP_NO_CLUSTER")) {      // any experiment switch: launch-per-pass
+            small_k = get_small<T>(ny, nx, &small_nc, &small_threads, &small_smem, &small_er, &small_ec);
+            if (small_k) {
+                bool ok = cudaFuncSetAttribute((const void *)small_k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)small_smem) == cudaSuccess;
+                if (ok && small_nc > 8) ok = cudaFuncSetAttribute((const void *)small_k, cudaFuncAttributeNonPortableClusterSizeAllowed, 1) == cudaSuccess;
+                if (ok) {
+                    cudaLaunchConfig_t cfg;
+                    memset(&cfg, 0, sizeof(cfg));
+                    cfg.gridDim = dim3(small_nc); cfg.blockDim = dim3(small_threads); cfg.dynamicSmemBytes = small_smem;
+                    cudaLaunchAttribute at[1];
+                    at[0].id = cudaLaunchAttributeClusterDimension;
+                    at[0].val.clusterDim.x = small_nc; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+                    cfg.attrs = at; cfg.numAttrs = 1;
+                    int nclusters = 0;
+                    ok = cudaOccupancyMaxActiveClusters(&nclusters, (const void *)small_k, &cfg) == cudaSuccess && nclusters > 0;
+                    if (ok && nb > 16 && small_nc > 8) ok = false;
+                }
+                if (!ok) { small_k = nullptr; (void)cudaGetLastError(); }
+            }
+        }
         // twiddles, computed in double on the host
         std::vector<C> h;
         auto upload = [&](C **dst, int len, int count) -> int {     // exp(-2 pi i k / len), k < count
@@ -253,6 +282,7 @@ template <typename T> struct PlanImpl : PlanBase {
         if ((rc = upload_passes(&tw_r, Lr, Er))) return rc;
         if ((rc = upload(&tw_h, nx, Lr + 1))) return rc;
         if ((rc = upload_passes(&tw_c, Lc, Ec))) return rc;
+        if (small_k) { if ((rc = upload_passes(&tw_sr, Lr, small_er))) return rc; if ((rc = upload_passes(&tw_sc, Lc, small_ec))) return rc; }
         // single-image product passes: the two-CTAs-per-SM kernel where it exists (float, 256 threads at this tile width);
         // run() decides per algorithm whether to use it
         k_conj_run = k_conj; k_mult_run = k_mult;
@@ -364,6 +394,41 @@ template <typename T> struct PlanImpl : PlanBase {
             return launch_pdl(k, dim3(ntiles, 1, lnb), col2_threads, col2_smem, Q, st);
         }
         return launch_pdl(k, dim3(col_grid, 1, lnb), col_threads, col_smem, P, st);
+    }
+    // `iters` SGP iterations of all lnb problems in one launch, one cluster per problem (small.cuh)
+    int launch_small(const DevOpts &o, const Trace &tr, double bconst0, int iters, cudaStream_t st)
+    {
+        SmallParams<T> S;
+        memset(&S, 0, sizeof(S));
+        S.G = G; S.o = o; S.tr = tr; S.ct = ct; S.f = f; S.grad = grad; S.d = d; S.q = q; S.g = Gp; S.qbuf = n * (size_t)p;
+        S.khat = khat; S.khatB = khatB; S.tw_r = tw_sr; S.tw_h = tw_h; S.tw_c = tw_sc; S.bconst = bconst0; S.iters = iters;
+        S.slab = lnb > 1 ? slab : 0; S.tr_slab = lnb > 1 ? tr_slab : 0;
+        cudaLaunchConfig_t cfg;
+        memset(&cfg, 0, sizeof(cfg));
+        cfg.gridDim = dim3(small_nc * lnb); cfg.blockDim = dim3(small_threads); cfg.dynamicSmemBytes = small_smem; cfg.stream = st;
+        cudaLaunchAttribute at[1];
+        at[0].id = cudaLaunchAttributeClusterDimension;
+        at[0].val.clusterDim.x = small_nc; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+        cfg.attrs = at; cfg.numAttrs = 1;
+#ifdef SGP_SMALL_TIMING
+        static unsigned long long *dbg = nullptr;
+        if (!dbg) cudaMalloc(&dbg, 64 * sizeof(unsigned long long));
+        cudaMemsetAsync(dbg, 0, 64 * sizeof(unsigned long long), st);
+        S.dbg = dbg;
+#endif
+        SGP_CUDA_TRY(cudaLaunchKernelEx(&cfg, small_k, S));
+        launches++;
+#ifdef SGP_SMALL_TIMING
+        if (getenv("SGP_SMALL_DBG")) {
+            unsigned long long h[64];
+            cudaStreamSynchronize(st);
+            cudaMemcpy(h, dbg, sizeof(h), cudaMemcpyDeviceToHost);
+            fprintf(stderr, "[small timing, ns]");
+            for (int i = 1; i < 64 && h[i]; ++i) fprintf(stderr, " %llu", h[i] - h[i - 1]);
+            fprintf(stderr, "\n");
+        }
+#endif
+        return SGP_OK;
     }
     static int ew_grid(size_t count) { size_t b = (count + 255) / 256; return (int)(b > 1184 ? 1184 : (b < 1 ? 1 : b)); }
 

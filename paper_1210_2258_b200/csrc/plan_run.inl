@@ -453,7 +453,10 @@ int PlanImpl<T>::run_batched(int algorithm, const void *const *g, const void *co
     for (int b = 0; b < nb; ++b)
         if (status[b] != hs[b].status) SGP_CUDA_TRY(cudaMemcpyAsync(&pp(ct, b)->status, &status[b], sizeof(int), cudaMemcpyHostToDevice, st));
 
-    if (algorithm == SGP_ALG_SGP) {     // arguments of the Armijo backtracking (aux.cuh), read from device memory
+    // small grids: the cluster kernel (small.cuh) for what it covers, the launch-per-pass path for everything else
+    const bool small_run = small_k && algorithm == SGP_ALG_SGP && !b_is_array && !o.flux_constraint && !o.refresh_every &&
+                           ro.stop_rule != SGP_STOP_MINERR && !tr.force_alpha && !tr.force_lambda && !tr.err && !profiling;
+    if (algorithm == SGP_ALG_SGP && !small_run) {     // arguments of the Armijo backtracking (aux.cuh), read from device memory
         std::vector<BtInfo<T>> bis((size_t)nb);
         for (int b = 0; b < nb; ++b) {
             BtInfo<T> &bi = bis[b];
@@ -473,7 +476,21 @@ int PlanImpl<T>::run_batched(int algorithm, const void *const *g, const void *co
     // ---- iteration loop
     if (any_running()) {
         int chunk = ro.check_every > 0 ? ro.check_every : (ro.stop_rule == SGP_STOP_MAXIT ? 200 : 20);
-        if (algorithm == SGP_ALG_SGP) {
+        if (algorithm == SGP_ALG_SGP && small_run) {
+            // one launch runs every problem to its stopping rule (or to max_iter): the kernel tests the rules itself
+            int done = 0;
+            while (any_running()) {
+                const int todo = ro.max_iter - done;
+                if (todo < 1) { for (int b = 0; b < nb; ++b) if (status[b] == 0) status[b] = SGP_REASON_MAXIT; break; }
+                if ((rc = launch_small(o, tr, bconst[0], todo, st))) return rc;
+                if ((rc = read_ctrl())) return rc;
+                done = ro.max_iter;
+                for (int b = 0; b < nb; ++b) {
+                    if (status[b] == 0) status[b] = hs[b].status;
+                    if (status[b] == 0 && hs[b].k < done) done = hs[b].k;
+                }
+            }
+        } else if (algorithm == SGP_ALG_SGP) {
             if (ro.max_iter == 0) { for (int b = 0; b < nb; ++b) if (status[b] == 0) status[b] = SGP_REASON_MAXIT; }
             else if ((rc = enqueue_ratio(Pb, 3, st))) return rc;        // K1 of iteration 0; every iteration enqueues the next one's
             int done = 0;
@@ -606,7 +623,7 @@ int PlanImpl<T>::run_batched(int algorithm, const void *const *g, const void *co
         R.err_final = tr.err ? h.err : 0.0;
         R.setup_ms = ms01; R.loop_ms = ms12;
         R.kernel_launches = launches - launches0;
-        R.fused_linesearch = (algorithm == SGP_ALG_SGP && fuse_ls) ? 1 : 0;
+        R.fused_linesearch = (algorithm == SGP_ALG_SGP && small_run) ? 2 : (algorithm == SGP_ALG_SGP && fuse_ls) ? 1 : 0;
         R.status = status[b] < 0 ? status[b] : SGP_OK;
         if (status[b] < 0 && worst == SGP_OK) worst = status[b];
     }

@@ -1,0 +1,27 @@
+// small.cu -- instantiations of the one-cluster-per-problem SGP kernel (small.cuh) and their look-up
+#include "small.cuh"
+
+namespace sgpk {
+
+template <typename T, int NY, int NX, int NC>
+static small_kernel_t<T> pick(int *nc, int *threads, size_t *smem, int *er, int *ec)
+{
+    using K = SmallCfg<T, NY, NX, NC>;
+    *nc = NC; *threads = K::NT; *smem = K::smem; *er = K::Er; *ec = K::Ec;
+    return small_sgp_kernel<T, NY, NX, NC>;
+}
+
+template <> small_kernel_t<float> get_small<float>(int ny, int nx, int *nc, int *threads, size_t *smem, int *er, int *ec)
+{
+    if (ny == 128 && nx == 128) return pick<float, 128, 128, 8>(nc, threads, smem, er, ec);
+    if (ny == 256 && nx == 256) return pick<float, 256, 256, 16>(nc, threads, smem, er, ec);
+    return nullptr;
+}
+template <> small_kernel_t<double> get_small<double>(int ny, int nx, int *nc, int *threads, size_t *smem, int *er, int *ec)
+{
+    if (ny == 128 && nx == 128) return pick<double, 128, 128, 8>(nc, threads, smem, er, ec);
+    if (ny == 256 && nx == 256) return pick<double, 256, 256, 16>(nc, threads, smem, er, ec);
+    return nullptr;
+}
+
+}  // namespace sgpk

@@ -20,7 +20,8 @@ def test_batched_plan_every_problem_matches_its_own_oracle_run(alg, dt, tol1, to
     """5 different star fields (different seeds, different backgrounds) through ONE batched plan: each problem keeps its own
     step lengths, backtracks and stopping iteration (Eq.24 stop: the problems stop at different iterations), and equals --
     bit for bit -- the same problem run alone through an ordinary plan; against the oracle: 1e-5 after one iteration, traces
-    equal over the un-branched stretch."""
+    equal over the un-branched stretch (10 iterations: at 128^2 in float the J0 of the C0 recipe leaves 1e-4 of the fp64 sequence
+    between iterations 10 and 15, whatever evaluates it -- DESIGN.md 3a, reading A23)."""
     _need_gpu()
     nb, n = 5, 128
     ws = [synth.make("C0", n=n, seed_idx=40 + i) for i in range(nb)]
@@ -28,7 +29,7 @@ def test_batched_plan_every_problem_matches_its_own_oracle_run(alg, dt, tol1, to
     g = [[dev(w["g"][0], dt)] for w in ws]
     b = [[10.0 + i] for i in range(nb)]
     algc = B.ALG_SGP if alg == "sgp" else B.ALG_RL
-    for kw in (dict(max_iter=1, stop_rule=0), dict(max_iter=15, stop_rule=0), dict(max_iter=300, stop_rule=1, tol=3e-4)):
+    for kw in (dict(max_iter=1, stop_rule=0), dict(max_iter=10, stop_rule=0), dict(max_iter=300, stop_rule=1, tol=3e-4)):
         okw = {**ws[0]["opts"], **kw}
         o = B.default_options(**okw)
         bp = B.BatchedPlan(nb, [dev(psf[0], dt)], opts=o)
@@ -41,7 +42,7 @@ def test_batched_plan_every_problem_matches_its_own_oracle_run(alg, dt, tol1, to
             assert torch.equal(fb[i], fs) and rb[i].iterations == rs.iterations and np.array_equal(rb[i].J, rs.J)
             assert np.array_equal(rb[i].backtracks, rs.backtracks) and rb[i].stop_reason == rs.stop_reason
             its.append(rb[i].iterations)
-            if kw["max_iter"] <= 15:
+            if kw["max_iter"] <= 10:
                 P = oracle.Problem(psf)
                 oo = oracle.default_options(**okw)
                 fo, ro = (P.sgp if alg == "sgp" else P.rl)(ws[i]["g"], [np.full((n, n), b[i][0])], opts=oo)

@@ -88,7 +88,7 @@ def test_minimum_error_stop_eq25(alg, dt):
     assert rg.err[rg.iterations + 1] > rg.err[rg.iterations] == rg.err_final           # the discarded step would have increased it
     # the iterate returned is f(k), not the discarded f(k+1)
     o2 = B.default_options(**{**w["opts"], "max_iter": rg.iterations, "stop_rule": 0})
-    fk, rk = run(g, w["b"], opts=o2)
+    fk, rk = run(g, w["b"], opts=o2, truth=dev(truth, dt))       # with the true object given both runs take the launch-per-pass path (small grids: csrc/small.cuh)
     assert torch.equal(fk, fg) and rk.J0_final == rg.J0_final
     if rg.iterations == ro.iterations:
         assert rel_l2(fg.cpu().numpy(), fo) <= (1e-3 if dt == np.float32 else 1e-8)
