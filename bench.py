@@ -372,15 +372,17 @@ def measure_other(name: str, alg_name: str, steps: int, dev, peak: float):
 
 
 def measure_batched(nb: int, steps: int, dev):
-    """nb problems of the C0 recipe (256^2, different seeds) through ONE batched plan (every kernel launched
-    once for all problems, blockIdx.z = problem) beside one C0 problem through an ordinary plan: aggregate iterations/s"""
+    """problems of the C0 recipe (256^2, different seeds) through ONE batched plan beside one C0 problem
+    through an ordinary plan: aggregate iterations/s.  One problem and small batches (<= 16) run one thread-block cluster per
+    problem (csrc/small.cuh, `path` = cluster); the large batch runs launch-per-pass, every kernel launched once for all problems
+    (blockIdx.z = problem)"""
     import torch
     from paper_1210_2258_b200 import binding as B, synth
     ws = [synth.c0_stars_gaussian(256, seed_idx=200 + i) for i in range(nb)]
     to_dev = lambda a: torch.as_tensor(np.ascontiguousarray(a, dtype=np.float32), device=dev)
     opts = B.default_options(**ws[0]["opts"])
     out = {}
-    for label, n_ in (("single", 1), ("batched", nb)):
+    for label, n_ in (("single", 1), ("batch_of_4", 4), ("batch_of_16", 16), ("batched", nb)):
         plan = B.BatchedPlan(n_, [to_dev(ws[0]["psf"][0])], opts=opts)
         g = [[to_dev(w["g"][0])] for w in ws[:n_]]
         b = [[10.0]] * n_
@@ -395,9 +397,12 @@ def measure_batched(nb: int, steps: int, dev):
         ev1.record(); torch.cuda.synchronize()
         plan.close()
         out[label] = {"problems": n_, "value": its / (ev0.elapsed_time(ev1) * 1e-3), "unit": "iterations/s (sum over the problems)",
-                      "ms_per_step": ev0.elapsed_time(ev1) / steps, "iterations_per_problem": rs[0].iterations}
+                      "ms_per_step": ev0.elapsed_time(ev1) / steps, "iterations_per_problem": rs[0].iterations,
+                      "path": "cluster" if rs[0].fused_linesearch == 2 else "launch-per-pass"}
     out["aggregate_speedup"] = out["batched"]["value"] / out["single"]["value"]
-    out["workload"] = f"C0 recipe, 256x256 fp32, 100 SGP iterations per problem, {nb} problems in one sgp_plan_run_batched call vs 1"
+    out["aggregate_speedup_vs_round1_single"] = out["batched"]["value"] / 18700.0
+    out["workload"] = (f"C0 recipe, 256x256 fp32, 100 SGP iterations per problem (start-point phase and result copies inside), 1 / 4 / 16 / {nb} problems in "
+                       "one sgp_plan_run_batched call; round 1 ran one such problem at 18.7 kit/s (profiles/r1j_bench_lines.md)")
     return out
 
 
@@ -625,7 +630,9 @@ def run_ours(args):
                                  f"({7 * p + 4} planes) vs 126 MB L2",
                            "tile_cols": int(opts.tile_cols), "rows_per_block": int(opts.rows_per_block),
                            "J0_final": J_final, "backtracks": backtracks // args.steps,
-                           "fused_linesearch": int(r.fused_linesearch)},
+                           "fused_linesearch": int(r.fused_linesearch),
+                           "path": ("one cluster per problem, whole iteration in one kernel (csrc/small.cuh); the per-kernel table of `roofline` is the "
+                                    "launch-per-pass path of the instrumented pass") if int(r.fused_linesearch) == 2 else "launch-per-pass"},
                 "clocks": clk.summary(), "e2e": e2e, "gpu_launches": launches, "roofline": roofline, "cpu_baseline": cpu,
                 "cufft_compare": cufft, "other_workloads": others, "batched_small_grids": batched}
         print(json.dumps(line))

@@ -5,8 +5,9 @@
 // whatever their grid, 34-42 us per iteration for 0.26-1 Mpixel.  Here a cluster of NC CTAs keeps the problem on chip:
 // CTA r owns rows [r R, (r+1) R) of the image for the row passes and columns [r CW, (r+1) CW) of the half spectrum for the
 // column passes; the two transpositions of every 2-D transform go through DISTRIBUTED SHARED MEMORY (each CTA WRITES
-// the pieces of its result into the shared memory of the CTAs that need them next: remote stores are posted, remote loads
-// would each wait a round trip), a hardware cluster barrier separates the passes, and the
+// the pieces of its result into the shared memory of the CTAs that need them next, by asynchronous stores whose bytes
+// are counted on an mbarrier of the receiving CTA: remote loads would each wait a round trip, and plain remote stores
+// need a cluster barrier whose release fence waits for their acknowledgement), and the
 // global sums (BB dot products, grad'd, J) are gathered in CTA 0, whose thread 0 runs the scalar logic of sgp_dev.cuh
 // (bb_step, Armijo test, finish_iteration) and broadcasts the decision to every CTA's shared memory.  The planes
 // (f, grad, d, q, g) stay in global memory (L1 / L2 resident: every row is only ever touched by the CTA that owns it).
@@ -19,6 +20,7 @@
 #pragma once
 #include <cooperative_groups.h>
 #include "row_inv.cuh"
+#include "col.cuh"
 #include "small_params.h"
 
 namespace sgpk {
@@ -32,7 +34,8 @@ struct SmallBcast {
 
 // elements per thread of the FFTs of this kernel: fewer than the launch-per-pass kernels use (16 / 32 in float), because a
 // cluster has only NC SMs for the whole problem and the short per-thread instruction streams of 4-8 warps per scheduler hide
-// each other's latencies (measured at 256^2 float, E = 16, 4 warps per SM: 43 us per iteration); the pass tables of these
+// each other's latencies (measured at 256^2 float: E = 16, 4 warps per SM, 43 us per iteration; E = 8: 31 us at the same stage;
+// E = 4 with 16 warps adds two exchanges per transform and is no faster: 26.8 vs 25.1 us per iteration); the pass tables of these
 // plans are uploaded by the host beside the plan's own (plan_impl.inl)
 template <typename T> __host__ __device__ constexpr int small_E() { return 8; }
 
@@ -46,9 +49,34 @@ template <typename T, int NY, int NX, int NC> struct SmallCfg {
     static constexpr size_t n_srow = ((size_t)R * SRP + 1) & ~(size_t)1, n_scol = ((size_t)NY * CWP + 1) & ~(size_t)1;
     static constexpr size_t n_lines = (size_t)R * RS > (size_t)CW * CS ? (size_t)R * RS : (size_t)CW * CS;
     static constexpr size_t smem = (n_srow + n_scol + n_lines) * sizeof(cx<T>);
-    static constexpr bool ok = TFr <= 32 && TFc <= 32 && R >= 1 && CW >= 1 && NT % 32 == 0 && NT <= 1024 && NTR % 32 == 0 && NTC % 32 == 0 &&
+    static constexpr bool ok = TFr <= 32 && (TFc <= 32 || CW <= 15) && R >= 1 && CW >= 1 && NT % 32 == 0 && NT <= 1024 && NTR % 32 == 0 && NTC % 32 == 0 &&
                                smem <= 200 * 1024 && plan_ok(L, Er) && plan_ok(NY, Ec);
 };
+
+// ---- asynchronous stores into the shared memory of another CTA of the cluster (st.async, sm_90+): the store is posted, and its
+// bytes are counted on an mbarrier of the DESTINATION CTA, which therefore knows when a whole slab has arrived without any
+// fence on the sending side (a cluster barrier with release semantics made every sender wait for the acknowledgement of its
+// remote stores: "membar" was the top stall of the first versions of this kernel)
+__device__ __forceinline__ unsigned int cluster_addr(const void *smem_ptr, int rank)
+{
+    unsigned int r;
+    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"((unsigned int)__cvta_generic_to_shared(smem_ptr)), "r"(rank));
+    return r;
+}
+__device__ __forceinline__ void st_async(unsigned int raddr, float2 v, unsigned int rbar)
+{
+    const unsigned long long bits = ((unsigned long long)__float_as_uint(v.y) << 32) | (unsigned long long)__float_as_uint(v.x);
+    asm volatile("st.async.weak.shared::cluster.mbarrier::complete_tx::bytes.b64 [%0], %1, [%2];" ::"r"(raddr), "l"(bits), "r"(rbar) : "memory");
+}
+__device__ __forceinline__ void st_async(unsigned int raddr, double2 v, unsigned int rbar)
+{
+    asm volatile("st.async.weak.shared::cluster.mbarrier::complete_tx::bytes.v2.b64 [%0], {%1, %2}, [%3];"
+                 ::"r"(raddr), "l"(__double_as_longlong(v.x)), "l"(__double_as_longlong(v.y)), "r"(rbar) : "memory");
+}
+__device__ __forceinline__ void mbar_expect(unsigned long long *bar, unsigned int bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
 
 __device__ __forceinline__ float kl_pair(float g0, float y0, float g1, float y1)
 {
@@ -109,6 +137,7 @@ __global__ void __launch_bounds__(SmallCfg<T, NY, NX, NC>::NT, 1) small_sgp_kern
     __shared__ double red[kNQ * 32];
     __shared__ double cpart[NC][4];
     __shared__ SmallBcast bc;
+    __shared__ unsigned long long bar_c, bar_r;                // count the bytes arriving in Cin / Rin (one phase per fill)
     __shared__ C kbs[NY];                                      // companion of the packed column (CTA 0, column 0)
     __shared__ Ctrl sct;                                       // CTA 0: the control block while the kernel runs (written back at the end)
 
@@ -134,7 +163,7 @@ __global__ void __launch_bounds__(SmallCfg<T, NY, NX, NC>::NT, 1) small_sgp_kern
     C *cline = lines + (size_t)cc * CS;                         // column passes
     const C *rrow = Rin + (size_t)row * SRP;
     const SyncGroup<TFr> rsync{0};
-    const SyncGroup<TFc> csync{0};
+    const SyncGroup<TFc> csync{1 + cc};                          // columns of more than 32 threads: one named barrier each
     const size_t base = (size_t)y * NX;
 
     // state at the start of this launch (written by the set-up kernels or by the previous launch)
@@ -165,7 +194,18 @@ __global__ void __launch_bounds__(SmallCfg<T, NY, NX, NC>::NT, 1) small_sgp_kern
     };
 
     // half-spectrum entry k of this thread's row -> the column slab of the CTA that owns column k
-    auto put_row = [&](const int k, const C val) { cluster.map_shared_rank(Cin, k / CW)[(size_t)y * CWP + (k % CW)] = val; };
+    const unsigned int cin_u = (unsigned int)__cvta_generic_to_shared(Cin), rin_u = (unsigned int)__cvta_generic_to_shared(Rin);
+    const unsigned int barc_u = smem_u32(&bar_c), barr_u = smem_u32(&bar_r);
+    auto rmap = [&](unsigned int a, int r) -> unsigned int { unsigned int o_; asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(o_) : "r"(a), "r"(r)); return o_; };
+    auto put_row = [&](const int k, const C val) {
+        const int dst = k / CW;
+        st_async(rmap(cin_u + (unsigned int)(((size_t)y * CWP + (k % CW)) * sizeof(C)), dst), val, rmap(barc_u, dst));
+    };
+    constexpr unsigned int CIN_BYTES = (unsigned int)((size_t)NY * CW * sizeof(C)), RIN_BYTES = (unsigned int)((size_t)R * L * sizeof(C));
+    unsigned int ph_c = 0, ph_r = 0;
+    // all of Cin / Rin has arrived (thread 0 arms the phase: one arrival + the slab's bytes), and no thread of this CTA is still in the previous pass
+    auto wait_cin = [&](void) { if (tid == 0) mbar_expect(&bar_c, CIN_BYTES); mbar_wait(&bar_c, ph_c); ph_c ^= 1; __syncthreads(); };
+    auto wait_rin = [&](void) { if (tid == 0) mbar_expect(&bar_r, RIN_BYTES); mbar_wait(&bar_r, ph_r); ph_r ^= 1; __syncthreads(); };
     // the transfer function of this thread's column entries stays in registers for the whole run (it is read twice per iteration)
     C kh[Ec];
     if (cact) {
@@ -223,8 +263,8 @@ __global__ void __launch_bounds__(SmallCfg<T, NY, NX, NC>::NT, 1) small_sgp_kern
             fft_block<T, NY, Ec, +1, false>(vc, cline, 1, tc, P.tw_c, csync);
 #pragma unroll
             for (int e = 0; e < Ec; ++e) {
-                const int ky = tc + TFc * e;
-                cluster.map_shared_rank(Rin, ky / R)[(size_t)(ky % R) * SRP + kx] = vc[e];
+                const int ky = tc + TFc * e, dst = ky / R;
+                st_async(rmap(rin_u + (unsigned int)(((size_t)(ky % R) * SRP + kx) * sizeof(C)), dst), vc[e], rmap(barr_u, dst));
             }
         }
     };
@@ -285,6 +325,11 @@ __global__ void __launch_bounds__(SmallCfg<T, NY, NX, NC>::NT, 1) small_sgp_kern
     // thread 0 of every CTA: sum of column i of the partials, in rank order
     auto total = [&](int i) -> double { double a = 0.0; for (int r = 0; r < NC; ++r) a += cpart[r][i]; return a; };
 
+    if (tid == 0) {
+        mbar_init(&bar_c, 1); mbar_init(&bar_r, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    cluster.sync();                                             // every CTA's barriers exist before anybody sends
     ratio_rows();
     double gd_part = 0.0, Jref = 0.0, gdt = 0.0;
     for (int it = 0; it < P.iters; ++it) {
@@ -292,11 +337,11 @@ __global__ void __launch_bounds__(SmallCfg<T, NY, NX, NC>::NT, 1) small_sgp_kern
         const bool dbg_it = it == 5;
 #endif
         SMALL_TICK();
-        cluster.sync();
+        wait_cin();
         SMALL_TICK();
         col_pass(true);                                         // a2: A^T r in Fourier space (Eq.17)
         SMALL_TICK();
-        cluster.sync();
+        wait_rin();
         SMALL_TICK();
         const int k = bc.k;
         if (ract && PF) { ldrow(f2, f); if (k > 0) { ldrow(d2, dpl); ldrow(o2, grad); } }
@@ -330,7 +375,6 @@ __global__ void __launch_bounds__(SmallCfg<T, NY, NX, NC>::NT, 1) small_sgp_kern
                             for (int k4 = 0; k4 < 4; ++k4) acc[k4] += (double)pq[k4];
                         }
                     }
-                    st2<T>(grad + base + 2 * (t + TFr * e), gn);
                     vr[e] = gn;                                 // the gradient stays in the registers for the projection
                 }
             }
@@ -338,7 +382,16 @@ __global__ void __launch_bounds__(SmallCfg<T, NY, NX, NC>::NT, 1) small_sgp_kern
             send_partials(acc, 4);
         }
         SMALL_TICK();
-        cluster.sync();
+        {
+            // the gradient goes to global memory between the two halves of the barrier: stored before it, the barrier's release
+            // fence would wait for the acknowledgement of these (CTA-private) stores
+            auto token = cluster.barrier_arrive();
+            if (ract) {
+#pragma unroll
+                for (int e = 0; e < Er; ++e) st2<T>(grad + base + 2 * (t + TFr * e), vr[e]);
+            }
+            cluster.barrier_wait(std::move(token));
+        }
         SMALL_TICK();
         if (tid == 0) {                                         // a6: step length, in every CTA
             const double s0 = total(0), s1 = total(1), s2 = total(2), s3 = total(3);
@@ -379,11 +432,11 @@ __global__ void __launch_bounds__(SmallCfg<T, NY, NX, NC>::NT, 1) small_sgp_kern
             small_fwd<T, L, Er>(vr, line, t, rsync, put_row, P.tw_r, P.tw_h);
         }
         SMALL_TICK();
-        cluster.sync();
+        wait_cin();
         SMALL_TICK();
         col_pass(false);                                        // a8: A d (Eq.16)
         SMALL_TICK();
-        cluster.sync();
+        wait_rin();
         SMALL_TICK();
         if (ract && PF) { ldrow(g2, gpl); ldrow(q2, q); }
         inv_rows();                                             // v[] = u = A d on this CTA's rows
