@@ -1,7 +1,7 @@
 """A small tour of the library for `compute-sanitizer`: every kernel family on tiny grids, incl.
 the Armijo backtracking (forced in every iteration), the fused and the separate line-search schedules, boundary masks, three images,
 RL / OSEM on the fused schedule, a 5-smooth grid with padded thread groups, a batched plan, the flux-constrained projection, the
-refresh round and the Eq.25 stop.  Not a pytest module: run as
+refresh round, the Eq.25 stop and the one-cluster-per-problem kernel of the small grids.  Not a pytest module: run as
 
     compute-sanitizer --tool memcheck  python tests/gpu_sanitize_case.py
     compute-sanitizer --tool racecheck python tests/gpu_sanitize_case.py
@@ -37,6 +37,20 @@ def main():
             assert r.iterations == 12 and r.total_backtracks > 0 and torch.isfinite(f).all()
             f, r = plan.rl([dev(w["g"][0], dt)], w["b"])
             plan.close()
+        # small grids: the whole iteration in one kernel, one cluster per problem (csrc/small.cuh) -- distributed shared memory,
+        # st.async + mbarrier, cluster barriers; backtracking in every iteration; a batch of three problems
+        w = synth.make("C0", n=128)
+        kw = {**w["opts"], "max_iter": 8, "alpha0": 1e5, "alpha_min": 1e3, "alpha_max": 1e6}
+        plan = B.Plan([dev(w["psf"][0], dt)], opts=B.default_options(**kw))
+        f, r = plan.sgp([dev(w["g"][0], dt)], w["b"])
+        assert r.fused_linesearch == 2 and r.iterations == 8 and r.total_backtracks > 0 and torch.isfinite(f).all()
+        plan.close()
+        ws = [synth.make("C0", n=128, seed_idx=80 + i) for i in range(3)]
+        o = B.default_options(**{**ws[0]["opts"], "max_iter": 30, "stop_rule": 1, "tol": 1e-3})
+        bp = B.BatchedPlan(3, [dev(ws[0]["psf"][0], dt)], opts=o)
+        fb, rb = bp.run_batched(B.ALG_SGP, [[dev(x["g"][0], dt)] for x in ws], [[10.0]] * 3, opts=o)
+        assert all(x.fused_linesearch == 2 for x in rb)
+        bp.close()
         # three images, 128^2: SGP, RL, OSEM; flux constraint; refresh round; Eq.25
         w = synth.make("C2", n=128, max_iter=12)
         g = [dev(a, dt) for a in w["g"]]
