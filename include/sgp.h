@@ -108,8 +108,8 @@ typedef struct sgp_options {
                                                     bit 1 = persistent column kernel, bit 2 / bit 3 = force the separate / the fused line-search
                                                     kernel (default: chosen by working set vs L2), bit 4 = never use the two-CTAs-per-SM column
                                                     kernel, bit 6 = RL / OSEM on the six separate launches of round 1 instead of the fused four,
-                                                    bit 7 = never use the one-cluster-per-problem kernel of the small grids (sgp_*, one image, no mask,
-                                                    128^2 ... 512^2: the whole iteration in one kernel, csrc/small.cuh) */
+                                                    bit 7 = never use the one-cluster-per-problem kernel of the small grids (sgp_*, one image,
+                                                    128^2 / 256^2, constant background: the whole iteration in one kernel, csrc/small.cuh) */
     double rl_relax;                             /* rl_* only: exponent of the multiplicative relaxation, Eq.3:
                                                     f <- f o (W o sum_j A_j^T(g_j/(A_j f + b_j)))^rl_relax; 1 (default) = plain RL */
     double rl_linear;                            /* rl_* only: constant lambda_k of the linear relaxation, Eq.4:

@@ -224,13 +224,13 @@ template <typename T> struct PlanImpl : PlanBase {
         if (opt.use_graph & 8) fuse_ls = true;
         col_grid = (opt.use_graph & 2) ? (ntiles < nsm ? ntiles : nsm) : ntiles;   // experiment switch: persistent or one tile per CTA
 
-        // Small grids: one image without a boundary mask at 128^2 ... 512^2 iterates inside ONE kernel run by
+        // Small grids: one image (with or without boundary-effect correction) at 128^2 / 256^2 iterates inside ONE kernel run by
         // one thread-block cluster per problem (small.cuh) when the device can co-schedule such a cluster; use_graph bit 7 (or any other
         // experiment switch) keeps the launch-per-pass path.  A batched plan of 256^2 problems uses it up to 16 problems (the device
         // holds about 7 clusters of 16 CTAs at once: 4 problems run 151 kit/s this way against 71 kit/s launch-per-pass, 16 problems 214
         // against 195, 32 problems 261 against 326, 64 problems 270 against 394); 128^2 (clusters of 8) always: 64 problems 1174 against 571.
-        if (p == 1 && !G.masked && (opt.use_graph & ~1) == 0 && !getenv("SGP_NO_CLUSTER")) {      // any experiment switch: launch-per-pass
-            small_k = get_small<T>(ny, nx, &small_nc, &small_threads, &small_smem, &small_er, &small_ec);
+        if (p == 1 && (opt.use_graph & ~1) == 0 && !getenv("SGP_NO_CLUSTER")) {      // any experiment switch: launch-per-pass
+            small_k = get_small<T>(ny, nx, G.masked != 0, &small_nc, &small_threads, &small_smem, &small_er, &small_ec);
             if (small_k) {
                 bool ok = cudaFuncSetAttribute((const void *)small_k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)small_smem) == cudaSuccess;
                 if (ok && small_nc > 8) ok = cudaFuncSetAttribute((const void *)small_k, cudaFuncAttributeNonPortableClusterSizeAllowed, 1) == cudaSuccess;
@@ -400,7 +400,7 @@ template <typename T> struct PlanImpl : PlanBase {
     {
         SmallParams<T> S;
         memset(&S, 0, sizeof(S));
-        S.G = G; S.o = o; S.tr = tr; S.ct = ct; S.f = f; S.grad = grad; S.d = d; S.q = q; S.g = Gp; S.qbuf = n * (size_t)p;
+        S.G = G; S.o = o; S.tr = tr; S.ct = ct; S.f = f; S.grad = grad; S.d = d; S.q = q; S.g = Gp; S.alphaR = alphaR; S.qbuf = n * (size_t)p;
         S.khat = khat; S.khatB = khatB; S.tw_r = tw_sr; S.tw_h = tw_h; S.tw_c = tw_sc; S.bconst = bconst0; S.iters = iters;
         S.slab = lnb > 1 ? slab : 0; S.tr_slab = lnb > 1 ? tr_slab : 0;
         cudaLaunchConfig_t cfg;

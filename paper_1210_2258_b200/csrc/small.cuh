@@ -15,7 +15,8 @@
 //
 // Same arithmetic per pixel as the launch-per-pass path (ew.cuh), same FFT (fft_core.cuh), same tables and transfer
 // functions; sums are grouped per CTA of this kernel, so the two paths agree to rounding, not bit for bit.
-// Scope: SGP, one image, no boundary mask, constant background, no replay / flux / refresh / Eq.25 options -- the host
+// Scope: SGP, one image, with or without boundary-effect correction, constant background, no replay / flux / refresh / Eq.25
+// options -- the host
 // (plan_run.inl) takes the launch-per-pass path for everything else.
 #pragma once
 #include <cooperative_groups.h>
@@ -87,6 +88,19 @@ __device__ __forceinline__ float kl_pair(float g0, float y0, float g1, float y1)
     return k0 + k1;
 }
 __device__ __forceinline__ double kl_pair(double g0, double y0, double g1, double y1) { return kl_term(g0, y0) + kl_term(g1, y1); }
+// the same over the pixels of the pair that lie in S (boundary-effect correction: J0 is summed over S, reading A12)
+__device__ __forceinline__ float kl_pair_s(float g0, float y0, float g1, float y1, bool s0, bool s1)
+{
+    bool ok0, ok1;
+    float k0 = kl_series(g0, y0, ok0), k1 = kl_series(g1, y1, ok1);
+    if (s0 && !ok0) k0 = kl_far(g0, y0);
+    if (s1 && !ok1) k1 = kl_far(g1, y1);
+    return (s0 ? k0 : 0.f) + (s1 ? k1 : 0.f);
+}
+__device__ __forceinline__ double kl_pair_s(double g0, double y0, double g1, double y1, bool s0, bool s1)
+{
+    return (s0 ? kl_term(g0, y0) : 0.0) + (s1 ? kl_term(g1, y1) : 0.0);
+}
 
 // forward transform of one row held as v[e] = (x[2m], x[2m+1]), m = t + TF e; its half spectrum (entry 0 packs kx = 0 and
 // nx/2) goes to dst[0 .. L-1] in shared memory (row_fwd.cuh: fwd_fft_store, with the store redirected)
@@ -121,7 +135,8 @@ __device__ __forceinline__ void small_fwd(cx<T> (&v)[E], cx<T> *line, const int 
     }
 }
 
-template <typename T, int NY, int NX, int NC>
+// MK: boundary-effect correction (Eq.16-23): S inside the grid, alphaR > 0 marks R and 1/alphaR is the weight M_R/alpha
+template <typename T, int NY, int NX, int NC, bool MK>
 __global__ void __launch_bounds__(SmallCfg<T, NY, NX, NC>::NT, 1) small_sgp_kernel(const SmallParams<T> P)
 {
     namespace cgx = cooperative_groups;
@@ -129,6 +144,7 @@ __global__ void __launch_bounds__(SmallCfg<T, NY, NX, NC>::NT, 1) small_sgp_kern
     using K = SmallCfg<T, NY, NX, NC>;
     constexpr int L = K::L, Er = K::Er, Ec = K::Ec, TFr = K::TFr, TFc = K::TFc, R = K::R, CW = K::CW;
     constexpr int SRP = K::SRP, RS = K::RS, CS = K::CS, CWP = K::CWP;
+    static_assert(K::Er <= 16, "the S mask of a thread's pixels is kept in 32 bits");
     static_assert(K::ok, "small_sgp_kernel: unsupported geometry");
     extern __shared__ __align__(16) unsigned char smem_raw[];
     C *Rin = reinterpret_cast<C *>(smem_raw);                  // [R][SRP]: this CTA's spectrum rows, written by the column passes of all CTAs
@@ -170,7 +186,27 @@ __global__ void __launch_bounds__(SmallCfg<T, NY, NX, NC>::NT, 1) small_sgp_kern
     if (ct->status != 0) return;                                // uniform over the cluster
     T *q = bshift(P.q, off) + (size_t)ct->qsel * P.qbuf;
     const T bcst = (T)(P.slab ? ct->bconst[0] : P.bconst);
-    const T pT = (T)1, Wc = (T)1;                               // one image: alpha = 1, W = 1 (Eq.10)
+    const T pT = (T)1, Wc = (T)1;                               // one image without a mask: alpha = 1, W = 1 (Eq.10)
+    // masks of this thread's pixels: bit 2e / 2e+1 of smask = pixel x0 / x0 + 1 of pair e lies in S; a2[e] = alpha on R, 0 outside R
+    unsigned int smask = 0xffffffffu;
+    C a2[MK ? Er : 1];
+    if constexpr (MK) {
+        smask = 0u;
+        const bool rowin = (unsigned)(y - P.G.oy) < (unsigned)P.G.sy;
+#pragma unroll
+        for (int e = 0; e < Er; ++e) {
+            const int x0 = 2 * (t + TFr * e);
+            if (rowin && (unsigned)(x0 - P.G.ox) < (unsigned)P.G.sx) smask |= 1u << (2 * e);
+            if (rowin && (unsigned)(x0 + 1 - P.G.ox) < (unsigned)P.G.sx) smask |= 2u << (2 * e);
+            a2[e] = ract ? ld2<T>(P.alphaR + base + x0) : mk<T>((T)0, (T)0);
+        }
+    }
+    auto in_s0 = [&](int e) -> bool { return !MK || ((smask >> (2 * e)) & 1u) != 0u; };
+    auto in_s1 = [&](int e) -> bool { return !MK || ((smask >> (2 * e + 1)) & 1u) != 0u; };
+    // ratio g / (q + b) on S, 0 elsewhere (Eq.18)
+    auto ratio_pair = [&](int e, const C g2_, const C q2_) -> C {
+        return mk<T>(in_s0(e) ? ratio_term(g2_.x, q2_.x + bcst) : (T)0, in_s1(e) ? ratio_term(g2_.y, q2_.y + bcst) : (T)0);
+    };
     if (tid == 0) {
         sct = *ct;                                              // every CTA keeps its own replica of the control block (see decide below)
         bc.alpha = sct.alpha; bc.lambda = sct.lambda; bc.L1 = sct.L1; bc.L2 = sct.L2; bc.state = 0; bc.status = 0; bc.k = sct.k;
@@ -230,7 +266,7 @@ __global__ void __launch_bounds__(SmallCfg<T, NY, NX, NC>::NT, 1) small_sgp_kern
             for (int e = 0; e < Er; ++e) {
                 const int x0 = 2 * (t + TFr * e);
                 const C g2 = ld2<T>(gpl + base + x0), q2 = ld2<T>(q + base + x0);
-                vr[e] = mk<T>(ratio_term(g2.x, q2.x + bcst), ratio_term(g2.y, q2.y + bcst));
+                vr[e] = ratio_pair(e, g2, q2);
             }
             small_fwd<T, L, Er>(vr, line, t, rsync, put_row, P.tw_r, P.tw_h);
         }
@@ -317,7 +353,8 @@ __global__ void __launch_bounds__(SmallCfg<T, NY, NX, NC>::NT, 1) small_sgp_kern
 #pragma unroll
             for (int e = 0; e < Er; ++e) {
                 const T y0 = (T)(q2[e].x + lam * vr[e].x) + bcst, y1 = (T)(q2[e].y + lam * vr[e].y) + bcst;
-                acc += (double)kl_pair(g2[e].x, y0, g2[e].y, y1);
+                if constexpr (MK) acc += (double)kl_pair_s(g2[e].x, y0, g2[e].y, y1, in_s0(e), in_s1(e));
+                else acc += (double)kl_pair(g2[e].x, y0, g2[e].y, y1);
             }
         }
         return acc;
@@ -354,16 +391,24 @@ __global__ void __launch_bounds__(SmallCfg<T, NY, NX, NC>::NT, 1) small_sgp_kern
                 if (!PF && k > 0) { ldrow(f2, f); ldrow(d2, dpl); ldrow(o2, grad); }
 #pragma unroll
                 for (int e = 0; e < Er; ++e) {
-                    const C gn = mk<T>(pT - vr[e].x, pT - vr[e].y);
+                    C gn = mk<T>(pT - vr[e].x, pT - vr[e].y);
+                    bool inR[2] = {true, true};
+                    T wv[2] = {Wc, Wc};
+                    if constexpr (MK) {
+                        inR[0] = a2[e].x > (T)0; inR[1] = a2[e].y > (T)0;
+                        wv[0] = inR[0] ? (T)1 / a2[e].x : (T)0; wv[1] = inR[1] ? (T)1 / a2[e].y : (T)0;
+                        gn = mk<T>(inR[0] ? a2[e].x - vr[e].x : (T)0, inR[1] ? a2[e].y - vr[e].y : (T)0);
+                    }
                     if (k > 0) {
                         const T fa[2] = {f2[e].x, f2[e].y}, da[2] = {d2[e].x, d2[e].y}, ga[2] = {gn.x, gn.y}, oa[2] = {o2[e].x, o2[e].y};
                         T pq[4] = {(T)0, (T)0, (T)0, (T)0};
 #pragma unroll
                         for (int c = 0; c < 2; ++c) {
                             const T s = lam * da[c];
-                            const T Di = Wc * clipT<T>(fa[c], L1, L2);
-                            const T zf = ga[c] - oa[c];
-                            const T si = fast_div(s, Di), zd = zf * Di;
+                            const T Di = wv[c] * clipT<T>(fa[c], L1, L2);
+                            const T zr = ga[c] - oa[c];
+                            const T zf = inR[c] ? zr : (T)0;
+                            const T si = inR[c] ? fast_div(s, Di) : (T)0, zd = inR[c] ? zr * Di : (T)0;
                             if constexpr (sizeof(T) == 8) {
                                 acc[0] += si * si; acc[1] += si * zf; acc[2] += s * zd; acc[3] += zd * zd;
                             } else {
@@ -412,12 +457,18 @@ __global__ void __launch_bounds__(SmallCfg<T, NY, NX, NC>::NT, 1) small_sgp_kern
             for (int e = 0; e < Er; ++e) {
                 const C fe = f2[e], ge = vr[e];
                 C de;
-                T D = Wc * clipT<T>(fe.x, L1, L2);
+                bool r0 = true, r1 = true;
+                T w0 = Wc, w1 = Wc;
+                if constexpr (MK) {
+                    r0 = a2[e].x > (T)0; r1 = a2[e].y > (T)0;
+                    w0 = r0 ? (T)1 / a2[e].x : (T)0; w1 = r1 ? (T)1 / a2[e].y : (T)0;
+                }
+                T D = w0 * clipT<T>(fe.x, L1, L2);
                 T yv = fe.x - alpha * D * ge.x;
-                de.x = (yv > (T)0 ? yv : (T)0) - fe.x;
-                D = Wc * clipT<T>(fe.y, L1, L2);
+                de.x = r0 ? ((yv > (T)0 ? yv : (T)0) - fe.x) : (T)0;
+                D = w1 * clipT<T>(fe.y, L1, L2);
                 yv = fe.y - alpha * D * ge.y;
-                de.y = (yv > (T)0 ? yv : (T)0) - fe.y;
+                de.y = r1 ? ((yv > (T)0 ? yv : (T)0) - fe.y) : (T)0;
                 if constexpr (sizeof(T) == 4) {
                     accf += ge.x * de.x + ge.y * de.y;
                     if ((e & 3) == 3) { gd_part += (double)accf; accf = 0.f; }
@@ -440,6 +491,12 @@ __global__ void __launch_bounds__(SmallCfg<T, NY, NX, NC>::NT, 1) small_sgp_kern
         SMALL_TICK();
         if (ract && PF) { ldrow(g2, gpl); ldrow(q2, q); }
         inv_rows();                                             // v[] = u = A d on this CTA's rows
+        if constexpr (MK) {                                     // u = M_S o (...) (Eq.16): q stays zero outside S
+            if (ract) {
+#pragma unroll
+                for (int e = 0; e < Er; ++e) { if (!in_s0(e)) vr[e].x = (T)0; if (!in_s1(e)) vr[e].y = (T)0; }
+            }
+        }
         if (ract && !PF) { ldrow(g2, gpl); ldrow(q2, q); }
         // ---- a9: Armijo rule, lambda = 1, theta, theta^2, ...; every trial is one reduction
         {
@@ -501,7 +558,7 @@ __global__ void __launch_bounds__(SmallCfg<T, NY, NX, NC>::NT, 1) small_sgp_kern
                 fn.x = f2[e].x + lam * d2[e].x; fn.y = f2[e].y + lam * d2[e].y;
                 st2<T>(q + base + x0, qn);
                 st2<T>(f + base + x0, fn);
-                vr[e] = mk<T>(ratio_term(g2[e].x, qn.x + bcst), ratio_term(g2[e].y, qn.y + bcst));
+                vr[e] = ratio_pair(e, g2[e], qn);
             }
             if (more) small_fwd<T, L, Er>(vr, line, t, rsync, put_row, P.tw_r, P.tw_h);
         }

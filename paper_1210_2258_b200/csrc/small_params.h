@@ -9,6 +9,7 @@ template <typename T> struct SmallParams {
     Geom G; DevOpts o; Trace tr; Ctrl *ct;
     T *f, *grad, *d, *q;              // planes of problem 0 (q: both buffers, Ctrl::qsel says which is current)
     const T *g;
+    const T *alphaR;                  // boundary problems: alpha on R, 0 outside (shared by the problems of a batch)
     size_t qbuf;
     const cx<T> *khat, *khatB;        // transfer function (tile-major, scaled by 1/(ny nx)) and its packed-column companion
     const cx<T> *tw_r, *tw_h, *tw_c;  // pass tables of the row / column FFTs, exp(-2 pi i k/nx)
@@ -21,7 +22,7 @@ template <typename T> struct SmallParams {
 template <typename T> using small_kernel_t = void (*)(const SmallParams<T>);
 // kernel for this geometry (nullptr: none), its cluster size, threads per CTA, dynamic shared memory and the elements per thread of
 // its row / column FFT plans (fft_core.cuh: plan_radix), whose pass tables the host supplies
-template <typename T> small_kernel_t<T> get_small(int ny, int nx, int *nc, int *threads, size_t *smem, int *er, int *ec);
+template <typename T> small_kernel_t<T> get_small(int ny, int nx, bool masked, int *nc, int *threads, size_t *smem, int *er, int *ec);
 
 
 }  // namespace sgpk

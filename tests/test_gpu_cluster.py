@@ -14,7 +14,7 @@ import oracle  # noqa: E402  (test infrastructure)
 from paper_1210_2258_b200 import binding as B  # noqa: E402
 from paper_1210_2258_b200 import synth  # noqa: E402
 
-from test_gpu_parity import _need_gpu, dev, rel_l2  # noqa: E402
+from test_gpu_parity import _need_gpu, dev, rel_l2, oracle_run  # noqa: E402
 
 NO_CLUSTER = 128          # use_graph bit 7 (include/sgp.h)
 TOL = {np.float32: dict(one=1e-5, run=1e-3, J=1e-4, alpha=5e-3, pix=1e-3), np.float64: dict(one=1e-11, run=1e-10, J=1e-10, alpha=1e-9, pix=1e-10)}
@@ -197,3 +197,52 @@ def test_cluster_kernel_in_batched_plans():
     for i in (0, 17, 39):
         fo, ro = _oracle(ws[i], n, **{**ws[0]["opts"], "max_iter": 1, "stop_rule": 0})
         assert rel_l2(fb[i].cpu().numpy(), fo) <= 1e-5
+
+
+@pytest.mark.parametrize("dt", [np.float32, np.float64])
+@pytest.mark.parametrize("s_,sbar", [(160, 256), (96, 128)])
+def test_cluster_kernel_with_boundary_effect_correction(s_, sbar, dt):
+    """Eq.16-23 inside the cluster kernel: a 160^2 image reconstructed on a 256^2 object grid -- the size of the paper's
+    sub-domain problems -- and 96^2 in 128^2 (C3 recipe: stars also outside the image, Gauss + Moffat PSF,
+    b = 5, paper-default options incl. the adaptive bounds).  One iteration at 1e-5 / 1e-11; 20 iterations: image over R, zero
+    outside R, J0 trace, identical rule / backtrack traces; and the launch-per-pass path to rounding"""
+    _need_gpu()
+    t = TOL[dt]
+    w = synth.make("C3", s=s_, sbar=sbar, n_stars=150, max_iter=20, fwhm=8.0)
+    S = w["S"]
+    for it in (1, 20):
+        kw = {**w["opts"], "max_iter": it, "stop_rule": 0}
+        fo, ro = oracle_run(w, max_iter=it, stop_rule=0)
+        out = {}
+        for ug in (1, 1 | NO_CLUSTER):
+            o = B.default_options(**{**kw, "use_graph": ug})
+            plan = B.Plan([dev(w["psf"][0], dt)], S=S, opts=o)
+            f, r = plan.sgp([dev(w["g"][0], dt)], w["b"], opts=o)
+            out[ug] = (f.cpu().numpy(), r)
+            plan.close()
+        fg, rg = out[1]
+        fp, rp = out[1 | NO_CLUSTER]
+        assert rg.fused_linesearch == 2 and rp.fused_linesearch != 2
+        e = rel_l2(fg, fo)
+        print(f"[measured] cluster_boundary_{s_}in{sbar} {np.dtype(dt).name} rel_l2_{it}it = {e:.3e}")
+        assert e <= (t["one"] if it == 1 else t["run"]) and np.max(np.abs(fg - fo)) <= t["pix"] * np.max(fo)
+        assert np.array_equal(fg == 0, fo == 0) or np.count_nonzero((fg == 0) != (fo == 0)) <= (8 if dt == np.float32 else 0)   # R (alpha_j >= sigma_R, Eq.20)
+        assert np.max(np.abs(rg.J - ro.J) / np.abs(ro.J)) <= (1e-3 if dt == np.float32 else t["J"])
+        assert np.array_equal(rg.rule, ro.rule) and np.array_equal(rg.backtracks, ro.backtracks) and rg.n_fft2 == ro.n_fft2
+        assert rel_l2(fg, fp) <= (1e-4 if dt == np.float32 else 1e-11) and np.array_equal(rg.rule, rp.rule)
+
+
+def test_mosaic_runs_its_sub_domains_through_the_cluster_kernel():
+    """a 256^2 image as four overlapping 160^2 sub-images, each reconstructed on a 256^2 grid with boundary-effect
+    correction -- one batched plan, one cluster per sub-domain; equal to the launch-per-pass path to rounding"""
+    _need_gpu()
+    w = synth.make("C1", n=256, max_iter=15, stop_rule=0)
+    res = {}
+    for ug in (1, 1 | NO_CLUSTER):
+        o = B.default_options(**{**w["opts"], "max_iter": 15, "stop_rule": 0, "use_graph": ug})
+        m, r = B.mosaic(B.ALG_SGP, [dev(a, np.float32) for a in w["g"]], [dev(k, np.float32) for k in w["psf"]], w["b"], 2, 2, (160, 160), opts=o)
+        res[ug] = (m.cpu().numpy(), r)
+    rs = res[1][1] if isinstance(res[1][1], (list, tuple)) else [res[1][1]]
+    rp = res[1 | NO_CLUSTER][1] if isinstance(res[1 | NO_CLUSTER][1], (list, tuple)) else [res[1 | NO_CLUSTER][1]]
+    assert all(x.fused_linesearch == 2 for x in rs) and all(x.fused_linesearch != 2 for x in rp)
+    assert rel_l2(res[1][0], res[1 | NO_CLUSTER][0]) <= 1e-4
