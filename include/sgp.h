@@ -194,8 +194,9 @@ size_t sgp_plan_workspace_bytes(const sgp_plan *plan);
  * Each host thread keeps the plan of its last one-shot call (device workspace, twiddle tables, the instantiated
  * CUDA graph; the *_host calls also keep their staging buffer) and uses it again when the next call has the same
  * device, kind, p, grid, window, dtype and plan-time options (tile_cols, rows_per_block, use_graph, psf_origin,
- * sigma_R); the PSFs are transformed again in every call.  sgp_release_cached_plans() frees what the calling thread
- * holds (the end of the thread does too); a call with another key frees the old plan first. */
+ * sigma_R); the PSFs are transformed again in every call.  sgp_mosaic keeps its batched sub-domain plan and its
+ * sub-image buffers the same way (a second slot, keyed also by the number of sub-domains).  sgp_release_cached_plans()
+ * frees what the calling thread holds (the end of the thread does too); a call with another key frees the old plan first. */
 void sgp_release_cached_plans(void);
 int sgp_single(const void *g, const void *psf, const void *b_arr, double b_const, const void *f0,
                void *f_out, int ny, int nx, int dtype, const sgp_options *opt, sgp_result *res,

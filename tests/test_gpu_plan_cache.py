@@ -83,3 +83,35 @@ def test_release_cached_plans_returns_the_memory():
     free2 = torch.cuda.mem_get_info()[0]
     assert free2 - free1 >= 11 * 1024 * 1024 * 4 and free0 - free2 < 8 * 1024 * 1024, (free0, free1, free2, ws)
     B.release_cached_plans()                                        # nothing to free: a no-op
+
+
+def test_mosaic_keeps_its_sub_domain_plan_between_calls():
+    """sgp_mosaic keeps the batched sub-domain plan and the sub-image buffers of the calling thread's last call: repeated calls give
+    the same bits (also after a call with another geometry in between, which replaces the plan), other data of the same geometry
+    give that data's result, and sgp_release_cached_plans returns the memory"""
+    _need_gpu()
+    B.release_cached_plans()
+    dt = np.float32
+    w = synth.make("C1", n=256, max_iter=8, stop_rule=0)
+    w2 = synth.make("C1", n=256, seed_idx=9, max_iter=8, stop_rule=0)
+    o = B.default_options(**{**w["opts"], "max_iter": 8, "stop_rule": 0})
+    run = lambda x, sub: B.mosaic(B.ALG_SGP, [dev(a, dt) for a in x["g"]], [dev(k, dt) for k in x["psf"]], x["b"], 2, 2, sub, opts=o)[0]
+    torch.cuda.synchronize()
+    free0 = torch.cuda.mem_get_info()[0]
+    m1 = run(w, (160, 160))
+    free1 = torch.cuda.mem_get_info()[0]
+    assert free0 - free1 >= 4 * 11 * 256 * 256 * 4                  # four sub-domain workspaces are still there
+    m2 = run(w, (160, 160))
+    assert torch.equal(m1, m2)
+    other = run(w2, (160, 160))
+    assert not torch.equal(other, m1)
+    m3 = run(w, (144, 144))                                         # another window: a new plan
+    assert not torch.equal(m3, m1)
+    m4 = run(w, (160, 160))
+    assert torch.equal(m4, m1)
+    B.release_cached_plans()
+    fresh = run(w2, (160, 160))                                     # and a plan created afresh gives what the kept one gave
+    assert torch.equal(fresh, other)
+    B.release_cached_plans()
+    torch.cuda.synchronize()
+    assert free0 - torch.cuda.mem_get_info()[0] < 8 * 1024 * 1024
