@@ -40,6 +40,7 @@ template <typename T> struct PlanImpl : PlanBase {
     size_t fx_chunks = 0, fx_batches = 1;
     C *khatB_tmp = nullptr;        // companion line of the Gaussian's transfer function (smoothed constant start)
     small_kernel_t<T> small_k = nullptr;   // small grids: the whole SGP iteration in one kernel, one cluster per problem (small.cuh)
+    small_kernel_t<T> small_k_rl = nullptr; // the same for Richardson-Lucy rounds
     int small_nc = 0, small_threads = 0, small_er = 0, small_ec = 0; size_t small_smem = 0;
     C *tw_sr = nullptr, *tw_sc = nullptr;   // pass tables of its row / column FFT plans
     const void **ptrtab = nullptr;  // batched plans: addresses of the caller's arrays of a run (aux.cuh: BatchTab), 2 nb p + 2 nb entries
@@ -230,10 +231,12 @@ template <typename T> struct PlanImpl : PlanBase {
         // holds about 7 clusters of 16 CTAs at once: 4 problems run 151 kit/s this way against 71 kit/s launch-per-pass, 16 problems 214
         // against 195, 32 problems 261 against 326, 64 problems 270 against 394); 128^2 (clusters of 8) always: 64 problems 1174 against 571.
         if (p == 1 && (opt.use_graph & ~1) == 0 && !getenv("SGP_NO_CLUSTER")) {      // any experiment switch: launch-per-pass
-            small_k = get_small<T>(ny, nx, G.masked != 0, &small_nc, &small_threads, &small_smem, &small_er, &small_ec);
-            if (small_k) {
-                bool ok = cudaFuncSetAttribute((const void *)small_k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)small_smem) == cudaSuccess;
-                if (ok && small_nc > 8) ok = cudaFuncSetAttribute((const void *)small_k, cudaFuncAttributeNonPortableClusterSizeAllowed, 1) == cudaSuccess;
+            small_k = get_small<T>(ny, nx, G.masked != 0, false, &small_nc, &small_threads, &small_smem, &small_er, &small_ec);
+            small_k_rl = small_k ? get_small<T>(ny, nx, G.masked != 0, true, &small_nc, &small_threads, &small_smem, &small_er, &small_ec) : nullptr;
+            for (small_kernel_t<T> *kk : {&small_k, &small_k_rl}) {
+                if (!*kk) continue;
+                bool ok = cudaFuncSetAttribute((const void *)*kk, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)small_smem) == cudaSuccess;
+                if (ok && small_nc > 8) ok = cudaFuncSetAttribute((const void *)*kk, cudaFuncAttributeNonPortableClusterSizeAllowed, 1) == cudaSuccess;
                 if (ok) {
                     cudaLaunchConfig_t cfg;
                     memset(&cfg, 0, sizeof(cfg));
@@ -243,11 +246,12 @@ template <typename T> struct PlanImpl : PlanBase {
                     at[0].val.clusterDim.x = small_nc; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
                     cfg.attrs = at; cfg.numAttrs = 1;
                     int nclusters = 0;
-                    ok = cudaOccupancyMaxActiveClusters(&nclusters, (const void *)small_k, &cfg) == cudaSuccess && nclusters > 0;
+                    ok = cudaOccupancyMaxActiveClusters(&nclusters, (const void *)*kk, &cfg) == cudaSuccess && nclusters > 0;
                     if (ok && nb > 16 && small_nc > 8) ok = false;
                 }
-                if (!ok) { small_k = nullptr; (void)cudaGetLastError(); }
+                if (!ok) { *kk = nullptr; (void)cudaGetLastError(); }
             }
+            if (!small_k) small_k_rl = nullptr;
         }
         // twiddles, computed in double on the host
         std::vector<C> h;
@@ -396,7 +400,7 @@ template <typename T> struct PlanImpl : PlanBase {
         return launch_pdl(k, dim3(col_grid, 1, lnb), col_threads, col_smem, P, st);
     }
     // `iters` SGP iterations of all lnb problems in one launch, one cluster per problem (small.cuh)
-    int launch_small(const DevOpts &o, const Trace &tr, double bconst0, int iters, cudaStream_t st)
+    int launch_small(small_kernel_t<T> kern, const DevOpts &o, const Trace &tr, double bconst0, int iters, cudaStream_t st)
     {
         SmallParams<T> S;
         memset(&S, 0, sizeof(S));
@@ -416,7 +420,7 @@ template <typename T> struct PlanImpl : PlanBase {
         cudaMemsetAsync(dbg, 0, 64 * sizeof(unsigned long long), st);
         S.dbg = dbg;
 #endif
-        SGP_CUDA_TRY(cudaLaunchKernelEx(&cfg, small_k, S));
+        SGP_CUDA_TRY(cudaLaunchKernelEx(&cfg, kern, S));
         launches++;
 #ifdef SGP_SMALL_TIMING
         if (getenv("SGP_SMALL_DBG")) {

@@ -454,8 +454,9 @@ int PlanImpl<T>::run_batched(int algorithm, const void *const *g, const void *co
         if (status[b] != hs[b].status) SGP_CUDA_TRY(cudaMemcpyAsync(&pp(ct, b)->status, &status[b], sizeof(int), cudaMemcpyHostToDevice, st));
 
     // small grids: the cluster kernel (small.cuh) for what it covers, the launch-per-pass path for everything else
-    const bool small_run = small_k && algorithm == SGP_ALG_SGP && !b_is_array && !o.flux_constraint && !o.refresh_every &&
-                           ro.stop_rule != SGP_STOP_MINERR && !tr.force_alpha && !tr.force_lambda && !tr.err && !profiling;
+    const bool small_ok = !b_is_array && ro.stop_rule != SGP_STOP_MINERR && !tr.force_alpha && !tr.force_lambda && !tr.err && !profiling;
+    const bool small_run = small_k && small_ok && algorithm == SGP_ALG_SGP && !o.flux_constraint && !o.refresh_every;
+    const bool small_rl = small_k_rl && small_ok && algorithm == SGP_ALG_RL;
     if (algorithm == SGP_ALG_SGP && !small_run) {     // arguments of the Armijo backtracking (aux.cuh), read from device memory
         std::vector<BtInfo<T>> bis((size_t)nb);
         for (int b = 0; b < nb; ++b) {
@@ -482,7 +483,7 @@ int PlanImpl<T>::run_batched(int algorithm, const void *const *g, const void *co
             while (any_running()) {
                 const int todo = ro.max_iter - done;
                 if (todo < 1) { for (int b = 0; b < nb; ++b) if (status[b] == 0) status[b] = SGP_REASON_MAXIT; break; }
-                if ((rc = launch_small(o, tr, bconst[0], todo, st))) return rc;
+                if ((rc = launch_small(small_k, o, tr, bconst[0], todo, st))) return rc;
                 if ((rc = read_ctrl())) return rc;
                 done = ro.max_iter;
                 for (int b = 0; b < nb; ++b) {
@@ -532,6 +533,16 @@ int PlanImpl<T>::run_batched(int algorithm, const void *const *g, const void *co
                     hs[b].k = done;
                     if (status[b] == 0) status[b] = SGP_REASON_MAXIT;
                 }
+            }
+        } else if (small_rl) {
+            // RL rounds inside the cluster kernel (small.cuh): one launch runs every problem to its stopping rule
+            int rounds = 0;
+            while (any_running()) {
+                int todo = ro.max_iter + 1 - rounds; if (todo < 1) todo = 1;
+                if ((rc = launch_small(small_k_rl, o, tr, bconst[0], todo, st))) return rc;
+                rounds += todo;
+                if ((rc = read_ctrl())) return rc;
+                for (int b = 0; b < nb; ++b) if (status[b] == 0) status[b] = hs[b].status;
             }
         } else {
             int rounds = 0;     // round k evaluates J0(f(k)) and, unless a rule fires, makes update k+1
@@ -623,7 +634,7 @@ int PlanImpl<T>::run_batched(int algorithm, const void *const *g, const void *co
         R.err_final = tr.err ? h.err : 0.0;
         R.setup_ms = ms01; R.loop_ms = ms12;
         R.kernel_launches = launches - launches0;
-        R.fused_linesearch = (algorithm == SGP_ALG_SGP && small_run) ? 2 : (algorithm == SGP_ALG_SGP && fuse_ls) ? 1 : 0;
+        R.fused_linesearch = ((algorithm == SGP_ALG_SGP && small_run) || small_rl) ? 2 : (algorithm == SGP_ALG_SGP && fuse_ls) ? 1 : 0;
         R.status = status[b] < 0 ? status[b] : SGP_OK;
         if (status[b] < 0 && worst == SGP_OK) worst = status[b];
     }

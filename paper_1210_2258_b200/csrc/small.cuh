@@ -15,8 +15,8 @@
 //
 // Same arithmetic per pixel as the launch-per-pass path (ew.cuh), same FFT (fft_core.cuh), same tables and transfer
 // functions; sums are grouped per CTA of this kernel, so the two paths agree to rounding, not bit for bit.
-// Scope: SGP, one image, with or without boundary-effect correction, constant background, no replay / flux / refresh / Eq.25
-// options -- the host
+// Scope: SGP and Richardson-Lucy, one image, with or without boundary-effect correction, constant background, no replay / flux /
+// refresh / Eq.25 options -- the host
 // (plan_run.inl) takes the launch-per-pass path for everything else.
 #pragma once
 #include <cooperative_groups.h>
@@ -136,7 +136,8 @@ __device__ __forceinline__ void small_fwd(cx<T> (&v)[E], cx<T> *line, const int 
 }
 
 // MK: boundary-effect correction (Eq.16-23): S inside the grid, alphaR > 0 marks R and 1/alphaR is the weight M_R/alpha
-template <typename T, int NY, int NX, int NC, bool MK>
+// RL: plain Richardson-Lucy (Eq.1 / Eq.21, with the relaxations Eq.3 / Eq.4) instead of SGP: the same passes, one global sum per round
+template <typename T, int NY, int NX, int NC, bool MK, bool RL>
 __global__ void __launch_bounds__(SmallCfg<T, NY, NX, NC>::NT, 1) small_sgp_kernel(const SmallParams<T> P)
 {
     namespace cgx = cooperative_groups;
@@ -367,6 +368,88 @@ __global__ void __launch_bounds__(SmallCfg<T, NY, NX, NC>::NT, 1) small_sgp_kern
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     cluster.sync();                                             // every CTA's barriers exist before anybody sends
+    if constexpr (RL) {
+        // ---- a12: round k = J0(f(k)), the stopping rules, and unless one fires f(k+1) = (M_R/alpha) o f o A^T(g / (A f + b)) (Eq.1 / Eq.21).
+        //      One cluster barrier per round (the sum of J0); the mbarriers of the four transposes order the re-use of the slabs.
+        const T rx = (T)o.rl_relax, lamr = (T)o.rl_linear;
+        const bool relax = o.rl_relax != 1.0, lin = o.rl_linear != 1.0;
+        if (ract) {
+            ldrow(f2, f);
+#pragma unroll
+            for (int e = 0; e < Er; ++e) vr[e] = f2[e];
+            small_fwd<T, L, Er>(vr, line, t, rsync, put_row, P.tw_r, P.tw_h);
+        }
+        for (int it = 0; it < P.iters; ++it) {
+            wait_cin();
+            col_pass(false);                                    // A f (Eq.16)
+            wait_rin();
+            if (ract) ldrow(g2, gpl);
+            inv_rows();                                         // v[] = A f on this CTA's rows
+            {
+                double pr[1] = {0.0};
+                if (ract) {
+#pragma unroll
+                    for (int e = 0; e < Er; ++e) {
+                        if (!in_s0(e)) vr[e].x = (T)0;
+                        if (!in_s1(e)) vr[e].y = (T)0;
+                        const T y0 = vr[e].x + bcst, y1 = vr[e].y + bcst;
+                        if constexpr (MK) pr[0] += (double)kl_pair_s(g2[e].x, y0, g2[e].y, y1, in_s0(e), in_s1(e));
+                        else pr[0] += (double)kl_pair(g2[e].x, y0, g2[e].y, y1);
+                    }
+                }
+                block_reduce_sum<1>(pr, red);
+                send_partials(pr, 1);
+            }
+            cluster.sync();
+            if (tid == 0) {                                     // J0(f(k)) and the stopping rules before the k-th update (row_inv.cuh: QJ_RL)
+                const double J = total(0);
+                const int k = ct->k;
+                const double Jold = ct->J;
+                ct->J = J;
+                if (tr.J) tr.J[k] = J;
+                ct->nfft += 2ULL;
+                if (!isfinite(J)) ct->status = SGP_ERR_NONFINITE;
+                else { const int r = stop_test(o, k, J, Jold, k > 0); if (r) ct->status = r; else ct->k = k + 1; }
+                bc.status = ct->status;
+            }
+            __syncthreads();
+            if (bc.status != 0) break;
+            if (ract) {
+#pragma unroll
+                for (int e = 0; e < Er; ++e) vr[e] = ratio_pair(e, g2[e], vr[e]);
+                small_fwd<T, L, Er>(vr, line, t, rsync, put_row, P.tw_r, P.tw_h);
+            }
+            wait_cin();
+            col_pass(true);                                     // A^T r (Eq.17)
+            wait_rin();
+            if (ract && !PF) ldrow(f2, f);
+            inv_rows();
+            const bool more = it + 1 < P.iters;
+            if (ract) {
+#pragma unroll
+                for (int e = 0; e < Er; ++e) {
+                    const T fa[2] = {f2[e].x, f2[e].y}, wa[2] = {vr[e].x, vr[e].y};
+                    T ya[2];
+#pragma unroll
+                    for (int c = 0; c < 2; ++c) {
+                        T wv = Wc;
+                        if constexpr (MK) { const T av = c == 0 ? a2[e].x : a2[e].y; wv = av > (T)0 ? (T)1 / av : (T)0; }
+                        ya[c] = wv * fa[c] * wa[c];
+                        if (relax) ya[c] = fa[c] * pow(fmax(wv * wa[c], (T)0), rx);                              // Eq.3
+                        if (lin) ya[c] = fmax(fa[c] - lamr * (fa[c] * ((T)1 - wv * wa[c])), (T)0);              // Eq.4, projected on f >= 0 (A25)
+                    }
+                    const C yn = mk<T>(ya[0], ya[1]);
+                    st2<T>(f + base + 2 * (t + TFr * e), yn);
+                    f2[e] = yn; vr[e] = yn;
+                }
+                if (more) small_fwd<T, L, Er>(vr, line, t, rsync, put_row, P.tw_r, P.tw_h);
+            }
+            if (tid == 0) ct->nfft += 2ULL;
+            if (!more) break;
+        }
+        if (rank == 0 && tid == 0) *gct = sct;
+        return;
+    }
     ratio_rows();
     double gd_part = 0.0, Jref = 0.0, gdt = 0.0;
     for (int it = 0; it < P.iters; ++it) {

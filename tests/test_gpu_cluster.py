@@ -246,3 +246,70 @@ def test_mosaic_runs_its_sub_domains_through_the_cluster_kernel():
     rp = res[1 | NO_CLUSTER][1] if isinstance(res[1 | NO_CLUSTER][1], (list, tuple)) else [res[1 | NO_CLUSTER][1]]
     assert all(x.fused_linesearch == 2 for x in rs) and all(x.fused_linesearch != 2 for x in rp)
     assert rel_l2(res[1][0], res[1 | NO_CLUSTER][0]) <= 1e-4
+
+
+# ------------------------------------------------------------------------------------------------ Richardson-Lucy rounds in the cluster kernel
+def _rl_both(w, dt, S=None, **kw):
+    """(f, result) of rl_* through the cluster kernel and through the launch-per-pass path"""
+    out = []
+    for ug in (1, 1 | NO_CLUSTER):
+        o = B.default_options(**{**kw, "use_graph": ug})
+        plan = B.Plan([dev(w["psf"][0], dt)], S=S, opts=o)
+        f, r = plan.rl([dev(w["g"][0], dt)], w["b"], opts=o)
+        out.append((f.cpu().numpy(), r))
+        plan.close()
+    return out
+
+
+@pytest.mark.parametrize("dt", [np.float32, np.float64])
+@pytest.mark.parametrize("variant", ["plain", "relax", "linear", "boundary"])
+def test_cluster_kernel_richardson_lucy(variant, dt):
+    """Eq.1 (plain), Eq.3 (multiplicative relaxation, exponent 1.5), Eq.4 (linear relaxation, lambda = 1.4) at 256^2 and Eq.21
+    (boundary-effect correction, 160^2 in 256^2): one update at 1e-5 / 1e-11, 30 updates at 1e-4 / 1e-10 with the whole J0 trace
+    (RL does not branch: DESIGN.md 3a), against the oracle; and the launch-per-pass path to rounding"""
+    _need_gpu()
+    if variant == "boundary":
+        w = synth.make("C3", s=160, sbar=256, n_stars=150, max_iter=30, fwhm=8.0)
+    else:
+        w = synth.make("C0", n=256)
+    extra = {"relax": {"rl_relax": 1.5}, "linear": {"rl_linear": 1.4}}.get(variant, {})
+    for it in (1, 30):
+        kw = {**w["opts"], "max_iter": it, "stop_rule": 0, **extra}
+        fo, ro = oracle_run(w, alg="rl", **{"max_iter": it, "stop_rule": 0, **extra})
+        (fg, rg), (fp, rp) = _rl_both(w, dt, S=w.get("S"), **kw)
+        assert rg.fused_linesearch == 2 and rp.fused_linesearch != 2
+        assert rg.iterations == ro.iterations == it and rg.n_fft2 == ro.n_fft2 == rp.n_fft2
+        e = rel_l2(fg, fo)
+        print(f"[measured] cluster_rl_{variant} {np.dtype(dt).name} rel_l2_{it}it = {e:.3e}")
+        assert e <= ((1e-5 if it == 1 else 1e-4) if dt == np.float32 else (1e-11 if it == 1 else 1e-10))
+        assert np.max(np.abs(fg - fo)) <= (1e-3 if dt == np.float32 else 1e-9) * np.max(fo) and np.all(fg >= 0)
+        assert np.max(np.abs(rg.J - ro.J) / np.abs(ro.J)) <= (1e-4 if dt == np.float32 else 1e-10)
+        assert rel_l2(fg, fp) <= (2e-5 if dt == np.float32 else 1e-12)
+
+
+@pytest.mark.parametrize("dt", [np.float32, np.float64])
+def test_cluster_kernel_rl_stop_rule_and_batches(dt):
+    """RL with the Eq.24 rule stops at the oracle's iteration; a batch of 5 problems (different backgrounds, different stopping
+    iterations) equals the same problems run alone, bit for bit"""
+    _need_gpu()
+    n, nb = 128, 5
+    ws = [synth.make("C0", n=n, seed_idx=90 + i) for i in range(nb)]
+    kw = {**ws[0]["opts"], "max_iter": 400, "stop_rule": 1, "tol": 1e-3}
+    o = B.default_options(**kw)
+    g = [[dev(w["g"][0], dt)] for w in ws]
+    b = [[10.0 + i] for i in range(nb)]
+    bp = B.BatchedPlan(nb, [dev(ws[0]["psf"][0], dt)], opts=o)
+    fb, rb = bp.run_batched(B.ALG_RL, g, b, opts=o)
+    bp.close()
+    single = B.Plan([dev(ws[0]["psf"][0], dt)], opts=o)
+    for i in range(nb):
+        fs, rs = single.run(B.ALG_RL, g[i], b[i], opts=o)
+        assert rb[i].fused_linesearch == 2 and rs.fused_linesearch == 2
+        assert torch.equal(fb[i], fs) and rb[i].iterations == rs.iterations and np.array_equal(rb[i].J, rs.J)
+        P = oracle.Problem(ws[0]["psf"])
+        fo, ro = P.rl(ws[i]["g"], [np.full((n, n), b[i][0])], opts=oracle.default_options(**kw))
+        assert rb[i].stop_reason == ro.stop_reason == 2 and abs(rb[i].iterations - ro.iterations) <= (1 if dt == np.float32 else 0)
+        if rb[i].iterations == ro.iterations:
+            assert rel_l2(fb[i].cpu().numpy(), fo) <= (1e-3 if dt == np.float32 else 1e-9)
+    single.close()
+    assert len({r.iterations for r in rb}) > 1
