@@ -373,7 +373,7 @@ def measure_other(name: str, alg_name: str, steps: int, dev, peak: float):
 
 def measure_batched(nb: int, steps: int, dev):
     """problems of the C0 recipe (256^2, different seeds) through ONE batched plan beside one C0 problem
-    through an ordinary plan: aggregate iterations/s.  One problem and small batches (<= 16) run one thread-block cluster per
+    through an ordinary plan: aggregate iterations/s.  One problem and batches of up to 32 run one thread-block cluster per
     problem (csrc/small.cuh, `path` = cluster); the large batch runs launch-per-pass, every kernel launched once for all problems
     (blockIdx.z = problem)"""
     import torch

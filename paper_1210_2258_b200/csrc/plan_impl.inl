@@ -227,16 +227,19 @@ template <typename T> struct PlanImpl : PlanBase {
 
         // Small grids: one image (with or without boundary-effect correction) at 128^2 / 256^2 iterates inside ONE kernel run by
         // one thread-block cluster per problem (small.cuh) when the device can co-schedule such a cluster; use_graph bit 7 (or any other
-        // experiment switch) keeps the launch-per-pass path.  A batched plan of 256^2 problems uses it up to 16 problems (the device
-        // holds about 7 clusters of 16 CTAs at once: 4 problems run 151 kit/s this way against 71 kit/s launch-per-pass, 16 problems 214
-        // against 195, 32 problems 261 against 326, 64 problems 270 against 394); 128^2 (clusters of 8) always: 64 problems 1174 against 571.
+        // experiment switch) keeps the launch-per-pass path.  Batched plans run one cluster per problem: the device holds 7 clusters of 16 CTAs
+        // in the one-CTA-per-SM form of the kernel and 14 in its two-CTAs-per-SM form, which is taken when the batch is larger than 7.
+        // Aggregate kit/s at 256^2, 100 iterations per problem (form 1 / form 2 / launch-per-pass): 4 problems 163 / 154 / 71, 8 problems
+        // 177 / 230 / 121, 16 problems 230 / 272 / 195, 32 problems 281 / 346 / 326, 64 problems 292 / 385 / 396 -- so 256^2 batches of more
+        // than 32 problems stay launch-per-pass; 128^2 (clusters of 8) always runs in clusters.
         if (p == 1 && (opt.use_graph & ~1) == 0 && !getenv("SGP_NO_CLUSTER")) {      // any experiment switch: launch-per-pass
-            small_k = get_small<T>(ny, nx, G.masked != 0, false, &small_nc, &small_threads, &small_smem, &small_er, &small_ec);
-            small_k_rl = small_k ? get_small<T>(ny, nx, G.masked != 0, true, &small_nc, &small_threads, &small_smem, &small_er, &small_ec) : nullptr;
-            for (small_kernel_t<T> *kk : {&small_k, &small_k_rl}) {
-                if (!*kk) continue;
-                bool ok = cudaFuncSetAttribute((const void *)*kk, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)small_smem) == cudaSuccess;
-                if (ok && small_nc > 8) ok = cudaFuncSetAttribute((const void *)*kk, cudaFuncAttributeNonPortableClusterSizeAllowed, 1) == cudaSuccess;
+            // which form: one CTA per SM (255 registers, planes prefetched) while the device holds all clusters of the plan at once,
+            // two CTAs per SM for larger batches; SGP_SMALL_FORM = 1 / 2 forces one (experiments)
+            auto max_clusters = [&](small_kernel_t<T> kk) -> int {
+                if (!kk) return 0;
+                bool ok = cudaFuncSetAttribute((const void *)kk, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)small_smem) == cudaSuccess;
+                if (ok && small_nc > 8) ok = cudaFuncSetAttribute((const void *)kk, cudaFuncAttributeNonPortableClusterSizeAllowed, 1) == cudaSuccess;
+                int nclusters = 0;
                 if (ok) {
                     cudaLaunchConfig_t cfg;
                     memset(&cfg, 0, sizeof(cfg));
@@ -245,12 +248,26 @@ template <typename T> struct PlanImpl : PlanBase {
                     at[0].id = cudaLaunchAttributeClusterDimension;
                     at[0].val.clusterDim.x = small_nc; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
                     cfg.attrs = at; cfg.numAttrs = 1;
-                    int nclusters = 0;
-                    ok = cudaOccupancyMaxActiveClusters(&nclusters, (const void *)*kk, &cfg) == cudaSuccess && nclusters > 0;
-                    if (ok && nb > 16 && small_nc > 8) ok = false;
+                    ok = cudaOccupancyMaxActiveClusters(&nclusters, (const void *)kk, &cfg) == cudaSuccess;
                 }
-                if (!ok) { *kk = nullptr; (void)cudaGetLastError(); }
+                if (!ok) { (void)cudaGetLastError(); return 0; }
+                return nclusters;
+            };
+            small_kernel_t<T> k1 = get_small<T>(ny, nx, G.masked != 0, false, false, &small_nc, &small_threads, &small_smem, &small_er, &small_ec);
+            const int c1 = max_clusters(k1);
+            bool two = false;
+            if (k1 && nb > c1) {     // only where the second form really holds more clusters (at 128^2 the first already has two CTAs per SM)
+                int a_, b_, e_, f_; size_t c_;
+                two = max_clusters(get_small<T>(ny, nx, G.masked != 0, false, true, &a_, &b_, &c_, &e_, &f_)) > c1;
             }
+            if (const char *f = getenv("SGP_SMALL_FORM")) two = f[0] == '2';
+            small_k = get_small<T>(ny, nx, G.masked != 0, false, two, &small_nc, &small_threads, &small_smem, &small_er, &small_ec);
+            small_k_rl = small_k ? get_small<T>(ny, nx, G.masked != 0, true, two, &small_nc, &small_threads, &small_smem, &small_er, &small_ec) : nullptr;
+            const int cs = max_clusters(small_k), cr = max_clusters(small_k_rl);
+            if (getenv("SGP_SMALL_DEBUG")) fprintf(stderr, "[sgp] cluster kernel: nb %d, clusters resident: form 1 %d, chosen form %d: %d (RL %d)\n", nb, c1, two ? 2 : 1, cs, cr);
+            if (cs < 1) small_k = nullptr;
+            if (cr < 1) small_k_rl = nullptr;
+            if (small_k && nb > 32 && small_nc > 8 && !getenv("SGP_SMALL_FORM")) { small_k = nullptr; small_k_rl = nullptr; }
             if (!small_k) small_k_rl = nullptr;
         }
         // twiddles, computed in double on the host

@@ -137,8 +137,10 @@ __device__ __forceinline__ void small_fwd(cx<T> (&v)[E], cx<T> *line, const int 
 
 // MK: boundary-effect correction (Eq.16-23): S inside the grid, alphaR > 0 marks R and 1/alphaR is the weight M_R/alpha
 // RL: plain Richardson-Lucy (Eq.1 / Eq.21, with the relaxations Eq.3 / Eq.4) instead of SGP: the same passes, one global sum per round
-template <typename T, int NY, int NX, int NC, bool MK, bool RL>
-__global__ void __launch_bounds__(SmallCfg<T, NY, NX, NC>::NT, 1) small_sgp_kernel(const SmallParams<T> P)
+// TWO: compiled for two resident CTAs per SM (128 registers instead of 255, planes loaded where they are used): two clusters share
+// the SMs of a GPC and hide each other's latencies -- the form for batches larger than the device can hold clusters of the first form
+template <typename T, int NY, int NX, int NC, bool MK, bool RL, bool TWO>
+__global__ void __launch_bounds__(SmallCfg<T, NY, NX, NC>::NT, TWO ? 2 : 1) small_sgp_kernel(const SmallParams<T> P)
 {
     namespace cgx = cooperative_groups;
     using C = cx<T>;
@@ -340,7 +342,7 @@ __global__ void __launch_bounds__(SmallCfg<T, NY, NX, NC>::NT, 1) small_sgp_kern
     // planes of this thread's pixels.  PF (float): they are requested BEFORE the transform whose epilogue needs them and stay in
     // registers while they are valid (f from the gradient step to the update, d from the projection, g and q from the line
     // search); double: loaded where they are used (twice the registers).
-    constexpr bool PF = sizeof(T) == 4;
+    constexpr bool PF = sizeof(T) == 4 && !TWO;
     C f2[Er], d2[Er], o2[Er], g2[Er], q2[Er];
     auto ldrow = [&](C (&a)[Er], const T *plane) {
 #pragma unroll

@@ -22,7 +22,8 @@ template <typename T> struct SmallParams {
 template <typename T> using small_kernel_t = void (*)(const SmallParams<T>);
 // kernel for this geometry (nullptr: none), its cluster size, threads per CTA, dynamic shared memory and the elements per thread of
 // its row / column FFT plans (fft_core.cuh: plan_radix), whose pass tables the host supplies
-template <typename T> small_kernel_t<T> get_small(int ny, int nx, bool masked, bool rl, int *nc, int *threads, size_t *smem, int *er, int *ec);
+// two: the form compiled for two resident CTAs per SM (larger batches)
+template <typename T> small_kernel_t<T> get_small(int ny, int nx, bool masked, bool rl, bool two, int *nc, int *threads, size_t *smem, int *er, int *ec);
 
 
 }  // namespace sgpk

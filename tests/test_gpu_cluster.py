@@ -165,9 +165,10 @@ def test_cluster_kernel_and_launch_per_pass_path_agree(dt, tol):
 
 
 def test_cluster_kernel_in_batched_plans():
-    """A batched plan runs one cluster per problem up to 16 problems of 256^2: 6 problems of 256^2 each equal --
+    """A batched plan runs one cluster per problem up to 32 problems of 256^2: 6 problems of 256^2 each equal --
     bit for bit -- the same problem run alone (every problem is summed by its own cluster in the same order), with different
-    backgrounds and stopping iterations; 40 problems take the launch-per-pass path and match the oracle all the same"""
+    backgrounds and stopping iterations; 12 problems run in the two-CTAs-per-SM form of the kernel; 40 problems take the launch-per-pass
+    path and match the oracle all the same"""
     _need_gpu()
     n, dt = 256, np.float32
     ws = [synth.make("C0", n=n, seed_idx=60 + i) for i in range(40)]
@@ -187,6 +188,18 @@ def test_cluster_kernel_in_batched_plans():
         assert torch.equal(fb[i], fs) and rb[i].iterations == rs.iterations and np.array_equal(rb[i].J, rs.J)
     single.close()
     assert len({r.iterations for r in rb}) > 1
+    # 12 problems: more than the device holds clusters of the one-CTA-per-SM form, so the two-CTAs-per-SM form runs them
+    nb2 = 12
+    g = [[dev(w["g"][0], dt)] for w in ws[:nb2]]
+    for it, tol in ((1, 1e-5), (12, 1e-3)):
+        oi = B.default_options(**{**ws[0]["opts"], "max_iter": it, "stop_rule": 0})
+        bp = B.BatchedPlan(nb2, [dev(psf[0], dt)], opts=oi)
+        fb, rb = bp.run_batched(B.ALG_SGP, g, [[10.0]] * nb2, opts=oi)
+        bp.close()
+        assert all(r.fused_linesearch == 2 for r in rb)
+        for i in (0, 5, 11):
+            fo, ro = _oracle(ws[i], n, **{**ws[0]["opts"], "max_iter": it, "stop_rule": 0})
+            assert rel_l2(fb[i].cpu().numpy(), fo) <= tol and np.array_equal(rb[i].rule, ro.rule) and np.array_equal(rb[i].backtracks, ro.backtracks)
     # many problems: launch-per-pass
     o1 = B.default_options(**{**ws[0]["opts"], "max_iter": 1, "stop_rule": 0})
     g = [[dev(w["g"][0], dt)] for w in ws]
