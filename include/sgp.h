@@ -150,7 +150,7 @@ typedef struct sgp_result {
      * (input; NULL = not given).  When given, trace_err[k] = ||f(k) - f~||_2 / ||f~||_2 for k = 0..iterations (optional HOST array
      * of max_iter + 2 doubles; entry iterations + 1 holds the error of the discarded step after a SGP_STOP_MINERR stop) and
      * err_final = the error of the returned iterate.  SGP_STOP_MINERR stops at the first k whose next step would increase the
-     * error and returns f(k) (sgp_* and rl_*; DESIGN reading A27). */
+     * error and returns f(k) (sgp_*, rl_* and, per cycle, osem_*; DESIGN reading A27). */
     const void *truth;
     double *trace_err;
     double err_final;
@@ -226,9 +226,11 @@ int rl_boundary(int p, const void *const *g, const void *const *psf, const void 
 /* OSEM, Algorithm 2 of the paper: one iteration is a cycle over the p images,
  *   h <- h o A_j^T( g_j / (A_j h + b_j) ), j = 1..p (Eq.15);  boundary form: h <- (M_R/alpha_j) o h o ... (Eq.22),
  * 4p two-dimensional FFTs per iteration, on the kernels of rl_*.  Same arguments as rl_multi /
- * rl_boundary (device pointers).  opt->max_iter cycles are run: stop_rule must be SGP_STOP_MAXIT (the paper stops
- * OSEM by the reconstruction error, which needs the true object), else SGP_ERR_UNSUPPORTED.  J0 (Eq.12) is evaluated
- * once, at the final iterate (res->J0_final); no per-iteration traces.  (sgp_plan_run takes SGP_ALG_OSEM as well.) */
+ * rl_boundary (device pointers).  opt->max_iter cycles are run: stop_rule must be SGP_STOP_MAXIT or -- the way the paper
+ * stops OSEM, by the reconstruction error of Eq.25, which needs the true object in res->truth --
+ * SGP_STOP_MINERR (the error is evaluated after every cycle; the first cycle that would increase it is discarded and the
+ * iterate before it returned), else SGP_ERR_UNSUPPORTED.  J0 (Eq.12) is evaluated once, at the returned iterate
+ * (res->J0_final); of the per-iteration traces only trace_err is filled.  (sgp_plan_run takes SGP_ALG_OSEM as well.) */
 int osem_multi(int p, const void *const *g, const void *const *psf, const void *const *b_arr,
                const double *b_const, const void *f0, void *f_out, int ny, int nx, int dtype,
                const sgp_options *opt, sgp_result *res, void *stream);

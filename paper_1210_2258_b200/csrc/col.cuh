@@ -21,6 +21,21 @@ namespace sgpk {
 
 enum ColMode { CM_FWD = 0, CM_CONJSUM = 1, CM_MULT = 2, CM_INV = 3 };
 
+// experiment: pass twiddles of the float column transforms as powers of one table entry (fft_core.cuh: TWP)
+#ifndef SGP_COL_TWP
+#define SGP_COL_TWP 0
+#endif
+template <typename T> constexpr bool kColTwp = SGP_COL_TWP && sizeof(T) == 4;
+// experiment: the tiles of the NEXT wave of CTAs requested into L2 by the CTAs of this one (ColParams::pf_ahead), so that DRAM
+// works while the SMs transform instead of idling until the next wave asks for its tiles all at once
+#ifndef SGP_COL_PF2
+#define SGP_COL_PF2 0
+#endif
+__device__ __forceinline__ void bulk_prefetch_l2(const void *gmem, unsigned int bytes)
+{
+    asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(gmem), "r"(bytes) : "memory");
+}
+
 // Bulk asynchronous copy global -> shared by the TMA engine (cp.async.bulk, SASS UBLKCP): ONE instruction of one
 // thread moves a whole tile (contiguous in the tile-major layout); completion is signalled on an mbarrier.
 __device__ __forceinline__ unsigned int smem_u32(const void *p) { return (unsigned int)__cvta_generic_to_shared(p); }
@@ -153,13 +168,22 @@ __device__ __forceinline__ void col_body(const ColParams<T> &P)
             for (int j = 0; j < p; ++j) {
                 const int u1 = it * p + j + 1, it1 = u1 / p, j1 = u1 - it1 * p;
                 mbar_wait(&bars[0], phA); phA ^= 1;                 // spectrum of this unit has landed
+                if constexpr (SGP_COL_PF2 != 0) {
+                    if (tid == 0 && it == 0 && j == 0 && P.pf_ahead > 0 && (int)blockIdx.x + P.pf_ahead < ntiles) {
+                        const size_t t2 = (size_t)P.pf_ahead * X.tile_len;
+                        for (int jj = 0; jj < p; ++jj) {
+                            bulk_prefetch_l2(P.in + (size_t)jj * P.specplane + X.tile_of(0) + t2, tile_bytes);
+                            bulk_prefetch_l2(P.khat + (size_t)jj * P.specplane + X.ktile_of(0) + t2, tile_bytes);
+                        }
+                    }
+                }
 #pragma unroll
                 for (int e = 0; e < E; ++e) v[e] = X.bufA[tid + e * nthr];
                 if (u1 < units) {
                     __syncthreads();
                     if (tid == 0) bulk_load(X.bufA, P.in + (size_t)j1 * P.specplane + X.tile_of(it1), tile_bytes, &bars[0]);
                 }
-                fft_block<T, L, E, -1>(v, X.smc, Cc, t, P.tw, sync);
+                fft_block<T, L, E, -1, false, kColTwp<T>>(v, X.smc, Cc, t, P.tw, sync);
                 if (packed) {
                     if (pk) {
 #pragma unroll
@@ -185,7 +209,7 @@ __device__ __forceinline__ void col_body(const ColParams<T> &P)
 #pragma unroll
                 for (int e = 0; e < E; ++e) v[e] = acc[e];
             }
-            fft_block<T, L, E, +1>(v, X.smc, Cc, t, P.tw, sync);
+            fft_block<T, L, E, +1, false, kColTwp<T>>(v, X.smc, Cc, t, P.tw, sync);
             C *dst = P.out + X.tile_of(it) + tid;
 #pragma unroll
             for (int e = 0; e < E; ++e) dst[(size_t)e * nthr] = v[e];
@@ -195,13 +219,20 @@ __device__ __forceinline__ void col_body(const ColParams<T> &P)
             const bool packed = (blockIdx.x == 0 && it == 0);
             const bool pk = packed && X.c == 0;
             mbar_wait(&bars[0], phA); phA ^= 1;                     // spectrum of tile it has landed
+            if constexpr (SGP_COL_PF2 != 0) {
+                if (tid == 0 && it == 0 && P.pf_ahead > 0 && (int)blockIdx.x + P.pf_ahead < ntiles) {
+                    const size_t t2 = (size_t)P.pf_ahead * X.tile_len;
+                    bulk_prefetch_l2(P.in + X.tile_of(0) + t2, tile_bytes);
+                    for (int jj = 0; jj < p; ++jj) bulk_prefetch_l2(P.khat + (size_t)jj * P.specplane + X.ktile_of(0) + t2, tile_bytes);
+                }
+            }
 #pragma unroll
             for (int e = 0; e < E; ++e) v[e] = X.bufA[tid + e * nthr];
             if (it + 1 < my_tiles) {
                 __syncthreads();
                 if (tid == 0) bulk_load(X.bufA, P.in + X.tile_of(it + 1), tile_bytes, &bars[0]);
             }
-            fft_block<T, L, E, -1>(v, X.smc, Cc, t, P.tw, sync);
+            fft_block<T, L, E, -1, false, kColTwp<T>>(v, X.smc, Cc, t, P.tw, sync);
             if (packed) {
                 if (pk) {
 #pragma unroll
@@ -222,7 +253,7 @@ __device__ __forceinline__ void col_body(const ColParams<T> &P)
                     }
                 }
                 if (pk) packed_fix<T, L, E, false>(w, pack, P.khatB + (size_t)j * L, t);
-                fft_block<T, L, E, +1>(w, X.smc, Cc, t, P.tw, sync);
+                fft_block<T, L, E, +1, false, kColTwp<T>>(w, X.smc, Cc, t, P.tw, sync);
                 C *dst = P.out + (size_t)j * P.specplane + X.tile_of(it) + tid;
 #pragma unroll
                 for (int e = 0; e < E; ++e) dst[(size_t)e * nthr] = w[e];

@@ -98,6 +98,7 @@ template <typename T> struct ColParams {
     int ntiles;                       // (nx/2)/C
     int check_status;
     size_t slab;                      // batched plans: bytes between the per-problem arrays (in, out, pack, ct) of consecutive problems
+    int pf_ahead;                     // > 0: CTA b asks L2 for the tiles of CTA b + pf_ahead (the next wave) once its own have landed
 };
 
 // ---------------------------------------------------------------- elementwise pieces

@@ -162,13 +162,15 @@ __global__ void plane_sum_tmp_kernel(const T *x, size_t n, Ctrl *ct)
 // candidate; with SGP_STOP_MINERR an increase discards the step (pending <- 0, k, J0 and the backtrack count are taken
 // back) and stops the run, so that the iterate of minimum error is returned (reading A27).  mode 2 (RL): the candidate is
 // the plane `cand` (the update was written there instead of f); ct->commit tells rl_commit_kernel whether to adopt it.
+// mode 3 (OSEM, per cycle): the candidate h(k+1) is already in f, h(k) was saved by osem_backup_kernel; the cycle counter
+// Ctrl::k advances here (nothing else on the device counts OSEM cycles), and a refused cycle is undone by osem_restore_kernel.
 template <typename T>
 __global__ void __launch_bounds__(256) err_kernel(const T *f, const T *d, const T *cand, const T *truth, size_t n, Ctrl *ct, DevOpts o,
                                                   Trace tr, double *part, int mode)
 {
     __shared__ double red[2 * 32];
     if (mode == 1 && ct->err_pending == 0) return;
-    if (mode == 2 && ct->status != 0) return;
+    if (mode >= 2 && ct->status != 0) return;
     const bool pend = mode == 1 && ct->pending != 0;
     const T lam = (T)ct->lambda;
     double acc[2] = {0.0, 0.0};
@@ -187,9 +189,10 @@ __global__ void __launch_bounds__(256) err_kernel(const T *f, const T *d, const 
                 ct->err = rho;
                 if (tr.err) tr.err[0] = rho;
             } else {
-                const int k = ct->k;                                   // index of the candidate iterate
+                const int k = ct->k + (mode == 3 ? 1 : 0);             // index of the candidate iterate
                 if (tr.err) tr.err[k] = rho;
                 ct->err_pending = 0;
+                if (mode == 3) ct->k = k;
                 if (o.stop_rule == SGP_STOP_MINERR && rho > ct->err) {
                     ct->status = SGP_REASON_MINERR;
                     ct->k = k - 1;
@@ -210,6 +213,22 @@ __global__ void rl_commit_kernel(T *f, const T *cand, size_t n, const Ctrl *ct)
 {
     if (ct->commit == 0) return;
     for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) f[i] = cand[i];
+}
+
+// OSEM with the Eq.25 rule: h(k) is kept in the plane `d` (unused by OSEM) while the cycle works on f in place ...
+template <typename T>
+__global__ void osem_backup_kernel(const T *f, T *keep, size_t n, const Ctrl *ct)
+{
+    if (ct->status != 0) return;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) keep[i] = f[i];
+}
+// ... and comes back when err_kernel (mode 3) refused the cycle: the run returns h(k), the iterate of minimum error.
+// (The cycles that remain in a captured graph find the status set and `keep` unchanged, so repeating the copy is harmless.)
+template <typename T>
+__global__ void osem_restore_kernel(T *f, const T *keep, size_t n, const Ctrl *ct)
+{
+    if (!(ct->status == SGP_REASON_MINERR && ct->commit == 0)) return;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) f[i] = keep[i];
 }
 
 // ---------------------------------------------------------------- refresh_every (reading A21)

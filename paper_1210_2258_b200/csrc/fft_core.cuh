@@ -369,7 +369,7 @@ template <int TF> struct SyncGroup {
 // tw = the per-pass twiddle tables of this plan (see above).  Every exchange is bracketed sync / store / sync / load, so shared memory
 // the caller used before the call is safe to reuse, and on return nobody is writing it.
 // TWS: the tables sit in shared memory (copied there by the caller), else in global memory (read-only path)
-template <typename T, int L, int E, int DIR, int IP, int NS, bool TWS, typename SYNC>
+template <typename T, int L, int E, int DIR, int IP, int NS, bool TWS, bool TWP, typename SYNC>
 __device__ __forceinline__ void fft_passes(cx<T> (&v)[E], cx<T> *__restrict__ sm, const int cs, const int t,
                                            const cx<T> *__restrict__ tw, const SYNC &sync)
 {
@@ -389,10 +389,20 @@ __device__ __forceinline__ void fft_passes(cx<T> (&v)[E], cx<T> *__restrict__ sm
         if constexpr (NS > 1) {
             const int jm = j % NS;                       // NS is a compile-time constant
             const C *twp = tw + tw_offset(L, E, IP) + jm;
+            if constexpr (TWP && R >= 8) {
+                // powers of the first table entry w = exp(-2 pi i jm / (NS R)): w^r = w^(r/2) w^(r - r/2), depth log2 R
+                C wp[R];
+                wp[1] = __ldg(&twp[0]);
 #pragma unroll
-            for (int r = 1; r < R; ++r) {
-                C w = TWS ? twp[(r - 1) * NS] : __ldg(&twp[(r - 1) * NS]);
-                a[r] = (DIR < 0) ? cmul(a[r], w) : cmulc(a[r], w);
+                for (int r = 2; r < R; ++r) wp[r] = cmul(wp[r / 2], wp[r - r / 2]);
+#pragma unroll
+                for (int r = 1; r < R; ++r) a[r] = (DIR < 0) ? cmul(a[r], wp[r]) : cmulc(a[r], wp[r]);
+            } else {
+#pragma unroll
+                for (int r = 1; r < R; ++r) {
+                    C w = TWS ? twp[(r - 1) * NS] : __ldg(&twp[(r - 1) * NS]);
+                    a[r] = (DIR < 0) ? cmul(a[r], w) : cmulc(a[r], w);
+                }
             }
             j0s[b] = (j / NS) * (NS * R) + jm;
         } else {
@@ -411,14 +421,14 @@ __device__ __forceinline__ void fft_passes(cx<T> (&v)[E], cx<T> *__restrict__ sm
         sync();
 #pragma unroll
         for (int e = 0; e < E; ++e) v[e] = sm[fft_pad<E>(t + TF * e) * cs];
-        fft_passes<T, L, E, DIR, IP + 1, NS * R, TWS>(v, sm, cs, t, tw, sync);
+        fft_passes<T, L, E, DIR, IP + 1, NS * R, TWS, TWP>(v, sm, cs, t, tw, sync);
     }
 }
 
-template <typename T, int L, int E, int DIR, bool TWS = false, typename SYNC>
+template <typename T, int L, int E, int DIR, bool TWS = false, bool TWP = false, typename SYNC>
 __device__ __forceinline__ void fft_block(cx<T> (&v)[E], cx<T> *sm, int cs, int t, const cx<T> *tw, const SYNC &sync)
 {
-    fft_passes<T, L, E, DIR, 0, 1, TWS>(v, sm, cs, t, tw, sync);
+    fft_passes<T, L, E, DIR, 0, 1, TWS, TWP>(v, sm, cs, t, tw, sync);
 }
 
 // Twiddle tables in shared memory.  The pass tables of a transform are read (R - 1)/R times per element and pass -- as

@@ -406,6 +406,7 @@ template <typename T> struct PlanImpl : PlanBase {
         memset(&P, 0, sizeof(P));
         P.G = G; P.ct = ct; P.in = spec; P.out = spec; P.khat = khat; P.khatB = khatB;
         P.specplane = nspec; P.tw = tw_c; P.pack = pack; P.p = p; P.ntiles = ntiles; P.slab = lnb > 1 ? slab : 0;
+        P.pf_ahead = (col_grid == ntiles && ntiles > nsm && lnb == 1) ? nsm : 0;      // col.cuh: SGP_COL_PF2
         return P;
     }
     int launch_col(col_kernel_t<T> k, const ColParams<T> &P, cudaStream_t st)

@@ -176,6 +176,11 @@ int PlanImpl<T>::enqueue_osem_cycle(const DevOpts &o, const Trace &tr, const dou
     RowParams<T> Pb = row_params();
     Pb.o = o; Pb.tr = tr; Pb.check_status = 1; Pb.b_is_array = b_is_array;
     Pb.G.p = 1;
+    if (tr.err) {      // Eq.25 per cycle (reading A27): h(k) is kept in `d` until the error of h(k+1) is known (extra.cuh)
+        osem_backup_kernel<T><<<ew_grid(n), 256, 0, st>>>(f, d, n, ct);
+        launches++;
+        SGP_CUDA_TRY(cudaGetLastError());
+    }
     for (int j = 0; j < p; ++j) {
         const size_t off = (size_t)j * n;
         Pb.bconst[0] = bconst[j];
@@ -204,6 +209,12 @@ int PlanImpl<T>::enqueue_osem_cycle(const DevOpts &o, const Trace &tr, const dou
         { RowParams<T> P = Pb; P.in0 = f; P.out0 = f; P.count_fft = 2; if ((rc = launch_row(k_rowi[rl_fused ? RI_RLUPF : RI_RLUPDATE], P, 1, st))) return rc; }
     }
     cur_slot = -1;
+    if (tr.err) {
+        err_kernel<T><<<ew_grid(n), 256, 0, st>>>(f, nullptr, nullptr, (const T *)run_truth, n, ct, o, tr, part_err, 3);
+        osem_restore_kernel<T><<<ew_grid(n), 256, 0, st>>>(f, d, n, ct);
+        launches += 2;
+        SGP_CUDA_TRY(cudaGetLastError());
+    }
     return SGP_OK;
 }
 
@@ -278,7 +289,7 @@ int PlanImpl<T>::run_batched(int algorithm, const void *const *g, const void *co
     sgp_options ro = ropt ? *ropt : opt;
     int rc = validate_options(&ro);
     if (rc) return rc;
-    if (algorithm == SGP_ALG_OSEM && ro.stop_rule != SGP_STOP_MAXIT) return SGP_ERR_UNSUPPORTED;   // include/sgp.h: osem_*
+    if (algorithm == SGP_ALG_OSEM && ro.stop_rule != SGP_STOP_MAXIT && ro.stop_rule != SGP_STOP_MINERR) return SGP_ERR_UNSUPPORTED;   // include/sgp.h: osem_*
     if (ro.stop_rule == SGP_STOP_MINERR && !res[0].truth) return SGP_ERR_ARG;                       // Eq.25 needs the true object
     // plan-level fields cannot change per run (include/sgp.h: sgp_plan_run)
     if (ro.tile_cols != opt.tile_cols || ro.rows_per_block != opt.rows_per_block || ro.sigma_R != opt.sigma_R ||
@@ -520,7 +531,13 @@ int PlanImpl<T>::run_batched(int algorithm, const void *const *g, const void *co
                 if ((rc = read_ctrl())) return rc;
                 for (int b = 0; b < nb; ++b) if (status[b] == 0) status[b] = hs[b].status;
             }
-            if (any_running()) {
+            // Eq.25 stop (OSEM runs are never batched): the cycle counter and the error come from the device; the kernels of
+            // the J0 phase test the device status, so it is cleared for them and the reason kept on the host
+            const bool minerr_stop = status[0] == SGP_REASON_MINERR;
+            const int k_minerr = hs[0].k;
+            const double err_minerr = hs[0].err;
+            if (minerr_stop) SGP_CUDA_TRY(cudaMemsetAsync(&ct->status, 0, sizeof(int), st));
+            if (any_running() || minerr_stop) {
                 Trace t0 = tr; t0.J = nullptr;
                 RowParams<T> Pj = Pb; Pj.tr = t0;
                 { RowParams<T> P = Pj; P.in0 = f; if ((rc = launch_row(k_rowf[RF_PLAIN], P, 1, st))) return rc; }
@@ -529,8 +546,9 @@ int PlanImpl<T>::run_batched(int algorithm, const void *const *g, const void *co
                   if ((rc = launch_row(k_rowi[RI_QJ], P, p, st))) return rc; }
                 if ((rc = read_ctrl())) return rc;
                 for (int b = 0; b < nb; ++b) {
-                    if (status[b] == 0) status[b] = hs[b].status;
-                    hs[b].k = done;
+                    if (status[b] == 0 || (minerr_stop && hs[b].status < 0)) status[b] = hs[b].status;
+                    hs[b].k = minerr_stop ? k_minerr : done;
+                    if (minerr_stop) hs[b].err = err_minerr;
                     if (status[b] == 0) status[b] = SGP_REASON_MAXIT;
                 }
             }

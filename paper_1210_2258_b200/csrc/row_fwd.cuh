@@ -61,6 +61,13 @@ template <typename T> __device__ __forceinline__ void untangle(cx<T> a, cx<T> zb
 // Forward transform of one row held as v[e] = (x[2m], x[2m+1]), m = t + TF e, by the TF threads of the row, and
 // store of its half spectrum (tile-major).  Shared by the forward row kernel and the fused line-search kernel.
 // tw / twh: the tables, in shared memory when TWS
+#ifndef SGP_LOCKSTEP
+#define SGP_LOCKSTEP 0
+#endif
+#ifndef SGP_ROW_TWP
+#define SGP_ROW_TWP 0      // experiment: pass twiddles of the float row transforms as powers of one table entry (fft_core.cuh: TWP)
+#endif
+template <typename T> constexpr bool kRowTwp = SGP_ROW_TWP && sizeof(T) == 4;
 template <typename T, int L, bool TWS, typename SYNC>
 __device__ __forceinline__ void fwd_fft_store(cx<T> (&v)[fft_E<T>(L)], cx<T> *smrow, const int t, const SYNC &sync,
                                               const RowParams<T> &P, const RowPtrs<T> &X, const int y, const int j, const cx<T> *tw, const cx<T> *twh)
@@ -70,7 +77,8 @@ __device__ __forceinline__ void fwd_fft_store(cx<T> (&v)[fft_E<T>(L)], cx<T> *sm
     constexpr int TF = L / E;
     const Geom &G = P.G;
     // ---- complex FFT of length L = nx/2 over z[m] = x[2m] + i x[2m+1]
-    fft_block<T, L, E, -1, TWS>(v, smrow, 1, t, tw, sync);
+    if constexpr ((SGP_LOCKSTEP & 2) != 0) __syncthreads();
+    fft_block<T, L, E, -1, TWS, kRowTwp<T>>(v, smrow, 1, t, tw, sync);
     sync();
 #pragma unroll
     for (int e = 0; e < E; ++e) smrow[fft_pad<E>(t + TF * e)] = v[e];

@@ -8,6 +8,23 @@
 
 namespace sgpk {
 
+#ifndef SGP_RED_LATE
+#define SGP_RED_LATE 0     // fused kernels (RI_LSF, RI_QJF): CTA barriers of the J reduction after the forward transform
+#endif
+#ifndef SGP_LOCKSTEP
+#define SGP_LOCKSTEP 0
+#endif
+#ifndef SGP_EPI_PF
+#define SGP_EPI_PF 0       // L2 prefetch of the epilogue's plane rows, issued once the spectrum row has landed (before the FFT)
+#endif
+// the nx elements of one plane row, 128-byte lines spread over the TF lanes of the row
+template <typename T, int TF> __device__ __forceinline__ void prefetch_row(const T *row, int nx, int t)
+{
+    const char *b = reinterpret_cast<const char *>(row);
+    const int bytes = nx * (int)sizeof(T);
+    for (int o = t * 128; o < bytes; o += TF * 128) prefetch_l2(b + o);
+}
+
 // re-tangling of one (k, L-k) pair: a = X[k], b = conj X[L-k], w = exp(-2 pi i k/nx):
 //   S = a + b, Tm = i conj(w) (a - b):  Z[k] = S + Tm, Z[L-k] = conj(S - Tm)
 template <typename T> __device__ __forceinline__ void retangle(cx<T> a, cx<T> xb, cx<T> w, cx<T> &zk, cx<T> &zlk)
@@ -97,11 +114,27 @@ __global__ void __launch_bounds__(256, SGP_ROW_MINB) row_inv_kernel(const RowPar
     }
     if (stop != 0) return;
     if constexpr (TWS) row_tables_wait(); else sync();
+    if constexpr ((SGP_LOCKSTEP & 1) != 0) __syncthreads();      // experiment: the rows of a CTA enter the transform together (instruction fetch)
+    if constexpr (SGP_EPI_PF != 0 && sizeof(T) == 4) {
+        // the spectrum row has landed: start the plane rows of the epilogue on their way to L2 while the transform computes
+        // (requested at the top of the kernel they compete with the spectrum loads, which the transform waits for)
+        const size_t rb = (size_t)y * nx, bs = (size_t)j * P.plane + rb;
+        if constexpr (MODE == RI_GRAD && SGP_EPI_PF == 1) {
+            prefetch_row<T, TF>(X.in0 + rb, nx, t); prefetch_row<T, TF>(X.in1 + rb, nx, t); prefetch_row<T, TF>(X.out0 + rb, nx, t);
+        } else if constexpr (MODE == RI_LS || MODE == RI_LSF) {
+            prefetch_row<T, TF>(X.in0 + bs, nx, t);
+            prefetch_row<T, TF>(X.in1 + (size_t)X.ct->qsel * P.qbuf + bs, nx, t);
+        } else if constexpr ((MODE == RI_QJ || MODE == RI_QJF) && SGP_EPI_PF == 1) {
+            prefetch_row<T, TF>(X.in0 + bs, nx, t);
+        } else if constexpr ((MODE == RI_RLUPDATE || MODE == RI_RLUPF) && (SGP_EPI_PF == 1 || SGP_EPI_PF == 3)) {
+            prefetch_row<T, TF>(X.in0 + rb, nx, t);
+        }
+    }
     {
         C v[E];
 #pragma unroll
         for (int e = 0; e < E; ++e) v[e] = smrow[fft_pad<E>(t + TF * e)];
-        fft_block<T, L, E, +1, TWS>(v, smrow, 1, t, tw, sync);
+        fft_block<T, L, E, +1, TWS, kRowTwp<T>>(v, smrow, 1, t, tw, sync);
         // park the row (w(y, 2m), w(y, 2m+1)), m = t + TF e, in natural order (no padding) for the epilogue
         sync();
 #pragma unroll
@@ -170,8 +203,18 @@ __global__ void __launch_bounds__(256, SGP_ROW_MINB) row_inv_kernel(const RowPar
         if (MODE == RI_QJ && P.submode == QJ_REFRESH) rowout += (size_t)X.ct->qsel * P.qbuf;
         epi_kl<T, L, TF, LS, MK, RATIO, MODE != RI_QJF, SPEC>(P, X, wrow, wmut, qin, qout, rowout, t, y, j, base, plain, acc);
         if (!act) acc[0] = 0.0;                                    // padding lanes repeat lane TF - 1
+        constexpr bool RED_LATE = RATIO && SGP_RED_LATE != 0;
+        if constexpr (RED_LATE) {
+            // the warp sums now, the CTA barriers of the reduction after the forward transform (sgp_dev.cuh)
+            if (!plain) block_reduce_sum_warps<1>(acc, red);
+            C v[E];
+            sync();
+#pragma unroll
+            for (int e = 0; e < E; ++e) v[e] = smrow[t + TF * e];
+            fwd_fft_store<T, L, TWS>(v, smrow, t, sync, P, X, y, j, tw, twh);
+        }
         if (!plain) {
-        block_reduce_sum<1>(acc, red);
+        if constexpr (RED_LATE) block_reduce_sum_finish<1>(acc, red); else block_reduce_sum<1>(acc, red);
         const int tk = LS ? TK_LS : TK_QJ;
         if (publish_partials<1>(acc, X.part, bid, nblk, &X.ct->counter[tk])) {
             final_sum<1>(acc, X.part, nblk, red);
@@ -225,7 +268,7 @@ __global__ void __launch_bounds__(256, SGP_ROW_MINB) row_inv_kernel(const RowPar
             }
         }
         }   // !plain
-        if constexpr (RATIO) {
+        if constexpr (RATIO && !RED_LATE) {
             // a1 of the next step (SGP: speculating on lambda = 1): forward row transform of the ratio parked in shared
             // memory by the epilogue; the spectrum row this warp read at the top is overwritten in place
             C v[E];

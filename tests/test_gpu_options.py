@@ -100,6 +100,48 @@ def test_minimum_error_stop_eq25(alg, dt):
     plan.close()
 
 
+@pytest.mark.parametrize("dt", [np.float32, np.float64])
+def test_minimum_error_stop_eq25_osem(dt):
+    """Eq.25 for OSEM on the device, per cycle (reading A27; the paper stops OSEM at the minimum r.m.s. error in its
+    diffuse-object experiments): the error trace against the oracle's, the stop at the first cycle that would
+    increase rho, the iterate returned = h(k) of the run stopped there by max_iter (bit for bit), J0 at that iterate."""
+    _need_gpu()
+    w = synth.make("C2", n=128)
+    # few counts (the object dimmed 3000 times, Poisson noise drawn again): semiconvergence after 16 cycles
+    rng = np.random.default_rng(26)
+    truth = w["truth"] / 3000.0
+    g = []
+    for j, k in enumerate(w["psf"]):
+        K = np.fft.rfft2(np.fft.ifftshift(k / k.sum()))
+        g.append(rng.poisson(np.maximum(np.fft.irfft2(K * np.fft.rfft2(truth), s=truth.shape) + w["b"][j], 0)).astype(np.float64))
+    w["g"] = g
+    w["name"] += "_dim"
+    K = 60
+    fo, ro, P = oracle_run(w, "osem", truth=truth, max_iter=K, stop_rule=oracle.STOP_MINERR)
+    assert ro.stop_reason == 4 and 3 < ro.iterations < K, "the oracle run must stop by Eq.25 for this test to mean anything"
+    plan, o = gpu_plan(w, dt, max_iter=K, stop_rule=B.STOP_MINERR)
+    gd = [dev(a, dt) for a in w["g"]]
+    fg, rg = plan.osem(gd, w["b"], opts=o, truth=dev(truth, dt))
+    assert rg.stop_reason == 4 and rg.iterations == ro.iterations, (rg.stop_reason, rg.iterations, ro.iterations)
+    n = rg.iterations
+    np.testing.assert_allclose(rg.err[:n + 2], ro.err[:n + 2], rtol=1e-5 if dt == np.float32 else 1e-11)
+    assert rg.err[n + 1] > rg.err[n] == rg.err_final                      # the discarded cycle would have increased it
+    assert abs(rg.J0_final - ro.J0_final) <= (1e-4 if dt == np.float32 else 1e-10) * abs(ro.J0_final)
+    assert rel_l2(fg.cpu().numpy(), fo) <= (1e-4 if dt == np.float32 else 1e-10)
+    assert rg.n_fft2 == ro.n_fft2 == 4 * len(g) * (rg.iterations + 1), (rg.n_fft2, ro.n_fft2)      # the discarded cycle was computed too
+    # the iterate returned is h(k), not the discarded h(k+1)
+    o2 = B.default_options(**{**w["opts"], "max_iter": n, "stop_rule": 0})
+    fk, rk = plan.osem(gd, w["b"], opts=o2)
+    assert torch.equal(fk, fg) and rk.J0_final == rg.J0_final and rk.iterations == n
+    # the error trace without the stopping rule; the rule without a true object is refused
+    f3, r3 = plan.osem(gd, w["b"], opts=B.default_options(**{**w["opts"], "max_iter": 8, "stop_rule": 0}), truth=dev(truth, dt))
+    np.testing.assert_allclose(r3.err[:9], ro.err[:9], rtol=1e-5 if dt == np.float32 else 1e-11)
+    assert r3.iterations == 8 and r3.stop_reason == 1
+    _, r4 = plan.osem(gd, w["b"], opts=o, check=False)
+    assert r4.rc == B.ERR_ARG
+    plan.close()
+
+
 # ------------------------------------------------------------------------------------------------ smoothed constant start
 @pytest.mark.parametrize("dt,tol", [(np.float32, 2e-6), (np.float64, 1e-12)])
 def test_gaussian_smoothed_constant_start(dt, tol):
