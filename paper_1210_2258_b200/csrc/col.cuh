@@ -21,13 +21,19 @@ namespace sgpk {
 
 enum ColMode { CM_FWD = 0, CM_CONJSUM = 1, CM_MULT = 2, CM_INV = 3 };
 
-// experiment: pass twiddles of the float column transforms as powers of one table entry (fft_core.cuh: TWP)
+// option: pass twiddles of the float column transforms from a few table entries and one product each (fft_core.cuh: TWP).
+// K2 / K5 43.3 / 40.2 -> 39.5 / 36.8 us at 3 x 2048^2 (the image loop repeats the passes p times per tile); OFF: it changes the
+// rounding of every transform, and that was enough to move the long free-running fp32 parity runs
 #ifndef SGP_COL_TWP
 #define SGP_COL_TWP 0
 #endif
-template <typename T> constexpr bool kColTwp = SGP_COL_TWP && sizeof(T) == 4;
+#ifndef SGP_TWP_F64
+#define SGP_TWP_F64 0      // experiment: the same in the double kernels
+#endif
+template <typename T> constexpr bool kColTwp = SGP_COL_TWP && (sizeof(T) == 4 || SGP_TWP_F64);
 // experiment: the tiles of the NEXT wave of CTAs requested into L2 by the CTAs of this one (ColParams::pf_ahead), so that DRAM
-// works while the SMs transform instead of idling until the next wave asks for its tiles all at once
+// works while the SMs transform instead of idling until the next wave asks for its tiles all at once.  Measured: K2 / K5
+// 43.3 / 40.2 -> 42.2 / 39.0 us at 3 x 2048^2, 22.9 / 20.9 -> 23.0 / 21.3 us at 2048^2 (RL 13 360 -> 13 260 it/s): off
 #ifndef SGP_COL_PF2
 #define SGP_COL_PF2 0
 #endif

@@ -80,6 +80,16 @@ __host__ __device__ constexpr double cos32(int k)
     return k <= 8 ? q32(k) : k <= 16 ? -q32(16 - k) : k <= 24 ? -q32(k - 16) : q32(32 - k);
 }
 __host__ __device__ constexpr double sin32(int k) { return cos32(k + 24); }
+// cos / sin of 2 pi k / 64, 0 <= k <= 16 (the real<->complex step of a row whose threads hold 32 elements: row_fwd.cuh, SGP_ROW_TWC)
+__host__ __device__ constexpr double cos64q(int k)
+{
+    return k == 0 ? 1.0 : k == 1 ? 0.99518472667219688624 : k == 2 ? 0.98078528040323044913 : k == 3 ? 0.95694033573220886494
+         : k == 4 ? 0.92387953251128675613 : k == 5 ? 0.88192126434835502971 : k == 6 ? 0.83146961230254523708
+         : k == 7 ? 0.77301045336273696081 : k == 8 ? 0.70710678118654752440 : k == 9 ? 0.63439328416364549822
+         : k == 10 ? 0.55557023301960222474 : k == 11 ? 0.47139673682599764856 : k == 12 ? 0.38268343236508977173
+         : k == 13 ? 0.29028467725446236764 : k == 14 ? 0.19509032201612826785 : k == 15 ? 0.09801714032956060199 : 0.0;
+}
+__host__ __device__ constexpr double sin64q(int k) { return cos64q(16 - k); }
 
 // 8-point DFT on references, natural order in and out
 template <int DIR, typename T, typename C>
@@ -389,14 +399,25 @@ __device__ __forceinline__ void fft_passes(cx<T> (&v)[E], cx<T> *__restrict__ sm
         if constexpr (NS > 1) {
             const int jm = j % NS;                       // NS is a compile-time constant
             const C *twp = tw + tw_offset(L, E, IP) + jm;
-            if constexpr (TWP && R >= 8) {
-                // powers of the first table entry w = exp(-2 pi i jm / (NS R)): w^r = w^(r/2) w^(r - r/2), depth log2 R
-                C wp[R];
-                wp[1] = __ldg(&twp[0]);
+            if constexpr (TWP && (R == 8 || R == 16 || R == 32)) {
+                // TWP: the R - 1 twiddles w^r, w = exp(-2 pi i jm / (NS R)), from H - 1 + R/H - 1 table entries and ONE product each:
+                // w^(aH + b) = w^(aH) w^b with w^1 .. w^(H-1) and w^H, w^2H, ... loaded (H = 4; 2 for radix 8): 6 loads + 9 products
+                // instead of 15 loads at radix 16, 10 + 21 instead of 31 at radix 32, 4 + 3 instead of 7 at radix 8.  Every value is
+                // a table entry or the product of two, so its error stays at two table roundings plus one product.  (Powers of the
+                // single entry w^1 -- one load -- are faster still and far too noisy: the rounding of w^1 comes back r times in w^r.)
+                // An option of the float kernels (col.cuh: SGP_COL_TWP, row_fwd.cuh: SGP_ROW_TWP), off by default.
+                constexpr int H = R >= 16 ? 4 : 2;
+                auto twmul = [](C x, C w) { return (DIR < 0) ? cmul(x, w) : cmulc(x, w); };
+                C wl[H];
 #pragma unroll
-                for (int r = 2; r < R; ++r) wp[r] = cmul(wp[r / 2], wp[r - r / 2]);
+                for (int lo = 1; lo < H; ++lo) { wl[lo] = __ldg(&twp[(lo - 1) * NS]); a[lo] = twmul(a[lo], wl[lo]); }
 #pragma unroll
-                for (int r = 1; r < R; ++r) a[r] = (DIR < 0) ? cmul(a[r], wp[r]) : cmulc(a[r], wp[r]);
+                for (int hi = 1; hi < R / H; ++hi) {
+                    const C wh = __ldg(&twp[(hi * H - 1) * NS]);
+                    a[hi * H] = twmul(a[hi * H], wh);
+#pragma unroll
+                    for (int lo = 1; lo < H; ++lo) a[hi * H + lo] = twmul(a[hi * H + lo], cmul(wh, wl[lo]));
+                }
             } else {
 #pragma unroll
                 for (int r = 1; r < R; ++r) {

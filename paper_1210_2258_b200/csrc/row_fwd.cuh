@@ -61,13 +61,25 @@ template <typename T> __device__ __forceinline__ void untangle(cx<T> a, cx<T> zb
 // Forward transform of one row held as v[e] = (x[2m], x[2m+1]), m = t + TF e, by the TF threads of the row, and
 // store of its half spectrum (tile-major).  Shared by the forward row kernel and the fused line-search kernel.
 // tw / twh: the tables, in shared memory when TWS
-#ifndef SGP_LOCKSTEP
-#define SGP_LOCKSTEP 0
-#endif
 #ifndef SGP_ROW_TWP
-#define SGP_ROW_TWP 0      // experiment: pass twiddles of the float row transforms as powers of one table entry (fft_core.cuh: TWP)
+#define SGP_ROW_TWP 0      // option: pass twiddles of the float row transforms from a few table entries and one product each (fft_core.cuh: TWP); off, see col.cuh
 #endif
-template <typename T> constexpr bool kRowTwp = SGP_ROW_TWP && sizeof(T) == 4;
+#ifndef SGP_TWP_F64
+#define SGP_TWP_F64 0
+#endif
+template <typename T> constexpr bool kRowTwp = SGP_ROW_TWP && (sizeof(T) == 4 || SGP_TWP_F64);
+// experiment: exp(-2 pi i k/nx), k = t + TF i, of the real<->complex step as (table entry t) x (constant exp(-i pi i/E)): one load
+// and E/2 - 1 products with immediates instead of E/2 loads (float, 32 or 16 elements per thread, tile width dividing TF)
+#ifndef SGP_ROW_TWC
+#define SGP_ROW_TWC 0
+#endif
+template <typename T, int E> constexpr bool kRowTwc = SGP_ROW_TWC && sizeof(T) == 4 && (E == 32 || E == 16);
+// exp(-i pi i / E), i < E/2
+template <typename T, int E> __device__ __forceinline__ cx<T> twc_const(int i)
+{
+    if constexpr (E == 32) return mk<T>((T)cos64q(i), (T)-sin64q(i));
+    else return mk<T>((T)cos32(i), (T)-sin32(i));
+}
 template <typename T, int L, bool TWS, typename SYNC>
 __device__ __forceinline__ void fwd_fft_store(cx<T> (&v)[fft_E<T>(L)], cx<T> *smrow, const int t, const SYNC &sync,
                                               const RowParams<T> &P, const RowPtrs<T> &X, const int y, const int j, const cx<T> *tw, const cx<T> *twh)
@@ -77,7 +89,6 @@ __device__ __forceinline__ void fwd_fft_store(cx<T> (&v)[fft_E<T>(L)], cx<T> *sm
     constexpr int TF = L / E;
     const Geom &G = P.G;
     // ---- complex FFT of length L = nx/2 over z[m] = x[2m] + i x[2m+1]
-    if constexpr ((SGP_LOCKSTEP & 2) != 0) __syncthreads();
     fft_block<T, L, E, -1, TWS, kRowTwp<T>>(v, smrow, 1, t, tw, sync);
     sync();
 #pragma unroll
@@ -103,11 +114,15 @@ __device__ __forceinline__ void fwd_fft_store(cx<T> (&v)[fft_E<T>(L)], cx<T> *sm
         const size_t stride = (size_t)TF * (size_t)G.ny;
         C *pa = dst + spec_index(G, y, t);
         C *pb = dst + spec_index(G, y, L - TF - t) + stride;
+        C wt = mk<T>((T)1, (T)0);
+        if constexpr (kRowTwc<T, E>) wt = TWS ? twh[t] : __ldg(&twh[t]);
 #pragma unroll
         for (int i = 1; i < E / 2; ++i) {
             const int k = t + TF * i;
             C xk, xlk;
-            untangle<T>(smrow[fft_pad<E>(k)], smrow[fft_pad<E>(L - k)], TWS ? twh[k] : __ldg(&twh[k]), xk, xlk);
+            C wk;
+            if constexpr (kRowTwc<T, E>) wk = cmul(wt, twc_const<T, E>(i)); else wk = TWS ? twh[k] : __ldg(&twh[k]);
+            untangle<T>(smrow[fft_pad<E>(k)], smrow[fft_pad<E>(L - k)], wk, xk, xlk);
             if (X.act) { pa[(size_t)i * stride] = xk; *(pb - (size_t)i * stride) = xlk; }
         }
     } else {

@@ -8,14 +8,14 @@
 
 namespace sgpk {
 
-#ifndef SGP_RED_LATE
-#define SGP_RED_LATE 0     // fused kernels (RI_LSF, RI_QJF): CTA barriers of the J reduction after the forward transform
-#endif
-#ifndef SGP_LOCKSTEP
-#define SGP_LOCKSTEP 0
-#endif
+// L2 prefetch of the plane rows the epilogue streams, issued once the spectrum row has landed, i.e. while the transform computes
+// (single-wave kernels: without it DRAM idles during the transforms and every warp asks for its rows at the same moment).
+// 0 = off; 2 = the line-search kernels only (g_j, q_j): K6 35.3 -> 33.1 us at 2048^2, 95.0 -> 93.0 us at 3 x 2048^2; 1 = also the
+// gradient kernel (f, d, grad(k-1): 28.5 -> 28.7 us), the RL ratio kernel (27.9 -> 28.7 us) and the RL update: slower, so 2 it is;
+// 3 = 2 + the RL update kernel (no change).  Requested at the top of the kernel the rows compete with the spectrum loads (round 1:
+// K3 + 10 %).
 #ifndef SGP_EPI_PF
-#define SGP_EPI_PF 0       // L2 prefetch of the epilogue's plane rows, issued once the spectrum row has landed (before the FFT)
+#define SGP_EPI_PF 2
 #endif
 // the nx elements of one plane row, 128-byte lines spread over the TF lanes of the row
 template <typename T, int TF> __device__ __forceinline__ void prefetch_row(const T *row, int nx, int t)
@@ -93,11 +93,15 @@ __global__ void __launch_bounds__(256, SGP_ROW_MINB) row_inv_kernel(const RowPar
             const size_t stride = (size_t)TF * (size_t)G.ny;
             const C *pa = src + spec_index(G, y, t);
             const C *pb = src + spec_index(G, y, L - TF - t) + stride;
+            C wt = mk<T>((T)1, (T)0);
+            if constexpr (kRowTwc<T, E>) wt = __ldg(&P.twh[t]);
 #pragma unroll
             for (int i = 1; i < E / 2; ++i) {
                 const int k = t + TF * i;
                 C zk, zlk;
-                retangle<T>(pa[(size_t)i * stride], *(pb - (size_t)i * stride), __ldg(&P.twh[k]), zk, zlk);
+                C wk;
+                if constexpr (kRowTwc<T, E>) wk = cmul(wt, twc_const<T, E>(i)); else wk = __ldg(&P.twh[k]);
+                retangle<T>(pa[(size_t)i * stride], *(pb - (size_t)i * stride), wk, zk, zlk);
                 smrow[fft_pad<E>(k)] = zk;
                 smrow[fft_pad<E>(L - k)] = zlk;
             }
@@ -114,7 +118,6 @@ __global__ void __launch_bounds__(256, SGP_ROW_MINB) row_inv_kernel(const RowPar
     }
     if (stop != 0) return;
     if constexpr (TWS) row_tables_wait(); else sync();
-    if constexpr ((SGP_LOCKSTEP & 1) != 0) __syncthreads();      // experiment: the rows of a CTA enter the transform together (instruction fetch)
     if constexpr (SGP_EPI_PF != 0 && sizeof(T) == 4) {
         // the spectrum row has landed: start the plane rows of the epilogue on their way to L2 while the transform computes
         // (requested at the top of the kernel they compete with the spectrum loads, which the transform waits for)
@@ -203,18 +206,8 @@ __global__ void __launch_bounds__(256, SGP_ROW_MINB) row_inv_kernel(const RowPar
         if (MODE == RI_QJ && P.submode == QJ_REFRESH) rowout += (size_t)X.ct->qsel * P.qbuf;
         epi_kl<T, L, TF, LS, MK, RATIO, MODE != RI_QJF, SPEC>(P, X, wrow, wmut, qin, qout, rowout, t, y, j, base, plain, acc);
         if (!act) acc[0] = 0.0;                                    // padding lanes repeat lane TF - 1
-        constexpr bool RED_LATE = RATIO && SGP_RED_LATE != 0;
-        if constexpr (RED_LATE) {
-            // the warp sums now, the CTA barriers of the reduction after the forward transform (sgp_dev.cuh)
-            if (!plain) block_reduce_sum_warps<1>(acc, red);
-            C v[E];
-            sync();
-#pragma unroll
-            for (int e = 0; e < E; ++e) v[e] = smrow[t + TF * e];
-            fwd_fft_store<T, L, TWS>(v, smrow, t, sync, P, X, y, j, tw, twh);
-        }
         if (!plain) {
-        if constexpr (RED_LATE) block_reduce_sum_finish<1>(acc, red); else block_reduce_sum<1>(acc, red);
+        block_reduce_sum<1>(acc, red);
         const int tk = LS ? TK_LS : TK_QJ;
         if (publish_partials<1>(acc, X.part, bid, nblk, &X.ct->counter[tk])) {
             final_sum<1>(acc, X.part, nblk, red);
@@ -268,7 +261,7 @@ __global__ void __launch_bounds__(256, SGP_ROW_MINB) row_inv_kernel(const RowPar
             }
         }
         }   // !plain
-        if constexpr (RATIO && !RED_LATE) {
+        if constexpr (RATIO) {
             // a1 of the next step (SGP: speculating on lambda = 1): forward row transform of the ratio parked in shared
             // memory by the epilogue; the spectrum row this warp read at the top is overwritten in place
             C v[E];

@@ -193,37 +193,6 @@ __device__ __forceinline__ void block_reduce_sum(double (&v)[NQ], double *red /*
     __syncthreads();
 }
 
-// block_reduce_sum in two halves, same arithmetic in the same order: the first (warp sums into red[], no barrier) where the
-// values are complete, the second (the two CTA barriers) wherever the warps may as well meet -- the fused row kernels put their
-// forward transform in between, so that no warp waits for the slowest row of its CTA in the middle of the kernel
-template <int NQ>
-__device__ __forceinline__ void block_reduce_sum_warps(double (&v)[NQ], double *red)
-{
-    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
-#pragma unroll
-    for (int q = 0; q < NQ; ++q) {
-#pragma unroll
-        for (int off = 16; off > 0; off >>= 1) v[q] += __shfl_down_sync(0xffffffffu, v[q], off);
-        if (lane == 0) red[q * 32 + wid] = v[q];
-    }
-}
-template <int NQ>
-__device__ __forceinline__ void block_reduce_sum_finish(double (&v)[NQ], double *red)
-{
-    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = (blockDim.x + 31) >> 5;
-    __syncthreads();
-    if (wid == 0) {
-#pragma unroll
-        for (int q = 0; q < NQ; ++q) {
-            double x = lane < nw ? red[q * 32 + lane] : 0.0;
-#pragma unroll
-            for (int off = 16; off > 0; off >>= 1) x += __shfl_down_sync(0xffffffffu, x, off);
-            v[q] = x;   // valid in thread 0
-        }
-    }
-    __syncthreads();
-}
-
 // Writes this block's partial sums, and returns true in EVERY thread of the last block to arrive
 // (threadfence-reduction pattern); that block then owns all partials.
 template <int NQ>
