@@ -462,7 +462,7 @@ template <typename T> struct PlanImpl : PlanBase {
         const int cy = opt.psf_origin == SGP_PSF_CENTER ? ny / 2 : 0, cxs = opt.psf_origin == SGP_PSF_CENTER ? nx / 2 : 0;
         int rc;
         for (int j = 0; j < p; ++j) {
-            plane_sum_kernel<T><<<1, 1024, 0, st>>>((const T *)psf[j], n, ct);
+            plane_sum_kernel<T><<<ew_grid(n), 256, 0, st>>>((const T *)psf[j], n, ct, part_err);
             launches++;
             Ctrl h;
             SGP_CUDA_TRY(cudaMemcpyAsync(&h, ct, sizeof(Ctrl), cudaMemcpyDeviceToHost, st));
